@@ -1,0 +1,186 @@
+/* cloak.h -- C ABI of the B200-native CloakLM cloaked-layout hot path (libcloak.so).
+ *
+ * What this library is.  CloakLM (arxiv/paper_2606_18400) obfuscates where an LLM's weights sit in
+ * HBM while the authorised reader keeps an unchanged logical view.  The paper does it with a
+ * random permutation computed before any page is allocated or any weight transferred
+ * (section 5), a random virtual->physical map of 2 MB pages through the CUDA VMM API
+ * (Table 1b :192-201), a random tensor order (Table 1a
+ * :181-190) and "inter- and intra-layer weight shuffling".  BASELINE.json's
+ * north_star fixes the calls: a keyed Philox4x32-10 permutation, a block scatter into a 2 MiB page
+ * pool, a function-preserving neuron/head permutation and a GEMV/GEMM that reads through the
+ * block table.  Concrete definitions (counter layout, direction of the table, padding, tile
+ * layout) are the readings O1-O12 / G1-G22 of SURVEY.md section 8(c), restated in DESIGN.md.
+ *
+ * Conventions.
+ *   - Every function returns a cloak_status: 0 = CLOAK_OK, negative = error.  No exceptions, no
+ *     aborts, no printing.  cloak_last_error() returns a thread-local, library-owned C string
+ *     describing the last failure on the calling thread.
+ *   - "d_" arguments are DEVICE pointers, "h_" arguments are HOST pointers.  The caller owns every
+ *     tensor it passes; the library owns pools and their tables.
+ *   - `stream` is a cudaStream_t passed as void* (NULL = the legacy default stream).  Every
+ *     device-side call is asynchronous on that stream and never synchronises it, except where
+ *     stated (pool create/destroy, *_host convenience calls).
+ *   - There is no CPU fallback: without a CUDA device every compute call fails with
+ *     CLOAK_ERR_CUDA.
+ */
+#ifndef CLOAK_H_
+#define CLOAK_H_
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef enum {
+    CLOAK_OK = 0,
+    CLOAK_ERR_INVALID = -1,     /* null pointer, n == 0, batch out of range, size mismatch          */
+    CLOAK_ERR_ALIGN = -2,       /* pointer / offset / size not 16-byte or block aligned             */
+    CLOAK_ERR_UNSUPPORTED = -3, /* dtype / layout / block-size combination not implemented          */
+    CLOAK_ERR_OOM = -4,         /* device or host allocation failed                                 */
+    CLOAK_ERR_CUDA = -5         /* driver / runtime error; text in cloak_last_error()               */
+} cloak_status;
+
+typedef enum { CLOAK_F32 = 0, CLOAK_BF16 = 1 } cloak_dtype;
+
+/* Storage layout of a logical [N, K] matrix inside the arena.
+ * ROWMAJOR: the tensor's bytes as given.  TILE128: tile (tn, tk) of 128 x 128 elements sits at tile
+ * index tn*(K/128)+tk; element (r, c) at element offset r*128+c inside the tile; no swizzle. */
+typedef enum { CLOAK_ROWMAJOR = 0, CLOAK_TILE128 = 1 } cloak_layout;
+
+const char* cloak_last_error(void);
+
+/* Library version / build info: a static string such as "cloak-b200 0.1 sm_100a". */
+const char* cloak_version(void);
+
+/* ---- S1 keyed permutation (north_star: "indices sorted by Philox(key, index)").
+ * For i in [0, n): o = Philox4x32-10(ctr = (i, 0, stream_id lo, stream_id hi), key = (key lo, key hi)),
+ * r_i = o[0]:o[1]; perm = indices sorted ascending by (r_i, i); inv[perm[j]] = j.
+ * d_perm / d_inv: caller-owned device buffers of n uint32; either may be NULL (not both).
+ * n in [1, 2^28].  Asynchronous on `stream` (workspace comes from the stream-ordered allocator). */
+cloak_status cloak_keygen(uint64_t key, uint64_t stream_id, uint32_t n,
+                          uint32_t* d_perm, uint32_t* d_inv, void* stream);
+
+/* ---- S2 page pool ("CUDA VMM ... tensor pointers unchanged").
+ * Geometry: nb = ceil(payload/block), bpp = page/block, npages = ceil(nb/bpp), nslots = npages*bpp.
+ * Tables: (blockperm, blockinv) = keygen(key, 1<<32, nslots); (pageperm, pageinv) = keygen(key, 2<<32, npages).
+ * Real pages (page_bytes a multiple of the VMM granularity and PLAIN_ALLOC not set): a VA range of
+ * npages*page_bytes is reserved, one physical handle per page is created (creation order stands for
+ * physical order, G6), and handle pageinv[v] is mapped at VA page v; the authorised table is
+ * T[i] = blockinv[i].  Emulated pages (any other page size, or PLAIN_ALLOC): one allocation that *is*
+ * the dump view D; T[i] = pageinv[blockinv[i]/bpp]*bpp + blockinv[i]%bpp.
+ * The pool memory is zero-filled.  block_bytes must be a power of two >= 16 and divide page_bytes.
+ * Synchronous (driver calls + one stream sync). */
+typedef struct cloak_pool cloak_pool;
+enum {
+    CLOAK_POOL_IDENTITY = 1,     /* identity block + page tables: the "native" layout              */
+    CLOAK_POOL_PLAIN_ALLOC = 2   /* one plain allocation instead of per-page VMM handles           */
+};
+cloak_status cloak_pool_create(int device, uint64_t payload_bytes, uint32_t block_bytes,
+                               uint64_t page_bytes, uint64_t key, uint32_t flags, cloak_pool** out);
+cloak_status cloak_pool_destroy(cloak_pool* pool);
+
+/* Any output pointer may be NULL.  *d_base: device address of the pool (the VA view V for real pages,
+ * the dump view D for emulated pages).  *d_table: device array T[0..nb).  *is_vmm: 1 for real pages. */
+cloak_status cloak_pool_info(const cloak_pool* pool, void** d_base, const uint32_t** d_table,
+                             uint32_t* nb, uint32_t* nslots, uint32_t* npages, int* is_vmm);
+
+/* Host copies of the four tables (caller-owned host arrays; any may be NULL): blockperm/blockinv have
+ * nslots entries, pageperm/pageinv npages.  Synchronous. */
+cloak_status cloak_pool_tables(const cloak_pool* pool, uint32_t* h_blockperm, uint32_t* h_blockinv,
+                               uint32_t* h_pageperm, uint32_t* h_pageinv);
+
+/* Copies the dump view D (pages in physical = handle-creation order, O5) into d_out (nslots*block bytes).
+ * Real pages: read through a second (alias) mapping of the same handles in creation order.
+ * Emulated pages: a plain copy of the pool.  Asynchronous on `stream`. */
+cloak_status cloak_pool_dump(const cloak_pool* pool, void* d_out, void* stream);
+
+/* Milliseconds the host-side mapper (reserve/create/map/set-access) took in cloak_pool_create. */
+cloak_status cloak_pool_map_ms(const cloak_pool* pool, double* ms);
+
+/* ---- S4 block shuffle / unshuffle, S8 re-layout (north_star (a)).
+ * shuffle:   pool[T[i]*b + o] = logical[i*b + o] for the arena range [logical_offset, +bytes);
+ * unshuffle: logical[i*b + o] = pool[T[i]*b + o] for the same range.
+ * d_logical points at the first byte of that range (e.g. a tensor's data), 16-byte aligned.
+ * logical_offset must be a block multiple; bytes a 16-byte multiple.  A final partial block is
+ * zero-padded on shuffle (G4) and truncated on unshuffle.  Asynchronous on `stream`. */
+cloak_status cloak_shuffle(cloak_pool* pool, const void* d_logical, uint64_t logical_offset,
+                           uint64_t bytes, void* stream);
+cloak_status cloak_unshuffle(const cloak_pool* pool, void* d_logical, uint64_t logical_offset,
+                             uint64_t bytes, void* stream);
+/* pool_b[T_b[i]] = pool_a[T_a[i]] for every logical block, without materialising the arena.
+ * Both pools must have the same payload and block size.  Asynchronous on `stream`. */
+cloak_status cloak_relayout(const cloak_pool* from_a, cloak_pool* to_b, void* stream);
+
+/* Host-buffer variants (end-to-end path): h_logical is a HOST buffer (pinned for full speed); the
+ * library stages it through device memory in chunks.  They synchronise `stream` before returning. */
+cloak_status cloak_shuffle_host(cloak_pool* pool, const void* h_logical, uint64_t logical_offset,
+                                uint64_t bytes, void* stream);
+cloak_status cloak_unshuffle_host(const cloak_pool* pool, void* h_logical, uint64_t logical_offset,
+                                  uint64_t bytes, void* stream);
+
+/* Selects the copy engine used by shuffle / unshuffle / relayout: 0 = automatic, 1 = 16-byte
+ * LDG/STG, 2 = TMA bulk copy through a shared-memory ring.  For A/B measurement; process-wide. */
+cloak_status cloak_set_copy_engine(int engine);
+
+/* ---- S3 tensor order.  Host helper, no device work.
+ * (order, _) = keygen(key, 3<<32, T); the arena holds tensors order[0], order[1], ... back to back, each
+ * padded to a multiple of block_bytes.  h_offsets_out: T entries; h_total_out: padded arena bytes. */
+cloak_status cloak_arena_plan(uint64_t key, uint32_t T, const uint64_t* h_bytes, uint32_t block_bytes,
+                              uint64_t* h_offsets_out, uint64_t* h_total_out);
+
+/* ---- S5 neuron / head permutation (north_star (b)).  Out of place; src and dst of one
+ * tensor have the same shape and must not overlap; any src/dst pair may be NULL/NULL to skip it.
+ * Shapes (row-major, [out, in]): gate, up [inter, hidden]; down [hidden, inter]; q [n_q*head_dim, hidden];
+ * k, v [n_kv*head_dim, hidden]; o [hidden, n_q*head_dim].
+ *   (pi, _) = keygen(key, (4<<32)|layer, inter): gate'[r,:] = gate[pi[r],:], up' likewise, down'[:,r] = down[:,pi[r]]
+ *   (kappa, _) = keygen(key, (5<<32)|layer, n_kv); (rho_g, _) = keygen(key, (6<<32)|(layer*n_kv+g), n_q/n_kv);
+ *   eta[g*G+j] = kappa[g]*G + rho_g[j]; k', v' row groups by kappa; q' row groups and o' column groups by eta.
+ * Asynchronous on `stream`. */
+typedef struct {
+    uint32_t hidden, inter, n_q, n_kv, head_dim;
+    cloak_dtype dt;
+    uint32_t layer;
+} cloak_block_shape;
+cloak_status cloak_permute_mlp_heads(uint64_t key, const cloak_block_shape* shape,
+                                     const void* d_gate, const void* d_up, const void* d_down,
+                                     const void* d_q, const void* d_k, const void* d_v, const void* d_o,
+                                     void* d_gate_o, void* d_up_o, void* d_down_o,
+                                     void* d_q_o, void* d_k_o, void* d_v_o, void* d_o_o, void* stream);
+
+/* Storage-layout conversion ROWMAJOR -> TILE128 of a logical [N, K] matrix (N, K multiples of 128).
+ * Out of place.  Asynchronous on `stream`. */
+cloak_status cloak_to_tile128(const void* d_src, void* d_dst, uint32_t N, uint32_t K, cloak_dtype dt,
+                              void* stream);
+
+/* ---- S6 / S7 the authorised read (north_star (c)).
+ * Y[m, n] = sum_k X[m, k] * W[n, k].  W lives in the pool at arena byte offset w_offset (a block
+ * multiple), logical shape [N, K], read through the pool's table T.  X [batch, K] and Y [batch, N] are
+ * row-major device buffers of W's dtype, 16-byte aligned.  Accumulation is fp32.
+ * cloak_gemv: batch 1..16, layout ROWMAJOR, K a multiple of 128 (bf16) / 128 (f32).
+ * cloak_gemm: batch 16..256 (multiple of 16), dtype BF16, layout TILE128, block_bytes >= 32 KiB
+ *             (tcgen05 tensor cores, accumulators in TMEM, tiles fetched by TMA through the table).
+ * Asynchronous on `stream`. */
+typedef struct {
+    uint64_t w_offset;
+    uint32_t N, K;
+    cloak_dtype dt;
+    cloak_layout layout;
+} cloak_tensor;
+cloak_status cloak_gemv(const cloak_pool* pool, const cloak_tensor* w, const void* d_x, void* d_y,
+                        uint32_t batch, void* stream);
+cloak_status cloak_gemm(const cloak_pool* pool, const cloak_tensor* w, const void* d_x, void* d_y,
+                        uint32_t batch, void* stream);
+/* Host-buffer variant of cloak_gemv (end-to-end path): copies X up, runs, copies Y back, synchronises. */
+cloak_status cloak_gemv_host(const cloak_pool* pool, const cloak_tensor* w, const void* h_x, void* h_y,
+                             uint32_t batch, void* stream);
+
+/* Decode-chain glue: out[i] = silu(g[i]) * u[i] (the gated MLP's activation, O9), n elements. */
+cloak_status cloak_silu_mul(const void* d_g, const void* d_u, void* d_out, uint64_t n, cloak_dtype dt,
+                            void* stream);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* CLOAK_H_ */

@@ -1,0 +1,213 @@
+"""Thin ctypes binding of libcloak.so: same names as include/cloak.h, argument marshalling only.
+
+Every step of the hot path runs in the CUDA library; this module adds no arithmetic.  PyTorch is used
+by callers for device memory and streams; here a "pointer" argument is a torch tensor (its data_ptr()
+is taken), a numpy array (host pointer) or a plain int address.  `stream` is a torch.cuda.Stream, an int
+cudaStream_t, or None (= torch's current stream when torch.cuda is initialised, else the default stream).
+
+The library must exist: importing this module raises if libcloak.so is missing (no CPU fallback).
+"""
+import ctypes
+import os
+from ctypes import (POINTER, Structure, byref, c_char_p, c_double, c_int, c_uint32, c_uint64, c_void_p)
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "libcloak.so")
+
+CLOAK_OK, CLOAK_ERR_INVALID, CLOAK_ERR_ALIGN, CLOAK_ERR_UNSUPPORTED, CLOAK_ERR_OOM, CLOAK_ERR_CUDA = 0, -1, -2, -3, -4, -5
+CLOAK_F32, CLOAK_BF16 = 0, 1
+CLOAK_ROWMAJOR, CLOAK_TILE128 = 0, 1
+CLOAK_POOL_IDENTITY, CLOAK_POOL_PLAIN_ALLOC = 1, 2
+STATUS_NAMES = {0: "CLOAK_OK", -1: "CLOAK_ERR_INVALID", -2: "CLOAK_ERR_ALIGN", -3: "CLOAK_ERR_UNSUPPORTED",
+                -4: "CLOAK_ERR_OOM", -5: "CLOAK_ERR_CUDA"}
+
+# every symbol include/cloak.h declares
+SYMBOLS = ["cloak_last_error", "cloak_version", "cloak_keygen", "cloak_pool_create", "cloak_pool_destroy",
+           "cloak_pool_info", "cloak_pool_tables", "cloak_pool_dump", "cloak_pool_map_ms", "cloak_shuffle",
+           "cloak_unshuffle", "cloak_relayout", "cloak_shuffle_host", "cloak_unshuffle_host",
+           "cloak_set_copy_engine", "cloak_arena_plan", "cloak_permute_mlp_heads", "cloak_to_tile128",
+           "cloak_gemv", "cloak_gemm", "cloak_gemv_host", "cloak_silu_mul"]
+
+
+class CloakError(RuntimeError):
+    def __init__(self, status, text):
+        super().__init__(f"{STATUS_NAMES.get(status, status)}: {text}")
+        self.status = status
+
+
+class cloak_block_shape(Structure):
+    _fields_ = [("hidden", c_uint32), ("inter", c_uint32), ("n_q", c_uint32), ("n_kv", c_uint32),
+                ("head_dim", c_uint32), ("dt", c_int), ("layer", c_uint32)]
+
+
+class cloak_tensor(Structure):
+    _fields_ = [("w_offset", c_uint64), ("N", c_uint32), ("K", c_uint32), ("dt", c_int), ("layout", c_int)]
+
+
+if not os.path.exists(LIB_PATH):
+    raise ImportError(f"{LIB_PATH} is missing: build it with `python -m paper_2606_18400_b200.build` "
+                      "(there is no CPU fallback)")
+lib = ctypes.CDLL(LIB_PATH)
+
+_P = c_void_p
+lib.cloak_last_error.restype = c_char_p
+lib.cloak_version.restype = c_char_p
+lib.cloak_keygen.argtypes = [c_uint64, c_uint64, c_uint32, _P, _P, _P]
+lib.cloak_pool_create.argtypes = [c_int, c_uint64, c_uint32, c_uint64, c_uint64, c_uint32, POINTER(_P)]
+lib.cloak_pool_destroy.argtypes = [_P]
+lib.cloak_pool_info.argtypes = [_P, POINTER(_P), POINTER(_P), POINTER(c_uint32), POINTER(c_uint32),
+                                POINTER(c_uint32), POINTER(c_int)]
+lib.cloak_pool_tables.argtypes = [_P, _P, _P, _P, _P]
+lib.cloak_pool_dump.argtypes = [_P, _P, _P]
+lib.cloak_pool_map_ms.argtypes = [_P, POINTER(c_double)]
+lib.cloak_shuffle.argtypes = [_P, _P, c_uint64, c_uint64, _P]
+lib.cloak_unshuffle.argtypes = [_P, _P, c_uint64, c_uint64, _P]
+lib.cloak_relayout.argtypes = [_P, _P, _P]
+lib.cloak_shuffle_host.argtypes = [_P, _P, c_uint64, c_uint64, _P]
+lib.cloak_unshuffle_host.argtypes = [_P, _P, c_uint64, c_uint64, _P]
+lib.cloak_set_copy_engine.argtypes = [c_int]
+lib.cloak_arena_plan.argtypes = [c_uint64, c_uint32, POINTER(c_uint64), c_uint32, POINTER(c_uint64), POINTER(c_uint64)]
+lib.cloak_permute_mlp_heads.argtypes = [c_uint64, POINTER(cloak_block_shape)] + [_P] * 15
+lib.cloak_to_tile128.argtypes = [_P, _P, c_uint32, c_uint32, c_int, _P]
+lib.cloak_gemv.argtypes = [_P, POINTER(cloak_tensor), _P, _P, c_uint32, _P]
+lib.cloak_gemm.argtypes = [_P, POINTER(cloak_tensor), _P, _P, c_uint32, _P]
+lib.cloak_gemv_host.argtypes = [_P, POINTER(cloak_tensor), _P, _P, c_uint32, _P]
+lib.cloak_silu_mul.argtypes = [_P, _P, _P, c_uint64, c_int, _P]
+for _n in SYMBOLS[2:]:
+    getattr(lib, _n).restype = c_int
+
+
+def _ptr(x):
+    """Address of a torch tensor / numpy array / int / None."""
+    if x is None:
+        return None
+    if isinstance(x, int):
+        return x
+    if hasattr(x, "data_ptr"):
+        return x.data_ptr()
+    if hasattr(x, "ctypes"):
+        return x.ctypes.data
+    raise TypeError(f"cannot take the address of {type(x)}")
+
+
+def _stream(s):
+    if s is None:
+        try:
+            import torch
+            if torch.cuda.is_available() and torch.cuda.is_initialized():
+                return torch.cuda.current_stream().cuda_stream
+        except ImportError:
+            pass
+        return None
+    if isinstance(s, int):
+        return s
+    return s.cuda_stream
+
+
+def _check(status):
+    if status != CLOAK_OK:
+        raise CloakError(status, lib.cloak_last_error().decode())
+
+
+def cloak_last_error():
+    return lib.cloak_last_error().decode()
+
+
+def cloak_version():
+    return lib.cloak_version().decode()
+
+
+def cloak_keygen(key, stream_id, n, d_perm, d_inv, stream=None):
+    _check(lib.cloak_keygen(key, stream_id, n, _ptr(d_perm), _ptr(d_inv), _stream(stream)))
+
+
+def cloak_pool_create(device, payload_bytes, block_bytes, page_bytes, key, flags=0):
+    out = _P()
+    _check(lib.cloak_pool_create(device, payload_bytes, block_bytes, page_bytes, key, flags, byref(out)))
+    return out
+
+
+def cloak_pool_destroy(pool):
+    _check(lib.cloak_pool_destroy(pool))
+
+
+def cloak_pool_info(pool):
+    base, tab = _P(), _P()
+    nb, nslots, npages, vmm = c_uint32(), c_uint32(), c_uint32(), c_int()
+    _check(lib.cloak_pool_info(pool, byref(base), byref(tab), byref(nb), byref(nslots), byref(npages), byref(vmm)))
+    return dict(d_base=base.value, d_table=tab.value, nb=nb.value, nslots=nslots.value, npages=npages.value,
+                is_vmm=bool(vmm.value))
+
+
+def cloak_pool_tables(pool, h_blockperm=None, h_blockinv=None, h_pageperm=None, h_pageinv=None):
+    _check(lib.cloak_pool_tables(pool, _ptr(h_blockperm), _ptr(h_blockinv), _ptr(h_pageperm), _ptr(h_pageinv)))
+
+
+def cloak_pool_dump(pool, d_out, stream=None):
+    _check(lib.cloak_pool_dump(pool, _ptr(d_out), _stream(stream)))
+
+
+def cloak_pool_map_ms(pool):
+    ms = c_double()
+    _check(lib.cloak_pool_map_ms(pool, byref(ms)))
+    return ms.value
+
+
+def cloak_shuffle(pool, d_logical, logical_offset, nbytes, stream=None):
+    _check(lib.cloak_shuffle(pool, _ptr(d_logical), logical_offset, nbytes, _stream(stream)))
+
+
+def cloak_unshuffle(pool, d_logical, logical_offset, nbytes, stream=None):
+    _check(lib.cloak_unshuffle(pool, _ptr(d_logical), logical_offset, nbytes, _stream(stream)))
+
+
+def cloak_relayout(from_a, to_b, stream=None):
+    _check(lib.cloak_relayout(from_a, to_b, _stream(stream)))
+
+
+def cloak_shuffle_host(pool, h_logical, logical_offset, nbytes, stream=None):
+    _check(lib.cloak_shuffle_host(pool, _ptr(h_logical), logical_offset, nbytes, _stream(stream)))
+
+
+def cloak_unshuffle_host(pool, h_logical, logical_offset, nbytes, stream=None):
+    _check(lib.cloak_unshuffle_host(pool, _ptr(h_logical), logical_offset, nbytes, _stream(stream)))
+
+
+def cloak_set_copy_engine(engine):
+    _check(lib.cloak_set_copy_engine(engine))
+
+
+def cloak_arena_plan(key, sizes, block_bytes):
+    T = len(sizes)
+    arr = (c_uint64 * max(T, 1))(*sizes)
+    offs = (c_uint64 * max(T, 1))()
+    total = c_uint64()
+    _check(lib.cloak_arena_plan(key, T, arr, block_bytes, offs, byref(total)))
+    return list(offs)[:T], total.value
+
+
+def cloak_permute_mlp_heads(key, shape, gate=None, up=None, down=None, q=None, k=None, v=None, o=None,
+                            gate_o=None, up_o=None, down_o=None, q_o=None, k_o=None, v_o=None, o_o=None,
+                            stream=None):
+    ptrs = [_ptr(t) for t in (gate, up, down, q, k, v, o, gate_o, up_o, down_o, q_o, k_o, v_o, o_o)]
+    _check(lib.cloak_permute_mlp_heads(key, byref(shape), *ptrs, _stream(stream)))
+
+
+def cloak_to_tile128(d_src, d_dst, N, K, dt, stream=None):
+    _check(lib.cloak_to_tile128(_ptr(d_src), _ptr(d_dst), N, K, dt, _stream(stream)))
+
+
+def cloak_gemv(pool, tensor, d_x, d_y, batch, stream=None):
+    _check(lib.cloak_gemv(pool, byref(tensor), _ptr(d_x), _ptr(d_y), batch, _stream(stream)))
+
+
+def cloak_gemm(pool, tensor, d_x, d_y, batch, stream=None):
+    _check(lib.cloak_gemm(pool, byref(tensor), _ptr(d_x), _ptr(d_y), batch, _stream(stream)))
+
+
+def cloak_gemv_host(pool, tensor, h_x, h_y, batch, stream=None):
+    _check(lib.cloak_gemv_host(pool, byref(tensor), _ptr(h_x), _ptr(h_y), batch, _stream(stream)))
+
+
+def cloak_silu_mul(d_g, d_u, d_out, n, dt, stream=None):
+    _check(lib.cloak_silu_mul(_ptr(d_g), _ptr(d_u), _ptr(d_out), n, dt, _stream(stream)))

@@ -1,0 +1,106 @@
+// Internal helpers of libcloak.so: status/error plumbing and the driver-API loader.
+// Not part of the C ABI (include/cloak.h is).
+#pragma once
+#include <cuda.h>
+#include <cuda_runtime.h>
+#include <stdint.h>
+#include <stdio.h>
+#include <vector>
+#include "cloak.h"
+
+namespace cloak {
+
+void set_error(const char* fmt, ...);
+cloak_status fail(cloak_status st, const char* fmt, ...);
+
+#define CLOAK_CUDA(call)                                                                        \
+    do {                                                                                        \
+        cudaError_t e__ = (call);                                                               \
+        if (e__ != cudaSuccess) {                                                               \
+            cudaGetLastError();                                                                 \
+            return ::cloak::fail(e__ == cudaErrorMemoryAllocation ? CLOAK_ERR_OOM : CLOAK_ERR_CUDA, \
+                                 "%s:%d %s: %s", __FILE__, __LINE__, #call, cudaGetErrorString(e__)); \
+        }                                                                                       \
+    } while (0)
+
+#define CLOAK_LAUNCH_CHECK()                                                                    \
+    do {                                                                                        \
+        cudaError_t e__ = cudaGetLastError();                                                   \
+        if (e__ != cudaSuccess)                                                                 \
+            return ::cloak::fail(CLOAK_ERR_CUDA, "%s:%d kernel launch: %s", __FILE__, __LINE__, \
+                                 cudaGetErrorString(e__));                                      \
+    } while (0)
+
+// Driver API entry points, resolved through the runtime (no link-time dependency on libcuda.so, so
+// the library loads on a box without a driver; calls then fail with CLOAK_ERR_CUDA).
+struct DriverApi {
+    CUresult (*MemGetAllocationGranularity)(size_t*, const CUmemAllocationProp*, CUmemAllocationGranularity_flags);
+    CUresult (*MemAddressReserve)(CUdeviceptr*, size_t, size_t, CUdeviceptr, unsigned long long);
+    CUresult (*MemAddressFree)(CUdeviceptr, size_t);
+    CUresult (*MemCreate)(CUmemGenericAllocationHandle*, size_t, const CUmemAllocationProp*, unsigned long long);
+    CUresult (*MemRelease)(CUmemGenericAllocationHandle);
+    CUresult (*MemMap)(CUdeviceptr, size_t, size_t, CUmemGenericAllocationHandle, unsigned long long);
+    CUresult (*MemUnmap)(CUdeviceptr, size_t);
+    CUresult (*MemSetAccess)(CUdeviceptr, size_t, const CUmemAccessDesc*, size_t);
+    CUresult (*GetErrorString)(CUresult, const char**);
+    CUresult (*TensorMapEncodeTiled)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*,
+                                     const cuuint64_t*, const cuuint32_t*, const cuuint32_t*,
+                                     CUtensorMapInterleave, CUtensorMapSwizzle, CUtensorMapL2promotion,
+                                     CUtensorMapFloatOOBfill);
+};
+// Returns nullptr (and sets the error text) when the driver is unavailable.
+const DriverApi* driver();
+const char* cu_err(CUresult r);
+
+#define CLOAK_CU(call)                                                                          \
+    do {                                                                                        \
+        CUresult r__ = (call);                                                                  \
+        if (r__ != CUDA_SUCCESS)                                                                \
+            return ::cloak::fail(r__ == CUDA_ERROR_OUT_OF_MEMORY ? CLOAK_ERR_OOM : CLOAK_ERR_CUDA, \
+                                 "%s:%d %s: %s", __FILE__, __LINE__, #call, ::cloak::cu_err(r__)); \
+    } while (0)
+
+// RAII guard: make `device` current for the duration of a call, restore afterwards.
+struct DeviceGuard {
+    int prev = -1;
+    bool ok = false;
+    explicit DeviceGuard(int device) {
+        if (cudaGetDevice(&prev) != cudaSuccess) { cudaGetLastError(); return; }
+        if (prev != device && cudaSetDevice(device) != cudaSuccess) { cudaGetLastError(); return; }
+        ok = true;
+    }
+    ~DeviceGuard() { if (ok && prev >= 0) cudaSetDevice(prev); }
+};
+
+int sm_count(int device);
+
+// keygen on the current device (keygen.cu).  Either output may be null.
+cloak_status keygen_device(uint64_t key, uint64_t stream_id, uint32_t n, uint32_t* d_perm, uint32_t* d_inv,
+                           cudaStream_t s);
+// Host-side Philox keygen used only by cloak_arena_plan (T is tiny; no device work wanted there).
+void keygen_host(uint64_t key, uint64_t stream_id, uint32_t n, std::vector<uint32_t>& perm);
+
+}  // namespace cloak
+
+// The pool object behind the opaque cloak_pool handle.
+struct cloak_pool {
+    int device = 0;
+    uint64_t payload = 0;       // B
+    uint32_t block = 0;         // b
+    uint32_t log2_block = 0;
+    uint64_t page = 0;          // P
+    uint64_t key = 0;
+    uint32_t flags = 0;
+    uint32_t nb = 0, bpp = 0, npages = 0, nslots = 0;
+    bool vmm = false;
+    double map_ms = 0.0;
+    char* base = nullptr;       // V (vmm) or D (emulated)
+    char* alias = nullptr;      // vmm only: handles mapped in creation order (the dump view), lazily
+    std::vector<CUmemGenericAllocationHandle> handles;   // index = physical page (creation order)
+    uint32_t* d_tables = nullptr;   // one allocation: blockperm | blockinv | pageperm | pageinv | T
+    uint32_t *d_blockperm = nullptr, *d_blockinv = nullptr, *d_pageperm = nullptr, *d_pageinv = nullptr,
+             *d_T = nullptr;
+    CUtensorMap tmap_tile128;   // GEMM: pool viewed as rows of 128 bf16 (gemm_sm100.cu), built lazily
+    bool tmap_ready = false;
+    uint64_t bytes() const { return (uint64_t)nslots * block; }
+};

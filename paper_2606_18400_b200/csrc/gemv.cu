@@ -1,0 +1,261 @@
+// S6 cloak_gemv: decode GEMV (batch 1..16) that reads W through the block table.
+//
+// Definition (north_star (c) "gather-fused GEMV (warp-level split-K reductions,
+// bandwidth-bound)"; "LLM inference is bandwidth-bound"):
+//     Y[m, n] = sum_k X[m, k] * W[n, k],  W row-major [N, K] at arena offset w_offset,
+//     byte x of the arena lives at  pool + (T[x >> log2 b] << log2 b) + (x & (b - 1)).
+// Weight bytes are read exactly once (N*K*e algorithmic bytes); HBM-bound.
+//
+// bf16 kernel.  One CTA = 16 output rows, 4 warps splitting K (split-K, reduced through shared memory in a
+// fixed order -> deterministic, and bit-identical between a cloaked and an identity-table pool).  Each lane
+// (g = lane/4, t = lane%4) loads 16-byte vectors W[g][k0+8t .. +8) and W[g+8][...], i.e. every load
+// instruction of a warp covers 8 rows x 64 contiguous bytes; two of them (k0, k0+32) consume whole 128-byte
+// lines.  The 8 bf16 of a vector feed two mma.sync.m16n8k16 (bf16 in, fp32 accumulate) as the A operand with
+// the batch as the N=8 operand: because a contraction may visit k in any order, lane t's vector elements
+// (8t+0..3 / 8t+4..7) are *declared* to be the MMA's k-slots (2t,2t+1,2t+8,2t+9); the X fragment is loaded
+// with the same rule (one 16-byte load of X[g][k0+8t .. +8)), so no shuffle or shared-memory transpose is
+// needed and the batch costs no extra weight traffic.  Tensor-pipe demand is ~0.1 PFLOP/s at batch 16:
+// the kernel stays on the HBM roofline where plain FMAs (52 TFMA/s needed, 37 available) could not.
+//
+// fp32 kernel (cfg0, correctness path): one warp per row, 16-byte loads, fp32 FMA, shuffle reduction.
+#include <cuda_bf16.h>
+#include "common.cuh"
+
+namespace cloak {
+
+struct GemvArgs {
+    const char* pool;
+    const uint32_t* T;
+    uint32_t log2b;
+    uint64_t w_offset;
+    uint32_t N, K;
+    const void* x;
+    void* y;
+    uint32_t batch;
+};
+
+__device__ __forceinline__ const char* xlate(const GemvArgs& a, uint64_t off) {
+    const uint32_t slot = __ldg(a.T + (off >> a.log2b));
+    return a.pool + ((uint64_t)slot << a.log2b) + (off & ((1ull << a.log2b) - 1));
+}
+
+__device__ __forceinline__ uint4 ld_w(const void* p) {
+    uint4 r;
+    asm volatile("ld.global.nc.L1::no_allocate.v4.u32 {%0,%1,%2,%3}, [%4];"
+                 : "=r"(r.x), "=r"(r.y), "=r"(r.z), "=r"(r.w) : "l"(p));
+    return r;
+}
+
+__device__ __forceinline__ void mma_bf16_16816(float c[4], uint32_t a0, uint32_t a1, uint32_t a2, uint32_t a3,
+                                               uint32_t b0, uint32_t b1) {
+    asm volatile("mma.sync.aligned.m16n8k16.row.col.f32.bf16.bf16.f32 {%0,%1,%2,%3}, {%4,%5,%6,%7}, {%8,%9}, {%0,%1,%2,%3};"
+                 : "+f"(c[0]), "+f"(c[1]), "+f"(c[2]), "+f"(c[3])
+                 : "r"(a0), "r"(a1), "r"(a2), "r"(a3), "r"(b0), "r"(b1));
+}
+
+constexpr int GV_WARPS = 4;
+constexpr int GV_ROWS = 16;
+constexpr int GV_KSTEP = 64;      // k elements per warp step: 2 vectors per row per lane
+constexpr int GV_UNROLL = 2;      // k-steps in flight per warp
+
+template <int NT>   // NT = number of 8-wide batch tiles (1: batch <= 8, 2: batch <= 16)
+__global__ void __launch_bounds__(GV_WARPS * 32) gemv_bf16_kernel(GemvArgs a) {
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const int g = lane >> 2, t = lane & 3;
+    const uint32_t n0 = blockIdx.x * GV_ROWS;
+    const uint64_t row_lo = a.w_offset + ((uint64_t)(n0 + g) * a.K + t * 8) * 2;
+    const uint64_t row_hi = row_lo + (uint64_t)8 * a.K * 2;
+    const uint16_t* X = static_cast<const uint16_t*>(a.x);
+    const bool xv0 = (uint32_t)g < a.batch, xv1 = (uint32_t)(g + 8) < a.batch;
+    const uint16_t* x0 = X + (size_t)g * a.K + t * 8;
+    const uint16_t* x1 = X + (size_t)(g + 8) * a.K + t * 8;
+
+    float acc[NT][4];
+#pragma unroll
+    for (int i = 0; i < NT; ++i)
+#pragma unroll
+        for (int j = 0; j < 4; ++j) acc[i][j] = 0.f;
+
+    const uint32_t ksteps = a.K / GV_KSTEP;
+    for (uint32_t ks = warp * GV_UNROLL; ks < ksteps; ks += GV_WARPS * GV_UNROLL) {
+        uint4 wl[GV_UNROLL][2], wh[GV_UNROLL][2], xa[GV_UNROLL][2], xb[GV_UNROLL][2];
+#pragma unroll
+        for (int u = 0; u < GV_UNROLL; ++u) {
+            const uint32_t k0 = (ks + u) * GV_KSTEP;
+            if (ks + u < ksteps) {
+                const char* pl = xlate(a, row_lo + (uint64_t)k0 * 2);   // 128-byte line of row g
+                const char* ph = xlate(a, row_hi + (uint64_t)k0 * 2);   // 128-byte line of row g+8
+                wl[u][0] = ld_w(pl);
+                wl[u][1] = ld_w(pl + 64);
+                wh[u][0] = ld_w(ph);
+                wh[u][1] = ld_w(ph + 64);
+            }
+        }
+#pragma unroll
+        for (int u = 0; u < GV_UNROLL; ++u) {
+            const uint32_t k0 = (ks + u) * GV_KSTEP;
+            const uint4 z = make_uint4(0, 0, 0, 0);
+            if (ks + u < ksteps) {
+                xa[u][0] = xv0 ? __ldg(reinterpret_cast<const uint4*>(x0 + k0)) : z;
+                xa[u][1] = xv0 ? __ldg(reinterpret_cast<const uint4*>(x0 + k0 + 32)) : z;
+                if (NT == 2) {
+                    xb[u][0] = xv1 ? __ldg(reinterpret_cast<const uint4*>(x1 + k0)) : z;
+                    xb[u][1] = xv1 ? __ldg(reinterpret_cast<const uint4*>(x1 + k0 + 32)) : z;
+                }
+            }
+        }
+#pragma unroll
+        for (int u = 0; u < GV_UNROLL; ++u) {
+            if (ks + u < ksteps) {
+#pragma unroll
+                for (int h = 0; h < 2; ++h) {
+                    mma_bf16_16816(acc[0], wl[u][h].x, wh[u][h].x, wl[u][h].y, wh[u][h].y, xa[u][h].x, xa[u][h].y);
+                    mma_bf16_16816(acc[0], wl[u][h].z, wh[u][h].z, wl[u][h].w, wh[u][h].w, xa[u][h].z, xa[u][h].w);
+                    if (NT == 2) {
+                        mma_bf16_16816(acc[1], wl[u][h].x, wh[u][h].x, wl[u][h].y, wh[u][h].y, xb[u][h].x, xb[u][h].y);
+                        mma_bf16_16816(acc[1], wl[u][h].z, wh[u][h].z, wl[u][h].w, wh[u][h].w, xb[u][h].z, xb[u][h].w);
+                    }
+                }
+            }
+        }
+    }
+
+    // Split-K reduction across the 4 warps in fixed order, then store Y[m, n0 + row] as bf16.
+    __shared__ float red[GV_WARPS][NT * 8][GV_ROWS + 1];      // [warp][batch m][row]
+#pragma unroll
+    for (int i = 0; i < NT; ++i) {
+        red[warp][i * 8 + 2 * t][g] = acc[i][0];
+        red[warp][i * 8 + 2 * t + 1][g] = acc[i][1];
+        red[warp][i * 8 + 2 * t][g + 8] = acc[i][2];
+        red[warp][i * 8 + 2 * t + 1][g + 8] = acc[i][3];
+    }
+    __syncthreads();
+    __nv_bfloat16* Y = static_cast<__nv_bfloat16*>(a.y);
+    for (uint32_t i = threadIdx.x; i < a.batch * GV_ROWS; i += blockDim.x) {
+        const uint32_t m = i / GV_ROWS, r = i % GV_ROWS;
+        float s = red[0][m][r];
+#pragma unroll
+        for (int w = 1; w < GV_WARPS; ++w) s += red[w][m][r];
+        Y[(size_t)m * a.N + n0 + r] = __float2bfloat16_rn(s);
+    }
+}
+
+// fp32: one warp per output row; lanes stride K in float4; batch accumulators in registers.
+template <int MB>
+__global__ void __launch_bounds__(256) gemv_f32_kernel(GemvArgs a) {
+    const int lane = threadIdx.x & 31;
+    const uint32_t row = blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5);
+    if (row >= a.N) return;
+    const float* X = static_cast<const float*>(a.x);
+    float acc[MB];
+#pragma unroll
+    for (int m = 0; m < MB; ++m) acc[m] = 0.f;
+    const uint64_t row_off = a.w_offset + (uint64_t)row * a.K * 4;
+    for (uint32_t k = lane * 4; k < a.K; k += 128) {
+        const float4 w = *reinterpret_cast<const float4*>(xlate(a, row_off + (uint64_t)k * 4));
+#pragma unroll
+        for (int m = 0; m < MB; ++m) {
+            if ((uint32_t)m < a.batch) {
+                const float4 x = __ldg(reinterpret_cast<const float4*>(X + (size_t)m * a.K + k));
+                acc[m] = fmaf(w.x, x.x, acc[m]);
+                acc[m] = fmaf(w.y, x.y, acc[m]);
+                acc[m] = fmaf(w.z, x.z, acc[m]);
+                acc[m] = fmaf(w.w, x.w, acc[m]);
+            }
+        }
+    }
+    float* Y = static_cast<float*>(a.y);
+#pragma unroll
+    for (int m = 0; m < MB; ++m) {
+        float s = acc[m];
+#pragma unroll
+        for (int d = 16; d > 0; d >>= 1) s += __shfl_xor_sync(0xffffffffu, s, d);
+        if (lane == 0 && (uint32_t)m < a.batch) Y[(size_t)m * a.N + row] = s;
+    }
+}
+
+cloak_status check_linear(const cloak_pool* pool, const cloak_tensor* w, const void* x, void* y, const char* who) {
+    if (!pool || !w || !x || !y) return fail(CLOAK_ERR_INVALID, "%s: NULL argument", who);
+    if (w->dt != CLOAK_F32 && w->dt != CLOAK_BF16) return fail(CLOAK_ERR_UNSUPPORTED, "%s: unknown dtype", who);
+    if (w->N == 0 || w->K == 0) return fail(CLOAK_ERR_INVALID, "%s: empty tensor", who);
+    if (w->w_offset % pool->block) return fail(CLOAK_ERR_ALIGN, "%s: w_offset is not a block multiple", who);
+    const uint64_t bytes = (uint64_t)w->N * w->K * (w->dt == CLOAK_F32 ? 4 : 2);
+    if (w->w_offset + bytes > (uint64_t)pool->nb * pool->block) return fail(CLOAK_ERR_INVALID, "%s: tensor exceeds the pool's arena", who);
+    if (((uintptr_t)x | (uintptr_t)y) & 15) return fail(CLOAK_ERR_ALIGN, "%s: x / y not 16-byte aligned", who);
+    return CLOAK_OK;
+}
+
+static cloak_status gemv_device(const cloak_pool* pool, const cloak_tensor* w, const void* d_x, void* d_y, uint32_t batch,
+                                cudaStream_t s) {
+    GemvArgs a;
+    a.pool = pool->base;
+    a.T = pool->d_T;
+    a.log2b = pool->log2_block;
+    a.w_offset = w->w_offset;
+    a.N = w->N;
+    a.K = w->K;
+    a.x = d_x;
+    a.y = d_y;
+    a.batch = batch;
+    if (w->dt == CLOAK_BF16) {
+        if (batch <= 8) gemv_bf16_kernel<1><<<w->N / GV_ROWS, GV_WARPS * 32, 0, s>>>(a);
+        else            gemv_bf16_kernel<2><<<w->N / GV_ROWS, GV_WARPS * 32, 0, s>>>(a);
+    } else {
+        const unsigned ctas = (w->N + 7) / 8;
+        if (batch <= 4) gemv_f32_kernel<4><<<ctas, 256, 0, s>>>(a);
+        else            gemv_f32_kernel<16><<<ctas, 256, 0, s>>>(a);
+    }
+    CLOAK_LAUNCH_CHECK();
+    return CLOAK_OK;
+}
+
+static cloak_status gemv_check(const cloak_pool* pool, const cloak_tensor* w, const void* x, void* y, uint32_t batch,
+                               const char* who) {
+    cloak_status st = check_linear(pool, w, x, y, who);
+    if (st != CLOAK_OK) return st;
+    if (batch < 1 || batch > 16) return fail(CLOAK_ERR_INVALID, "%s: batch must be in 1..16", who);
+    if (w->layout != CLOAK_ROWMAJOR) return fail(CLOAK_ERR_UNSUPPORTED, "%s: only CLOAK_ROWMAJOR is implemented", who);
+    if (w->dt == CLOAK_BF16) {
+        if (w->K % 64 || w->N % 16) return fail(CLOAK_ERR_ALIGN, "%s: bf16 needs K %% 64 == 0 and N %% 16 == 0", who);
+        if (pool->block < 128) return fail(CLOAK_ERR_UNSUPPORTED, "%s: bf16 needs block_bytes >= 128", who);
+    } else if (w->K % 4) {
+        return fail(CLOAK_ERR_ALIGN, "%s: f32 needs K %% 4 == 0", who);
+    }
+    return CLOAK_OK;
+}
+
+}  // namespace cloak
+
+using namespace cloak;
+
+extern "C" cloak_status cloak_gemv(const cloak_pool* pool, const cloak_tensor* w, const void* d_x, void* d_y,
+                                   uint32_t batch, void* stream) {
+    cloak_status st = gemv_check(pool, w, d_x, d_y, batch, "gemv");
+    if (st != CLOAK_OK) return st;
+    DeviceGuard g(pool->device);
+    return gemv_device(pool, w, d_x, d_y, batch, (cudaStream_t)stream);
+}
+
+extern "C" cloak_status cloak_gemv_host(const cloak_pool* pool, const cloak_tensor* w, const void* h_x, void* h_y,
+                                        uint32_t batch, void* stream) {
+    cloak_status st = gemv_check(pool, w, h_x, h_y, batch, "gemv_host");
+    if (st != CLOAK_OK) return st;
+    DeviceGuard g(pool->device);
+    cudaStream_t s = (cudaStream_t)stream;
+    const size_t e = w->dt == CLOAK_F32 ? 4 : 2;
+    const size_t xb = (size_t)batch * w->K * e, yb = (size_t)batch * w->N * e;
+    const size_t xpad = (xb + 255) & ~(size_t)255;
+    char* buf = nullptr;
+    CLOAK_CUDA(cudaMallocAsync((void**)&buf, xpad + yb, s));
+    cudaError_t err = cudaMemcpyAsync(buf, h_x, xb, cudaMemcpyHostToDevice, s);
+    if (err == cudaSuccess) {
+        st = gemv_device(pool, w, buf, buf + xpad, batch, s);
+        if (st == CLOAK_OK) err = cudaMemcpyAsync(h_y, buf + xpad, yb, cudaMemcpyDeviceToHost, s);
+    }
+    cudaFreeAsync(buf, s);
+    cudaError_t e2 = cudaStreamSynchronize(s);
+    if (st != CLOAK_OK) return st;
+    if (err != cudaSuccess) return fail(CLOAK_ERR_CUDA, "gemv_host copy: %s", cudaGetErrorString(err));
+    if (e2 != cudaSuccess) return fail(CLOAK_ERR_CUDA, "gemv_host sync: %s", cudaGetErrorString(e2));
+    return CLOAK_OK;
+}

@@ -1,0 +1,285 @@
+// S5 cloak_permute_mlp_heads (+ the TILE128 storage conversion and the gated-MLP activation glue).
+//
+// Definition (north_star (b) "rows of W_gate/W_up and columns of W_down, and whole attention
+// heads, permuted together"; PAPER.md:11 "intra-layer weight shuffling", :143 "tensor layout"):
+//   pi = keygen(key, (4<<32)|layer, inter);  gate'[r,:] = gate[pi[r],:], up'[r,:] = up[pi[r],:], down'[:,r] = down[:,pi[r]]
+//   kappa = keygen(key, (5<<32)|layer, n_kv); rho_g = keygen(key, (6<<32)|(layer*n_kv+g), G)
+//   eta[g*G+j] = kappa[g]*G + rho_g[j];  k',v' row groups by kappa; q' row groups, o' column groups by eta.
+// Bytes move exactly; HBM-bound (1 read + 1 write per byte).
+//   rows    : whole-row gather, 16-byte vectors, 4 rows in flight per CTA iteration.
+//   columns : the source row is staged in shared memory with coalesced 16-byte loads, the expanded column
+//             map sits in shared memory too, output vectors are assembled from shared memory and stored
+//             coalesced.
+#include "common.cuh"
+#include "philox.cuh"
+
+namespace cloak {
+
+// One CTA: kappa[n_kv] and eta[n_q] of O8 by rank counting in shared memory (n_kv, G <= 1024).
+__global__ void __launch_bounds__(1024) head_maps_kernel(uint32_t key_lo, uint32_t key_hi, uint32_t layer, uint32_t n_q,
+                                                         uint32_t n_kv, uint32_t* __restrict__ kappa,
+                                                         uint32_t* __restrict__ eta) {
+    __shared__ uint64_t r[1024];
+    __shared__ uint32_t kap[1024];
+    const uint32_t t = threadIdx.x;
+    const uint32_t G = n_q / n_kv;
+    if (t < n_kv) r[t] = philox_key64(t, layer, 5u, key_lo, key_hi);
+    __syncthreads();
+    if (t < n_kv) {
+        uint32_t rank = 0;
+        for (uint32_t k = 0; k < n_kv; ++k) rank += (r[k] < r[t]) || (r[k] == r[t] && k < t);
+        kap[rank] = t;
+        kappa[rank] = t;
+    }
+    __syncthreads();
+    for (uint32_t g = 0; g < n_kv; ++g) {
+        if (t < G) r[t] = philox_key64(t, layer * n_kv + g, 6u, key_lo, key_hi);
+        __syncthreads();
+        if (t < G) {
+            uint32_t rank = 0;
+            for (uint32_t k = 0; k < G; ++k) rank += (r[k] < r[t]) || (r[k] == r[t] && k < t);
+            eta[g * G + rank] = kap[g] * G + t;      // rho_g[rank] = t
+        }
+        __syncthreads();
+    }
+}
+
+__device__ __forceinline__ int4 ldg_stream(const void* p) {
+    int4 r;
+    asm volatile("ld.global.nc.L1::no_allocate.v4.s32 {%0,%1,%2,%3}, [%4];"
+                 : "=r"(r.x), "=r"(r.y), "=r"(r.z), "=r"(r.w) : "l"(p));
+    return r;
+}
+
+// dst row r' <- src row map[r' / seg] * seg + r' % seg;  rows of vpr 16-byte vectors.
+constexpr int ROWS_PER_IT = 4;
+__global__ void __launch_bounds__(256) gather_rows_kernel(const int4* __restrict__ src, int4* __restrict__ dst,
+                                                          const uint32_t* __restrict__ map, uint32_t seg,
+                                                          uint32_t nrows, uint32_t vpr) {
+    for (uint32_t r0 = blockIdx.x * ROWS_PER_IT; r0 < nrows; r0 += gridDim.x * ROWS_PER_IT) {
+        uint32_t srow[ROWS_PER_IT];
+#pragma unroll
+        for (int k = 0; k < ROWS_PER_IT; ++k) {
+            const uint32_t r = r0 + k;
+            srow[k] = r < nrows ? __ldg(map + r / seg) * seg + r % seg : 0u;
+        }
+        for (uint32_t v = threadIdx.x; v < vpr; v += blockDim.x) {
+            int4 x[ROWS_PER_IT];
+#pragma unroll
+            for (int k = 0; k < ROWS_PER_IT; ++k)
+                if (r0 + k < nrows) x[k] = ldg_stream(src + (uint64_t)srow[k] * vpr + v);
+#pragma unroll
+            for (int k = 0; k < ROWS_PER_IT; ++k)
+                if (r0 + k < nrows) dst[(uint64_t)(r0 + k) * vpr + v] = x[k];
+        }
+    }
+}
+
+// dst[row, c'] <- src[row, map[c' / seg] * seg + c' % seg], element type E (2 or 4 bytes).
+// Dynamic shared memory: colmap[ncols] (uint32) followed by one source row.
+template <typename E>
+__global__ void __launch_bounds__(256) gather_cols_kernel(const E* __restrict__ src, E* __restrict__ dst,
+                                                          const uint32_t* __restrict__ map, uint32_t seg,
+                                                          uint32_t nrows, uint32_t ncols) {
+    extern __shared__ __align__(16) unsigned char sm[];
+    uint32_t* colmap = reinterpret_cast<uint32_t*>(sm);
+    E* row = reinterpret_cast<E*>(sm + (((size_t)ncols * 4 + 15) & ~(size_t)15));
+    for (uint32_t c = threadIdx.x; c < ncols; c += blockDim.x) colmap[c] = __ldg(map + c / seg) * seg + c % seg;
+    constexpr int EPV = 16 / sizeof(E);
+    const uint32_t vpr = ncols / EPV;
+    for (uint32_t r = blockIdx.x; r < nrows; r += gridDim.x) {
+        __syncthreads();                                       // previous row fully consumed; colmap ready
+        const int4* s4 = reinterpret_cast<const int4*>(src + (uint64_t)r * ncols);
+        for (uint32_t v = threadIdx.x; v < vpr; v += blockDim.x) reinterpret_cast<int4*>(row)[v] = ldg_stream(s4 + v);
+        __syncthreads();
+        int4* d4 = reinterpret_cast<int4*>(dst + (uint64_t)r * ncols);
+        for (uint32_t v = threadIdx.x; v < vpr; v += blockDim.x) {
+            union { int4 q; E e[EPV]; } out;
+#pragma unroll
+            for (int k = 0; k < EPV; ++k) out.e[k] = row[colmap[v * EPV + k]];
+            d4[v] = out.q;
+        }
+    }
+}
+
+// Fallback when a row (+ map) does not fit in shared memory: gather straight from global memory.
+template <typename E>
+__global__ void __launch_bounds__(256) gather_cols_global_kernel(const E* __restrict__ src, E* __restrict__ dst,
+                                                                 const uint32_t* __restrict__ map, uint32_t seg,
+                                                                 uint32_t nrows, uint32_t ncols) {
+    const uint64_t total = (uint64_t)nrows * ncols;
+    for (uint64_t i = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x; i < total; i += (uint64_t)gridDim.x * blockDim.x) {
+        const uint32_t r = (uint32_t)(i / ncols), c = (uint32_t)(i % ncols);
+        dst[i] = src[(uint64_t)r * ncols + __ldg(map + c / seg) * seg + c % seg];
+    }
+}
+
+// ROWMAJOR [N, K] -> TILE128 (O11): one CTA per 128 x 128 tile, pure 16-byte index remap.
+__global__ void __launch_bounds__(256) tile128_kernel(const int4* __restrict__ src, int4* __restrict__ dst, uint32_t N,
+                                                      uint32_t K, uint32_t vptr /* vectors per tile row */) {
+    const uint32_t tiles_k = K / 128;
+    const uint32_t ntiles = (N / 128) * tiles_k;
+    const uint32_t vrow = tiles_k * vptr;                       // vectors per matrix row
+    for (uint32_t t = blockIdx.x; t < ntiles; t += gridDim.x) {
+        const uint32_t tn = t / tiles_k, tk = t % tiles_k;
+        const int4* s = src + (uint64_t)tn * 128 * vrow + (uint64_t)tk * vptr;
+        int4* d = dst + (uint64_t)t * 128 * vptr;
+        for (uint32_t v = threadIdx.x; v < 128 * vptr; v += 4 * blockDim.x) {
+            int4 x[4];
+#pragma unroll
+            for (int k = 0; k < 4; ++k) {
+                const uint32_t vv = v + k * blockDim.x;
+                x[k] = ldg_stream(s + (uint64_t)(vv / vptr) * vrow + vv % vptr);
+            }
+#pragma unroll
+            for (int k = 0; k < 4; ++k) d[v + k * blockDim.x] = x[k];
+        }
+    }
+}
+
+__global__ void silu_mul_f32_kernel(const float* __restrict__ g, const float* __restrict__ u, float* __restrict__ o,
+                                    uint64_t n) {
+    for (uint64_t i = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (uint64_t)gridDim.x * blockDim.x) {
+        const float z = g[i];
+        o[i] = z / (1.0f + __expf(-z)) * u[i];
+    }
+}
+__global__ void silu_mul_bf16_kernel(const uint16_t* __restrict__ g, const uint16_t* __restrict__ u,
+                                     uint16_t* __restrict__ o, uint64_t n) {
+    for (uint64_t i = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (uint64_t)gridDim.x * blockDim.x) {
+        const float z = __uint_as_float((uint32_t)g[i] << 16), w = __uint_as_float((uint32_t)u[i] << 16);
+        const float y = z / (1.0f + __expf(-z)) * w;
+        uint32_t b = __float_as_uint(y);
+        b += 0x7FFFu + ((b >> 16) & 1u);                       // round to nearest even
+        o[i] = (uint16_t)(b >> 16);
+    }
+}
+
+static cloak_status rows(const void* src, void* dst, const uint32_t* map, uint32_t seg, uint32_t nrows,
+                         uint64_t row_bytes, int sms, cudaStream_t s) {
+    uint32_t ctas = (nrows + ROWS_PER_IT - 1) / ROWS_PER_IT;
+    const uint32_t cap = (uint32_t)sms * 8;
+    if (ctas > cap) ctas = cap;
+    gather_rows_kernel<<<ctas, 256, 0, s>>>((const int4*)src, (int4*)dst, map, seg, nrows, (uint32_t)(row_bytes / 16));
+    CLOAK_LAUNCH_CHECK();
+    return CLOAK_OK;
+}
+
+template <typename E>
+static cloak_status cols(const void* src, void* dst, const uint32_t* map, uint32_t seg, uint32_t nrows, uint32_t ncols,
+                         int sms, cudaStream_t s) {
+    const size_t smem = (((size_t)ncols * 4 + 15) & ~(size_t)15) + (size_t)ncols * sizeof(E);
+    if (smem <= 200 * 1024) {
+        static bool attr_set = false;
+        if (!attr_set) {
+            CLOAK_CUDA(cudaFuncSetAttribute(gather_cols_kernel<E>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024));
+            attr_set = true;
+        }
+        const uint32_t per_sm = smem <= 100 * 1024 ? 2u : 1u;
+        uint32_t ctas = nrows < (uint32_t)sms * per_sm ? nrows : (uint32_t)sms * per_sm;
+        gather_cols_kernel<E><<<ctas, 256, smem, s>>>((const E*)src, (E*)dst, map, seg, nrows, ncols);
+    } else {
+        gather_cols_global_kernel<E><<<sms * 8, 256, 0, s>>>((const E*)src, (E*)dst, map, seg, nrows, ncols);
+    }
+    CLOAK_LAUNCH_CHECK();
+    return CLOAK_OK;
+}
+
+}  // namespace cloak
+
+using namespace cloak;
+
+extern "C" cloak_status cloak_permute_mlp_heads(uint64_t key, const cloak_block_shape* sh, const void* d_gate,
+                                                const void* d_up, const void* d_down, const void* d_q, const void* d_k,
+                                                const void* d_v, const void* d_o, void* d_gate_o, void* d_up_o,
+                                                void* d_down_o, void* d_q_o, void* d_k_o, void* d_v_o, void* d_o_o,
+                                                void* stream) {
+    if (!sh) return fail(CLOAK_ERR_INVALID, "permute: shape is NULL");
+    if (sh->dt != CLOAK_F32 && sh->dt != CLOAK_BF16) return fail(CLOAK_ERR_UNSUPPORTED, "permute: unknown dtype");
+    const void* in[7] = {d_gate, d_up, d_down, d_q, d_k, d_v, d_o};
+    void* out[7] = {d_gate_o, d_up_o, d_down_o, d_q_o, d_k_o, d_v_o, d_o_o};
+    bool any = false, mlp = false, heads = false;
+    for (int i = 0; i < 7; ++i) {
+        if ((in[i] == nullptr) != (out[i] == nullptr)) return fail(CLOAK_ERR_INVALID, "permute: src/dst %d must both be set or both NULL", i);
+        if (in[i]) {
+            if (in[i] == out[i]) return fail(CLOAK_ERR_INVALID, "permute: in-place permutation is not supported");
+            if (((uintptr_t)in[i] | (uintptr_t)out[i]) & 15) return fail(CLOAK_ERR_ALIGN, "permute: tensor %d not 16-byte aligned", i);
+            any = true;
+            (i < 3 ? mlp : heads) = true;
+        }
+    }
+    if (!any) return fail(CLOAK_ERR_INVALID, "permute: nothing to do");
+    const uint32_t e = sh->dt == CLOAK_F32 ? 4 : 2;
+    const uint32_t epv = 16 / e;
+    if (sh->hidden == 0 || sh->hidden % epv) return fail(CLOAK_ERR_ALIGN, "permute: hidden must be a multiple of %u", epv);
+    if (mlp && (sh->inter == 0 || sh->inter % epv)) return fail(CLOAK_ERR_ALIGN, "permute: inter must be a multiple of %u", epv);
+    if (heads) {
+        if (sh->n_q == 0 || sh->n_kv == 0 || sh->head_dim == 0 || sh->n_q % sh->n_kv)
+            return fail(CLOAK_ERR_INVALID, "permute: n_q must be a non-zero multiple of n_kv, head_dim > 0");
+        if (sh->n_kv > 1024 || sh->n_q / sh->n_kv > 1024) return fail(CLOAK_ERR_UNSUPPORTED, "permute: more than 1024 KV heads or group size");
+        if ((sh->n_q * sh->head_dim) % epv) return fail(CLOAK_ERR_ALIGN, "permute: n_q*head_dim must be a multiple of %u", epv);
+    }
+    cudaStream_t s = (cudaStream_t)stream;
+    int dev = 0;
+    CLOAK_CUDA(cudaGetDevice(&dev));
+    const int sms = sm_count(dev);
+    const size_t n_scratch = (size_t)(mlp ? sh->inter : 0) + (heads ? sh->n_kv + sh->n_q : 0);
+    uint32_t* scratch = nullptr;
+    CLOAK_CUDA(cudaMallocAsync((void**)&scratch, n_scratch * 4, s));
+    uint32_t* pi = scratch;
+    uint32_t* kappa = scratch + (mlp ? sh->inter : 0);
+    uint32_t* eta = kappa + sh->n_kv;
+    cloak_status st = CLOAK_OK;
+    const uint64_t hrow = (uint64_t)sh->hidden * e;
+    if (mlp) {
+        st = keygen_device(key, (4ull << 32) | sh->layer, sh->inter, pi, nullptr, s);
+        if (st == CLOAK_OK && d_gate) st = rows(d_gate, d_gate_o, pi, 1, sh->inter, hrow, sms, s);
+        if (st == CLOAK_OK && d_up) st = rows(d_up, d_up_o, pi, 1, sh->inter, hrow, sms, s);
+        if (st == CLOAK_OK && d_down)
+            st = e == 4 ? cols<uint32_t>(d_down, d_down_o, pi, 1, sh->hidden, sh->inter, sms, s)
+                        : cols<uint16_t>(d_down, d_down_o, pi, 1, sh->hidden, sh->inter, sms, s);
+    }
+    if (st == CLOAK_OK && heads) {
+        head_maps_kernel<<<1, 1024, 0, s>>>((uint32_t)key, (uint32_t)(key >> 32), sh->layer, sh->n_q, sh->n_kv, kappa, eta);
+        if (cudaGetLastError() != cudaSuccess) st = fail(CLOAK_ERR_CUDA, "permute: head_maps launch failed");
+        const uint32_t d = sh->head_dim;
+        if (st == CLOAK_OK && d_q) st = rows(d_q, d_q_o, eta, d, sh->n_q * d, hrow, sms, s);
+        if (st == CLOAK_OK && d_k) st = rows(d_k, d_k_o, kappa, d, sh->n_kv * d, hrow, sms, s);
+        if (st == CLOAK_OK && d_v) st = rows(d_v, d_v_o, kappa, d, sh->n_kv * d, hrow, sms, s);
+        if (st == CLOAK_OK && d_o)
+            st = e == 4 ? cols<uint32_t>(d_o, d_o_o, eta, d, sh->hidden, sh->n_q * d, sms, s)
+                        : cols<uint16_t>(d_o, d_o_o, eta, d, sh->hidden, sh->n_q * d, sms, s);
+    }
+    cudaFreeAsync(scratch, s);
+    return st;
+}
+
+extern "C" cloak_status cloak_to_tile128(const void* d_src, void* d_dst, uint32_t N, uint32_t K, cloak_dtype dt,
+                                         void* stream) {
+    if (!d_src || !d_dst || d_src == d_dst) return fail(CLOAK_ERR_INVALID, "to_tile128: NULL or aliased pointers");
+    if (dt != CLOAK_F32 && dt != CLOAK_BF16) return fail(CLOAK_ERR_UNSUPPORTED, "to_tile128: unknown dtype");
+    if (N == 0 || K == 0 || N % 128 || K % 128) return fail(CLOAK_ERR_ALIGN, "to_tile128: N and K must be multiples of 128");
+    if (((uintptr_t)d_src | (uintptr_t)d_dst) & 15) return fail(CLOAK_ERR_ALIGN, "to_tile128: pointers not 16-byte aligned");
+    int dev = 0;
+    CLOAK_CUDA(cudaGetDevice(&dev));
+    const uint32_t ntiles = (N / 128) * (K / 128);
+    const uint32_t cap = (uint32_t)sm_count(dev) * 8;
+    tile128_kernel<<<ntiles < cap ? ntiles : cap, 256, 0, (cudaStream_t)stream>>>(
+        (const int4*)d_src, (int4*)d_dst, N, K, dt == CLOAK_F32 ? 32u : 16u);
+    CLOAK_LAUNCH_CHECK();
+    return CLOAK_OK;
+}
+
+extern "C" cloak_status cloak_silu_mul(const void* d_g, const void* d_u, void* d_out, uint64_t n, cloak_dtype dt,
+                                       void* stream) {
+    if (!d_g || !d_u || !d_out || n == 0) return fail(CLOAK_ERR_INVALID, "silu_mul: NULL argument or n == 0");
+    const unsigned blocks = (unsigned)((n + 255) / 256 < 1184 ? (n + 255) / 256 : 1184);
+    if (dt == CLOAK_F32)
+        silu_mul_f32_kernel<<<blocks, 256, 0, (cudaStream_t)stream>>>((const float*)d_g, (const float*)d_u, (float*)d_out, n);
+    else if (dt == CLOAK_BF16)
+        silu_mul_bf16_kernel<<<blocks, 256, 0, (cudaStream_t)stream>>>((const uint16_t*)d_g, (const uint16_t*)d_u, (uint16_t*)d_out, n);
+    else
+        return fail(CLOAK_ERR_UNSUPPORTED, "silu_mul: unknown dtype");
+    CLOAK_LAUNCH_CHECK();
+    return CLOAK_OK;
+}

@@ -1,0 +1,256 @@
+// S2 the page pool: geometry, keyed block/page tables, and the VMM mapper (host C++).
+//
+// Paper: Tier 2 "randomizes the mapping of virtual addresses to physical HBM pages" with the CUDA VMM
+// API at 2 MB granularity; "tensor pointers and access semantics remain unchanged" (
+// Table 1b :192-201); pages are allocated in permuted order *before* any weight is transferred
+// (PAPER.md:217).  Definitions O4-O5 and reading G6 of SURVEY.md 8(c): handle-creation order stands for
+// physical order; emulated pages fold the page map into the table.
+#include <chrono>
+#include "common.cuh"
+
+namespace cloak {
+
+__global__ void iota_kernel(uint32_t* a, uint32_t n) {
+    uint32_t i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i < n) a[i] = i;
+}
+
+// T[i] = blockinv[i] (real pages)  or  pageinv[blockinv[i] / bpp] * bpp + blockinv[i] % bpp (emulated).
+__global__ void build_table_kernel(const uint32_t* __restrict__ blockinv, const uint32_t* __restrict__ pageinv,
+                                   uint32_t* __restrict__ T, uint32_t nb, uint32_t bpp, int vmm) {
+    uint32_t i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i < nb) {
+        uint32_t s = blockinv[i];
+        T[i] = vmm ? s : pageinv[s / bpp] * bpp + s % bpp;
+    }
+}
+
+static cloak_status destroy_impl(cloak_pool* p) {
+    if (!p) return CLOAK_OK;
+    DeviceGuard g(p->device);
+    const DriverApi* d = driver();
+    cudaDeviceSynchronize();
+    if (p->vmm && d) {
+        if (p->alias) {
+            d->MemUnmap((CUdeviceptr)p->alias, p->bytes());
+            d->MemAddressFree((CUdeviceptr)p->alias, p->bytes());
+        }
+        if (p->base) {
+            d->MemUnmap((CUdeviceptr)p->base, p->bytes());
+            d->MemAddressFree((CUdeviceptr)p->base, p->bytes());
+        }
+        for (auto h : p->handles) d->MemRelease(h);
+    } else if (p->base) {
+        cudaFree(p->base);
+    }
+    if (p->d_tables) cudaFree(p->d_tables);
+    cudaGetLastError();
+    delete p;
+    return CLOAK_OK;
+}
+
+static cloak_status map_pages(cloak_pool* p, const std::vector<uint32_t>& pageinv) {
+    const DriverApi* d = driver();
+    if (!d) return CLOAK_ERR_CUDA;
+    CUmemAllocationProp prop = {};
+    prop.type = CU_MEM_ALLOCATION_TYPE_PINNED;
+    prop.location.type = CU_MEM_LOCATION_TYPE_DEVICE;
+    prop.location.id = p->device;
+    auto t0 = std::chrono::steady_clock::now();
+    CUdeviceptr va = 0;
+    CLOAK_CU(d->MemAddressReserve(&va, p->bytes(), 0, 0, 0));
+    p->base = (char*)va;
+    p->handles.reserve(p->npages);
+    for (uint32_t i = 0; i < p->npages; ++i) {          // creation order == physical page index (G6)
+        CUmemGenericAllocationHandle h;
+        CLOAK_CU(d->MemCreate(&h, p->page, &prop, 0));
+        p->handles.push_back(h);
+    }
+    for (uint32_t v = 0; v < p->npages; ++v)             // VA page v is backed by physical page pageinv[v]
+        CLOAK_CU(d->MemMap(va + (uint64_t)v * p->page, p->page, 0, p->handles[pageinv[v]], 0));
+    CUmemAccessDesc acc = {};
+    acc.location = prop.location;
+    acc.flags = CU_MEM_ACCESS_FLAGS_PROT_READWRITE;
+    CLOAK_CU(d->MemSetAccess(va, p->bytes(), &acc, 1));
+    p->map_ms = std::chrono::duration<double, std::milli>(std::chrono::steady_clock::now() - t0).count();
+    return CLOAK_OK;
+}
+
+static cloak_status ensure_alias(cloak_pool* p) {
+    if (p->alias) return CLOAK_OK;
+    const DriverApi* d = driver();
+    if (!d) return CLOAK_ERR_CUDA;
+    CUdeviceptr va = 0;
+    CLOAK_CU(d->MemAddressReserve(&va, p->bytes(), 0, 0, 0));
+    for (uint32_t i = 0; i < p->npages; ++i) {
+        CUresult r = d->MemMap(va + (uint64_t)i * p->page, p->page, 0, p->handles[i], 0);
+        if (r != CUDA_SUCCESS) {
+            if (i) d->MemUnmap(va, (uint64_t)i * p->page);
+            d->MemAddressFree(va, p->bytes());
+            return fail(CLOAK_ERR_CUDA, "alias cuMemMap: %s", cu_err(r));
+        }
+    }
+    CUmemAccessDesc acc = {};
+    acc.location.type = CU_MEM_LOCATION_TYPE_DEVICE;
+    acc.location.id = p->device;
+    acc.flags = CU_MEM_ACCESS_FLAGS_PROT_READWRITE;
+    CLOAK_CU(d->MemSetAccess(va, p->bytes(), &acc, 1));
+    p->alias = (char*)va;
+    return CLOAK_OK;
+}
+
+static cloak_status create_impl(cloak_pool* p) {
+    DeviceGuard g(p->device);
+    if (!g.ok) return fail(CLOAK_ERR_CUDA, "pool_create: cannot select device %d", p->device);
+    const bool identity = p->flags & CLOAK_POOL_IDENTITY;
+    size_t gran = 0;
+    if (!(p->flags & CLOAK_POOL_PLAIN_ALLOC)) {
+        const DriverApi* d = driver();
+        if (!d) return CLOAK_ERR_CUDA;
+        CUmemAllocationProp prop = {};
+        prop.type = CU_MEM_ALLOCATION_TYPE_PINNED;
+        prop.location.type = CU_MEM_LOCATION_TYPE_DEVICE;
+        prop.location.id = p->device;
+        CLOAK_CUDA(cudaFree(0));   // make sure the primary context exists before driver calls
+        CLOAK_CU(d->MemGetAllocationGranularity(&gran, &prop, CU_MEM_ALLOC_GRANULARITY_MINIMUM));
+        p->vmm = gran != 0 && p->page % gran == 0;
+    }
+    const size_t ntab = 2 * (size_t)p->nslots + 2 * (size_t)p->npages + p->nb;
+    CLOAK_CUDA(cudaMalloc((void**)&p->d_tables, ntab * sizeof(uint32_t)));
+    p->d_blockperm = p->d_tables;
+    p->d_blockinv = p->d_blockperm + p->nslots;
+    p->d_pageperm = p->d_blockinv + p->nslots;
+    p->d_pageinv = p->d_pageperm + p->npages;
+    p->d_T = p->d_pageinv + p->npages;
+
+    cudaStream_t s;
+    CLOAK_CUDA(cudaStreamCreateWithFlags(&s, cudaStreamNonBlocking));
+    cloak_status st = CLOAK_OK;
+    auto run = [&]() -> cloak_status {
+        if (identity) {
+            iota_kernel<<<(p->nslots + 255) / 256, 256, 0, s>>>(p->d_blockperm, p->nslots);
+            iota_kernel<<<(p->nslots + 255) / 256, 256, 0, s>>>(p->d_blockinv, p->nslots);
+            iota_kernel<<<(p->npages + 255) / 256, 256, 0, s>>>(p->d_pageperm, p->npages);
+            iota_kernel<<<(p->npages + 255) / 256, 256, 0, s>>>(p->d_pageinv, p->npages);
+            CLOAK_LAUNCH_CHECK();
+        } else {
+            cloak_status e = keygen_device(p->key, 1ull << 32, p->nslots, p->d_blockperm, p->d_blockinv, s);
+            if (e != CLOAK_OK) return e;
+            e = keygen_device(p->key, 2ull << 32, p->npages, p->d_pageperm, p->d_pageinv, s);
+            if (e != CLOAK_OK) return e;
+        }
+        build_table_kernel<<<(p->nb + 255) / 256, 256, 0, s>>>(p->d_blockinv, p->d_pageinv, p->d_T, p->nb, p->bpp,
+                                                               p->vmm ? 1 : 0);
+        CLOAK_LAUNCH_CHECK();
+        std::vector<uint32_t> pageinv(p->npages);
+        CLOAK_CUDA(cudaMemcpyAsync(pageinv.data(), p->d_pageinv, (size_t)p->npages * 4, cudaMemcpyDeviceToHost, s));
+        CLOAK_CUDA(cudaStreamSynchronize(s));
+        if (p->vmm) {
+            cloak_status e = map_pages(p, pageinv);
+            if (e != CLOAK_OK) return e;
+        } else {
+            CLOAK_CUDA(cudaMalloc((void**)&p->base, p->bytes()));
+        }
+        CLOAK_CUDA(cudaMemsetAsync(p->base, 0, p->bytes(), s));
+        CLOAK_CUDA(cudaStreamSynchronize(s));
+        return CLOAK_OK;
+    };
+    st = run();
+    cudaStreamDestroy(s);
+    return st;
+}
+
+}  // namespace cloak
+
+extern "C" cloak_status cloak_pool_create(int device, uint64_t payload_bytes, uint32_t block_bytes,
+                                          uint64_t page_bytes, uint64_t key, uint32_t flags, cloak_pool** out) {
+    using namespace cloak;
+    if (!out) return fail(CLOAK_ERR_INVALID, "pool_create: out is NULL");
+    *out = nullptr;
+    if (payload_bytes == 0 || device < 0) return fail(CLOAK_ERR_INVALID, "pool_create: payload_bytes == 0 or bad device");
+    if (block_bytes < 16 || (block_bytes & (block_bytes - 1)))
+        return fail(CLOAK_ERR_UNSUPPORTED, "pool_create: block_bytes must be a power of two >= 16");
+    if (page_bytes == 0 || page_bytes % block_bytes)
+        return fail(CLOAK_ERR_ALIGN, "pool_create: page_bytes must be a non-zero multiple of block_bytes");
+    if (flags & ~(uint32_t)(CLOAK_POOL_IDENTITY | CLOAK_POOL_PLAIN_ALLOC))
+        return fail(CLOAK_ERR_INVALID, "pool_create: unknown flag bits");
+    const uint64_t nb = (payload_bytes + block_bytes - 1) / block_bytes;
+    const uint64_t bpp = page_bytes / block_bytes;
+    const uint64_t npages = (nb + bpp - 1) / bpp;
+    const uint64_t nslots = npages * bpp;
+    if (nslots > (1ull << 28) || bpp > 0xffffffffull)
+        return fail(CLOAK_ERR_UNSUPPORTED, "pool_create: more than 2^28 block slots");
+    cloak_pool* p = new (std::nothrow) cloak_pool();
+    if (!p) return fail(CLOAK_ERR_OOM, "pool_create: host allocation failed");
+    p->device = device;
+    p->payload = payload_bytes;
+    p->block = block_bytes;
+    p->log2_block = 0;
+    while ((1u << p->log2_block) < block_bytes) ++p->log2_block;
+    p->page = page_bytes;
+    p->key = key;
+    p->flags = flags;
+    p->nb = (uint32_t)nb;
+    p->bpp = (uint32_t)bpp;
+    p->npages = (uint32_t)npages;
+    p->nslots = (uint32_t)nslots;
+    cloak_status st = create_impl(p);
+    if (st != CLOAK_OK) {
+        char keep[512];
+        snprintf(keep, sizeof(keep), "%s", cloak_last_error());
+        destroy_impl(p);
+        set_error("%s", keep);
+        return st;
+    }
+    *out = p;
+    return CLOAK_OK;
+}
+
+extern "C" cloak_status cloak_pool_destroy(cloak_pool* pool) {
+    if (!pool) return cloak::fail(CLOAK_ERR_INVALID, "pool_destroy: NULL pool");
+    return cloak::destroy_impl(pool);
+}
+
+extern "C" cloak_status cloak_pool_info(const cloak_pool* pool, void** d_base, const uint32_t** d_table, uint32_t* nb,
+                                        uint32_t* nslots, uint32_t* npages, int* is_vmm) {
+    if (!pool) return cloak::fail(CLOAK_ERR_INVALID, "pool_info: NULL pool");
+    if (d_base) *d_base = pool->base;
+    if (d_table) *d_table = pool->d_T;
+    if (nb) *nb = pool->nb;
+    if (nslots) *nslots = pool->nslots;
+    if (npages) *npages = pool->npages;
+    if (is_vmm) *is_vmm = pool->vmm ? 1 : 0;
+    return CLOAK_OK;
+}
+
+extern "C" cloak_status cloak_pool_tables(const cloak_pool* pool, uint32_t* h_blockperm, uint32_t* h_blockinv,
+                                          uint32_t* h_pageperm, uint32_t* h_pageinv) {
+    using namespace cloak;
+    if (!pool) return fail(CLOAK_ERR_INVALID, "pool_tables: NULL pool");
+    DeviceGuard g(pool->device);
+    if (h_blockperm) CLOAK_CUDA(cudaMemcpy(h_blockperm, pool->d_blockperm, (size_t)pool->nslots * 4, cudaMemcpyDeviceToHost));
+    if (h_blockinv) CLOAK_CUDA(cudaMemcpy(h_blockinv, pool->d_blockinv, (size_t)pool->nslots * 4, cudaMemcpyDeviceToHost));
+    if (h_pageperm) CLOAK_CUDA(cudaMemcpy(h_pageperm, pool->d_pageperm, (size_t)pool->npages * 4, cudaMemcpyDeviceToHost));
+    if (h_pageinv) CLOAK_CUDA(cudaMemcpy(h_pageinv, pool->d_pageinv, (size_t)pool->npages * 4, cudaMemcpyDeviceToHost));
+    return CLOAK_OK;
+}
+
+extern "C" cloak_status cloak_pool_dump(const cloak_pool* pool, void* d_out, void* stream) {
+    using namespace cloak;
+    if (!pool || !d_out) return fail(CLOAK_ERR_INVALID, "pool_dump: NULL argument");
+    DeviceGuard g(pool->device);
+    const char* src = pool->base;
+    if (pool->vmm) {
+        cloak_status st = ensure_alias(const_cast<cloak_pool*>(pool));
+        if (st != CLOAK_OK) return st;
+        src = pool->alias;
+    }
+    CLOAK_CUDA(cudaMemcpyAsync(d_out, src, pool->bytes(), cudaMemcpyDeviceToDevice, (cudaStream_t)stream));
+    return CLOAK_OK;
+}
+
+extern "C" cloak_status cloak_pool_map_ms(const cloak_pool* pool, double* ms) {
+    if (!pool || !ms) return cloak::fail(CLOAK_ERR_INVALID, "pool_map_ms: NULL argument");
+    *ms = pool->map_ms;
+    return CLOAK_OK;
+}

@@ -1,0 +1,359 @@
+"""GPU parity: the CUDA library (through the C ABI binding) against the CPU oracle, element by element.
+
+Integer / byte / index work must be bit-exact.  GEMV outputs: O12 norm-wise error <= 2e-2 (bf16) and
+<= 1e-5 (fp32), the tolerances BASELINE.json's north_star states.
+"""
+import numpy as np
+import pytest
+import torch
+
+import oracle as O
+from synth import gen
+
+pytestmark = pytest.mark.gpu
+
+if torch.cuda.is_available():
+    import paper_2606_18400_b200 as C
+    from synth import cuda as synth_cuda
+    from gpu_util import (Pool, dev_bytes, to_dev_bytes, to_host_bytes, bf16_dev_from_bits, bits_from_bf16_dev)
+
+TOL = {"bf16": 2e-2, "f32": 1e-5}
+
+
+# ------------------------------------------------------------------ harness twin
+@pytest.mark.parametrize("dtype", ["f32", "bf16"])
+def test_synth_twins_agree(dtype):
+    n, start = 100003, (1 << 32) + 12345
+    t = torch.empty(n, dtype=torch.float32 if dtype == "f32" else torch.bfloat16, device="cuda")
+    for kind in (gen.KIND_WEIGHT, gen.KIND_NORMAL):
+        synth_cuda.fill(t, 7, 3, kind=kind, start=start)
+        ref = gen.synth(7, 3, (n,), dtype, kind=kind, start=start)
+        got = t.cpu().numpy() if dtype == "f32" else bits_from_bf16_dev(t)
+        assert np.array_equal(got, ref)
+
+
+# ------------------------------------------------------------------ S1 keygen
+@pytest.mark.parametrize("n", [1, 2, 8, 16, 256, 1024, 4096, 4097, 14336, 245056, 1 << 20, (1 << 20) + 77])
+def test_keygen_bit_exact(n):
+    perm = torch.empty(n, dtype=torch.int32, device="cuda")
+    inv = torch.empty(n, dtype=torch.int32, device="cuda")
+    for key, stream in [(0x1234, 0), (0xDEADBEEF12345678, (5 << 32) | 9)]:
+        C.cloak_keygen(key, stream, n, perm, inv)
+        rp, ri = O.keygen(key, stream, n)
+        assert np.array_equal(perm.cpu().numpy().view(np.uint32), rp)
+        assert np.array_equal(inv.cpu().numpy().view(np.uint32), ri)
+    C.cloak_keygen(0x1234, 0, n, perm, None)          # either output may be NULL
+    inv.zero_()
+    C.cloak_keygen(0x1234, 0, n, None, inv)
+    rp, ri = O.keygen(0x1234, 0, n)
+    assert np.array_equal(perm.cpu().numpy().view(np.uint32), rp)
+    assert np.array_equal(inv.cpu().numpy().view(np.uint32), ri)
+
+
+# ------------------------------------------------------------------ S2/S4 pool, shuffle, unshuffle
+POOLS = [
+    # (payload, block, page, flags)             what it covers
+    (1 << 20, 4096, 65536, 0),                   # cfg0 one matrix: 256 blocks, 16 emulated 64 KiB pages
+    (3 << 20, 4096, 65536, 0),                   # cfg0 three matrices: 768 blocks, 48 pages
+    ((1 << 20) + 4096 * 3 + 1040, 4096, 65536, 0),   # ragged: partial last block, partial last page
+    (5 << 20, 65536, 2 << 20, 0),                # real VMM pages, partial last page
+    (7 * 65536 + 512, 65536, 2 << 20, 0),        # real VMM, single page, ragged
+    (6 << 20, 1 << 20, 2 << 20, 2),              # PLAIN_ALLOC with 2 MiB pages (emulated)
+    (4 << 20, 2 << 20, 2 << 20, 0),              # block == page
+    (100 * 256, 256, 1024, 0),                   # tiny blocks (LDG engine only)
+]
+
+
+@pytest.mark.parametrize("engine", [1, 2])
+@pytest.mark.parametrize("payload,block,page,flags", POOLS)
+def test_shuffle_unshuffle_bit_exact(payload, block, page, flags, engine):
+    key = 0x1234
+    g = O.pool_geometry(payload, block, page)
+    t = O.pool_tables(key, g)
+    L = np.random.default_rng(payload).integers(0, 256, payload, dtype=np.uint8)
+    C.cloak_set_copy_engine(engine)
+    try:
+        with Pool(payload, block, page, key, flags) as p:
+            assert (p.info["nb"], p.info["nslots"], p.info["npages"]) == (g.nb, g.nslots, g.npages)
+            bp, bi, pp, pi = p.tables()
+            assert np.array_equal(bp, t.blockperm) and np.array_equal(bi, t.blockinv)
+            assert np.array_equal(pp, t.pageperm) and np.array_equal(pi, t.pageinv)
+            vmm = p.info["is_vmm"]
+            assert vmm == (page % (2 << 20) == 0 and not (flags & 2))
+            assert np.array_equal(p.table_T(), t.T_vmm if vmm else t.T_emulated)
+            dL = to_dev_bytes(L)
+            padded = (payload + 15) // 16 * 16
+            if padded != payload:
+                dL = torch.cat([dL, dev_bytes(padded - payload)])
+            C.cloak_shuffle(p.h, dL, 0, padded)
+            V = O.shuffle_va(L, g, t.blockinv)
+            D = O.dump_view(V, g, t.pageinv)
+            assert np.array_equal(p.raw(), V if vmm else D)       # zero pad slots are compared too (G4)
+            assert np.array_equal(p.dump(), D)                    # physical-order view (alias mapping for VMM)
+            out = dev_bytes(padded)
+            C.cloak_unshuffle(p.h, out, 0, padded)
+            assert np.array_equal(out.cpu().numpy()[:payload], L)
+            # a sub-range: blocks [1, 3) plus a 48-byte tail of the next
+            if g.nb >= 4:
+                sub = dev_bytes(2 * block + 48)
+                C.cloak_unshuffle(p.h, sub, block, 2 * block + 48)
+                assert np.array_equal(sub.cpu().numpy(), L[block:3 * block + 48])
+    finally:
+        C.cloak_set_copy_engine(0)
+
+
+def test_shuffle_by_tensor_ranges_and_zero_padding():
+    """Tensors placed by cloak_arena_plan, each shuffled on its own; padding after a short tensor is zero."""
+    block, page, key = 4096, 65536, 0x1234
+    sizes = [5000 * 16, 4096 * 3, 16, 70000 * 16 // 16 * 16]
+    offs, total = C.cloak_arena_plan(key, sizes, block)
+    o_offs, o_total, _ = O.arena_plan(key, sizes, block)
+    assert offs == o_offs and total == o_total
+    g = O.pool_geometry(total, block, page)
+    t = O.pool_tables(key, g)
+    rng = np.random.default_rng(0)
+    datas = [rng.integers(1, 256, s, dtype=np.uint8) for s in sizes]
+    ref = np.zeros(g.nslots * block, np.uint8)
+    with Pool(total, block, page, key) as p:
+        for d, o in zip(datas, offs):
+            C.cloak_shuffle(p.h, to_dev_bytes(d), o, d.size)
+            O.shuffle_into(ref, t.T_emulated, d, o, block)
+        assert np.array_equal(p.raw(), ref)
+
+
+def test_identity_pool_is_the_native_layout():
+    payload, block, page = 3 << 20, 65536, 2 << 20
+    L = np.random.default_rng(3).integers(0, 256, payload, dtype=np.uint8)
+    for flags in (C.CLOAK_POOL_IDENTITY, C.CLOAK_POOL_IDENTITY | C.CLOAK_POOL_PLAIN_ALLOC):
+        with Pool(payload, block, page, 0x1234, flags) as p:
+            C.cloak_shuffle(p.h, to_dev_bytes(L), 0, payload)
+            raw = p.raw()
+            assert np.array_equal(raw[:payload], L) and not raw[payload:].any()
+            assert np.array_equal(p.table_T(), np.arange(p.info["nb"], dtype=np.uint32))
+
+
+@pytest.mark.parametrize("engine", [1, 2])
+@pytest.mark.parametrize("payload,block,page", [(3 << 20, 4096, 65536), (5 << 20, 65536, 2 << 20),
+                                                ((2 << 20) + 4096 * 5 + 160, 4096, 2 << 20)])
+def test_relayout_bit_exact(payload, block, page, engine):
+    ka, kb = 0x1234, 0x5678
+    g = O.pool_geometry(payload, block, page)
+    ta, tb = O.pool_tables(ka, g), O.pool_tables(kb, g)
+    L = np.random.default_rng(11).integers(0, 256, payload, dtype=np.uint8)
+    padded = (payload + 15) // 16 * 16
+    C.cloak_set_copy_engine(engine)
+    try:
+        with Pool(payload, block, page, ka) as pa, Pool(payload, block, page, kb) as pb:
+            vmm = pa.info["is_vmm"]
+            TA, TB = (ta.T_vmm, tb.T_vmm) if vmm else (ta.T_emulated, tb.T_emulated)
+            dL = torch.cat([to_dev_bytes(L), dev_bytes(padded - payload)]) if padded != payload else to_dev_bytes(L)
+            C.cloak_shuffle(pa.h, dL, 0, padded)
+            ref_a = pa.raw()
+            C.cloak_relayout(pa.h, pb.h)
+            assert np.array_equal(pb.raw(), O.relayout(ref_a, TA, TB, g))       # = shuffle_B(unshuffle_A)
+            with Pool(payload, block, page, ka) as pa2:
+                C.cloak_relayout(pb.h, pa2.h)                                   # A -> B -> A restores pool A
+                assert np.array_equal(pa2.raw(), ref_a)
+    finally:
+        C.cloak_set_copy_engine(0)
+
+
+def test_host_buffer_round_trip():
+    payload, block, page, key = (5 << 20) + 4096 + 32, 4096, 2 << 20, 0x1234
+    g = O.pool_geometry(payload, block, page)
+    t = O.pool_tables(key, g)
+    L = np.random.default_rng(21).integers(0, 256, payload, dtype=np.uint8)
+    hL = torch.from_numpy(L.copy()).pin_memory()
+    out = torch.zeros(payload, dtype=torch.uint8).pin_memory()
+    with Pool(payload, block, page, key) as p:
+        C.cloak_shuffle_host(p.h, hL, 0, payload)
+        assert np.array_equal(p.raw(), O.shuffle_va(L, g, t.blockinv))
+        C.cloak_unshuffle_host(p.h, out, 0, payload)
+        assert np.array_equal(out.numpy(), L)
+
+
+# ------------------------------------------------------------------ S5 neuron / head permutation
+def _dev(a, dtype):
+    return torch.from_numpy(a.copy()).cuda() if dtype == "f32" else bf16_dev_from_bits(a)
+
+
+def _host(t, dtype):
+    return t.cpu().numpy() if dtype == "f32" else bits_from_bf16_dev(t)
+
+
+PERM_SHAPES = [
+    # hidden, inter, n_q, n_kv, d, dtype, layer
+    (256, 1024, 4, 4, 64, "f32", 0),        # cfg0's MLP block (+ an MHA head set, G = 1)
+    (256, 1000, 8, 2, 32, "bf16", 3),       # ragged inter, GQA
+    (4096, 14336, 32, 8, 128, "bf16", 0),   # cfg1 at full size
+    (640, 1536, 40, 8, 16, "bf16", 63),     # cfg3's head structure (40 q / 8 kv), non-power-of-two rows
+]
+
+
+@pytest.mark.parametrize("hidden,inter,n_q,n_kv,d,dtype,layer", PERM_SHAPES)
+def test_permute_mlp_heads_bit_exact(hidden, inter, n_q, n_kv, d, dtype, layer):
+    key, seed = 0x1234, 5
+    shapes = dict(gate=(inter, hidden), up=(inter, hidden), down=(hidden, inter), q=(n_q * d, hidden),
+                  k=(n_kv * d, hidden), v=(n_kv * d, hidden), o=(hidden, n_q * d))
+    W = {nm: gen.synth(seed, i, shp, dtype) for i, (nm, shp) in enumerate(shapes.items())}
+    dW = {nm: _dev(a, dtype) for nm, a in W.items()}
+    dO = {nm: torch.zeros_like(t) for nm, t in dW.items()}
+    sh = C.cloak_block_shape(hidden, inter, n_q, n_kv, d, C.CLOAK_F32 if dtype == "f32" else C.CLOAK_BF16, layer)
+    C.cloak_permute_mlp_heads(key, sh, **dW, **{k + "_o": v for k, v in dO.items()})
+    pi = O.mlp_perm(key, layer, inter)
+    kappa, eta = O.head_maps(key, layer, n_q, n_kv)
+    g2, u2, d2 = O.permute_mlp(W["gate"], W["up"], W["down"], pi)
+    q2, k2, v2, o2 = O.permute_heads(W["q"], W["k"], W["v"], W["o"], kappa, eta, d)
+    for nm, ref in dict(gate=g2, up=u2, down=d2, q=q2, k=k2, v=v2, o=o2).items():
+        assert np.array_equal(_host(dO[nm], dtype), ref), nm
+    # subsets: MLP only / heads only leave the other outputs untouched
+    z = {nm: torch.zeros_like(t) for nm, t in dW.items()}
+    C.cloak_permute_mlp_heads(key, sh, gate=dW["gate"], gate_o=z["gate"], o=dW["o"], o_o=z["o"])
+    assert np.array_equal(_host(z["gate"], dtype), g2) and np.array_equal(_host(z["o"], dtype), o2)
+    assert not z["down"].any() and not z["q"].any()
+
+
+def test_tile128_bit_exact():
+    for dtype, (N, K) in [("bf16", (256, 384)), ("f32", (128, 256)), ("bf16", (1024, 5120))]:
+        W = gen.synth(9, 0, (N, K), dtype)
+        src = _dev(W, dtype)
+        dst = torch.zeros_like(src).reshape(-1)
+        C.cloak_to_tile128(src, dst, N, K, C.CLOAK_F32 if dtype == "f32" else C.CLOAK_BF16)
+        assert np.array_equal(_host(dst, dtype), O.to_tile128(W))
+
+
+# ------------------------------------------------------------------ S6 cloaked GEMV
+def _load_pool(p, tensors, offs, dtype):
+    for (nm, a), o in zip(tensors, offs):
+        d = _dev(a, dtype)
+        C.cloak_shuffle(p.h, d, o, d.numel() * d.element_size())
+
+
+GEMV_CASES = [
+    # dtype, block, page, shapes [(N, K)], batches
+    ("f32", 4096, 65536, [(1024, 256), (1024, 256), (256, 1024)], [1, 3]),                 # cfg0
+    ("bf16", 4096, 65536, [(64, 256), (256, 128), (48, 1024)], [1, 4, 8, 9, 16]),          # several tiles, ragged N/16
+    ("bf16", 65536, 2 << 20, [(1024, 4096), (4096, 14336)], [1, 4, 16]),                   # cfg1's k and down shapes
+    ("bf16", 65536, 2 << 20, [(5120, 5120), (1024, 5120)], [1, 16]),                       # cfg3's non-power-of-two rows
+]
+
+
+@pytest.mark.parametrize("dtype,block,page,shapes,batches", GEMV_CASES)
+def test_gemv_vs_oracle_and_identity_bit_identical(dtype, block, page, shapes, batches):
+    key, seed = 0x1234, 1
+    e = 4 if dtype == "f32" else 2
+    dt = C.CLOAK_F32 if dtype == "f32" else C.CLOAK_BF16
+    tensors = [(f"t{i}", gen.synth(seed, i, shp, dtype)) for i, shp in enumerate(shapes)]
+    sizes = [a.size * e for _, a in tensors]
+    offs, total = C.cloak_arena_plan(key, sizes, block)
+    with Pool(total, block, page, key) as pc, Pool(total, block, page, key, C.CLOAK_POOL_IDENTITY) as pi:
+        _load_pool(pc, tensors, offs, dtype)
+        _load_pool(pi, tensors, offs, dtype)
+        for (nm, Wm), off, (N, K) in zip(tensors, offs, shapes):
+            for batch in batches:
+                X = gen.synth(seed + 100, batch, (batch, K), dtype, kind=gen.KIND_NORMAL)
+                dX = _dev(X, dtype)
+                yc, yi = torch.zeros(batch, N, dtype=dX.dtype, device="cuda"), torch.zeros(batch, N, dtype=dX.dtype, device="cuda")
+                w = C.cloak_tensor(off, N, K, dt, C.CLOAK_ROWMAJOR)
+                C.cloak_gemv(pc.h, w, dX, yc, batch)
+                C.cloak_gemv(pi.h, w, dX, yi, batch)
+                assert torch.equal(yc, yi)                                   # exact pin: same kernel, only addresses differ
+                ref = O.linear_f64(X, Wm)
+                got = yc.float().cpu().numpy()
+                assert O.err_normwise(got, ref) <= TOL[dtype], (nm, batch, O.err_normwise(got, ref))
+
+
+def test_gemv_closed_forms_through_the_table():
+    """W = I gives Y = X; W = ones gives row sums -- read through a shuffled pool."""
+    block, page, key, n = 4096, 65536, 0x1234, 256
+    eye = np.eye(n, dtype=np.float32)
+    ones = np.ones((n, n), dtype=np.float32)
+    offs, total = C.cloak_arena_plan(key, [n * n * 4, n * n * 4], block)
+    with Pool(total, block, page, key) as p:
+        _load_pool(p, [("eye", eye), ("ones", ones)], offs, "f32")
+        x = torch.randn(2, n, device="cuda")
+        y = torch.zeros(2, n, device="cuda")
+        C.cloak_gemv(p.h, C.cloak_tensor(offs[0], n, n, C.CLOAK_F32, C.CLOAK_ROWMAJOR), x, y, 2)
+        assert torch.equal(x, y)
+        C.cloak_gemv(p.h, C.cloak_tensor(offs[1], n, n, C.CLOAK_F32, C.CLOAK_ROWMAJOR), x, y, 2)
+        assert torch.allclose(y, x.double().sum(dim=1, keepdim=True).float().expand(2, n), rtol=1e-5, atol=1e-5)
+    # bf16: W = I exactly representable; x in bf16 comes back unchanged
+    eyeb = O.f32_to_bf16_bits(eye)
+    offs, total = C.cloak_arena_plan(key, [n * n * 2], block)
+    with Pool(total, block, page, key) as p:
+        _load_pool(p, [("eye", eyeb)], offs, "bf16")
+        x = torch.randn(5, n, device="cuda").bfloat16()
+        y = torch.zeros(5, n, device="cuda", dtype=torch.bfloat16)
+        C.cloak_gemv(p.h, C.cloak_tensor(offs[0], n, n, C.CLOAK_BF16, C.CLOAK_ROWMAJOR), x, y, 5)
+        assert torch.equal(x, y)
+
+
+def test_gemv_host_entry_point():
+    block, page, key, N, K = 65536, 2 << 20, 0x1234, 512, 1024
+    Wm = gen.synth(1, 0, (N, K), "bf16")
+    X = gen.synth(2, 0, (4, K), "bf16", kind=gen.KIND_NORMAL)
+    with Pool(N * K * 2, block, page, key) as p:
+        _load_pool(p, [("w", Wm)], [0], "bf16")
+        hx = torch.from_numpy(X.view(np.int16).copy()).pin_memory()
+        hy = torch.zeros(4, N, dtype=torch.int16).pin_memory()
+        C.cloak_gemv_host(p.h, C.cloak_tensor(0, N, K, C.CLOAK_BF16, C.CLOAK_ROWMAJOR), hx, hy, 4)
+        got = O.bf16_bits_to_f32(hy.numpy().view(np.uint16))
+        assert O.err_normwise(got, O.linear_f64(X, Wm)) <= TOL["bf16"]
+
+
+def test_cfg0_mlp_end_to_end_permuted_and_cloaked():
+    """cfg0: permute -> shuffle -> three GEMVs + silu*up; equals the unpermuted MLP of the oracle (fp32 tol)."""
+    c = gen.CONFIGS[0]
+    H, I, key, block, page = c["hidden"], c["inter"], c["key"], c["block"], c["page"]
+    gate, up, down = (gen.synth(c["seed"], i, s, "f32") for i, s in enumerate([(I, H), (I, H), (H, I)]))
+    x = gen.synth(c["seed"], 10, (1, H), "f32", kind=gen.KIND_NORMAL)
+    dg, du, dd = (torch.from_numpy(a.copy()).cuda() for a in (gate, up, down))
+    pg, pu, pd = torch.empty_like(dg), torch.empty_like(du), torch.empty_like(dd)
+    sh = C.cloak_block_shape(H, I, 0, 0, 0, C.CLOAK_F32, 0)
+    C.cloak_permute_mlp_heads(key, sh, gate=dg, up=du, down=dd, gate_o=pg, up_o=pu, down_o=pd)
+    offs, total = C.cloak_arena_plan(key, [4 * H * I] * 3, block)
+    assert total == 3 << 20
+    with Pool(total, block, page, key) as p:
+        assert p.info["npages"] == 48
+        for t, o in zip((pg, pu, pd), offs):
+            C.cloak_shuffle(p.h, t, o, t.numel() * 4)
+        dx = torch.from_numpy(x.copy()).cuda()
+        yg, yu = torch.empty(1, I, device="cuda"), torch.empty(1, I, device="cuda")
+        C.cloak_gemv(p.h, C.cloak_tensor(offs[0], I, H, C.CLOAK_F32, C.CLOAK_ROWMAJOR), dx, yg, 1)
+        C.cloak_gemv(p.h, C.cloak_tensor(offs[1], I, H, C.CLOAK_F32, C.CLOAK_ROWMAJOR), dx, yu, 1)
+        # the permuted gate output is the unpermuted one gathered by pi (the paper-level invariant, O9)
+        pi = O.mlp_perm(key, 0, I).astype(np.int64)
+        ref_g = O.linear_f64(x, gate)
+        assert O.err_normwise(yg.cpu().numpy(), ref_g[:, pi]) <= TOL["f32"]
+        act = torch.empty(1, I, device="cuda")
+        C.cloak_silu_mul(yg, yu, act, I, C.CLOAK_F32)
+        y = torch.empty(1, H, device="cuda")
+        C.cloak_gemv(p.h, C.cloak_tensor(offs[2], H, I, C.CLOAK_F32, C.CLOAK_ROWMAJOR), act, y, 1)
+        ref = O.mlp_f64(x, gate, up, down)                         # the UNpermuted MLP
+        assert O.err_normwise(y.cpu().numpy(), ref) <= 2e-5
+
+
+# ------------------------------------------------------------------ errors
+def test_error_codes_on_device():
+    with Pool(1 << 20, 4096, 65536, 1) as p:
+        buf = dev_bytes(8192)
+        for fn, args, st in [
+            (C.cloak_shuffle, (p.h, buf, 100, 4096), C.CLOAK_ERR_ALIGN),
+            (C.cloak_shuffle, (p.h, buf, 0, 100), C.CLOAK_ERR_ALIGN),
+            (C.cloak_shuffle, (p.h, buf, 1 << 20, 4096), C.CLOAK_ERR_INVALID),
+            (C.cloak_unshuffle, (p.h, None, 0, 4096), C.CLOAK_ERR_INVALID),
+            (C.cloak_relayout, (p.h, p.h), C.CLOAK_ERR_INVALID),
+        ]:
+            with pytest.raises(C.CloakError) as ei:
+                fn(*args)
+            assert ei.value.status == st
+        x = torch.zeros(1, 256, device="cuda")
+        with pytest.raises(C.CloakError) as ei:
+            C.cloak_gemv(p.h, C.cloak_tensor(0, 1024, 256, C.CLOAK_F32, C.CLOAK_ROWMAJOR), x, x, 17)
+        assert ei.value.status == C.CLOAK_ERR_INVALID
+        with pytest.raises(C.CloakError) as ei:
+            C.cloak_gemv(p.h, C.cloak_tensor(0, 1024, 256, C.CLOAK_F32, C.CLOAK_TILE128), x, x, 1)
+        assert ei.value.status == C.CLOAK_ERR_UNSUPPORTED
+        with pytest.raises(C.CloakError) as ei:
+            C.cloak_gemv(p.h, C.cloak_tensor(0, 1 << 20, 256, C.CLOAK_F32, C.CLOAK_ROWMAJOR), x, x, 1)
+        assert ei.value.status == C.CLOAK_ERR_INVALID
