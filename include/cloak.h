@@ -54,6 +54,9 @@ const char* cloak_last_error(void);
 /* Library version / build info: a static string such as "cloak-b200 0.1 sm_100a". */
 const char* cloak_version(void);
 
+/* Process-wide number of CUDA kernels this library has launched so far (for bench.py's gpu_launches). */
+uint64_t cloak_launch_count(void);
+
 /* ---- S1 keyed permutation (north_star: "indices sorted by Philox(key, index)").
  * For i in [0, n): o = Philox4x32-10(ctr = (i, 0, stream_id lo, stream_id hi), key = (key lo, key hi)),
  * r_i = o[0]:o[1]; perm = indices sorted ascending by (r_i, i); inv[perm[j]] = j.
@@ -172,6 +175,9 @@ cloak_status cloak_gemv(const cloak_pool* pool, const cloak_tensor* w, const voi
                         uint32_t batch, void* stream);
 cloak_status cloak_gemm(const cloak_pool* pool, const cloak_tensor* w, const void* d_x, void* d_y,
                         uint32_t batch, void* stream);
+/* Selects the bf16 GEMV kernel: 0 = automatic (streaming TMA kernel when K % 256 == 0), 1 = always the
+ * one-shot split-K kernel.  For A/B measurement; process-wide. */
+cloak_status cloak_set_gemv_engine(int engine);
 /* Host-buffer variant of cloak_gemv (end-to-end path): copies X up, runs, copies Y back, synchronises. */
 cloak_status cloak_gemv_host(const cloak_pool* pool, const cloak_tensor* w, const void* h_x, void* h_y,
                              uint32_t batch, void* stream);

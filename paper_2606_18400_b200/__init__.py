@@ -1,7 +1,21 @@
 """B200-native CloakLM cloaked-layout hot path: ctypes binding of the C-ABI CUDA library libcloak.so.
 
-See include/cloak.h for the boundary and DESIGN.md for the design.  Importing `binding` requires the
-built library (`python -m paper_2606_18400_b200.build`); there is no CPU fallback.
+See include/cloak.h for the boundary and DESIGN.md for the design.  The binding (`.binding`) is loaded on
+first attribute access so that `paper_2606_18400_b200.build` can run before the library exists; using any
+cloak_* name without the built library raises ImportError -- there is no CPU fallback.
 """
-from .binding import *  # noqa: F401,F403
-from .binding import (SYMBOLS, LIB_PATH, CloakError, cloak_block_shape, cloak_tensor, lib)  # noqa: F401
+import importlib
+
+_binding = None
+
+
+def __getattr__(name):
+    global _binding
+    if name.startswith("__"):
+        raise AttributeError(name)
+    if _binding is None:
+        _binding = importlib.import_module(".binding", __name__)
+    try:
+        return getattr(_binding, name)
+    except AttributeError:
+        raise AttributeError(f"module {__name__!r} has no attribute {name!r}") from None

@@ -22,11 +22,11 @@ STATUS_NAMES = {0: "CLOAK_OK", -1: "CLOAK_ERR_INVALID", -2: "CLOAK_ERR_ALIGN", -
                 -4: "CLOAK_ERR_OOM", -5: "CLOAK_ERR_CUDA"}
 
 # every symbol include/cloak.h declares
-SYMBOLS = ["cloak_last_error", "cloak_version", "cloak_keygen", "cloak_pool_create", "cloak_pool_destroy",
+SYMBOLS = ["cloak_last_error", "cloak_version", "cloak_launch_count", "cloak_keygen", "cloak_pool_create", "cloak_pool_destroy",
            "cloak_pool_info", "cloak_pool_tables", "cloak_pool_dump", "cloak_pool_map_ms", "cloak_shuffle",
            "cloak_unshuffle", "cloak_relayout", "cloak_shuffle_host", "cloak_unshuffle_host",
            "cloak_set_copy_engine", "cloak_arena_plan", "cloak_permute_mlp_heads", "cloak_to_tile128",
-           "cloak_gemv", "cloak_gemm", "cloak_gemv_host", "cloak_silu_mul"]
+           "cloak_gemv", "cloak_gemm", "cloak_set_gemv_engine", "cloak_gemv_host", "cloak_silu_mul"]
 
 
 class CloakError(RuntimeError):
@@ -66,6 +66,7 @@ lib.cloak_relayout.argtypes = [_P, _P, _P]
 lib.cloak_shuffle_host.argtypes = [_P, _P, c_uint64, c_uint64, _P]
 lib.cloak_unshuffle_host.argtypes = [_P, _P, c_uint64, c_uint64, _P]
 lib.cloak_set_copy_engine.argtypes = [c_int]
+lib.cloak_set_gemv_engine.argtypes = [c_int]
 lib.cloak_arena_plan.argtypes = [c_uint64, c_uint32, POINTER(c_uint64), c_uint32, POINTER(c_uint64), POINTER(c_uint64)]
 lib.cloak_permute_mlp_heads.argtypes = [c_uint64, POINTER(cloak_block_shape)] + [_P] * 15
 lib.cloak_to_tile128.argtypes = [_P, _P, c_uint32, c_uint32, c_int, _P]
@@ -73,7 +74,8 @@ lib.cloak_gemv.argtypes = [_P, POINTER(cloak_tensor), _P, _P, c_uint32, _P]
 lib.cloak_gemm.argtypes = [_P, POINTER(cloak_tensor), _P, _P, c_uint32, _P]
 lib.cloak_gemv_host.argtypes = [_P, POINTER(cloak_tensor), _P, _P, c_uint32, _P]
 lib.cloak_silu_mul.argtypes = [_P, _P, _P, c_uint64, c_int, _P]
-for _n in SYMBOLS[2:]:
+lib.cloak_launch_count.restype = c_uint64
+for _n in SYMBOLS[3:]:
     getattr(lib, _n).restype = c_int
 
 
@@ -115,6 +117,10 @@ def cloak_last_error():
 
 def cloak_version():
     return lib.cloak_version().decode()
+
+
+def cloak_launch_count():
+    return int(lib.cloak_launch_count())
 
 
 def cloak_keygen(key, stream_id, n, d_perm, d_inv, stream=None):
@@ -175,6 +181,10 @@ def cloak_unshuffle_host(pool, h_logical, logical_offset, nbytes, stream=None):
 
 def cloak_set_copy_engine(engine):
     _check(lib.cloak_set_copy_engine(engine))
+
+
+def cloak_set_gemv_engine(engine):
+    _check(lib.cloak_set_gemv_engine(engine))
 
 
 def cloak_arena_plan(key, sizes, block_bytes):

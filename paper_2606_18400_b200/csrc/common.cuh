@@ -5,6 +5,7 @@
 #include <cuda_runtime.h>
 #include <stdint.h>
 #include <stdio.h>
+#include <atomic>
 #include <vector>
 #include "cloak.h"
 
@@ -74,9 +75,18 @@ struct DeviceGuard {
 
 int sm_count(int device);
 
+// Process-wide count of kernels this library has launched (cloak_launch_count()).
+extern std::atomic<unsigned long long> g_launches;
+inline void launched(unsigned n = 1) { g_launches.fetch_add(n, std::memory_order_relaxed); }
+
 // keygen on the current device (keygen.cu).  Either output may be null.
 cloak_status keygen_device(uint64_t key, uint64_t stream_id, uint32_t n, uint32_t* d_perm, uint32_t* d_inv,
                            cudaStream_t s);
+constexpr size_t WS_COUNTER_BYTES = 1u << 20;
+cloak_status pool_workspace(const cloak_pool* pool, size_t bytes);
+// gemv_stream.cu: persistent TMA-fed bf16 GEMV (K % 256 == 0).
+cloak_status gemv_stream_bf16(const cloak_pool* pool, const cloak_tensor* w, const void* d_x, void* d_y, uint32_t batch,
+                              cudaStream_t s);
 // Host-side Philox keygen used only by cloak_arena_plan (T is tiny; no device work wanted there).
 void keygen_host(uint64_t key, uint64_t stream_id, uint32_t n, std::vector<uint32_t>& perm);
 
@@ -102,5 +112,7 @@ struct cloak_pool {
              *d_T = nullptr;
     CUtensorMap tmap_tile128;   // GEMM: pool viewed as rows of 128 bf16 (gemm_sm100.cu), built lazily
     bool tmap_ready = false;
+    mutable char* ws = nullptr;     // library-owned scratch (GEMV / GEMM split-K partials + counters), lazily grown
+    mutable size_t ws_bytes = 0;
     uint64_t bytes() const { return (uint64_t)nslots * block; }
 };

@@ -15,6 +15,7 @@
 //         registers or LSU instructions touch the payload.
 #include <new>
 #include "common.cuh"
+#include "async.cuh"
 
 namespace cloak {
 
@@ -82,36 +83,6 @@ __global__ void __launch_bounds__(LDG_THREADS) copy_ldg_kernel(CopyArgs a, uint6
 // ---------------------------------------------------------------- TMA bulk engine
 constexpr int TMA_WARPS = 4;        // independent pipelines per CTA
 constexpr int TMA_STAGES = 4;
-
-__device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
-
-__device__ __forceinline__ void mbar_init(uint32_t bar, uint32_t count) {
-    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" :: "r"(bar), "r"(count));
-}
-__device__ __forceinline__ void mbar_expect_tx(uint32_t bar, uint32_t bytes) {
-    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" :: "r"(bar), "r"(bytes) : "memory");
-}
-__device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
-    asm volatile(
-        "{\n\t.reg .pred p;\n\t"
-        "WAIT_%=:\n\t"
-        "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n\t"
-        "@p bra DONE_%=;\n\t"
-        "bra WAIT_%=;\n\t"
-        "DONE_%=:\n\t}" :: "r"(bar), "r"(parity) : "memory");
-}
-__device__ __forceinline__ void bulk_g2s(uint32_t dst_smem, const void* src, uint32_t bytes, uint32_t bar) {
-    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
-                 :: "r"(dst_smem), "l"(src), "r"(bytes), "r"(bar) : "memory");
-}
-__device__ __forceinline__ void bulk_s2g(void* dst, uint32_t src_smem, uint32_t bytes) {
-    asm volatile("cp.async.bulk.global.shared::cta.bulk_group [%0], [%1], %2;"
-                 :: "l"(dst), "r"(src_smem), "r"(bytes) : "memory");
-}
-__device__ __forceinline__ void bulk_commit() { asm volatile("cp.async.bulk.commit_group;" ::: "memory"); }
-template <int N>
-__device__ __forceinline__ void bulk_wait_read() { asm volatile("cp.async.bulk.wait_group.read %0;" :: "n"(N) : "memory"); }
-__device__ __forceinline__ void bulk_wait_all() { asm volatile("cp.async.bulk.wait_group 0;" ::: "memory"); }
 
 // Unit u (0 <= u < nblocks << (log2b - log2c)) is chunk (u & cmask) of block (u >> (log2b - log2c)).
 __global__ void __launch_bounds__(TMA_WARPS * 32) copy_tma_kernel(CopyArgs a, uint64_t total_units, uint32_t log2c) {
@@ -187,6 +158,7 @@ static cloak_status launch_copy(const cloak_pool* pool, const CopyArgs& a, cudaS
         const uint64_t cap = (uint64_t)sms * (smem <= 100 * 1024 ? 2 : 1);
         if (ctas > cap) ctas = cap;
         copy_tma_kernel<<<(unsigned)ctas, TMA_WARPS * 32, smem, s>>>(a, units, log2c);
+        launched();
     } else {
         const bool wide = a.log2b >= 5 && (((uintptr_t)a.src | (uintptr_t)a.dst) & 31) == 0;
         const uint32_t logv = wide ? 5 : 4;
@@ -197,6 +169,7 @@ static cloak_status launch_copy(const cloak_pool* pool, const CopyArgs& a, cudaS
         if (ctas > cap) ctas = cap;
         if (wide) copy_ldg_kernel<V32, U><<<(unsigned)ctas, LDG_THREADS, 0, s>>>(a, vecs);
         else      copy_ldg_kernel<V16, U><<<(unsigned)ctas, LDG_THREADS, 0, s>>>(a, vecs);
+        launched();
     }
     CLOAK_LAUNCH_CHECK();
     return CLOAK_OK;
@@ -256,6 +229,7 @@ static cloak_status launch_tail(const cloak_pool* pool, char* logical_tail, uint
                                 int to_pool, cudaStream_t s) {
     copy_tail_indirect_kernel<<<1, 256, 0, s>>>(pool->base, pool->d_T, block_index, pool->log2_block, logical_tail,
                                                 tail / 16, to_pool);
+    launched();
     CLOAK_LAUNCH_CHECK();
     return CLOAK_OK;
 }

@@ -8,6 +8,7 @@
 namespace cloak {
 
 static thread_local char g_err[512] = "";
+std::atomic<unsigned long long> g_launches{0};
 
 void set_error(const char* fmt, ...) {
     va_list ap;
@@ -112,6 +113,8 @@ void keygen_host(uint64_t key, uint64_t stream_id, uint32_t n, std::vector<uint3
 }  // namespace cloak
 
 extern "C" const char* cloak_last_error(void) { return cloak::g_err; }
+
+extern "C" uint64_t cloak_launch_count(void) { return cloak::g_launches.load(); }
 
 extern "C" const char* cloak_version(void) { return "cloak-b200 0.1 sm_100a"; }
 

@@ -32,6 +32,7 @@ struct GemvArgs {
     const void* x;
     void* y;
     uint32_t batch;
+    uint32_t zero;      // always 0; see the scheduling fence in gemv_bf16_kernel
 };
 
 __device__ __forceinline__ const char* xlate(const GemvArgs& a, uint64_t off) {
@@ -55,73 +56,95 @@ __device__ __forceinline__ void mma_bf16_16816(float c[4], uint32_t a0, uint32_t
 
 constexpr int GV_WARPS = 4;
 constexpr int GV_ROWS = 16;
-constexpr int GV_KSTEP = 64;      // k elements per warp step: 2 vectors per row per lane
-constexpr int GV_UNROLL = 2;      // k-steps in flight per warp
+constexpr int GV_KSTEP = 64;                          // k elements per warp step: 2 vectors per row per lane
+constexpr int GV_STEPS = 4;                           // k-steps per warp: all issued before the first MMA
+constexpr int GV_KCTA = GV_WARPS * GV_STEPS * GV_KSTEP;   // 1024 k elements per CTA
+constexpr uint32_t GV_MAX_TILES = (uint32_t)(WS_COUNTER_BYTES / 4);          // row tiles per launch the split-K counters cover
 
-template <int NT>   // NT = number of 8-wide batch tiles (1: batch <= 8, 2: batch <= 16)
-__global__ void __launch_bounds__(GV_WARPS * 32) gemv_bf16_kernel(GemvArgs a) {
+// One CTA = 16 rows x 1024 k, one shot: every lane issues its 16 weight loads (8 KiB per warp, 32 KiB per
+// CTA) before the first MMA, so the bytes in flight per SM are occupancy x 32 KiB with no loop-carried
+// latency and a tail of one short CTA lifetime.  K is split over S = ceil(K/1024) CTAs (blockIdx = tile*S+s).
+// S > 1: every CTA stores its fp32 partial, and the last CTA to arrive at the tile's counter sums the S
+// partials in s order (fixed order -> deterministic, bit-identical between cloaked and identity pools).
+// FULL: K is a multiple of 1024, so no k-step needs a bounds check.
+template <int NT, bool FULL>   // NT = number of 8-wide batch tiles (1: batch <= 8, 2: batch <= 16)
+__global__ void __launch_bounds__(GV_WARPS * 32) gemv_bf16_kernel(GemvArgs a, uint32_t S, float* __restrict__ part,
+                                                                  uint32_t* __restrict__ counters) {
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     const int g = lane >> 2, t = lane & 3;
-    const uint32_t n0 = blockIdx.x * GV_ROWS;
-    const uint64_t row_lo = a.w_offset + ((uint64_t)(n0 + g) * a.K + t * 8) * 2;
+    const uint32_t tile = blockIdx.x / S, split = blockIdx.x - tile * S;
+    const uint32_t n0 = tile * GV_ROWS;
+    const uint32_t kbase = split * GV_KCTA + warp * (GV_STEPS * GV_KSTEP);
+    const uint64_t row_lo = a.w_offset + ((uint64_t)(n0 + g) * a.K + kbase + t * 8) * 2;
     const uint64_t row_hi = row_lo + (uint64_t)8 * a.K * 2;
     const uint16_t* X = static_cast<const uint16_t*>(a.x);
     const bool xv0 = (uint32_t)g < a.batch, xv1 = (uint32_t)(g + 8) < a.batch;
-    const uint16_t* x0 = X + (size_t)g * a.K + t * 8;
-    const uint16_t* x1 = X + (size_t)(g + 8) * a.K + t * 8;
+    const uint16_t* x0 = X + (size_t)g * a.K + kbase + t * 8;
+    const uint16_t* x1 = X + (size_t)(g + 8) * a.K + kbase + t * 8;
 
+    // All table lookups first (independent L2 hits), then all 16 weight loads: nothing serialises.
+    const char* pl[GV_STEPS];
+    const char* ph[GV_STEPS];
+#pragma unroll
+    for (int u = 0; u < GV_STEPS; ++u) {
+        const bool in = FULL || kbase + u * GV_KSTEP < a.K;
+        pl[u] = in ? xlate(a, row_lo + (uint64_t)u * GV_KSTEP * 2) : nullptr;   // 128-byte line of row g
+        ph[u] = in ? xlate(a, row_hi + (uint64_t)u * GV_KSTEP * 2) : nullptr;   // 128-byte line of row g+8
+    }
+    uint4 wl[GV_STEPS][2], wh[GV_STEPS][2];
+#pragma unroll
+    for (int u = 0; u < GV_STEPS; ++u) {
+        if (FULL || pl[u]) {
+            wl[u][0] = ld_w(pl[u]);
+            wl[u][1] = ld_w(pl[u] + 64);
+            wh[u][0] = ld_w(ph[u]);
+            wh[u][1] = ld_w(ph[u] + 64);
+        }
+    }
+    // The activations (L2-resident, shared by every CTA) are requested right behind the weights.
+    uint4 xa[GV_STEPS][2], xb[GV_STEPS][2];
+#pragma unroll
+    for (int u = 0; u < GV_STEPS; ++u) {
+        const uint4 z = make_uint4(0, 0, 0, 0);
+        const bool in = FULL || kbase + u * GV_KSTEP < a.K;
+#pragma unroll
+        for (int h = 0; h < 2; ++h) {
+            xa[u][h] = (xv0 && in) ? __ldg(reinterpret_cast<const uint4*>(x0 + u * GV_KSTEP + h * 32)) : z;
+            if (NT == 2) xb[u][h] = (xv1 && in) ? __ldg(reinterpret_cast<const uint4*>(x1 + u * GV_KSTEP + h * 32)) : z;
+        }
+    }
+    // Scheduling fence.  ptxas otherwise sinks the loads between the MMAs to save registers, which
+    // serialises the memory latency.  The accumulators are seeded with (xor of one word of every weight
+    // vector) & a.zero -- a.zero is 0 at run time but opaque to the compiler -- so the first MMA of each
+    // chain depends on all 16 loads and every request is in flight before any of them is consumed.
+    uint32_t dep = 0;
+#pragma unroll
+    for (int u = 0; u < GV_STEPS; ++u)
+        if (FULL || pl[u]) dep ^= wl[u][0].x ^ wl[u][1].x ^ wh[u][0].x ^ wh[u][1].x;
+    const float seed = __uint_as_float(dep & a.zero);
     float acc[NT][4];
 #pragma unroll
     for (int i = 0; i < NT; ++i)
 #pragma unroll
-        for (int j = 0; j < 4; ++j) acc[i][j] = 0.f;
-
-    const uint32_t ksteps = a.K / GV_KSTEP;
-    for (uint32_t ks = warp * GV_UNROLL; ks < ksteps; ks += GV_WARPS * GV_UNROLL) {
-        uint4 wl[GV_UNROLL][2], wh[GV_UNROLL][2], xa[GV_UNROLL][2], xb[GV_UNROLL][2];
+        for (int j = 0; j < 4; ++j) acc[i][j] = seed;
 #pragma unroll
-        for (int u = 0; u < GV_UNROLL; ++u) {
-            const uint32_t k0 = (ks + u) * GV_KSTEP;
-            if (ks + u < ksteps) {
-                const char* pl = xlate(a, row_lo + (uint64_t)k0 * 2);   // 128-byte line of row g
-                const char* ph = xlate(a, row_hi + (uint64_t)k0 * 2);   // 128-byte line of row g+8
-                wl[u][0] = ld_w(pl);
-                wl[u][1] = ld_w(pl + 64);
-                wh[u][0] = ld_w(ph);
-                wh[u][1] = ld_w(ph + 64);
-            }
-        }
+    for (int u = 0; u < GV_STEPS; ++u) {
+        if (FULL || kbase + u * GV_KSTEP < a.K) {
 #pragma unroll
-        for (int u = 0; u < GV_UNROLL; ++u) {
-            const uint32_t k0 = (ks + u) * GV_KSTEP;
-            const uint4 z = make_uint4(0, 0, 0, 0);
-            if (ks + u < ksteps) {
-                xa[u][0] = xv0 ? __ldg(reinterpret_cast<const uint4*>(x0 + k0)) : z;
-                xa[u][1] = xv0 ? __ldg(reinterpret_cast<const uint4*>(x0 + k0 + 32)) : z;
+            for (int h = 0; h < 2; ++h) {
+                mma_bf16_16816(acc[0], wl[u][h].x, wh[u][h].x, wl[u][h].y, wh[u][h].y, xa[u][h].x, xa[u][h].y);
+                mma_bf16_16816(acc[0], wl[u][h].z, wh[u][h].z, wl[u][h].w, wh[u][h].w, xa[u][h].z, xa[u][h].w);
                 if (NT == 2) {
-                    xb[u][0] = xv1 ? __ldg(reinterpret_cast<const uint4*>(x1 + k0)) : z;
-                    xb[u][1] = xv1 ? __ldg(reinterpret_cast<const uint4*>(x1 + k0 + 32)) : z;
-                }
-            }
-        }
-#pragma unroll
-        for (int u = 0; u < GV_UNROLL; ++u) {
-            if (ks + u < ksteps) {
-#pragma unroll
-                for (int h = 0; h < 2; ++h) {
-                    mma_bf16_16816(acc[0], wl[u][h].x, wh[u][h].x, wl[u][h].y, wh[u][h].y, xa[u][h].x, xa[u][h].y);
-                    mma_bf16_16816(acc[0], wl[u][h].z, wh[u][h].z, wl[u][h].w, wh[u][h].w, xa[u][h].z, xa[u][h].w);
-                    if (NT == 2) {
-                        mma_bf16_16816(acc[1], wl[u][h].x, wh[u][h].x, wl[u][h].y, wh[u][h].y, xb[u][h].x, xb[u][h].y);
-                        mma_bf16_16816(acc[1], wl[u][h].z, wh[u][h].z, wl[u][h].w, wh[u][h].w, xb[u][h].z, xb[u][h].w);
-                    }
+                    mma_bf16_16816(acc[1], wl[u][h].x, wh[u][h].x, wl[u][h].y, wh[u][h].y, xb[u][h].x, xb[u][h].y);
+                    mma_bf16_16816(acc[1], wl[u][h].z, wh[u][h].z, wl[u][h].w, wh[u][h].w, xb[u][h].z, xb[u][h].w);
                 }
             }
         }
     }
 
-    // Split-K reduction across the 4 warps in fixed order, then store Y[m, n0 + row] as bf16.
+    // In-CTA split-K reduction across the 4 warps in fixed order.
     __shared__ float red[GV_WARPS][NT * 8][GV_ROWS + 1];      // [warp][batch m][row]
+    __shared__ uint32_t is_last;
 #pragma unroll
     for (int i = 0; i < NT; ++i) {
         red[warp][i * 8 + 2 * t][g] = acc[i][0];
@@ -131,11 +154,39 @@ __global__ void __launch_bounds__(GV_WARPS * 32) gemv_bf16_kernel(GemvArgs a) {
     }
     __syncthreads();
     __nv_bfloat16* Y = static_cast<__nv_bfloat16*>(a.y);
-    for (uint32_t i = threadIdx.x; i < a.batch * GV_ROWS; i += blockDim.x) {
+    const uint32_t nout = a.batch * GV_ROWS;
+    if (S == 1) {
+        for (uint32_t i = threadIdx.x; i < nout; i += blockDim.x) {
+            const uint32_t m = i / GV_ROWS, r = i % GV_ROWS;
+            float s = red[0][m][r];
+#pragma unroll
+            for (int w = 1; w < GV_WARPS; ++w) s += red[w][m][r];
+            Y[(size_t)m * a.N + n0 + r] = __float2bfloat16_rn(s);
+        }
+        return;
+    }
+    // Cross-CTA split-K: partial[split][m][n], then the last arriver reduces in split order.
+    for (uint32_t i = threadIdx.x; i < nout; i += blockDim.x) {
         const uint32_t m = i / GV_ROWS, r = i % GV_ROWS;
         float s = red[0][m][r];
 #pragma unroll
         for (int w = 1; w < GV_WARPS; ++w) s += red[w][m][r];
+        __stcg(part + ((size_t)split * a.batch + m) * a.N + n0 + r, s);
+    }
+    __threadfence();
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        const uint32_t old = atomicAdd(counters + tile, 1u);
+        is_last = (old == S - 1);
+        if (old == S - 1) counters[tile] = 0;          // self-reset for the next launch
+    }
+    __syncthreads();
+    if (!is_last) return;
+    __threadfence();
+    for (uint32_t i = threadIdx.x; i < nout; i += blockDim.x) {
+        const uint32_t m = i / GV_ROWS, r = i % GV_ROWS;
+        float s = 0.f;
+        for (uint32_t q = 0; q < S; ++q) s += __ldcg(part + ((size_t)q * a.batch + m) * a.N + n0 + r);
         Y[(size_t)m * a.N + n0 + r] = __float2bfloat16_rn(s);
     }
 }
@@ -185,6 +236,26 @@ cloak_status check_linear(const cloak_pool* pool, const cloak_tensor* w, const v
     return CLOAK_OK;
 }
 
+// Library-owned scratch of a pool: WS_COUNTER_BYTES of self-resetting split-K counters (zeroed on
+// (re)allocation) followed by fp32 partials.  Grown on demand.  Calls that use it on one pool must be
+// stream-ordered with respect to each other.
+cloak_status pool_workspace(const cloak_pool* pool, size_t bytes) {
+    if (pool->ws_bytes >= bytes) return CLOAK_OK;
+    if (pool->ws) {
+        CLOAK_CUDA(cudaDeviceSynchronize());
+        cudaFree(pool->ws);
+        pool->ws = nullptr;
+        pool->ws_bytes = 0;
+    }
+    size_t want = bytes < (8u << 20) ? (8u << 20) : bytes;
+    CLOAK_CUDA(cudaMalloc((void**)&pool->ws, want));
+    CLOAK_CUDA(cudaMemset(pool->ws, 0, WS_COUNTER_BYTES));
+    pool->ws_bytes = want;
+    return CLOAK_OK;
+}
+
+static bool g_force_oneshot = false;     // A/B switch (cloak_set_gemv_engine)
+
 static cloak_status gemv_device(const cloak_pool* pool, const cloak_tensor* w, const void* d_x, void* d_y, uint32_t batch,
                                 cudaStream_t s) {
     GemvArgs a;
@@ -197,13 +268,37 @@ static cloak_status gemv_device(const cloak_pool* pool, const cloak_tensor* w, c
     a.x = d_x;
     a.y = d_y;
     a.batch = batch;
+    a.zero = 0;
+    if (w->dt == CLOAK_BF16 && w->K % 256 == 0 && pool->block >= 512 && !g_force_oneshot)
+        return gemv_stream_bf16(pool, w, d_x, d_y, batch, s);
     if (w->dt == CLOAK_BF16) {
-        if (batch <= 8) gemv_bf16_kernel<1><<<w->N / GV_ROWS, GV_WARPS * 32, 0, s>>>(a);
-        else            gemv_bf16_kernel<2><<<w->N / GV_ROWS, GV_WARPS * 32, 0, s>>>(a);
+        const uint32_t tiles = w->N / GV_ROWS;
+        const uint32_t S = (w->K + GV_KCTA - 1) / GV_KCTA;
+        float* part = nullptr;
+        uint32_t* counters = nullptr;
+        if (S > 1) {
+            if (tiles > GV_MAX_TILES) return fail(CLOAK_ERR_UNSUPPORTED, "gemv: N too large for the split-K counters");
+            const size_t need = WS_COUNTER_BYTES + (size_t)S * batch * w->N * 4;
+            cloak_status st = pool_workspace(pool, need);
+            if (st != CLOAK_OK) return st;
+            counters = reinterpret_cast<uint32_t*>(pool->ws);
+            part = reinterpret_cast<float*>(pool->ws + WS_COUNTER_BYTES);
+        }
+        const bool full = w->K % GV_KCTA == 0;
+        const dim3 grid(tiles * S), blk(GV_WARPS * 32);
+        if (batch <= 8) {
+            if (full) gemv_bf16_kernel<1, true><<<grid, blk, 0, s>>>(a, S, part, counters);
+            else      gemv_bf16_kernel<1, false><<<grid, blk, 0, s>>>(a, S, part, counters);
+        } else {
+            if (full) gemv_bf16_kernel<2, true><<<grid, blk, 0, s>>>(a, S, part, counters);
+            else      gemv_bf16_kernel<2, false><<<grid, blk, 0, s>>>(a, S, part, counters);
+        }
+        launched();
     } else {
         const unsigned ctas = (w->N + 7) / 8;
         if (batch <= 4) gemv_f32_kernel<4><<<ctas, 256, 0, s>>>(a);
         else            gemv_f32_kernel<16><<<ctas, 256, 0, s>>>(a);
+        launched();
     }
     CLOAK_LAUNCH_CHECK();
     return CLOAK_OK;
@@ -227,6 +322,12 @@ static cloak_status gemv_check(const cloak_pool* pool, const cloak_tensor* w, co
 }  // namespace cloak
 
 using namespace cloak;
+
+extern "C" cloak_status cloak_set_gemv_engine(int engine) {
+    if (engine < 0 || engine > 2) return fail(CLOAK_ERR_INVALID, "set_gemv_engine: engine must be 0, 1 or 2");
+    g_force_oneshot = engine == 1;
+    return CLOAK_OK;
+}
 
 extern "C" cloak_status cloak_gemv(const cloak_pool* pool, const cloak_tensor* w, const void* d_x, void* d_y,
                                    uint32_t batch, void* stream) {

@@ -136,15 +136,16 @@ __global__ void __launch_bounds__(RADIX_THREADS) radix_scatter_kernel(
         const uint32_t d = (uint32_t)(k[j] >> shift) & 255u;
         const uint32_t active = __ballot_sync(0xffffffffu, valid);
         rank[j] = 0;
+        // Every lane reads its digit's running count, then the lowest lane of each digit group bumps it:
+        // reads and writes are separated by warp barriers, so there is no divergent shuffle.
+        uint32_t peers = 0, old = 0;
         if (valid) {
-            const uint32_t peers = __match_any_sync(active, d);
-            const int leader = __ffs(peers) - 1;
-            uint32_t old = 0;
-            if (lane == leader) {
-                old = cnt[warp][d];
-                cnt[warp][d] = old + __popc(peers);
-            }
-            old = __shfl_sync(peers, old, leader);
+            peers = __match_any_sync(active, d);
+            old = cnt[warp][d];
+        }
+        __syncwarp();
+        if (valid) {
+            if ((peers & lt) == 0) cnt[warp][d] = old + __popc(peers);
             rank[j] = old + __popc(peers & lt);
         }
         __syncwarp();
@@ -184,6 +185,7 @@ cloak_status keygen_device(uint64_t key, uint64_t stream_id, uint32_t n, uint32_
     const uint32_t k0 = (uint32_t)key, k1 = (uint32_t)(key >> 32);
     if (n <= SMALL_N) {
         keygen_small_kernel<<<(n + 255) / 256, 256, 0, s>>>(n, s_lo, s_hi, k0, k1, d_perm, d_inv);
+        launched();
         CLOAK_LAUNCH_CHECK();
         return CLOAK_OK;
     }
@@ -191,27 +193,45 @@ cloak_status keygen_device(uint64_t key, uint64_t stream_id, uint32_t n, uint32_
     const size_t keys_b = (size_t)n * 8, idx_b = (size_t)n * 4, hist_b = (size_t)256 * ntiles * 4;
     const size_t total = 2 * keys_b + 2 * idx_b + hist_b;
     char* ws = nullptr;
+    {   // keep freed workspace cached in the stream-ordered pool instead of returning it to the OS at every sync
+        static bool tuned = false;
+        if (!tuned) {
+            int dev = 0;
+            cudaMemPool_t mp;
+            if (cudaGetDevice(&dev) == cudaSuccess && cudaDeviceGetDefaultMemPool(&mp, dev) == cudaSuccess) {
+                uint64_t keep = ~0ull;
+                cudaMemPoolSetAttribute(mp, cudaMemPoolAttrReleaseThreshold, &keep);
+            }
+            cudaGetLastError();
+            tuned = true;
+        }
+    }
     CLOAK_CUDA(cudaMallocAsync((void**)&ws, total, s));
     uint64_t* keys[2] = {(uint64_t*)ws, (uint64_t*)(ws + keys_b)};
     uint32_t* idx[2] = {(uint32_t*)(ws + 2 * keys_b), (uint32_t*)(ws + 2 * keys_b + idx_b)};
     uint32_t* hist = (uint32_t*)(ws + 2 * keys_b + 2 * idx_b);
     philox_keys_kernel<<<(n + 255) / 256, 256, 0, s>>>(n, s_lo, s_hi, k0, k1, keys[0], idx[0]);
+    launched();
     CLOAK_LAUNCH_CHECK();
     int cur = 0;
     for (int pass = 0; pass < 8; ++pass) {
         const int shift = pass * 8;
         radix_hist_kernel<<<ntiles, RADIX_THREADS, 0, s>>>(keys[cur], n, shift, hist, ntiles);
+        launched();
         scan_exclusive_kernel<<<1, 1024, 0, s>>>(hist, 256 * ntiles);
+        launched();
         const bool last = pass == 7;
         uint32_t* idx_dst = (last && d_perm) ? d_perm : idx[cur ^ 1];
         radix_scatter_kernel<<<ntiles, RADIX_THREADS, 0, s>>>(keys[cur], idx[cur], last ? nullptr : keys[cur ^ 1],
                                                               idx_dst, n, shift, hist, ntiles);
+        launched();
         CLOAK_LAUNCH_CHECK();
         cur ^= 1;
     }
     if (d_inv) {
         const uint32_t* perm = d_perm ? d_perm : idx[cur];
         invert_kernel<<<(n + 255) / 256, 256, 0, s>>>(perm, d_inv, n);
+        launched();
         CLOAK_LAUNCH_CHECK();
     }
     CLOAK_CUDA(cudaFreeAsync(ws, s));

@@ -161,6 +161,7 @@ static cloak_status rows(const void* src, void* dst, const uint32_t* map, uint32
     const uint32_t cap = (uint32_t)sms * 8;
     if (ctas > cap) ctas = cap;
     gather_rows_kernel<<<ctas, 256, 0, s>>>((const int4*)src, (int4*)dst, map, seg, nrows, (uint32_t)(row_bytes / 16));
+    launched();
     CLOAK_LAUNCH_CHECK();
     return CLOAK_OK;
 }
@@ -178,8 +179,10 @@ static cloak_status cols(const void* src, void* dst, const uint32_t* map, uint32
         const uint32_t per_sm = smem <= 100 * 1024 ? 2u : 1u;
         uint32_t ctas = nrows < (uint32_t)sms * per_sm ? nrows : (uint32_t)sms * per_sm;
         gather_cols_kernel<E><<<ctas, 256, smem, s>>>((const E*)src, (E*)dst, map, seg, nrows, ncols);
+        launched();
     } else {
         gather_cols_global_kernel<E><<<sms * 8, 256, 0, s>>>((const E*)src, (E*)dst, map, seg, nrows, ncols);
+        launched();
     }
     CLOAK_LAUNCH_CHECK();
     return CLOAK_OK;
@@ -241,6 +244,7 @@ extern "C" cloak_status cloak_permute_mlp_heads(uint64_t key, const cloak_block_
     }
     if (st == CLOAK_OK && heads) {
         head_maps_kernel<<<1, 1024, 0, s>>>((uint32_t)key, (uint32_t)(key >> 32), sh->layer, sh->n_q, sh->n_kv, kappa, eta);
+        launched();
         if (cudaGetLastError() != cudaSuccess) st = fail(CLOAK_ERR_CUDA, "permute: head_maps launch failed");
         const uint32_t d = sh->head_dim;
         if (st == CLOAK_OK && d_q) st = rows(d_q, d_q_o, eta, d, sh->n_q * d, hrow, sms, s);
@@ -266,6 +270,7 @@ extern "C" cloak_status cloak_to_tile128(const void* d_src, void* d_dst, uint32_
     const uint32_t cap = (uint32_t)sm_count(dev) * 8;
     tile128_kernel<<<ntiles < cap ? ntiles : cap, 256, 0, (cudaStream_t)stream>>>(
         (const int4*)d_src, (int4*)d_dst, N, K, dt == CLOAK_F32 ? 32u : 16u);
+    launched();
     CLOAK_LAUNCH_CHECK();
     return CLOAK_OK;
 }
@@ -280,6 +285,7 @@ extern "C" cloak_status cloak_silu_mul(const void* d_g, const void* d_u, void* d
         silu_mul_bf16_kernel<<<blocks, 256, 0, (cudaStream_t)stream>>>((const uint16_t*)d_g, (const uint16_t*)d_u, (uint16_t*)d_out, n);
     else
         return fail(CLOAK_ERR_UNSUPPORTED, "silu_mul: unknown dtype");
+    launched();
     CLOAK_LAUNCH_CHECK();
     return CLOAK_OK;
 }

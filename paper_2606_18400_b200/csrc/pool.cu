@@ -44,6 +44,7 @@ static cloak_status destroy_impl(cloak_pool* p) {
         cudaFree(p->base);
     }
     if (p->d_tables) cudaFree(p->d_tables);
+    if (p->ws) cudaFree(p->ws);
     cudaGetLastError();
     delete p;
     return CLOAK_OK;
@@ -129,9 +130,13 @@ static cloak_status create_impl(cloak_pool* p) {
     auto run = [&]() -> cloak_status {
         if (identity) {
             iota_kernel<<<(p->nslots + 255) / 256, 256, 0, s>>>(p->d_blockperm, p->nslots);
+            launched();
             iota_kernel<<<(p->nslots + 255) / 256, 256, 0, s>>>(p->d_blockinv, p->nslots);
+            launched();
             iota_kernel<<<(p->npages + 255) / 256, 256, 0, s>>>(p->d_pageperm, p->npages);
+            launched();
             iota_kernel<<<(p->npages + 255) / 256, 256, 0, s>>>(p->d_pageinv, p->npages);
+            launched();
             CLOAK_LAUNCH_CHECK();
         } else {
             cloak_status e = keygen_device(p->key, 1ull << 32, p->nslots, p->d_blockperm, p->d_blockinv, s);
@@ -141,6 +146,7 @@ static cloak_status create_impl(cloak_pool* p) {
         }
         build_table_kernel<<<(p->nb + 255) / 256, 256, 0, s>>>(p->d_blockinv, p->d_pageinv, p->d_T, p->nb, p->bpp,
                                                                p->vmm ? 1 : 0);
+        launched();
         CLOAK_LAUNCH_CHECK();
         std::vector<uint32_t> pageinv(p->npages);
         CLOAK_CUDA(cudaMemcpyAsync(pageinv.data(), p->d_pageinv, (size_t)p->npages * 4, cudaMemcpyDeviceToHost, s));
