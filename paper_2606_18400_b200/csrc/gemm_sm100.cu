@@ -1,7 +1,309 @@
-// S7 cloak_gemm: placeholder until the tcgen05 kernel lands (returns CLOAK_ERR_UNSUPPORTED).
+// S7 cloak_gemm: batch 16..256 contraction on tcgen05 tensor cores, W tiles fetched by TMA through the table.
+//
+// Definition (north_star (c) "batch>1 gather-fused GEMM ... tcgen05/TMEM tiles fed by TMA through
+// the permutation table"; BASELINE.json configs[3]):  Y[m, n] = sum_k X[m, k] * W[n, k], W in CLOAK_TILE128
+// storage (tile (tn,tk) of 128x128 bf16 = 32 KiB contiguous, row-major inside), block_bytes >= 32 KiB.
+//
+// Mapping to the hardware.
+//   * The pool is ONE 2-D TMA tensor map: rows of 128 bf16 (256 B).  Tile index i of the tensor sits at arena
+//     byte w_offset + i*32 KiB = pool byte (T[blk] << log2 b) + within, i.e. at map row that/256: the permutation
+//     enters only as a TMA coordinate.  A tile is fetched as two boxes of [128 rows x 64 cols] with
+//     SWIZZLE_128B, which land in shared memory in the canonical K-major UMMA layout (8-row atoms of 1 KiB).
+//   * A operand = the W tile (M = 128 output features), B operand = X[batch, 64] boxes of a second map over X
+//     (N = batch), D = 128 lanes x batch fp32 columns in TMEM, two accumulator buffers.
+//   * Units = tiles, numbered tn-major (= TILE128 storage order), cut into equal contiguous ranges, one per
+//     persistent CTA (stream-K): HBM-bound (AI = batch flop/B < ridge), so what matters is that every SM
+//     streams the same bytes with a full TMA ring.  Roles: warp 0 TMA producer, warp 1 MMA issuer (one lane)
+//     + TMEM allocator, warps 2-5 epilogue (tcgen05.ld 32x32b, one TMEM lane quarter each).
+//   * A tile row wholly inside a CTA's range is stored as bf16 straight from TMEM; one cut by a range boundary
+//     writes fp32 partials and the last contributor sums them in contributor order (deterministic; identical
+//     for cloaked and identity-table pools).
+#include <cuda_bf16.h>
 #include "common.cuh"
+#include "async.cuh"
+
+namespace cloak {
+
+struct GemmArgs {
+    const uint32_t* T;
+    uint32_t log2b;
+    uint64_t w_offset;
+    uint32_t N, K, batch;
+    __nv_bfloat16* y;
+    uint32_t kt;         // k tiles per tile row = K/128
+    uint32_t units;      // (N/128) * kt
+    uint32_t per;        // units per CTA
+    uint32_t maxc;       // max contributors per tile row
+    uint32_t stages;
+    uint32_t stage_bytes;
+    uint32_t tmem_cols;  // power of two >= 2*batch
+    float* part;         // [tile row][maxc][batch][128]
+    uint32_t* counters;
+};
+
+constexpr int GM_THREADS = 192;            // warp 0 TMA, warp 1 MMA, warps 2..5 epilogue
+constexpr int GM_MAX_STAGES = 6;
+
+__device__ __forceinline__ void tma_load_2d(uint32_t dst, const CUtensorMap* map, uint32_t c0, uint32_t c1, uint32_t bar) {
+    asm volatile("cp.async.bulk.tensor.2d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3}], [%4];"
+                 :: "r"(dst), "l"(map), "r"(c0), "r"(c1), "r"(bar) : "memory");
+}
+__device__ __forceinline__ void tc_fence_after() { asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory"); }
+__device__ __forceinline__ void tc_fence_before() { asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory"); }
+__device__ __forceinline__ void tc_commit(uint32_t bar) {
+    asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];" :: "r"(bar) : "memory");
+}
+__device__ __forceinline__ void tc_mma_bf16(uint32_t d_tmem, uint64_t adesc, uint64_t bdesc, uint32_t idesc, uint32_t acc) {
+    asm volatile(
+        "{\n\t.reg .pred p;\n\t"
+        "setp.ne.b32 p, %4, 0;\n\t"
+        "tcgen05.mma.cta_group::1.kind::f16 [%0], %1, %2, %3, p;\n\t}"
+        :: "r"(d_tmem), "l"(adesc), "l"(bdesc), "r"(idesc), "r"(acc) : "memory");
+}
+__device__ __forceinline__ void tc_ld16(uint32_t taddr, uint32_t (&r)[16]) {
+    asm volatile("tcgen05.ld.sync.aligned.32x32b.x16.b32 {%0,%1,%2,%3,%4,%5,%6,%7,%8,%9,%10,%11,%12,%13,%14,%15}, [%16];"
+                 : "=r"(r[0]), "=r"(r[1]), "=r"(r[2]), "=r"(r[3]), "=r"(r[4]), "=r"(r[5]), "=r"(r[6]), "=r"(r[7]),
+                   "=r"(r[8]), "=r"(r[9]), "=r"(r[10]), "=r"(r[11]), "=r"(r[12]), "=r"(r[13]), "=r"(r[14]), "=r"(r[15])
+                 : "r"(taddr));
+    asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
+}
+// K-major, SWIZZLE_128B shared-memory matrix descriptor (sm_100 format): 8-row atoms of 1024 B.
+__device__ __forceinline__ uint64_t umma_desc_sw128(uint32_t smem_addr) {
+    return (uint64_t)((smem_addr & 0x3FFFF) >> 4) | ((uint64_t)(1024 >> 4) << 32) | (1ull << 46) | (2ull << 61);
+}
+__device__ __forceinline__ void epi_bar() { asm volatile("bar.sync 1, 128;" ::: "memory"); }
+
+__global__ void __launch_bounds__(GM_THREADS, 1) gemm_tile128_kernel(const __grid_constant__ CUtensorMap map_w,
+                                                                     const __grid_constant__ CUtensorMap map_x,
+                                                                     GemmArgs a) {
+    extern __shared__ __align__(1024) unsigned char smem_raw[];
+    __shared__ __align__(8) uint64_t full[GM_MAX_STAGES], empty[GM_MAX_STAGES], tmem_full[2], tmem_empty[2];
+    __shared__ uint32_t tmem_base_s, last_flag;
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    // dynamic shared memory is only guaranteed 16-byte aligned: round up to the 1 KiB the 128-byte swizzle needs
+    const uint32_t smem_base = (smem_u32(smem_raw) + 1023u) & ~1023u;
+
+    if (threadIdx.x == 0) {
+        for (uint32_t s = 0; s < a.stages; ++s) {
+            mbar_init(smem_u32(&full[s]), 1);
+            mbar_init(smem_u32(&empty[s]), 1);
+        }
+        for (int i = 0; i < 2; ++i) {
+            mbar_init(smem_u32(&tmem_full[i]), 1);
+            mbar_init(smem_u32(&tmem_empty[i]), 4);
+        }
+        fence_barrier_init();
+    }
+    if (warp == 1) {
+        asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;"
+                     :: "r"(smem_u32(&tmem_base_s)), "r"(a.tmem_cols) : "memory");
+        asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
+    }
+    tc_fence_before();
+    __syncthreads();
+    tc_fence_after();
+    const uint32_t tmem_base = tmem_base_s;
+
+    const uint32_t ubeg = blockIdx.x * a.per;
+    const uint32_t uend = min(ubeg + a.per, a.units);
+    const uint32_t xbox = a.batch * 128;                     // bytes of one X box [batch x 64 bf16]
+
+    if (warp == 0 && lane == 0 && ubeg < uend) {
+        // ---------------------------------------------------------------- TMA producer
+        uint32_t it = 0;
+        for (uint32_t u = ubeg; u < uend; ++u, ++it) {
+            const uint32_t s = it % a.stages, f = it / a.stages;
+            if (f > 0) mbar_wait(smem_u32(&empty[s]), (f - 1) & 1);
+            const uint32_t tk = u % a.kt;
+            const uint64_t off = a.w_offset + (uint64_t)u * 32768;               // tile index == unit index
+            const uint32_t slot = __ldg(a.T + (off >> a.log2b));
+            const uint64_t byte = ((uint64_t)slot << a.log2b) + (off & ((1ull << a.log2b) - 1));
+            const uint32_t row = (uint32_t)(byte >> 8);                          // pool viewed as rows of 256 B
+            const uint32_t st = smem_base + s * a.stage_bytes;
+            const uint32_t bar = smem_u32(&full[s]);
+            mbar_expect_tx(bar, 32768 + 2 * xbox);
+            tma_load_2d(st, &map_w, 0, row, bar);
+            tma_load_2d(st + 16384, &map_w, 64, row, bar);
+            tma_load_2d(st + 32768, &map_x, tk * 128, 0, bar);
+            tma_load_2d(st + 32768 + xbox, &map_x, tk * 128 + 64, 0, bar);
+        }
+    } else if (warp == 1 && lane == 0 && ubeg < uend) {
+        // ---------------------------------------------------------------- MMA issuer
+        const uint32_t idesc = (1u << 4) | (1u << 7) | (1u << 10) | ((a.batch >> 3) << 17) | ((128u >> 4) << 24);
+        uint32_t it = 0, seg = 0, cur_tn = ubeg / a.kt;
+        bool first = true;
+        for (uint32_t u = ubeg; u < uend; ++u, ++it) {
+            const uint32_t tn = u / a.kt;
+            if (tn != cur_tn) {
+                tc_commit(smem_u32(&tmem_full[seg & 1]));                        // accumulator of the finished tile row
+                ++seg;
+                cur_tn = tn;
+                first = true;
+            }
+            if (first && seg >= 2) {
+                mbar_wait(smem_u32(&tmem_empty[seg & 1]), ((seg >> 1) - 1) & 1);
+                tc_fence_after();
+            }
+            const uint32_t s = it % a.stages, f = it / a.stages;
+            mbar_wait(smem_u32(&full[s]), f & 1);
+            tc_fence_after();
+            const uint32_t st = smem_base + s * a.stage_bytes;
+            const uint32_t d = tmem_base + (seg & 1) * a.batch;
+#pragma unroll
+            for (int box = 0; box < 2; ++box) {
+                const uint64_t ad = umma_desc_sw128(st + box * 16384);
+                const uint64_t bd = umma_desc_sw128(st + 32768 + box * xbox);
+#pragma unroll
+                for (int k = 0; k < 4; ++k)                                      // UMMA_K = 16 bf16 = 32 B inside the atom
+                    tc_mma_bf16(d, ad + 2 * k, bd + 2 * k, idesc, (first && box == 0 && k == 0) ? 0u : 1u);
+            }
+            first = false;
+            tc_commit(smem_u32(&empty[s]));                                      // frees the stage when the MMAs retire
+        }
+        tc_commit(smem_u32(&tmem_full[seg & 1]));
+    } else if (warp >= 2 && ubeg < uend) {
+        // ---------------------------------------------------------------- epilogue (4 warps = 4 TMEM lane quarters)
+        const uint32_t q = warp & 3, r = q * 32 + lane;
+        const int etid = threadIdx.x - 64;
+        uint32_t seg = 0;
+        for (uint32_t u = ubeg; u < uend; ++seg) {
+            const uint32_t tn = u / a.kt;
+            const uint32_t t_first = tn * a.kt, t_last = t_first + a.kt - 1;
+            const uint32_t seg_last = min(uend - 1, t_last);
+            const bool complete = (u == t_first) && (seg_last == t_last);
+            mbar_wait(smem_u32(&tmem_full[seg & 1]), (seg >> 1) & 1);
+            tc_fence_after();
+            const uint32_t taddr = tmem_base + ((q * 32) << 16) + (seg & 1) * a.batch;
+            const size_t n = (size_t)tn * 128 + r;
+            const uint32_t nout = a.batch * 128;
+            const uint32_t c_first = t_first / a.per, c_last = t_last / a.per;
+            const uint32_t ncontrib = c_last - c_first + 1, me = blockIdx.x - c_first;
+            float* mine = a.part + ((size_t)tn * a.maxc + me) * nout;
+            for (uint32_t c = 0; c < a.batch; c += 16) {
+                uint32_t v[16];
+                tc_ld16(taddr + c, v);
+                if (complete) {
+#pragma unroll
+                    for (int j = 0; j < 16; ++j) a.y[(size_t)(c + j) * a.N + n] = __float2bfloat16_rn(__uint_as_float(v[j]));
+                } else {
+#pragma unroll
+                    for (int j = 0; j < 16; ++j) __stcg(mine + (size_t)(c + j) * 128 + r, __uint_as_float(v[j]));
+                }
+            }
+            tc_fence_before();
+            __syncwarp();
+            if (lane == 0) mbar_arrive(smem_u32(&tmem_empty[seg & 1]));
+            if (!complete) {
+                __threadfence();
+                epi_bar();
+                if (etid == 0) {
+                    const uint32_t old = atomicAdd(a.counters + tn, 1u);
+                    last_flag = (old == ncontrib - 1);
+                    if (old == ncontrib - 1) a.counters[tn] = 0;                 // self-reset for the next launch
+                }
+                epi_bar();
+                if (last_flag) {
+                    __threadfence();
+                    const float* base = a.part + (size_t)tn * a.maxc * nout;
+                    for (uint32_t m = 0; m < a.batch; ++m) {
+                        float s = 0.f;
+                        for (uint32_t p = 0; p < ncontrib; ++p) s += __ldcg(base + (size_t)p * nout + (size_t)m * 128 + r);
+                        a.y[(size_t)m * a.N + n] = __float2bfloat16_rn(s);
+                    }
+                }
+                epi_bar();
+            }
+            u = seg_last + 1;
+        }
+    }
+    tc_fence_before();
+    __syncthreads();
+    if (warp == 1) {
+        tc_fence_after();
+        asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" :: "r"(tmem_base), "r"(a.tmem_cols) : "memory");
+    }
+}
+
+static cloak_status make_map(CUtensorMap* map, const void* base, uint64_t inner, uint64_t rows, uint64_t pitch_bytes,
+                             uint32_t box_inner, uint32_t box_rows) {
+    const DriverApi* d = driver();
+    if (!d) return CLOAK_ERR_CUDA;
+    cuuint64_t dims[2] = {inner, rows};
+    cuuint64_t strides[1] = {pitch_bytes};
+    cuuint32_t box[2] = {box_inner, box_rows};
+    cuuint32_t estr[2] = {1, 1};
+    CLOAK_CU(d->TensorMapEncodeTiled(map, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 2, const_cast<void*>(base), dims, strides, box,
+                                     estr, CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B,
+                                     CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE));
+    return CLOAK_OK;
+}
+
+cloak_status check_linear(const cloak_pool* pool, const cloak_tensor* w, const void* x, void* y, const char* who);
+
+}  // namespace cloak
+
+using namespace cloak;
+
 extern "C" cloak_status cloak_gemm(const cloak_pool* pool, const cloak_tensor* w, const void* d_x, void* d_y,
                                    uint32_t batch, void* stream) {
-    (void)pool; (void)w; (void)d_x; (void)d_y; (void)batch; (void)stream;
-    return cloak::fail(CLOAK_ERR_UNSUPPORTED, "gemm: not implemented yet");
+    cloak_status st = check_linear(pool, w, d_x, d_y, "gemm");
+    if (st != CLOAK_OK) return st;
+    if (batch < 16 || batch > 256 || batch % 16) return fail(CLOAK_ERR_INVALID, "gemm: batch must be a multiple of 16 in 16..256");
+    if (w->dt != CLOAK_BF16 || w->layout != CLOAK_TILE128) return fail(CLOAK_ERR_UNSUPPORTED, "gemm: needs CLOAK_BF16 in CLOAK_TILE128 layout");
+    if (w->N % 128 || w->K % 128) return fail(CLOAK_ERR_ALIGN, "gemm: N and K must be multiples of 128");
+    if (pool->block < 32768) return fail(CLOAK_ERR_UNSUPPORTED, "gemm: block_bytes must be >= 32 KiB (one 128x128 bf16 tile)");
+    DeviceGuard g(pool->device);
+    cudaStream_t s = (cudaStream_t)stream;
+
+    if (!pool->tmap_ready) {
+        cloak_pool* p = const_cast<cloak_pool*>(pool);
+        st = make_map(&p->tmap_tile128, pool->base, 128, pool->bytes() / 256, 256, 64, 128);
+        if (st != CLOAK_OK) return st;
+        p->tmap_ready = true;
+    }
+    CUtensorMap map_x;
+    st = make_map(&map_x, d_x, w->K, batch, (uint64_t)w->K * 2, 64, batch);
+    if (st != CLOAK_OK) return st;
+
+    GemmArgs a;
+    a.T = pool->d_T;
+    a.log2b = pool->log2_block;
+    a.w_offset = w->w_offset;
+    a.N = w->N;
+    a.K = w->K;
+    a.batch = batch;
+    a.y = static_cast<__nv_bfloat16*>(d_y);
+    a.kt = w->K / 128;
+    const uint32_t tile_rows = w->N / 128;
+    const uint64_t units64 = (uint64_t)tile_rows * a.kt;
+    if (units64 > 0xffffffffull) return fail(CLOAK_ERR_UNSUPPORTED, "gemm: tensor too large");
+    a.units = (uint32_t)units64;
+    const int sms = sm_count(pool->device);
+    a.per = (a.units + sms - 1) / sms;
+    const int ctas = (int)((a.units + a.per - 1) / a.per);
+    a.maxc = (a.kt + a.per - 1) / a.per + 1;
+    a.stage_bytes = 32768 + batch * 256;
+    uint32_t stages = (uint32_t)((218u * 1024u) / a.stage_bytes);
+    if (stages > GM_MAX_STAGES) stages = GM_MAX_STAGES;
+    if (stages < 2) return fail(CLOAK_ERR_UNSUPPORTED, "gemm: batch too large for the shared-memory ring");
+    a.stages = stages;
+    a.tmem_cols = 32;
+    while (a.tmem_cols < 2 * batch) a.tmem_cols <<= 1;
+    if ((size_t)tile_rows * 4 > WS_COUNTER_BYTES) return fail(CLOAK_ERR_UNSUPPORTED, "gemm: N too large for the tile counters");
+    const size_t need = WS_COUNTER_BYTES + (size_t)tile_rows * a.maxc * batch * 128 * 4;
+    st = pool_workspace(pool, need);
+    if (st != CLOAK_OK) return st;
+    a.counters = reinterpret_cast<uint32_t*>(pool->ws);
+    a.part = reinterpret_cast<float*>(pool->ws + WS_COUNTER_BYTES);
+
+    const size_t smem = (size_t)stages * a.stage_bytes + 1024;
+    static bool attr_set = false;
+    if (!attr_set) {
+        CLOAK_CUDA(cudaFuncSetAttribute(gemm_tile128_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 225 * 1024));
+        attr_set = true;
+    }
+    gemm_tile128_kernel<<<ctas, GM_THREADS, smem, s>>>(pool->tmap_tile128, map_x, a);
+    launched();
+    CLOAK_LAUNCH_CHECK();
+    return CLOAK_OK;
 }

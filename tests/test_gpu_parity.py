@@ -333,6 +333,66 @@ def test_cfg0_mlp_end_to_end_permuted_and_cloaked():
         assert O.err_normwise(y.cpu().numpy(), ref) <= 2e-5
 
 
+# ------------------------------------------------------------------ S7 cloaked GEMM (tcgen05, TILE128)
+GEMM_CASES = [
+    # block, shapes [(N, K)], batches
+    (32768, [(128, 128), (256, 384)], [16, 32]),                        # one tile; several tiles, one tile per block
+    (65536, [(1024, 5120), (5120, 1024)], [32, 128]),                   # cfg3's k/v shape and a tall one; stream-K cuts
+    (65536, [(384, 640)], [48, 256]),                                   # odd tile counts, widest batch
+    (2 << 20, [(512, 512)], [64]),                                      # block == page
+]
+
+
+@pytest.mark.parametrize("block,shapes,batches", GEMM_CASES)
+def test_gemm_vs_oracle_and_identity_bit_identical(block, shapes, batches):
+    key, seed, page = 0x1234, 3, 2 << 20
+    tensors = [(f"t{i}", gen.synth(seed, i, shp, "bf16")) for i, shp in enumerate(shapes)]
+    sizes = [a.size * 2 for _, a in tensors]
+    offs, total = C.cloak_arena_plan(key, sizes, block)
+    with Pool(total, block, page, key) as pc, Pool(total, block, page, key, C.CLOAK_POOL_IDENTITY) as pi:
+        for (nm, Wm), off in zip(tensors, offs):
+            N, K = Wm.shape
+            src = bf16_dev_from_bits(Wm)
+            til = torch.empty(N * K, dtype=torch.bfloat16, device="cuda")
+            C.cloak_to_tile128(src, til, N, K, C.CLOAK_BF16)                 # O0 stage (2): storage layout
+            assert np.array_equal(bits_from_bf16_dev(til), O.to_tile128(Wm))
+            for p in (pc, pi):
+                C.cloak_shuffle(p.h, til, off, N * K * 2)
+        for (nm, Wm), off in zip(tensors, offs):
+            N, K = Wm.shape
+            w = C.cloak_tensor(off, N, K, C.CLOAK_BF16, C.CLOAK_TILE128)
+            for batch in batches:
+                X = gen.synth(seed + 100, batch, (batch, K), "bf16", kind=gen.KIND_NORMAL)
+                dX = bf16_dev_from_bits(X)
+                yc = torch.zeros(batch, N, dtype=torch.bfloat16, device="cuda")
+                yi = torch.zeros_like(yc)
+                C.cloak_gemm(pc.h, w, dX, yc, batch)
+                C.cloak_gemm(pi.h, w, dX, yi, batch)
+                torch.cuda.synchronize()
+                assert torch.equal(yc, yi)
+                ref = O.linear_f64(X, Wm)
+                err = O.err_normwise(yc.float().cpu().numpy(), ref)
+                assert err <= TOL["bf16"], (nm, batch, err)
+                yc2 = torch.zeros_like(yc)                                   # second launch: counters self-reset
+                C.cloak_gemm(pc.h, w, dX, yc2, batch)
+                assert torch.equal(yc, yc2)
+
+
+def test_gemm_argument_checks():
+    with Pool(1 << 20, 4096, 65536, 1) as p:
+        x = torch.zeros(32, 128, dtype=torch.bfloat16, device="cuda")
+        y = torch.zeros(32, 128, dtype=torch.bfloat16, device="cuda")
+        for w, batch, st in [
+            (C.cloak_tensor(0, 128, 128, C.CLOAK_BF16, C.CLOAK_TILE128), 32, C.CLOAK_ERR_UNSUPPORTED),   # 4 KiB blocks
+            (C.cloak_tensor(0, 128, 128, C.CLOAK_BF16, C.CLOAK_ROWMAJOR), 32, C.CLOAK_ERR_UNSUPPORTED),
+            (C.cloak_tensor(0, 128, 128, C.CLOAK_BF16, C.CLOAK_TILE128), 8, C.CLOAK_ERR_INVALID),
+            (C.cloak_tensor(0, 100, 128, C.CLOAK_BF16, C.CLOAK_TILE128), 32, C.CLOAK_ERR_ALIGN),
+        ]:
+            with pytest.raises(C.CloakError) as ei:
+                C.cloak_gemm(p.h, w, x, y, batch)
+            assert ei.value.status == st
+
+
 # ------------------------------------------------------------------ errors
 def test_error_codes_on_device():
     with Pool(1 << 20, 4096, 65536, 1) as p:
