@@ -14,7 +14,7 @@
 //   * Units = tiles, numbered tn-major (= TILE128 storage order), cut into equal contiguous ranges, one per
 //     persistent CTA (stream-K): HBM-bound (AI = batch flop/B < ridge), so what matters is that every SM
 //     streams the same bytes with a full TMA ring.  Roles: warp 0 TMA producer, warp 1 MMA issuer (one lane)
-//     + TMEM allocator, warps 2-5 epilogue (tcgen05.ld 32x32b, one TMEM lane quarter each).
+//     + TMEM allocator, warp 2 TMA producer for X (own shallow ring), warps 3-6 epilogue (tcgen05.ld 32x32b, one TMEM lane quarter each).
 //   * A tile row wholly inside a CTA's range is stored as bf16 straight from TMEM; one cut by a range boundary
 //     writes fp32 partials and the last contributor sums them in contributor order (deterministic; identical
 //     for cloaked and identity-table pools).
@@ -34,14 +34,14 @@ struct GemmArgs {
     uint32_t units;      // (N/128) * kt
     uint32_t per;        // units per CTA
     uint32_t maxc;       // max contributors per tile row
-    uint32_t stages;
-    uint32_t stage_bytes;
+    uint32_t wstages;    // ring of 32 KiB weight tiles (HBM latency: deep)
+    uint32_t xstages;    // ring of X tiles [batch x 128] (L2 latency: shallow)
     uint32_t tmem_cols;  // power of two >= 2*batch
     float* part;         // [tile row][maxc][batch][128]
     uint32_t* counters;
 };
 
-constexpr int GM_THREADS = 192;            // warp 0 TMA, warp 1 MMA, warps 2..5 epilogue
+constexpr int GM_THREADS = 224;            // warp 0 TMA (W), warp 1 MMA, warp 2 TMA (X), warps 3..6 epilogue
 constexpr int GM_MAX_STAGES = 6;
 
 __device__ __forceinline__ void tma_load_2d(uint32_t dst, const CUtensorMap* map, uint32_t c0, uint32_t c1, uint32_t bar) {
@@ -77,16 +77,19 @@ __global__ void __launch_bounds__(GM_THREADS, 1) gemm_tile128_kernel(const __gri
                                                                      const __grid_constant__ CUtensorMap map_x,
                                                                      GemmArgs a) {
     extern __shared__ __align__(1024) unsigned char smem_raw[];
-    __shared__ __align__(8) uint64_t full[GM_MAX_STAGES], empty[GM_MAX_STAGES], tmem_full[2], tmem_empty[2];
+    __shared__ __align__(8) uint64_t wfull[GM_MAX_STAGES], wempty[GM_MAX_STAGES], xfull[GM_MAX_STAGES], xempty[GM_MAX_STAGES],
+        tmem_full[2], tmem_empty[2];
     __shared__ uint32_t tmem_base_s, last_flag;
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     // dynamic shared memory is only guaranteed 16-byte aligned: round up to the 1 KiB the 128-byte swizzle needs
     const uint32_t smem_base = (smem_u32(smem_raw) + 1023u) & ~1023u;
 
     if (threadIdx.x == 0) {
-        for (uint32_t s = 0; s < a.stages; ++s) {
-            mbar_init(smem_u32(&full[s]), 1);
-            mbar_init(smem_u32(&empty[s]), 1);
+        for (uint32_t s = 0; s < GM_MAX_STAGES; ++s) {
+            mbar_init(smem_u32(&wfull[s]), 1);
+            mbar_init(smem_u32(&wempty[s]), 1);
+            mbar_init(smem_u32(&xfull[s]), 1);
+            mbar_init(smem_u32(&xempty[s]), 1);
         }
         for (int i = 0; i < 2; ++i) {
             mbar_init(smem_u32(&tmem_full[i]), 1);
@@ -108,24 +111,37 @@ __global__ void __launch_bounds__(GM_THREADS, 1) gemm_tile128_kernel(const __gri
     const uint32_t uend = min(ubeg + a.per, a.units);
     const uint32_t xbox = a.batch * 128;                     // bytes of one X box [batch x 64 bf16]
 
+    const uint32_t xtile = 2 * xbox;
+    const uint32_t x_base = smem_base + a.wstages * 32768;
+
     if (warp == 0 && lane == 0 && ubeg < uend) {
-        // ---------------------------------------------------------------- TMA producer
+        // ---------------------------------------------------------------- TMA producer, weight tiles (through T)
         uint32_t it = 0;
         for (uint32_t u = ubeg; u < uend; ++u, ++it) {
-            const uint32_t s = it % a.stages, f = it / a.stages;
-            if (f > 0) mbar_wait(smem_u32(&empty[s]), (f - 1) & 1);
-            const uint32_t tk = u % a.kt;
+            const uint32_t s = it % a.wstages, f = it / a.wstages;
+            if (f > 0) mbar_wait(smem_u32(&wempty[s]), (f - 1) & 1);
             const uint64_t off = a.w_offset + (uint64_t)u * 32768;               // tile index == unit index
             const uint32_t slot = __ldg(a.T + (off >> a.log2b));
             const uint64_t byte = ((uint64_t)slot << a.log2b) + (off & ((1ull << a.log2b) - 1));
             const uint32_t row = (uint32_t)(byte >> 8);                          // pool viewed as rows of 256 B
-            const uint32_t st = smem_base + s * a.stage_bytes;
-            const uint32_t bar = smem_u32(&full[s]);
-            mbar_expect_tx(bar, 32768 + 2 * xbox);
+            const uint32_t st = smem_base + s * 32768;
+            const uint32_t bar = smem_u32(&wfull[s]);
+            mbar_expect_tx(bar, 32768);
             tma_load_2d(st, &map_w, 0, row, bar);
             tma_load_2d(st + 16384, &map_w, 64, row, bar);
-            tma_load_2d(st + 32768, &map_x, tk * 128, 0, bar);
-            tma_load_2d(st + 32768 + xbox, &map_x, tk * 128 + 64, 0, bar);
+        }
+    } else if (warp == 2 && lane == 0 && ubeg < uend) {
+        // ---------------------------------------------------------------- TMA producer, activation tiles (L2-resident)
+        uint32_t it = 0;
+        for (uint32_t u = ubeg; u < uend; ++u, ++it) {
+            const uint32_t s = it % a.xstages, f = it / a.xstages;
+            if (f > 0) mbar_wait(smem_u32(&xempty[s]), (f - 1) & 1);
+            const uint32_t tk = u % a.kt;
+            const uint32_t st = x_base + s * xtile;
+            const uint32_t bar = smem_u32(&xfull[s]);
+            mbar_expect_tx(bar, xtile);
+            tma_load_2d(st, &map_x, tk * 128, 0, bar);
+            tma_load_2d(st + xbox, &map_x, tk * 128 + 64, 0, bar);
         }
     } else if (warp == 1 && lane == 0 && ubeg < uend) {
         // ---------------------------------------------------------------- MMA issuer
@@ -144,27 +160,29 @@ __global__ void __launch_bounds__(GM_THREADS, 1) gemm_tile128_kernel(const __gri
                 mbar_wait(smem_u32(&tmem_empty[seg & 1]), ((seg >> 1) - 1) & 1);
                 tc_fence_after();
             }
-            const uint32_t s = it % a.stages, f = it / a.stages;
-            mbar_wait(smem_u32(&full[s]), f & 1);
+            const uint32_t ws = it % a.wstages, xs = it % a.xstages;
+            mbar_wait(smem_u32(&xfull[xs]), (it / a.xstages) & 1);
+            mbar_wait(smem_u32(&wfull[ws]), (it / a.wstages) & 1);
             tc_fence_after();
-            const uint32_t st = smem_base + s * a.stage_bytes;
+            const uint32_t st = smem_base + ws * 32768, sx = x_base + xs * xtile;
             const uint32_t d = tmem_base + (seg & 1) * a.batch;
 #pragma unroll
             for (int box = 0; box < 2; ++box) {
                 const uint64_t ad = umma_desc_sw128(st + box * 16384);
-                const uint64_t bd = umma_desc_sw128(st + 32768 + box * xbox);
+                const uint64_t bd = umma_desc_sw128(sx + box * xbox);
 #pragma unroll
                 for (int k = 0; k < 4; ++k)                                      // UMMA_K = 16 bf16 = 32 B inside the atom
                     tc_mma_bf16(d, ad + 2 * k, bd + 2 * k, idesc, (first && box == 0 && k == 0) ? 0u : 1u);
             }
             first = false;
-            tc_commit(smem_u32(&empty[s]));                                      // frees the stage when the MMAs retire
+            tc_commit(smem_u32(&wempty[ws]));                                    // frees both stages when the MMAs retire
+            tc_commit(smem_u32(&xempty[xs]));
         }
         tc_commit(smem_u32(&tmem_full[seg & 1]));
-    } else if (warp >= 2 && ubeg < uend) {
+    } else if (warp >= 3 && ubeg < uend) {
         // ---------------------------------------------------------------- epilogue (4 warps = 4 TMEM lane quarters)
         const uint32_t q = warp & 3, r = q * 32 + lane;
-        const int etid = threadIdx.x - 64;
+        const int etid = threadIdx.x - 96;
         uint32_t seg = 0;
         for (uint32_t u = ubeg; u < uend; ++seg) {
             const uint32_t tn = u / a.kt;
@@ -205,10 +223,17 @@ __global__ void __launch_bounds__(GM_THREADS, 1) gemm_tile128_kernel(const __gri
                 if (last_flag) {
                     __threadfence();
                     const float* base = a.part + (size_t)tn * a.maxc * nout;
-                    for (uint32_t m = 0; m < a.batch; ++m) {
-                        float s = 0.f;
-                        for (uint32_t p = 0; p < ncontrib; ++p) s += __ldcg(base + (size_t)p * nout + (size_t)m * 128 + r);
-                        a.y[(size_t)m * a.N + n] = __float2bfloat16_rn(s);
+                    for (uint32_t m = 0; m < a.batch; m += 16) {                 // 16 independent sums in flight
+                        float sum[16];
+#pragma unroll
+                        for (int j = 0; j < 16; ++j) sum[j] = 0.f;
+                        for (uint32_t p = 0; p < ncontrib; ++p) {
+                            const float* src = base + (size_t)p * nout + (size_t)m * 128 + r;
+#pragma unroll
+                            for (int j = 0; j < 16; ++j) sum[j] += __ldcg(src + j * 128);
+                        }
+#pragma unroll
+                        for (int j = 0; j < 16; ++j) a.y[(size_t)(m + j) * a.N + n] = __float2bfloat16_rn(sum[j]);
                     }
                 }
                 epi_bar();
@@ -280,13 +305,15 @@ extern "C" cloak_status cloak_gemm(const cloak_pool* pool, const cloak_tensor* w
     a.units = (uint32_t)units64;
     const int sms = sm_count(pool->device);
     a.per = (a.units + sms - 1) / sms;
+    if (a.per < (a.kt + 3) / 4) a.per = (a.kt + 3) / 4;      // at most ~5 contributors per tile row (partials traffic)
     const int ctas = (int)((a.units + a.per - 1) / a.per);
     a.maxc = (a.kt + a.per - 1) / a.per + 1;
-    a.stage_bytes = 32768 + batch * 256;
-    uint32_t stages = (uint32_t)((218u * 1024u) / a.stage_bytes);
-    if (stages > GM_MAX_STAGES) stages = GM_MAX_STAGES;
-    if (stages < 2) return fail(CLOAK_ERR_UNSUPPORTED, "gemm: batch too large for the shared-memory ring");
-    a.stages = stages;
+    const uint32_t xtile = batch * 256;
+    a.xstages = 2;
+    uint32_t wst = (224u * 1024u - a.xstages * xtile) / 32768u;
+    if (wst > GM_MAX_STAGES) wst = GM_MAX_STAGES;
+    if (wst < 2) return fail(CLOAK_ERR_UNSUPPORTED, "gemm: batch too large for the shared-memory ring");
+    a.wstages = wst;
     a.tmem_cols = 32;
     while (a.tmem_cols < 2 * batch) a.tmem_cols <<= 1;
     if ((size_t)tile_rows * 4 > WS_COUNTER_BYTES) return fail(CLOAK_ERR_UNSUPPORTED, "gemm: N too large for the tile counters");
@@ -296,10 +323,10 @@ extern "C" cloak_status cloak_gemm(const cloak_pool* pool, const cloak_tensor* w
     a.counters = reinterpret_cast<uint32_t*>(pool->ws);
     a.part = reinterpret_cast<float*>(pool->ws + WS_COUNTER_BYTES);
 
-    const size_t smem = (size_t)stages * a.stage_bytes + 1024;
+    const size_t smem = (size_t)a.wstages * 32768 + (size_t)a.xstages * xtile + 1024;
     static bool attr_set = false;
     if (!attr_set) {
-        CLOAK_CUDA(cudaFuncSetAttribute(gemm_tile128_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 225 * 1024));
+        CLOAK_CUDA(cudaFuncSetAttribute(gemm_tile128_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 226 * 1024));
         attr_set = true;
     }
     gemm_tile128_kernel<<<ctas, GM_THREADS, smem, s>>>(pool->tmap_tile128, map_x, a);
