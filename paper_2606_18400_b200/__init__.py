@@ -13,6 +13,8 @@ def __getattr__(name):
     global _binding
     if name.startswith("__"):
         raise AttributeError(name)
+    if name in ("build", "binding"):  # submodules: `from paper_2606_18400_b200 import build` must not load the .so
+        return importlib.import_module("." + name, __name__)
     if _binding is None:
         _binding = importlib.import_module(".binding", __name__)
     try:
