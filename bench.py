@@ -405,7 +405,14 @@ def main():
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="cloak", choices=["cloak", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--workload", default="cfg1", choices=["cfg1", "cfg2", "cfg3", "cfg4"],
+                    help="cfg1 (default) is the headline step; cfg2-4 are the other BASELINE.json configs "
+                         "(paper_2606_18400_b200/workloads.py), each printing its own JSON line")
+    ap.add_argument("--reps", type=int, default=10, help="repetitions per measurement for --workload cfg2-4")
     args = ap.parse_args()
+    if args.workload != "cfg1":
+        from paper_2606_18400_b200 import workloads
+        return workloads.main([args.workload, "--reps", str(args.reps)])
     args.warmup = max(args.warmup, 3) if args.impl == "cloak" else args.warmup
     return run_reference(args) if args.impl == "reference" else run_cloak(args)
 

@@ -161,7 +161,13 @@ cloak_status cloak_to_tile128(const void* d_src, void* d_dst, uint32_t N, uint32
  * Y[m, n] = sum_k X[m, k] * W[n, k].  W lives in the pool at arena byte offset w_offset (a block
  * multiple), logical shape [N, K], read through the pool's table T.  X [batch, K] and Y [batch, N] are
  * row-major device buffers of W's dtype, 16-byte aligned.  Accumulation is fp32.
- * cloak_gemv: batch 1..16, layout ROWMAJOR, K a multiple of 128 (bf16) / 128 (f32).
+ * cloak_gemv: batch 1..16, layout ROWMAJOR, K a multiple of 64 and N of 16 (bf16) / K of 4 (f32).
+ *             Stream order: X, Y and the library's scratch are touched in stream order.  The bf16 streaming
+ *             kernel is launched with programmatic dependent launch and may begin fetching W while the
+ *             preceding kernel of `stream` drains; the library withholds that for the first GEMV that follows
+ *             a cloak_shuffle* / cloak_relayout into the pool (those calls mark the pool).  Code that writes
+ *             pool memory by other means (through cloak_pool_info's d_base) must synchronise before the
+ *             next cloak_gemv.
  * cloak_gemm: batch 16..256 (multiple of 16), dtype BF16, layout TILE128, block_bytes >= 32 KiB
  *             (tcgen05 tensor cores, accumulators in TMEM, tiles fetched by TMA through the table).
  * Asynchronous on `stream`. */
@@ -175,8 +181,9 @@ cloak_status cloak_gemv(const cloak_pool* pool, const cloak_tensor* w, const voi
                         uint32_t batch, void* stream);
 cloak_status cloak_gemm(const cloak_pool* pool, const cloak_tensor* w, const void* d_x, void* d_y,
                         uint32_t batch, void* stream);
-/* Selects the bf16 GEMV kernel: 0 = automatic (streaming TMA kernel when K % 256 == 0), 1 = always the
- * one-shot split-K kernel.  For A/B measurement; process-wide. */
+/* Selects the bf16 GEMV kernel: 0 = automatic (streaming TMA kernel when K % 256 == 0, launched with
+ * programmatic dependent launch), 1 = always the one-shot split-K kernel, 2 = automatic without
+ * programmatic dependent launch.  For A/B measurement; process-wide. */
 cloak_status cloak_set_gemv_engine(int engine);
 /* Host-buffer variant of cloak_gemv (end-to-end path): copies X up, runs, copies Y back, synchronises. */
 cloak_status cloak_gemv_host(const cloak_pool* pool, const cloak_tensor* w, const void* h_x, void* h_y,

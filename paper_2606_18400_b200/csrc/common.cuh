@@ -112,6 +112,11 @@ struct cloak_pool {
              *d_T = nullptr;
     CUtensorMap tmap_tile128;   // GEMM: pool viewed as rows of 128 bf16 (gemm_sm100.cu), built lazily
     bool tmap_ready = false;
+    // Set (with the stream) by every library call that writes pool memory; consumed by the streaming GEMV, which
+    // may prefetch W ahead of its stream predecessor only when that predecessor cannot have written W.
+    mutable bool dirty = true;
+    mutable cudaStream_t dirty_stream = nullptr;
+    void wrote(cudaStream_t s) const { dirty = true; dirty_stream = s; }
     mutable char* ws = nullptr;     // library-owned scratch (GEMV / GEMM split-K partials + counters), lazily grown
     mutable size_t ws_bytes = 0;
     uint64_t bytes() const { return (uint64_t)nslots * block; }

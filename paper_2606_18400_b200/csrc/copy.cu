@@ -198,7 +198,7 @@ static cloak_status move_range(const cloak_pool* pool, char* d_logical, uint64_t
     a.first = first;
     a.nblocks = full;
     a.log2b = pool->log2_block;
-    if (dir == TO_POOL) { a.src = d_logical; a.dst = pool->base; a.src_tab = nullptr; a.dst_tab = pool->d_T; }
+    if (dir == TO_POOL) { a.src = d_logical; a.dst = pool->base; a.src_tab = nullptr; a.dst_tab = pool->d_T; pool->wrote(s); }
     else                { a.src = pool->base; a.dst = d_logical; a.src_tab = pool->d_T; a.dst_tab = nullptr; }
     cloak_status st = launch_copy(pool, a, s);
     if (st != CLOAK_OK) return st;
@@ -320,5 +320,6 @@ extern "C" cloak_status cloak_relayout(const cloak_pool* from_a, cloak_pool* to_
     a.first = 0;
     a.nblocks = from_a->nb;       // whole blocks: the zero tail of the last block travels with it
     a.log2b = from_a->log2_block;
+    to_b->wrote((cudaStream_t)stream);
     return launch_copy(from_a, a, (cudaStream_t)stream);
 }

@@ -255,6 +255,7 @@ cloak_status pool_workspace(const cloak_pool* pool, size_t bytes) {
 }
 
 static bool g_force_oneshot = false;     // A/B switch (cloak_set_gemv_engine)
+extern bool g_gemv_pdl;                   // gemv_stream.cu
 
 static cloak_status gemv_device(const cloak_pool* pool, const cloak_tensor* w, const void* d_x, void* d_y, uint32_t batch,
                                 cudaStream_t s) {
@@ -326,6 +327,7 @@ using namespace cloak;
 extern "C" cloak_status cloak_set_gemv_engine(int engine) {
     if (engine < 0 || engine > 2) return fail(CLOAK_ERR_INVALID, "set_gemv_engine: engine must be 0, 1 or 2");
     g_force_oneshot = engine == 1;
+    g_gemv_pdl = engine != 2;
     return CLOAK_OK;
 }
 

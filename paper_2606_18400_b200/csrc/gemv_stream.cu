@@ -35,6 +35,8 @@ struct GemvStreamArgs {
     uint32_t maxc;       // max contributors per tile
     float* part;         // [tile][maxc][batch][16]
     uint32_t* counters;  // [tile], zero between launches
+    uint32_t early;      // 1: W is unchanged since before the preceding kernel, so the producer may stream it
+                         //    ahead of griddepcontrol.wait (programmatic dependent launch)
 };
 
 constexpr int GS_STAGES = 6;
@@ -54,6 +56,12 @@ __device__ __forceinline__ uint4 lds128(uint32_t addr) {
     asm volatile("ld.shared.v4.u32 {%0,%1,%2,%3}, [%4];" : "=r"(r.x), "=r"(r.y), "=r"(r.z), "=r"(r.w) : "r"(addr));
     return r;
 }
+// Programmatic dependent launch (PDL): this grid may start while its stream predecessor is still draining.
+// grid_dep_wait returns once the predecessor has completed and its writes are visible; grid_dep_launch lets the
+// stream successor start.  Every kernel here triggers only AFTER its own wait, so whatever a successor does ahead
+// of its wait still observes everything older than its immediate predecessor.
+__device__ __forceinline__ void grid_dep_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
+__device__ __forceinline__ void grid_dep_launch() { asm volatile("griddepcontrol.launch_dependents;" ::: "memory"); }
 __device__ __forceinline__ void consumer_bar() { asm volatile("bar.sync 1, %0;" :: "n"(GS_CONSUMERS * 32) : "memory"); }
 
 // LOG2CB: log2 of the chunk bytes per row (9, 10 or 11).  NT: 8-wide batch tiles.
@@ -86,6 +94,9 @@ __global__ void __launch_bounds__(GS_THREADS, 1) gemv_stream_kernel(GemvStreamAr
 
     if (warp == 0) {
         // ------------------------------------------------------------ producer
+        // The table is immutable after cloak_pool_create; the weights may have been written by the preceding
+        // kernel (a shuffle / re-layout) unless the host says otherwise.
+        if (!a.early) grid_dep_wait();
         uint32_t it = 0;
         for (uint32_t u = ubeg; u < uend; ++u, ++it) {
             const uint32_t s = it % GS_STAGES, f = it / GS_STAGES;
@@ -118,6 +129,11 @@ __global__ void __launch_bounds__(GS_THREADS, 1) gemv_stream_kernel(GemvStreamAr
     for (int i = 0; i < NT; ++i)
 #pragma unroll
         for (int j = 0; j < 4; ++j) acc[i][j] = 0.f;
+
+    // X, Y, the split-K partials and counters all belong to stream order: nothing below touches them before the
+    // predecessor has completed.  Meanwhile the producer is already filling the ring.
+    grid_dep_wait();
+    if (ctid == 0) grid_dep_launch();
 
     auto flush = [&](uint32_t tile, uint32_t u_first, uint32_t u_last) {
         // u_first / u_last: the units of `tile` this CTA has accumulated (inclusive range)
@@ -175,26 +191,33 @@ __global__ void __launch_bounds__(GS_THREADS, 1) gemv_stream_kernel(GemvStreamAr
         consumer_bar();      // red[] and last_flag are reused by the next tile
     };
 
+    // Activations of one unit: this lane's 16-byte vectors of X rows g (and g+8).  They come from L2 (X is up to
+    // 16 x K x 2 bytes, more than the L1 left beside the ring), so the next unit's are fetched before this unit's
+    // weights are waited for: their latency hides behind the LDS/MMA work.
+    uint4 xa[KS][2], xb[KS][2], na[KS][2], nb[KS][2];
+    auto load_x = [&](uint4 (&pa)[KS][2], uint4 (&pb)[KS][2], uint32_t c) {
+        const uint32_t xk = c * (CB / 2);
+        const uint4 z = make_uint4(0, 0, 0, 0);
+#pragma unroll
+        for (int ks = 0; ks < KS; ++ks)
+#pragma unroll
+            for (int h = 0; h < 2; ++h) {
+                pa[ks][h] = xv0 ? __ldg(reinterpret_cast<const uint4*>(x0 + xk + ks * 64 + h * 32)) : z;
+                if (NT == 2) pb[ks][h] = xv1 ? __ldg(reinterpret_cast<const uint4*>(x1 + xk + ks * 64 + h * 32)) : z;
+            }
+    };
+    load_x(xa, xb, ubeg % a.kch);
+
     uint32_t cur_tile = ubeg / a.kch, tile_first_u = ubeg;
     uint32_t it = 0;
     for (uint32_t u = ubeg; u < uend; ++u, ++it) {
-        const uint32_t tile = u / a.kch, c = u - tile * a.kch;
+        const uint32_t tile = u / a.kch;
         if (tile != cur_tile) {
             flush(cur_tile, tile_first_u, u - 1);
             cur_tile = tile;
             tile_first_u = u;
         }
-        // activations first (L2/L1 hits, independent of the stage), then wait for the weights
-        uint4 xa[KS][2], xb[KS][2];
-        const uint32_t xk = c * (CB / 2);
-#pragma unroll
-        for (int ks = 0; ks < KS; ++ks)
-#pragma unroll
-            for (int h = 0; h < 2; ++h) {
-                const uint4 z = make_uint4(0, 0, 0, 0);
-                xa[ks][h] = xv0 ? __ldg(reinterpret_cast<const uint4*>(x0 + xk + ks * 64 + h * 32)) : z;
-                if (NT == 2) xb[ks][h] = xv1 ? __ldg(reinterpret_cast<const uint4*>(x1 + xk + ks * 64 + h * 32)) : z;
-            }
+        if (u + 1 < uend) load_x(na, nb, (u + 1) % a.kch);
         const uint32_t s = it % GS_STAGES, f = it / GS_STAGES;
         mbar_wait(smem_u32(&full[s]), f & 1);
         const uint32_t lo = smem_base + s * STAGE + g * RS + lane_off;
@@ -214,9 +237,18 @@ __global__ void __launch_bounds__(GS_THREADS, 1) gemv_stream_kernel(GemvStreamAr
             }
         __syncwarp();
         if (lane == 0) mbar_arrive(smem_u32(&empty[s]));
+#pragma unroll
+        for (int ks = 0; ks < KS; ++ks)
+#pragma unroll
+            for (int h = 0; h < 2; ++h) {
+                xa[ks][h] = na[ks][h];
+                if (NT == 2) xb[ks][h] = nb[ks][h];
+            }
     }
     flush(cur_tile, tile_first_u, uend - 1);
 }
+
+bool g_gemv_pdl = true;      // A/B switch (cloak_set_gemv_engine(2) turns PDL off)
 
 template <int LOG2CB, int NT>
 static cloak_status launch(const GemvStreamArgs& a, int ctas, cudaStream_t s) {
@@ -226,7 +258,17 @@ static cloak_status launch(const GemvStreamArgs& a, int ctas, cudaStream_t s) {
         CLOAK_CUDA(cudaFuncSetAttribute(gemv_stream_kernel<LOG2CB, NT>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
         attr_set = true;
     }
-    gemv_stream_kernel<LOG2CB, NT><<<ctas, GS_THREADS, smem, s>>>(a);
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = dim3(ctas);
+    cfg.blockDim = dim3(GS_THREADS);
+    cfg.dynamicSmemBytes = smem;
+    cfg.stream = s;
+    cudaLaunchAttribute at[1];
+    at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    at[0].val.programmaticStreamSerializationAllowed = 1;
+    cfg.attrs = at;
+    cfg.numAttrs = g_gemv_pdl ? 1 : 0;
+    CLOAK_CUDA(cudaLaunchKernelEx(&cfg, gemv_stream_kernel<LOG2CB, NT>, a));
     launched();
     CLOAK_LAUNCH_CHECK();
     return CLOAK_OK;
@@ -265,6 +307,8 @@ cloak_status gemv_stream_bf16(const cloak_pool* pool, const cloak_tensor* w, con
     if (st != CLOAK_OK) return st;
     a.counters = reinterpret_cast<uint32_t*>(pool->ws);
     a.part = reinterpret_cast<float*>(pool->ws + WS_COUNTER_BYTES);
+    a.early = (g_gemv_pdl && !pool->dirty) ? 1u : 0u;
+    if (pool->dirty && pool->dirty_stream == s) pool->dirty = false;   // this launch waits for the writer in full
     const bool nt2 = batch > 8;
     switch (log2cb) {
         case 11: return nt2 ? launch<11, 2>(a, ctas, s) : launch<11, 1>(a, ctas, s);

@@ -1,0 +1,334 @@
+"""Measurement drivers for BASELINE.json configs[2..4]; configs[1] is bench.py's own step.
+
+    python -m paper_2606_18400_b200.workloads cfg2|cfg3|cfg4 [--reps R] [--out file.json]
+    python bench.py --workload cfg2|cfg3|cfg4            (same thing)
+
+Each prints ONE JSON line.  Everything on the timed path is a C-ABI call of libcloak.so (through the ctypes
+binding); torch supplies device buffers, streams, events and CUDA-graph capture.  Inputs are seeded and
+synthetic (synth/, the shared generator: shapes of the paper's Llama-3.1-8B / Qwen3-32B checkpoints, values
+~N(0, 0.02)).  Parity of these sizes against the CPU oracle is the job of tests/test_gpu_fullsize.py; here the
+only checks are self-consistency ones (round trip restores the bytes, cloaked == identity-table output).
+"""
+import argparse
+import json
+import os
+import sys
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+NOMINAL_HBM_GBS = 8000.0
+FALLBACK_HBM_GBS = 6650.0
+
+
+def hbm_peak():
+    try:
+        with open(os.path.join(ROOT, "MEASURED_PEAKS.json")) as f:
+            return float(json.load(f)["hbm_gbs"]), "measured"
+    except Exception:
+        return FALLBACK_HBM_GBS, "fallback"
+
+
+def _imports():
+    import torch
+    import paper_2606_18400_b200 as C
+    from synth import cuda as synth_cuda
+    from synth import gen
+    if not torch.cuda.is_available():
+        raise SystemExit("workloads: no CUDA device; the cloak path has no CPU fallback")
+    return torch, C, synth_cuda, gen
+
+
+def time_gpu(torch, fn, reps, warmup=3, stream=None):
+    """Median and min milliseconds of fn() over `reps` runs, CUDA events on the launching stream."""
+    stream = stream or torch.cuda.current_stream()
+    for _ in range(warmup):
+        fn()
+    torch.cuda.synchronize()
+    ev = [torch.cuda.Event(enable_timing=True) for _ in range(reps + 1)]
+    ev[0].record(stream)
+    for i in range(reps):
+        fn()
+        ev[i + 1].record(stream)
+    torch.cuda.synchronize()
+    ts = [ev[i].elapsed_time(ev[i + 1]) for i in range(reps)]
+    return float(np.median(ts)), float(np.min(ts))
+
+
+def graphed(torch, fn):
+    """Capture fn() (asynchronous C-ABI launches on torch's current stream) into a CUDA graph; returns the replay
+    callable.  Capture runs on a side stream, which is the current stream inside the `with`."""
+    fn()
+    torch.cuda.synchronize()
+    g = torch.cuda.CUDAGraph()
+    with torch.cuda.graph(g):
+        fn()
+    torch.cuda.synchronize()
+    return g.replay
+
+
+def rate(nbytes, ms, peak):
+    gbs = nbytes / ms / 1e6
+    return {"ms": ms, "gbs": gbs, "frac_measured": gbs / peak, "frac_nominal": gbs / NOMINAL_HBM_GBS}
+
+
+# ------------------------------------------------------------------------------------------ cfg4
+def run_cfg4(args):
+    """Granularity sweep (BASELINE.json configs[4]): shuffle, unshuffle, re-layout A->B of a 4 GiB buffer at block
+    sizes 4 KiB .. 2 MiB, beside a device-to-device cudaMemcpy and the same kernel on an identity table."""
+    torch, C, synth_cuda, gen = _imports()
+    c = gen.CONFIGS[4]
+    nbytes = int(args.bytes or c["bytes"])
+    peak, peak_kind = hbm_peak()
+    L = synth_cuda.fill(torch.empty(nbytes // 2, dtype=torch.bfloat16, device="cuda"), c["seed"], 0)
+    back = torch.empty_like(L)
+    memcpy_ms, _ = time_gpu(torch, lambda: back.copy_(L), args.reps)
+    rows, ok = [], True
+    launches0 = C.cloak_launch_count()
+    for b in c["blocks"]:
+        pa = C.cloak_pool_create(0, nbytes, b, c["page"], c["key"])
+        pb = C.cloak_pool_create(0, nbytes, b, c["page"], c["key_b"])
+        pn = C.cloak_pool_create(0, nbytes, b, c["page"], c["key"], C.CLOAK_POOL_IDENTITY)
+        try:
+            r = {"block_bytes": b, "nblocks": nbytes // b, "pool_map_ms": C.cloak_pool_map_ms(pa)}
+            for name, fn in (("shuffle", lambda: C.cloak_shuffle(pa, L, 0, nbytes)),
+                             ("unshuffle", lambda: C.cloak_unshuffle(pa, back, 0, nbytes)),
+                             ("relayout", lambda: C.cloak_relayout(pa, pb)),
+                             ("identity_table", lambda: C.cloak_shuffle(pn, L, 0, nbytes))):
+                med, mn = time_gpu(torch, fn, args.reps)
+                r[name] = rate(2 * nbytes, med, peak)
+                r[name]["ms_min"] = mn
+            # self-consistency: the round trip and the re-laid-out pool both give the buffer back
+            back.zero_()
+            C.cloak_unshuffle(pa, back, 0, nbytes)
+            r["roundtrip_bit_exact"] = bool(torch.equal(back, L))
+            back.zero_()
+            C.cloak_unshuffle(pb, back, 0, nbytes)
+            r["relayout_bit_exact"] = bool(torch.equal(back, L))
+            ok = ok and r["roundtrip_bit_exact"] and r["relayout_bit_exact"]
+            rows.append(r)
+        finally:
+            torch.cuda.synchronize()
+            for p in (pa, pb, pn):
+                C.cloak_pool_destroy(p)
+    return {"workload": "cfg4: granularity sweep, %.2f GiB bf16 buffer, 2 MiB VMM pages" % (nbytes / 2**30),
+            "bytes": nbytes, "reps": args.reps, "hbm_peak_gbs": peak, "hbm_peak_kind": peak_kind,
+            "hbm_nominal_gbs": NOMINAL_HBM_GBS, "memcpy_d2d": rate(2 * nbytes, memcpy_ms, peak),
+            "sweep": rows, "all_bit_exact": ok, "gpu_launches": C.cloak_launch_count() - launches0,
+            "convention": "GB/s = 2 x payload bytes / time (one read + one write), as MEASURED_PEAKS.json's hbm_gbs"}
+
+
+# ------------------------------------------------------------------------------------------ cfg2
+def _load_model(torch, C, synth_cuda, gen, cfg, pools, offs, tile128, keep=None, layers=None):
+    """Generates every tensor of a model config on the GPU (tensor id = position in gen.model_tensors), applies the
+    S5 neuron/head permutation per layer (and the TILE128 conversion when asked), and shuffles it into each pool.
+    keep: optional dict name -> tensor that receives the permuted logical bytes (cfg2's shuffle timing needs them
+    resident).  Returns seconds spent."""
+    c = gen.CONFIGS[cfg]
+    tensors = gen.model_tensors(cfg)
+    off = {nm: o for (nm, _), o in zip(tensors, offs)}
+    tid = {nm: i for i, (nm, _) in enumerate(tensors)}
+    t0 = time.perf_counter()
+    lshapes = gen.layer_shapes(c["hidden"], c["inter"], c["n_q"], c["n_kv"], c["head_dim"])
+    raw = {nm: torch.empty(shp, dtype=torch.bfloat16, device="cuda") for nm, shp in lshapes}
+    prm = {nm: torch.empty(shp, dtype=torch.bfloat16, device="cuda") for nm, shp in lshapes}
+    til = {nm: torch.empty(shp, dtype=torch.bfloat16, device="cuda") for nm, shp in lshapes} if tile128 else None
+
+    def put(name, t):
+        for p in pools:
+            C.cloak_shuffle(p, t, off[name], t.numel() * 2)
+
+    for l in range(c.get("layers", 1) if layers is None else layers):
+        for nm, _ in lshapes:
+            synth_cuda.fill(raw[nm], c["seed"], tid[f"l{l}.{nm}"])
+        sh = C.cloak_block_shape(c["hidden"], c["inter"], c["n_q"], c["n_kv"], c["head_dim"], C.CLOAK_BF16, l)
+        dst = {nm: (keep[f"l{l}.{nm}"] if keep is not None else prm[nm]) for nm, _ in lshapes}
+        C.cloak_permute_mlp_heads(c["key"], sh, **raw, **{k + "_o": v for k, v in dst.items()})
+        for nm, (n, k) in lshapes:
+            src = dst[nm]
+            if tile128:
+                C.cloak_to_tile128(src, til[nm], n, k, C.CLOAK_BF16)
+                src = til[nm]
+            put(f"l{l}.{nm}", src)
+    for nm in ("embed", "lm_head"):
+        if nm in tid:
+            t = keep[nm] if keep is not None else torch.empty(tensors[tid[nm]][1], dtype=torch.bfloat16, device="cuda")
+            synth_cuda.fill(t, c["seed"], tid[nm])
+            put(nm, t)
+    torch.cuda.synchronize()
+    return time.perf_counter() - t0
+
+
+def run_cfg2(args):
+    """Full 32-layer LLaMA-8B-shaped model (BASELINE.json configs[2]): VMM mapper ms, whole-model shuffle GB/s,
+    and the batch-1 decode chain of all projection GEMVs + lm_head, cloaked vs identity table."""
+    torch, C, synth_cuda, gen = _imports()
+    c = gen.CONFIGS[2]
+    peak, peak_kind = hbm_peak()
+    tensors = gen.model_tensors(2)
+    sizes = [2 * n * k for _, (n, k) in tensors]
+    offs, total = C.cloak_arena_plan(c["key"], sizes, c["block"])
+    off = {nm: o for (nm, _), o in zip(tensors, offs)}
+    payload = sum(sizes)
+    t0 = time.perf_counter()
+    pc = C.cloak_pool_create(0, total, c["block"], c["page"], c["key"])
+    create_s = time.perf_counter() - t0
+    pn = C.cloak_pool_create(0, total, c["block"], c["page"], c["key"], C.CLOAK_POOL_IDENTITY)
+    info = C.cloak_pool_info(pc)
+    launches0 = C.cloak_launch_count()
+    try:
+        keep = {nm: torch.empty(shp, dtype=torch.bfloat16, device="cuda") for nm, shp in tensors}
+        load_s = _load_model(torch, C, synth_cuda, gen, 2, (pc, pn), offs, False, keep=keep)
+
+        # ---- S4 at model scale: all 226 tensors, one call each
+        def shuffle_all():
+            for nm, _ in tensors:
+                C.cloak_shuffle(pc, keep[nm], off[nm], keep[nm].numel() * 2)
+        sh_med, sh_min = time_gpu(torch, shuffle_all, args.reps)
+        back = torch.empty(payload // 2, dtype=torch.bfloat16, device="cuda")
+        views, at = {}, 0
+        for nm, (n, k) in tensors:
+            views[nm] = back[at:at + n * k].view(n, k)
+            at += n * k
+
+        def unshuffle_all():
+            for nm, _ in tensors:
+                C.cloak_unshuffle(pc, views[nm], off[nm], views[nm].numel() * 2)
+        un_med, un_min = time_gpu(torch, unshuffle_all, args.reps)
+        roundtrip = all(torch.equal(views[nm], keep[nm]) for nm, _ in tensors)
+        del back, views
+
+        # ---- S6 decode chain at batch 1: q,k,v <- xh; o <- xa; gate,up <- xh; down <- silu(gate)*up; lm_head <- xh
+        H, I, Q = c["hidden"], c["inter"], c["n_q"] * c["head_dim"]
+        xh = synth_cuda.fill(torch.empty(1, H, dtype=torch.bfloat16, device="cuda"), c["seed"] + 100, 0, kind=gen.KIND_NORMAL)
+        xa = synth_cuda.fill(torch.empty(1, Q, dtype=torch.bfloat16, device="cuda"), c["seed"] + 100, 1, kind=gen.KIND_NORMAL)
+        T = {nm: C.cloak_tensor(off[nm], shp[0], shp[1], C.CLOAK_BF16, C.CLOAK_ROWMAJOR) for nm, shp in tensors}
+        Y = {pool_name: {nm: torch.zeros(1, shp[0], dtype=torch.bfloat16, device="cuda") for nm, shp in tensors if nm != "embed"}
+             for pool_name in ("cloaked", "native")}
+        act = torch.empty(1, I, dtype=torch.bfloat16, device="cuda")
+
+        def chain(pool, y):
+            for l in range(c["layers"]):
+                p = f"l{l}."
+                for nm in ("q", "k", "v"):
+                    C.cloak_gemv(pool, T[p + nm], xh, y[p + nm], 1)
+                C.cloak_gemv(pool, T[p + "o"], xa, y[p + "o"], 1)
+                C.cloak_gemv(pool, T[p + "gate"], xh, y[p + "gate"], 1)
+                C.cloak_gemv(pool, T[p + "up"], xh, y[p + "up"], 1)
+                C.cloak_silu_mul(y[p + "gate"], y[p + "up"], act, I, C.CLOAK_BF16)
+                C.cloak_gemv(pool, T[p + "down"], act, y[p + "down"], 1)
+            C.cloak_gemv(pool, T["lm_head"], xh, y["lm_head"], 1)
+
+        read_bytes = payload - sizes[0]                     # every tensor but the embedding table
+        res = {}
+        for pool_name, pool in (("cloaked", pc), ("native", pn)):
+            y = Y[pool_name]
+            med, mn = time_gpu(torch, lambda: chain(pool, y), args.reps)
+            gmed, gmn = time_gpu(torch, graphed(torch, lambda: chain(pool, y)), args.reps)
+            res[pool_name] = {"stream": dict(rate(read_bytes, med, peak), ms_min=mn, tokens_per_s=1e3 / med),
+                              "graph": dict(rate(read_bytes, gmed, peak), ms_min=gmn, tokens_per_s=1e3 / gmed)}
+        identical = all(torch.equal(Y["cloaked"][nm], Y["native"][nm]) for nm in Y["cloaked"])
+        ov = {k: (res["cloaked"][k]["ms"] - res["native"][k]["ms"]) / res["native"][k]["ms"] * 100 for k in ("stream", "graph")}
+    finally:
+        torch.cuda.synchronize()
+        map_ms = C.cloak_pool_map_ms(pc)
+        C.cloak_pool_destroy(pc)
+        C.cloak_pool_destroy(pn)
+    return {"workload": "cfg2: 32-layer LLaMA-8B-shaped model, bf16, 226 tensors, 64 KiB blocks, 2 MiB VMM pages",
+            "payload_bytes": payload, "arena_bytes": total, "npages": info["npages"], "nblocks": info["nb"],
+            "reps": args.reps, "hbm_peak_gbs": peak, "hbm_peak_kind": peak_kind, "hbm_nominal_gbs": NOMINAL_HBM_GBS,
+            "pool_map_ms": map_ms, "pool_create_s": create_s, "generate_permute_load_s": load_s,
+            "shuffle": dict(rate(2 * payload, sh_med, peak), ms_min=sh_min),
+            "unshuffle": dict(rate(2 * payload, un_med, peak), ms_min=un_min), "roundtrip_bit_exact": bool(roundtrip),
+            "decode_chain": res, "decode_read_bytes": read_bytes, "decode_launches": 32 * 8 + 1,
+            "ideal_tokens_per_s_at_measured_peak": peak * 1e9 / read_bytes,
+            "cloaked_vs_native_overhead_pct": ov, "cloaked_identical_to_native": bool(identical),
+            "gpu_launches": C.cloak_launch_count() - launches0}
+
+
+# ------------------------------------------------------------------------------------------ cfg3
+def run_cfg3(args):
+    """Qwen-32B-shaped model, 64 layers, TILE128 storage (BASELINE.json configs[3]): cloaked decode GEMM of every
+    projection at batch 32 and 128 on the tcgen05 path, cloaked vs identity table.  Layers are generated on the GPU
+    one at a time; the host never holds the model."""
+    torch, C, synth_cuda, gen = _imports()
+    c = gen.CONFIGS[3]
+    layers = int(args.layers or c["layers"])
+    peak, peak_kind = hbm_peak()
+    tensors = gen.model_tensors(3)[:7 * layers]
+    sizes = [2 * n * k for _, (n, k) in tensors]
+    offs, total = C.cloak_arena_plan(c["key"], sizes, c["block"])
+    off = {nm: o for (nm, _), o in zip(tensors, offs)}
+    payload = sum(sizes)
+    t0 = time.perf_counter()
+    pc = C.cloak_pool_create(0, total, c["block"], c["page"], c["key"])
+    create_s = time.perf_counter() - t0
+    pn = C.cloak_pool_create(0, total, c["block"], c["page"], c["key"], C.CLOAK_POOL_IDENTITY)
+    info = C.cloak_pool_info(pc)
+    launches0 = C.cloak_launch_count()
+    try:
+        load_s = _load_model(torch, C, synth_cuda, gen, 3, (pc, pn), offs, True, layers=layers)
+        H, I, Q = c["hidden"], c["inter"], c["n_q"] * c["head_dim"]
+        T = {nm: C.cloak_tensor(off[nm], shp[0], shp[1], C.CLOAK_BF16, C.CLOAK_TILE128) for nm, shp in tensors}
+        lnames = [nm for nm, _ in gen.layer_shapes(H, I, c["n_q"], c["n_kv"], c["head_dim"])]
+        out = {}
+        for batch in (32, 128):
+            X = {k: synth_cuda.fill(torch.empty(batch, k, dtype=torch.bfloat16, device="cuda"), c["seed"] + 100,
+                                    2 * batch + i, kind=gen.KIND_NORMAL) for i, k in enumerate(sorted({H, I, Q}))}
+            Y = {pn_: {nm: torch.zeros(batch, dict(tensors)[f"l0.{nm}"][0], dtype=torch.bfloat16, device="cuda") for nm in lnames}
+                 for pn_ in ("cloaked", "native")}
+
+            def sweep(pool, y):
+                for l in range(layers):
+                    for nm in lnames:
+                        t = T[f"l{l}.{nm}"]
+                        C.cloak_gemm(pool, t, X[t.K], y[nm], batch)
+
+            res = {}
+            for pool_name, pool in (("cloaked", pc), ("native", pn)):
+                y = Y[pool_name]
+                med, mn = time_gpu(torch, lambda: sweep(pool, y), args.reps, warmup=2)
+                gmed, gmn = time_gpu(torch, graphed(torch, lambda: sweep(pool, y)), args.reps, warmup=2)
+                flops = 2.0 * batch * (payload / 2)
+                res[pool_name] = {"stream": dict(rate(payload, med, peak), ms_min=mn, tflops=flops / med / 1e9),
+                                  "graph": dict(rate(payload, gmed, peak), ms_min=gmn, tflops=flops / gmed / 1e9)}
+            res["identical"] = bool(all(torch.equal(Y["cloaked"][nm], Y["native"][nm]) for nm in lnames))
+            res["overhead_pct"] = {k: (res["cloaked"][k]["ms"] - res["native"][k]["ms"]) / res["native"][k]["ms"] * 100
+                                   for k in ("stream", "graph")}
+            out[f"b{batch}"] = res
+    finally:
+        torch.cuda.synchronize()
+        map_ms = C.cloak_pool_map_ms(pc)
+        C.cloak_pool_destroy(pc)
+        C.cloak_pool_destroy(pn)
+    return {"workload": "cfg3: Qwen-32B-shaped model, %d layers, bf16 TILE128, 64 KiB blocks, 2 MiB VMM pages" % layers,
+            "payload_bytes": payload, "npages": info["npages"], "nblocks": info["nb"], "reps": args.reps,
+            "hbm_peak_gbs": peak, "hbm_peak_kind": peak_kind, "hbm_nominal_gbs": NOMINAL_HBM_GBS,
+            "pool_map_ms": map_ms, "pool_create_s": create_s, "generate_permute_tile_load_s": load_s,
+            "gemm": out, "launches_per_sweep": 7 * layers, "gpu_launches": C.cloak_launch_count() - launches0}
+
+
+RUNNERS = {"cfg2": run_cfg2, "cfg3": run_cfg3, "cfg4": run_cfg4}
+
+
+def main(argv=None):
+    ap = argparse.ArgumentParser(description=__doc__.split("\n")[0])
+    ap.add_argument("workload", choices=sorted(RUNNERS))
+    ap.add_argument("--reps", type=int, default=10)
+    ap.add_argument("--bytes", type=int, default=0, help="cfg4: buffer bytes (default 4 GiB)")
+    ap.add_argument("--layers", type=int, default=0, help="cfg3: number of layers (default 64)")
+    ap.add_argument("--out", default="")
+    args = ap.parse_args(argv)
+    line = json.dumps(RUNNERS[args.workload](args))
+    print(line)
+    if args.out:
+        with open(args.out, "w") as f:
+            f.write(line + "\n")
+    return 0
+
+
+if __name__ == "__main__":
+    if ROOT not in sys.path:
+        sys.path.insert(0, ROOT)
+    sys.exit(main())
