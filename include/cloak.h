@@ -181,6 +181,30 @@ cloak_status cloak_gemv(const cloak_pool* pool, const cloak_tensor* w, const voi
                         uint32_t batch, void* stream);
 cloak_status cloak_gemm(const cloak_pool* pool, const cloak_tensor* w, const void* d_x, void* d_y,
                         uint32_t batch, void* stream);
+/* A chain of GEMVs over one pool in ONE persistent launch (SURVEY.md 8(a) S6 at cfg2: "end-to-end cloaked decode
+ * of all layers' projection GEMVs"; decode is bandwidth-bound, so the weight stream should
+ * never stop).  Op i computes Y_i = X_i W_i^T like cloak_gemv, with two additions:
+ *   - d_gate / d_act, both or neither: the op ALSO writes d_act[m, n] = silu(d_gate[m, n]) * Y_i[m, n] ([batch, N],
+ *     fp32 arithmetic on the bf16 values, rounded to bf16 exactly as cloak_silu_mul does; O9: the gated MLP's
+ *     activation, fused into the up projection's epilogue).  d_gate must be the d_y of an earlier op of this
+ *     chain with the same N and K (the usual gate projection), or a buffer complete before the call;
+ *   - after != 0 says that X_i is written by an earlier op of this chain: the op then starts only when ALL
+ *     earlier ops have completed.  Ops with after == 0 must not read what earlier ops of the chain write.
+ * The weight stream of op i+1 is already being fetched while op i finishes, dependent or not.
+ * All ops: CLOAK_BF16, CLOAK_ROWMAJOR, K % 256 == 0, N % 16 == 0, pool block_bytes >= 512, batch 1..16, outputs
+ * distinct.  h_ops is a HOST array (copied into the launch parameters; not referenced after the call returns).
+ * Chains longer than 48 ops, or mixing row sizes that need different chunk sizes, are split into several
+ * launches (stream order keeps the semantics).  Asynchronous on `stream`. */
+typedef struct {
+    cloak_tensor w;
+    const void* d_x;
+    void* d_y;
+    const void* d_gate;
+    void* d_act;
+    uint32_t after;
+} cloak_gemv_op;
+cloak_status cloak_gemv_chain(const cloak_pool* pool, const cloak_gemv_op* h_ops, uint32_t n_ops, uint32_t batch,
+                              void* stream);
 /* Selects the bf16 GEMV kernel: 0 = automatic (streaming TMA kernel when K % 256 == 0, launched with
  * programmatic dependent launch), 1 = always the one-shot split-K kernel, 2 = automatic without
  * programmatic dependent launch.  For A/B measurement; process-wide. */

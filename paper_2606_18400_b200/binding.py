@@ -26,7 +26,7 @@ SYMBOLS = ["cloak_last_error", "cloak_version", "cloak_launch_count", "cloak_key
            "cloak_pool_info", "cloak_pool_tables", "cloak_pool_dump", "cloak_pool_map_ms", "cloak_shuffle",
            "cloak_unshuffle", "cloak_relayout", "cloak_shuffle_host", "cloak_unshuffle_host",
            "cloak_set_copy_engine", "cloak_arena_plan", "cloak_permute_mlp_heads", "cloak_to_tile128",
-           "cloak_gemv", "cloak_gemm", "cloak_set_gemv_engine", "cloak_gemv_host", "cloak_silu_mul"]
+           "cloak_gemv", "cloak_gemv_chain", "cloak_gemm", "cloak_set_gemv_engine", "cloak_gemv_host", "cloak_silu_mul"]
 
 
 class CloakError(RuntimeError):
@@ -42,6 +42,11 @@ class cloak_block_shape(Structure):
 
 class cloak_tensor(Structure):
     _fields_ = [("w_offset", c_uint64), ("N", c_uint32), ("K", c_uint32), ("dt", c_int), ("layout", c_int)]
+
+
+class cloak_gemv_op(Structure):
+    _fields_ = [("w", cloak_tensor), ("d_x", c_void_p), ("d_y", c_void_p), ("d_gate", c_void_p), ("d_act", c_void_p),
+                ("after", c_uint32)]
 
 
 if not os.path.exists(LIB_PATH):
@@ -71,6 +76,7 @@ lib.cloak_arena_plan.argtypes = [c_uint64, c_uint32, POINTER(c_uint64), c_uint32
 lib.cloak_permute_mlp_heads.argtypes = [c_uint64, POINTER(cloak_block_shape)] + [_P] * 15
 lib.cloak_to_tile128.argtypes = [_P, _P, c_uint32, c_uint32, c_int, _P]
 lib.cloak_gemv.argtypes = [_P, POINTER(cloak_tensor), _P, _P, c_uint32, _P]
+lib.cloak_gemv_chain.argtypes = [_P, POINTER(cloak_gemv_op), c_uint32, c_uint32, _P]
 lib.cloak_gemm.argtypes = [_P, POINTER(cloak_tensor), _P, _P, c_uint32, _P]
 lib.cloak_gemv_host.argtypes = [_P, POINTER(cloak_tensor), _P, _P, c_uint32, _P]
 lib.cloak_silu_mul.argtypes = [_P, _P, _P, c_uint64, c_int, _P]
@@ -209,6 +215,22 @@ def cloak_to_tile128(d_src, d_dst, N, K, dt, stream=None):
 
 def cloak_gemv(pool, tensor, d_x, d_y, batch, stream=None):
     _check(lib.cloak_gemv(pool, byref(tensor), _ptr(d_x), _ptr(d_y), batch, _stream(stream)))
+
+
+def cloak_gemv_ops(ops):
+    """Marshals [(tensor, d_x, d_y, after) or (tensor, d_x, d_y, after, d_gate, d_act), ...] into a ctypes array
+    for cloak_gemv_chain (reusable across calls)."""
+    arr = (cloak_gemv_op * len(ops))()
+    for o, op in zip(arr, ops):
+        t, x, y, after = op[:4]
+        gate, act = op[4:] if len(op) == 6 else (None, None)
+        o.w, o.d_x, o.d_y, o.d_gate, o.d_act, o.after = t, _ptr(x), _ptr(y), _ptr(gate), _ptr(act), int(after)
+    return arr
+
+
+def cloak_gemv_chain(pool, ops, batch, stream=None):
+    arr = ops if isinstance(ops, ctypes.Array) else cloak_gemv_ops(ops)
+    _check(lib.cloak_gemv_chain(pool, arr, len(arr), batch, _stream(stream)))
 
 
 def cloak_gemm(pool, tensor, d_x, d_y, batch, stream=None):

@@ -84,9 +84,12 @@ cloak_status keygen_device(uint64_t key, uint64_t stream_id, uint32_t n, uint32_
                            cudaStream_t s);
 constexpr size_t WS_COUNTER_BYTES = 1u << 20;
 cloak_status pool_workspace(const cloak_pool* pool, size_t bytes);
-// gemv_stream.cu: persistent TMA-fed bf16 GEMV (K % 256 == 0).
-cloak_status gemv_stream_bf16(const cloak_pool* pool, const cloak_tensor* w, const void* d_x, void* d_y, uint32_t batch,
-                              cudaStream_t s);
+// gemv_stream.cu: persistent TMA-fed bf16 GEMV chain (K % 256 == 0).  gemv_stream_log2cb: the row-chunk size the
+// kernel would use for a tensor, or -1 if it cannot take it; gemv_stream_launch: one launch of <= 48 ops that
+// share that chunk size.
+int gemv_stream_log2cb(const cloak_pool* pool, const cloak_tensor* w);
+cloak_status gemv_stream_launch(const cloak_pool* pool, const cloak_gemv_op* ops, uint32_t n, int log2cb, uint32_t batch,
+                                cudaStream_t s);
 // Host-side Philox keygen used only by cloak_arena_plan (T is tiny; no device work wanted there).
 void keygen_host(uint64_t key, uint64_t stream_id, uint32_t n, std::vector<uint32_t>& perm);
 

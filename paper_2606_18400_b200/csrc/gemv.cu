@@ -270,8 +270,19 @@ static cloak_status gemv_device(const cloak_pool* pool, const cloak_tensor* w, c
     a.y = d_y;
     a.batch = batch;
     a.zero = 0;
-    if (w->dt == CLOAK_BF16 && w->K % 256 == 0 && pool->block >= 512 && !g_force_oneshot)
-        return gemv_stream_bf16(pool, w, d_x, d_y, batch, s);
+    if (!g_force_oneshot) {
+        const int log2cb = gemv_stream_log2cb(pool, w);
+        if (log2cb >= 9) {
+            cloak_gemv_op op;
+            op.w = *w;
+            op.d_x = d_x;
+            op.d_y = d_y;
+            op.d_gate = nullptr;
+            op.d_act = nullptr;
+            op.after = 0;
+            return gemv_stream_launch(pool, &op, 1, log2cb, batch, s);
+        }
+    }
     if (w->dt == CLOAK_BF16) {
         const uint32_t tiles = w->N / GV_ROWS;
         const uint32_t S = (w->K + GV_KCTA - 1) / GV_KCTA;
@@ -337,6 +348,39 @@ extern "C" cloak_status cloak_gemv(const cloak_pool* pool, const cloak_tensor* w
     if (st != CLOAK_OK) return st;
     DeviceGuard g(pool->device);
     return gemv_device(pool, w, d_x, d_y, batch, (cudaStream_t)stream);
+}
+
+extern "C" cloak_status cloak_gemv_chain(const cloak_pool* pool, const cloak_gemv_op* h_ops, uint32_t n_ops, uint32_t batch,
+                                         void* stream) {
+    if (!h_ops || n_ops == 0) return fail(CLOAK_ERR_INVALID, "gemv_chain: no ops");
+    std::vector<int> cb(n_ops);
+    for (uint32_t i = 0; i < n_ops; ++i) {
+        cloak_status st = gemv_check(pool, &h_ops[i].w, h_ops[i].d_x, h_ops[i].d_y, batch, "gemv_chain");
+        if (st != CLOAK_OK) return st;
+        if ((h_ops[i].d_gate == nullptr) != (h_ops[i].d_act == nullptr))
+            return fail(CLOAK_ERR_INVALID, "gemv_chain: op %u: d_gate and d_act go together", i);
+        if (h_ops[i].d_gate)                       // written by an earlier op?  then by one of the same shape
+            for (uint32_t k = 0; k < i; ++k)
+                if (h_ops[k].d_y == h_ops[i].d_gate && (h_ops[k].w.N != h_ops[i].w.N || h_ops[k].w.K != h_ops[i].w.K))
+                    return fail(CLOAK_ERR_INVALID, "gemv_chain: op %u: d_gate is the output of op %u, which has another shape", i, k);
+        cb[i] = gemv_stream_log2cb(pool, &h_ops[i].w);
+        if (cb[i] < 9) return fail(CLOAK_ERR_UNSUPPORTED, "gemv_chain: op %u needs bf16 ROWMAJOR, K %% 256 == 0, block >= 512", i);
+    }
+    DeviceGuard g(pool->device);
+    // consecutive ops with one chunk size, at most 48 at a time and within the row-tile counters, share a launch
+    uint32_t i = 0;
+    while (i < n_ops) {
+        uint32_t n = 1;
+        uint64_t tiles = h_ops[i].w.N / 8;
+        while (i + n < n_ops && n < 48 && cb[i + n] == cb[i] && tiles + h_ops[i + n].w.N / 8 <= 200000) {
+            tiles += h_ops[i + n].w.N / 8;
+            ++n;
+        }
+        cloak_status st = gemv_stream_launch(pool, h_ops + i, n, cb[i], batch, (cudaStream_t)stream);
+        if (st != CLOAK_OK) return st;
+        i += n;
+    }
+    return CLOAK_OK;
 }
 
 extern "C" cloak_status cloak_gemv_host(const cloak_pool* pool, const cloak_tensor* w, const void* h_x, void* h_y,

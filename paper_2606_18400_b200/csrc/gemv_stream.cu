@@ -1,10 +1,10 @@
-// S6 cloak_gemv, bf16, K % 256 == 0: the streaming (persistent, TMA-fed) kernel.
+// S6 cloak_gemv / cloak_gemv_chain, bf16, K % 256 == 0: the streaming (persistent, TMA-fed) kernel.
 //
 // Same contraction and table translation as gemv.cu (north_star (c)), organised for the
 // HBM roofline.  Measured on B200: a pure stream of 16 x 2 KiB row pieces per stage tops out
 // at 5.5 TB/s, 8 x 4 KiB pieces at 6.4 TB/s, so a unit of work is (8 weight rows) x (CB = 4 KiB of each row):
-//   * one persistent CTA per SM; units are numbered tile-major (u = tile * kch + chunk) and cut into equal
-//     contiguous ranges, one per CTA (stream-K): every SM moves the same bytes, no wave tail;
+//   * one persistent CTA per SM; an op's units are numbered tile-major (u = tile * kch + chunk) and cut into
+//     equal contiguous ranges, one per CTA (stream-K): every SM moves the same bytes, no wave tail;
 //   * warp 0 produces: 8 lanes each translate one row piece through the block table and issue one
 //     cp.async.bulk (TMA 1-D) into a shared-memory ring (6 stages of 32 KiB), completion on an mbarrier;
 //   * warps 1-8 consume: each owns one eighth of the k-range of a chunk.  The weights are the B operand of
@@ -14,13 +14,21 @@
 //     X is loaded by the same rule: both operands are plain 16-byte loads, no transposes;
 //   * inside its range a CTA walks groups of TG = 8 row tiles chunk-major (all tiles of the group for chunk 0,
 //     then chunk 1, ...), so a warp's X fragments are fetched once per (group, chunk) and reused for 64 weight
-//     rows: X traffic from L2 is batch/64 of the weight traffic instead of batch/16 (at batch 16 the old
-//     tile-major walk spent as many L2 bytes on X as on W);
+//     rows: X traffic from L2 is batch/64 of the weight traffic;
 //   * accumulators (one m16n8 tile per row tile of the group, two interleaved to halve the dependency chain)
 //     stay in registers until the group is done, are reduced over the 8 warps in shared memory, and stored.
-//     A row tile cut by a range boundary writes fp32 partials and the last contributor to arrive sums them in
-//     contributor order: deterministic, and bit-identical between a cloaked and an identity-table pool, which
-//     differ only in addresses.
+//   * a row tile cut by a range boundary is finished by its OWNER, the CTA that holds the tile's first unit (for
+//     which it is the last tile of the range).  Every other contributor meets the tile first, publishes its fp32
+//     partial early (release), and moves on; the owner, done with everything else, waits for those arrivals
+//     (acquire; all CTAs are co-resident, one per SM) and adds the partials in contributor order:
+//     deterministic, and bit-identical between a cloaked and an identity-table pool, which differ only in
+//     addresses.  No fence, atomic round trip or reduction sits at the end of the other CTAs.
+//   * a launch executes a CHAIN of ops (cloak_gemv_chain; cloak_gemv is a chain of one).  The producer warp
+//     runs straight through the chain -- weights do not depend on activations -- so HBM stays busy across op
+//     boundaries; only the consumers of an op marked `after` wait, on a grid-wide arrival counter, for all CTAs
+//     to have finished the earlier ops (its X is their Y).  An op may also emit silu(G) * Y next to Y in its
+//     epilogue (the gated MLP's activation, O9), where G is the output of an earlier op of the same shape -- the
+//     same CTA wrote those very elements, so no wait is needed -- and gate/up -> down costs no separate pass.
 //   * programmatic dependent launch: the grid may start while its stream predecessor drains; the producer
 //     streams W (immutable during decode) ahead of griddepcontrol.wait, everything else waits.
 #include <cuda_bf16.h>
@@ -29,23 +37,36 @@
 
 namespace cloak {
 
-struct GemvStreamArgs {
+struct ChainOp {             // 72 bytes of kernel parameter space per op
+    uint64_t w_offset;
+    const uint16_t* x;       // [batch, K]
+    __nv_bfloat16* y;        // [batch, N]
+    const uint16_t* gate;    // NULL, or [batch, N] written by an earlier op with the same (N, K): then also
+    uint16_t* act;           //   act[m, n] = silu(gate[m, n]) * y[m, n]   (O9, the gated MLP's activation)
+    uint32_t N, K;
+    uint32_t kch;            // chunks per row = K*2 / CB
+    uint32_t units;          // tiles * kch
+    uint32_t per;            // units per CTA
+    uint32_t ctas;           // CTAs that own units of this op (indices 0 .. ctas-1)
+    uint32_t tile_base;      // index of this op's first row-tile counter
+    uint32_t flags;          // OP_AFTER | OP_SIGNAL
+};
+enum { OP_AFTER = 1,         // consumers wait until every CTA has finished all earlier ops of the chain
+       OP_SIGNAL = 2 };      // the next op is OP_AFTER: every CTA reports here when it is done with this op
+constexpr int GS_MAX_OPS = 48;              // 48 x 72 B + header < 4 KiB of kernel parameters
+
+struct ChainArgs {
     const char* pool;
     const uint32_t* T;
+    float* part;             // [op][cta][batch * 8]: partial of the cut row tile a CTA meets first in that op
+    uint32_t* counters;      // [tile_base + tile]: arrivals of the non-owning contributors; owner resets to 0
+    uint32_t* opsync;        // [op][2]: arrivals / departures of the grid-wide wait; last departure resets both
     uint32_t log2b;
-    uint64_t w_offset;
-    uint32_t N, K;
-    const uint16_t* x;
-    __nv_bfloat16* y;
     uint32_t batch;
-    uint32_t kch;        // chunks per row = K*2 / CB
-    uint32_t units;      // tiles * kch
-    uint32_t per;        // units per CTA
-    uint32_t maxc;       // max contributors per tile
-    float* part;         // [tile][maxc][batch][8]
-    uint32_t* counters;  // [tile], zero between launches
-    uint32_t early;      // 1: W is unchanged since before the preceding kernel, so the producer may stream it
-                         //    ahead of griddepcontrol.wait (programmatic dependent launch)
+    uint32_t nops;
+    uint32_t early;          // 1: W is unchanged since before the preceding kernel, so the producer may stream it
+                             //    ahead of griddepcontrol.wait (programmatic dependent launch)
+    ChainOp ops[GS_MAX_OPS];
 };
 
 constexpr int GS_CONSUMERS = 8;                       // consumer warps
@@ -56,8 +77,8 @@ constexpr int GS_PAD = 64;                            // bytes of padding per st
 // 8 tiles x 2 accumulators measured best for both batch ranges: 16 x 1 halves the X traffic at batch 16 but its
 // 16-deep dependent MMA chain costs more than that saves; staggering the group boundaries over the CTAs (so the
 // SMs do not all wait for X at once) adds a group per CTA and was slower too.
-constexpr int gs_tg(int nt) { return 8; }
-constexpr int gs_nacc(int nt) { return 2; }
+constexpr int GS_TG = 8;
+constexpr int GS_NACC = 2;
 constexpr int GS_TGR = 4;                             // row tiles reduced across warps per shared-memory pass
 constexpr int GS_MAX_STAGES = 12;
 constexpr uint32_t gs_stages(int log2cb) {            // ~192 KiB of weights in flight per SM
@@ -75,6 +96,21 @@ __device__ __forceinline__ uint4 lds128(uint32_t addr) {
     asm volatile("ld.shared.v4.u32 {%0,%1,%2,%3}, [%4];" : "=r"(r.x), "=r"(r.y), "=r"(r.z), "=r"(r.w) : "r"(addr));
     return r;
 }
+// Activations may have been written earlier in this same kernel by other SMs (an OP_AFTER op reads its
+// predecessors' Y): a coherent load, ordered behind the acquire that ended the grid-wide wait -- never ld.global.nc.
+__device__ __forceinline__ uint4 ldg_coherent(const void* p) {
+    uint4 r;
+    asm volatile("ld.global.v4.u32 {%0,%1,%2,%3}, [%4];" : "=r"(r.x), "=r"(r.y), "=r"(r.z), "=r"(r.w) : "l"(p) : "memory");
+    return r;
+}
+__device__ __forceinline__ uint32_t ld_acquire(const uint32_t* p) {
+    uint32_t v;
+    asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
+    return v;
+}
+__device__ __forceinline__ void red_release_add(uint32_t* p, uint32_t v) {
+    asm volatile("red.release.gpu.global.add.u32 [%0], %1;" :: "l"(p), "r"(v) : "memory");
+}
 // Programmatic dependent launch (PDL): this grid may start while its stream predecessor is still draining.
 // grid_dep_wait returns once the predecessor has completed and its writes are visible; grid_dep_launch lets the
 // stream successor start.  Every kernel here triggers only AFTER its own wait, so whatever a successor does ahead
@@ -83,19 +119,31 @@ __device__ __forceinline__ void grid_dep_wait() { asm volatile("griddepcontrol.w
 __device__ __forceinline__ void grid_dep_launch() { asm volatile("griddepcontrol.launch_dependents;" ::: "memory"); }
 __device__ __forceinline__ void consumer_bar() { asm volatile("bar.sync 1, %0;" :: "n"(GS_CONSUMERS * 32) : "memory"); }
 
+// silu(g) * u for bf16 inputs, fp32 arithmetic, round to nearest even: bit for bit cloak_silu_mul's result.
+__device__ __forceinline__ uint16_t silu_mul_bf16(uint16_t g, __nv_bfloat16 u) {
+    const float z = __uint_as_float((uint32_t)g << 16), w = __bfloat162float(u);
+    uint32_t b = __float_as_uint(z / (1.0f + __expf(-z)) * w);
+    b += 0x7FFFu + ((b >> 16) & 1u);
+    return (uint16_t)(b >> 16);
+}
+__device__ __forceinline__ uint16_t ld_coherent_u16(const uint16_t* p) {
+    uint16_t v;
+    asm volatile("ld.global.u16 %0, [%1];" : "=h"(v) : "l"(p) : "memory");
+    return v;
+}
+
 // LOG2CB: log2 of the chunk bytes per row (9..12).  NT: 1 = batch <= 8 (upper half of the MMA's M is zero), 2 = batch <= 16.
 template <int LOG2CB, int NT>
-__global__ void __launch_bounds__(GS_THREADS, 1) gemv_stream_kernel(GemvStreamArgs a) {
+__global__ void __launch_bounds__(GS_THREADS, 1) gemv_chain_kernel(const __grid_constant__ ChainArgs a) {
     constexpr uint32_t CB = 1u << LOG2CB;
     constexpr uint32_t RS = CB + GS_PAD;                       // staged row stride
     constexpr uint32_t STAGE = GS_ROWS * RS;
     constexpr uint32_t NST = gs_stages(LOG2CB);
-    constexpr int GS_TG = gs_tg(NT), NACC = gs_nacc(NT);
     constexpr int KS = CB / (GS_CONSUMERS * 64);               // 64-byte steps (one 16-byte vector per lane) per warp per unit
     extern __shared__ __align__(128) unsigned char smem[];
     __shared__ __align__(8) uint64_t full[NST], empty[NST];
     __shared__ float red[GS_CONSUMERS][GS_TGR][NT * 64];      // [warp][tile][batch m][row r]
-    __shared__ uint32_t last_flag[2];
+    __shared__ float own[NT * 64];                             // this CTA's own sums of the cut tile it owns
 
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     if (threadIdx.x == 0) {
@@ -107,37 +155,40 @@ __global__ void __launch_bounds__(GS_THREADS, 1) gemv_stream_kernel(GemvStreamAr
         fence_barrier_init();
     }
     __syncthreads();
-
-    const uint32_t ubeg = blockIdx.x * a.per;
-    const uint32_t uend = min(ubeg + a.per, a.units);
-    if (ubeg >= uend) return;
     const uint32_t smem_base = smem_u32(smem);
-    const uint32_t tile_lo = ubeg / a.kch, tile_hi = (uend - 1) / a.kch;
 
     if (warp == 0) {
-        // ------------------------------------------------------------ producer
+        // ------------------------------------------------------------ producer: straight through the chain
         // The table is immutable after cloak_pool_create; the weights may have been written by the preceding
         // kernel (a shuffle / re-layout) unless the host says otherwise.
         if (!a.early) grid_dep_wait();
         uint32_t s = 0, ph = 0;
         bool wrapped = false;
-        for (uint32_t g0 = tile_lo; g0 <= tile_hi; g0 += GS_TG) {
-            const uint32_t g1 = min(g0 + GS_TG - 1, tile_hi);
-            for (uint32_t c = 0; c < a.kch; ++c) {
-                for (uint32_t tile = g0; tile <= g1; ++tile) {
-                    const uint32_t u = tile * a.kch + c;
-                    if (u < ubeg || u >= uend) continue;
-                    if (wrapped) mbar_wait(smem_u32(&empty[s]), ph ^ 1);
-                    const uint32_t bar = smem_u32(&full[s]);
-                    if (lane == 0) mbar_expect_tx(bar, GS_ROWS * CB);
-                    __syncwarp();
-                    if (lane < GS_ROWS) {
-                        const uint64_t off = a.w_offset + ((uint64_t)(tile * GS_ROWS + lane) * a.K) * 2 + (uint64_t)c * CB;
-                        const uint32_t slot = __ldg(a.T + (off >> a.log2b));
-                        const char* src = a.pool + ((uint64_t)slot << a.log2b) + (off & ((1ull << a.log2b) - 1));
-                        bulk_g2s(smem_base + s * STAGE + lane * RS, src, CB, bar);
+        for (uint32_t j = 0; j < a.nops; ++j) {
+            const ChainOp& op = a.ops[j];
+            const uint32_t kch = op.kch;
+            const uint32_t ubeg = blockIdx.x * op.per, uend = min(ubeg + op.per, op.units);
+            if (ubeg >= uend) continue;
+            const uint32_t tile_lo = ubeg / kch, tile_hi = (uend - 1) / kch;
+            const uint64_t row_bytes = (uint64_t)op.K * 2;
+            for (uint32_t g0 = tile_lo; g0 <= tile_hi; g0 += GS_TG) {
+                const uint32_t g1 = min(g0 + GS_TG - 1, tile_hi);
+                for (uint32_t c = 0; c < kch; ++c) {
+                    for (uint32_t tile = g0; tile <= g1; ++tile) {
+                        const uint32_t u = tile * kch + c;
+                        if (u < ubeg || u >= uend) continue;
+                        if (wrapped) mbar_wait(smem_u32(&empty[s]), ph ^ 1);
+                        const uint32_t bar = smem_u32(&full[s]);
+                        if (lane == 0) mbar_expect_tx(bar, GS_ROWS * CB);
+                        __syncwarp();
+                        if (lane < GS_ROWS) {
+                            const uint64_t off = op.w_offset + (uint64_t)(tile * GS_ROWS + lane) * row_bytes + (uint64_t)c * CB;
+                            const uint32_t slot = __ldg(a.T + (off >> a.log2b));
+                            const char* src = a.pool + ((uint64_t)slot << a.log2b) + (off & ((1ull << a.log2b) - 1));
+                            bulk_g2s(smem_base + s * STAGE + lane * RS, src, CB, bar);
+                        }
+                        if (++s == NST) { s = 0; ph ^= 1; wrapped = true; }
                     }
-                    if (++s == NST) { s = 0; ph ^= 1; wrapped = true; }
                 }
             }
         }
@@ -150,128 +201,155 @@ __global__ void __launch_bounds__(GS_THREADS, 1) gemv_stream_kernel(GemvStreamAr
     const uint32_t ctid = threadIdx.x - 32;                        // 0..255 among consumers
     const bool xv0 = (uint32_t)g < a.batch, xv1 = (uint32_t)(g + 8) < a.batch;
     const uint32_t lane_off = cw * (CB / GS_CONSUMERS) + t * 16;   // byte offset of this lane inside a row chunk
-    const uint16_t* x0 = a.x + (size_t)g * a.K + lane_off / 2;
-    const uint16_t* x1 = a.x + (size_t)(g + 8) * a.K + lane_off / 2;
     const uint32_t nout = a.batch * GS_ROWS;
 
-    // X, Y, the split-K partials and counters all belong to stream order: nothing below touches them before the
-    // predecessor has completed.  Meanwhile the producer is already filling the ring.
+    // X, Y, partials and counters all belong to stream order: nothing below touches them before the predecessor
+    // has completed.  Meanwhile the producer is already filling the ring.
     grid_dep_wait();
     if (ctid == 0) grid_dep_launch();
 
-    auto is_cut = [&](uint32_t tile) {       // does a range boundary cut this row tile?
-        return (tile == tile_lo && ubeg > tile * a.kch) || (tile == tile_hi && uend < (tile + 1) * a.kch);
-    };
-
     uint32_t s = 0, ph = 0;
-    for (uint32_t g0 = tile_lo; g0 <= tile_hi; g0 += GS_TG) {
-        const uint32_t g1 = min(g0 + GS_TG - 1, tile_hi);
-        float acc[GS_TG][NACC][4];
-#pragma unroll
-        for (int j = 0; j < GS_TG; ++j)
-#pragma unroll
-            for (int n = 0; n < NACC; ++n)
-#pragma unroll
-                for (int i = 0; i < 4; ++i) acc[j][n][i] = 0.f;
+    for (uint32_t j = 0; j < a.nops; ++j) {
+        const ChainOp& op = a.ops[j];
+        const uint32_t kch = op.kch, per = op.per;
+        const uint32_t ubeg = blockIdx.x * per, uend = min(ubeg + per, op.units);
+        const bool have = ubeg < uend;
 
-        for (uint32_t c = 0; c < a.kch; ++c) {
-            // this warp's X fragments for chunk c: fetched once, reused for every row tile of the group
-            uint4 xa[KS], xb[KS];
-            const uint32_t xk = c * (CB / 2);
-            const uint4 z = make_uint4(0, 0, 0, 0);
-#pragma unroll
-            for (int ks = 0; ks < KS; ++ks) {
-                xa[ks] = xv0 ? __ldg(reinterpret_cast<const uint4*>(x0 + xk + ks * 32)) : z;
-                xb[ks] = (NT == 2 && xv1) ? __ldg(reinterpret_cast<const uint4*>(x1 + xk + ks * 32)) : z;
-            }
-#pragma unroll
-            for (int j = 0; j < GS_TG; ++j) {
-                const uint32_t tile = g0 + j, u = tile * a.kch + c;
-                if (tile > g1 || u < ubeg || u >= uend) continue;
-                mbar_wait(smem_u32(&full[s]), ph);
-                const uint32_t base = smem_base + s * STAGE + g * RS + lane_off;
-#pragma unroll
-                for (int ks = 0; ks < KS; ++ks) {
-                    const uint4 w = lds128(base + ks * 64);
-                    mma_16816(acc[j][0], xa[ks].x, xb[ks].x, xa[ks].y, xb[ks].y, w.x, w.y);
-                    mma_16816(acc[j][NACC - 1], xa[ks].z, xb[ks].z, xa[ks].w, xb[ks].w, w.z, w.w);
+        if (have && (op.flags & OP_AFTER) && j > 0) {
+            // grid-wide wait: every CTA has reported at op j-1, i.e. has finished all ops before this one
+            uint32_t* sync = a.opsync + 2 * (j - 1);
+            if (ctid == 0) {
+                while (ld_acquire(sync) != gridDim.x) __nanosleep(32);
+                if (atomicAdd(sync + 1, 1u) == op.ctas - 1) {      // last waiter to leave: reset for the next launch
+                    sync[0] = 0;
+                    sync[1] = 0;
                 }
-                __syncwarp();
-                if (lane == 0) mbar_arrive(smem_u32(&empty[s]));
-                if (++s == NST) { s = 0; ph ^= 1; }
             }
+            consumer_bar();
         }
 
-        // ---- the group is done: reduce over the 8 warps (each summed its own k-slice), GS_TGR row tiles per pass
+        if (have) {
+            const uint32_t tile_lo = ubeg / kch, tile_hi = (uend - 1) / kch;
+            // A cut tile at the head of the range is owned by an earlier CTA (publish our partial); one at the tail
+            // is ours to finish, unless the range lies inside a single tile that started before us.
+            const bool cut_head = ubeg > tile_lo * kch;
+            const bool cut_tail = uend < (tile_hi + 1) * kch && !(tile_hi == tile_lo && cut_head);
+            const uint16_t* x0 = op.x + (size_t)g * op.K + lane_off / 2;
+            const uint16_t* x1 = op.x + (size_t)(g + 8) * op.K + lane_off / 2;
+            float* mypart = a.part + ((size_t)j * gridDim.x + blockIdx.x) * nout;
+            // Every Y element is stored exactly once, by the CTA that owns its row tile.  The gate op had the same
+            // (N, K), hence the same split: gate[idx] was stored by this CTA, before consumer barriers passed since.
+            auto store_y = [&](size_t idx, float sum) {
+                const __nv_bfloat16 v = __float2bfloat16_rn(sum);
+                op.y[idx] = v;
+                if (op.gate) op.act[idx] = silu_mul_bf16(ld_coherent_u16(op.gate + idx), v);
+            };
+
+            for (uint32_t g0 = tile_lo; g0 <= tile_hi; g0 += GS_TG) {
+                const uint32_t g1 = min(g0 + GS_TG - 1, tile_hi);
+                float acc[GS_TG][GS_NACC][4];
 #pragma unroll
-        for (int sb = 0; sb < GS_TG / GS_TGR; ++sb) {
-            const uint32_t tb = g0 + sb * GS_TGR;
-            if (tb <= g1) {
+                for (int q = 0; q < GS_TG; ++q)
 #pragma unroll
-                for (int jj = 0; jj < GS_TGR; ++jj) {
-                    const int j = sb * GS_TGR + jj;
-                    float* r = red[cw][jj];
-                    float v[4];
+                    for (int n = 0; n < GS_NACC; ++n)
 #pragma unroll
-                    for (int i = 0; i < 4; ++i) v[i] = NACC == 2 ? acc[j][0][i] + acc[j][NACC - 1][i] : acc[j][0][i];
-                    r[g * 8 + 2 * t] = v[0];
-                    r[g * 8 + 2 * t + 1] = v[1];
-                    if (NT == 2) {
-                        r[(g + 8) * 8 + 2 * t] = v[2];
-                        r[(g + 8) * 8 + 2 * t + 1] = v[3];
+                        for (int i = 0; i < 4; ++i) acc[q][n][i] = 0.f;
+
+                for (uint32_t c = 0; c < kch; ++c) {
+                    // this warp's X fragments for chunk c: fetched once, reused for every row tile of the group
+                    uint4 xa[KS], xb[KS];
+                    const uint32_t xk = c * (CB / 2);
+                    const uint4 z = make_uint4(0, 0, 0, 0);
+#pragma unroll
+                    for (int ks = 0; ks < KS; ++ks) {
+                        xa[ks] = xv0 ? ldg_coherent(x0 + xk + ks * 32) : z;
+                        xb[ks] = (NT == 2 && xv1) ? ldg_coherent(x1 + xk + ks * 32) : z;
                     }
+#pragma unroll
+                    for (int q = 0; q < GS_TG; ++q) {
+                        const uint32_t tile = g0 + q, u = tile * kch + c;
+                        if (tile > g1 || u < ubeg || u >= uend) continue;
+                        mbar_wait(smem_u32(&full[s]), ph);
+                        const uint32_t base = smem_base + s * STAGE + g * RS + lane_off;
+#pragma unroll
+                        for (int ks = 0; ks < KS; ++ks) {
+                            const uint4 w = lds128(base + ks * 64);
+                            mma_16816(acc[q][0], xa[ks].x, xb[ks].x, xa[ks].y, xb[ks].y, w.x, w.y);
+                            mma_16816(acc[q][GS_NACC - 1], xa[ks].z, xb[ks].z, xa[ks].w, xb[ks].w, w.z, w.w);
+                        }
+                        __syncwarp();
+                        if (lane == 0) mbar_arrive(smem_u32(&empty[s]));
+                        if (++s == NST) { s = 0; ph ^= 1; }
+                    }
+                }
+
+                // ---- the group is done: reduce over the 8 warps (each summed its own k-slice), GS_TGR row tiles per pass
+#pragma unroll
+                for (int sb = 0; sb < GS_TG / GS_TGR; ++sb) {
+                    const uint32_t tb = g0 + sb * GS_TGR;
+                    if (tb <= g1) {
+#pragma unroll
+                        for (int jj = 0; jj < GS_TGR; ++jj) {
+                            const int q = sb * GS_TGR + jj;
+                            float* r = red[cw][jj];
+                            float v[4];
+#pragma unroll
+                            for (int i = 0; i < 4; ++i) v[i] = GS_NACC == 2 ? acc[q][0][i] + acc[q][GS_NACC - 1][i] : acc[q][0][i];
+                            r[g * 8 + 2 * t] = v[0];
+                            r[g * 8 + 2 * t + 1] = v[1];
+                            if (NT == 2) {
+                                r[(g + 8) * 8 + 2 * t] = v[2];
+                                r[(g + 8) * 8 + 2 * t + 1] = v[3];
+                            }
+                        }
+                        consumer_bar();
+                        for (uint32_t o = ctid; o < GS_TGR * NT * 64; o += GS_CONSUMERS * 32) {
+                            const uint32_t jj = o / (NT * 64), rem = o % (NT * 64), m = rem / 8, r = rem % 8;
+                            const uint32_t tile = tb + jj;
+                            if (tile > g1 || m >= a.batch) continue;
+                            float sum = red[0][jj][rem];
+#pragma unroll
+                            for (int w = 1; w < GS_CONSUMERS; ++w) sum += red[w][jj][rem];
+                            if (tile == tile_lo && cut_head) __stcg(mypart + m * GS_ROWS + r, sum);
+                            else if (tile == tile_hi && cut_tail) own[rem] = sum;
+                            else store_y((size_t)m * op.N + tile * GS_ROWS + r, sum);
+                        }
+                        if (cut_head && tb == tile_lo) {
+                            // publish the head partial now, early in the range: the tile's owner needs it only at its end
+                            __threadfence();
+                            consumer_bar();
+                            if (ctid == 0) red_release_add(a.counters + op.tile_base + tile_lo, 1u);
+                        } else {
+                            consumer_bar();      // red[] is reused by the next pass
+                        }
+                    }
+                }
+            }
+
+            if (cut_tail) {
+                // owner of the tail tile: wait for the other contributors (CTAs after this one), add in CTA order
+                const uint32_t nc = (tile_hi * kch + kch - 1) / per - blockIdx.x;
+                uint32_t* cnt = a.counters + op.tile_base + tile_hi;
+                if (ctid == 0) {
+                    while (ld_acquire(cnt) != nc) __nanosleep(32);
+                    *cnt = 0;                                   // self-reset for the next launch
                 }
                 consumer_bar();
-                for (uint32_t o = ctid; o < GS_TGR * NT * 64; o += GS_CONSUMERS * 32) {
-                    const uint32_t jj = o / (NT * 64), rem = o % (NT * 64), m = rem / 8, r = rem % 8;
-                    const uint32_t tile = tb + jj;
-                    if (tile > g1 || m >= a.batch) continue;
-                    float sum = red[0][jj][rem];
-#pragma unroll
-                    for (int w = 1; w < GS_CONSUMERS; ++w) sum += red[w][jj][rem];
-                    if (!is_cut(tile)) {
-                        a.y[(size_t)m * a.N + tile * GS_ROWS + r] = __float2bfloat16_rn(sum);
-                    } else {
-                        const uint32_t me = blockIdx.x - (tile * a.kch) / a.per;
-                        __stcg(a.part + ((size_t)tile * a.maxc + me) * nout + m * GS_ROWS + r, sum);
-                    }
+                for (uint32_t i = ctid; i < nout; i += GS_CONSUMERS * 32) {
+                    float sum = own[i];
+                    for (uint32_t q = 1; q <= nc; ++q) sum += __ldcg(mypart + (size_t)q * nout + i);
+                    store_y((size_t)(i / GS_ROWS) * op.N + tile_hi * GS_ROWS + (i % GS_ROWS), sum);
                 }
-                consumer_bar();      // red[] is reused by the next pass
+                consumer_bar();                                  // own[] is reused by the next op
             }
         }
-    }
 
-    // ---- row tiles cut by a range boundary (at most the first and the last of the range): their partials were
-    // written above; publish them once, at the end, and let the last contributor to arrive sum them in order.
-    const bool cut_lo = is_cut(tile_lo), cut_hi = tile_hi != tile_lo && is_cut(tile_hi);
-    if (cut_lo || cut_hi) {
-        __threadfence();
-        consumer_bar();
-        if (ctid < 2) {
-            const uint32_t tile = ctid == 0 ? tile_lo : tile_hi;
-            uint32_t flag = 0;
-            if (ctid == 0 ? cut_lo : cut_hi) {
-                const uint32_t ncontrib = (tile * a.kch + a.kch - 1) / a.per - (tile * a.kch) / a.per + 1;
-                const uint32_t old = atomicAdd(a.counters + tile, 1u);
-                if (old == ncontrib - 1) {
-                    a.counters[tile] = 0;               // self-reset for the next launch
-                    flag = ncontrib;
-                }
-            }
-            last_flag[ctid] = flag;
-        }
-        consumer_bar();
-#pragma unroll
-        for (int e = 0; e < 2; ++e) {
-            const uint32_t nc = last_flag[e];
-            if (nc == 0) continue;
-            __threadfence();
-            const uint32_t tile = e == 0 ? tile_lo : tile_hi;
-            const float* base = a.part + (size_t)tile * a.maxc * nout;
-            for (uint32_t i = ctid; i < nout; i += GS_CONSUMERS * 32) {
-                float sum = 0.f;
-                for (uint32_t q = 0; q < nc; ++q) sum += __ldcg(base + (size_t)q * nout + i);
-                a.y[(size_t)(i / GS_ROWS) * a.N + tile * GS_ROWS + (i % GS_ROWS)] = __float2bfloat16_rn(sum);
+        if (op.flags & OP_SIGNAL) {
+            // report: this CTA is done with op j and everything before it (its Y stores are ordered by the barrier)
+            consumer_bar();
+            if (ctid == 0) {
+                __threadfence();
+                red_release_add(a.opsync + 2 * j, 1u);
             }
         }
     }
@@ -279,12 +357,15 @@ __global__ void __launch_bounds__(GS_THREADS, 1) gemv_stream_kernel(GemvStreamAr
 
 bool g_gemv_pdl = true;      // A/B switch (cloak_set_gemv_engine(2) turns PDL off)
 
+// Counter words [0, GS_TILE_COUNTERS) of the pool's scratch are row-tile arrival counters, the rest op barriers.
+constexpr uint32_t GS_TILE_COUNTERS = (uint32_t)(WS_COUNTER_BYTES / 4) - 4 * GS_MAX_OPS;
+
 template <int LOG2CB, int NT>
-static cloak_status launch(const GemvStreamArgs& a, int ctas, cudaStream_t s) {
+static cloak_status launch(const ChainArgs& a, int ctas, cudaStream_t s) {
     constexpr size_t smem = (size_t)gs_stages(LOG2CB) * GS_ROWS * ((1u << LOG2CB) + GS_PAD);
     static bool attr_set = false;
     if (!attr_set) {
-        CLOAK_CUDA(cudaFuncSetAttribute(gemv_stream_kernel<LOG2CB, NT>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        CLOAK_CUDA(cudaFuncSetAttribute(gemv_chain_kernel<LOG2CB, NT>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
         attr_set = true;
     }
     cudaLaunchConfig_t cfg = {};
@@ -297,43 +378,64 @@ static cloak_status launch(const GemvStreamArgs& a, int ctas, cudaStream_t s) {
     at[0].val.programmaticStreamSerializationAllowed = 1;
     cfg.attrs = at;
     cfg.numAttrs = g_gemv_pdl ? 1 : 0;
-    CLOAK_CUDA(cudaLaunchKernelEx(&cfg, gemv_stream_kernel<LOG2CB, NT>, a));
+    CLOAK_CUDA(cudaLaunchKernelEx(&cfg, gemv_chain_kernel<LOG2CB, NT>, a));
     launched();
     return CLOAK_OK;
 }
 
-// Entry used by gemv.cu.  Preconditions (checked there): bf16, ROWMAJOR, K % 256 == 0, N % 16 == 0, block >= 512 B.
-cloak_status gemv_stream_bf16(const cloak_pool* pool, const cloak_tensor* w, const void* d_x, void* d_y, uint32_t batch,
-                              cudaStream_t s) {
+// log2 of the row-chunk size the streaming kernel would use for this tensor, or -1 if it cannot take it.
+int gemv_stream_log2cb(const cloak_pool* pool, const cloak_tensor* w) {
+    if (w->dt != CLOAK_BF16 || w->layout != CLOAK_ROWMAJOR || w->K % 256 || w->N % GS_ROWS || pool->block < 512) return -1;
     const uint64_t row_bytes = (uint64_t)w->K * 2;
     int log2cb = 12;
     while (log2cb > 9 && (row_bytes & ((1u << log2cb) - 1))) --log2cb;
     if ((uint32_t)log2cb > pool->log2_block) log2cb = (int)pool->log2_block;
-    if (log2cb < 9 || (row_bytes & ((1u << log2cb) - 1))) return fail(CLOAK_ERR_UNSUPPORTED, "gemv_stream: K*2 not a multiple of 512");
-    GemvStreamArgs a;
+    return log2cb;
+}
+
+// One launch: n <= GS_MAX_OPS ops that all stream with the same chunk size.  Preconditions checked by the callers.
+cloak_status gemv_stream_launch(const cloak_pool* pool, const cloak_gemv_op* ops, uint32_t n, int log2cb, uint32_t batch,
+                                cudaStream_t s) {
+    ChainArgs a;
     a.pool = pool->base;
     a.T = pool->d_T;
     a.log2b = pool->log2_block;
-    a.w_offset = w->w_offset;
-    a.N = w->N;
-    a.K = w->K;
-    a.x = static_cast<const uint16_t*>(d_x);
-    a.y = static_cast<__nv_bfloat16*>(d_y);
     a.batch = batch;
-    a.kch = (uint32_t)(row_bytes >> log2cb);
-    const uint32_t tiles = w->N / GS_ROWS;
-    const uint64_t units64 = (uint64_t)tiles * a.kch;
-    if (units64 > 0xffffffffull) return fail(CLOAK_ERR_UNSUPPORTED, "gemv_stream: tensor too large");
-    a.units = (uint32_t)units64;
+    a.nops = n;
     const int sms = sm_count(pool->device);
-    a.per = (a.units + sms - 1) / sms;
-    const int ctas = (int)((a.units + a.per - 1) / a.per);
-    a.maxc = (a.kch + a.per - 1) / a.per + 1;
-    const size_t need = WS_COUNTER_BYTES + (size_t)tiles * a.maxc * batch * GS_ROWS * 4;
-    if ((size_t)tiles * 4 > WS_COUNTER_BYTES) return fail(CLOAK_ERR_UNSUPPORTED, "gemv_stream: N too large for the tile counters");
+    uint64_t max_units = 0, tile_base = 0;
+    for (uint32_t j = 0; j < n; ++j) {
+        const cloak_tensor& w = ops[j].w;
+        ChainOp& o = a.ops[j];
+        o.w_offset = w.w_offset;
+        o.x = static_cast<const uint16_t*>(ops[j].d_x);
+        o.y = static_cast<__nv_bfloat16*>(ops[j].d_y);
+        o.gate = static_cast<const uint16_t*>(ops[j].d_gate);
+        o.act = static_cast<uint16_t*>(ops[j].d_act);
+        o.N = w.N;
+        o.K = w.K;
+        o.kch = (uint32_t)(((uint64_t)w.K * 2) >> log2cb);
+        const uint64_t units64 = (uint64_t)(w.N / GS_ROWS) * o.kch;
+        if (units64 > 0xffffffffull) return fail(CLOAK_ERR_UNSUPPORTED, "gemv: tensor too large");
+        o.units = (uint32_t)units64;
+        o.tile_base = (uint32_t)tile_base;
+        tile_base += w.N / GS_ROWS;
+        o.flags = (j > 0 && ops[j].after) ? OP_AFTER : 0;
+        if (j > 0 && ops[j].after) a.ops[j - 1].flags |= OP_SIGNAL;
+        if (units64 > max_units) max_units = units64;
+    }
+    if (tile_base > GS_TILE_COUNTERS) return fail(CLOAK_ERR_UNSUPPORTED, "gemv: too many output rows for the row-tile counters");
+    const int ctas = max_units < (uint64_t)sms ? (int)max_units : sms;
+    for (uint32_t j = 0; j < n; ++j) {
+        ChainOp& o = a.ops[j];
+        o.per = (o.units + ctas - 1) / ctas;
+        o.ctas = (o.units + o.per - 1) / o.per;
+    }
+    const size_t need = WS_COUNTER_BYTES + (size_t)n * ctas * batch * GS_ROWS * 4;
     cloak_status st = pool_workspace(pool, need);
     if (st != CLOAK_OK) return st;
     a.counters = reinterpret_cast<uint32_t*>(pool->ws);
+    a.opsync = a.counters + GS_TILE_COUNTERS;
     a.part = reinterpret_cast<float*>(pool->ws + WS_COUNTER_BYTES);
     a.early = (g_gemv_pdl && !pool->dirty) ? 1u : 0u;
     if (pool->dirty && pool->dirty_stream == s) pool->dirty = false;   // this launch waits for the writer in full

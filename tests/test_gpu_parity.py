@@ -333,6 +333,86 @@ def test_cfg0_mlp_end_to_end_permuted_and_cloaked():
         assert O.err_normwise(y.cpu().numpy(), ref) <= 2e-5
 
 
+# ------------------------------------------------------------------ S6 as one launch: cloak_gemv_chain
+CHAIN_CASES = [
+    # hidden, inter, n_q, n_kv, d, block, batches
+    (256, 768, 4, 2, 64, 4096, [1, 5, 16]),             # small: 512 B / 1.5 KiB rows, several chunk sizes in one chain
+    (1024, 3584, 8, 2, 128, 65536, [1, 4, 9]),          # 2 KiB and 7 KiB rows: two launch groups
+    (4096, 14336, 32, 8, 128, 65536, [1, 16]),          # cfg1's layer: 4 KiB chunks, every CTA's range cut twice
+]
+
+
+@pytest.mark.parametrize("H,I,n_q,n_kv,d,block,batches", CHAIN_CASES)
+def test_gemv_chain_layer_vs_single_calls_and_oracle(H, I, n_q, n_kv, d, block, batches):
+    """One decoder layer's projections as ONE chain (q,k,v | o | gate,up | down with the fused silu*up input):
+    bit-identical to the call-by-call path (cloak_gemv + cloak_silu_mul), bit-identical between the cloaked and
+    the identity-table pool, within tolerance of the fp64 oracle (linear_f64 / mlp_f64), and repeatable."""
+    key, seed, page = 0x1234, 1, 2 << 20 if block >= 65536 else 65536
+    shapes = gen.layer_shapes(H, I, n_q, n_kv, d)
+    Ws = {nm: gen.synth(seed, i, shp, "bf16") for i, (nm, shp) in enumerate(shapes)}
+    sizes = [2 * n * k for _, (n, k) in shapes]
+    offs, total = C.cloak_arena_plan(key, sizes, block)
+    off = {nm: o for (nm, _), o in zip(shapes, offs)}
+    with Pool(total, block, page, key) as pc, Pool(total, block, page, key, C.CLOAK_POOL_IDENTITY) as pi:
+        for p in (pc, pi):
+            _load_pool(p, [(nm, Ws[nm]) for nm, _ in shapes], offs, "bf16")
+        T = {nm: C.cloak_tensor(off[nm], shp[0], shp[1], C.CLOAK_BF16, C.CLOAK_ROWMAJOR) for nm, shp in shapes}
+        for batch in batches:
+            xh = gen.synth(seed + 100, batch, (batch, H), "bf16", kind=gen.KIND_NORMAL)
+            xa = gen.synth(seed + 200, batch, (batch, n_q * d), "bf16", kind=gen.KIND_NORMAL)
+            dxh, dxa = bf16_dev_from_bits(xh), bf16_dev_from_bits(xa)
+
+            def outputs():
+                y = {nm: torch.zeros(batch, shp[0], dtype=torch.bfloat16, device="cuda") for nm, shp in shapes}
+                y["act"] = torch.zeros(batch, I, dtype=torch.bfloat16, device="cuda")
+                return y
+
+            def run_chain(pool, y):
+                ops = [(T["q"], dxh, y["q"], 0), (T["k"], dxh, y["k"], 0), (T["v"], dxh, y["v"], 0),
+                       (T["o"], dxa, y["o"], 0), (T["gate"], dxh, y["gate"], 0),
+                       (T["up"], dxh, y["up"], 0, y["gate"], y["act"]), (T["down"], y["act"], y["down"], 1)]
+                C.cloak_gemv_chain(pool.h, ops, batch)
+
+            yc, yi, ys, yr = outputs(), outputs(), outputs(), outputs()
+            run_chain(pc, yc)
+            run_chain(pi, yi)
+            for nm in ("q", "k", "v", "gate", "up"):                       # call by call
+                C.cloak_gemv(pc.h, T[nm], dxh, ys[nm], batch)
+            C.cloak_gemv(pc.h, T["o"], dxa, ys["o"], batch)
+            C.cloak_silu_mul(ys["gate"], ys["up"], ys["act"], batch * I, C.CLOAK_BF16)
+            C.cloak_gemv(pc.h, T["down"], ys["act"], ys["down"], batch)
+            run_chain(pc, yr)                                              # counters and barriers self-reset
+            torch.cuda.synchronize()
+            for nm in yc:
+                assert torch.equal(yc[nm], yi[nm]), (nm, batch, "cloaked vs identity")
+                assert torch.equal(yc[nm], ys[nm]), (nm, batch, "chain vs single calls")
+                assert torch.equal(yc[nm], yr[nm]), (nm, batch, "second launch")
+            for nm in ("q", "k", "v", "gate", "up"):
+                assert O.err_normwise(yc[nm].float().cpu().numpy(), O.linear_f64(xh, Ws[nm])) <= TOL["bf16"], (nm, batch)
+            assert O.err_normwise(yc["o"].float().cpu().numpy(), O.linear_f64(xa, Ws["o"])) <= TOL["bf16"]
+            ref = O.mlp_f64(xh, Ws["gate"], Ws["up"], Ws["down"])           # fp64 all the way, no bf16 intermediates
+            assert O.err_normwise(yc["down"].float().cpu().numpy(), ref) <= TOL["bf16"], (batch,)
+
+
+def test_gemv_chain_argument_checks():
+    with Pool(1 << 20, 4096, 65536, 0x1234) as p:
+        x = torch.zeros(1, 256, dtype=torch.bfloat16, device="cuda")
+        y = torch.zeros(1, 64, dtype=torch.bfloat16, device="cuda")
+        good = C.cloak_tensor(0, 64, 256, C.CLOAK_BF16, C.CLOAK_ROWMAJOR)
+        C.cloak_gemv_chain(p.h, [(good, x, y, 0)], 1)
+        for bad, status in ((C.cloak_tensor(0, 64, 64, C.CLOAK_BF16, C.CLOAK_ROWMAJOR), C.CLOAK_ERR_UNSUPPORTED),   # K % 256
+                            (C.cloak_tensor(0, 64, 256, C.CLOAK_F32, C.CLOAK_ROWMAJOR), C.CLOAK_ERR_UNSUPPORTED),
+                            (C.cloak_tensor(4096 * 255, 64, 256, C.CLOAK_BF16, C.CLOAK_ROWMAJOR), C.CLOAK_ERR_INVALID)):
+            with pytest.raises(C.CloakError) as e:
+                C.cloak_gemv_chain(p.h, [(good, x, y, 0), (bad, x, y, 0)], 1)
+            assert e.value.status == status
+        with pytest.raises(C.CloakError):
+            C.cloak_gemv_chain(p.h, [(good, x, y, 0)], 17)
+        with pytest.raises(C.CloakError):                                   # d_gate without d_act
+            C.cloak_gemv_chain(p.h, [(good, x, y, 0, y, None)], 1)
+        torch.cuda.synchronize()
+
+
 # ------------------------------------------------------------------ S7 cloaked GEMM (tcgen05, TILE128)
 GEMM_CASES = [
     # block, shapes [(N, K)], batches
