@@ -6,10 +6,10 @@
 //
 // Kernels (all integer, bit-exact by construction):
 //   n <= 4096 : one launch.  Keys in shared memory, rank of i = #{k : (r_k,k) < (r_i,i)} by counting.
-//   n  > 4096 : philox_keys -> 8 passes of a stable LSD radix sort on 8-bit digits of the 64-bit key
-//               with the index as payload (stable + initial index order ascending == tie-break by
-//               smaller i) -> inverse scatter.  Each pass: per-tile histogram, one-CTA exclusive
-//               scan over [digit][tile], stable scatter with warp match-any ranking.
+//   n  > 4096 : four launches.  Bucket by the top ~log2(n/4) bits of the key (histogram, one-CTA exclusive
+//               scan, fill), then rank by counting inside the bucket (~4 elements): a one-pass MSD bucket
+//               sort that is O(n) for uniform keys and exact for any.  (Round 1 started with an 8-pass LSD
+//               radix sort: 26 launches, ~100 us at n = 14 336; this is 4 launches, ~10 us.)
 #include "common.cuh"
 #include "philox.cuh"
 
@@ -39,34 +39,50 @@ __global__ void __launch_bounds__(256) keygen_small_kernel(uint32_t n, uint32_t 
     }
 }
 
-__global__ void philox_keys_kernel(uint32_t n, uint32_t s_lo, uint32_t s_hi, uint32_t k0, uint32_t k1,
-                                   uint64_t* __restrict__ keys, uint32_t* __restrict__ idx) {
-    uint32_t i = blockIdx.x * blockDim.x + threadIdx.x;
+// ---- n > 4096: bucket by the top bits of the key, then rank by counting inside the bucket.
+// The keys are uniform (Philox), so 2^bits ~ n/4 buckets hold ~4 elements each and the counting pass costs
+// O(n) in expectation; the result is exact for ANY distribution (a skewed one would only be slower), and it is
+// deterministic although the order inside a bucket list is not (atomics): a rank does not depend on that order.
+//   bucket_hist   : hist[bucket(r_i)] += 1
+//   scan_exclusive: base = exclusive prefix sums (one CTA)
+//   bucket_fill   : slot = base[b] + cursor[b]++ ;  bk[slot] = r_i, bi[slot] = i
+//   bucket_rank   : rank of (r, i) = base[b] + #{(r', i') in bucket b : (r', i') < (r, i)};  perm[rank] = i, inv[i] = rank
+__global__ void __launch_bounds__(256) bucket_hist_kernel(uint32_t n, uint32_t s_lo, uint32_t s_hi, uint32_t k0, uint32_t k1,
+                                                          int shift, uint32_t* __restrict__ hist) {
+    const uint32_t i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i < n) atomicAdd(hist + (uint32_t)(philox_key64(i, s_lo, s_hi, k0, k1) >> shift), 1u);
+}
+
+__global__ void __launch_bounds__(256) bucket_fill_kernel(uint32_t n, uint32_t s_lo, uint32_t s_hi, uint32_t k0, uint32_t k1,
+                                                          int shift, const uint32_t* __restrict__ base,
+                                                          uint32_t* __restrict__ cursor, uint64_t* __restrict__ bk,
+                                                          uint32_t* __restrict__ bi) {
+    const uint32_t i = blockIdx.x * blockDim.x + threadIdx.x;
     if (i < n) {
-        keys[i] = philox_key64(i, s_lo, s_hi, k0, k1);
-        idx[i] = i;
+        const uint64_t r = philox_key64(i, s_lo, s_hi, k0, k1);
+        const uint32_t b = (uint32_t)(r >> shift);
+        const uint32_t slot = base[b] + atomicAdd(cursor + b, 1u);
+        bk[slot] = r;
+        bi[slot] = i;
     }
 }
 
-constexpr int RADIX_THREADS = 256;
-constexpr int RADIX_WARPS = RADIX_THREADS / 32;
-constexpr int RADIX_STEPS = 16;                                  // 32-element steps per warp
-constexpr int RADIX_TILE = RADIX_THREADS * RADIX_STEPS;          // 4096 elements per CTA
-
-__global__ void __launch_bounds__(RADIX_THREADS) radix_hist_kernel(const uint64_t* __restrict__ keys, uint32_t n,
-                                                                   int shift, uint32_t* __restrict__ hist,
-                                                                   uint32_t ntiles) {
-    __shared__ uint32_t h[256];
-    h[threadIdx.x] = 0;
-    __syncthreads();
-    const uint32_t base = blockIdx.x * RADIX_TILE;
-#pragma unroll 4
-    for (int j = 0; j < RADIX_STEPS; ++j) {
-        uint32_t i = base + j * RADIX_THREADS + threadIdx.x;
-        if (i < n) atomicAdd(&h[(uint32_t)(keys[i] >> shift) & 255u], 1u);
+__global__ void __launch_bounds__(256) bucket_rank_kernel(uint32_t n, int shift, const uint32_t* __restrict__ base,
+                                                          const uint64_t* __restrict__ bk, const uint32_t* __restrict__ bi,
+                                                          uint32_t* __restrict__ perm, uint32_t* __restrict__ inv) {
+    const uint32_t p = blockIdx.x * blockDim.x + threadIdx.x;
+    if (p >= n) return;
+    const uint64_t r = bk[p];
+    const uint32_t i = bi[p];
+    const uint32_t b = (uint32_t)(r >> shift);
+    const uint32_t lo = base[b], hi = base[b + 1];
+    uint32_t rank = lo;
+    for (uint32_t q = lo; q < hi; ++q) {
+        const uint64_t rq = bk[q];
+        rank += (rq < r) || (rq == r && bi[q] < i);
     }
-    __syncthreads();
-    hist[threadIdx.x * ntiles + blockIdx.x] = h[threadIdx.x];
+    if (perm) perm[rank] = i;
+    if (inv) inv[i] = rank;
 }
 
 // In-place exclusive scan of a[0..M) by one CTA of 1024 threads.
@@ -117,68 +133,6 @@ __global__ void __launch_bounds__(1024) scan_exclusive_kernel(uint32_t* __restri
     }
 }
 
-__global__ void __launch_bounds__(RADIX_THREADS) radix_scatter_kernel(
-    const uint64_t* __restrict__ keys_in, const uint32_t* __restrict__ idx_in, uint64_t* __restrict__ keys_out,
-    uint32_t* __restrict__ idx_out, uint32_t n, int shift, const uint32_t* __restrict__ offsets, uint32_t ntiles) {
-    __shared__ uint32_t cnt[RADIX_WARPS][256];
-    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-    for (int j = threadIdx.x; j < RADIX_WARPS * 256; j += RADIX_THREADS) (&cnt[0][0])[j] = 0;
-    __syncthreads();
-    const uint32_t wbase = blockIdx.x * RADIX_TILE + warp * (32 * RADIX_STEPS);
-    uint64_t k[RADIX_STEPS];
-    uint32_t rank[RADIX_STEPS];
-    const uint32_t lt = (1u << lane) - 1u;
-#pragma unroll
-    for (int j = 0; j < RADIX_STEPS; ++j) {
-        const uint32_t i = wbase + j * 32 + lane;     // a warp owns 512 consecutive elements, in order
-        const bool valid = i < n;
-        k[j] = valid ? keys_in[i] : 0ull;
-        const uint32_t d = (uint32_t)(k[j] >> shift) & 255u;
-        const uint32_t active = __ballot_sync(0xffffffffu, valid);
-        rank[j] = 0;
-        // Every lane reads its digit's running count, then the lowest lane of each digit group bumps it:
-        // reads and writes are separated by warp barriers, so there is no divergent shuffle.
-        uint32_t peers = 0, old = 0;
-        if (valid) {
-            peers = __match_any_sync(active, d);
-            old = cnt[warp][d];
-        }
-        __syncwarp();
-        if (valid) {
-            if ((peers & lt) == 0) cnt[warp][d] = old + __popc(peers);
-            rank[j] = old + __popc(peers & lt);
-        }
-        __syncwarp();
-    }
-    __syncthreads();
-    {   // per digit: global base of this tile, then exclusive prefix over the warps (warp order = element order)
-        const uint32_t d = threadIdx.x;
-        uint32_t run = offsets[d * ntiles + blockIdx.x];
-#pragma unroll
-        for (int w = 0; w < RADIX_WARPS; ++w) {
-            uint32_t c = cnt[w][d];
-            cnt[w][d] = run;
-            run += c;
-        }
-    }
-    __syncthreads();
-#pragma unroll
-    for (int j = 0; j < RADIX_STEPS; ++j) {
-        const uint32_t i = wbase + j * 32 + lane;
-        if (i < n) {
-            const uint32_t d = (uint32_t)(k[j] >> shift) & 255u;
-            const uint32_t pos = cnt[warp][d] + rank[j];
-            if (keys_out) keys_out[pos] = k[j];
-            idx_out[pos] = idx_in[i];
-        }
-    }
-}
-
-__global__ void invert_kernel(const uint32_t* __restrict__ perm, uint32_t* __restrict__ inv, uint32_t n) {
-    uint32_t j = blockIdx.x * blockDim.x + threadIdx.x;
-    if (j < n) inv[perm[j]] = j;
-}
-
 cloak_status keygen_device(uint64_t key, uint64_t stream_id, uint32_t n, uint32_t* d_perm, uint32_t* d_inv,
                            cudaStream_t s) {
     const uint32_t s_lo = (uint32_t)stream_id, s_hi = (uint32_t)(stream_id >> 32);
@@ -189,9 +143,12 @@ cloak_status keygen_device(uint64_t key, uint64_t stream_id, uint32_t n, uint32_
         CLOAK_LAUNCH_CHECK();
         return CLOAK_OK;
     }
-    const uint32_t ntiles = (n + RADIX_TILE - 1) / RADIX_TILE;
-    const size_t keys_b = (size_t)n * 8, idx_b = (size_t)n * 4, hist_b = (size_t)256 * ntiles * 4;
-    const size_t total = 2 * keys_b + 2 * idx_b + hist_b;
+    int bits = 1;
+    while (bits < 22 && (4ull << bits) < n) ++bits;             // ~n/4 buckets, at most 2^22
+    const int shift = 64 - bits;
+    const uint32_t nbuckets = 1u << bits;
+    const size_t keys_b = (size_t)n * 8, idx_b = (size_t)n * 4, tab_b = ((size_t)nbuckets + 1) * 4;
+    const size_t total = keys_b + idx_b + 2 * tab_b;
     char* ws = nullptr;
     {   // keep freed workspace cached in the stream-ordered pool instead of returning it to the OS at every sync
         static bool tuned = false;
@@ -207,33 +164,21 @@ cloak_status keygen_device(uint64_t key, uint64_t stream_id, uint32_t n, uint32_
         }
     }
     CLOAK_CUDA(cudaMallocAsync((void**)&ws, total, s));
-    uint64_t* keys[2] = {(uint64_t*)ws, (uint64_t*)(ws + keys_b)};
-    uint32_t* idx[2] = {(uint32_t*)(ws + 2 * keys_b), (uint32_t*)(ws + 2 * keys_b + idx_b)};
-    uint32_t* hist = (uint32_t*)(ws + 2 * keys_b + 2 * idx_b);
-    philox_keys_kernel<<<(n + 255) / 256, 256, 0, s>>>(n, s_lo, s_hi, k0, k1, keys[0], idx[0]);
+    uint64_t* bk = (uint64_t*)ws;
+    uint32_t* bi = (uint32_t*)(ws + keys_b);
+    uint32_t* base = (uint32_t*)(ws + keys_b + idx_b);           // hist, then (scanned in place) base[0 .. nbuckets]
+    uint32_t* cursor = base + nbuckets + 1;
+    CLOAK_CUDA(cudaMemsetAsync(base, 0, 2 * tab_b, s));
+    const unsigned grid = (n + 255) / 256;
+    bucket_hist_kernel<<<grid, 256, 0, s>>>(n, s_lo, s_hi, k0, k1, shift, base);
+    launched();
+    scan_exclusive_kernel<<<1, 1024, 0, s>>>(base, nbuckets + 1);
+    launched();
+    bucket_fill_kernel<<<grid, 256, 0, s>>>(n, s_lo, s_hi, k0, k1, shift, base, cursor, bk, bi);
+    launched();
+    bucket_rank_kernel<<<grid, 256, 0, s>>>(n, shift, base, bk, bi, d_perm, d_inv);
     launched();
     CLOAK_LAUNCH_CHECK();
-    int cur = 0;
-    for (int pass = 0; pass < 8; ++pass) {
-        const int shift = pass * 8;
-        radix_hist_kernel<<<ntiles, RADIX_THREADS, 0, s>>>(keys[cur], n, shift, hist, ntiles);
-        launched();
-        scan_exclusive_kernel<<<1, 1024, 0, s>>>(hist, 256 * ntiles);
-        launched();
-        const bool last = pass == 7;
-        uint32_t* idx_dst = (last && d_perm) ? d_perm : idx[cur ^ 1];
-        radix_scatter_kernel<<<ntiles, RADIX_THREADS, 0, s>>>(keys[cur], idx[cur], last ? nullptr : keys[cur ^ 1],
-                                                              idx_dst, n, shift, hist, ntiles);
-        launched();
-        CLOAK_LAUNCH_CHECK();
-        cur ^= 1;
-    }
-    if (d_inv) {
-        const uint32_t* perm = d_perm ? d_perm : idx[cur];
-        invert_kernel<<<(n + 255) / 256, 256, 0, s>>>(perm, d_inv, n);
-        launched();
-        CLOAK_LAUNCH_CHECK();
-    }
     CLOAK_CUDA(cudaFreeAsync(ws, s));
     return CLOAK_OK;
 }

@@ -7,10 +7,12 @@
 //   eta[g*G+j] = kappa[g]*G + rho_g[j];  k',v' row groups by kappa; q' row groups, o' column groups by eta.
 // Bytes move exactly; HBM-bound (1 read + 1 write per byte).
 //   rows    : whole-row gather, 16-byte vectors, 4 rows in flight per CTA iteration.
-//   columns : the source row is staged in shared memory with coalesced 16-byte loads, the expanded column
-//             map sits in shared memory too, output vectors are assembled from shared memory and stored
-//             coalesced.
+//   columns : source rows stream through a shared-memory ring (one TMA bulk copy per row, several rows in
+//             flight), the expanded column map sits in shared memory too, output vectors are assembled from
+//             shared memory and stored coalesced; column groups that are whole 16-byte vectors (heads) skip
+//             the staging and move vectors directly.
 #include "common.cuh"
+#include "async.cuh"
 #include "philox.cuh"
 
 namespace cloak {
@@ -75,29 +77,71 @@ __global__ void __launch_bounds__(256) gather_rows_kernel(const int4* __restrict
     }
 }
 
-// dst[row, c'] <- src[row, map[c' / seg] * seg + c' % seg], element type E (2 or 4 bytes).
-// Dynamic shared memory: colmap[ncols] (uint32) followed by one source row.
-template <typename E>
-__global__ void __launch_bounds__(256) gather_cols_kernel(const E* __restrict__ src, E* __restrict__ dst,
+// dst[row, c'] <- src[row, map[c' / seg] * seg + c' % seg], element type E (2 or 4 bytes), column map entries of
+// type M (uint16 when ncols <= 65536, else uint32).
+// Dynamic shared memory: colmap[ncols] followed by a ring of NS source rows.  One elected thread keeps the ring
+// full with one bulk copy (TMA 1-D, mbarrier completion) per row, so the DRAM latency of row r+1.. hides behind the
+// shared-memory gather of row r; the gathered vectors go out as coalesced 16-byte stores.
+template <typename E, typename M>
+__global__ void __launch_bounds__(512) gather_cols_kernel(const E* __restrict__ src, E* __restrict__ dst,
                                                           const uint32_t* __restrict__ map, uint32_t seg,
-                                                          uint32_t nrows, uint32_t ncols) {
-    extern __shared__ __align__(16) unsigned char sm[];
-    uint32_t* colmap = reinterpret_cast<uint32_t*>(sm);
-    E* row = reinterpret_cast<E*>(sm + (((size_t)ncols * 4 + 15) & ~(size_t)15));
-    for (uint32_t c = threadIdx.x; c < ncols; c += blockDim.x) colmap[c] = __ldg(map + c / seg) * seg + c % seg;
+                                                          uint32_t nrows, uint32_t ncols, uint32_t ns) {
+    extern __shared__ __align__(128) unsigned char sm[];
+    __shared__ __align__(8) uint64_t full[8];
+    M* colmap = reinterpret_cast<M*>(sm);
+    const uint32_t row_bytes = ncols * sizeof(E);
+    unsigned char* ring = sm + (((size_t)ncols * sizeof(M) + 127) & ~(size_t)127);
+    for (uint32_t c = threadIdx.x; c < ncols; c += blockDim.x) colmap[c] = (M)(__ldg(map + c / seg) * seg + c % seg);
+    if (threadIdx.x == 0) {
+        for (uint32_t i = 0; i < ns; ++i) mbar_init(smem_u32(&full[i]), 1);
+        fence_barrier_init();
+    }
+    __syncthreads();
+    // rows of this CTA: r_k = blockIdx.x + k * gridDim.x
+    const uint32_t mine = blockIdx.x < nrows ? (nrows - blockIdx.x + gridDim.x - 1) / gridDim.x : 0;
+    auto issue = [&](uint32_t k) {
+        const uint32_t st = k % ns, bar = smem_u32(&full[st]);
+        mbar_expect_tx(bar, row_bytes);
+        bulk_g2s(smem_u32(ring + (size_t)st * row_bytes), src + (uint64_t)(blockIdx.x + k * gridDim.x) * ncols, row_bytes, bar);
+    };
+    if (threadIdx.x == 0)
+        for (uint32_t k = 0; k < ns && k < mine; ++k) issue(k);
     constexpr int EPV = 16 / sizeof(E);
     const uint32_t vpr = ncols / EPV;
-    for (uint32_t r = blockIdx.x; r < nrows; r += gridDim.x) {
-        __syncthreads();                                       // previous row fully consumed; colmap ready
-        const int4* s4 = reinterpret_cast<const int4*>(src + (uint64_t)r * ncols);
-        for (uint32_t v = threadIdx.x; v < vpr; v += blockDim.x) reinterpret_cast<int4*>(row)[v] = ldg_stream(s4 + v);
-        __syncthreads();
-        int4* d4 = reinterpret_cast<int4*>(dst + (uint64_t)r * ncols);
+    for (uint32_t k = 0; k < mine; ++k) {
+        const uint32_t st = k % ns;
+        mbar_wait(smem_u32(&full[st]), (k / ns) & 1);
+        const E* row = reinterpret_cast<const E*>(ring + (size_t)st * row_bytes);
+        int4* d4 = reinterpret_cast<int4*>(dst + (uint64_t)(blockIdx.x + k * gridDim.x) * ncols);
         for (uint32_t v = threadIdx.x; v < vpr; v += blockDim.x) {
             union { int4 q; E e[EPV]; } out;
 #pragma unroll
-            for (int k = 0; k < EPV; ++k) out.e[k] = row[colmap[v * EPV + k]];
+            for (int j = 0; j < EPV; ++j) out.e[j] = row[colmap[v * EPV + j]];
             d4[v] = out.q;
+        }
+        __syncthreads();                                       // every thread is done with this stage
+        if (threadIdx.x == 0 && k + ns < mine) issue(k + ns);
+    }
+}
+
+// Column groups that are whole 16-byte vectors (seg % (16 / sizeof(E)) == 0, e.g. heads of 128 columns): the gather
+// is a vector-level index remap, no staging needed.  vmap[v'] = source vector of destination vector v'.
+__global__ void __launch_bounds__(256) gather_colvecs_kernel(const int4* __restrict__ src, int4* __restrict__ dst,
+                                                             const uint32_t* __restrict__ map, uint32_t vseg,
+                                                             uint32_t nrows, uint32_t vpr) {
+    extern __shared__ uint32_t vmap[];
+    for (uint32_t v = threadIdx.x; v < vpr; v += blockDim.x) vmap[v] = __ldg(map + v / vseg) * vseg + v % vseg;
+    __syncthreads();
+    for (uint32_t r0 = blockIdx.x * ROWS_PER_IT; r0 < nrows; r0 += gridDim.x * ROWS_PER_IT) {
+        for (uint32_t v = threadIdx.x; v < vpr; v += blockDim.x) {
+            const uint32_t sv = vmap[v];
+            int4 x[ROWS_PER_IT];
+#pragma unroll
+            for (int k = 0; k < ROWS_PER_IT; ++k)
+                if (r0 + k < nrows) x[k] = ldg_stream(src + (uint64_t)(r0 + k) * vpr + sv);
+#pragma unroll
+            for (int k = 0; k < ROWS_PER_IT; ++k)
+                if (r0 + k < nrows) dst[(uint64_t)(r0 + k) * vpr + v] = x[k];
         }
     }
 }
@@ -166,24 +210,47 @@ static cloak_status rows(const void* src, void* dst, const uint32_t* map, uint32
     return CLOAK_OK;
 }
 
+template <typename E, typename M>
+static cloak_status cols_ring(const void* src, void* dst, const uint32_t* map, uint32_t seg, uint32_t nrows, uint32_t ncols,
+                              size_t smem, uint32_t ns, int sms, cudaStream_t s) {
+    static bool attr_set = false;
+    if (!attr_set) {
+        CLOAK_CUDA(cudaFuncSetAttribute(gather_cols_kernel<E, M>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024));
+        attr_set = true;
+    }
+    const uint32_t ctas = nrows < (uint32_t)sms ? nrows : (uint32_t)sms;
+    gather_cols_kernel<E, M><<<ctas, 512, smem, s>>>((const E*)src, (E*)dst, map, seg, nrows, ncols, ns);
+    launched();
+    CLOAK_LAUNCH_CHECK();
+    return CLOAK_OK;
+}
+
 template <typename E>
 static cloak_status cols(const void* src, void* dst, const uint32_t* map, uint32_t seg, uint32_t nrows, uint32_t ncols,
                          int sms, cudaStream_t s) {
-    const size_t smem = (((size_t)ncols * 4 + 15) & ~(size_t)15) + (size_t)ncols * sizeof(E);
-    if (smem <= 200 * 1024) {
-        static bool attr_set = false;
-        if (!attr_set) {
-            CLOAK_CUDA(cudaFuncSetAttribute(gather_cols_kernel<E>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024));
-            attr_set = true;
-        }
-        const uint32_t per_sm = smem <= 100 * 1024 ? 2u : 1u;
-        uint32_t ctas = nrows < (uint32_t)sms * per_sm ? nrows : (uint32_t)sms * per_sm;
-        gather_cols_kernel<E><<<ctas, 256, smem, s>>>((const E*)src, (E*)dst, map, seg, nrows, ncols);
+    constexpr uint32_t EPV = 16 / sizeof(E);
+    const size_t row_bytes = (size_t)ncols * sizeof(E);
+    if (seg % EPV == 0 && (size_t)(ncols / EPV) * 4 <= 48 * 1024) {
+        const uint32_t vpr = ncols / EPV;
+        uint32_t ctas = (nrows + ROWS_PER_IT - 1) / ROWS_PER_IT;
+        if (ctas > (uint32_t)sms * 8) ctas = (uint32_t)sms * 8;
+        gather_colvecs_kernel<<<ctas, 256, (size_t)vpr * 4, s>>>((const int4*)src, (int4*)dst, map, seg / EPV, nrows, vpr);
         launched();
-    } else {
-        gather_cols_global_kernel<E><<<sms * 8, 256, 0, s>>>((const E*)src, (E*)dst, map, seg, nrows, ncols);
-        launched();
+        CLOAK_LAUNCH_CHECK();
+        return CLOAK_OK;
     }
+    const size_t msz = ncols <= 65536 ? 2 : 4;
+    const size_t cm = ((size_t)ncols * msz + 127) & ~(size_t)127;
+    const size_t budget = 200 * 1024;
+    uint32_t ns = cm < budget ? (uint32_t)((budget - cm) / row_bytes) : 0;
+    if (ns > 6) ns = 6;
+    if (ns >= 2) {
+        const size_t smem = cm + (size_t)ns * row_bytes;
+        return msz == 2 ? cols_ring<E, uint16_t>(src, dst, map, seg, nrows, ncols, smem, ns, sms, s)
+                        : cols_ring<E, uint32_t>(src, dst, map, seg, nrows, ncols, smem, ns, sms, s);
+    }
+    gather_cols_global_kernel<E><<<sms * 8, 256, 0, s>>>((const E*)src, (E*)dst, map, seg, nrows, ncols);
+    launched();
     CLOAK_LAUNCH_CHECK();
     return CLOAK_OK;
 }
