@@ -178,6 +178,23 @@ def run_reference(args):
     return 0
 
 
+# ------------------------------------------------------------------------------------------ replicas (N > 1)
+def max_over_ranks(ms, dist, device):
+    """The path does not shard (replicas only): every rank times its own replica of the step and the
+    job's time is the slowest rank's.  One scalar all_reduce(MAX); `dist` is None on a single rank."""
+    if dist is None:
+        return float(ms)
+    import torch
+    t = torch.tensor([ms], device=device, dtype=torch.float64)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+def whole_job_gbs(bytes_per_replica_step, ms_per_step, world):
+    """`value`: bytes all replicas moved per step / the slowest replica's step time (weak scaling)."""
+    return world * bytes_per_replica_step / ms_per_step / 1e6
+
+
 # ------------------------------------------------------------------------------------------ GPU arm
 def run_cloak(args):
     import torch
@@ -319,10 +336,7 @@ def run_cloak(args):
     total_ms = evs[0][0].elapsed_time(evs[-1][-1])
     stage_ms = {s: float(np.mean([evs[k][i].elapsed_time(evs[k][i + 1]) for k in range(args.steps)]))
                 for i, s in enumerate(STAGES)}
-    if dist is not None:
-        t = torch.tensor([total_ms], device="cuda", dtype=torch.float64)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        total_ms = float(t.item())
+    total_ms = max_over_ranks(total_ms, dist, "cuda")
 
     # ---- the same GEMV chains on the identity-table ("native") pool: the overhead denominator.  Same launch mode,
     # cloaked and native interleaved rep by rep so that drift hits both alike.
@@ -406,7 +420,7 @@ def run_cloak(args):
     gemv_launches = len(BATCHES)                        # one chain launch (7 projections) per batch
     achieved = gbs(sb["gemv"], gemv_ms)
     line = {
-        "metric": METRIC, "value": world * gbs(sb["total"], ms_per_step), "unit": "GB/s", "n_gpus": world,
+        "metric": METRIC, "value": whole_job_gbs(sb["total"], ms_per_step, world), "unit": "GB/s", "n_gpus": world,
         "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms_per_step, "higher_is_better": True,
         "scaling": "weak", "vs_baseline": None, "dtype": "bf16", "data": "synthetic",
         "config": {"workload": "cfg1: one LLaMA-8B-shaped decoder layer, bf16, 436.2 MB, 64 KiB blocks, 2 MiB VMM pages",

@@ -1,0 +1,299 @@
+"""GPU parity at BASELINE.json's full sizes, in the launch configurations bench.py / workloads.py time.
+
+Small-size element-by-element parity lives in test_gpu_parity.py.  Here the sizes are the real ones (cfg1's
+436 MB layer, cfg2's 16 GB / 245 056-block pool, cfg3's 62 GB / 952 320-block TILE128 pool, cfg4's 4 GiB
+buffer at five block sizes).  Tables and bytes must be bit-exact with the CPU oracle; GEMV / GEMM outputs are
+compared with the fp64 oracle on every output (cfg1) or on seeded samples of output rows (cfg2, cfg3), within
+north_star's tolerance (O12 norm-wise error <= 2e-2 for bf16).
+
+Inputs: the shared synthetic generator (synth/).  Multi-GB tensors are filled by its CUDA twin and copied to the
+host for the oracle; every test re-checks a slice of each such tensor against the numpy twin, so the oracle's
+inputs are the generator's values, never the CUDA path's.  Set CLOAK_SKIP_FULLSIZE=1 to skip this file.
+"""
+import ctypes
+import os
+
+import numpy as np
+import pytest
+import torch
+
+import oracle as O
+from synth import gen
+
+pytestmark = [pytest.mark.gpu,
+              pytest.mark.skipif(os.environ.get("CLOAK_SKIP_FULLSIZE") == "1", reason="CLOAK_SKIP_FULLSIZE=1")]
+
+if torch.cuda.is_available():
+    import paper_2606_18400_b200 as C
+    from synth import cuda as synth_cuda
+    from gpu_util import Pool, ctypes_cudart_copy
+
+TOL_BF16 = 2e-2
+KEY = 0x1234
+
+
+# ------------------------------------------------------------------ plumbing (no method arithmetic)
+def fill_bf16(shape, seed, tid, kind=0):
+    """A tensor from the generator's CUDA twin + its host copy as uint16 bit patterns; a slice is re-checked
+    against the numpy twin."""
+    t = synth_cuda.fill(torch.empty(shape, dtype=torch.bfloat16, device="cuda"), seed, tid, kind=kind)
+    h = t.view(torch.int16).cpu().numpy().view(np.uint16)
+    n = h.size
+    for start in (0, max(0, n // 2 - 1000), max(0, n - 4096)):
+        cnt = min(4096, n - start)
+        assert np.array_equal(h.reshape(-1)[start:start + cnt], gen.synth_bf16_bits(seed, tid, start, cnt, kind))
+    return t, h
+
+
+def bits(t):
+    return t.detach().contiguous().view(torch.int16).cpu().numpy().view(np.uint16)
+
+
+def read_slots(pool, slots, block):
+    """Host copy of the given block slots of a pool, read through its base pointer (the VA view V)."""
+    out = np.empty((len(slots), block), np.uint8)
+    torch.cuda.synchronize()
+    base = pool.info["d_base"]
+    for k, s in enumerate(slots):
+        ctypes_cudart_copy(out[k].ctypes.data, base + int(s) * block, block)
+    return out
+
+
+def check_tensor_in_pool(pool, T, data_u8, off, block):
+    """pool[T[i]*b : +b] == arena block i for every block of the tensor at arena offset `off` (last block zero-padded)."""
+    nblk = (data_u8.size + block - 1) // block
+    first = off // block
+    got = read_slots(pool, T[first:first + nblk], block)
+    ref = np.zeros(nblk * block, np.uint8)
+    ref[:data_u8.size] = data_u8
+    assert np.array_equal(got.reshape(-1), ref)
+
+
+def sample_rows(n, count, seed):
+    return np.sort(np.random.default_rng(seed).choice(n, size=min(count, n), replace=False))
+
+
+# ------------------------------------------------------------------ cfg1: one LLaMA-8B-shaped layer, everything
+def test_cfg1_full_layer_every_stage():
+    """bench.py's step at full size: permute -> per-tensor shuffle into 208 real 2 MiB pages -> re-layout to key B ->
+    the 7 projections as one cloak_gemv_chain per batch (1, 4, 16; plain launch and CUDA-graph replay) -> unshuffle.
+    Bytes bit-exact (V, D, re-laid-out pool, round trip), every GEMV output within tolerance of the fp64 oracle."""
+    c = gen.CONFIGS[1]
+    H, I, nq, nkv, d, block, page, seed = (c[k] for k in ("hidden", "inter", "n_q", "n_kv", "head_dim", "block", "page", "seed"))
+    shapes = gen.layer_shapes(H, I, nq, nkv, d)
+    dev, host = {}, {}
+    for i, (nm, shp) in enumerate(shapes):
+        dev[nm], host[nm] = fill_bf16(shp, seed, i)
+    # S5
+    prm = {nm: torch.empty_like(t) for nm, t in dev.items()}
+    sh = C.cloak_block_shape(H, I, nq, nkv, d, C.CLOAK_BF16, 0)
+    C.cloak_permute_mlp_heads(KEY, sh, **dev, **{k + "_o": v for k, v in prm.items()})
+    pi = O.mlp_perm(KEY, 0, I)
+    kappa, eta = O.head_maps(KEY, 0, nq, nkv)
+    ref = dict(zip(("gate", "up", "down"), O.permute_mlp(host["gate"], host["up"], host["down"], pi)))
+    ref.update(zip(("q", "k", "v", "o"), O.permute_heads(host["q"], host["k"], host["v"], host["o"], kappa, eta, d)))
+    for nm in ref:
+        assert np.array_equal(bits(prm[nm]), ref[nm]), nm
+    # S3 + S2 + S4
+    sizes = [2 * n * k for _, (n, k) in shapes]
+    offs, total = C.cloak_arena_plan(KEY, sizes, block)
+    o_offs, o_total, _ = O.arena_plan(KEY, sizes, block)
+    assert offs == o_offs and total == o_total == 436207616
+    g = O.pool_geometry(total, block, page)
+    ta, tb = O.pool_tables(KEY, g), O.pool_tables(0x5678, g)
+    assert (g.nb, g.npages) == (6656, 208)
+    with Pool(total, block, page, KEY) as pa, Pool(total, block, page, 0x5678) as pb:
+        assert pa.info["is_vmm"]
+        bp, bi, pp, pinv = pa.tables()
+        assert np.array_equal(bp, ta.blockperm) and np.array_equal(bi, ta.blockinv)
+        assert np.array_equal(pp, ta.pageperm) and np.array_equal(pinv, ta.pageinv)
+        refV = np.zeros(g.nslots * block, np.uint8)
+        for (nm, _), o in zip(shapes, offs):
+            C.cloak_shuffle(pa.h, prm[nm], o, prm[nm].numel() * 2)
+            O.shuffle_into(refV, ta.T_vmm, ref[nm].view(np.uint8).ravel(), o, block)
+        assert np.array_equal(pa.raw(), refV)                                   # the VA view V
+        assert np.array_equal(pa.dump(), O.dump_view(refV, g, ta.pageinv))      # pages in physical (creation) order
+        # S8
+        C.cloak_relayout(pa.h, pb.h)
+        assert np.array_equal(pb.raw(), O.relayout(refV, ta.T_vmm, tb.T_vmm, g))
+        # S6, as bench.py launches it
+        tens = {nm: C.cloak_tensor(o, shp[0], shp[1], C.CLOAK_BF16, C.CLOAK_ROWMAJOR) for (nm, shp), o in zip(shapes, offs)}
+        for batch in (1, 4, 16):
+            X, dX = {}, {}
+            for j, k in enumerate((H, I)):
+                dX[k], X[k] = fill_bf16((batch, k), seed + 100, 2 * batch + j, kind=gen.KIND_NORMAL)
+            Y = {nm: torch.zeros(batch, shp[0], dtype=torch.bfloat16, device="cuda") for nm, shp in shapes}
+            ops = C.cloak_gemv_ops([(tens[nm], dX[k], Y[nm], 0) for nm, (n, k) in shapes])
+            C.cloak_gemv_chain(pa.h, ops, batch)
+            torch.cuda.synchronize()
+            first = {nm: y.clone() for nm, y in Y.items()}
+            for nm, (n, k) in shapes:
+                err = O.err_normwise(Y[nm].float().cpu().numpy(), O.linear_f64(X[k], ref[nm]))
+                assert err <= TOL_BF16, (nm, batch, err)
+            gph = torch.cuda.CUDAGraph()                                        # the replayed graph computes the same
+            with torch.cuda.graph(gph):
+                C.cloak_gemv_chain(pa.h, ops, batch)
+            for y in Y.values():
+                y.zero_()
+            gph.replay()
+            torch.cuda.synchronize()
+            assert all(torch.equal(Y[nm], first[nm]) for nm in Y)
+            del gph
+        # S4^-1
+        for (nm, _), o in zip(shapes, offs):
+            back = torch.zeros_like(prm[nm])
+            C.cloak_unshuffle(pa.h, back, o, back.numel() * 2)
+            assert torch.equal(back, prm[nm]), nm
+
+
+# ------------------------------------------------------------------ cfg2: the 16 GB model pool
+def _permuted_layer(cfg, l, tid):
+    """One layer: generator -> S5 on the GPU and in the oracle; returns (device permuted, host permuted bit arrays)."""
+    c = gen.CONFIGS[cfg]
+    H, I, nq, nkv, d = (c[k] for k in ("hidden", "inter", "n_q", "n_kv", "head_dim"))
+    shapes = gen.layer_shapes(H, I, nq, nkv, d)
+    dev, host = {}, {}
+    for nm, shp in shapes:
+        dev[nm], host[nm] = fill_bf16(shp, c["seed"], tid[f"l{l}.{nm}"])
+    prm = {nm: torch.empty_like(t) for nm, t in dev.items()}
+    sh = C.cloak_block_shape(H, I, nq, nkv, d, C.CLOAK_BF16, l)
+    C.cloak_permute_mlp_heads(KEY, sh, **dev, **{k + "_o": v for k, v in prm.items()})
+    pi = O.mlp_perm(KEY, l, I)
+    kappa, eta = O.head_maps(KEY, l, nq, nkv)
+    ref = dict(zip(("gate", "up", "down"), O.permute_mlp(host["gate"], host["up"], host["down"], pi)))
+    ref.update(zip(("q", "k", "v", "o"), O.permute_heads(host["q"], host["k"], host["v"], host["o"], kappa, eta, d)))
+    for nm in ref:
+        assert np.array_equal(bits(prm[nm]), ref[nm]), (l, nm)
+    return prm, ref, host
+
+
+def test_cfg2_model_pool_tables_bytes_and_decode_chain():
+    """cfg2 at full size: tensor order over 226 tensors, the 245 056-block / 7 658-page tables, the pool bytes of
+    layers 0, 15, 31 and lm_head, and those layers' decode chain (one cloak_gemv_chain: q,k,v | o | gate | up with
+    the fused silu*up epilogue | down waiting for it) + lm_head at batch 1 against the fp64 oracle."""
+    c = gen.CONFIGS[2]
+    H, I, nq, d, block, page, seed = (c[k] for k in ("hidden", "inter", "n_q", "head_dim", "block", "page", "seed"))
+    tensors = gen.model_tensors(2)
+    tid = {nm: i for i, (nm, _) in enumerate(tensors)}
+    sizes = [2 * n * k for _, (n, k) in tensors]
+    offs, total = C.cloak_arena_plan(KEY, sizes, block)
+    o_offs, o_total, _ = O.arena_plan(KEY, sizes, block)
+    assert offs == o_offs and total == o_total and sum(sizes) == 16059990016
+    off = {nm: o for (nm, _), o in zip(tensors, offs)}
+    g = O.pool_geometry(total, block, page)
+    assert (g.nb, g.npages) == (245056, 7658)
+    t = O.pool_tables(KEY, g)
+    with Pool(total, block, page, KEY) as p:
+        assert p.info["is_vmm"]
+        bp, bi, pp, pinv = p.tables()
+        assert np.array_equal(bp, t.blockperm) and np.array_equal(bi, t.blockinv)
+        assert np.array_equal(pp, t.pageperm) and np.array_equal(pinv, t.pageinv)
+        assert np.array_equal(p.table_T(), t.T_vmm[:g.nb])
+        xh_d, xh = fill_bf16((1, H), seed + 100, 0, kind=gen.KIND_NORMAL)
+        xa_d, xa = fill_bf16((1, nq * d), seed + 100, 1, kind=gen.KIND_NORMAL)
+        T = {nm: C.cloak_tensor(off[nm], shp[0], shp[1], C.CLOAK_BF16, C.CLOAK_ROWMAJOR) for nm, shp in tensors}
+        for l in (0, 15, 31):
+            prm, ref, host = _permuted_layer(2, l, tid)
+            for nm in prm:
+                C.cloak_shuffle(p.h, prm[nm], off[f"l{l}.{nm}"], prm[nm].numel() * 2)
+            for nm in ("k", "o", "down"):            # bytes where the table says (one small, one square, one large tensor)
+                check_tensor_in_pool(p, t.T_vmm, ref[nm].view(np.uint8).ravel(), off[f"l{l}.{nm}"], block)
+            y = {nm: torch.zeros(1, w.shape[0], dtype=torch.bfloat16, device="cuda") for nm, w in prm.items()}
+            act = torch.zeros(1, I, dtype=torch.bfloat16, device="cuda")
+            pre = f"l{l}."
+            ops = [(T[pre + nm], xh_d, y[nm], 0) for nm in ("q", "k", "v")]
+            ops += [(T[pre + "o"], xa_d, y["o"], 0), (T[pre + "gate"], xh_d, y["gate"], 0),
+                    (T[pre + "up"], xh_d, y["up"], 0, y["gate"], act), (T[pre + "down"], act, y["down"], 1)]
+            C.cloak_gemv_chain(p.h, ops, 1)
+            torch.cuda.synchronize()
+            for nm in ("q", "k", "v", "gate", "up"):
+                err = O.err_normwise(y[nm].float().cpu().numpy(), O.linear_f64(xh, ref[nm]))
+                assert err <= TOL_BF16, (l, nm, err)
+            assert O.err_normwise(y["o"].float().cpu().numpy(), O.linear_f64(xa, ref["o"])) <= TOL_BF16
+            # the permuted MLP equals the UNpermuted one (O9), fp64 all the way
+            err = O.err_normwise(y["down"].float().cpu().numpy(), O.mlp_f64(xh, host["gate"], host["up"], host["down"]))
+            assert err <= TOL_BF16, (l, "mlp", err)
+            del prm, ref, host
+        w_d, w = fill_bf16(tensors[-1][1], seed, tid["lm_head"])
+        C.cloak_shuffle(p.h, w_d, off["lm_head"], w_d.numel() * 2)
+        check_tensor_in_pool(p, t.T_vmm, w.view(np.uint8).ravel(), off["lm_head"], block)
+        y = torch.zeros(1, w.shape[0], dtype=torch.bfloat16, device="cuda")
+        C.cloak_gemv_chain(p.h, [(T["lm_head"], xh_d, y, 0)], 1)
+        assert O.err_normwise(y.float().cpu().numpy(), O.linear_f64(xh, w)) <= TOL_BF16
+        # a slot nothing was shuffled into is still zero (G4): the embedding's first block
+        assert not read_slots(p, t.T_vmm[off["embed"] // block:off["embed"] // block + 1], block).any()
+
+
+# ------------------------------------------------------------------ cfg3: the 62 GB TILE128 pool, tcgen05 GEMM
+def test_cfg3_tile128_pool_tables_bytes_and_gemm():
+    """cfg3 at full size: the 952 320-block / 29 760-page tables, and for layers 0, 63 and two seeded random layers
+    the TILE128 pool bytes (q, down) and cloak_gemm at batch 32 and 128 on every projection, checked on 1 024 seeded
+    output rows per tensor against the fp64 oracle ("cfg3 checks layers 0, 63 and two seeded random
+    ones")."""
+    c = gen.CONFIGS[3]
+    H, I, nq, d, block, page, seed = (c[k] for k in ("hidden", "inter", "n_q", "head_dim", "block", "page", "seed"))
+    tensors = gen.model_tensors(3)
+    tid = {nm: i for i, (nm, _) in enumerate(tensors)}
+    sizes = [2 * n * k for _, (n, k) in tensors]
+    offs, total = C.cloak_arena_plan(KEY, sizes, block)
+    o_offs, o_total, _ = O.arena_plan(KEY, sizes, block)
+    assert offs == o_offs and total == o_total == 62411243520
+    off = {nm: o for (nm, _), o in zip(tensors, offs)}
+    g = O.pool_geometry(total, block, page)
+    assert (g.nb, g.npages) == (952320, 29760)
+    t = O.pool_tables(KEY, g)
+    layers = [0, 63] + sorted(int(x) for x in np.random.default_rng(seed).choice(np.arange(1, 63), 2, replace=False))
+    with Pool(total, block, page, KEY) as p:
+        bp, bi, pp, pinv = p.tables()
+        assert np.array_equal(bp, t.blockperm) and np.array_equal(bi, t.blockinv)
+        assert np.array_equal(pp, t.pageperm) and np.array_equal(pinv, t.pageinv)
+        X, dX = {}, {}
+        for batch in (32, 128):
+            for j, k in enumerate(sorted({H, I})):
+                dX[batch, k], X[batch, k] = fill_bf16((batch, k), seed + 100, 2 * batch + j, kind=gen.KIND_NORMAL)
+        for l in layers:
+            prm, ref, _ = _permuted_layer(3, l, tid)
+            for nm, w in prm.items():
+                n, k = w.shape
+                til = torch.empty_like(w)
+                C.cloak_to_tile128(w, til, n, k, C.CLOAK_BF16)
+                C.cloak_shuffle(p.h, til, off[f"l{l}.{nm}"], n * k * 2)
+                if nm in ("q", "down"):
+                    check_tensor_in_pool(p, t.T_vmm, O.to_tile128(ref[nm]).view(np.uint8), off[f"l{l}.{nm}"], block)
+                del til
+            for nm, w in prm.items():
+                n, k = w.shape
+                rows = sample_rows(n, 1024, seed * 1000 + l)
+                for batch in (32, 128):
+                    y = torch.zeros(batch, n, dtype=torch.bfloat16, device="cuda")
+                    C.cloak_gemm(p.h, C.cloak_tensor(off[f"l{l}.{nm}"], n, k, C.CLOAK_BF16, C.CLOAK_TILE128), dX[batch, k], y, batch)
+                    got = y.float().cpu().numpy()[:, rows]
+                    err = O.err_normwise(got, O.linear_f64(X[batch, k], ref[nm][rows]))
+                    assert err <= TOL_BF16, (l, nm, batch, err)
+            del prm, ref
+
+
+# ------------------------------------------------------------------ cfg4: 4 GiB at five block sizes
+@pytest.mark.parametrize("block", gen.CONFIGS[4]["blocks"])
+def test_cfg4_granularity_sweep_bit_exact(block):
+    """cfg4: V after cloak_shuffle, the re-laid-out pool under key B, and the round trip, bit for bit against the
+    oracle over the whole 4 GiB buffer at each block size."""
+    c = gen.CONFIGS[4]
+    nbytes, page = c["bytes"], c["page"]
+    g = O.pool_geometry(nbytes, block, page)
+    ta, tb = O.pool_tables(c["key"], g), O.pool_tables(c["key_b"], g)
+    L_d = synth_cuda.fill(torch.empty(nbytes // 2, dtype=torch.bfloat16, device="cuda"), c["seed"], 0)
+    L = L_d.view(torch.uint8).cpu().numpy()
+    for start in (0, nbytes // 4 - 8192, nbytes // 2 - 4096):                 # elements; numpy twin of the generator
+        assert np.array_equal(L.view(np.uint16)[start:start + 4096], gen.synth_bf16_bits(c["seed"], 0, start, 4096))
+    with Pool(nbytes, block, page, c["key"]) as pa, Pool(nbytes, block, page, c["key_b"]) as pb:
+        assert np.array_equal(pa.table_T(), ta.T_vmm) and np.array_equal(pb.table_T(), tb.T_vmm)
+        C.cloak_shuffle(pa.h, L_d, 0, nbytes)
+        V = O.shuffle_va(L, g, ta.blockinv)
+        assert np.array_equal(pa.raw(), V)
+        C.cloak_relayout(pa.h, pb.h)
+        assert np.array_equal(pb.raw(), O.relayout(V, ta.T_vmm, tb.T_vmm, g))
+        del V
+        back = torch.zeros_like(L_d)
+        C.cloak_unshuffle(pb.h, back, 0, nbytes)
+        assert torch.equal(back, L_d)
