@@ -39,6 +39,7 @@ struct GemmArgs {
     uint32_t tmem_cols;  // power of two >= 2*batch
     float* part;         // [tile row][maxc][batch][128]
     uint32_t* counters;
+    uint32_t early;      // 1: W unchanged since before the preceding kernel -> stream it ahead of griddepcontrol.wait
 };
 
 constexpr int GM_THREADS = 224;            // warp 0 TMA (W), warp 1 MMA, warp 2 TMA (X), warps 3..6 epilogue
@@ -71,6 +72,10 @@ __device__ __forceinline__ void tc_ld16(uint32_t taddr, uint32_t (&r)[16]) {
 __device__ __forceinline__ uint64_t umma_desc_sw128(uint32_t smem_addr) {
     return (uint64_t)((smem_addr & 0x3FFFF) >> 4) | ((uint64_t)(1024 >> 4) << 32) | (1ull << 46) | (2ull << 61);
 }
+// Programmatic dependent launch, as in gemv_stream.cu: W (immutable during decode) may be fetched while the stream
+// predecessor drains; X, Y, partials and counters wait.  The trigger comes after this grid's own wait.
+__device__ __forceinline__ void gm_dep_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
+__device__ __forceinline__ void gm_dep_launch() { asm volatile("griddepcontrol.launch_dependents;" ::: "memory"); }
 __device__ __forceinline__ void epi_bar() { asm volatile("bar.sync 1, 128;" ::: "memory"); }
 
 __global__ void __launch_bounds__(GM_THREADS, 1) gemm_tile128_kernel(const __grid_constant__ CUtensorMap map_w,
@@ -116,6 +121,7 @@ __global__ void __launch_bounds__(GM_THREADS, 1) gemm_tile128_kernel(const __gri
 
     if (warp == 0 && lane == 0 && ubeg < uend) {
         // ---------------------------------------------------------------- TMA producer, weight tiles (through T)
+        if (!a.early) gm_dep_wait();
         uint32_t it = 0;
         for (uint32_t u = ubeg; u < uend; ++u, ++it) {
             const uint32_t s = it % a.wstages, f = it / a.wstages;
@@ -132,6 +138,7 @@ __global__ void __launch_bounds__(GM_THREADS, 1) gemm_tile128_kernel(const __gri
         }
     } else if (warp == 2 && lane == 0 && ubeg < uend) {
         // ---------------------------------------------------------------- TMA producer, activation tiles (L2-resident)
+        gm_dep_wait();
         uint32_t it = 0;
         for (uint32_t u = ubeg; u < uend; ++u, ++it) {
             const uint32_t s = it % a.xstages, f = it / a.xstages;
@@ -183,6 +190,8 @@ __global__ void __launch_bounds__(GM_THREADS, 1) gemm_tile128_kernel(const __gri
         // ---------------------------------------------------------------- epilogue (4 warps = 4 TMEM lane quarters)
         const uint32_t q = warp & 3, r = q * 32 + lane;
         const int etid = threadIdx.x - 96;
+        gm_dep_wait();
+        if (etid == 0) gm_dep_launch();
         uint32_t seg = 0;
         for (uint32_t u = ubeg; u < uend; ++seg) {
             const uint32_t tn = u / a.kt;
@@ -263,6 +272,7 @@ static cloak_status make_map(CUtensorMap* map, const void* base, uint64_t inner,
     return CLOAK_OK;
 }
 
+extern bool g_gemv_pdl;      // gemv_stream.cu: the PDL A/B switch (cloak_set_gemv_engine(2) turns it off)
 cloak_status check_linear(const cloak_pool* pool, const cloak_tensor* w, const void* x, void* y, const char* who);
 
 }  // namespace cloak
@@ -305,7 +315,11 @@ extern "C" cloak_status cloak_gemm(const cloak_pool* pool, const cloak_tensor* w
     a.units = (uint32_t)units64;
     const int sms = sm_count(pool->device);
     a.per = (a.units + sms - 1) / sms;
-    if (a.per < (a.kt + 3) / 4) a.per = (a.kt + 3) / 4;      // at most ~5 contributors per tile row (partials traffic)
+    {   // cap the contributors per tile row (fp32 partials are batch * 512 B per contributor): ~10 at batch 32, ~4 at 128
+        uint32_t cap = 512 / batch;
+        cap = cap < 4 ? 4 : (cap > 10 ? 10 : cap);
+        if (a.per < (a.kt + cap - 1) / cap) a.per = (a.kt + cap - 1) / cap;
+    }
     const int ctas = (int)((a.units + a.per - 1) / a.per);
     a.maxc = (a.kt + a.per - 1) / a.per + 1;
     const uint32_t xtile = batch * 256;
@@ -329,8 +343,19 @@ extern "C" cloak_status cloak_gemm(const cloak_pool* pool, const cloak_tensor* w
         CLOAK_CUDA(cudaFuncSetAttribute(gemm_tile128_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 226 * 1024));
         attr_set = true;
     }
-    gemm_tile128_kernel<<<ctas, GM_THREADS, smem, s>>>(pool->tmap_tile128, map_x, a);
+    a.early = (g_gemv_pdl && !pool->dirty) ? 1u : 0u;
+    if (pool->dirty && pool->dirty_stream == s) pool->dirty = false;   // this launch waits for the writer in full
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = dim3(ctas);
+    cfg.blockDim = dim3(GM_THREADS);
+    cfg.dynamicSmemBytes = smem;
+    cfg.stream = s;
+    cudaLaunchAttribute at[1];
+    at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    at[0].val.programmaticStreamSerializationAllowed = 1;
+    cfg.attrs = at;
+    cfg.numAttrs = g_gemv_pdl ? 1 : 0;
+    CLOAK_CUDA(cudaLaunchKernelEx(&cfg, gemm_tile128_kernel, pool->tmap_tile128, map_x, a));
     launched();
-    CLOAK_LAUNCH_CHECK();
     return CLOAK_OK;
 }
