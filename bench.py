@@ -28,6 +28,10 @@ import numpy as np  # noqa: E402
 METRIC = "shuffle GB/s and cloaked decode GEMV GB/s (frac of HBM peak); cloaked-vs-native overhead %"
 BATCHES = (1, 4, 16)
 KEY_A, KEY_B = 0x1234, 0x5678          # G11
+# dram__bytes_read.sum + dram__bytes_write.sum of one gemv_chain_kernel launch (the 7 projections at one batch), mean of
+# the three launches of a step in the committed `ncu --set full` capture; algorithmic bytes are 436 207 616.
+NCU_TRAFFIC_PER_LAUNCH = 442.3e6
+NCU_TRAFFIC_SOURCE = "profiles/r1_ncu_full_gemv_chain.md"
 FALLBACK_HBM_GBS = 6650.0              # B200_PROFILING.md fallback when MEASURED_PEAKS.json is absent
 
 
@@ -348,7 +352,7 @@ def run_cloak(args):
         rn, _ = capture(lambda: gemv_chain(pool_n, b))
         rc, _ = capture(lambda: gemv_chain(pool_a, b))
         rp, _ = capture(lambda: gemv_chain(pool_a, b, per_call=True))
-        reps = max(args.steps, 20)
+        reps = max(args.steps, 5)
         tn, tc, tp = [], [], []
         for r_, acc_ in ((rn, tn), (rc, tc), (rp, tp)):
             for _ in range(3):
@@ -438,7 +442,8 @@ def run_cloak(args):
         "hbm_peak_gbs": peak, "hbm_peak_kind": peak_kind, "hbm_nominal_gbs": 8000.0,
         "pool_map_ms": map_ms, "pool_create_s": pool_create_s, "roundtrip_bit_exact": bool(ok),
         "roofline": {"bound": "hbm", "kernel": "gemv_stream_kernel", "achieved": achieved, "peak": peak, "unit": "GB/s",
-                     "frac": achieved / peak, "traffic": None, "launches_per_step": gemv_launches,
+                     "frac": achieved / peak, "traffic": NCU_TRAFFIC_PER_LAUNCH, "traffic_source": NCU_TRAFFIC_SOURCE,
+                     "launches_per_step": gemv_launches,
                      "bytes_per_launch": sb["gemv"] / gemv_launches, "avg_launch_us": gemv_ms / gemv_launches * 1e3,
                      "peak_kind": peak_kind},
         "clocks": clk, "e2e": e2e, "gpu_launches": int(launches),
