@@ -152,6 +152,17 @@ cloak_status cloak_permute_mlp_heads(uint64_t key, const cloak_block_shape* shap
                                      void* d_gate_o, void* d_up_o, void* d_down_o,
                                      void* d_q_o, void* d_k_o, void* d_v_o, void* d_o_o, void* stream);
 
+/* ---- S5 + S4 in one pass: the fused load path (the layout is decided before
+ * any weight lands).  Same permutation as cloak_permute_mlp_heads, but every permuted tensor is written straight into
+ * `pool` through its block table at arena byte offset h_offsets[i] (i = gate, up, down, q, k, v, o; a block
+ * multiple; ignored where the source is NULL), CLOAK_ROWMAJOR.  The pool bytes afterwards equal those of
+ * cloak_permute_mlp_heads followed by cloak_shuffle of each tensor (the tail of a final partial block is zeroed),
+ * at 2 bytes of traffic per payload byte instead of 4.  h_offsets is a HOST array of 7.  Asynchronous on `stream`. */
+cloak_status cloak_load_mlp_heads(uint64_t key, const cloak_block_shape* shape, cloak_pool* pool,
+                                  const void* d_gate, const void* d_up, const void* d_down,
+                                  const void* d_q, const void* d_k, const void* d_v, const void* d_o,
+                                  const uint64_t* h_offsets, void* stream);
+
 /* Storage-layout conversion ROWMAJOR -> TILE128 of a logical [N, K] matrix (N, K multiples of 128).
  * Out of place.  Asynchronous on `stream`. */
 cloak_status cloak_to_tile128(const void* d_src, void* d_dst, uint32_t N, uint32_t K, cloak_dtype dt,

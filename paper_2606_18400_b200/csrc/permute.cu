@@ -53,9 +53,29 @@ __device__ __forceinline__ int4 ldg_stream(const void* p) {
     return r;
 }
 
+// Where a gathered 16-byte vector goes.  PlainDst: a caller-owned tensor.  PoolDst: straight into a pool through its
+// block table (the fused load path: permutation and block scatter in ONE pass over the bytes
+// instead of two) -- vector index v of the tensor is arena byte off + 16 v, translated like every other access.
+struct PlainDst {
+    int4* p;
+    __device__ __forceinline__ void store(uint64_t v, const int4& x) const { p[v] = x; }
+};
+struct PoolDst {
+    char* pool;
+    const uint32_t* T;
+    uint64_t off;
+    uint32_t log2b;
+    __device__ __forceinline__ void store(uint64_t v, const int4& x) const {
+        const uint64_t a = off + (v << 4);
+        const uint32_t slot = __ldg(T + (a >> log2b));
+        *reinterpret_cast<int4*>(pool + ((uint64_t)slot << log2b) + (a & ((1ull << log2b) - 1))) = x;
+    }
+};
+
 // dst row r' <- src row map[r' / seg] * seg + r' % seg;  rows of vpr 16-byte vectors.
 constexpr int ROWS_PER_IT = 4;
-__global__ void __launch_bounds__(256) gather_rows_kernel(const int4* __restrict__ src, int4* __restrict__ dst,
+template <typename Dst>
+__global__ void __launch_bounds__(256) gather_rows_kernel(const int4* __restrict__ src, Dst dst,
                                                           const uint32_t* __restrict__ map, uint32_t seg,
                                                           uint32_t nrows, uint32_t vpr) {
     for (uint32_t r0 = blockIdx.x * ROWS_PER_IT; r0 < nrows; r0 += gridDim.x * ROWS_PER_IT) {
@@ -72,7 +92,7 @@ __global__ void __launch_bounds__(256) gather_rows_kernel(const int4* __restrict
                 if (r0 + k < nrows) x[k] = ldg_stream(src + (uint64_t)srow[k] * vpr + v);
 #pragma unroll
             for (int k = 0; k < ROWS_PER_IT; ++k)
-                if (r0 + k < nrows) dst[(uint64_t)(r0 + k) * vpr + v] = x[k];
+                if (r0 + k < nrows) dst.store((uint64_t)(r0 + k) * vpr + v, x[k]);
         }
     }
 }
@@ -82,8 +102,8 @@ __global__ void __launch_bounds__(256) gather_rows_kernel(const int4* __restrict
 // Dynamic shared memory: colmap[ncols] followed by a ring of NS source rows.  One elected thread keeps the ring
 // full with one bulk copy (TMA 1-D, mbarrier completion) per row, so the DRAM latency of row r+1.. hides behind the
 // shared-memory gather of row r; the gathered vectors go out as coalesced 16-byte stores.
-template <typename E, typename M>
-__global__ void __launch_bounds__(512) gather_cols_kernel(const E* __restrict__ src, E* __restrict__ dst,
+template <typename E, typename M, typename Dst>
+__global__ void __launch_bounds__(512) gather_cols_kernel(const E* __restrict__ src, Dst dst,
                                                           const uint32_t* __restrict__ map, uint32_t seg,
                                                           uint32_t nrows, uint32_t ncols, uint32_t ns) {
     extern __shared__ __align__(128) unsigned char sm[];
@@ -112,12 +132,12 @@ __global__ void __launch_bounds__(512) gather_cols_kernel(const E* __restrict__ 
         const uint32_t st = k % ns;
         mbar_wait(smem_u32(&full[st]), (k / ns) & 1);
         const E* row = reinterpret_cast<const E*>(ring + (size_t)st * row_bytes);
-        int4* d4 = reinterpret_cast<int4*>(dst + (uint64_t)(blockIdx.x + k * gridDim.x) * ncols);
+        const uint64_t v0 = (uint64_t)(blockIdx.x + k * gridDim.x) * vpr;
         for (uint32_t v = threadIdx.x; v < vpr; v += blockDim.x) {
             union { int4 q; E e[EPV]; } out;
 #pragma unroll
             for (int j = 0; j < EPV; ++j) out.e[j] = row[colmap[v * EPV + j]];
-            d4[v] = out.q;
+            dst.store(v0 + v, out.q);
         }
         __syncthreads();                                       // every thread is done with this stage
         if (threadIdx.x == 0 && k + ns < mine) issue(k + ns);
@@ -126,7 +146,8 @@ __global__ void __launch_bounds__(512) gather_cols_kernel(const E* __restrict__ 
 
 // Column groups that are whole 16-byte vectors (seg % (16 / sizeof(E)) == 0, e.g. heads of 128 columns): the gather
 // is a vector-level index remap, no staging needed.  vmap[v'] = source vector of destination vector v'.
-__global__ void __launch_bounds__(256) gather_colvecs_kernel(const int4* __restrict__ src, int4* __restrict__ dst,
+template <typename Dst>
+__global__ void __launch_bounds__(256) gather_colvecs_kernel(const int4* __restrict__ src, Dst dst,
                                                              const uint32_t* __restrict__ map, uint32_t vseg,
                                                              uint32_t nrows, uint32_t vpr) {
     extern __shared__ uint32_t vmap[];
@@ -141,7 +162,7 @@ __global__ void __launch_bounds__(256) gather_colvecs_kernel(const int4* __restr
                 if (r0 + k < nrows) x[k] = ldg_stream(src + (uint64_t)(r0 + k) * vpr + sv);
 #pragma unroll
             for (int k = 0; k < ROWS_PER_IT; ++k)
-                if (r0 + k < nrows) dst[(uint64_t)(r0 + k) * vpr + v] = x[k];
+                if (r0 + k < nrows) dst.store((uint64_t)(r0 + k) * vpr + v, x[k]);
         }
     }
 }
@@ -199,34 +220,49 @@ __global__ void silu_mul_bf16_kernel(const uint16_t* __restrict__ g, const uint1
     }
 }
 
-static cloak_status rows(const void* src, void* dst, const uint32_t* map, uint32_t seg, uint32_t nrows,
+template <typename Dst>
+static cloak_status rows(const void* src, Dst dst, const uint32_t* map, uint32_t seg, uint32_t nrows,
                          uint64_t row_bytes, int sms, cudaStream_t s) {
     uint32_t ctas = (nrows + ROWS_PER_IT - 1) / ROWS_PER_IT;
     const uint32_t cap = (uint32_t)sms * 8;
     if (ctas > cap) ctas = cap;
-    gather_rows_kernel<<<ctas, 256, 0, s>>>((const int4*)src, (int4*)dst, map, seg, nrows, (uint32_t)(row_bytes / 16));
+    gather_rows_kernel<Dst><<<ctas, 256, 0, s>>>((const int4*)src, dst, map, seg, nrows, (uint32_t)(row_bytes / 16));
     launched();
     CLOAK_LAUNCH_CHECK();
     return CLOAK_OK;
 }
 
-template <typename E, typename M>
-static cloak_status cols_ring(const void* src, void* dst, const uint32_t* map, uint32_t seg, uint32_t nrows, uint32_t ncols,
+template <typename E, typename M, typename Dst>
+static cloak_status cols_ring(const void* src, Dst dst, const uint32_t* map, uint32_t seg, uint32_t nrows, uint32_t ncols,
                               size_t smem, uint32_t ns, int sms, cudaStream_t s) {
     static bool attr_set = false;
     if (!attr_set) {
-        CLOAK_CUDA(cudaFuncSetAttribute(gather_cols_kernel<E, M>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024));
+        CLOAK_CUDA(cudaFuncSetAttribute(gather_cols_kernel<E, M, Dst>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024));
         attr_set = true;
     }
     const uint32_t ctas = nrows < (uint32_t)sms ? nrows : (uint32_t)sms;
-    gather_cols_kernel<E, M><<<ctas, 512, smem, s>>>((const E*)src, (E*)dst, map, seg, nrows, ncols, ns);
+    gather_cols_kernel<E, M, Dst><<<ctas, 512, smem, s>>>((const E*)src, dst, map, seg, nrows, ncols, ns);
     launched();
     CLOAK_LAUNCH_CHECK();
     return CLOAK_OK;
 }
 
+// Only a caller-owned tensor can take the element-by-element fallback.
 template <typename E>
-static cloak_status cols(const void* src, void* dst, const uint32_t* map, uint32_t seg, uint32_t nrows, uint32_t ncols,
+static cloak_status cols_fallback(const void* src, PlainDst dst, const uint32_t* map, uint32_t seg, uint32_t nrows,
+                                  uint32_t ncols, int sms, cudaStream_t s) {
+    gather_cols_global_kernel<E><<<sms * 8, 256, 0, s>>>((const E*)src, (E*)dst.p, map, seg, nrows, ncols);
+    launched();
+    CLOAK_LAUNCH_CHECK();
+    return CLOAK_OK;
+}
+template <typename E>
+static cloak_status cols_fallback(const void*, PoolDst, const uint32_t*, uint32_t, uint32_t, uint32_t, int, cudaStream_t) {
+    return fail(CLOAK_ERR_UNSUPPORTED, "load: a row of this tensor does not fit the shared-memory ring of the column gather");
+}
+
+template <typename E, typename Dst>
+static cloak_status cols(const void* src, Dst dst, const uint32_t* map, uint32_t seg, uint32_t nrows, uint32_t ncols,
                          int sms, cudaStream_t s) {
     constexpr uint32_t EPV = 16 / sizeof(E);
     const size_t row_bytes = (size_t)ncols * sizeof(E);
@@ -234,7 +270,7 @@ static cloak_status cols(const void* src, void* dst, const uint32_t* map, uint32
         const uint32_t vpr = ncols / EPV;
         uint32_t ctas = (nrows + ROWS_PER_IT - 1) / ROWS_PER_IT;
         if (ctas > (uint32_t)sms * 8) ctas = (uint32_t)sms * 8;
-        gather_colvecs_kernel<<<ctas, 256, (size_t)vpr * 4, s>>>((const int4*)src, (int4*)dst, map, seg / EPV, nrows, vpr);
+        gather_colvecs_kernel<Dst><<<ctas, 256, (size_t)vpr * 4, s>>>((const int4*)src, dst, map, seg / EPV, nrows, vpr);
         launched();
         CLOAK_LAUNCH_CHECK();
         return CLOAK_OK;
@@ -246,18 +282,80 @@ static cloak_status cols(const void* src, void* dst, const uint32_t* map, uint32
     if (ns > 6) ns = 6;
     if (ns >= 2) {
         const size_t smem = cm + (size_t)ns * row_bytes;
-        return msz == 2 ? cols_ring<E, uint16_t>(src, dst, map, seg, nrows, ncols, smem, ns, sms, s)
-                        : cols_ring<E, uint32_t>(src, dst, map, seg, nrows, ncols, smem, ns, sms, s);
+        return msz == 2 ? cols_ring<E, uint16_t, Dst>(src, dst, map, seg, nrows, ncols, smem, ns, sms, s)
+                        : cols_ring<E, uint32_t, Dst>(src, dst, map, seg, nrows, ncols, smem, ns, sms, s);
     }
-    gather_cols_global_kernel<E><<<sms * 8, 256, 0, s>>>((const E*)src, (E*)dst, map, seg, nrows, ncols);
-    launched();
-    CLOAK_LAUNCH_CHECK();
-    return CLOAK_OK;
+    return cols_fallback<E>(src, dst, map, seg, nrows, ncols, sms, s);
 }
 
 }  // namespace cloak
 
 using namespace cloak;
+
+namespace cloak {
+
+static cloak_status check_shape(const cloak_block_shape* sh, bool mlp, bool heads, const char* who) {
+    const uint32_t e = sh->dt == CLOAK_F32 ? 4 : 2;
+    const uint32_t epv = 16 / e;
+    if (sh->hidden == 0 || sh->hidden % epv) return fail(CLOAK_ERR_ALIGN, "%s: hidden must be a multiple of %u", who, epv);
+    if (mlp && (sh->inter == 0 || sh->inter % epv)) return fail(CLOAK_ERR_ALIGN, "%s: inter must be a multiple of %u", who, epv);
+    if (heads) {
+        if (sh->n_q == 0 || sh->n_kv == 0 || sh->head_dim == 0 || sh->n_q % sh->n_kv)
+            return fail(CLOAK_ERR_INVALID, "%s: n_q must be a non-zero multiple of n_kv, head_dim > 0", who);
+        if (sh->n_kv > 1024 || sh->n_q / sh->n_kv > 1024) return fail(CLOAK_ERR_UNSUPPORTED, "%s: more than 1024 KV heads or group size", who);
+        if ((sh->n_q * sh->head_dim) % epv) return fail(CLOAK_ERR_ALIGN, "%s: n_q*head_dim must be a multiple of %u", who, epv);
+    }
+    return CLOAK_OK;
+}
+
+// The permutation proper.  in[i] (gate, up, down, q, k, v, o) may be NULL to skip a tensor; mk(i) says where tensor i goes.
+template <typename MakeDst>
+static cloak_status permute_impl(uint64_t key, const cloak_block_shape* sh, const void* const in[7], MakeDst mk, int dev,
+                                 cudaStream_t s) {
+    const bool mlp = in[0] || in[1] || in[2], heads = in[3] || in[4] || in[5] || in[6];
+    const uint32_t e = sh->dt == CLOAK_F32 ? 4 : 2;
+    const int sms = sm_count(dev);
+    const size_t n_scratch = (size_t)(mlp ? sh->inter : 0) + (heads ? sh->n_kv + sh->n_q : 0);
+    uint32_t* scratch = nullptr;
+    CLOAK_CUDA(cudaMallocAsync((void**)&scratch, n_scratch * 4, s));
+    uint32_t* pi = scratch;
+    uint32_t* kappa = scratch + (mlp ? sh->inter : 0);
+    uint32_t* eta = kappa + sh->n_kv;
+    cloak_status st = CLOAK_OK;
+    const uint64_t hrow = (uint64_t)sh->hidden * e;
+    if (mlp) {
+        st = keygen_device(key, (4ull << 32) | sh->layer, sh->inter, pi, nullptr, s);
+        if (st == CLOAK_OK && in[0]) st = rows(in[0], mk(0), pi, 1, sh->inter, hrow, sms, s);
+        if (st == CLOAK_OK && in[1]) st = rows(in[1], mk(1), pi, 1, sh->inter, hrow, sms, s);
+        if (st == CLOAK_OK && in[2])
+            st = e == 4 ? cols<uint32_t>(in[2], mk(2), pi, 1, sh->hidden, sh->inter, sms, s)
+                        : cols<uint16_t>(in[2], mk(2), pi, 1, sh->hidden, sh->inter, sms, s);
+    }
+    if (st == CLOAK_OK && heads) {
+        head_maps_kernel<<<1, 1024, 0, s>>>((uint32_t)key, (uint32_t)(key >> 32), sh->layer, sh->n_q, sh->n_kv, kappa, eta);
+        launched();
+        if (cudaGetLastError() != cudaSuccess) st = fail(CLOAK_ERR_CUDA, "permute: head_maps launch failed");
+        const uint32_t d = sh->head_dim;
+        if (st == CLOAK_OK && in[3]) st = rows(in[3], mk(3), eta, d, sh->n_q * d, hrow, sms, s);
+        if (st == CLOAK_OK && in[4]) st = rows(in[4], mk(4), kappa, d, sh->n_kv * d, hrow, sms, s);
+        if (st == CLOAK_OK && in[5]) st = rows(in[5], mk(5), kappa, d, sh->n_kv * d, hrow, sms, s);
+        if (st == CLOAK_OK && in[6])
+            st = e == 4 ? cols<uint32_t>(in[6], mk(6), eta, d, sh->hidden, sh->n_q * d, sms, s)
+                        : cols<uint16_t>(in[6], mk(6), eta, d, sh->hidden, sh->n_q * d, sms, s);
+    }
+    cudaFreeAsync(scratch, s);
+    return st;
+}
+
+// Zero the rest of the block that holds arena byte `end` (G4: the tail of a tensor's last block is zero).
+__global__ void zero_block_tail_kernel(char* pool, const uint32_t* T, uint64_t end, uint32_t log2b) {
+    const uint64_t mask = (1ull << log2b) - 1;
+    char* p = pool + ((uint64_t)T[end >> log2b] << log2b);
+    for (uint64_t o = (end & mask) + threadIdx.x * 16ull; o <= mask; o += blockDim.x * 16ull)
+        *reinterpret_cast<int4*>(p + o) = make_int4(0, 0, 0, 0);
+}
+
+}  // namespace cloak
 
 extern "C" cloak_status cloak_permute_mlp_heads(uint64_t key, const cloak_block_shape* sh, const void* d_gate,
                                                 const void* d_up, const void* d_down, const void* d_q, const void* d_k,
@@ -279,49 +377,51 @@ extern "C" cloak_status cloak_permute_mlp_heads(uint64_t key, const cloak_block_
         }
     }
     if (!any) return fail(CLOAK_ERR_INVALID, "permute: nothing to do");
-    const uint32_t e = sh->dt == CLOAK_F32 ? 4 : 2;
-    const uint32_t epv = 16 / e;
-    if (sh->hidden == 0 || sh->hidden % epv) return fail(CLOAK_ERR_ALIGN, "permute: hidden must be a multiple of %u", epv);
-    if (mlp && (sh->inter == 0 || sh->inter % epv)) return fail(CLOAK_ERR_ALIGN, "permute: inter must be a multiple of %u", epv);
-    if (heads) {
-        if (sh->n_q == 0 || sh->n_kv == 0 || sh->head_dim == 0 || sh->n_q % sh->n_kv)
-            return fail(CLOAK_ERR_INVALID, "permute: n_q must be a non-zero multiple of n_kv, head_dim > 0");
-        if (sh->n_kv > 1024 || sh->n_q / sh->n_kv > 1024) return fail(CLOAK_ERR_UNSUPPORTED, "permute: more than 1024 KV heads or group size");
-        if ((sh->n_q * sh->head_dim) % epv) return fail(CLOAK_ERR_ALIGN, "permute: n_q*head_dim must be a multiple of %u", epv);
-    }
-    cudaStream_t s = (cudaStream_t)stream;
+    cloak_status st = check_shape(sh, mlp, heads, "permute");
+    if (st != CLOAK_OK) return st;
     int dev = 0;
     CLOAK_CUDA(cudaGetDevice(&dev));
-    const int sms = sm_count(dev);
-    const size_t n_scratch = (size_t)(mlp ? sh->inter : 0) + (heads ? sh->n_kv + sh->n_q : 0);
-    uint32_t* scratch = nullptr;
-    CLOAK_CUDA(cudaMallocAsync((void**)&scratch, n_scratch * 4, s));
-    uint32_t* pi = scratch;
-    uint32_t* kappa = scratch + (mlp ? sh->inter : 0);
-    uint32_t* eta = kappa + sh->n_kv;
-    cloak_status st = CLOAK_OK;
-    const uint64_t hrow = (uint64_t)sh->hidden * e;
-    if (mlp) {
-        st = keygen_device(key, (4ull << 32) | sh->layer, sh->inter, pi, nullptr, s);
-        if (st == CLOAK_OK && d_gate) st = rows(d_gate, d_gate_o, pi, 1, sh->inter, hrow, sms, s);
-        if (st == CLOAK_OK && d_up) st = rows(d_up, d_up_o, pi, 1, sh->inter, hrow, sms, s);
-        if (st == CLOAK_OK && d_down)
-            st = e == 4 ? cols<uint32_t>(d_down, d_down_o, pi, 1, sh->hidden, sh->inter, sms, s)
-                        : cols<uint16_t>(d_down, d_down_o, pi, 1, sh->hidden, sh->inter, sms, s);
-    }
-    if (st == CLOAK_OK && heads) {
-        head_maps_kernel<<<1, 1024, 0, s>>>((uint32_t)key, (uint32_t)(key >> 32), sh->layer, sh->n_q, sh->n_kv, kappa, eta);
-        launched();
-        if (cudaGetLastError() != cudaSuccess) st = fail(CLOAK_ERR_CUDA, "permute: head_maps launch failed");
-        const uint32_t d = sh->head_dim;
-        if (st == CLOAK_OK && d_q) st = rows(d_q, d_q_o, eta, d, sh->n_q * d, hrow, sms, s);
-        if (st == CLOAK_OK && d_k) st = rows(d_k, d_k_o, kappa, d, sh->n_kv * d, hrow, sms, s);
-        if (st == CLOAK_OK && d_v) st = rows(d_v, d_v_o, kappa, d, sh->n_kv * d, hrow, sms, s);
-        if (st == CLOAK_OK && d_o)
-            st = e == 4 ? cols<uint32_t>(d_o, d_o_o, eta, d, sh->hidden, sh->n_q * d, sms, s)
-                        : cols<uint16_t>(d_o, d_o_o, eta, d, sh->hidden, sh->n_q * d, sms, s);
-    }
-    cudaFreeAsync(scratch, s);
+    return permute_impl(key, sh, in, [&](int i) { return PlainDst{static_cast<int4*>(out[i])}; }, dev, (cudaStream_t)stream);
+}
+
+extern "C" cloak_status cloak_load_mlp_heads(uint64_t key, const cloak_block_shape* sh, cloak_pool* pool,
+                                             const void* d_gate, const void* d_up, const void* d_down, const void* d_q,
+                                             const void* d_k, const void* d_v, const void* d_o, const uint64_t* h_offsets,
+                                             void* stream) {
+    if (!sh || !pool || !h_offsets) return fail(CLOAK_ERR_INVALID, "load: NULL argument");
+    if (sh->dt != CLOAK_F32 && sh->dt != CLOAK_BF16) return fail(CLOAK_ERR_UNSUPPORTED, "load: unknown dtype");
+    const void* in[7] = {d_gate, d_up, d_down, d_q, d_k, d_v, d_o};
+    bool mlp = false, heads = false;
+    for (int i = 0; i < 7; ++i)
+        if (in[i]) {
+            if ((uintptr_t)in[i] & 15) return fail(CLOAK_ERR_ALIGN, "load: tensor %d not 16-byte aligned", i);
+            (i < 3 ? mlp : heads) = true;
+        }
+    if (!mlp && !heads) return fail(CLOAK_ERR_INVALID, "load: nothing to do");
+    cloak_status st = check_shape(sh, mlp, heads, "load");
+    if (st != CLOAK_OK) return st;
+    const uint64_t e = sh->dt == CLOAK_F32 ? 4 : 2;
+    const uint64_t qd = (uint64_t)sh->n_q * sh->head_dim, kvd = (uint64_t)sh->n_kv * sh->head_dim;
+    const uint64_t bytes[7] = {(uint64_t)sh->inter * sh->hidden * e, (uint64_t)sh->inter * sh->hidden * e,
+                               (uint64_t)sh->hidden * sh->inter * e, qd * sh->hidden * e, kvd * sh->hidden * e,
+                               kvd * sh->hidden * e, (uint64_t)sh->hidden * qd * e};
+    if (pool->block < 16) return fail(CLOAK_ERR_UNSUPPORTED, "load: block_bytes must be >= 16");
+    for (int i = 0; i < 7; ++i)
+        if (in[i]) {
+            if (h_offsets[i] % pool->block) return fail(CLOAK_ERR_ALIGN, "load: offset %d is not a block multiple", i);
+            if (h_offsets[i] + bytes[i] > (uint64_t)pool->nb * pool->block) return fail(CLOAK_ERR_INVALID, "load: tensor %d exceeds the pool's arena", i);
+        }
+    DeviceGuard g(pool->device);
+    cudaStream_t s = (cudaStream_t)stream;
+    pool->wrote(s);
+    st = permute_impl(key, sh, in, [&](int i) { return PoolDst{pool->base, pool->d_T, h_offsets[i], pool->log2_block}; },
+                      pool->device, s);
+    for (int i = 0; i < 7 && st == CLOAK_OK; ++i)
+        if (in[i] && (h_offsets[i] + bytes[i]) % pool->block) {
+            zero_block_tail_kernel<<<1, 256, 0, s>>>(pool->base, pool->d_T, h_offsets[i] + bytes[i], pool->log2_block);
+            launched();
+            CLOAK_LAUNCH_CHECK();
+        }
     return st;
 }
 

@@ -213,6 +213,61 @@ def test_permute_mlp_heads_bit_exact(hidden, inter, n_q, n_kv, d, dtype, layer):
     assert not z["down"].any() and not z["q"].any()
 
 
+@pytest.mark.parametrize("hidden,inter,n_q,n_kv,d,dtype,layer,block,page", [
+    (256, 1024, 4, 4, 64, "f32", 0, 4096, 65536),            # cfg0's block, emulated pages
+    (256, 1000, 8, 2, 32, "bf16", 3, 4096, 65536),           # ragged inter: rows straddle blocks, partial last blocks
+    (4096, 14336, 32, 8, 128, "bf16", 0, 65536, 2 << 20),    # cfg1 at full size, real VMM pages
+    (640, 1536, 40, 8, 16, "bf16", 63, 1024, 65536),         # blocks smaller than a row
+])
+def test_fused_load_equals_permute_then_shuffle(hidden, inter, n_q, n_kv, d, dtype, layer, block, page):
+    """cloak_load_mlp_heads: the pool bytes are the oracle's shuffle(permute(W)) -- and the two-pass GPU path's."""
+    key, seed = 0x1234, 7
+    e = 4 if dtype == "f32" else 2
+    shapes = gen.layer_shapes(hidden, inter, n_q, n_kv, d)
+    W = {nm: gen.synth(seed, i, shp, dtype) for i, (nm, shp) in enumerate(shapes)}
+    dW = {nm: _dev(a, dtype) for nm, a in W.items()}
+    sizes = [e * n * k for _, (n, k) in shapes]
+    offs, total = C.cloak_arena_plan(key, sizes, block)
+    off = {nm: o for (nm, _), o in zip(shapes, offs)}
+    pi = O.mlp_perm(key, layer, inter)
+    kappa, eta = O.head_maps(key, layer, n_q, n_kv)
+    ref = dict(zip(("gate", "up", "down"), O.permute_mlp(W["gate"], W["up"], W["down"], pi)))
+    ref.update(zip(("q", "k", "v", "o"), O.permute_heads(W["q"], W["k"], W["v"], W["o"], kappa, eta, d)))
+    g = O.pool_geometry(total, block, page)
+    t = O.pool_tables(key, g)
+    sh = C.cloak_block_shape(hidden, inter, n_q, n_kv, d, C.CLOAK_F32 if dtype == "f32" else C.CLOAK_BF16, layer)
+    with Pool(total, block, page, key) as pf, Pool(total, block, page, key) as p2:
+        T = t.T_vmm if pf.info["is_vmm"] else t.T_emulated
+        refpool = np.zeros(g.nslots * block, np.uint8)
+        for nm, _ in shapes:
+            O.shuffle_into(refpool, T, ref[nm].view(np.uint8).ravel(), off[nm], block)
+        # stale bytes everywhere first: the fused path must leave exactly the oracle's pool, zero tails included
+        junk = torch.full((total,), 0xA5, dtype=torch.uint8, device="cuda")
+        C.cloak_shuffle(pf.h, junk, 0, total)
+        C.cloak_load_mlp_heads(key, sh, pf.h, off, **dW)
+        got = pf.raw()
+        for (nm, _), sz in zip(shapes, sizes):                      # every block a tensor owns, padding included
+            first, nblk = off[nm] // block, (sz + block - 1) // block
+            for i in range(first, first + nblk):
+                s0 = int(T[i]) * block
+                assert np.array_equal(got[s0:s0 + block], refpool[s0:s0 + block]), (nm, i - first)
+        dP = {nm: torch.zeros_like(x) for nm, x in dW.items()}
+        C.cloak_permute_mlp_heads(key, sh, **dW, **{k + "_o": v for k, v in dP.items()})
+        for nm, _ in shapes:
+            C.cloak_shuffle(p2.h, dP[nm], off[nm], dP[nm].numel() * e)
+        assert np.array_equal(p2.raw(), refpool)
+        # a subset of the tensors only
+        C.cloak_shuffle(pf.h, junk, 0, total)
+        C.cloak_load_mlp_heads(key, sh, pf.h, off, down=dW["down"], k=dW["k"])
+        got = pf.raw()
+        for nm in ("down", "k"):
+            i = off[nm] // block
+            s0 = int(T[i]) * block
+            assert np.array_equal(got[s0:s0 + block], refpool[s0:s0 + block])
+        i = off["gate"] // block
+        assert (got[int(T[i]) * block:int(T[i]) * block + block] == 0xA5).all()      # untouched
+
+
 def test_tile128_bit_exact():
     for dtype, (N, K) in [("bf16", (256, 384)), ("f32", (128, 256)), ("bf16", (1024, 5120))]:
         W = gen.synth(9, 0, (N, K), dtype)
