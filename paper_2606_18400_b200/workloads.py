@@ -178,6 +178,36 @@ def run_cfg2(args):
     info = C.cloak_pool_info(pc)
     launches0 = C.cloak_launch_count()
     try:
+        # ---- load path, two ways, on one layer's worth of source tensors reused for all 32 layers (timing only; the
+        # real contents are loaded right after): S5 then S4 (permute into a scratch tensor, shuffle it) against the
+        # fused cloak_load_mlp_heads (permuted rows/columns written straight through the block table)
+        lshapes = gen.layer_shapes(c["hidden"], c["inter"], c["n_q"], c["n_kv"], c["head_dim"])
+        raw = {nm: synth_cuda.fill(torch.empty(shp, dtype=torch.bfloat16, device="cuda"), c["seed"], i)
+               for i, (nm, shp) in enumerate(lshapes)}
+        tmp = {nm: torch.empty_like(t) for nm, t in raw.items()}
+        shs = [C.cloak_block_shape(c["hidden"], c["inter"], c["n_q"], c["n_kv"], c["head_dim"], C.CLOAK_BF16, l)
+               for l in range(c["layers"])]
+        loffs = [{nm: off[f"l{l}.{nm}"] for nm, _ in lshapes} for l in range(c["layers"])]
+
+        def load_two_pass():
+            for l in range(c["layers"]):
+                C.cloak_permute_mlp_heads(c["key"], shs[l], **raw, **{k + "_o": v for k, v in tmp.items()})
+                for nm, t in tmp.items():
+                    C.cloak_shuffle(pc, t, loffs[l][nm], t.numel() * 2)
+
+        def load_fused():
+            for l in range(c["layers"]):
+                C.cloak_load_mlp_heads(c["key"], shs[l], pc, loffs[l], **raw)
+
+        layer_bytes = sum(t.numel() * 2 for t in raw.values()) * c["layers"]
+        two_med, _ = time_gpu(torch, load_two_pass, max(3, args.reps // 2), warmup=1)
+        fus_med, _ = time_gpu(torch, load_fused, max(3, args.reps // 2), warmup=1)
+        load_paths = {"layers_bytes": layer_bytes,
+                      "permute_then_shuffle": dict(rate(2 * layer_bytes, two_med, peak), passes=2),
+                      "fused_load": dict(rate(2 * layer_bytes, fus_med, peak), passes=1),
+                      "note": "GB/s = 2 x payload / time for both, so the fused path's advantage shows as a higher rate"}
+        del raw, tmp
+
         keep = {nm: torch.empty(shp, dtype=torch.bfloat16, device="cuda") for nm, shp in tensors}
         load_s = _load_model(torch, C, synth_cuda, gen, 2, (pc, pn), offs, False, keep=keep)
 
@@ -262,6 +292,7 @@ def run_cfg2(args):
             "pool_map_ms": map_ms, "pool_create_s": create_s, "generate_permute_load_s": load_s,
             "shuffle": dict(rate(2 * payload, sh_med, peak), ms_min=sh_min),
             "unshuffle": dict(rate(2 * payload, un_med, peak), ms_min=un_min), "roundtrip_bit_exact": bool(roundtrip),
+            "load_paths": load_paths,
             "decode_chain": res, "decode_read_bytes": read_bytes,
             "ideal_tokens_per_s_at_measured_peak": peak * 1e9 / read_bytes,
             "cloaked_vs_native_overhead_pct": ov, "cloaked_identical_to_native": bool(identical),
