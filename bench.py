@@ -441,7 +441,7 @@ def run_cloak(args):
         "cloaked_vs_native_overhead_pct": overhead,
         "hbm_peak_gbs": peak, "hbm_peak_kind": peak_kind, "hbm_nominal_gbs": 8000.0,
         "pool_map_ms": map_ms, "pool_create_s": pool_create_s, "roundtrip_bit_exact": bool(ok),
-        "roofline": {"bound": "hbm", "kernel": "gemv_stream_kernel", "achieved": achieved, "peak": peak, "unit": "GB/s",
+        "roofline": {"bound": "hbm", "kernel": "gemv_chain_kernel", "achieved": achieved, "peak": peak, "unit": "GB/s",
                      "frac": achieved / peak, "traffic": NCU_TRAFFIC_PER_LAUNCH, "traffic_source": NCU_TRAFFIC_SOURCE,
                      "launches_per_step": gemv_launches,
                      "bytes_per_launch": sb["gemv"] / gemv_launches, "avg_launch_us": gemv_ms / gemv_launches * 1e3,
