@@ -271,7 +271,7 @@ static cloak_status gemv_device(const cloak_pool* pool, const cloak_tensor* w, c
     a.batch = batch;
     a.zero = 0;
     if (!g_force_oneshot) {
-        const int log2cb = gemv_stream_log2cb(pool, w);
+        const int log2cb = gemv_stream_log2cb(pool, w, batch);
         if (log2cb >= 9) {
             cloak_gemv_op op;
             op.w = *w;
@@ -363,7 +363,7 @@ extern "C" cloak_status cloak_gemv_chain(const cloak_pool* pool, const cloak_gem
             for (uint32_t k = 0; k < i; ++k)
                 if (h_ops[k].d_y == h_ops[i].d_gate && (h_ops[k].w.N != h_ops[i].w.N || h_ops[k].w.K != h_ops[i].w.K))
                     return fail(CLOAK_ERR_INVALID, "gemv_chain: op %u: d_gate is the output of op %u, which has another shape", i, k);
-        cb[i] = gemv_stream_log2cb(pool, &h_ops[i].w);
+        cb[i] = gemv_stream_log2cb(pool, &h_ops[i].w, batch);
         if (cb[i] < 9) return fail(CLOAK_ERR_UNSUPPORTED, "gemv_chain: op %u needs bf16 ROWMAJOR, K %% 256 == 0, block >= 512", i);
     }
     DeviceGuard g(pool->device);

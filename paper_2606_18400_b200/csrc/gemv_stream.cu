@@ -70,15 +70,21 @@ struct ChainArgs {
 };
 
 constexpr int GS_CONSUMERS = 8;                       // consumer warps
-constexpr int GS_THREADS = 32 * (1 + GS_CONSUMERS);
+// Warps ahead of the consumers.  batch <= 8: the producer warp alone.  batch 9..16: a whole warpgroup (producer + three
+// warps that retire at once), so that the register file can be re-split per warpgroup with setmaxnreg: the producer
+// group drops to 40 registers per thread, the two consumer groups rise to 232 -- room for a second set of X fragments.
+constexpr int gs_lead_warps(int nt) { return nt == 2 ? 4 : 1; }
+constexpr int gs_threads(int nt) { return 32 * (gs_lead_warps(nt) + GS_CONSUMERS); }
 constexpr int GS_ROWS = 8;                            // weight rows per tile (the MMA's N)
 constexpr int GS_PAD = 64;                            // bytes of padding per staged row (conflict-free LDS.128)
 // Row tiles per group (X reuse; one register accumulator set per tile) and interleaved accumulators per tile.
 // 8 tiles x 2 accumulators measured best for both batch ranges: 16 x 1 halves the X traffic at batch 16 but its
 // 16-deep dependent MMA chain costs more than that saves; staggering the group boundaries over the CTAs (so the
 // SMs do not all wait for X at once) adds a group per CTA and was slower too.
-constexpr int GS_TG = 8;
-constexpr int GS_NACC = 2;
+// (With the X prefetch in place at batch 9..16, 16 x 1, 12 x 1 and 12 x 2 were measured again: 94.5, 96.1, 101.4 us for the
+// cfg1 layer against 93.6 us for 8 x 2.)
+constexpr int gs_tg(int) { return 8; }
+constexpr int gs_nacc(int) { return 2; }
 constexpr int GS_TGR = 4;                             // row tiles reduced across warps per shared-memory pass
 constexpr int GS_MAX_STAGES = 12;
 constexpr uint32_t gs_stages(int log2cb) {            // ~192 KiB of weights in flight per SM
@@ -134,12 +140,15 @@ __device__ __forceinline__ uint16_t ld_coherent_u16(const uint16_t* p) {
 
 // LOG2CB: log2 of the chunk bytes per row (9..12).  NT: 1 = batch <= 8 (upper half of the MMA's M is zero), 2 = batch <= 16.
 template <int LOG2CB, int NT>
-__global__ void __launch_bounds__(GS_THREADS, 1) gemv_chain_kernel(const __grid_constant__ ChainArgs a) {
+__global__ void __launch_bounds__(gs_threads(NT), 1) gemv_chain_kernel(const __grid_constant__ ChainArgs a) {
     constexpr uint32_t CB = 1u << LOG2CB;
     constexpr uint32_t RS = CB + GS_PAD;                       // staged row stride
     constexpr uint32_t STAGE = GS_ROWS * RS;
     constexpr uint32_t NST = gs_stages(LOG2CB);
     constexpr int KS = CB / (GS_CONSUMERS * 64);               // 64-byte steps (one 16-byte vector per lane) per warp per unit
+    constexpr bool PF = (NT == 2);                             // prefetch the next phase's X fragments (see below)
+    constexpr int LEAD = gs_lead_warps(NT);
+    constexpr int GS_TG = gs_tg(NT), GS_NACC = gs_nacc(NT);
     extern __shared__ __align__(128) unsigned char smem[];
     __shared__ __align__(8) uint64_t full[NST], empty[NST];
     __shared__ float red[GS_CONSUMERS][GS_TGR][NT * 64];      // [warp][tile][batch m][row r]
@@ -157,7 +166,9 @@ __global__ void __launch_bounds__(GS_THREADS, 1) gemv_chain_kernel(const __grid_
     __syncthreads();
     const uint32_t smem_base = smem_u32(smem);
 
-    if (warp == 0) {
+    if (warp < LEAD) {
+        if (NT == 2) asm volatile("setmaxnreg.dec.sync.aligned.u32 56;");
+        if (warp > 0) return;
         // ------------------------------------------------------------ producer: straight through the chain
         // The table is immutable after cloak_pool_create; the weights may have been written by the preceding
         // kernel (a shuffle / re-layout) unless the host says otherwise.
@@ -196,9 +207,10 @@ __global__ void __launch_bounds__(GS_THREADS, 1) gemv_chain_kernel(const __grid_
     }
 
     // ---------------------------------------------------------------- consumers
-    const int cw = warp - 1;
+    if (NT == 2) asm volatile("setmaxnreg.inc.sync.aligned.u32 224;");
+    const int cw = warp - LEAD;
     const int g = lane >> 2, t = lane & 3;
-    const uint32_t ctid = threadIdx.x - 32;                        // 0..255 among consumers
+    const uint32_t ctid = threadIdx.x - 32 * LEAD;                 // 0..255 among consumers
     const bool xv0 = (uint32_t)g < a.batch, xv1 = (uint32_t)(g + 8) < a.batch;
     const uint32_t lane_off = cw * (CB / GS_CONSUMERS) + t * 16;   // byte offset of this lane inside a row chunk
     const uint32_t nout = a.batch * GS_ROWS;
@@ -245,6 +257,21 @@ __global__ void __launch_bounds__(GS_THREADS, 1) gemv_chain_kernel(const __grid_
                 if (op.gate) op.act[idx] = silu_mul_bf16(ld_coherent_u16(op.gate + idx), v);
             };
 
+            // X fragments of one (group, chunk) phase.  Batch <= 8 re-reads them mostly from L1; batch 9..16 (X is up to
+            // 16 x K x 2 B, more than the L1 left beside the ring) pays an L2 round trip per phase, so there the next
+            // phase's fragments are fetched one phase ahead (PF) into a second register set (see gs_lead_warps).
+            uint4 xa[KS], xb[KS], na[KS], nb[KS];
+            auto load_x = [&](uint4 (&pa)[KS], uint4 (&pb)[KS], uint32_t c) {
+                const uint32_t xk = c * (CB / 2);
+                const uint4 z = make_uint4(0, 0, 0, 0);
+#pragma unroll
+                for (int ks = 0; ks < KS; ++ks) {
+                    pa[ks] = xv0 ? ldg_coherent(x0 + xk + ks * 32) : z;
+                    pb[ks] = (NT == 2 && xv1) ? ldg_coherent(x1 + xk + ks * 32) : z;
+                }
+            };
+            if (PF) load_x(xa, xb, 0);
+
             for (uint32_t g0 = tile_lo; g0 <= tile_hi; g0 += GS_TG) {
                 const uint32_t g1 = min(g0 + GS_TG - 1, tile_hi);
                 float acc[GS_TG][GS_NACC][4];
@@ -257,13 +284,12 @@ __global__ void __launch_bounds__(GS_THREADS, 1) gemv_chain_kernel(const __grid_
 
                 for (uint32_t c = 0; c < kch; ++c) {
                     // this warp's X fragments for chunk c: fetched once, reused for every row tile of the group
-                    uint4 xa[KS], xb[KS];
-                    const uint32_t xk = c * (CB / 2);
-                    const uint4 z = make_uint4(0, 0, 0, 0);
-#pragma unroll
-                    for (int ks = 0; ks < KS; ++ks) {
-                        xa[ks] = xv0 ? ldg_coherent(x0 + xk + ks * 32) : z;
-                        xb[ks] = (NT == 2 && xv1) ? ldg_coherent(x1 + xk + ks * 32) : z;
+                    bool more = false;
+                    if (!PF) {
+                        load_x(xa, xb, c);
+                    } else {
+                        more = (c + 1 < kch) || (g0 + GS_TG <= tile_hi);
+                        if (more) load_x(na, nb, c + 1 < kch ? c + 1 : 0);      // the next phase's, behind this phase's work
                     }
 #pragma unroll
                     for (int q = 0; q < GS_TG; ++q) {
@@ -280,6 +306,13 @@ __global__ void __launch_bounds__(GS_THREADS, 1) gemv_chain_kernel(const __grid_
                         __syncwarp();
                         if (lane == 0) mbar_arrive(smem_u32(&empty[s]));
                         if (++s == NST) { s = 0; ph ^= 1; }
+                    }
+                    if (PF && more) {
+#pragma unroll
+                        for (int ks = 0; ks < KS; ++ks) {
+                            xa[ks] = na[ks];
+                            xb[ks] = nb[ks];
+                        }
                     }
                 }
 
@@ -370,7 +403,7 @@ static cloak_status launch(const ChainArgs& a, int ctas, cudaStream_t s) {
     }
     cudaLaunchConfig_t cfg = {};
     cfg.gridDim = dim3(ctas);
-    cfg.blockDim = dim3(GS_THREADS);
+    cfg.blockDim = dim3(gs_threads(NT));
     cfg.dynamicSmemBytes = smem;
     cfg.stream = s;
     cudaLaunchAttribute at[1];
@@ -384,12 +417,13 @@ static cloak_status launch(const ChainArgs& a, int ctas, cudaStream_t s) {
 }
 
 // log2 of the row-chunk size the streaming kernel would use for this tensor, or -1 if it cannot take it.
-int gemv_stream_log2cb(const cloak_pool* pool, const cloak_tensor* w) {
+int gemv_stream_log2cb(const cloak_pool* pool, const cloak_tensor* w, uint32_t batch) {
     if (w->dt != CLOAK_BF16 || w->layout != CLOAK_ROWMAJOR || w->K % 256 || w->N % GS_ROWS || pool->block < 512) return -1;
     const uint64_t row_bytes = (uint64_t)w->K * 2;
     int log2cb = 12;
     while (log2cb > 9 && (row_bytes & ((1u << log2cb) - 1))) --log2cb;
     if ((uint32_t)log2cb > pool->log2_block) log2cb = (int)pool->log2_block;
+    (void)batch;   // measured: forcing 2 KiB chunks at batch 9..16 so that the X prefetch fits costs 35 % (8 x 2 KiB stages)
     return log2cb;
 }
 
