@@ -401,6 +401,7 @@ def run_cloak(args):
                "what": "cloak_shuffle_host of the layer from pinned host memory + 7 cloak_gemv_host (batch 1)"}
 
     map_ms = C.cloak_pool_map_ms(pool_a)
+    adjacency = C.cloak_pool_adjacency(pool_a)          # layout quality (G8): neighbours that stayed neighbours
     torch.cuda.synchronize()
     for p in (pool_a, pool_b, pool_n):
         C.cloak_pool_destroy(p)
@@ -440,7 +441,7 @@ def run_cloak(args):
         "gemv_isolated_ms": {"cloaked": cloaked_iso_ms, "native": native_ms, "cloaked_7_separate_calls": per_call_ms},
         "cloaked_vs_native_overhead_pct": overhead,
         "hbm_peak_gbs": peak, "hbm_peak_kind": peak_kind, "hbm_nominal_gbs": 8000.0,
-        "pool_map_ms": map_ms, "pool_create_s": pool_create_s, "roundtrip_bit_exact": bool(ok),
+        "pool_map_ms": map_ms, "layout_adjacency": adjacency, "pool_create_s": pool_create_s, "roundtrip_bit_exact": bool(ok),
         "roofline": {"bound": "hbm", "kernel": "gemv_chain_kernel", "achieved": achieved, "peak": peak, "unit": "GB/s",
                      "frac": achieved / peak, "traffic": NCU_TRAFFIC_PER_LAUNCH, "traffic_source": NCU_TRAFFIC_SOURCE,
                      "launches_per_step": gemv_launches,

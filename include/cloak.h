@@ -102,6 +102,15 @@ cloak_status cloak_pool_dump(const cloak_pool* pool, void* d_out, void* stream);
 /* Milliseconds the host-side mapper (reserve/create/map/set-access) took in cloak_pool_create. */
 cloak_status cloak_pool_map_ms(const cloak_pool* pool, double* ms);
 
+/* Layout-quality report (the paper's only security-side metric that needs no attacker is a
+ * contiguity percentage).  Fractions of logical neighbours that are still neighbours:
+ *   *va_blocks       = #{i : T_va[i+1] == T_va[i] + 1} / (nb - 1),  T_va[i] = blockinv[i]   (the VA view V)
+ *   *physical_blocks = the same through the page map, slot(i) = pageinv[blockinv[i] / bpp] * bpp + blockinv[i] % bpp
+ *                      (the dump view D: what reading pages in physical order sees; G8: expect about 1 / nslots)
+ *   *pages           = #{v : pageinv[v+1] == pageinv[v] + 1} / (npages - 1)
+ * An identity pool reports 1, 1, 1.  Any output may be NULL.  Synchronous. */
+cloak_status cloak_pool_adjacency(const cloak_pool* pool, double* va_blocks, double* physical_blocks, double* pages);
+
 /* ---- S4 block shuffle / unshuffle, S8 re-layout (north_star (a)).
  * shuffle:   pool[T[i]*b + o] = logical[i*b + o] for the arena range [logical_offset, +bytes);
  * unshuffle: logical[i*b + o] = pool[T[i]*b + o] for the same range.

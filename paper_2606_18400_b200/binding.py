@@ -23,7 +23,7 @@ STATUS_NAMES = {0: "CLOAK_OK", -1: "CLOAK_ERR_INVALID", -2: "CLOAK_ERR_ALIGN", -
 
 # every symbol include/cloak.h declares
 SYMBOLS = ["cloak_last_error", "cloak_version", "cloak_launch_count", "cloak_keygen", "cloak_pool_create", "cloak_pool_destroy",
-           "cloak_pool_info", "cloak_pool_tables", "cloak_pool_dump", "cloak_pool_map_ms", "cloak_shuffle",
+           "cloak_pool_info", "cloak_pool_tables", "cloak_pool_dump", "cloak_pool_map_ms", "cloak_pool_adjacency", "cloak_shuffle",
            "cloak_unshuffle", "cloak_relayout", "cloak_shuffle_host", "cloak_unshuffle_host",
            "cloak_set_copy_engine", "cloak_arena_plan", "cloak_permute_mlp_heads", "cloak_load_mlp_heads", "cloak_to_tile128",
            "cloak_gemv", "cloak_gemv_chain", "cloak_gemm", "cloak_set_gemv_engine", "cloak_gemv_host", "cloak_silu_mul"]
@@ -65,6 +65,7 @@ lib.cloak_pool_info.argtypes = [_P, POINTER(_P), POINTER(_P), POINTER(c_uint32),
 lib.cloak_pool_tables.argtypes = [_P, _P, _P, _P, _P]
 lib.cloak_pool_dump.argtypes = [_P, _P, _P]
 lib.cloak_pool_map_ms.argtypes = [_P, POINTER(c_double)]
+lib.cloak_pool_adjacency.argtypes = [_P, POINTER(c_double), POINTER(c_double), POINTER(c_double)]
 lib.cloak_shuffle.argtypes = [_P, _P, c_uint64, c_uint64, _P]
 lib.cloak_unshuffle.argtypes = [_P, _P, c_uint64, c_uint64, _P]
 lib.cloak_relayout.argtypes = [_P, _P, _P]
@@ -164,6 +165,12 @@ def cloak_pool_map_ms(pool):
     ms = c_double()
     _check(lib.cloak_pool_map_ms(pool, byref(ms)))
     return ms.value
+
+
+def cloak_pool_adjacency(pool):
+    va, ph, pg = c_double(), c_double(), c_double()
+    _check(lib.cloak_pool_adjacency(pool, byref(va), byref(ph), byref(pg)))
+    return dict(va_blocks=va.value, physical_blocks=ph.value, pages=pg.value)
 
 
 def cloak_shuffle(pool, d_logical, logical_offset, nbytes, stream=None):

@@ -25,6 +25,29 @@ __global__ void build_table_kernel(const uint32_t* __restrict__ blockinv, const 
     }
 }
 
+// Layout quality: how many logical neighbours (i, i+1) are still neighbours in the VA view, in the
+// physical (dump) view, and how many neighbouring VA pages are backed by neighbouring physical pages.
+__global__ void adjacency_kernel(const uint32_t* __restrict__ blockinv, const uint32_t* __restrict__ pageinv, uint32_t nb,
+                                 uint32_t bpp, uint32_t npages, unsigned long long* __restrict__ out) {
+    const uint32_t i = blockIdx.x * blockDim.x + threadIdx.x;
+    unsigned va = 0, ph = 0, pg = 0;
+    if (i + 1 < nb) {
+        const uint32_t a = blockinv[i], b = blockinv[i + 1];
+        va = b == a + 1;
+        const uint32_t da = pageinv[a / bpp] * bpp + a % bpp, db = pageinv[b / bpp] * bpp + b % bpp;
+        ph = db == da + 1;
+    }
+    if (i + 1 < npages) pg = pageinv[i + 1] == pageinv[i] + 1;
+    va = __reduce_add_sync(0xffffffffu, va);
+    ph = __reduce_add_sync(0xffffffffu, ph);
+    pg = __reduce_add_sync(0xffffffffu, pg);
+    if ((threadIdx.x & 31) == 0) {
+        if (va) atomicAdd(out + 0, (unsigned long long)va);
+        if (ph) atomicAdd(out + 1, (unsigned long long)ph);
+        if (pg) atomicAdd(out + 2, (unsigned long long)pg);
+    }
+}
+
 static cloak_status destroy_impl(cloak_pool* p) {
     if (!p) return CLOAK_OK;
     DeviceGuard g(p->device);
@@ -252,6 +275,26 @@ extern "C" cloak_status cloak_pool_dump(const cloak_pool* pool, void* d_out, voi
         src = pool->alias;
     }
     CLOAK_CUDA(cudaMemcpyAsync(d_out, src, pool->bytes(), cudaMemcpyDeviceToDevice, (cudaStream_t)stream));
+    return CLOAK_OK;
+}
+
+extern "C" cloak_status cloak_pool_adjacency(const cloak_pool* pool, double* va_blocks, double* physical_blocks, double* pages) {
+    using namespace cloak;
+    if (!pool) return fail(CLOAK_ERR_INVALID, "pool_adjacency: NULL pool");
+    DeviceGuard g(pool->device);
+    unsigned long long* d = nullptr;
+    CLOAK_CUDA(cudaMalloc((void**)&d, 3 * sizeof(unsigned long long)));
+    cudaMemset(d, 0, 3 * sizeof(unsigned long long));
+    const uint32_t n = pool->nb > pool->npages ? pool->nb : pool->npages;
+    adjacency_kernel<<<(n + 255) / 256, 256>>>(pool->d_blockinv, pool->d_pageinv, pool->nb, pool->bpp, pool->npages, d);
+    launched();
+    unsigned long long h[3] = {0, 0, 0};
+    cudaError_t e = cudaMemcpy(h, d, sizeof(h), cudaMemcpyDeviceToHost);
+    cudaFree(d);
+    if (e != cudaSuccess) return fail(CLOAK_ERR_CUDA, "pool_adjacency: %s", cudaGetErrorString(e));
+    if (va_blocks) *va_blocks = pool->nb > 1 ? (double)h[0] / (pool->nb - 1) : 0.0;
+    if (physical_blocks) *physical_blocks = pool->nb > 1 ? (double)h[1] / (pool->nb - 1) : 0.0;
+    if (pages) *pages = pool->npages > 1 ? (double)h[2] / (pool->npages - 1) : 0.0;
     return CLOAK_OK;
 }
 

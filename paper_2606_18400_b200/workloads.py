@@ -176,6 +176,7 @@ def run_cfg2(args):
     create_s = time.perf_counter() - t0
     pn = C.cloak_pool_create(0, total, c["block"], c["page"], c["key"], C.CLOAK_POOL_IDENTITY)
     info = C.cloak_pool_info(pc)
+    adjacency = C.cloak_pool_adjacency(pc)
     launches0 = C.cloak_launch_count()
     try:
         # ---- load path, two ways, on one layer's worth of source tensors reused for all 32 layers (timing only; the
@@ -290,6 +291,7 @@ def run_cfg2(args):
             "payload_bytes": payload, "arena_bytes": total, "npages": info["npages"], "nblocks": info["nb"],
             "reps": args.reps, "hbm_peak_gbs": peak, "hbm_peak_kind": peak_kind, "hbm_nominal_gbs": NOMINAL_HBM_GBS,
             "pool_map_ms": map_ms, "pool_create_s": create_s, "generate_permute_load_s": load_s,
+            "layout_adjacency": adjacency,
             "shuffle": dict(rate(2 * payload, sh_med, peak), ms_min=sh_min),
             "unshuffle": dict(rate(2 * payload, un_med, peak), ms_min=un_min), "roundtrip_bit_exact": bool(roundtrip),
             "load_paths": load_paths,

@@ -33,7 +33,8 @@ def test_synth_twins_agree(dtype):
 
 
 # ------------------------------------------------------------------ S1 keygen
-@pytest.mark.parametrize("n", [1, 2, 8, 16, 256, 1024, 4096, 4097, 14336, 245056, 1 << 20, (1 << 20) + 77])
+@pytest.mark.parametrize("n", [1, 2, 8, 16, 256, 1024, 4096, 4097, 14336, 245056, 1 << 20, (1 << 20) + 77,
+                               (1 << 24) + 3])      # the last one: more elements than 4 x the 2^22 bucket cap
 def test_keygen_bit_exact(n):
     perm = torch.empty(n, dtype=torch.int32, device="cuda")
     inv = torch.empty(n, dtype=torch.int32, device="cuda")
@@ -119,6 +120,20 @@ def test_shuffle_by_tensor_ranges_and_zero_padding():
             C.cloak_shuffle(p.h, to_dev_bytes(d), o, d.size)
             O.shuffle_into(ref, t.T_emulated, d, o, block)
         assert np.array_equal(p.raw(), ref)
+
+
+@pytest.mark.parametrize("payload,block,page", [(3 << 20, 4096, 65536), (40 << 20, 65536, 2 << 20), (1 << 20, 256, 1024)])
+def test_pool_adjacency_matches_the_oracle(payload, block, page):
+    """NEXT-3 layout-quality report: adjacent-block / adjacent-page fractions equal oracle.adjacent_fraction."""
+    g = O.pool_geometry(payload, block, page)
+    t = O.pool_tables(0x1234, g)
+    with Pool(payload, block, page, 0x1234) as p, Pool(payload, block, page, 0x1234, C.CLOAK_POOL_IDENTITY) as pi:
+        a = C.cloak_pool_adjacency(p.h)
+        assert a["va_blocks"] == pytest.approx(O.adjacent_fraction(t.T_vmm), abs=1e-15)
+        assert a["physical_blocks"] == pytest.approx(O.adjacent_fraction(t.T_emulated), abs=1e-15)
+        assert a["pages"] == pytest.approx(O.adjacent_fraction(t.pageinv), abs=1e-15)
+        assert a["physical_blocks"] < 0.02                          # G8: about 1 / nslots for a uniform permutation
+        assert C.cloak_pool_adjacency(pi.h) == dict(va_blocks=1.0, physical_blocks=1.0, pages=1.0)
 
 
 def test_identity_pool_is_the_native_layout():
