@@ -225,6 +225,17 @@ typedef struct {
 } cloak_gemv_op;
 cloak_status cloak_gemv_chain(const cloak_pool* pool, const cloak_gemv_op* h_ops, uint32_t n_ops, uint32_t batch,
                               void* stream);
+/* A list of INDEPENDENT GEMMs over one pool in one persistent launch (per 16 ops): Y_i = X_i W_i^T as cloak_gemm computes
+ * it, bit for bit; no op may read what another op of the list writes.  The weight stream runs on across op boundaries
+ * (BASELINE.json configs[3]: "cloaked decode GEMM" of every projection of the model).  h_ops is a HOST array, not
+ * referenced after the call returns.  Asynchronous on `stream`. */
+typedef struct {
+    cloak_tensor w;
+    const void* d_x;
+    void* d_y;
+} cloak_gemm_op;
+cloak_status cloak_gemm_chain(const cloak_pool* pool, const cloak_gemm_op* h_ops, uint32_t n_ops, uint32_t batch,
+                              void* stream);
 /* Selects the bf16 GEMV kernel: 0 = automatic (streaming TMA kernel when K % 256 == 0, launched with
  * programmatic dependent launch), 1 = always the one-shot split-K kernel, 2 = automatic without
  * programmatic dependent launch.  For A/B measurement; process-wide. */

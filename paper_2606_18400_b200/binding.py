@@ -26,7 +26,7 @@ SYMBOLS = ["cloak_last_error", "cloak_version", "cloak_launch_count", "cloak_key
            "cloak_pool_info", "cloak_pool_tables", "cloak_pool_dump", "cloak_pool_map_ms", "cloak_pool_adjacency", "cloak_shuffle",
            "cloak_unshuffle", "cloak_relayout", "cloak_shuffle_host", "cloak_unshuffle_host",
            "cloak_set_copy_engine", "cloak_arena_plan", "cloak_permute_mlp_heads", "cloak_load_mlp_heads", "cloak_to_tile128",
-           "cloak_gemv", "cloak_gemv_chain", "cloak_gemm", "cloak_set_gemv_engine", "cloak_gemv_host", "cloak_silu_mul"]
+           "cloak_gemv", "cloak_gemv_chain", "cloak_gemm", "cloak_gemm_chain", "cloak_set_gemv_engine", "cloak_gemv_host", "cloak_silu_mul"]
 
 
 class CloakError(RuntimeError):
@@ -47,6 +47,10 @@ class cloak_tensor(Structure):
 class cloak_gemv_op(Structure):
     _fields_ = [("w", cloak_tensor), ("d_x", c_void_p), ("d_y", c_void_p), ("d_gate", c_void_p), ("d_act", c_void_p),
                 ("after", c_uint32)]
+
+
+class cloak_gemm_op(Structure):
+    _fields_ = [("w", cloak_tensor), ("d_x", c_void_p), ("d_y", c_void_p)]
 
 
 if not os.path.exists(LIB_PATH):
@@ -79,6 +83,7 @@ lib.cloak_load_mlp_heads.argtypes = [c_uint64, POINTER(cloak_block_shape), _P] +
 lib.cloak_to_tile128.argtypes = [_P, _P, c_uint32, c_uint32, c_int, _P]
 lib.cloak_gemv.argtypes = [_P, POINTER(cloak_tensor), _P, _P, c_uint32, _P]
 lib.cloak_gemv_chain.argtypes = [_P, POINTER(cloak_gemv_op), c_uint32, c_uint32, _P]
+lib.cloak_gemm_chain.argtypes = [_P, POINTER(cloak_gemm_op), c_uint32, c_uint32, _P]
 lib.cloak_gemm.argtypes = [_P, POINTER(cloak_tensor), _P, _P, c_uint32, _P]
 lib.cloak_gemv_host.argtypes = [_P, POINTER(cloak_tensor), _P, _P, c_uint32, _P]
 lib.cloak_silu_mul.argtypes = [_P, _P, _P, c_uint64, c_int, _P]
@@ -254,6 +259,19 @@ def cloak_gemv_chain(pool, ops, batch, stream=None):
 
 def cloak_gemm(pool, tensor, d_x, d_y, batch, stream=None):
     _check(lib.cloak_gemm(pool, byref(tensor), _ptr(d_x), _ptr(d_y), batch, _stream(stream)))
+
+
+def cloak_gemm_ops(ops):
+    """Marshals [(tensor, d_x, d_y), ...] into a ctypes array for cloak_gemm_chain (reusable across calls)."""
+    arr = (cloak_gemm_op * len(ops))()
+    for o, (t, x, y) in zip(arr, ops):
+        o.w, o.d_x, o.d_y = t, _ptr(x), _ptr(y)
+    return arr
+
+
+def cloak_gemm_chain(pool, ops, batch, stream=None):
+    arr = ops if isinstance(ops, ctypes.Array) else cloak_gemm_ops(ops)
+    _check(lib.cloak_gemm_chain(pool, arr, len(arr), batch, _stream(stream)))
 
 
 def cloak_gemv_host(pool, tensor, h_x, h_y, batch, stream=None):

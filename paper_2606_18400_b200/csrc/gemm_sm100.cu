@@ -24,22 +24,33 @@
 
 namespace cloak {
 
-struct GemmArgs {
-    const uint32_t* T;
-    uint32_t log2b;
+constexpr int GM_MAX_OPS = 16;             // ops per launch (one X tensor map of 128 B each in the kernel parameters)
+
+struct GemmOp {
     uint64_t w_offset;
-    uint32_t N, K, batch;
     __nv_bfloat16* y;
+    uint64_t part_base;  // float offset of this op's partials: [tile row][maxc][batch][128]
+    uint32_t N;
     uint32_t kt;         // k tiles per tile row = K/128
     uint32_t units;      // (N/128) * kt
     uint32_t per;        // units per CTA
     uint32_t maxc;       // max contributors per tile row
+    uint32_t row_base;   // index of this op's first tile-row counter
+};
+
+struct GemmArgs {
+    const uint32_t* T;
+    float* part;
+    uint32_t* counters;
+    uint32_t log2b;
+    uint32_t batch;
+    uint32_t nops;
     uint32_t wstages;    // ring of 32 KiB weight tiles (HBM latency: deep)
     uint32_t xstages;    // ring of X tiles [batch x 128] (L2 latency: shallow)
     uint32_t tmem_cols;  // power of two >= 2*batch
-    float* part;         // [tile row][maxc][batch][128]
-    uint32_t* counters;
     uint32_t early;      // 1: W unchanged since before the preceding kernel -> stream it ahead of griddepcontrol.wait
+    GemmOp ops[GM_MAX_OPS];
+    alignas(64) CUtensorMap map_x[GM_MAX_OPS];   // X of op j as a 2-D map [batch, K], boxes of [batch x 64]
 };
 
 constexpr int GM_THREADS = 224;            // warp 0 TMA (W), warp 1 MMA, warp 2 TMA (X), warps 3..6 epilogue
@@ -78,9 +89,12 @@ __device__ __forceinline__ void gm_dep_wait() { asm volatile("griddepcontrol.wai
 __device__ __forceinline__ void gm_dep_launch() { asm volatile("griddepcontrol.launch_dependents;" ::: "memory"); }
 __device__ __forceinline__ void epi_bar() { asm volatile("bar.sync 1, 128;" ::: "memory"); }
 
+// A launch runs a list of independent ops (cloak_gemm_chain; cloak_gemm is a list of one): every role walks the list,
+// the rings, the accumulator double buffer and their phases simply continue from op to op, so the weight stream does not
+// stop at an op boundary (per-launch head and tail cost ~4 us each; q, k, v, o of a Qwen-32B layer are 13 % of the bytes
+// and were 35 % of the time as separate launches).
 __global__ void __launch_bounds__(GM_THREADS, 1) gemm_tile128_kernel(const __grid_constant__ CUtensorMap map_w,
-                                                                     const __grid_constant__ CUtensorMap map_x,
-                                                                     GemmArgs a) {
+                                                                     const __grid_constant__ GemmArgs a) {
     extern __shared__ __align__(1024) unsigned char smem_raw[];
     __shared__ __align__(8) uint64_t wfull[GM_MAX_STAGES], wempty[GM_MAX_STAGES], xfull[GM_MAX_STAGES], xempty[GM_MAX_STAGES],
         tmem_full[2], tmem_empty[2];
@@ -112,153 +126,177 @@ __global__ void __launch_bounds__(GM_THREADS, 1) gemm_tile128_kernel(const __gri
     tc_fence_after();
     const uint32_t tmem_base = tmem_base_s;
 
-    const uint32_t ubeg = blockIdx.x * a.per;
-    const uint32_t uend = min(ubeg + a.per, a.units);
     const uint32_t xbox = a.batch * 128;                     // bytes of one X box [batch x 64 bf16]
-
     const uint32_t xtile = 2 * xbox;
     const uint32_t x_base = smem_base + a.wstages * 32768;
 
-    if (warp == 0 && lane == 0 && ubeg < uend) {
+    if (warp == 0 && lane == 0) {
         // ---------------------------------------------------------------- TMA producer, weight tiles (through T)
         if (!a.early) gm_dep_wait();
         uint32_t it = 0;
-        for (uint32_t u = ubeg; u < uend; ++u, ++it) {
-            const uint32_t s = it % a.wstages, f = it / a.wstages;
-            if (f > 0) mbar_wait(smem_u32(&wempty[s]), (f - 1) & 1);
-            const uint64_t off = a.w_offset + (uint64_t)u * 32768;               // tile index == unit index
-            const uint32_t slot = __ldg(a.T + (off >> a.log2b));
-            const uint64_t byte = ((uint64_t)slot << a.log2b) + (off & ((1ull << a.log2b) - 1));
-            const uint32_t row = (uint32_t)(byte >> 8);                          // pool viewed as rows of 256 B
-            const uint32_t st = smem_base + s * 32768;
-            const uint32_t bar = smem_u32(&wfull[s]);
-            mbar_expect_tx(bar, 32768);
-            tma_load_2d(st, &map_w, 0, row, bar);
-            tma_load_2d(st + 16384, &map_w, 64, row, bar);
+        for (uint32_t j = 0; j < a.nops; ++j) {
+            const GemmOp& op = a.ops[j];
+            const uint32_t ubeg = blockIdx.x * op.per, uend = min(ubeg + op.per, op.units);
+            for (uint32_t u = ubeg; u < uend; ++u, ++it) {
+                const uint32_t s = it % a.wstages, f = it / a.wstages;
+                if (f > 0) mbar_wait(smem_u32(&wempty[s]), (f - 1) & 1);
+                const uint64_t off = op.w_offset + (uint64_t)u * 32768;              // tile index == unit index
+                const uint32_t slot = __ldg(a.T + (off >> a.log2b));
+                const uint64_t byte = ((uint64_t)slot << a.log2b) + (off & ((1ull << a.log2b) - 1));
+                const uint32_t row = (uint32_t)(byte >> 8);                          // pool viewed as rows of 256 B
+                const uint32_t st = smem_base + s * 32768;
+                const uint32_t bar = smem_u32(&wfull[s]);
+                mbar_expect_tx(bar, 32768);
+                tma_load_2d(st, &map_w, 0, row, bar);
+                tma_load_2d(st + 16384, &map_w, 64, row, bar);
+            }
         }
-    } else if (warp == 2 && lane == 0 && ubeg < uend) {
+    } else if (warp == 2 && lane == 0) {
         // ---------------------------------------------------------------- TMA producer, activation tiles (L2-resident)
         gm_dep_wait();
         uint32_t it = 0;
-        for (uint32_t u = ubeg; u < uend; ++u, ++it) {
-            const uint32_t s = it % a.xstages, f = it / a.xstages;
-            if (f > 0) mbar_wait(smem_u32(&xempty[s]), (f - 1) & 1);
-            const uint32_t tk = u % a.kt;
-            const uint32_t st = x_base + s * xtile;
-            const uint32_t bar = smem_u32(&xfull[s]);
-            mbar_expect_tx(bar, xtile);
-            tma_load_2d(st, &map_x, tk * 128, 0, bar);
-            tma_load_2d(st + xbox, &map_x, tk * 128 + 64, 0, bar);
+        for (uint32_t j = 0; j < a.nops; ++j) {
+            const GemmOp& op = a.ops[j];
+            const uint32_t ubeg = blockIdx.x * op.per, uend = min(ubeg + op.per, op.units);
+            for (uint32_t u = ubeg; u < uend; ++u, ++it) {
+                const uint32_t s = it % a.xstages, f = it / a.xstages;
+                if (f > 0) mbar_wait(smem_u32(&xempty[s]), (f - 1) & 1);
+                const uint32_t tk = u % op.kt;
+                const uint32_t st = x_base + s * xtile;
+                const uint32_t bar = smem_u32(&xfull[s]);
+                mbar_expect_tx(bar, xtile);
+                tma_load_2d(st, &a.map_x[j], tk * 128, 0, bar);
+                tma_load_2d(st + xbox, &a.map_x[j], tk * 128 + 64, 0, bar);
+            }
         }
-    } else if (warp == 1 && lane == 0 && ubeg < uend) {
+    }
+ else if (warp == 1 && lane == 0) {
         // ---------------------------------------------------------------- MMA issuer
         const uint32_t idesc = (1u << 4) | (1u << 7) | (1u << 10) | ((a.batch >> 3) << 17) | ((128u >> 4) << 24);
-        uint32_t it = 0, seg = 0, cur_tn = ubeg / a.kt;
-        bool first = true;
-        for (uint32_t u = ubeg; u < uend; ++u, ++it) {
-            const uint32_t tn = u / a.kt;
-            if (tn != cur_tn) {
-                tc_commit(smem_u32(&tmem_full[seg & 1]));                        // accumulator of the finished tile row
-                ++seg;
-                cur_tn = tn;
-                first = true;
-            }
-            if (first && seg >= 2) {
+        uint32_t it = 0, seg = 0;                                               // both run on across the ops
+        auto acquire_acc = [&]() {                                              // accumulator seg & 1 drained by the epilogue?
+            if (seg >= 2) {
                 mbar_wait(smem_u32(&tmem_empty[seg & 1]), ((seg >> 1) - 1) & 1);
                 tc_fence_after();
             }
-            const uint32_t ws = it % a.wstages, xs = it % a.xstages;
-            mbar_wait(smem_u32(&xfull[xs]), (it / a.xstages) & 1);
-            mbar_wait(smem_u32(&wfull[ws]), (it / a.wstages) & 1);
-            tc_fence_after();
-            const uint32_t st = smem_base + ws * 32768, sx = x_base + xs * xtile;
-            const uint32_t d = tmem_base + (seg & 1) * a.batch;
+        };
+        for (uint32_t j = 0; j < a.nops; ++j) {
+            const GemmOp& op = a.ops[j];
+            const uint32_t ubeg = blockIdx.x * op.per, uend = min(ubeg + op.per, op.units);
+            if (ubeg >= uend) continue;
+            uint32_t cur_tn = ubeg / op.kt;
+            bool first = true;
+            acquire_acc();
+            for (uint32_t u = ubeg; u < uend; ++u, ++it) {
+                const uint32_t tn = u / op.kt;
+                if (tn != cur_tn) {
+                    tc_commit(smem_u32(&tmem_full[seg & 1]));                    // accumulator of the finished tile row
+                    ++seg;
+                    cur_tn = tn;
+                    first = true;
+                    acquire_acc();
+                }
+                const uint32_t ws = it % a.wstages, xs = it % a.xstages;
+                mbar_wait(smem_u32(&xfull[xs]), (it / a.xstages) & 1);
+                mbar_wait(smem_u32(&wfull[ws]), (it / a.wstages) & 1);
+                tc_fence_after();
+                const uint32_t st = smem_base + ws * 32768, sx = x_base + xs * xtile;
+                const uint32_t d = tmem_base + (seg & 1) * a.batch;
 #pragma unroll
-            for (int box = 0; box < 2; ++box) {
-                const uint64_t ad = umma_desc_sw128(st + box * 16384);
-                const uint64_t bd = umma_desc_sw128(sx + box * xbox);
+                for (int box = 0; box < 2; ++box) {
+                    const uint64_t ad = umma_desc_sw128(st + box * 16384);
+                    const uint64_t bd = umma_desc_sw128(sx + box * xbox);
 #pragma unroll
-                for (int k = 0; k < 4; ++k)                                      // UMMA_K = 16 bf16 = 32 B inside the atom
-                    tc_mma_bf16(d, ad + 2 * k, bd + 2 * k, idesc, (first && box == 0 && k == 0) ? 0u : 1u);
+                    for (int k = 0; k < 4; ++k)                                  // UMMA_K = 16 bf16 = 32 B inside the atom
+                        tc_mma_bf16(d, ad + 2 * k, bd + 2 * k, idesc, (first && box == 0 && k == 0) ? 0u : 1u);
+                }
+                first = false;
+                tc_commit(smem_u32(&wempty[ws]));                                // frees both stages when the MMAs retire
+                tc_commit(smem_u32(&xempty[xs]));
             }
-            first = false;
-            tc_commit(smem_u32(&wempty[ws]));                                    // frees both stages when the MMAs retire
-            tc_commit(smem_u32(&xempty[xs]));
+            tc_commit(smem_u32(&tmem_full[seg & 1]));
+            ++seg;
         }
-        tc_commit(smem_u32(&tmem_full[seg & 1]));
-    } else if (warp >= 3 && ubeg < uend) {
+    } else if (warp >= 3) {
         // ---------------------------------------------------------------- epilogue (4 warps = 4 TMEM lane quarters)
         const uint32_t q = warp & 3, r = q * 32 + lane;
         const int etid = threadIdx.x - 96;
         gm_dep_wait();
         if (etid == 0) gm_dep_launch();
+        const uint32_t nout = a.batch * 128;
         uint32_t seg = 0;
-        for (uint32_t u = ubeg; u < uend; ++seg) {
-            const uint32_t tn = u / a.kt;
-            const uint32_t t_first = tn * a.kt, t_last = t_first + a.kt - 1;
-            const uint32_t seg_last = min(uend - 1, t_last);
-            const bool complete = (u == t_first) && (seg_last == t_last);
-            mbar_wait(smem_u32(&tmem_full[seg & 1]), (seg >> 1) & 1);
-            tc_fence_after();
-            const uint32_t taddr = tmem_base + ((q * 32) << 16) + (seg & 1) * a.batch;
-            const size_t n = (size_t)tn * 128 + r;
-            const uint32_t nout = a.batch * 128;
-            const uint32_t c_first = t_first / a.per, c_last = t_last / a.per;
-            const uint32_t ncontrib = c_last - c_first + 1, me = blockIdx.x - c_first;
-            float* mine = a.part + ((size_t)tn * a.maxc + me) * nout;
-            for (uint32_t c = 0; c < a.batch; c += 16) {
-                uint32_t v[16];
-                tc_ld16(taddr + c, v);
-                if (complete) {
+        for (uint32_t j = 0; j < a.nops; ++j) {
+            const GemmOp& op = a.ops[j];
+            const uint32_t kt = op.kt;
+            const uint32_t ubeg = blockIdx.x * op.per, uend = min(ubeg + op.per, op.units);
+            float* part = a.part + op.part_base;
+            uint32_t* counters = a.counters + op.row_base;
+            for (uint32_t u = ubeg; u < uend; ++seg) {
+                const uint32_t tn = u / kt;
+                const uint32_t t_first = tn * kt, t_last = t_first + kt - 1;
+                const uint32_t seg_last = min(uend - 1, t_last);
+                const bool complete = (u == t_first) && (seg_last == t_last);
+                mbar_wait(smem_u32(&tmem_full[seg & 1]), (seg >> 1) & 1);
+                tc_fence_after();
+                const uint32_t taddr = tmem_base + ((q * 32) << 16) + (seg & 1) * a.batch;
+                const size_t n = (size_t)tn * 128 + r;
+                const uint32_t c_first = t_first / op.per, c_last = t_last / op.per;
+                const uint32_t ncontrib = c_last - c_first + 1, me = blockIdx.x - c_first;
+                float* mine = part + ((size_t)tn * op.maxc + me) * nout;
+                for (uint32_t c = 0; c < a.batch; c += 16) {
+                    uint32_t v[16];
+                    tc_ld16(taddr + c, v);
+                    if (complete) {
 #pragma unroll
-                    for (int j = 0; j < 16; ++j) a.y[(size_t)(c + j) * a.N + n] = __float2bfloat16_rn(__uint_as_float(v[j]));
-                } else {
+                        for (int i = 0; i < 16; ++i) op.y[(size_t)(c + i) * op.N + n] = __float2bfloat16_rn(__uint_as_float(v[i]));
+                    } else {
 #pragma unroll
-                    for (int j = 0; j < 16; ++j) __stcg(mine + (size_t)(c + j) * 128 + r, __uint_as_float(v[j]));
-                }
-            }
-            tc_fence_before();
-            __syncwarp();
-            if (lane == 0) mbar_arrive(smem_u32(&tmem_empty[seg & 1]));
-            if (!complete) {
-                __threadfence();
-                epi_bar();
-                if (etid == 0) {
-                    const uint32_t old = atomicAdd(a.counters + tn, 1u);
-                    last_flag = (old == ncontrib - 1);
-                    if (old == ncontrib - 1) a.counters[tn] = 0;                 // self-reset for the next launch
-                }
-                epi_bar();
-                if (last_flag) {
-                    __threadfence();
-                    const float* base = a.part + (size_t)tn * a.maxc * nout;
-                    for (uint32_t m = 0; m < a.batch; m += 16) {                 // 16 independent sums in flight
-                        float sum[16];
-#pragma unroll
-                        for (int j = 0; j < 16; ++j) sum[j] = 0.f;
-                        // 4 contributors x 16 values = 64 loads in flight per thread (the loop is L2-latency bound: with 16
-                        // in flight a [128 x 128] tile row took ~25 us); the additions stay in contributor order.
-                        for (uint32_t p = 0; p < ncontrib; p += 4) {
-                            float v[4][16];
-#pragma unroll
-                            for (int pp = 0; pp < 4; ++pp) {
-                                const float* src = base + (size_t)(p + pp) * nout + (size_t)m * 128 + r;
-#pragma unroll
-                                for (int j = 0; j < 16; ++j) v[pp][j] = (p + pp < ncontrib) ? __ldcg(src + j * 128) : 0.f;
-                            }
-#pragma unroll
-                            for (int pp = 0; pp < 4; ++pp)
-                                if (p + pp < ncontrib)
-#pragma unroll
-                                    for (int j = 0; j < 16; ++j) sum[j] += v[pp][j];
-                        }
-#pragma unroll
-                        for (int j = 0; j < 16; ++j) a.y[(size_t)(m + j) * a.N + n] = __float2bfloat16_rn(sum[j]);
+                        for (int i = 0; i < 16; ++i) __stcg(mine + (size_t)(c + i) * 128 + r, __uint_as_float(v[i]));
                     }
                 }
-                epi_bar();
+                tc_fence_before();
+                __syncwarp();
+                if (lane == 0) mbar_arrive(smem_u32(&tmem_empty[seg & 1]));
+                if (!complete) {
+                    __threadfence();
+                    epi_bar();
+                    if (etid == 0) {
+                        const uint32_t old = atomicAdd(counters + tn, 1u);
+                        last_flag = (old == ncontrib - 1);
+                        if (old == ncontrib - 1) counters[tn] = 0;               // self-reset for the next launch
+                    }
+                    epi_bar();
+                    if (last_flag) {
+                        __threadfence();
+                        const float* base = part + (size_t)tn * op.maxc * nout;
+                        for (uint32_t m = 0; m < a.batch; m += 16) {
+                            float sum[16];
+#pragma unroll
+                            for (int i = 0; i < 16; ++i) sum[i] = 0.f;
+                            // 4 contributors x 16 values = 64 loads in flight per thread (the loop is L2-latency bound: with
+                            // 16 in flight a [128 x 128] tile row took ~25 us); the additions stay in contributor order.
+                            for (uint32_t p = 0; p < ncontrib; p += 4) {
+                                float v[4][16];
+#pragma unroll
+                                for (int pp = 0; pp < 4; ++pp) {
+                                    const float* src = base + (size_t)(p + pp) * nout + (size_t)m * 128 + r;
+#pragma unroll
+                                    for (int i = 0; i < 16; ++i) v[pp][i] = (p + pp < ncontrib) ? __ldcg(src + i * 128) : 0.f;
+                                }
+#pragma unroll
+                                for (int pp = 0; pp < 4; ++pp)
+                                    if (p + pp < ncontrib)
+#pragma unroll
+                                        for (int i = 0; i < 16; ++i) sum[i] += v[pp][i];
+                            }
+#pragma unroll
+                            for (int i = 0; i < 16; ++i) op.y[(size_t)(m + i) * op.N + n] = __float2bfloat16_rn(sum[i]);
+                        }
+                    }
+                    epi_bar();
+                }
+                u = seg_last + 1;
             }
-            u = seg_last + 1;
         }
     }
     tc_fence_before();
@@ -290,49 +328,62 @@ cloak_status check_linear(const cloak_pool* pool, const cloak_tensor* w, const v
 
 using namespace cloak;
 
-extern "C" cloak_status cloak_gemm(const cloak_pool* pool, const cloak_tensor* w, const void* d_x, void* d_y,
-                                   uint32_t batch, void* stream) {
-    cloak_status st = check_linear(pool, w, d_x, d_y, "gemm");
-    if (st != CLOAK_OK) return st;
-    if (batch < 16 || batch > 256 || batch % 16) return fail(CLOAK_ERR_INVALID, "gemm: batch must be a multiple of 16 in 16..256");
-    if (w->dt != CLOAK_BF16 || w->layout != CLOAK_TILE128) return fail(CLOAK_ERR_UNSUPPORTED, "gemm: needs CLOAK_BF16 in CLOAK_TILE128 layout");
-    if (w->N % 128 || w->K % 128) return fail(CLOAK_ERR_ALIGN, "gemm: N and K must be multiples of 128");
-    if (pool->block < 32768) return fail(CLOAK_ERR_UNSUPPORTED, "gemm: block_bytes must be >= 32 KiB (one 128x128 bf16 tile)");
-    DeviceGuard g(pool->device);
-    cudaStream_t s = (cudaStream_t)stream;
+namespace cloak {
 
+static cloak_status gemm_check(const cloak_pool* pool, const cloak_tensor* w, const void* d_x, void* d_y, uint32_t batch,
+                               const char* who) {
+    cloak_status st = check_linear(pool, w, d_x, d_y, who);
+    if (st != CLOAK_OK) return st;
+    if (batch < 16 || batch > 256 || batch % 16) return fail(CLOAK_ERR_INVALID, "%s: batch must be a multiple of 16 in 16..256", who);
+    if (w->dt != CLOAK_BF16 || w->layout != CLOAK_TILE128) return fail(CLOAK_ERR_UNSUPPORTED, "%s: needs CLOAK_BF16 in CLOAK_TILE128 layout", who);
+    if (w->N % 128 || w->K % 128) return fail(CLOAK_ERR_ALIGN, "%s: N and K must be multiples of 128", who);
+    if (pool->block < 32768) return fail(CLOAK_ERR_UNSUPPORTED, "%s: block_bytes must be >= 32 KiB (one 128x128 bf16 tile)", who);
+    return CLOAK_OK;
+}
+
+// One launch of n <= GM_MAX_OPS checked ops.
+static cloak_status gemm_launch(const cloak_pool* pool, const cloak_gemm_op* ops, uint32_t n, uint32_t batch, cudaStream_t s) {
+    cloak_status st;
     if (!pool->tmap_ready) {
         cloak_pool* p = const_cast<cloak_pool*>(pool);
         st = make_map(&p->tmap_tile128, pool->base, 128, pool->bytes() / 256, 256, 64, 128);
         if (st != CLOAK_OK) return st;
         p->tmap_ready = true;
     }
-    CUtensorMap map_x;
-    st = make_map(&map_x, d_x, w->K, batch, (uint64_t)w->K * 2, 64, batch);
-    if (st != CLOAK_OK) return st;
-
     GemmArgs a;
     a.T = pool->d_T;
     a.log2b = pool->log2_block;
-    a.w_offset = w->w_offset;
-    a.N = w->N;
-    a.K = w->K;
     a.batch = batch;
-    a.y = static_cast<__nv_bfloat16*>(d_y);
-    a.kt = w->K / 128;
-    const uint32_t tile_rows = w->N / 128;
-    const uint64_t units64 = (uint64_t)tile_rows * a.kt;
-    if (units64 > 0xffffffffull) return fail(CLOAK_ERR_UNSUPPORTED, "gemm: tensor too large");
-    a.units = (uint32_t)units64;
+    a.nops = n;
     const int sms = sm_count(pool->device);
-    a.per = (a.units + sms - 1) / sms;
-    {   // cap the contributors per tile row (fp32 partials are batch * 512 B per contributor): ~10 at batch 32, ~4 at 128
-        uint32_t cap = 512 / batch;
-        cap = cap < 4 ? 4 : (cap > 10 ? 10 : cap);
-        if (a.per < (a.kt + cap - 1) / cap) a.per = (a.kt + cap - 1) / cap;
+    uint32_t cap = 512 / batch;         // contributors per tile row (fp32 partials are batch * 512 B each): ~10 at batch 32, 4 at 128
+    cap = cap < 4 ? 4 : (cap > 10 ? 10 : cap);
+    uint64_t rows = 0, part = 0;
+    uint32_t ctas = 1;
+    for (uint32_t j = 0; j < n; ++j) {
+        const cloak_tensor& w = ops[j].w;
+        st = make_map(&a.map_x[j], ops[j].d_x, w.K, batch, (uint64_t)w.K * 2, 64, batch);
+        if (st != CLOAK_OK) return st;
+        GemmOp& o = a.ops[j];
+        o.w_offset = w.w_offset;
+        o.y = static_cast<__nv_bfloat16*>(ops[j].d_y);
+        o.N = w.N;
+        o.kt = w.K / 128;
+        const uint32_t tile_rows = w.N / 128;
+        const uint64_t units64 = (uint64_t)tile_rows * o.kt;
+        if (units64 > 0xffffffffull) return fail(CLOAK_ERR_UNSUPPORTED, "gemm: tensor too large");
+        o.units = (uint32_t)units64;
+        o.per = (o.units + sms - 1) / sms;
+        if (o.per < (o.kt + cap - 1) / cap) o.per = (o.kt + cap - 1) / cap;
+        const uint32_t c = (o.units + o.per - 1) / o.per;
+        if (c > ctas) ctas = c;
+        o.maxc = (o.kt + o.per - 1) / o.per + 1;
+        o.row_base = (uint32_t)rows;
+        o.part_base = part;
+        rows += tile_rows;
+        part += (uint64_t)tile_rows * o.maxc * batch * 128;
     }
-    const int ctas = (int)((a.units + a.per - 1) / a.per);
-    a.maxc = (a.kt + a.per - 1) / a.per + 1;
+    if (rows * 4 > WS_COUNTER_BYTES) return fail(CLOAK_ERR_UNSUPPORTED, "gemm: too many output rows for the tile counters");
     const uint32_t xtile = batch * 256;
     a.xstages = 2;
     uint32_t wst = (224u * 1024u - a.xstages * xtile) / 32768u;
@@ -341,9 +392,7 @@ extern "C" cloak_status cloak_gemm(const cloak_pool* pool, const cloak_tensor* w
     a.wstages = wst;
     a.tmem_cols = 32;
     while (a.tmem_cols < 2 * batch) a.tmem_cols <<= 1;
-    if ((size_t)tile_rows * 4 > WS_COUNTER_BYTES) return fail(CLOAK_ERR_UNSUPPORTED, "gemm: N too large for the tile counters");
-    const size_t need = WS_COUNTER_BYTES + (size_t)tile_rows * a.maxc * batch * 128 * 4;
-    st = pool_workspace(pool, need);
+    st = pool_workspace(pool, WS_COUNTER_BYTES + part * 4);
     if (st != CLOAK_OK) return st;
     a.counters = reinterpret_cast<uint32_t*>(pool->ws);
     a.part = reinterpret_cast<float*>(pool->ws + WS_COUNTER_BYTES);
@@ -366,7 +415,41 @@ extern "C" cloak_status cloak_gemm(const cloak_pool* pool, const cloak_tensor* w
     at[0].val.programmaticStreamSerializationAllowed = 1;
     cfg.attrs = at;
     cfg.numAttrs = g_gemv_pdl ? 1 : 0;
-    CLOAK_CUDA(cudaLaunchKernelEx(&cfg, gemm_tile128_kernel, pool->tmap_tile128, map_x, a));
+    CLOAK_CUDA(cudaLaunchKernelEx(&cfg, gemm_tile128_kernel, pool->tmap_tile128, a));
     launched();
+    return CLOAK_OK;
+}
+
+}  // namespace cloak
+
+extern "C" cloak_status cloak_gemm(const cloak_pool* pool, const cloak_tensor* w, const void* d_x, void* d_y,
+                                   uint32_t batch, void* stream) {
+    cloak_status st = gemm_check(pool, w, d_x, d_y, batch, "gemm");
+    if (st != CLOAK_OK) return st;
+    DeviceGuard g(pool->device);
+    cloak_gemm_op op;
+    op.w = *w;
+    op.d_x = d_x;
+    op.d_y = d_y;
+    return gemm_launch(pool, &op, 1, batch, (cudaStream_t)stream);
+}
+
+extern "C" cloak_status cloak_gemm_chain(const cloak_pool* pool, const cloak_gemm_op* h_ops, uint32_t n_ops, uint32_t batch,
+                                         void* stream) {
+    if (!h_ops || n_ops == 0) return fail(CLOAK_ERR_INVALID, "gemm_chain: no ops");
+    for (uint32_t i = 0; i < n_ops; ++i) {
+        cloak_status st = gemm_check(pool, &h_ops[i].w, h_ops[i].d_x, h_ops[i].d_y, batch, "gemm_chain");
+        if (st != CLOAK_OK) return st;
+    }
+    DeviceGuard g(pool->device);
+    for (uint32_t i = 0; i < n_ops;) {                      // at most GM_MAX_OPS ops and 2^18 tile rows per launch
+        uint32_t n = 0;
+        uint64_t rows = 0;
+        while (i + n < n_ops && n < (uint32_t)GM_MAX_OPS && rows + h_ops[i + n].w.N / 128 <= 200000) rows += h_ops[i + n++].w.N / 128;
+        if (n == 0) return fail(CLOAK_ERR_UNSUPPORTED, "gemm_chain: op %u has too many output rows", i);
+        cloak_status st = gemm_launch(pool, h_ops + i, n, batch, (cudaStream_t)stream);
+        if (st != CLOAK_OK) return st;
+        i += n;
+    }
     return CLOAK_OK;
 }

@@ -334,22 +334,38 @@ def run_cfg3(args):
                  for pn_ in ("cloaked", "native")}
 
             def sweep(pool, y):
+                """Call by call: 7 cloak_gemm per layer."""
                 for l in range(layers):
                     for nm in lnames:
                         t = T[f"l{l}.{nm}"]
                         C.cloak_gemm(pool, t, X[t.K], y[nm], batch)
 
+            def sweep_ops(yl):
+                """The same 7 x layers GEMMs as one cloak_gemm_chain (the library launches 16 ops at a time).  The
+                inputs are fixed synthetic matrices, so no op depends on another; every op has its own output."""
+                return C.cloak_gemm_ops([(T[f"l{l}.{nm}"], X[T[f"l{l}.{nm}"].K], yl[l][nm]) for l in range(layers) for nm in lnames])
+
             res = {}
             for pool_name, pool in (("cloaked", pc), ("native", pn)):
                 y = Y[pool_name]
-                med, mn = time_gpu(torch, lambda: sweep(pool, y), args.reps, warmup=2)
-                gmed, gmn = time_gpu(torch, graphed(torch, lambda: sweep(pool, y)), args.reps, warmup=2)
+                yl = [{nm: torch.zeros_like(y[nm]) for nm in lnames} for _ in range(layers)]
+                ops = sweep_ops(yl)
                 flops = 2.0 * batch * (payload / 2)
-                res[pool_name] = {"stream": dict(rate(payload, med, peak), ms_min=mn, tflops=flops / med / 1e9),
-                                  "graph": dict(rate(payload, gmed, peak), ms_min=gmn, tflops=flops / gmed / 1e9)}
-            res["identical"] = bool(all(torch.equal(Y["cloaked"][nm], Y["native"][nm]) for nm in lnames))
-            res["overhead_pct"] = {k: (res["cloaked"][k]["ms"] - res["native"][k]["ms"]) / res["native"][k]["ms"] * 100
-                                   for k in ("stream", "graph")}
+                r = {}
+                for mode, fn in (("per_call", lambda: sweep(pool, y)), ("chain", lambda: C.cloak_gemm_chain(pool, ops, batch))):
+                    med, mn = time_gpu(torch, fn, args.reps, warmup=2)
+                    gmed, gmn = time_gpu(torch, graphed(torch, fn), args.reps, warmup=2)
+                    r[mode] = {"stream": dict(rate(payload, med, peak), ms_min=mn, tflops=flops / med / 1e9),
+                               "graph": dict(rate(payload, gmed, peak), ms_min=gmn, tflops=flops / gmed / 1e9)}
+                # the call-by-call sweep reuses one output set, so what it leaves behind is the last layer's
+                r["chain_identical_to_per_call"] = bool(all(torch.equal(yl[layers - 1][nm], y[nm]) for nm in lnames))
+                res[pool_name] = r
+                Y[pool_name + "_chain"] = yl
+            res["identical"] = bool(all(torch.equal(Y["cloaked"][nm], Y["native"][nm]) for nm in lnames)
+                                    and all(torch.equal(a[nm], b[nm]) for a, b in zip(Y["cloaked_chain"], Y["native_chain"]) for nm in lnames))
+            del Y
+            res["overhead_pct"] = {f"{mode}_{k}": (res["cloaked"][mode][k]["ms"] - res["native"][mode][k]["ms"])
+                                   / res["native"][mode][k]["ms"] * 100 for mode in ("per_call", "chain") for k in ("stream", "graph")}
             out[f"b{batch}"] = res
     finally:
         torch.cuda.synchronize()

@@ -528,6 +528,42 @@ def test_gemm_vs_oracle_and_identity_bit_identical(block, shapes, batches):
                 assert torch.equal(yc, yc2)
 
 
+@pytest.mark.parametrize("batch", [32, 128])
+def test_gemm_chain_equals_single_calls(batch):
+    """cloak_gemm_chain: 20 ops of mixed shapes (two launches of <= 16 ops), bit-identical to cloak_gemm op by op, on
+    the cloaked and the identity-table pool, repeatable; a sample of ops against the fp64 oracle."""
+    key, seed, block, page = 0x1234, 3, 65536, 2 << 20
+    shapes = [(1024, 5120), (5120, 1024), (384, 640), (128, 128), (2560, 2560)] * 4
+    Ws = [gen.synth(seed, i, shp, "bf16") for i, shp in enumerate(shapes[:5])]
+    sizes = [2 * n * k for n, k in shapes]
+    offs, total = C.cloak_arena_plan(key, sizes, block)
+    with Pool(total, block, page, key) as pc, Pool(total, block, page, key, C.CLOAK_POOL_IDENTITY) as pi:
+        for i, ((n, k), off) in enumerate(zip(shapes, offs)):
+            src = bf16_dev_from_bits(Ws[i % 5])
+            til = torch.empty(n * k, dtype=torch.bfloat16, device="cuda")
+            C.cloak_to_tile128(src, til, n, k, C.CLOAK_BF16)
+            for p in (pc, pi):
+                C.cloak_shuffle(p.h, til, off, n * k * 2)
+        X = {k: gen.synth(seed + 100, k, (batch, k), "bf16", kind=gen.KIND_NORMAL) for k in {k for _, k in shapes}}
+        dX = {k: bf16_dev_from_bits(v) for k, v in X.items()}
+        T = [C.cloak_tensor(off, n, k, C.CLOAK_BF16, C.CLOAK_TILE128) for (n, k), off in zip(shapes, offs)]
+
+        def outs():
+            return [torch.zeros(batch, n, dtype=torch.bfloat16, device="cuda") for n, _ in shapes]
+        yc, yi, ys, yr = outs(), outs(), outs(), outs()
+        C.cloak_gemm_chain(pc.h, [(T[i], dX[shapes[i][1]], yc[i]) for i in range(len(shapes))], batch)
+        C.cloak_gemm_chain(pi.h, [(T[i], dX[shapes[i][1]], yi[i]) for i in range(len(shapes))], batch)
+        for i in range(len(shapes)):
+            C.cloak_gemm(pc.h, T[i], dX[shapes[i][1]], ys[i], batch)
+        C.cloak_gemm_chain(pc.h, [(T[i], dX[shapes[i][1]], yr[i]) for i in range(len(shapes))], batch)
+        torch.cuda.synchronize()
+        for i in range(len(shapes)):
+            assert torch.equal(yc[i], yi[i]) and torch.equal(yc[i], ys[i]) and torch.equal(yc[i], yr[i]), i
+        for i in (0, 1, 2, 3, 4, 17):
+            err = O.err_normwise(yc[i].float().cpu().numpy(), O.linear_f64(X[shapes[i][1]], Ws[i % 5]))
+            assert err <= TOL["bf16"], (i, err)
+
+
 def test_gemm_argument_checks():
     with Pool(1 << 20, 4096, 65536, 1) as p:
         x = torch.zeros(32, 128, dtype=torch.bfloat16, device="cuda")
