@@ -127,20 +127,36 @@ __global__ void __launch_bounds__(512) gather_cols_kernel(const E* __restrict__ 
     if (threadIdx.x == 0)
         for (uint32_t k = 0; k < ns && k < mine; ++k) issue(k);
     constexpr int EPV = 16 / sizeof(E);
+    struct alignas(sizeof(M) * EPV) CmVec { M m[EPV]; };      // the EPV map entries of one output vector: one LDS
+    const CmVec* cmv = reinterpret_cast<const CmVec*>(colmap);
     const uint32_t vpr = ncols / EPV;
-    for (uint32_t k = 0; k < mine; ++k) {
-        const uint32_t st = k % ns;
-        mbar_wait(smem_u32(&full[st]), (k / ns) & 1);
-        const E* row = reinterpret_cast<const E*>(ring + (size_t)st * row_bytes);
-        const uint64_t v0 = (uint64_t)(blockIdx.x + k * gridDim.x) * vpr;
+    // Two rows per pass: the map entries are read once (vectorised) for both, which takes the shared-memory
+    // instruction count per output vector from 2 x EPV to EPV + 1/2 -- the gather is LDS-bound, not HBM-bound.
+    for (uint32_t k = 0; k < mine; k += 2) {
+        const bool two = k + 1 < mine;
+        const uint32_t sa = k % ns, sb = (k + 1) % ns;
+        mbar_wait(smem_u32(&full[sa]), (k / ns) & 1);
+        if (two) mbar_wait(smem_u32(&full[sb]), ((k + 1) / ns) & 1);
+        const E* ra = reinterpret_cast<const E*>(ring + (size_t)sa * row_bytes);
+        const E* rb = reinterpret_cast<const E*>(ring + (size_t)sb * row_bytes);
+        const uint64_t va = (uint64_t)(blockIdx.x + k * gridDim.x) * vpr, vb = va + (uint64_t)gridDim.x * vpr;
         for (uint32_t v = threadIdx.x; v < vpr; v += blockDim.x) {
-            union { int4 q; E e[EPV]; } out;
+            const CmVec c = cmv[v];
+            union { int4 q; E e[EPV]; } oa, ob;
 #pragma unroll
-            for (int j = 0; j < EPV; ++j) out.e[j] = row[colmap[v * EPV + j]];
-            dst.store(v0 + v, out.q);
+            for (int j = 0; j < EPV; ++j) oa.e[j] = ra[c.m[j]];
+            dst.store(va + v, oa.q);
+            if (two) {
+#pragma unroll
+                for (int j = 0; j < EPV; ++j) ob.e[j] = rb[c.m[j]];
+                dst.store(vb + v, ob.q);
+            }
         }
-        __syncthreads();                                       // every thread is done with this stage
-        if (threadIdx.x == 0 && k + ns < mine) issue(k + ns);
+        __syncthreads();                                       // every thread is done with both stages
+        if (threadIdx.x == 0) {
+            if (k + ns < mine) issue(k + ns);
+            if (two && k + 1 + ns < mine) issue(k + 1 + ns);
+        }
     }
 }
 
