@@ -125,6 +125,16 @@ cloak_status cloak_unshuffle(const cloak_pool* pool, void* d_logical, uint64_t l
  * Both pools must have the same payload and block size.  Asynchronous on `stream`. */
 cloak_status cloak_relayout(const cloak_pool* from_a, cloak_pool* to_b, void* stream);
 
+/* Re-key the block permutation of a pool IN PLACE ("reshuffled periodically ...
+ * no additional memory footprint"): afterwards the pool holds, under the block tables of `new_key` and its unchanged page
+ * map, exactly what it held before:  pool[T_new[i]] = old pool[T_old[i]]  for every block slot i, bit for bit what
+ * cloak_relayout into a second pool would give, zero pad slots included.  Pages are not re-mapped.  The only extra memory
+ * is a spare buffer of about spare_bytes (0 = one page): the permutation's cycles are cut into segments whose first block
+ * is saved there, and the more segments, the more of them move in parallel (one page is enough for full speed only on
+ * pools of a few hundred MB; 1/64 of the pool is on any).  The cycle decomposition runs on the host: the call
+ * synchronises `stream` and returns when the pool is re-keyed; GEMVs issued afterwards read through the new table. */
+cloak_status cloak_rekey_inplace(cloak_pool* pool, uint64_t new_key, uint64_t spare_bytes, void* stream);
+
 /* Host-buffer variants (end-to-end path): h_logical is a HOST buffer (pinned for full speed); the
  * library stages it through device memory in chunks.  They synchronise `stream` before returning. */
 cloak_status cloak_shuffle_host(cloak_pool* pool, const void* h_logical, uint64_t logical_offset,

@@ -173,6 +173,45 @@ def test_relayout_bit_exact(payload, block, page, engine):
         C.cloak_set_copy_engine(0)
 
 
+@pytest.mark.parametrize("payload,block,page,spare", [
+    (3 << 20, 4096, 65536, 0),                     # emulated pages, one page of spare
+    ((1 << 20) + 4096 * 3 + 1040, 4096, 65536, 4096),   # ragged payload, a single spare block: one long chain per cycle
+    (40 << 20, 65536, 2 << 20, 0),                 # real VMM pages
+    (40 << 20, 65536, 2 << 20, 16 << 20),          # lots of spare: many short segments
+    (100 * 256, 256, 1024, 0),                     # tiny blocks
+])
+def test_rekey_inplace_equals_oracle_relayout(payload, block, page, spare):
+    """NEXT-1: cloak_rekey_inplace leaves the pool exactly as the oracle's relayout(pool, T_A, T_B) over the unchanged page
+    map, the tables are key B's block tables + key A's page tables, and reads through the new table give the data."""
+    key_a, key_b = 0x1234, 0x5678
+    g = O.pool_geometry(payload, block, page)
+    ta, tb = O.pool_tables(key_a, g), O.pool_tables(key_b, g)
+    L = np.random.default_rng(11).integers(0, 256, payload, dtype=np.uint8)
+    padded = (payload + 15) // 16 * 16
+    dL = torch.cat([to_dev_bytes(L), dev_bytes(padded - payload)]) if padded != payload else to_dev_bytes(L)
+    with Pool(payload, block, page, key_a) as p:
+        vmm = p.info["is_vmm"]
+        C.cloak_shuffle(p.h, dL, 0, padded)
+        before = p.raw()
+        # O5 over an unchanged page map: the memory slot of logical block i under key B
+        sb = tb.blockinv[:g.nb].astype(np.int64)
+        T_b = tb.T_vmm if vmm else (ta.pageinv[sb // g.bpp].astype(np.int64) * g.bpp + sb % g.bpp).astype(np.uint32)
+        T_a = ta.T_vmm if vmm else ta.T_emulated
+        C.cloak_rekey_inplace(p.h, key_b, spare)
+        assert np.array_equal(p.raw(), O.relayout(before, T_a, T_b, g))
+        bp, bi, pp, pinv = p.tables()
+        assert np.array_equal(bp, tb.blockperm) and np.array_equal(bi, tb.blockinv)
+        assert np.array_equal(pp, ta.pageperm) and np.array_equal(pinv, ta.pageinv)
+        assert np.array_equal(p.table_T(), T_b)
+        out = dev_bytes(padded)
+        C.cloak_unshuffle(p.h, out, 0, padded)
+        assert np.array_equal(out.cpu().numpy()[:payload], L)
+        C.cloak_rekey_inplace(p.h, key_b, spare)                   # same key again: nothing moves
+        assert np.array_equal(p.table_T(), T_b)
+        C.cloak_rekey_inplace(p.h, key_a, spare)                   # and back
+        assert np.array_equal(p.raw(), before)
+
+
 def test_host_buffer_round_trip():
     payload, block, page, key = (5 << 20) + 4096 + 32, 4096, 2 << 20, 0x1234
     g = O.pool_geometry(payload, block, page)
