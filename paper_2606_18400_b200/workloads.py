@@ -103,6 +103,21 @@ def run_cfg4(args):
             back.zero_()
             C.cloak_unshuffle(pa, back, 0, nbytes)
             r["roundtrip_bit_exact"] = bool(torch.equal(back, L))
+            # NEXT-1: the same re-key in place (A -> B -> A -> ...), spare buffer 1/64 of the pool; host work included
+            keys = (c["key_b"], c["key"])
+            ts = []
+            for i in range(4):
+                torch.cuda.synchronize()
+                t0 = time.perf_counter()
+                C.cloak_rekey_inplace(pa, keys[i % 2], nbytes // 64)
+                torch.cuda.synchronize()
+                ts.append((time.perf_counter() - t0) * 1e3)
+            r["rekey_inplace"] = dict(rate(2 * nbytes, float(np.median(ts)), peak), spare_bytes=nbytes // 64,
+                                      note="wall clock: host cycle decomposition + upload + the two move passes")
+            back.zero_()
+            C.cloak_unshuffle(pa, back, 0, nbytes)
+            r["rekey_inplace_bit_exact"] = bool(torch.equal(back, L))
+            ok = ok and r["rekey_inplace_bit_exact"]
             back.zero_()
             C.cloak_unshuffle(pb, back, 0, nbytes)
             r["relayout_bit_exact"] = bool(torch.equal(back, L))
@@ -280,6 +295,26 @@ def run_cfg2(args):
             r["chain_identical_to_per_call"] = bool(all(torch.equal(snap[nm], y[nm]) for nm in y))
             res[pool_name] = r
         identical = all(torch.equal(Y["cloaked"][nm], Y["native"][nm]) for nm in Y["cloaked"])
+
+        # ---- NEXT-1: periodic in-place re-key under decode.  Wall clock of one re-key (host cycle decomposition included)
+        # for three spare-buffer sizes; the decode chain afterwards must give the same outputs through the new table.
+        ops_c = chain_ops(Y["cloaked"])
+        t_dec = res["cloaked"]["chain"]["graph"]["ms"]
+        rekey = {}
+        for label, spare, newkey in (("one_page", 0, 0x5678), ("64MiB", 64 << 20, 0x9abc), ("256MiB", 256 << 20, c["key"])):
+            torch.cuda.synchronize()
+            t0 = time.perf_counter()
+            C.cloak_rekey_inplace(pc, newkey, spare)
+            torch.cuda.synchronize()
+            ms = (time.perf_counter() - t0) * 1e3
+            snap = {nm: t.clone() for nm, t in Y["cloaked"].items()}
+            for t in Y["cloaked"].values():
+                t.zero_()
+            C.cloak_gemv_chain(pc, ops_c, 1)
+            torch.cuda.synchronize()
+            rekey[label] = {"spare_bytes": spare or c["page"], "ms": ms, "gbs": 2 * total / ms / 1e6,
+                            "decode_identical_after": bool(all(torch.equal(snap[nm], Y["cloaked"][nm]) for nm in snap)),
+                            "amortised_overhead_pct": {f"every_{n}": ms / (n * t_dec) * 100 for n in (1000, 1500)}}
         ov = {f"{mode}_{k}": (res["cloaked"][mode][k]["ms"] - res["native"][mode][k]["ms"]) / res["native"][mode][k]["ms"] * 100
               for mode in ("per_call", "chain") for k in ("stream", "graph")}
     finally:
@@ -298,6 +333,7 @@ def run_cfg2(args):
             "decode_chain": res, "decode_read_bytes": read_bytes,
             "ideal_tokens_per_s_at_measured_peak": peak * 1e9 / read_bytes,
             "cloaked_vs_native_overhead_pct": ov, "cloaked_identical_to_native": bool(identical),
+            "rekey_inplace": rekey,
             "gpu_launches": C.cloak_launch_count() - launches0}
 
 
