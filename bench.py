@@ -1,8 +1,9 @@
 #!/usr/bin/env python
 """bench.py -- one "step" = one pass of the whole cloaked-layout hot path over one LLaMA-8B-shaped decoder
 layer (BASELINE.json configs[1]): S1 keygen -> S3 arena plan -> S5 neuron/head permutation -> S4 block
-shuffle into the 2 MiB page pool -> S8 re-layout key A -> key B -> S6 cloaked GEMV of the 7 projections at
-batch 1, 4, 16 -> S4 unshuffle.  (S2, the VMM mapper, is load-time setup: timed separately, `pool_map_ms`.)
+shuffle into the 2 MiB page pool (the 7 tensors in one cloak_shuffle_many call) -> S8 re-layout key A -> key B ->
+S6 cloaked GEMV of the 7 projections at batch 1, 4, 16 (one cloak_gemv_chain call per batch) -> S4 unshuffle.
+(S2, the VMM mapper, is load-time setup: timed separately, `pool_map_ms`.)
 
     python bench.py [--gpus N] [--steps K] [--warmup W] [--impl cloak|reference]
 
@@ -265,16 +266,18 @@ def run_cloak(args):
     def st_permute():                                                                                      # S5
         C.cloak_permute_mlp_heads(KEY_A, sh, **raw, **{k + "_o": v for k, v in perm.items()})
 
-    def st_shuffle():                                                                                      # S4
-        for (nm, _), o in zip(shapes, offs):
-            C.cloak_shuffle(pool_a, perm[nm], o, perm[nm].numel() * 2)
+    lay_t = [perm[nm] for nm, _ in shapes]
+    lay_back = [back[nm] for nm, _ in shapes]
+    lay_b = [perm[nm].numel() * 2 for nm, _ in shapes]
+
+    def st_shuffle():                                                                                      # S4, the layer's 7 tensors in one call
+        C.cloak_shuffle_many(pool_a, lay_t, offs, lay_b)
 
     def st_relayout():                                                                                     # S8
         C.cloak_relayout(pool_a, pool_b)
 
     def st_unshuffle():                                                                                    # S4^-1
-        for (nm, _), o in zip(shapes, offs):
-            C.cloak_unshuffle(pool_a, back[nm], o, back[nm].numel() * 2)
+        C.cloak_unshuffle_many(pool_a, lay_back, offs, lay_b)
 
     stage_fns = ([st_keygen, st_permute, st_shuffle, st_relayout]
                  + [(lambda b=b: gemv_chain(pool_a, b)) for b in BATCHES] + [st_unshuffle])

@@ -121,6 +121,14 @@ cloak_status cloak_shuffle(cloak_pool* pool, const void* d_logical, uint64_t log
                            uint64_t bytes, void* stream);
 cloak_status cloak_unshuffle(const cloak_pool* pool, void* d_logical, uint64_t logical_offset,
                              uint64_t bytes, void* stream);
+/* The same for n arena ranges in one launch (per 128 ranges): range r is h_bytes[r] bytes at arena offset h_offsets[r],
+ * in the caller's device buffer d_logical[r]; h_logical pointers, offsets and sizes are HOST arrays of n entries, not
+ * referenced after the call returns.  Ranges must not overlap.  A model is hundreds of tensors and one launch per tensor
+ * leaves the small ones launch-bound.  Asynchronous on `stream`. */
+cloak_status cloak_shuffle_many(cloak_pool* pool, uint32_t n, const void* const* d_logical,
+                                const uint64_t* h_offsets, const uint64_t* h_bytes, void* stream);
+cloak_status cloak_unshuffle_many(const cloak_pool* pool, uint32_t n, void* const* d_logical,
+                                  const uint64_t* h_offsets, const uint64_t* h_bytes, void* stream);
 /* pool_b[T_b[i]] = pool_a[T_a[i]] for every logical block, without materialising the arena.
  * Both pools must have the same payload and block size.  Asynchronous on `stream`. */
 cloak_status cloak_relayout(const cloak_pool* from_a, cloak_pool* to_b, void* stream);

@@ -24,7 +24,7 @@ STATUS_NAMES = {0: "CLOAK_OK", -1: "CLOAK_ERR_INVALID", -2: "CLOAK_ERR_ALIGN", -
 # every symbol include/cloak.h declares
 SYMBOLS = ["cloak_last_error", "cloak_version", "cloak_launch_count", "cloak_keygen", "cloak_pool_create", "cloak_pool_destroy",
            "cloak_pool_info", "cloak_pool_tables", "cloak_pool_dump", "cloak_pool_map_ms", "cloak_pool_adjacency", "cloak_shuffle",
-           "cloak_unshuffle", "cloak_relayout", "cloak_rekey_inplace", "cloak_shuffle_host", "cloak_unshuffle_host",
+           "cloak_unshuffle", "cloak_shuffle_many", "cloak_unshuffle_many", "cloak_relayout", "cloak_rekey_inplace", "cloak_shuffle_host", "cloak_unshuffle_host",
            "cloak_set_copy_engine", "cloak_arena_plan", "cloak_permute_mlp_heads", "cloak_load_mlp_heads", "cloak_to_tile128",
            "cloak_gemv", "cloak_gemv_chain", "cloak_gemm", "cloak_gemm_chain", "cloak_set_gemv_engine", "cloak_gemv_host", "cloak_silu_mul"]
 
@@ -72,6 +72,8 @@ lib.cloak_pool_map_ms.argtypes = [_P, POINTER(c_double)]
 lib.cloak_pool_adjacency.argtypes = [_P, POINTER(c_double), POINTER(c_double), POINTER(c_double)]
 lib.cloak_shuffle.argtypes = [_P, _P, c_uint64, c_uint64, _P]
 lib.cloak_unshuffle.argtypes = [_P, _P, c_uint64, c_uint64, _P]
+lib.cloak_shuffle_many.argtypes = [_P, c_uint32, POINTER(c_void_p), POINTER(c_uint64), POINTER(c_uint64), _P]
+lib.cloak_unshuffle_many.argtypes = [_P, c_uint32, POINTER(c_void_p), POINTER(c_uint64), POINTER(c_uint64), _P]
 lib.cloak_relayout.argtypes = [_P, _P, _P]
 lib.cloak_rekey_inplace.argtypes = [_P, c_uint64, c_uint64, _P]
 lib.cloak_shuffle_host.argtypes = [_P, _P, c_uint64, c_uint64, _P]
@@ -185,6 +187,20 @@ def cloak_shuffle(pool, d_logical, logical_offset, nbytes, stream=None):
 
 def cloak_unshuffle(pool, d_logical, logical_offset, nbytes, stream=None):
     _check(lib.cloak_unshuffle(pool, _ptr(d_logical), logical_offset, nbytes, _stream(stream)))
+
+
+def _many(tensors, offsets, nbytes):
+    n = len(tensors)
+    ptrs = (c_void_p * n)(*[_ptr(t) for t in tensors])
+    return n, ptrs, (c_uint64 * n)(*offsets), (c_uint64 * n)(*nbytes)
+
+
+def cloak_shuffle_many(pool, tensors, offsets, nbytes, stream=None):
+    _check(lib.cloak_shuffle_many(pool, *_many(tensors, offsets, nbytes), _stream(stream)))
+
+
+def cloak_unshuffle_many(pool, tensors, offsets, nbytes, stream=None):
+    _check(lib.cloak_unshuffle_many(pool, *_many(tensors, offsets, nbytes), _stream(stream)))
 
 
 def cloak_relayout(from_a, to_b, stream=None):

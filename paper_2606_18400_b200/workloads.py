@@ -232,6 +232,8 @@ def run_cfg2(args):
             for nm, _ in tensors:
                 C.cloak_shuffle(pc, keep[nm], off[nm], keep[nm].numel() * 2)
         sh_med, sh_min = time_gpu(torch, shuffle_all, args.reps)
+        m_t, m_o, m_b = [keep[nm] for nm, _ in tensors], [off[nm] for nm, _ in tensors], [keep[nm].numel() * 2 for nm, _ in tensors]
+        shm_med, shm_min = time_gpu(torch, lambda: C.cloak_shuffle_many(pc, m_t, m_o, m_b), args.reps)
         back = torch.empty(payload // 2, dtype=torch.bfloat16, device="cuda")
         views, at = {}, 0
         for nm, (n, k) in tensors:
@@ -242,6 +244,8 @@ def run_cfg2(args):
             for nm, _ in tensors:
                 C.cloak_unshuffle(pc, views[nm], off[nm], views[nm].numel() * 2)
         un_med, un_min = time_gpu(torch, unshuffle_all, args.reps)
+        m_v = [views[nm] for nm, _ in tensors]
+        unm_med, unm_min = time_gpu(torch, lambda: C.cloak_unshuffle_many(pc, m_v, m_o, m_b), args.reps)
         roundtrip = all(torch.equal(views[nm], keep[nm]) for nm, _ in tensors)
         del back, views
 
@@ -329,6 +333,8 @@ def run_cfg2(args):
             "layout_adjacency": adjacency,
             "shuffle": dict(rate(2 * payload, sh_med, peak), ms_min=sh_min),
             "unshuffle": dict(rate(2 * payload, un_med, peak), ms_min=un_min), "roundtrip_bit_exact": bool(roundtrip),
+            "shuffle_many": dict(rate(2 * payload, shm_med, peak), ms_min=shm_min, launches=2),
+            "unshuffle_many": dict(rate(2 * payload, unm_med, peak), ms_min=unm_min, launches=2),
             "load_paths": load_paths,
             "decode_chain": res, "decode_read_bytes": read_bytes,
             "ideal_tokens_per_s_at_measured_peak": peak * 1e9 / read_bytes,

@@ -136,6 +136,33 @@ def test_pool_adjacency_matches_the_oracle(payload, block, page):
         assert C.cloak_pool_adjacency(pi.h) == dict(va_blocks=1.0, physical_blocks=1.0, pages=1.0)
 
 
+@pytest.mark.parametrize("block,page,n", [(4096, 65536, 5), (65536, 2 << 20, 150), (256, 1024, 4)])
+def test_shuffle_many_equals_one_call_per_range(block, page, n):
+    """cloak_shuffle_many / cloak_unshuffle_many: n tensors of mixed sizes (ragged tails, > 128 ranges -> two launches) in
+    one call leave the pool exactly as the oracle's shuffle_into of each, and come back bit for bit."""
+    key = 0x1234
+    rng = np.random.default_rng(5)
+    sizes = [int(rng.integers(1, 40)) * block // 2 // 16 * 16 + (16 if i % 3 == 0 else 0) for i in range(n)]
+    offs, total = C.cloak_arena_plan(key, sizes, block)
+    g = O.pool_geometry(total, block, page)
+    t = O.pool_tables(key, g)
+    datas = [rng.integers(1, 256, s_, dtype=np.uint8) for s_ in sizes]
+    with Pool(total, block, page, key) as p:
+        T = t.T_vmm if p.info["is_vmm"] else t.T_emulated
+        ref = np.zeros(g.nslots * block, np.uint8)
+        for d, o in zip(datas, offs):
+            O.shuffle_into(ref, T, d, o, block)
+        dev = [to_dev_bytes(d) for d in datas]
+        C.cloak_shuffle_many(p.h, dev, offs, sizes)
+        assert np.array_equal(p.raw(), ref)
+        outs = [dev_bytes(s_) for s_ in sizes]
+        C.cloak_unshuffle_many(p.h, outs, offs, sizes)
+        for d, o_ in zip(datas, outs):
+            assert np.array_equal(o_.cpu().numpy(), d)
+        with pytest.raises(C.CloakError):
+            C.cloak_shuffle_many(p.h, dev[:1], [offs[0] + 16], sizes[:1])        # offset not a block multiple
+
+
 def test_identity_pool_is_the_native_layout():
     payload, block, page = 3 << 20, 65536, 2 << 20
     L = np.random.default_rng(3).integers(0, 256, payload, dtype=np.uint8)
