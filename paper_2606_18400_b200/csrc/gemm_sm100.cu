@@ -36,6 +36,8 @@ struct GemmOp {
     uint32_t per;        // units per CTA
     uint32_t maxc;       // max contributors per tile row
     uint32_t row_base;   // index of this op's first tile-row counter
+    uint32_t rot;        // range r of this op belongs to CTA (r + rot) % grid: ops with fewer ranges than CTAs start where
+                         // the previous op stopped, so the idle CTAs are different ones each time
 };
 
 struct GemmArgs {
@@ -136,7 +138,8 @@ __global__ void __launch_bounds__(GM_THREADS, 1) gemm_tile128_kernel(const __gri
         uint32_t it = 0;
         for (uint32_t j = 0; j < a.nops; ++j) {
             const GemmOp& op = a.ops[j];
-            const uint32_t ubeg = blockIdx.x * op.per, uend = min(ubeg + op.per, op.units);
+            const uint32_t vr = (blockIdx.x + gridDim.x - op.rot) % gridDim.x;      // this CTA's range of the op
+            const uint32_t ubeg = vr * op.per, uend = min(ubeg + op.per, op.units);
             for (uint32_t u = ubeg; u < uend; ++u, ++it) {
                 const uint32_t s = it % a.wstages, f = it / a.wstages;
                 if (f > 0) mbar_wait(smem_u32(&wempty[s]), (f - 1) & 1);
@@ -157,7 +160,8 @@ __global__ void __launch_bounds__(GM_THREADS, 1) gemm_tile128_kernel(const __gri
         uint32_t it = 0;
         for (uint32_t j = 0; j < a.nops; ++j) {
             const GemmOp& op = a.ops[j];
-            const uint32_t ubeg = blockIdx.x * op.per, uend = min(ubeg + op.per, op.units);
+            const uint32_t vr = (blockIdx.x + gridDim.x - op.rot) % gridDim.x;      // this CTA's range of the op
+            const uint32_t ubeg = vr * op.per, uend = min(ubeg + op.per, op.units);
             for (uint32_t u = ubeg; u < uend; ++u, ++it) {
                 const uint32_t s = it % a.xstages, f = it / a.xstages;
                 if (f > 0) mbar_wait(smem_u32(&xempty[s]), (f - 1) & 1);
@@ -182,7 +186,8 @@ __global__ void __launch_bounds__(GM_THREADS, 1) gemm_tile128_kernel(const __gri
         };
         for (uint32_t j = 0; j < a.nops; ++j) {
             const GemmOp& op = a.ops[j];
-            const uint32_t ubeg = blockIdx.x * op.per, uend = min(ubeg + op.per, op.units);
+            const uint32_t vr = (blockIdx.x + gridDim.x - op.rot) % gridDim.x;      // this CTA's range of the op
+            const uint32_t ubeg = vr * op.per, uend = min(ubeg + op.per, op.units);
             if (ubeg >= uend) continue;
             uint32_t cur_tn = ubeg / op.kt;
             bool first = true;
@@ -228,7 +233,8 @@ __global__ void __launch_bounds__(GM_THREADS, 1) gemm_tile128_kernel(const __gri
         for (uint32_t j = 0; j < a.nops; ++j) {
             const GemmOp& op = a.ops[j];
             const uint32_t kt = op.kt;
-            const uint32_t ubeg = blockIdx.x * op.per, uend = min(ubeg + op.per, op.units);
+            const uint32_t vr = (blockIdx.x + gridDim.x - op.rot) % gridDim.x;      // this CTA's range of the op
+            const uint32_t ubeg = vr * op.per, uend = min(ubeg + op.per, op.units);
             float* part = a.part + op.part_base;
             uint32_t* counters = a.counters + op.row_base;
             for (uint32_t u = ubeg; u < uend; ++seg) {
@@ -241,7 +247,7 @@ __global__ void __launch_bounds__(GM_THREADS, 1) gemm_tile128_kernel(const __gri
                 const uint32_t taddr = tmem_base + ((q * 32) << 16) + (seg & 1) * a.batch;
                 const size_t n = (size_t)tn * 128 + r;
                 const uint32_t c_first = t_first / op.per, c_last = t_last / op.per;
-                const uint32_t ncontrib = c_last - c_first + 1, me = blockIdx.x - c_first;
+                const uint32_t ncontrib = c_last - c_first + 1, me = vr - c_first;
                 float* mine = part + ((size_t)tn * op.maxc + me) * nout;
                 for (uint32_t c = 0; c < a.batch; c += 16) {
                     uint32_t v[16];
@@ -359,7 +365,7 @@ static cloak_status gemm_launch(const cloak_pool* pool, const cloak_gemm_op* ops
     uint32_t cap = 512 / batch;         // contributors per tile row (fp32 partials are batch * 512 B each): ~10 at batch 32, 4 at 128
     cap = cap < 4 ? 4 : (cap > 10 ? 10 : cap);
     uint64_t rows = 0, part = 0;
-    uint32_t ctas = 1;
+    uint32_t ctas = 1, nranges_so_far = 0;
     for (uint32_t j = 0; j < n; ++j) {
         const cloak_tensor& w = ops[j].w;
         st = make_map(&a.map_x[j], ops[j].d_x, w.K, batch, (uint64_t)w.K * 2, 64, batch);
@@ -379,10 +385,13 @@ static cloak_status gemm_launch(const cloak_pool* pool, const cloak_gemm_op* ops
         if (c > ctas) ctas = c;
         o.maxc = (o.kt + o.per - 1) / o.per + 1;
         o.row_base = (uint32_t)rows;
+        o.rot = nranges_so_far;
+        nranges_so_far += c;
         o.part_base = part;
         rows += tile_rows;
         part += (uint64_t)tile_rows * o.maxc * batch * 128;
     }
+    for (uint32_t j = 0; j < n; ++j) a.ops[j].rot %= ctas;
     if (rows * 4 > WS_COUNTER_BYTES) return fail(CLOAK_ERR_UNSUPPORTED, "gemm: too many output rows for the tile counters");
     const uint32_t xtile = batch * 256;
     a.xstages = 2;
