@@ -18,7 +18,8 @@ Parity pins (tests/test_oracle_*.py, all `-m "not gpu"`): Philox known answers +
 generator; worked examples W1-W5 of SURVEY.md 8(c).4 under tests/golden/; O(n^2) brute-force
 rank; bijection / restriction / forced-tie properties; byte-at-a-time restatement of O5;
 unshuffle(shuffle)=id; relayout A->A = id, A->B->A; MLP' = MLP and attention' = attention
-brute-forced in fp64; W = I and W = ones closed forms for GEMV.  Parity unpinned: none.
+brute-forced in fp64; MoE' = MoE (expert + per-expert neuron permutation) brute-forced in fp64 with negative controls and
+the E = 1 / k = 1 reductions to the dense MLP; W = I and W = ones closed forms for GEMV.  Parity unpinned: none.
 
 Citations: `P:<n>` = /root/reference/PAPER.md line n; `BJ:` = BASELINE.json north_star /
 configs; `O<n>`/`G<n>` = SURVEY.md section 8(c) definitions / readings.
@@ -30,6 +31,8 @@ from .pool import (PoolGeometry, pool_geometry, PoolTables, pool_tables, shuffle
                    shuffle_into, dump_view, unshuffle, relayout, arena_plan,
                    adjacent_fraction)
 from .permute import (mlp_perm, head_maps, permute_mlp, permute_heads, expand_head_rows)
+from .moe import (stream_expert, stream_expert_mlp, expert_perm, expert_mlp_perm, permute_experts,
+                  topk_experts, moe_f64)
 from .linear import (to_f64, f32_to_bf16_bits, bf16_bits_to_f32, linear_f64, mlp_f64,
                      attention_f64, to_tile128, from_tile128, err_normwise,
                      err_elementwise_floored)

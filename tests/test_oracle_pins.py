@@ -377,3 +377,41 @@ def test_adjacent_fraction_is_about_one_over_n():
     t = O.pool_tables(0x1234, g)
     assert O.adjacent_fraction(np.arange(100)) == 1.0
     assert O.adjacent_fraction(t.T_vmm) < 0.05
+
+
+# ------------------------------------------------------------------ NEXT-4: mixture-of-experts symmetry
+def test_moe_expert_permutation_preserves_the_function():
+    """MoE' = MoE brute-forced in fp64; negative controls: experts moved without the router, neurons moved in gate only."""
+    rng = np.random.default_rng(0)
+    E, H, I, k, key, layer = 6, 8, 12, 2, 0x1234, 3
+    router, x = rng.standard_normal((E, H)), rng.standard_normal((5, H))
+    gate, up, down = rng.standard_normal((E, I, H)), rng.standard_normal((E, I, H)), rng.standard_normal((E, H, I))
+    eps = O.expert_perm(key, layer, E)
+    pis = [O.expert_mlp_perm(key, layer, E, e, I) for e in range(E)]
+    assert sorted(eps.tolist()) == list(range(E)) and any(int(eps[i]) != i for i in range(E))
+    ref = O.moe_f64(x, router, gate, up, down, k)
+    r2, g2, u2, d2 = O.permute_experts(router, gate, up, down, eps, pis)
+    assert np.max(np.abs(O.moe_f64(x, r2, g2, u2, d2, k) - ref)) <= 1e-10 * np.max(np.abs(ref))
+    assert np.max(np.abs(O.moe_f64(x, router, g2, u2, d2, k) - ref)) > 1e-3            # router left behind
+    ident = [np.arange(I) for _ in range(E)]
+    _, g3, _, _ = O.permute_experts(router, gate, up, down, np.arange(E), pis)
+    assert np.max(np.abs(O.moe_f64(x, router, g3, up, down, k) - ref)) > 1e-3          # gate rows moved alone
+    same = O.permute_experts(router, gate, up, down, np.arange(E), ident)             # identity maps: a no-op
+    assert all(np.array_equal(a, b) for a, b in zip(same, (router, gate, up, down)))
+    # every permuted expert is the old one with its OWN neuron permutation (row pin)
+    e_old = int(eps[1])
+    assert np.array_equal(g2[1][0], gate[e_old][int(pis[e_old][0])]) and np.array_equal(r2[1], router[e_old])
+
+
+def test_moe_reduces_to_the_dense_mlp_and_topk_is_a_sort():
+    rng = np.random.default_rng(1)
+    H, I = 8, 12
+    x = rng.standard_normal((3, H))
+    gate, up, down = rng.standard_normal((1, I, H)), rng.standard_normal((1, I, H)), rng.standard_normal((1, H, I))
+    one = O.moe_f64(x, rng.standard_normal((1, H)), gate, up, down, 1)               # E = 1, k = 1: softmax weight is 1
+    assert np.max(np.abs(one - O.mlp_f64(x, gate[0], up[0], down[0]))) <= 1e-12
+    logits = np.array([0.5, 2.0, 2.0, -1.0, 0.5])
+    assert O.topk_experts(logits, 3) == [1, 2, 0]                                     # ties to the smaller index
+    assert O.topk_experts(logits, 5) == list(np.lexsort((np.arange(5), -logits)))
+    # streams of the expert maps do not collide with O3's
+    assert O.stream_expert(3) == (7 << 32) | 3 and O.stream_expert_mlp(2, 8, 5) == (8 << 32) | 21
