@@ -179,6 +179,22 @@ cloak_status cloak_permute_mlp_heads(uint64_t key, const cloak_block_shape* shap
                                      void* d_gate_o, void* d_up_o, void* d_down_o,
                                      void* d_q_o, void* d_k_o, void* d_v_o, void* d_o_o, void* stream);
 
+/* ---- S5 for mixture-of-experts layers (the paper evaluates Qwen3-MoE).
+ * Shapes (row-major, contiguous): router [n_experts, hidden]; gate, up [n_experts, inter, hidden]; down [n_experts, hidden, inter].
+ *   (eps, _)  = keygen(key, (7<<32)|layer, n_experts):  new expert e' is old expert eps[e'];  router'[e',:] = router[eps[e'],:]
+ *   (pi_e, _) = keygen(key, (8<<32)|(layer*n_experts + e), inter) for every OLD expert e, and with e = eps[e']:
+ *               gate'[e'] = gate[e][pi_e,:],  up'[e'] = up[e][pi_e,:],  down'[e'] = down[e][:,pi_e]
+ * The sparse MLP (top-k by router logit, softmax over the selected logits) is unchanged as a function.  Out of place, all
+ * four tensors required.  Asynchronous on `stream` (a few launches per expert: a load-time call). */
+typedef struct {
+    uint32_t hidden, inter, n_experts;
+    cloak_dtype dt;
+    uint32_t layer;
+} cloak_moe_shape;
+cloak_status cloak_permute_experts(uint64_t key, const cloak_moe_shape* shape, const void* d_router, const void* d_gate,
+                                   const void* d_up, const void* d_down, void* d_router_o, void* d_gate_o, void* d_up_o,
+                                   void* d_down_o, void* stream);
+
 /* ---- S5 + S4 in one pass: the fused load path (the layout is decided before
  * any weight lands).  Same permutation as cloak_permute_mlp_heads, but every permuted tensor is written straight into
  * `pool` through its block table at arena byte offset h_offsets[i] (i = gate, up, down, q, k, v, o; a block

@@ -25,7 +25,7 @@ STATUS_NAMES = {0: "CLOAK_OK", -1: "CLOAK_ERR_INVALID", -2: "CLOAK_ERR_ALIGN", -
 SYMBOLS = ["cloak_last_error", "cloak_version", "cloak_launch_count", "cloak_keygen", "cloak_pool_create", "cloak_pool_destroy",
            "cloak_pool_info", "cloak_pool_tables", "cloak_pool_dump", "cloak_pool_map_ms", "cloak_pool_adjacency", "cloak_shuffle",
            "cloak_unshuffle", "cloak_shuffle_many", "cloak_unshuffle_many", "cloak_relayout", "cloak_rekey_inplace", "cloak_shuffle_host", "cloak_unshuffle_host",
-           "cloak_set_copy_engine", "cloak_arena_plan", "cloak_permute_mlp_heads", "cloak_load_mlp_heads", "cloak_to_tile128",
+           "cloak_set_copy_engine", "cloak_arena_plan", "cloak_permute_mlp_heads", "cloak_permute_experts", "cloak_load_mlp_heads", "cloak_to_tile128",
            "cloak_gemv", "cloak_gemv_chain", "cloak_gemm", "cloak_gemm_chain", "cloak_set_gemv_engine", "cloak_gemv_host", "cloak_silu_mul"]
 
 
@@ -38,6 +38,10 @@ class CloakError(RuntimeError):
 class cloak_block_shape(Structure):
     _fields_ = [("hidden", c_uint32), ("inter", c_uint32), ("n_q", c_uint32), ("n_kv", c_uint32),
                 ("head_dim", c_uint32), ("dt", c_int), ("layer", c_uint32)]
+
+
+class cloak_moe_shape(Structure):
+    _fields_ = [("hidden", c_uint32), ("inter", c_uint32), ("n_experts", c_uint32), ("dt", c_int), ("layer", c_uint32)]
 
 
 class cloak_tensor(Structure):
@@ -82,6 +86,7 @@ lib.cloak_set_copy_engine.argtypes = [c_int]
 lib.cloak_set_gemv_engine.argtypes = [c_int]
 lib.cloak_arena_plan.argtypes = [c_uint64, c_uint32, POINTER(c_uint64), c_uint32, POINTER(c_uint64), POINTER(c_uint64)]
 lib.cloak_permute_mlp_heads.argtypes = [c_uint64, POINTER(cloak_block_shape)] + [_P] * 15
+lib.cloak_permute_experts.argtypes = [c_uint64, POINTER(cloak_moe_shape)] + [_P] * 9
 lib.cloak_load_mlp_heads.argtypes = [c_uint64, POINTER(cloak_block_shape), _P] + [_P] * 7 + [POINTER(c_uint64), _P]
 lib.cloak_to_tile128.argtypes = [_P, _P, c_uint32, c_uint32, c_int, _P]
 lib.cloak_gemv.argtypes = [_P, POINTER(cloak_tensor), _P, _P, c_uint32, _P]
@@ -241,6 +246,11 @@ def cloak_permute_mlp_heads(key, shape, gate=None, up=None, down=None, q=None, k
                             stream=None):
     ptrs = [_ptr(t) for t in (gate, up, down, q, k, v, o, gate_o, up_o, down_o, q_o, k_o, v_o, o_o)]
     _check(lib.cloak_permute_mlp_heads(key, byref(shape), *ptrs, _stream(stream)))
+
+
+def cloak_permute_experts(key, shape, router, gate, up, down, router_o, gate_o, up_o, down_o, stream=None):
+    ptrs = [_ptr(t) for t in (router, gate, up, down, router_o, gate_o, up_o, down_o)]
+    _check(lib.cloak_permute_experts(key, byref(shape), *ptrs, _stream(stream)))
 
 
 def cloak_load_mlp_heads(key, shape, pool, offsets, gate=None, up=None, down=None, q=None, k=None, v=None, o=None,

@@ -441,6 +441,52 @@ extern "C" cloak_status cloak_load_mlp_heads(uint64_t key, const cloak_block_sha
     return st;
 }
 
+extern "C" cloak_status cloak_permute_experts(uint64_t key, const cloak_moe_shape* sh, const void* d_router,
+                                              const void* d_gate, const void* d_up, const void* d_down, void* d_router_o,
+                                              void* d_gate_o, void* d_up_o, void* d_down_o, void* stream) {
+    if (!sh) return fail(CLOAK_ERR_INVALID, "permute_experts: shape is NULL");
+    if (sh->dt != CLOAK_F32 && sh->dt != CLOAK_BF16) return fail(CLOAK_ERR_UNSUPPORTED, "permute_experts: unknown dtype");
+    const void* in[4] = {d_router, d_gate, d_up, d_down};
+    void* out[4] = {d_router_o, d_gate_o, d_up_o, d_down_o};
+    for (int i = 0; i < 4; ++i) {
+        if (!in[i] || !out[i] || in[i] == out[i]) return fail(CLOAK_ERR_INVALID, "permute_experts: tensor %d NULL or in place", i);
+        if (((uintptr_t)in[i] | (uintptr_t)out[i]) & 15) return fail(CLOAK_ERR_ALIGN, "permute_experts: tensor %d not 16-byte aligned", i);
+    }
+    const uint32_t e = sh->dt == CLOAK_F32 ? 4 : 2, epv = 16 / e;
+    const uint32_t E = sh->n_experts, H = sh->hidden, I = sh->inter;
+    if (E == 0 || H == 0 || I == 0 || H % epv || I % epv) return fail(CLOAK_ERR_ALIGN, "permute_experts: hidden and inter must be non-zero multiples of %u", epv);
+    if (E > 65536) return fail(CLOAK_ERR_UNSUPPORTED, "permute_experts: more than 65536 experts");
+    cudaStream_t s = (cudaStream_t)stream;
+    int dev = 0;
+    CLOAK_CUDA(cudaGetDevice(&dev));
+    const int sms = sm_count(dev);
+    // eps on the host (to walk the experts) and on the device (to gather the router's rows): the same Philox keygen
+    std::vector<uint32_t> eps;
+    keygen_host(key, (7ull << 32) | sh->layer, E, eps);
+    uint32_t* scratch = nullptr;
+    CLOAK_CUDA(cudaMallocAsync((void**)&scratch, ((size_t)E + I) * 4, s));
+    uint32_t* d_eps = scratch;
+    uint32_t* d_pi = scratch + E;
+    cloak_status st = keygen_device(key, (7ull << 32) | sh->layer, E, d_eps, nullptr, s);
+    const uint64_t hrow = (uint64_t)H * e, emat = (uint64_t)I * H * e;
+    if (st == CLOAK_OK) st = rows(d_router, PlainDst{static_cast<int4*>(d_router_o)}, d_eps, 1, E, hrow, sms, s);
+    for (uint32_t en = 0; en < E && st == CLOAK_OK; ++en) {
+        const uint32_t eo = eps[en];                               // new expert en is old expert eo, with eo's own pi
+        st = keygen_device(key, (8ull << 32) | ((uint64_t)sh->layer * E + eo), I, d_pi, nullptr, s);
+        const char* g = (const char*)d_gate + eo * emat;
+        const char* u = (const char*)d_up + eo * emat;
+        const char* d = (const char*)d_down + eo * emat;
+        if (st == CLOAK_OK) st = rows(g, PlainDst{reinterpret_cast<int4*>((char*)d_gate_o + en * emat)}, d_pi, 1, I, hrow, sms, s);
+        if (st == CLOAK_OK) st = rows(u, PlainDst{reinterpret_cast<int4*>((char*)d_up_o + en * emat)}, d_pi, 1, I, hrow, sms, s);
+        if (st == CLOAK_OK) {
+            PlainDst dd{reinterpret_cast<int4*>((char*)d_down_o + en * emat)};
+            st = e == 4 ? cols<uint32_t>(d, dd, d_pi, 1, H, I, sms, s) : cols<uint16_t>(d, dd, d_pi, 1, H, I, sms, s);
+        }
+    }
+    cudaFreeAsync(scratch, s);
+    return st;
+}
+
 extern "C" cloak_status cloak_to_tile128(const void* d_src, void* d_dst, uint32_t N, uint32_t K, cloak_dtype dt,
                                          void* stream) {
     if (!d_src || !d_dst || d_src == d_dst) return fail(CLOAK_ERR_INVALID, "to_tile128: NULL or aliased pointers");

@@ -669,3 +669,72 @@ def test_error_codes_on_device():
         with pytest.raises(C.CloakError) as ei:
             C.cloak_gemv(p.h, C.cloak_tensor(0, 1 << 20, 256, C.CLOAK_F32, C.CLOAK_ROWMAJOR), x, x, 1)
         assert ei.value.status == C.CLOAK_ERR_INVALID
+
+
+# ------------------------------------------------------------------ NEXT-4: mixture-of-experts layers
+@pytest.mark.parametrize("E,H,I,dtype,layer", [(6, 64, 40, "f32", 0), (8, 256, 1000, "bf16", 3), (32, 2048, 768, "bf16", 47)])
+def test_permute_experts_bit_exact(E, H, I, dtype, layer):
+    """cloak_permute_experts against the oracle: router rows and whole experts by eps, each expert's neurons by its own pi."""
+    key, seed = 0x1234, 9
+    router = gen.synth(seed, 0, (E, H), dtype)
+    gate, up = gen.synth(seed, 1, (E, I, H), dtype), gen.synth(seed, 2, (E, I, H), dtype)
+    down = gen.synth(seed, 3, (E, H, I), dtype)
+    dev = [_dev(a, dtype) for a in (router, gate, up, down)]
+    out = [torch.zeros_like(t) for t in dev]
+    sh = C.cloak_moe_shape(H, I, E, C.CLOAK_F32 if dtype == "f32" else C.CLOAK_BF16, layer)
+    C.cloak_permute_experts(key, sh, *dev, *out)
+    eps = O.expert_perm(key, layer, E)
+    pis = [O.expert_mlp_perm(key, layer, E, e, I) for e in range(E)]
+    ref = O.permute_experts(router, gate, up, down, eps, pis)
+    for o_, r_ in zip(out, ref):
+        got = o_.cpu().numpy() if dtype == "f32" else bits_from_bf16_dev(o_)
+        assert np.array_equal(got, r_)
+
+
+def test_moe_decode_through_the_cloaked_pool_equals_the_unpermuted_moe():
+    """Expert permutation -> block shuffle -> router GEMV + one cloak_gemv_chain over the selected experts (gate | up with
+    the silu*up epilogue | down): equals the oracle's UNpermuted MoE forward (fp64) within the bf16 tolerance."""
+    key, seed, layer, E, H, I, k, block, page = 0x1234, 4, 1, 8, 512, 256, 2, 65536, 2 << 20
+    router = gen.synth(seed, 0, (E, H), "bf16", kind=gen.KIND_NORMAL)       # O(1) logits so that the top-k is well separated
+    gate, up, down = gen.synth(seed, 1, (E, I, H), "bf16"), gen.synth(seed, 2, (E, I, H), "bf16"), gen.synth(seed, 3, (E, H, I), "bf16")
+    dev = [bf16_dev_from_bits(a) for a in (router, gate, up, down)]
+    prm = [torch.zeros_like(t) for t in dev]
+    C.cloak_permute_experts(key, C.cloak_moe_shape(H, I, E, C.CLOAK_BF16, layer), *dev, *prm)
+    eps = O.expert_perm(key, layer, E)
+    new_of_old = {int(eps[en]): en for en in range(E)}
+    # arena: padded router (16 rows at least for the GEMV), then gate_e, up_e, down_e of every (new) expert
+    rpad = torch.zeros(16, H, dtype=torch.bfloat16, device="cuda")
+    rpad[:E] = prm[0]
+    sizes = [16 * H * 2] + [I * H * 2] * (3 * E)
+    offs, total = C.cloak_arena_plan(key, sizes, block)
+    with Pool(total, block, page, key) as p:
+        C.cloak_shuffle(p.h, rpad, offs[0], rpad.numel() * 2)
+        T = {}
+        for en in range(E):
+            for j, (nm, t, n, kk) in enumerate((("gate", prm[1], I, H), ("up", prm[2], I, H), ("down", prm[3], H, I))):
+                o = offs[1 + 3 * en + j]
+                C.cloak_shuffle(p.h, t[en], o, I * H * 2)
+                T[nm, en] = C.cloak_tensor(o, n, kk, C.CLOAK_BF16, C.CLOAK_ROWMAJOR)
+        for tok in range(3):
+            x = gen.synth(seed + 100, tok, (1, H), "bf16", kind=gen.KIND_NORMAL)
+            dx = bf16_dev_from_bits(x)
+            logits_d = torch.zeros(1, 16, dtype=torch.bfloat16, device="cuda")
+            C.cloak_gemv(p.h, C.cloak_tensor(offs[0], 16, H, C.CLOAK_BF16, C.CLOAK_ROWMAJOR), dx, logits_d, 1)
+            ref_logits = O.linear_f64(x, router)[0]
+            got_logits = logits_d.float().cpu().numpy()[0, :E]
+            assert O.err_normwise(got_logits, ref_logits[eps.astype(np.int64)]) <= TOL["bf16"]      # logits move with the experts
+            sel_old = O.topk_experts(ref_logits, k)                         # routing decided in fp64, then relabelled
+            z = ref_logits[sel_old]
+            w = np.exp(z - z.max())
+            w /= w.sum()
+            ys, ops = [], []
+            for e_old in sel_old:
+                en = new_of_old[e_old]
+                yg, yu, act = (torch.zeros(1, I, dtype=torch.bfloat16, device="cuda") for _ in range(3))
+                yd = torch.zeros(1, H, dtype=torch.bfloat16, device="cuda")
+                ops += [(T["gate", en], dx, yg, 0), (T["up", en], dx, yu, 0, yg, act), (T["down", en], act, yd, 1)]
+                ys.append(yd)
+            C.cloak_gemv_chain(p.h, ops, 1)
+            torch.cuda.synchronize()
+            got = sum(wi * y.double().cpu().numpy() for wi, y in zip(w, ys))
+            assert O.err_normwise(got, O.moe_f64(x, router, gate, up, down, k)) <= TOL["bf16"], tok
