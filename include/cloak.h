@@ -242,8 +242,12 @@ cloak_status cloak_gemm(const cloak_pool* pool, const cloak_tensor* w, const voi
  *     fp32 arithmetic on the bf16 values, rounded to bf16 exactly as cloak_silu_mul does; O9: the gated MLP's
  *     activation, fused into the up projection's epilogue).  d_gate must be the d_y of an earlier op of this
  *     chain with the same N and K (the usual gate projection), or a buffer complete before the call;
- *   - after != 0 says that X_i is written by an earlier op of this chain: the op then starts only when ALL
- *     earlier ops have completed.  Ops with after == 0 must not read what earlier ops of the chain write.
+ *   - after != 0 says that X_i is written by an earlier op of this chain.  after == 1: the op starts only when ALL
+ *     earlier ops have completed (one grid-wide arrival).  after == 2: it has the same dependency as the nearest
+ *     earlier op with after != 0 and shares that arrival -- e.g. the down projections of several experts, all of which
+ *     follow all the up projections: the first says 1, the others 2.  (In a split chain -- more than 48 ops, or mixed
+ *     chunk sizes -- after == 2 on the first op of a launch needs nothing: the launch boundary orders it.)
+ *     Ops with after == 0 must not read what earlier ops of the chain write.
  * The weight stream of op i+1 is already being fetched while op i finishes, dependent or not.
  * All ops: CLOAK_BF16, CLOAK_ROWMAJOR, K % 256 == 0, N % 16 == 0, pool block_bytes >= 512, batch 1..16, outputs
  * distinct.  h_ops is a HOST array (copied into the launch parameters; not referenced after the call returns).

@@ -26,7 +26,7 @@
 //   * a launch executes a CHAIN of ops (cloak_gemv_chain; cloak_gemv is a chain of one).  The producer warp
 //     runs straight through the chain -- weights do not depend on activations -- so HBM stays busy across op
 //     boundaries; only the consumers of an op marked `after` wait, on a grid-wide arrival counter, for all CTAs
-//     to have finished the earlier ops (its X is their Y).  An op may also emit silu(G) * Y next to Y in its
+//     to have finished the earlier ops (its X is their Y); several ops can share one such arrival.  An op may also emit silu(G) * Y next to Y in its
 //     epilogue (the gated MLP's activation, O9), where G is the output of an earlier op of the same shape -- the
 //     same CTA wrote those very elements, so no wait is needed -- and gate/up -> down costs no separate pass.
 //   * programmatic dependent launch: the grid may start while its stream predecessor drains; the producer
@@ -37,7 +37,7 @@
 
 namespace cloak {
 
-struct ChainOp {             // 72 bytes of kernel parameter space per op
+struct ChainOp {             // 80 bytes of kernel parameter space per op
     uint64_t w_offset;
     const uint16_t* x;       // [batch, K]
     __nv_bfloat16* y;        // [batch, N]
@@ -49,23 +49,25 @@ struct ChainOp {             // 72 bytes of kernel parameter space per op
     uint32_t per;            // units per CTA
     uint32_t ctas;           // CTAs that own units of this op (indices 0 .. ctas-1)
     uint32_t tile_base;      // index of this op's first row-tile counter
-    uint32_t flags;          // OP_AFTER | OP_SIGNAL
+    uint32_t flags;          // OP_SIGNAL
+    uint32_t wait_op;        // NO_WAIT, or the index of the op whose completion by ALL CTAs this op's consumers wait for
 };
-enum { OP_AFTER = 1,         // consumers wait until every CTA has finished all earlier ops of the chain
-       OP_SIGNAL = 2 };      // the next op is OP_AFTER: every CTA reports here when it is done with this op
-constexpr int GS_MAX_OPS = 48;              // 48 x 72 B + header < 4 KiB of kernel parameters
+enum { OP_SIGNAL = 2 };      // some later op waits for this one: every CTA reports here when it is done with it (and all before)
+constexpr uint32_t NO_WAIT = 0xffffffffu;
+constexpr int GS_MAX_OPS = 48;              // 48 x 80 B + header < 4 KiB of kernel parameters
 
 struct ChainArgs {
     const char* pool;
     const uint32_t* T;
     float* part;             // [op][cta][batch * 8]: partial of the cut row tile a CTA meets first in that op
     uint32_t* counters;      // [tile_base + tile]: arrivals of the non-owning contributors; owner resets to 0
-    uint32_t* opsync;        // [op][2]: arrivals / departures of the grid-wide wait; last departure resets both
+    uint32_t* opsync;        // [GS_MAX_OPS] arrivals per signalling op, [GS_MAX_OPS] CTAs done with the launch: the last resets all
     uint32_t log2b;
     uint32_t batch;
     uint32_t nops;
     uint32_t early;          // 1: W is unchanged since before the preceding kernel, so the producer may stream it
                              //    ahead of griddepcontrol.wait (programmatic dependent launch)
+    uint32_t any_signal;     // some op of this launch signals
     ChainOp ops[GS_MAX_OPS];
 };
 
@@ -227,16 +229,10 @@ __global__ void __launch_bounds__(gs_threads(NT), 1) gemv_chain_kernel(const __g
         const uint32_t ubeg = blockIdx.x * per, uend = min(ubeg + per, op.units);
         const bool have = ubeg < uend;
 
-        if (have && (op.flags & OP_AFTER) && j > 0) {
-            // grid-wide wait: every CTA has reported at op j-1, i.e. has finished all ops before this one
-            uint32_t* sync = a.opsync + 2 * (j - 1);
-            if (ctid == 0) {
-                while (ld_acquire(sync) != gridDim.x) __nanosleep(32);
-                if (atomicAdd(sync + 1, 1u) == op.ctas - 1) {      // last waiter to leave: reset for the next launch
-                    sync[0] = 0;
-                    sync[1] = 0;
-                }
-            }
+        if (have && op.wait_op != NO_WAIT) {
+            // grid-wide wait: every CTA has reported at op wait_op, i.e. has finished that op and all ops before it
+            if (ctid == 0)
+                while (ld_acquire(a.opsync + op.wait_op) != gridDim.x) __nanosleep(32);
             consumer_bar();
         }
 
@@ -382,8 +378,15 @@ __global__ void __launch_bounds__(gs_threads(NT), 1) gemv_chain_kernel(const __g
             consumer_bar();
             if (ctid == 0) {
                 __threadfence();
-                red_release_add(a.opsync + 2 * j, 1u);
+                red_release_add(a.opsync + j, 1u);
             }
+        }
+    }
+    // the arrival counters are reset for the next launch by the last CTA to get here (nobody reads them any more)
+    if (a.any_signal && ctid == 0) {
+        if (atomicAdd(a.opsync + GS_MAX_OPS, 1u) == gridDim.x - 1) {
+            for (uint32_t j = 0; j < a.nops; ++j) a.opsync[j] = 0;
+            a.opsync[GS_MAX_OPS] = 0;
         }
     }
 }
@@ -438,6 +441,8 @@ cloak_status gemv_stream_launch(const cloak_pool* pool, const cloak_gemv_op* ops
     a.nops = n;
     const int sms = sm_count(pool->device);
     uint64_t max_units = 0, tile_base = 0;
+    uint32_t last_wait = NO_WAIT;
+    a.any_signal = 0;
     for (uint32_t j = 0; j < n; ++j) {
         const cloak_tensor& w = ops[j].w;
         ChainOp& o = a.ops[j];
@@ -454,8 +459,17 @@ cloak_status gemv_stream_launch(const cloak_pool* pool, const cloak_gemv_op* ops
         o.units = (uint32_t)units64;
         o.tile_base = (uint32_t)tile_base;
         tile_base += w.N / GS_ROWS;
-        o.flags = (j > 0 && ops[j].after) ? OP_AFTER : 0;
-        if (j > 0 && ops[j].after) a.ops[j - 1].flags |= OP_SIGNAL;
+        // after = 1: wait for every earlier op of the chain (i.e. for op j-1 to be reported by all CTAs);
+        // after = 2: the same dependency as the nearest earlier waiting op (no new grid-wide arrival needed)
+        o.flags = 0;
+        o.wait_op = NO_WAIT;
+        if (j > 0 && ops[j].after == 1) o.wait_op = j - 1;
+        else if (j > 0 && ops[j].after >= 2) o.wait_op = last_wait;
+        if (o.wait_op != NO_WAIT) {
+            a.ops[o.wait_op].flags |= OP_SIGNAL;
+            a.any_signal = 1;
+            last_wait = o.wait_op;
+        }
         if (units64 > max_units) max_units = units64;
     }
     if (tile_base > GS_TILE_COUNTERS) return fail(CLOAK_ERR_UNSUPPORTED, "gemv: too many output rows for the row-tile counters");

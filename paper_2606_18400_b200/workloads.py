@@ -1,6 +1,6 @@
 """Measurement drivers for BASELINE.json configs[2..4]; configs[1] is bench.py's own step.
 
-    python -m paper_2606_18400_b200.workloads cfg2|cfg3|cfg4 [--reps R] [--out file.json]
+    python -m paper_2606_18400_b200.workloads cfg2|cfg3|cfg4|moe [--reps R] [--out file.json]
     python bench.py --workload cfg2|cfg3|cfg4            (same thing)
 
 Each prints ONE JSON line.  Everything on the timed path is a C-ABI call of libcloak.so (through the ctypes
@@ -421,7 +421,113 @@ def run_cfg3(args):
             "gemm": out, "launches_per_sweep": 7 * layers, "gpu_launches": C.cloak_launch_count() - launches0}
 
 
-RUNNERS = {"cfg2": run_cfg2, "cfg3": run_cfg3, "cfg4": run_cfg4}
+# ------------------------------------------------------------------------------------------ MoE (NEXT-4)
+def run_moe(args):
+    """Qwen3-30B-A3B-shaped sparse layers (hidden 2048, 128 experts of 768, top-8; attention 32 q / 4 kv heads): expert
+    permutation + shuffle at load, then the batch-1 decode chain of every layer -- q, k, v, o, router, and gate | up | down
+    of 8 (seeded) selected experts -- as one cloak_gemv_chain, cloaked vs identity table.  --layers picks the depth
+    (default 12 of the model's 48: 15 GB per pool)."""
+    torch, C, synth_cuda, gen = _imports()
+    c = gen.CONFIGS[5]
+    L = int(args.layers or 12)
+    H, I, E, K = c["hidden"], c["inter"], c["n_experts"], c["top_k"]
+    Q, KV = c["n_q"] * c["head_dim"], c["n_kv"] * c["head_dim"]
+    peak, peak_kind = hbm_peak()
+    names, sizes = [], []
+    for l in range(L):
+        for nm, n, k in (("q", Q, H), ("k", KV, H), ("v", KV, H), ("o", H, Q), ("router", E, H)):
+            names.append((l, nm, n, k))
+        for e in range(E):
+            names += [(l, f"gate{e}", I, H), (l, f"up{e}", I, H), (l, f"down{e}", H, I)]
+    sizes = [2 * n * k for _, _, n, k in names]
+    offs, total = C.cloak_arena_plan(c["key"], sizes, c["block"])
+    off = {(l, nm): o for (l, nm, _, _), o in zip(names, offs)}
+    T = {(l, nm): C.cloak_tensor(o, n, k, C.CLOAK_BF16, C.CLOAK_ROWMAJOR) for (l, nm, n, k), o in zip(names, offs)}
+    pc = C.cloak_pool_create(0, total, c["block"], c["page"], c["key"])
+    pn = C.cloak_pool_create(0, total, c["block"], c["page"], c["key"], C.CLOAK_POOL_IDENTITY)
+    launches0 = C.cloak_launch_count()
+    try:
+        # ---- load: generator -> S5 (heads; experts) -> shuffle_many, layer by layer
+        t0 = time.perf_counter()
+        att = {nm: torch.empty(n, k, dtype=torch.bfloat16, device="cuda") for nm, n, k in (("q", Q, H), ("k", KV, H), ("v", KV, H), ("o", H, Q))}
+        att_p = {nm: torch.empty_like(t) for nm, t in att.items()}
+        raw = [torch.empty(s_, dtype=torch.bfloat16, device="cuda") for s_ in ((E, H), (E, I, H), (E, I, H), (E, H, I))]
+        prm = [torch.empty_like(t) for t in raw]
+        perm_ms = 0.0
+        for l in range(L):
+            for i, nm in enumerate(att):
+                synth_cuda.fill(att[nm], c["seed"], l * 8 + i)
+            for i, t in enumerate(raw):
+                synth_cuda.fill(t, c["seed"], l * 8 + 4 + i, kind=gen.KIND_NORMAL if i == 0 else gen.KIND_WEIGHT)
+            sh = C.cloak_block_shape(H, I, c["n_q"], c["n_kv"], c["head_dim"], C.CLOAK_BF16, l)
+            C.cloak_permute_mlp_heads(c["key"], sh, **att, **{k + "_o": v for k, v in att_p.items()})
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record()
+            C.cloak_permute_experts(c["key"], C.cloak_moe_shape(H, I, E, C.CLOAK_BF16, l), *raw, *prm)
+            e1.record()
+            ts = [att_p[nm] for nm in att] + [prm[0]]
+            os_ = [off[l, nm] for nm in att] + [off[l, "router"]]
+            for e in range(E):
+                ts += [prm[1][e], prm[2][e], prm[3][e]]
+                os_ += [off[l, f"gate{e}"], off[l, f"up{e}"], off[l, f"down{e}"]]
+            for p in (pc, pn):
+                C.cloak_shuffle_many(p, ts, os_, [t.numel() * 2 for t in ts])
+            torch.cuda.synchronize()
+            perm_ms += e0.elapsed_time(e1)
+        load_s = time.perf_counter() - t0
+
+        # ---- decode chain: fixed synthetic inputs, 8 seeded experts per layer
+        xh = synth_cuda.fill(torch.empty(1, H, dtype=torch.bfloat16, device="cuda"), c["seed"] + 100, 0, kind=gen.KIND_NORMAL)
+        xa = synth_cuda.fill(torch.empty(1, Q, dtype=torch.bfloat16, device="cuda"), c["seed"] + 100, 1, kind=gen.KIND_NORMAL)
+        rng = np.random.default_rng(c["seed"])
+        sel = [sorted(int(e) for e in rng.choice(E, K, replace=False)) for _ in range(L)]
+        read_bytes = 0
+
+        def build(tag):
+            nonlocal read_bytes
+            ops, outs, rb = [], [], 0
+            z = lambda n: torch.zeros(1, n, dtype=torch.bfloat16, device="cuda")       # noqa: E731
+            for l in range(L):
+                y = {nm: z(n) for nm, n in (("q", Q), ("k", KV), ("v", KV), ("o", H), ("router", E))}
+                ops += [(T[l, nm], xa if nm == "o" else xh, y[nm], 0) for nm in y]
+                rb += 2 * (2 * Q * H + 2 * KV * H + E * H)
+                downs = []
+                for i, e in enumerate(sel[l]):
+                    yg, yu, act, yd = z(I), z(I), z(I), z(H)
+                    ops += [(T[l, f"gate{e}"], xh, yg, 0), (T[l, f"up{e}"], xh, yu, 0, yg, act)]
+                    downs.append((T[l, f"down{e}"], act, yd, 1 if i == 0 else 2))
+                    outs += [yg, yu, act, yd]
+                    rb += 2 * 3 * I * H
+                ops += downs
+                outs += list(y.values())
+            read_bytes = rb
+            return C.cloak_gemv_ops(ops), outs
+
+        res, outs = {}, {}
+        for pool_name, pool in (("cloaked", pc), ("native", pn)):
+            ops, outs[pool_name] = build(pool_name)
+            fn = lambda: C.cloak_gemv_chain(pool, ops, 1)        # noqa: E731
+            med, mn = time_gpu(torch, fn, args.reps)
+            gmed, gmn = time_gpu(torch, graphed(torch, fn), args.reps)
+            res[pool_name] = {"stream": dict(rate(read_bytes, med, peak), ms_min=mn), "graph": dict(rate(read_bytes, gmed, peak), ms_min=gmn),
+                              "ops": len(ops)}
+        identical = all(torch.equal(a_, b_) for a_, b_ in zip(outs["cloaked"], outs["native"]))
+        ov = {k: (res["cloaked"][k]["ms"] - res["native"][k]["ms"]) / res["native"][k]["ms"] * 100 for k in ("stream", "graph")}
+    finally:
+        torch.cuda.synchronize()
+        C.cloak_pool_destroy(pc)
+        C.cloak_pool_destroy(pn)
+    return {"workload": "moe: Qwen3-30B-A3B-shaped sparse layers, %d of 48 layers, 128 experts, top-8, bf16, 64 KiB blocks" % L,
+            "arena_bytes": total, "layers": L, "reps": args.reps, "hbm_peak_gbs": peak, "hbm_peak_kind": peak_kind,
+            "load_s": load_s, "permute_experts_ms_per_layer": perm_ms / L,
+            "permute_experts_gbs": 2 * 2 * (E * H + 3 * E * I * H) / (perm_ms / L) / 1e6,
+            "decode_chain": res, "decode_read_bytes": read_bytes, "decode_read_bytes_full_model": read_bytes // L * 48,
+            "tokens_per_s_extrapolated_48_layers": 1e3 / (res["cloaked"]["graph"]["ms"] / L * 48),
+            "cloaked_vs_native_overhead_pct": ov, "cloaked_identical_to_native": bool(identical),
+            "gpu_launches": C.cloak_launch_count() - launches0}
+
+
+RUNNERS = {"cfg2": run_cfg2, "cfg3": run_cfg3, "cfg4": run_cfg4, "moe": run_moe}
 
 
 def main(argv=None):
@@ -429,7 +535,7 @@ def main(argv=None):
     ap.add_argument("workload", choices=sorted(RUNNERS))
     ap.add_argument("--reps", type=int, default=10)
     ap.add_argument("--bytes", type=int, default=0, help="cfg4: buffer bytes (default 4 GiB)")
-    ap.add_argument("--layers", type=int, default=0, help="cfg3: number of layers (default 64)")
+    ap.add_argument("--layers", type=int, default=0, help="cfg3: number of layers (default 64); moe: default 12 of 48")
     ap.add_argument("--out", default="")
     args = ap.parse_args(argv)
     line = json.dumps(RUNNERS[args.workload](args))

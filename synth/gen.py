@@ -107,6 +107,9 @@ CONFIGS = {
     # cfg4: 4 GiB granularity sweep (BJ:configs[4]); key B = 0x5678 (G11)
     4: dict(seed=4, key=0x1234, key_b=0x5678, dtype="bf16", bytes=4 << 30, page=2 << 20,
             blocks=[4 << 10, 16 << 10, 64 << 10, 256 << 10, 2 << 20]),
+    # cfg5 (NEXT-4, not in BASELINE.json): Qwen3-30B-A3B-shaped sparse layers (the paper's MoE model)
+    5: dict(seed=5, key=0x1234, dtype="bf16", hidden=2048, inter=768, n_experts=128, top_k=8, n_q=32, n_kv=4, head_dim=128,
+            block=65536, page=2 << 20, layers=48),
 }
 
 
