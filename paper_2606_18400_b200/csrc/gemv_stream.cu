@@ -37,7 +37,7 @@
 
 namespace cloak {
 
-struct ChainOp {             // 80 bytes of kernel parameter space per op
+struct ChainOp {             // 80 bytes of kernel parameter space per op (10 x 8)
     uint64_t w_offset;
     const uint16_t* x;       // [batch, K]
     __nv_bfloat16* y;        // [batch, N]
@@ -51,6 +51,9 @@ struct ChainOp {             // 80 bytes of kernel parameter space per op
     uint32_t tile_base;      // index of this op's first row-tile counter
     uint32_t flags;          // OP_SIGNAL
     uint32_t wait_op;        // NO_WAIT, or the index of the op whose completion by ALL CTAs this op's consumers wait for
+    uint32_t rot;            // range r of this op belongs to CTA (r + rot) % grid: an op with fewer ranges than CTAs starts
+                             // where the previous one stopped, so the idle CTAs are different ones each time (an op with a
+                             // gate epilogue keeps the rotation of the op that produced the gate: same rows, same CTA)
 };
 enum { OP_SIGNAL = 2 };      // some later op waits for this one: every CTA reports here when it is done with it (and all before)
 constexpr uint32_t NO_WAIT = 0xffffffffu;
@@ -180,7 +183,8 @@ __global__ void __launch_bounds__(gs_threads(NT), 1) gemv_chain_kernel(const __g
         for (uint32_t j = 0; j < a.nops; ++j) {
             const ChainOp& op = a.ops[j];
             const uint32_t kch = op.kch;
-            const uint32_t ubeg = blockIdx.x * op.per, uend = min(ubeg + op.per, op.units);
+            const uint32_t vr = (blockIdx.x + gridDim.x - op.rot) % gridDim.x;   // this CTA's range of the op
+            const uint32_t ubeg = vr * op.per, uend = min(ubeg + op.per, op.units);
             if (ubeg >= uend) continue;
             const uint32_t tile_lo = ubeg / kch, tile_hi = (uend - 1) / kch;
             const uint64_t row_bytes = (uint64_t)op.K * 2;
@@ -226,7 +230,8 @@ __global__ void __launch_bounds__(gs_threads(NT), 1) gemv_chain_kernel(const __g
     for (uint32_t j = 0; j < a.nops; ++j) {
         const ChainOp& op = a.ops[j];
         const uint32_t kch = op.kch, per = op.per;
-        const uint32_t ubeg = blockIdx.x * per, uend = min(ubeg + per, op.units);
+        const uint32_t vr = (blockIdx.x + gridDim.x - op.rot) % gridDim.x;       // this CTA's range of the op
+        const uint32_t ubeg = vr * per, uend = min(ubeg + per, op.units);
         const bool have = ubeg < uend;
 
         if (have && op.wait_op != NO_WAIT) {
@@ -244,7 +249,7 @@ __global__ void __launch_bounds__(gs_threads(NT), 1) gemv_chain_kernel(const __g
             const bool cut_tail = uend < (tile_hi + 1) * kch && !(tile_hi == tile_lo && cut_head);
             const uint16_t* x0 = op.x + (size_t)g * op.K + lane_off / 2;
             const uint16_t* x1 = op.x + (size_t)(g + 8) * op.K + lane_off / 2;
-            float* mypart = a.part + ((size_t)j * gridDim.x + blockIdx.x) * nout;
+            float* mypart = a.part + ((size_t)j * gridDim.x + vr) * nout;
             // Every Y element is stored exactly once, by the CTA that owns its row tile.  The gate op had the same
             // (N, K), hence the same split: gate[idx] was stored by this CTA, before consumer barriers passed since.
             auto store_y = [&](size_t idx, float sum) {
@@ -357,7 +362,7 @@ __global__ void __launch_bounds__(gs_threads(NT), 1) gemv_chain_kernel(const __g
 
             if (cut_tail) {
                 // owner of the tail tile: wait for the other contributors (CTAs after this one), add in CTA order
-                const uint32_t nc = (tile_hi * kch + kch - 1) / per - blockIdx.x;
+                const uint32_t nc = (tile_hi * kch + kch - 1) / per - vr;
                 uint32_t* cnt = a.counters + op.tile_base + tile_hi;
                 if (ctid == 0) {
                     while (ld_acquire(cnt) != nc) __nanosleep(32);
@@ -474,10 +479,26 @@ cloak_status gemv_stream_launch(const cloak_pool* pool, const cloak_gemv_op* ops
     }
     if (tile_base > GS_TILE_COUNTERS) return fail(CLOAK_ERR_UNSUPPORTED, "gemv: too many output rows for the row-tile counters");
     const int ctas = max_units < (uint64_t)sms ? (int)max_units : sms;
+    // Rotation of the ranges over the CTAs.  Measured: it pays when most of a launch is small ops that leave CTAs idle
+    // (MoE experts: 96 units for 148 CTAs; 12 Qwen3-MoE-shaped layers 0.735 -> 0.618 ms) and costs 2 % on dense layers whose
+    // ops fill the grid anyway (cfg2 2.54 -> 2.61 ms), so: all ops rotate if ops that leave at least an eighth of the CTAs idle
+    // hold most of the launch's units, else only the ops that leave a quarter idle do.
+    uint64_t small_units = 0, all_units = 0;
     for (uint32_t j = 0; j < n; ++j) {
         ChainOp& o = a.ops[j];
         o.per = (o.units + ctas - 1) / ctas;
         o.ctas = (o.units + o.per - 1) / o.per;
+        all_units += o.units;
+        if (o.ctas * 8 <= (uint32_t)ctas * 7) small_units += o.units;
+    }
+    const bool rotate_all = 2 * small_units > all_units;
+    uint32_t ranges_so_far = 0;
+    for (uint32_t j = 0; j < n; ++j) {
+        ChainOp& o = a.ops[j];
+        o.rot = (rotate_all || o.ctas * 4 <= (uint32_t)ctas * 3) ? ranges_so_far % ctas : 0;
+        for (uint32_t k = 0; k < j; ++k)
+            if (o.gate && (const void*)a.ops[k].y == (const void*)o.gate) o.rot = a.ops[k].rot;     // same rows, same CTA
+        ranges_so_far += o.ctas;
     }
     const size_t need = WS_COUNTER_BYTES + (size_t)n * ctas * batch * GS_ROWS * 4;
     cloak_status st = pool_workspace(pool, need);
