@@ -264,7 +264,7 @@ typedef struct {
 cloak_status cloak_gemv_chain(const cloak_pool* pool, const cloak_gemv_op* h_ops, uint32_t n_ops, uint32_t batch,
                               void* stream);
 /* A list of INDEPENDENT GEMMs over one pool in one persistent launch (per 16 ops): Y_i = X_i W_i^T as cloak_gemm computes
- * it, bit for bit; no op may read what another op of the list writes.  The weight stream runs on across op boundaries
+ * it, bit for bit; every op has its own output and no op may read what another op of the list writes.  The weight stream runs on across op boundaries
  * (BASELINE.json configs[3]: "cloaked decode GEMM" of every projection of the model).  h_ops is a HOST array, not
  * referenced after the call returns.  Asynchronous on `stream`. */
 typedef struct {

@@ -90,6 +90,17 @@ __global__ void __launch_bounds__(RK_WARPS * 32) rekey_moves_kernel(RekeyArgs a)
 
 using namespace cloak;
 
+namespace {
+// stream-ordered allocation that is released on every exit path
+struct AsyncBuf {
+    void* p = nullptr;
+    cudaStream_t s;
+    explicit AsyncBuf(cudaStream_t st) : s(st) {}
+    ~AsyncBuf() { if (p) cudaFreeAsync(p, s); }
+    cudaError_t alloc(size_t bytes) { return cudaMallocAsync(&p, bytes, s); }
+};
+}  // namespace
+
 extern "C" cloak_status cloak_rekey_inplace(cloak_pool* pool, uint64_t new_key, uint64_t spare_bytes, void* stream) {
     if (!pool) return fail(CLOAK_ERR_INVALID, "rekey_inplace: NULL pool");
     if (pool->flags & CLOAK_POOL_IDENTITY) return fail(CLOAK_ERR_INVALID, "rekey_inplace: an identity pool has no key");
@@ -99,10 +110,11 @@ extern "C" cloak_status cloak_rekey_inplace(cloak_pool* pool, uint64_t new_key, 
     const uint32_t n = pool->nslots, b = pool->block, bpp = pool->bpp;
 
     // ---- new block tables on the device, both block tables on the host
-    uint32_t* d_new = nullptr;                                  // blockperm_B | blockinv_B
-    CLOAK_CUDA(cudaMallocAsync((void**)&d_new, (size_t)2 * n * 4, s));
+    AsyncBuf new_tables(s), work(s);
+    CLOAK_CUDA(new_tables.alloc((size_t)2 * n * 4));
+    uint32_t* d_new = static_cast<uint32_t*>(new_tables.p);    // blockperm_B | blockinv_B
     cloak_status st = keygen_device(new_key, 1ull << 32, n, d_new, d_new + n, s);
-    if (st != CLOAK_OK) { cudaFreeAsync(d_new, s); return st; }
+    if (st != CLOAK_OK) return st;
     std::vector<uint32_t> inv_a(n), inv_b(n), pageinv(pool->npages);
     CLOAK_CUDA(cudaMemcpyAsync(inv_a.data(), pool->d_blockinv, (size_t)n * 4, cudaMemcpyDeviceToHost, s));
     CLOAK_CUDA(cudaMemcpyAsync(inv_b.data(), d_new + n, (size_t)n * 4, cudaMemcpyDeviceToHost, s));
@@ -141,10 +153,7 @@ extern "C" cloak_status cloak_rekey_inplace(cloak_pool* pool, uint64_t new_key, 
             run[p].push_back(make_uint2(RK_SPARE | nseg, cyc[(a0 + 1) % L]));        // saved block -> s_{a0+1}
         }
     }
-    if (nseg == 0) {                                            // sigma is the identity (same key): tables only
-        cudaFreeAsync(d_new, s);
-        return CLOAK_OK;
-    }
+    if (nseg == 0) return CLOAK_OK;                             // sigma is the identity (same key): nothing moves
 
     // ---- upload, run the two passes, swap the tables in stream order
     std::vector<uint2> moves;
@@ -157,10 +166,10 @@ extern "C" cloak_status cloak_rekey_inplace(cloak_pool* pool, uint64_t new_key, 
         }
         start[pass * (npipes + 1) + npipes] = (uint32_t)moves.size();
     }
-    char* d_buf = nullptr;
     const size_t mv_b = moves.size() * sizeof(uint2), st_b = start.size() * 4, sp_b = (size_t)nseg * b;
     const size_t mv_pad = (mv_b + 255) & ~(size_t)255, st_pad = (st_b + 255) & ~(size_t)255;
-    CLOAK_CUDA(cudaMallocAsync((void**)&d_buf, mv_pad + st_pad + sp_b, s));
+    CLOAK_CUDA(work.alloc(mv_pad + st_pad + sp_b));
+    char* d_buf = static_cast<char*>(work.p);
     CLOAK_CUDA(cudaMemcpyAsync(d_buf, moves.data(), mv_b, cudaMemcpyHostToDevice, s));
     CLOAK_CUDA(cudaMemcpyAsync(d_buf + mv_pad, start.data(), st_b, cudaMemcpyHostToDevice, s));
     RekeyArgs a;
@@ -190,7 +199,5 @@ extern "C" cloak_status cloak_rekey_inplace(cloak_pool* pool, uint64_t new_key, 
     pool->key = new_key;
     // the host lists were copied from pageable memory: the copies above have consumed them when the calls returned
     CLOAK_CUDA(cudaStreamSynchronize(s));
-    cudaFreeAsync(d_buf, s);
-    cudaFreeAsync(d_new, s);
     return CLOAK_OK;
 }
