@@ -324,6 +324,28 @@ static cloak_status check_shape(const cloak_block_shape* sh, bool mlp, bool head
     return CLOAK_OK;
 }
 
+// A second stream for the head path.  The MLP path (keygen over `inter`, three large gathers) and the head path (head maps,
+// four small launch-bound gathers) are independent: forked from the caller's stream and joined back into it with events --
+// which stream capture records as graph dependencies -- the small kernels run in the shadow of the large ones.
+struct ForkJoin {
+    cudaStream_t aux = nullptr;
+    cudaEvent_t fork = nullptr, join = nullptr, mid = nullptr;
+    bool ok = false;
+    bool init() {
+        if (ok) return true;
+        ok = cudaStreamCreateWithFlags(&aux, cudaStreamNonBlocking) == cudaSuccess &&
+             cudaEventCreateWithFlags(&fork, cudaEventDisableTiming) == cudaSuccess &&
+             cudaEventCreateWithFlags(&join, cudaEventDisableTiming) == cudaSuccess &&
+             cudaEventCreateWithFlags(&mid, cudaEventDisableTiming) == cudaSuccess;
+        if (!ok) cudaGetLastError();
+        return ok;
+    }
+};
+static ForkJoin& fork_join(int dev) {
+    static thread_local ForkJoin fj[16];
+    return fj[dev & 15];
+}
+
 // The permutation proper.  in[i] (gate, up, down, q, k, v, o) may be NULL to skip a tensor; mk(i) says where tensor i goes.
 template <typename MakeDst>
 static cloak_status permute_impl(uint64_t key, const cloak_block_shape* sh, const void* const in[7], MakeDst mk, int dev,
@@ -339,26 +361,39 @@ static cloak_status permute_impl(uint64_t key, const cloak_block_shape* sh, cons
     uint32_t* eta = kappa + sh->n_kv;
     cloak_status st = CLOAK_OK;
     const uint64_t hrow = (uint64_t)sh->hidden * e;
-    if (mlp) {
-        st = keygen_device(key, (4ull << 32) | sh->layer, sh->inter, pi, nullptr, s);
-        if (st == CLOAK_OK && in[0]) st = rows(in[0], mk(0), pi, 1, sh->inter, hrow, sms, s);
-        if (st == CLOAK_OK && in[1]) st = rows(in[1], mk(1), pi, 1, sh->inter, hrow, sms, s);
-        if (st == CLOAK_OK && in[2])
-            st = e == 4 ? cols<uint32_t>(in[2], mk(2), pi, 1, sh->hidden, sh->inter, sms, s)
-                        : cols<uint16_t>(in[2], mk(2), pi, 1, sh->hidden, sh->inter, sms, s);
-    }
-    if (st == CLOAK_OK && heads) {
-        head_maps_kernel<<<1, 1024, 0, s>>>((uint32_t)key, (uint32_t)(key >> 32), sh->layer, sh->n_q, sh->n_kv, kappa, eta);
+    // head path on the forked stream when there is an MLP path to overlap with
+    ForkJoin& fj = fork_join(dev);
+    const bool forked = mlp && heads && fj.init() && cudaEventRecord(fj.fork, s) == cudaSuccess &&
+                        cudaStreamWaitEvent(fj.aux, fj.fork, 0) == cudaSuccess;
+    cudaStream_t hs = forked ? fj.aux : s;
+    if (heads) {
+        head_maps_kernel<<<1, 1024, 0, hs>>>((uint32_t)key, (uint32_t)(key >> 32), sh->layer, sh->n_q, sh->n_kv, kappa, eta);
         launched();
         if (cudaGetLastError() != cudaSuccess) st = fail(CLOAK_ERR_CUDA, "permute: head_maps launch failed");
         const uint32_t d = sh->head_dim;
-        if (st == CLOAK_OK && in[3]) st = rows(in[3], mk(3), eta, d, sh->n_q * d, hrow, sms, s);
-        if (st == CLOAK_OK && in[4]) st = rows(in[4], mk(4), kappa, d, sh->n_kv * d, hrow, sms, s);
-        if (st == CLOAK_OK && in[5]) st = rows(in[5], mk(5), kappa, d, sh->n_kv * d, hrow, sms, s);
+        if (st == CLOAK_OK && in[3]) st = rows(in[3], mk(3), eta, d, sh->n_q * d, hrow, sms, hs);
+        if (st == CLOAK_OK && in[4]) st = rows(in[4], mk(4), kappa, d, sh->n_kv * d, hrow, sms, hs);
+        if (st == CLOAK_OK && in[5]) st = rows(in[5], mk(5), kappa, d, sh->n_kv * d, hrow, sms, hs);
         if (st == CLOAK_OK && in[6])
-            st = e == 4 ? cols<uint32_t>(in[6], mk(6), eta, d, sh->hidden, sh->n_q * d, sms, s)
-                        : cols<uint16_t>(in[6], mk(6), eta, d, sh->hidden, sh->n_q * d, sms, s);
+            st = e == 4 ? cols<uint32_t>(in[6], mk(6), eta, d, sh->hidden, sh->n_q * d, sms, hs)
+                        : cols<uint16_t>(in[6], mk(6), eta, d, sh->hidden, sh->n_q * d, sms, hs);
     }
+    if (st == CLOAK_OK && mlp) {
+        st = keygen_device(key, (4ull << 32) | sh->layer, sh->inter, pi, nullptr, s);
+        // the column gather of `down` is bound by shared memory, not HBM: it too goes to the forked stream (once pi is
+        // there), beside the HBM-bound row gathers of gate and up
+        cudaStream_t ds = s;
+        if (forked && st == CLOAK_OK && in[2] && cudaEventRecord(fj.mid, s) == cudaSuccess &&
+            cudaStreamWaitEvent(fj.aux, fj.mid, 0) == cudaSuccess)
+            ds = fj.aux;
+        if (st == CLOAK_OK && in[2])
+            st = e == 4 ? cols<uint32_t>(in[2], mk(2), pi, 1, sh->hidden, sh->inter, sms, ds)
+                        : cols<uint16_t>(in[2], mk(2), pi, 1, sh->hidden, sh->inter, sms, ds);
+        if (st == CLOAK_OK && in[0]) st = rows(in[0], mk(0), pi, 1, sh->inter, hrow, sms, s);
+        if (st == CLOAK_OK && in[1]) st = rows(in[1], mk(1), pi, 1, sh->inter, hrow, sms, s);
+    }
+    if (forked) cudaEventRecord(fj.join, fj.aux);
+    if (forked) cudaStreamWaitEvent(s, fj.join, 0);                // join: everything after this call sees both paths done
     cudaFreeAsync(scratch, s);
     return st;
 }
