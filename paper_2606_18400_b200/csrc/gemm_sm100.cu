@@ -100,7 +100,7 @@ __global__ void __launch_bounds__(GM_THREADS, 1) gemm_tile128_kernel(const __gri
     extern __shared__ __align__(1024) unsigned char smem_raw[];
     __shared__ __align__(8) uint64_t wfull[GM_MAX_STAGES], wempty[GM_MAX_STAGES], xfull[GM_MAX_STAGES], xempty[GM_MAX_STAGES],
         tmem_full[2], tmem_empty[2];
-    __shared__ uint32_t tmem_base_s, last_flag;
+    __shared__ uint32_t tmem_base_s;
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     // dynamic shared memory is only guaranteed 16-byte aligned: round up to the 1 KiB the 128-byte swizzle needs
     const uint32_t smem_base = (smem_u32(smem_raw) + 1023u) & ~1023u;
@@ -266,13 +266,24 @@ __global__ void __launch_bounds__(GM_THREADS, 1) gemm_tile128_kernel(const __gri
                 if (!complete) {
                     __threadfence();
                     epi_bar();
+                    // The row's FIRST contributor finishes it (for that CTA it is the last row of its range, so the others --
+                    // which met the row at the start of theirs -- have published long before): every CTA reduces exactly one
+                    // row per op.  (With "last to arrive reduces", whoever was last fell behind, was last again, and the
+                    // launch ended with its slowest CTA: SMs active 70 % of the time at batch 128.)
                     if (etid == 0) {
-                        const uint32_t old = atomicAdd(counters + tn, 1u);
-                        last_flag = (old == ncontrib - 1);
-                        if (old == ncontrib - 1) counters[tn] = 0;               // self-reset for the next launch
+                        if (me != 0) {
+                            asm volatile("red.release.gpu.global.add.u32 [%0], %1;" :: "l"(counters + tn), "r"(1u) : "memory");
+                        } else {
+                            uint32_t seen;
+                            do {
+                                asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(seen) : "l"(counters + tn) : "memory");
+                                if (seen != ncontrib - 1) __nanosleep(64);
+                            } while (seen != ncontrib - 1);
+                            counters[tn] = 0;                                    // self-reset for the next launch
+                        }
                     }
                     epi_bar();
-                    if (last_flag) {
+                    if (me == 0) {
                         __threadfence();
                         const float* base = part + (size_t)tn * op.maxc * nout;
                         for (uint32_t m = 0; m < a.batch; m += 16) {
