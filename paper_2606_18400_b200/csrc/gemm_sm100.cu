@@ -16,7 +16,7 @@
 //     streams the same bytes with a full TMA ring.  Roles: warp 0 TMA producer, warp 1 MMA issuer (one lane)
 //     + TMEM allocator, warp 2 TMA producer for X (own shallow ring), warps 3-6 epilogue (tcgen05.ld 32x32b, one TMEM lane quarter each).
 //   * A tile row wholly inside a CTA's range is stored as bf16 straight from TMEM; one cut by a range boundary
-//     writes fp32 partials and the last contributor sums them in contributor order (deterministic; identical
+//     writes fp32 partials and the row's first contributor sums them in contributor order (deterministic; identical
 //     for cloaked and identity-table pools).
 #include <cuda_bf16.h>
 #include "common.cuh"
