@@ -739,3 +739,81 @@ def test_moe_decode_through_the_cloaked_pool_equals_the_unpermuted_moe():
             torch.cuda.synchronize()
             got = sum(wi * y.double().cpu().numpy() for wi, y in zip(w, ys))
             assert O.err_normwise(got, O.moe_f64(x, router, gate, up, down, k)) <= TOL["bf16"], tok
+
+
+# ------------------------------------------------------------------ randomised chains (shapes, lengths, dependencies)
+@pytest.mark.parametrize("seed", [0, 1, 2, 3])
+def test_gemv_chain_random_lists_equal_single_calls(seed):
+    """Random op lists (1..60 ops, rows of 512 B .. 28 KiB, N from 16 to 4 096, mixed chunk sizes -> several launches,
+    random `after` 0/1/2 with real data dependencies, random gate epilogues): bit-identical to the same ops issued one
+    cloak_gemv / cloak_silu_mul at a time, and every op fed by a generator vector against the fp64 oracle."""
+    rng = np.random.default_rng(100 + seed)
+    key, block, page = 0x1234, 65536, 2 << 20
+    batch = int(rng.choice([1, 3, 8, 9, 16]))
+    n_w = 6
+    shapes = [(int(rng.choice([16, 48, 256, 1024, 4096])), int(rng.choice([256, 512, 768, 2048, 3584, 14336]))) for _ in range(n_w)]
+    Ws = [gen.synth(seed, i, shp, "bf16") for i, shp in enumerate(shapes)]
+    offs, total = C.cloak_arena_plan(key, [2 * n * k for n, k in shapes], block)
+    with Pool(total, block, page, key) as p:
+        _load_pool(p, [(f"w{i}", w) for i, w in enumerate(Ws)], offs, "bf16")
+        T = [C.cloak_tensor(o, n, k, C.CLOAK_BF16, C.CLOAK_ROWMAJOR) for (n, k), o in zip(shapes, offs)]
+        X0 = {k: bf16_dev_from_bits(gen.synth(seed + 50, k, (batch, k), "bf16", kind=gen.KIND_NORMAL)) for k in {k for _, k in shapes}}
+        n_ops = int(rng.integers(1, 61))
+        ops_c, ops_s, outs_c, outs_s, last_dep = [], [], [], [], False
+        for j in range(n_ops):
+            wi = int(rng.integers(0, n_w))
+            n, k = shapes[wi]
+            yc = torch.zeros(batch, n, dtype=torch.bfloat16, device="cuda")
+            ys = torch.zeros_like(yc)
+            # input: a fresh vector, or the output of an earlier op with matching width (a real dependency)
+            cands = [i for i in range(j) if outs_c[i].shape[1] == k]
+            if cands and rng.random() < 0.4:
+                src = int(rng.choice(cands))
+                xc, xs = outs_c[src], outs_s[src]
+                after = 2 if (last_dep and rng.random() < 0.5) else 1
+                last_dep = True
+            else:
+                xc = xs = X0[k]
+                after = 0
+            # gate epilogue from an earlier op of the same shape
+            gates = [i for i in range(j) if ops_c[i][0] is T[wi]]
+            if gates and rng.random() < 0.3:
+                gi = int(rng.choice(gates))
+                ac, as_ = torch.zeros_like(yc), torch.zeros_like(yc)
+                ops_c.append((T[wi], xc, yc, after, outs_c[gi], ac))
+                ops_s.append((T[wi], xs, ys, outs_s[gi], as_))
+            else:
+                ops_c.append((T[wi], xc, yc, after))
+                ops_s.append((T[wi], xs, ys, None, None))
+            outs_c.append(yc)
+            outs_s.append(ys)
+        # `after = 2` must follow a waiting op whose dependency covers it: make every dependent op wait for everything before it
+        ops_c = [op if op[3] != 2 else op[:3] + (1,) + op[4:] for op in ops_c] if rng.random() < 0.5 else ops_c
+        # an `after = 2` op shares the arrival of the nearest earlier waiting op, so its source must precede that op: enforce
+        fixed, last_wait_at = [], -1
+        for j, op in enumerate(ops_c):
+            if op[3] == 1:
+                last_wait_at = j
+            if op[3] == 2:
+                srcs = [i for i in range(j) if outs_c[i] is op[1]]
+                if last_wait_at < 0 or (srcs and srcs[0] >= last_wait_at):
+                    op = op[:3] + (1,) + op[4:]
+                    last_wait_at = j
+            fixed.append(op)
+        C.cloak_gemv_chain(p.h, fixed, batch)
+        for t, x, y, g, a_ in ops_s:
+            C.cloak_gemv(p.h, t, x, y, batch)
+            if g is not None:
+                C.cloak_silu_mul(g, y, a_, y.numel(), C.CLOAK_BF16)
+        torch.cuda.synchronize()
+        for j in range(n_ops):
+            assert torch.equal(outs_c[j], outs_s[j]), (seed, j, n_ops)
+            if len(fixed[j]) == 6:
+                assert torch.equal(fixed[j][5], ops_s[j][4]), (seed, j, "act")
+        # against the oracle: every op whose input is a generator vector (never an oracle input from the CUDA path)
+        Xh = {k: gen.synth(seed + 50, k, (batch, k), "bf16", kind=gen.KIND_NORMAL) for k in X0}
+        for j in range(n_ops):
+            if any(ops_s[j][1] is X0[k] for k in X0):
+                wi = [i for i in range(n_w) if T[i] is ops_s[j][0]][0]
+                ref = O.linear_f64(Xh[shapes[wi][1]], Ws[wi])
+                assert O.err_normwise(outs_c[j].float().cpu().numpy(), ref) <= TOL["bf16"], (seed, j)
