@@ -84,11 +84,11 @@ cloak_status keygen_device(uint64_t key, uint64_t stream_id, uint32_t n, uint32_
                            cudaStream_t s);
 constexpr size_t WS_COUNTER_BYTES = 1u << 20;
 cloak_status pool_workspace(const cloak_pool* pool, size_t bytes);
-// gemv_stream.cu: persistent TMA-fed bf16 GEMV chain (K % 256 == 0).  gemv_stream_log2cb: the row-chunk size the
+// gemv_stream.cu: persistent TMA-fed bf16 GEMV chain (K % 256 == 0).  gemv_stream_chunk: the row-chunk size (in 512-byte units) the
 // kernel would use for a tensor, or -1 if it cannot take it; gemv_stream_launch: one launch of <= 48 ops that
 // share that chunk size.
-int gemv_stream_log2cb(const cloak_pool* pool, const cloak_tensor* w, uint32_t batch);
-cloak_status gemv_stream_launch(const cloak_pool* pool, const cloak_gemv_op* ops, uint32_t n, int log2cb, uint32_t batch,
+int gemv_stream_chunk(const cloak_pool* pool, const cloak_tensor* w, uint32_t batch);
+cloak_status gemv_stream_launch(const cloak_pool* pool, const cloak_gemv_op* ops, uint32_t n, int cu, uint32_t batch,
                                 cudaStream_t s);
 // Host-side Philox keygen used only by cloak_arena_plan (T is tiny; no device work wanted there).
 void keygen_host(uint64_t key, uint64_t stream_id, uint32_t n, std::vector<uint32_t>& perm);

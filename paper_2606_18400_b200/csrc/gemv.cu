@@ -271,8 +271,8 @@ static cloak_status gemv_device(const cloak_pool* pool, const cloak_tensor* w, c
     a.batch = batch;
     a.zero = 0;
     if (!g_force_oneshot) {
-        const int log2cb = gemv_stream_log2cb(pool, w, batch);
-        if (log2cb >= 9) {
+        const int cu = gemv_stream_chunk(pool, w, batch);
+        if (cu >= 1) {
             cloak_gemv_op op;
             op.w = *w;
             op.d_x = d_x;
@@ -280,7 +280,7 @@ static cloak_status gemv_device(const cloak_pool* pool, const cloak_tensor* w, c
             op.d_gate = nullptr;
             op.d_act = nullptr;
             op.after = 0;
-            return gemv_stream_launch(pool, &op, 1, log2cb, batch, s);
+            return gemv_stream_launch(pool, &op, 1, cu, batch, s);
         }
     }
     if (w->dt == CLOAK_BF16) {
@@ -363,8 +363,8 @@ extern "C" cloak_status cloak_gemv_chain(const cloak_pool* pool, const cloak_gem
             for (uint32_t k = 0; k < i; ++k)
                 if (h_ops[k].d_y == h_ops[i].d_gate && (h_ops[k].w.N != h_ops[i].w.N || h_ops[k].w.K != h_ops[i].w.K))
                     return fail(CLOAK_ERR_INVALID, "gemv_chain: op %u: d_gate is the output of op %u, which has another shape", i, k);
-        cb[i] = gemv_stream_log2cb(pool, &h_ops[i].w, batch);
-        if (cb[i] < 9) return fail(CLOAK_ERR_UNSUPPORTED, "gemv_chain: op %u needs bf16 ROWMAJOR, K %% 256 == 0, block >= 512", i);
+        cb[i] = gemv_stream_chunk(pool, &h_ops[i].w, batch);
+        if (cb[i] < 1) return fail(CLOAK_ERR_UNSUPPORTED, "gemv_chain: op %u needs bf16 ROWMAJOR, K %% 256 == 0, block >= 512", i);
     }
     DeviceGuard g(pool->device);
     // consecutive ops with one chunk size, at most 48 at a time and within the row-tile counters, share a launch

@@ -92,8 +92,8 @@ constexpr int gs_tg(int) { return 8; }
 constexpr int gs_nacc(int) { return 2; }
 constexpr int GS_TGR = 4;                             // row tiles reduced across warps per shared-memory pass
 constexpr int GS_MAX_STAGES = 12;
-constexpr uint32_t gs_stages(int log2cb) {            // ~192 KiB of weights in flight per SM
-    return (196608u >> (log2cb + 3)) > GS_MAX_STAGES ? GS_MAX_STAGES : (196608u >> (log2cb + 3));
+constexpr uint32_t gs_stages(int cu) {                // cu = chunk bytes / 512; ~192 KiB of weights in flight per SM
+    return 196608u / (GS_ROWS * (cu * 512u + GS_PAD)) > GS_MAX_STAGES ? GS_MAX_STAGES : 196608u / (GS_ROWS * (cu * 512u + GS_PAD));
 }
 
 __device__ __forceinline__ void mma_16816(float c[4], uint32_t a0, uint32_t a1, uint32_t a2, uint32_t a3, uint32_t b0,
@@ -143,13 +143,15 @@ __device__ __forceinline__ uint16_t ld_coherent_u16(const uint16_t* p) {
     return v;
 }
 
-// LOG2CB: log2 of the chunk bytes per row (9..12).  NT: 1 = batch <= 8 (upper half of the MMA's M is zero), 2 = batch <= 16.
-template <int LOG2CB, int NT>
+// CU: chunk bytes per row / 512 (1..8; the largest divisor of the row's 512-byte units that is <= 8, so a 10 KiB row is cut
+// into 2.5 KiB chunks and a 1.5 KiB row is one chunk -- larger TMA pieces than a power of two would allow).
+// NT: 1 = batch <= 8 (upper half of the MMA's M is zero), 2 = batch <= 16.
+template <int CU, int NT>
 __global__ void __launch_bounds__(gs_threads(NT), 1) gemv_chain_kernel(const __grid_constant__ ChainArgs a) {
-    constexpr uint32_t CB = 1u << LOG2CB;
+    constexpr uint32_t CB = CU * 512u;
     constexpr uint32_t RS = CB + GS_PAD;                       // staged row stride
     constexpr uint32_t STAGE = GS_ROWS * RS;
-    constexpr uint32_t NST = gs_stages(LOG2CB);
+    constexpr uint32_t NST = gs_stages(CU);
     constexpr int KS = CB / (GS_CONSUMERS * 64);               // 64-byte steps (one 16-byte vector per lane) per warp per unit
     constexpr bool PF = (NT == 2);                             // prefetch the next phase's X fragments (see below)
     constexpr int LEAD = gs_lead_warps(NT);
@@ -199,10 +201,19 @@ __global__ void __launch_bounds__(gs_threads(NT), 1) gemv_chain_kernel(const __g
                         if (lane == 0) mbar_expect_tx(bar, GS_ROWS * CB);
                         __syncwarp();
                         if (lane < GS_ROWS) {
-                            const uint64_t off = op.w_offset + (uint64_t)(tile * GS_ROWS + lane) * row_bytes + (uint64_t)c * CB;
-                            const uint32_t slot = __ldg(a.T + (off >> a.log2b));
-                            const char* src = a.pool + ((uint64_t)slot << a.log2b) + (off & ((1ull << a.log2b) - 1));
-                            bulk_g2s(smem_base + s * STAGE + lane * RS, src, CB, bar);
+                            // a chunk that is not a power of two may cross a block boundary: one bulk copy per block touched
+                            uint64_t off = op.w_offset + (uint64_t)(tile * GS_ROWS + lane) * row_bytes + (uint64_t)c * CB;
+                            uint32_t dst = smem_base + s * STAGE + lane * RS, left = CB;
+                            while (left) {
+                                const uint64_t in_block = off & ((1ull << a.log2b) - 1);
+                                const uint64_t room = (1ull << a.log2b) - in_block;
+                                const uint32_t n = room < left ? (uint32_t)room : left;
+                                const uint32_t slot = __ldg(a.T + (off >> a.log2b));
+                                bulk_g2s(dst, a.pool + ((uint64_t)slot << a.log2b) + in_block, n, bar);
+                                off += n;
+                                dst += n;
+                                left -= n;
+                            }
                         }
                         if (++s == NST) { s = 0; ph ^= 1; wrapped = true; }
                     }
@@ -401,12 +412,12 @@ bool g_gemv_pdl = true;      // A/B switch (cloak_set_gemv_engine(2) turns PDL o
 // Counter words [0, GS_TILE_COUNTERS) of the pool's scratch are row-tile arrival counters, the rest op barriers.
 constexpr uint32_t GS_TILE_COUNTERS = (uint32_t)(WS_COUNTER_BYTES / 4) - 4 * GS_MAX_OPS;
 
-template <int LOG2CB, int NT>
+template <int CU, int NT>
 static cloak_status launch(const ChainArgs& a, int ctas, cudaStream_t s) {
-    constexpr size_t smem = (size_t)gs_stages(LOG2CB) * GS_ROWS * ((1u << LOG2CB) + GS_PAD);
+    constexpr size_t smem = (size_t)gs_stages(CU) * GS_ROWS * (CU * 512u + GS_PAD);
     static bool attr_set = false;
     if (!attr_set) {
-        CLOAK_CUDA(cudaFuncSetAttribute(gemv_chain_kernel<LOG2CB, NT>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        CLOAK_CUDA(cudaFuncSetAttribute(gemv_chain_kernel<CU, NT>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
         attr_set = true;
     }
     cudaLaunchConfig_t cfg = {};
@@ -419,24 +430,23 @@ static cloak_status launch(const ChainArgs& a, int ctas, cudaStream_t s) {
     at[0].val.programmaticStreamSerializationAllowed = 1;
     cfg.attrs = at;
     cfg.numAttrs = g_gemv_pdl ? 1 : 0;
-    CLOAK_CUDA(cudaLaunchKernelEx(&cfg, gemv_chain_kernel<LOG2CB, NT>, a));
+    CLOAK_CUDA(cudaLaunchKernelEx(&cfg, gemv_chain_kernel<CU, NT>, a));
     launched();
     return CLOAK_OK;
 }
 
 // log2 of the row-chunk size the streaming kernel would use for this tensor, or -1 if it cannot take it.
-int gemv_stream_log2cb(const cloak_pool* pool, const cloak_tensor* w, uint32_t batch) {
+int gemv_stream_chunk(const cloak_pool* pool, const cloak_tensor* w, uint32_t batch) {
     if (w->dt != CLOAK_BF16 || w->layout != CLOAK_ROWMAJOR || w->K % 256 || w->N % GS_ROWS || pool->block < 512) return -1;
-    const uint64_t row_bytes = (uint64_t)w->K * 2;
-    int log2cb = 12;
-    while (log2cb > 9 && (row_bytes & ((1u << log2cb) - 1))) --log2cb;
-    if ((uint32_t)log2cb > pool->log2_block) log2cb = (int)pool->log2_block;
-    (void)batch;   // measured: forcing 2 KiB chunks at batch 9..16 so that the X prefetch fits costs 35 % (8 x 2 KiB stages)
-    return log2cb;
+    (void)batch;   // measured: forcing 2 KiB chunks at batch 9..16 so that the X prefetch fits 168 registers costs 35 %
+    const uint32_t u = (uint32_t)(((uint64_t)w->K * 2) / 512);          // the row in 512-byte units
+    int cu = 8;
+    while (u % cu) --cu;
+    return cu;
 }
 
-// One launch: n <= GS_MAX_OPS ops that all stream with the same chunk size.  Preconditions checked by the callers.
-cloak_status gemv_stream_launch(const cloak_pool* pool, const cloak_gemv_op* ops, uint32_t n, int log2cb, uint32_t batch,
+// One launch: n <= GS_MAX_OPS ops that all stream with the same chunk size (cu x 512 bytes).  Preconditions checked by the callers.
+cloak_status gemv_stream_launch(const cloak_pool* pool, const cloak_gemv_op* ops, uint32_t n, int cu, uint32_t batch,
                                 cudaStream_t s) {
     ChainArgs a;
     a.pool = pool->base;
@@ -458,7 +468,7 @@ cloak_status gemv_stream_launch(const cloak_pool* pool, const cloak_gemv_op* ops
         o.act = static_cast<uint16_t*>(ops[j].d_act);
         o.N = w.N;
         o.K = w.K;
-        o.kch = (uint32_t)(((uint64_t)w.K * 2) >> log2cb);
+        o.kch = (uint32_t)(((uint64_t)w.K * 2) / (512u * cu));
         const uint64_t units64 = (uint64_t)(w.N / GS_ROWS) * o.kch;
         if (units64 > 0xffffffffull) return fail(CLOAK_ERR_UNSUPPORTED, "gemv: tensor too large");
         o.units = (uint32_t)units64;
@@ -509,12 +519,12 @@ cloak_status gemv_stream_launch(const cloak_pool* pool, const cloak_gemv_op* ops
     a.early = (g_gemv_pdl && !pool->dirty) ? 1u : 0u;
     if (pool->dirty && pool->dirty_stream == s) pool->dirty = false;   // this launch waits for the writer in full
     const bool nt2 = batch > 8;
-    switch (log2cb) {
-        case 12: return nt2 ? launch<12, 2>(a, ctas, s) : launch<12, 1>(a, ctas, s);
-        case 11: return nt2 ? launch<11, 2>(a, ctas, s) : launch<11, 1>(a, ctas, s);
-        case 10: return nt2 ? launch<10, 2>(a, ctas, s) : launch<10, 1>(a, ctas, s);
-        default: return nt2 ? launch<9, 2>(a, ctas, s) : launch<9, 1>(a, ctas, s);
+#define GS_CASE(C) case C: return nt2 ? launch<C, 2>(a, ctas, s) : launch<C, 1>(a, ctas, s)
+    switch (cu) {
+        GS_CASE(8); GS_CASE(7); GS_CASE(6); GS_CASE(5); GS_CASE(4); GS_CASE(3); GS_CASE(2);
+        default: return nt2 ? launch<1, 2>(a, ctas, s) : launch<1, 1>(a, ctas, s);
     }
+#undef GS_CASE
 }
 
 }  // namespace cloak
