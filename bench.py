@@ -235,6 +235,8 @@ def run_cloak(args):
     pool_create_s = time.perf_counter() - t0
     pool_b = C.cloak_pool_create(local, total, block, page, KEY_B)
     pool_n = C.cloak_pool_create(local, total, block, page, KEY_A, C.CLOAK_POOL_IDENTITY)   # the "native" layout
+    # the same identity layout in ONE plain allocation: exposes any cost of the 2 MiB-fragmented VMM mapping
+    pool_p = C.cloak_pool_create(local, total, block, page, KEY_A, C.CLOAK_POOL_IDENTITY | C.CLOAK_POOL_PLAIN_ALLOC)
     info = C.cloak_pool_info(pool_a)
     scratch = torch.empty(2 * info["nslots"] + 2 * info["npages"], dtype=torch.int32, device="cuda")
     X = {b: {k: synth_cuda.fill(torch.empty(b, k, dtype=torch.bfloat16, device="cuda"), seed + 100, b * 2 + (k != c["hidden"]),
@@ -327,6 +329,7 @@ def run_cloak(args):
     step()
     for (nm, _), o in zip(shapes, offs):
         C.cloak_shuffle(pool_n, perm[nm], o, perm[nm].numel() * 2, stream)
+        C.cloak_shuffle(pool_p, perm[nm], o, perm[nm].numel() * 2, stream)
     for _ in range(max(args.warmup - 1, 0)):
         step()
     barrier()
@@ -347,31 +350,35 @@ def run_cloak(args):
 
     # ---- the same GEMV chains on the identity-table ("native") pool: the overhead denominator.  Same launch mode,
     # cloaked and native interleaved rep by rep so that drift hits both alike.
-    native_ms, cloaked_iso_ms, per_call_ms = {}, {}, {}
+    native_ms, cloaked_iso_ms, per_call_ms, plain_ms, matmul_ms = {}, {}, {}, {}, {}
     for b in BATCHES:
         gemv_chain(pool_n, b)
+        gemv_chain(pool_p, b)
         gemv_chain(pool_n, b, per_call=True)
+
+        def torch_matmul():                       # context only: cuBLAS on the plain permuted tensors, same shapes
+            for nm, (n, k) in shapes:
+                torch.matmul(X[b][k], perm[nm].t(), out=Y[b][nm])
+        torch_matmul()
         torch.cuda.synchronize()
-        rn, _ = capture(lambda: gemv_chain(pool_n, b))
-        rc, _ = capture(lambda: gemv_chain(pool_a, b))
-        rp, _ = capture(lambda: gemv_chain(pool_a, b, per_call=True))
+        variants = [(capture(lambda: gemv_chain(pool_n, b))[0], []), (capture(lambda: gemv_chain(pool_a, b))[0], []),
+                    (capture(lambda: gemv_chain(pool_a, b, per_call=True))[0], []), (capture(lambda: gemv_chain(pool_p, b))[0], []),
+                    (capture(torch_matmul)[0], [])]
         reps = max(args.steps, 5)
-        tn, tc, tp = [], [], []
-        for r_, acc_ in ((rn, tn), (rc, tc), (rp, tp)):
+        for r_, _ in variants:
             for _ in range(3):
                 r_()
         torch.cuda.synchronize()
         for _ in range(reps):
-            for r_, acc_ in ((rn, tn), (rc, tc), (rp, tp)):
+            for r_, acc_ in variants:
                 e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
                 e0.record(stream)
                 r_()
                 e1.record(stream)
                 acc_.append((e0, e1))
         torch.cuda.synchronize()
-        native_ms[b] = float(np.median([e0.elapsed_time(e1) for e0, e1 in tn]))
-        cloaked_iso_ms[b] = float(np.median([e0.elapsed_time(e1) for e0, e1 in tc]))
-        per_call_ms[b] = float(np.median([e0.elapsed_time(e1) for e0, e1 in tp]))
+        med = [float(np.median([e0.elapsed_time(e1) for e0, e1 in acc_])) for _, acc_ in variants]
+        native_ms[b], cloaked_iso_ms[b], per_call_ms[b], plain_ms[b], matmul_ms[b] = med
 
     # ---- correctness inside the bench: the round trip restores the permuted weights bit for bit
     ok = all(torch.equal(back[nm], perm[nm]) for nm in perm)
@@ -406,7 +413,7 @@ def run_cloak(args):
     map_ms = C.cloak_pool_map_ms(pool_a)
     adjacency = C.cloak_pool_adjacency(pool_a)          # layout quality (G8): neighbours that stayed neighbours
     torch.cuda.synchronize()
-    for p in (pool_a, pool_b, pool_n):
+    for p in (pool_a, pool_b, pool_n, pool_p):
         C.cloak_pool_destroy(p)
 
     if rank != 0:
@@ -441,7 +448,8 @@ def run_cloak(args):
         "shuffle_gbs": stages["shuffle"]["gbs"], "shuffle_frac_hbm": stages["shuffle"]["frac_hbm"],
         "gemv_gbs": {f"b{b}": stages[f"gemv_b{b}"]["gbs"] for b in BATCHES},
         "gemv_frac_hbm": {f"b{b}": stages[f"gemv_b{b}"]["frac_hbm"] for b in BATCHES},
-        "gemv_isolated_ms": {"cloaked": cloaked_iso_ms, "native": native_ms, "cloaked_7_separate_calls": per_call_ms},
+        "gemv_isolated_ms": {"cloaked": cloaked_iso_ms, "native": native_ms, "cloaked_7_separate_calls": per_call_ms,
+                             "native_one_plain_allocation": plain_ms, "torch_matmul_context": matmul_ms},
         "cloaked_vs_native_overhead_pct": overhead,
         "hbm_peak_gbs": peak, "hbm_peak_kind": peak_kind, "hbm_nominal_gbs": 8000.0,
         "pool_map_ms": map_ms, "layout_adjacency": adjacency, "pool_create_s": pool_create_s, "roundtrip_bit_exact": bool(ok),
