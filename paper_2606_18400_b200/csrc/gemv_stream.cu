@@ -2,7 +2,8 @@
 //
 // Same contraction and table translation as gemv.cu (north_star (c)), organised for the
 // HBM roofline.  Measured on B200: a pure stream of 16 x 2 KiB row pieces per stage tops out
-// at 5.5 TB/s, 8 x 4 KiB pieces at 6.4 TB/s, so a unit of work is (8 weight rows) x (CB = 4 KiB of each row):
+// at 5.5 TB/s, 8 x 4 KiB pieces at 6.4 TB/s, so a unit of work is (8 weight rows) x (CB of each row), CB = the largest
+// multiple of 512 B up to 4 KiB that divides the row (4 KiB for every LLaMA / Qwen projection but a few):
 //   * one persistent CTA per SM; an op's units are numbered tile-major (u = tile * kch + chunk) and cut into
 //     equal contiguous ranges, one per CTA (stream-K): every SM moves the same bytes, no wave tail;
 //   * warp 0 produces: 8 lanes each translate one row piece through the block table and issue one
@@ -25,7 +26,8 @@
 //     addresses.  No fence, atomic round trip or reduction sits at the end of the other CTAs.
 //   * a launch executes a CHAIN of ops (cloak_gemv_chain; cloak_gemv is a chain of one).  The producer warp
 //     runs straight through the chain -- weights do not depend on activations -- so HBM stays busy across op
-//     boundaries; only the consumers of an op marked `after` wait, on a grid-wide arrival counter, for all CTAs
+//     boundaries (an op with fewer ranges than CTAs starts at the CTA where the previous one stopped when such ops
+//     dominate the launch); only the consumers of an op marked `after` wait, on a grid-wide arrival counter, for all CTAs
 //     to have finished the earlier ops (its X is their Y); several ops can share one such arrival.  An op may also emit silu(G) * Y next to Y in its
 //     epilogue (the gated MLP's activation, O9), where G is the output of an earlier op of the same shape -- the
 //     same CTA wrote those very elements, so no wait is needed -- and gate/up -> down costs no separate pass.
