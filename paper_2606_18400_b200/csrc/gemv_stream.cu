@@ -95,7 +95,7 @@ constexpr int gs_nacc(int) { return 2; }
 constexpr int GS_TGR = 4;                             // row tiles reduced across warps per shared-memory pass
 constexpr int GS_MAX_STAGES = 12;
 constexpr uint32_t gs_stages(int cu) {                // cu = chunk bytes / 512; ~192 KiB of weights in flight per SM
-    return 196608u / (GS_ROWS * (cu * 512u + GS_PAD)) > GS_MAX_STAGES ? GS_MAX_STAGES : 196608u / (GS_ROWS * (cu * 512u + GS_PAD));
+    return 196608u / (GS_ROWS * cu * 512u) > GS_MAX_STAGES ? GS_MAX_STAGES : 196608u / (GS_ROWS * cu * 512u);
 }
 
 __device__ __forceinline__ void mma_16816(float c[4], uint32_t a0, uint32_t a1, uint32_t a2, uint32_t a3, uint32_t b0,
@@ -206,6 +206,11 @@ __global__ void __launch_bounds__(gs_threads(NT), 1) gemv_chain_kernel(const __g
                             // a chunk that is not a power of two may cross a block boundary: one bulk copy per block touched
                             uint64_t off = op.w_offset + (uint64_t)(tile * GS_ROWS + lane) * row_bytes + (uint64_t)c * CB;
                             uint32_t dst = smem_base + s * STAGE + lane * RS, left = CB;
+                            if ((CU & (CU - 1)) == 0 && CB <= (1u << a.log2b)) {       // power of two within a block: one copy
+                                const uint32_t slot = __ldg(a.T + (off >> a.log2b));
+                                bulk_g2s(dst, a.pool + ((uint64_t)slot << a.log2b) + (off & ((1ull << a.log2b) - 1)), CB, bar);
+                                left = 0;
+                            }
                             while (left) {
                                 const uint64_t in_block = off & ((1ull << a.log2b) - 1);
                                 const uint64_t room = (1ull << a.log2b) - in_block;
