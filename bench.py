@@ -31,7 +31,7 @@ BATCHES = (1, 4, 16)
 KEY_A, KEY_B = 0x1234, 0x5678          # G11
 # dram__bytes_read.sum + dram__bytes_write.sum of one gemv_chain_kernel launch (the 7 projections at one batch), mean of
 # the three launches of a step in the committed `ncu --set full` capture; algorithmic bytes are 436 207 616.
-NCU_TRAFFIC_PER_LAUNCH = 441.4e6
+NCU_TRAFFIC_PER_LAUNCH = 442.2e6
 NCU_TRAFFIC_SOURCE = "profiles/r1_ncu_full_gemv_chain.md"
 FALLBACK_HBM_GBS = 6650.0              # B200_PROFILING.md fallback when MEASURED_PEAKS.json is absent
 
