@@ -11,13 +11,18 @@
 //     SWIZZLE_128B, which land in shared memory in the canonical K-major UMMA layout (8-row atoms of 1 KiB).
 //   * A operand = the W tile (M = 128 output features), B operand = X[batch, 64] boxes of a second map over X
 //     (N = batch), D = 128 lanes x batch fp32 columns in TMEM, two accumulator buffers.
-//   * Units = tiles, numbered tn-major (= TILE128 storage order), cut into equal contiguous ranges, one per
-//     persistent CTA (stream-K): HBM-bound (AI = batch flop/B < ridge), so what matters is that every SM
+//   * Units = tiles, numbered tn-major (= TILE128 storage order), the ops of a launch back to back, cut into equal
+//     contiguous ranges, one per persistent CTA (stream-K over the whole op list): HBM-bound (AI = batch flop/B < ridge), so what matters is that every SM
 //     streams the same bytes with a full TMA ring.  Roles: warp 0 TMA producer, warp 1 MMA issuer (one lane)
 //     + TMEM allocator, warp 2 TMA producer for X (own shallow ring), warps 3-6 epilogue (tcgen05.ld 32x32b, one TMEM lane quarter each).
 //   * A tile row wholly inside a CTA's range is stored as bf16 straight from TMEM; one cut by a range boundary
-//     writes fp32 partials and the row's first contributor sums them in contributor order (deterministic; identical
-//     for cloaked and identity-table pools).
+//     has its later contributors write fp32 partials; the row's first contributor adds them, in contributor order, to
+//     its own accumulator as it drains it (deterministic; identical for cloaked and identity-table pools).
+//   * PAIR variant (batch >= 64 by default): the grid is launched as clusters of two CTAs (one TPC) that work as a
+//     `cta_group::2` pair on TWO adjacent tile rows with the same k tile: each CTA streams its own W tile and only HALF
+//     of the X tile (batch/2 rows), the leader issues one M = 256 MMA that reads B from both CTAs' shared memory, and
+//     each CTA drains its own 128 TMEM lanes.  Units are then (tile-row pair, k tile), one range per pair.  At batch
+//     128 the X tile is as large as the W tile, so this takes the L2 -> SM traffic from 2 x W to 1.5 x W.
 #include <cuda_bf16.h>
 #include "common.cuh"
 #include "async.cuh"
@@ -32,12 +37,10 @@ struct GemmOp {
     uint64_t part_base;  // float offset of this op's partials: [tile row][maxc][batch][128]
     uint32_t N;
     uint32_t kt;         // k tiles per tile row = K/128
-    uint32_t units;      // (N/128) * kt
-    uint32_t per;        // units per CTA
+    uint32_t units;      // (N/128) * kt; pair variant: ceil(N/256) * kt
+    uint32_t ubase;      // this op's first unit in the launch's unit sequence (ops back to back)
     uint32_t maxc;       // max contributors per tile row
     uint32_t row_base;   // index of this op's first tile-row counter
-    uint32_t rot;        // range r of this op belongs to CTA (r + rot) % grid: ops with fewer ranges than CTAs start where
-                         // the previous op stopped, so the idle CTAs are different ones each time
 };
 
 struct GemmArgs {
@@ -47,6 +50,8 @@ struct GemmArgs {
     uint32_t log2b;
     uint32_t batch;
     uint32_t nops;
+    uint32_t per;        // units per range: the launch's units (all ops back to back) are cut into equal contiguous ranges
+    uint32_t total;      // units of the launch
     uint32_t wstages;    // ring of 32 KiB weight tiles (HBM latency: deep)
     uint32_t xstages;    // ring of X tiles [batch x 128] (L2 latency: shallow)
     uint32_t tmem_cols;  // power of two >= 2*batch
@@ -62,10 +67,46 @@ __device__ __forceinline__ void tma_load_2d(uint32_t dst, const CUtensorMap* map
     asm volatile("cp.async.bulk.tensor.2d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3}], [%4];"
                  :: "r"(dst), "l"(map), "r"(c0), "r"(c1), "r"(bar) : "memory");
 }
+// cta_group::2 flavour: executed by both CTAs of the pair, the data lands in the issuing CTA's shared memory, the bytes
+// are counted on the LEADER's barrier (`bar` is a shared::cluster address).
+__device__ __forceinline__ void tma_load_2d_pair(uint32_t dst, const CUtensorMap* map, uint32_t c0, uint32_t c1, uint32_t bar) {
+    asm volatile("cp.async.bulk.tensor.2d.cta_group::2.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3}], [%4];"
+                 :: "r"(dst), "l"(map), "r"(c0), "r"(c1), "r"(bar) : "memory");
+}
+__device__ __forceinline__ uint32_t cluster_ctarank() {
+    uint32_t r;
+    asm volatile("mov.u32 %0, %%cluster_ctarank;" : "=r"(r));
+    return r;
+}
+// shared::cluster address of the same shared-memory offset in CTA `rank` of the cluster
+__device__ __forceinline__ uint32_t map_to_cta(uint32_t smem_addr, uint32_t rank) {
+    uint32_t r;
+    asm volatile("mapa.shared::cluster.u32 %0, %1, %2;" : "=r"(r) : "r"(smem_addr), "r"(rank));
+    return r;
+}
+__device__ __forceinline__ void mbar_arrive_cluster(uint32_t cluster_bar) {
+    asm volatile("mbarrier.arrive.release.cluster.shared::cluster.b64 _, [%0];" :: "r"(cluster_bar) : "memory");
+}
+__device__ __forceinline__ void cluster_sync_all() {
+    asm volatile("barrier.cluster.arrive.release;" ::: "memory");
+    asm volatile("barrier.cluster.wait.acquire;" ::: "memory");
+}
 __device__ __forceinline__ void tc_fence_after() { asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory"); }
 __device__ __forceinline__ void tc_fence_before() { asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory"); }
 __device__ __forceinline__ void tc_commit(uint32_t bar) {
     asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];" :: "r"(bar) : "memory");
+}
+// Pair flavours: the arrival goes to the barrier at this offset in BOTH CTAs; the MMA spans both CTAs' tensor cores.
+__device__ __forceinline__ void tc_commit_pair(uint32_t bar) {
+    asm volatile("tcgen05.commit.cta_group::2.mbarrier::arrive::one.shared::cluster.multicast::cluster.b64 [%0], %1;"
+                 :: "r"(bar), "h"((uint16_t)3) : "memory");
+}
+__device__ __forceinline__ void tc_mma_bf16_pair(uint32_t d_tmem, uint64_t adesc, uint64_t bdesc, uint32_t idesc, uint32_t acc) {
+    asm volatile(
+        "{\n\t.reg .pred p;\n\t"
+        "setp.ne.b32 p, %4, 0;\n\t"
+        "tcgen05.mma.cta_group::2.kind::f16 [%0], %1, %2, %3, p;\n\t}"
+        :: "r"(d_tmem), "l"(adesc), "l"(bdesc), "r"(idesc), "r"(acc) : "memory");
 }
 __device__ __forceinline__ void tc_mma_bf16(uint32_t d_tmem, uint64_t adesc, uint64_t bdesc, uint32_t idesc, uint32_t acc) {
     asm volatile(
@@ -95,6 +136,7 @@ __device__ __forceinline__ void epi_bar() { asm volatile("bar.sync 1, 128;" ::: 
 // the rings, the accumulator double buffer and their phases simply continue from op to op, so the weight stream does not
 // stop at an op boundary (per-launch head and tail cost ~4 us each; q, k, v, o of a Qwen-32B layer are 13 % of the bytes
 // and were 35 % of the time as separate launches).
+template <bool PAIR>
 __global__ void __launch_bounds__(GM_THREADS, 1) gemm_tile128_kernel(const __grid_constant__ CUtensorMap map_w,
                                                                      const __grid_constant__ GemmArgs a) {
     extern __shared__ __align__(1024) unsigned char smem_raw[];
@@ -103,7 +145,11 @@ __global__ void __launch_bounds__(GM_THREADS, 1) gemm_tile128_kernel(const __gri
     __shared__ uint32_t tmem_base_s;
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     // dynamic shared memory is only guaranteed 16-byte aligned: round up to the 1 KiB the 128-byte swizzle needs
+    // (same offset in both CTAs of a pair: same kernel, same static shared memory)
     const uint32_t smem_base = (smem_u32(smem_raw) + 1023u) & ~1023u;
+    const uint32_t crank = PAIR ? cluster_ctarank() : 0u;             // 0 = leader (issues the MMAs, owns the full barriers)
+    const uint32_t rank_in_grid = PAIR ? blockIdx.x / 2 : blockIdx.x;  // one range per CTA, or per CTA pair
+    const uint32_t gbeg = rank_in_grid * a.per, gend = min(gbeg + a.per, a.total);
 
     if (threadIdx.x == 0) {
         for (uint32_t s = 0; s < GM_MAX_STAGES; ++s) {
@@ -114,21 +160,28 @@ __global__ void __launch_bounds__(GM_THREADS, 1) gemm_tile128_kernel(const __gri
         }
         for (int i = 0; i < 2; ++i) {
             mbar_init(smem_u32(&tmem_full[i]), 1);
-            mbar_init(smem_u32(&tmem_empty[i]), 4);
+            mbar_init(smem_u32(&tmem_empty[i]), PAIR ? 8 : 4);        // the epilogue warps of both CTAs arrive at the leader's
         }
         fence_barrier_init();
     }
     if (warp == 1) {
-        asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;"
-                     :: "r"(smem_u32(&tmem_base_s)), "r"(a.tmem_cols) : "memory");
-        asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
+        if (PAIR) {
+            asm volatile("tcgen05.alloc.cta_group::2.sync.aligned.shared::cta.b32 [%0], %1;"
+                         :: "r"(smem_u32(&tmem_base_s)), "r"(a.tmem_cols) : "memory");
+            asm volatile("tcgen05.relinquish_alloc_permit.cta_group::2.sync.aligned;" ::: "memory");
+        } else {
+            asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;"
+                         :: "r"(smem_u32(&tmem_base_s)), "r"(a.tmem_cols) : "memory");
+            asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
+        }
     }
     tc_fence_before();
     __syncthreads();
+    if (PAIR) cluster_sync_all();                                     // the peer's barriers are initialised before anything lands
     tc_fence_after();
     const uint32_t tmem_base = tmem_base_s;
 
-    const uint32_t xbox = a.batch * 128;                     // bytes of one X box [batch x 64 bf16]
+    const uint32_t xbox = (PAIR ? a.batch / 2 : a.batch) * 128;      // bytes of this CTA's X box [rows x 64 bf16]
     const uint32_t xtile = 2 * xbox;
     const uint32_t x_base = smem_base + a.wstages * 32768;
 
@@ -138,20 +191,36 @@ __global__ void __launch_bounds__(GM_THREADS, 1) gemm_tile128_kernel(const __gri
         uint32_t it = 0;
         for (uint32_t j = 0; j < a.nops; ++j) {
             const GemmOp& op = a.ops[j];
-            const uint32_t vr = (blockIdx.x + gridDim.x - op.rot) % gridDim.x;      // this CTA's range of the op
-            const uint32_t ubeg = vr * op.per, uend = min(ubeg + op.per, op.units);
+            if (op.ubase + op.units <= gbeg || op.ubase >= gend) continue;         // this range's part of the op, in op units
+            const uint32_t ubeg = max(gbeg, op.ubase) - op.ubase, uend = min(gend, op.ubase + op.units) - op.ubase;
+            const uint32_t tile_rows = op.N / 128;
             for (uint32_t u = ubeg; u < uend; ++u, ++it) {
                 const uint32_t s = it % a.wstages, f = it / a.wstages;
                 if (f > 0) mbar_wait(smem_u32(&wempty[s]), (f - 1) & 1);
-                const uint64_t off = op.w_offset + (uint64_t)u * 32768;              // tile index == unit index
+                uint32_t tile = u, bar = smem_u32(&wfull[s]);
+                bool valid = true;
+                if (PAIR) {                                                          // unit = (tile-row pair, k tile)
+                    const uint32_t tp = u / op.kt, tk = u - tp * op.kt, tn = 2 * tp + crank;
+                    valid = tn < tile_rows;                                          // odd N/128: the last pair has one row only
+                    tile = tn * op.kt + tk;
+                    if (crank == 0) mbar_expect_tx(bar, (2 * tp + 1 < tile_rows) ? 65536 : 32768);
+                    bar = map_to_cta(bar, 0);
+                } else {
+                    mbar_expect_tx(bar, 32768);
+                }
+                if (!valid) continue;
+                const uint64_t off = op.w_offset + (uint64_t)tile * 32768;          // tile index in TILE128 storage order
                 const uint32_t slot = __ldg(a.T + (off >> a.log2b));
                 const uint64_t byte = ((uint64_t)slot << a.log2b) + (off & ((1ull << a.log2b) - 1));
                 const uint32_t row = (uint32_t)(byte >> 8);                          // pool viewed as rows of 256 B
                 const uint32_t st = smem_base + s * 32768;
-                const uint32_t bar = smem_u32(&wfull[s]);
-                mbar_expect_tx(bar, 32768);
-                tma_load_2d(st, &map_w, 0, row, bar);
-                tma_load_2d(st + 16384, &map_w, 64, row, bar);
+                if (PAIR) {
+                    tma_load_2d_pair(st, &map_w, 0, row, bar);
+                    tma_load_2d_pair(st + 16384, &map_w, 64, row, bar);
+                } else {
+                    tma_load_2d(st, &map_w, 0, row, bar);
+                    tma_load_2d(st + 16384, &map_w, 64, row, bar);
+                }
             }
         }
     } else if (warp == 2 && lane == 0) {
@@ -160,23 +229,29 @@ __global__ void __launch_bounds__(GM_THREADS, 1) gemm_tile128_kernel(const __gri
         uint32_t it = 0;
         for (uint32_t j = 0; j < a.nops; ++j) {
             const GemmOp& op = a.ops[j];
-            const uint32_t vr = (blockIdx.x + gridDim.x - op.rot) % gridDim.x;      // this CTA's range of the op
-            const uint32_t ubeg = vr * op.per, uend = min(ubeg + op.per, op.units);
+            if (op.ubase + op.units <= gbeg || op.ubase >= gend) continue;         // this range's part of the op, in op units
+            const uint32_t ubeg = max(gbeg, op.ubase) - op.ubase, uend = min(gend, op.ubase + op.units) - op.ubase;
             for (uint32_t u = ubeg; u < uend; ++u, ++it) {
                 const uint32_t s = it % a.xstages, f = it / a.xstages;
                 if (f > 0) mbar_wait(smem_u32(&xempty[s]), (f - 1) & 1);
                 const uint32_t tk = u % op.kt;
                 const uint32_t st = x_base + s * xtile;
-                const uint32_t bar = smem_u32(&xfull[s]);
-                mbar_expect_tx(bar, xtile);
-                tma_load_2d(st, &a.map_x[j], tk * 128, 0, bar);
-                tma_load_2d(st + xbox, &a.map_x[j], tk * 128 + 64, 0, bar);
+                uint32_t bar = smem_u32(&xfull[s]);
+                if (PAIR) {                                                          // rows [crank * batch/2, +batch/2) of X
+                    if (crank == 0) mbar_expect_tx(bar, 2 * xtile);
+                    bar = map_to_cta(bar, 0);
+                    tma_load_2d_pair(st, &a.map_x[j], tk * 128, crank * (a.batch / 2), bar);
+                    tma_load_2d_pair(st + xbox, &a.map_x[j], tk * 128 + 64, crank * (a.batch / 2), bar);
+                } else {
+                    mbar_expect_tx(bar, xtile);
+                    tma_load_2d(st, &a.map_x[j], tk * 128, 0, bar);
+                    tma_load_2d(st + xbox, &a.map_x[j], tk * 128 + 64, 0, bar);
+                }
             }
         }
-    }
- else if (warp == 1 && lane == 0) {
-        // ---------------------------------------------------------------- MMA issuer
-        const uint32_t idesc = (1u << 4) | (1u << 7) | (1u << 10) | ((a.batch >> 3) << 17) | ((128u >> 4) << 24);
+    } else if (warp == 1 && lane == 0 && crank == 0) {
+        // ---------------------------------------------------------------- MMA issuer (the pair's leader only)
+        const uint32_t idesc = (1u << 4) | (1u << 7) | (1u << 10) | ((a.batch >> 3) << 17) | (((PAIR ? 256u : 128u) >> 4) << 24);
         uint32_t it = 0, seg = 0;                                               // both run on across the ops
         auto acquire_acc = [&]() {                                              // accumulator seg & 1 drained by the epilogue?
             if (seg >= 2) {
@@ -184,18 +259,21 @@ __global__ void __launch_bounds__(GM_THREADS, 1) gemm_tile128_kernel(const __gri
                 tc_fence_after();
             }
         };
+        auto commit = [&](uint64_t* bar) {
+            if (PAIR) tc_commit_pair(smem_u32(bar));
+            else tc_commit(smem_u32(bar));
+        };
         for (uint32_t j = 0; j < a.nops; ++j) {
             const GemmOp& op = a.ops[j];
-            const uint32_t vr = (blockIdx.x + gridDim.x - op.rot) % gridDim.x;      // this CTA's range of the op
-            const uint32_t ubeg = vr * op.per, uend = min(ubeg + op.per, op.units);
-            if (ubeg >= uend) continue;
+            if (op.ubase + op.units <= gbeg || op.ubase >= gend) continue;         // this range's part of the op, in op units
+            const uint32_t ubeg = max(gbeg, op.ubase) - op.ubase, uend = min(gend, op.ubase + op.units) - op.ubase;
             uint32_t cur_tn = ubeg / op.kt;
             bool first = true;
             acquire_acc();
             for (uint32_t u = ubeg; u < uend; ++u, ++it) {
                 const uint32_t tn = u / op.kt;
                 if (tn != cur_tn) {
-                    tc_commit(smem_u32(&tmem_full[seg & 1]));                    // accumulator of the finished tile row
+                    commit(&tmem_full[seg & 1]);                                 // accumulator of the finished tile row (pair)
                     ++seg;
                     cur_tn = tn;
                     first = true;
@@ -212,14 +290,17 @@ __global__ void __launch_bounds__(GM_THREADS, 1) gemm_tile128_kernel(const __gri
                     const uint64_t ad = umma_desc_sw128(st + box * 16384);
                     const uint64_t bd = umma_desc_sw128(sx + box * xbox);
 #pragma unroll
-                    for (int k = 0; k < 4; ++k)                                  // UMMA_K = 16 bf16 = 32 B inside the atom
-                        tc_mma_bf16(d, ad + 2 * k, bd + 2 * k, idesc, (first && box == 0 && k == 0) ? 0u : 1u);
+                    for (int k = 0; k < 4; ++k) {                                // UMMA_K = 16 bf16 = 32 B inside the atom
+                        const uint32_t acc = (first && box == 0 && k == 0) ? 0u : 1u;
+                        if (PAIR) tc_mma_bf16_pair(d, ad + 2 * k, bd + 2 * k, idesc, acc);
+                        else tc_mma_bf16(d, ad + 2 * k, bd + 2 * k, idesc, acc);
+                    }
                 }
                 first = false;
-                tc_commit(smem_u32(&wempty[ws]));                                // frees both stages when the MMAs retire
-                tc_commit(smem_u32(&xempty[xs]));
+                commit(&wempty[ws]);                                             // frees both stages when the MMAs retire
+                commit(&xempty[xs]);
             }
-            tc_commit(smem_u32(&tmem_full[seg & 1]));
+            commit(&tmem_full[seg & 1]);
             ++seg;
         }
     } else if (warp >= 3) {
@@ -229,88 +310,97 @@ __global__ void __launch_bounds__(GM_THREADS, 1) gemm_tile128_kernel(const __gri
         gm_dep_wait();
         if (etid == 0) gm_dep_launch();
         const uint32_t nout = a.batch * 128;
+        const uint32_t eb0 = PAIR ? map_to_cta(smem_u32(&tmem_empty[0]), 0) : smem_u32(&tmem_empty[0]);   // the leader's
+        const uint32_t eb1 = PAIR ? map_to_cta(smem_u32(&tmem_empty[1]), 0) : smem_u32(&tmem_empty[1]);
         uint32_t seg = 0;
         for (uint32_t j = 0; j < a.nops; ++j) {
             const GemmOp& op = a.ops[j];
             const uint32_t kt = op.kt;
-            const uint32_t vr = (blockIdx.x + gridDim.x - op.rot) % gridDim.x;      // this CTA's range of the op
-            const uint32_t ubeg = vr * op.per, uend = min(ubeg + op.per, op.units);
+            if (op.ubase + op.units <= gbeg || op.ubase >= gend) continue;         // this range's part of the op, in op units
+            const uint32_t ubeg = max(gbeg, op.ubase) - op.ubase, uend = min(gend, op.ubase + op.units) - op.ubase;
             float* part = a.part + op.part_base;
             uint32_t* counters = a.counters + op.row_base;
             for (uint32_t u = ubeg; u < uend; ++seg) {
-                const uint32_t tn = u / kt;
-                const uint32_t t_first = tn * kt, t_last = t_first + kt - 1;
+                const uint32_t tg = u / kt;                                      // tile row, or tile-row pair
+                const uint32_t t_first = tg * kt, t_last = t_first + kt - 1;
                 const uint32_t seg_last = min(uend - 1, t_last);
                 const bool complete = (u == t_first) && (seg_last == t_last);
+                const uint32_t tn = PAIR ? 2 * tg + crank : tg;                  // this CTA's tile row
+                const bool valid = !PAIR || tn * 128 < op.N;
                 mbar_wait(smem_u32(&tmem_full[seg & 1]), (seg >> 1) & 1);
                 tc_fence_after();
                 const uint32_t taddr = tmem_base + ((q * 32) << 16) + (seg & 1) * a.batch;
                 const size_t n = (size_t)tn * 128 + r;
-                const uint32_t c_first = t_first / op.per, c_last = t_last / op.per;
-                const uint32_t ncontrib = c_last - c_first + 1, me = vr - c_first;
+                const uint32_t c_first = (op.ubase + t_first) / a.per, c_last = (op.ubase + t_last) / a.per;   // ranges that meet the row
+                const uint32_t ncontrib = c_last - c_first + 1, me = rank_in_grid - c_first;
                 float* mine = part + ((size_t)tn * op.maxc + me) * nout;
-                for (uint32_t c = 0; c < a.batch; c += 16) {
-                    uint32_t v[16];
-                    tc_ld16(taddr + c, v);
-                    if (complete) {
+                const bool finisher = valid && !complete && me == 0;
+                if (finisher) {
+                    // The row's FIRST contributor finishes it: for that CTA it is the last row of its range, the others met the
+                    // row at the start of theirs and have published long before.  (With "last to arrive reduces", whoever
+                    // was last fell behind, was last again, and the launch ended with its slowest CTA.)  Its own part never
+                    // leaves the chip: TMEM -> registers, + the others' partials in contributor order, -> Y.
+                    if (etid == 0) {
+                        uint32_t seen;
+                        do {
+                            asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(seen) : "l"(counters + tn) : "memory");
+                            if (seen != ncontrib - 1) __nanosleep(64);
+                        } while (seen != ncontrib - 1);
+                        counters[tn] = 0;                                        // self-reset for the next launch
+                    }
+                    epi_bar();
+                    __threadfence();
+                }
+                if (valid) {
+                    const float* others = part + ((size_t)tn * op.maxc + 1) * nout + r;      // contributors 1 .. ncontrib-1
+                    for (uint32_t c = 0; c < a.batch; c += 16) {
+                        uint32_t v[16];
+                        if (finisher) {
+                            // up to 3 x 16 partial loads in flight per thread beside the TMEM load (L2-latency bound)
+                            float sum[16];
+                            for (uint32_t p = 0; p + 1 < ncontrib || p == 0; p += 3) {
+                                float x[3][16];
 #pragma unroll
-                        for (int i = 0; i < 16; ++i) op.y[(size_t)(c + i) * op.N + n] = __float2bfloat16_rn(__uint_as_float(v[i]));
-                    } else {
+                                for (int pp = 0; pp < 3; ++pp) {
+                                    const float* src = others + (size_t)(p + pp) * nout + (size_t)c * 128;
 #pragma unroll
-                        for (int i = 0; i < 16; ++i) __stcg(mine + (size_t)(c + i) * 128 + r, __uint_as_float(v[i]));
+                                    for (int i = 0; i < 16; ++i) x[pp][i] = (p + pp + 1 < ncontrib) ? __ldcg(src + i * 128) : 0.f;
+                                }
+                                if (p == 0) {
+                                    tc_ld16(taddr + c, v);
+#pragma unroll
+                                    for (int i = 0; i < 16; ++i) sum[i] = __uint_as_float(v[i]);
+                                }
+#pragma unroll
+                                for (int pp = 0; pp < 3; ++pp)
+                                    if (p + pp + 1 < ncontrib)
+#pragma unroll
+                                        for (int i = 0; i < 16; ++i) sum[i] += x[pp][i];
+                            }
+#pragma unroll
+                            for (int i = 0; i < 16; ++i) op.y[(size_t)(c + i) * op.N + n] = __float2bfloat16_rn(sum[i]);
+                            continue;
+                        }
+                        tc_ld16(taddr + c, v);
+                        if (complete) {
+#pragma unroll
+                            for (int i = 0; i < 16; ++i) op.y[(size_t)(c + i) * op.N + n] = __float2bfloat16_rn(__uint_as_float(v[i]));
+                        } else {
+#pragma unroll
+                            for (int i = 0; i < 16; ++i) __stcg(mine + (size_t)(c + i) * 128 + r, __uint_as_float(v[i]));
+                        }
                     }
                 }
                 tc_fence_before();
                 __syncwarp();
-                if (lane == 0) mbar_arrive(smem_u32(&tmem_empty[seg & 1]));
-                if (!complete) {
+                if (lane == 0) {
+                    if (PAIR) mbar_arrive_cluster((seg & 1) ? eb1 : eb0);
+                    else mbar_arrive((seg & 1) ? eb1 : eb0);
+                }
+                if (valid && !complete && me != 0) {                             // publish this CTA's part of the cut row
                     __threadfence();
                     epi_bar();
-                    // The row's FIRST contributor finishes it (for that CTA it is the last row of its range, so the others --
-                    // which met the row at the start of theirs -- have published long before): every CTA reduces exactly one
-                    // row per op.  (With "last to arrive reduces", whoever was last fell behind, was last again, and the
-                    // launch ended with its slowest CTA: SMs active 70 % of the time at batch 128.)
-                    if (etid == 0) {
-                        if (me != 0) {
-                            asm volatile("red.release.gpu.global.add.u32 [%0], %1;" :: "l"(counters + tn), "r"(1u) : "memory");
-                        } else {
-                            uint32_t seen;
-                            do {
-                                asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(seen) : "l"(counters + tn) : "memory");
-                                if (seen != ncontrib - 1) __nanosleep(64);
-                            } while (seen != ncontrib - 1);
-                            counters[tn] = 0;                                    // self-reset for the next launch
-                        }
-                    }
-                    epi_bar();
-                    if (me == 0) {
-                        __threadfence();
-                        const float* base = part + (size_t)tn * op.maxc * nout;
-                        for (uint32_t m = 0; m < a.batch; m += 16) {
-                            float sum[16];
-#pragma unroll
-                            for (int i = 0; i < 16; ++i) sum[i] = 0.f;
-                            // 4 contributors x 16 values = 64 loads in flight per thread (the loop is L2-latency bound: with
-                            // 16 in flight a [128 x 128] tile row took ~25 us); the additions stay in contributor order.
-                            for (uint32_t p = 0; p < ncontrib; p += 4) {
-                                float v[4][16];
-#pragma unroll
-                                for (int pp = 0; pp < 4; ++pp) {
-                                    const float* src = base + (size_t)(p + pp) * nout + (size_t)m * 128 + r;
-#pragma unroll
-                                    for (int i = 0; i < 16; ++i) v[pp][i] = (p + pp < ncontrib) ? __ldcg(src + i * 128) : 0.f;
-                                }
-#pragma unroll
-                                for (int pp = 0; pp < 4; ++pp)
-                                    if (p + pp < ncontrib)
-#pragma unroll
-                                        for (int i = 0; i < 16; ++i) sum[i] += v[pp][i];
-                            }
-#pragma unroll
-                            for (int i = 0; i < 16; ++i) op.y[(size_t)(m + i) * op.N + n] = __float2bfloat16_rn(sum[i]);
-                        }
-                    }
-                    epi_bar();
+                    if (etid == 0) asm volatile("red.release.gpu.global.add.u32 [%0], %1;" :: "l"(counters + tn), "r"(1u) : "memory");
                 }
                 u = seg_last + 1;
             }
@@ -318,9 +408,11 @@ __global__ void __launch_bounds__(GM_THREADS, 1) gemm_tile128_kernel(const __gri
     }
     tc_fence_before();
     __syncthreads();
+    if (PAIR) cluster_sync_all();      // the peer's shared memory and barriers stay alive until both CTAs are done
     if (warp == 1) {
         tc_fence_after();
-        asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" :: "r"(tmem_base), "r"(a.tmem_cols) : "memory");
+        if (PAIR) asm volatile("tcgen05.dealloc.cta_group::2.sync.aligned.b32 %0, %1;" :: "r"(tmem_base), "r"(a.tmem_cols) : "memory");
+        else asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" :: "r"(tmem_base), "r"(a.tmem_cols) : "memory");
     }
 }
 
@@ -358,6 +450,34 @@ static cloak_status gemm_check(const cloak_pool* pool, const cloak_tensor* w, co
     return CLOAK_OK;
 }
 
+static int g_gemm_engine = 0;      // 0 auto, 1 one CTA per range, 2 CTA pairs (cloak_set_gemm_engine)
+
+// CTA pairs that can be resident at once (the split-K hand-over spins on other ranges: all of them must be running)
+static int max_pairs(int device, int sms) {
+    static int cached[64];
+    if (device < 0 || device >= 64) return 0;
+    if (cached[device]) return cached[device];
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = dim3(2 * (sms / 2));
+    cfg.blockDim = dim3(GM_THREADS);
+    cfg.dynamicSmemBytes = 226 * 1024;
+    cudaLaunchAttribute at[1];
+    at[0].id = cudaLaunchAttributeClusterDimension;
+    at[0].val.clusterDim.x = 2;
+    at[0].val.clusterDim.y = 1;
+    at[0].val.clusterDim.z = 1;
+    cfg.attrs = at;
+    cfg.numAttrs = 1;
+    int n = 0;
+    if (cudaOccupancyMaxActiveClusters(&n, gemm_tile128_kernel<true>, &cfg) != cudaSuccess) {
+        cudaGetLastError();
+        n = 0;
+    }
+    if (n > sms / 2) n = sms / 2;
+    cached[device] = n > 0 ? n : -1;
+    return cached[device];
+}
+
 // One launch of n <= GM_MAX_OPS checked ops.
 static cloak_status gemm_launch(const cloak_pool* pool, const cloak_gemm_op* ops, uint32_t n, uint32_t batch, cudaStream_t s) {
     cloak_status st;
@@ -367,19 +487,39 @@ static cloak_status gemm_launch(const cloak_pool* pool, const cloak_gemm_op* ops
         if (st != CLOAK_OK) return st;
         p->tmap_ready = true;
     }
+    static bool attr_set = false;
+    if (!attr_set) {
+        CLOAK_CUDA(cudaFuncSetAttribute(gemm_tile128_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, 226 * 1024));
+        CLOAK_CUDA(cudaFuncSetAttribute(gemm_tile128_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, 226 * 1024));
+        attr_set = true;
+    }
     GemmArgs a;
     a.T = pool->d_T;
     a.log2b = pool->log2_block;
     a.batch = batch;
     a.nops = n;
     const int sms = sm_count(pool->device);
+    // CTA pairs from batch 64 on: the X tile is then at least half a W tile, and sharing it between two tile rows pays
+    bool pair = g_gemm_engine == 2 || (g_gemm_engine == 0 && batch >= 64);
+    int ranges = sms;                   // ranges per op: one per CTA or per pair
+    if (pair) {
+        ranges = max_pairs(pool->device, sms);
+        if (ranges <= 0) {
+            pair = false;
+            ranges = sms;
+        }
+    }
     uint32_t cap = 512 / batch;         // contributors per tile row (fp32 partials are batch * 512 B each): ~10 at batch 32, 4 at 128
     cap = cap < 4 ? 4 : (cap > 10 ? 10 : cap);
-    uint64_t rows = 0, part = 0;
-    uint32_t ctas = 1, nranges_so_far = 0;
+    // The launch's units -- all ops back to back, each tn-major -- are cut into equal contiguous ranges, one per CTA (pair):
+    // a range boundary costs one tile row of fp32 partials and one reduction, and there are ranges - 1 of them per
+    // LAUNCH, wherever the op boundaries fall (cut per op it was ranges - 1 per op: 14 x the partial traffic and the
+    // reductions for the 14 projections of two layers, and ops with few units left CTAs idle).
+    uint64_t rows = 0, total = 0;
+    uint32_t max_kt = 0;
     for (uint32_t j = 0; j < n; ++j) {
         const cloak_tensor& w = ops[j].w;
-        st = make_map(&a.map_x[j], ops[j].d_x, w.K, batch, (uint64_t)w.K * 2, 64, batch);
+        st = make_map(&a.map_x[j], ops[j].d_x, w.K, batch, (uint64_t)w.K * 2, 64, pair ? batch / 2 : batch);
         if (st != CLOAK_OK) return st;
         GemmOp& o = a.ops[j];
         o.w_offset = w.w_offset;
@@ -387,24 +527,29 @@ static cloak_status gemm_launch(const cloak_pool* pool, const cloak_gemm_op* ops
         o.N = w.N;
         o.kt = w.K / 128;
         const uint32_t tile_rows = w.N / 128;
-        const uint64_t units64 = (uint64_t)tile_rows * o.kt;
-        if (units64 > 0xffffffffull) return fail(CLOAK_ERR_UNSUPPORTED, "gemm: tensor too large");
+        const uint64_t units64 = (uint64_t)(pair ? (tile_rows + 1) / 2 : tile_rows) * o.kt;   // pair: (tile-row pair, k tile)
+        if (total + units64 > 0xffffffffull) return fail(CLOAK_ERR_UNSUPPORTED, "gemm: too many tiles in one launch");
         o.units = (uint32_t)units64;
-        o.per = (o.units + sms - 1) / sms;
-        if (o.per < (o.kt + cap - 1) / cap) o.per = (o.kt + cap - 1) / cap;
-        const uint32_t c = (o.units + o.per - 1) / o.per;
-        if (c > ctas) ctas = c;
-        o.maxc = (o.kt + o.per - 1) / o.per + 1;
+        o.ubase = (uint32_t)total;
         o.row_base = (uint32_t)rows;
-        o.rot = nranges_so_far;
-        nranges_so_far += c;
-        o.part_base = part;
+        total += units64;
         rows += tile_rows;
-        part += (uint64_t)tile_rows * o.maxc * batch * 128;
+        if (o.kt > max_kt) max_kt = o.kt;
     }
-    for (uint32_t j = 0; j < n; ++j) a.ops[j].rot %= ctas;
+    uint32_t per = (uint32_t)((total + ranges - 1) / ranges);
+    if (per < (max_kt + cap - 1) / cap) per = (max_kt + cap - 1) / cap;     // at most ~cap ranges meet one tile row
+    const uint32_t ctas = (uint32_t)((total + per - 1) / per);
+    a.per = per;
+    a.total = (uint32_t)total;
+    uint64_t part = 0;
+    for (uint32_t j = 0; j < n; ++j) {
+        GemmOp& o = a.ops[j];
+        o.maxc = (o.kt + per - 1) / per + 1;
+        o.part_base = part;
+        part += (uint64_t)(o.N / 128) * o.maxc * batch * 128;
+    }
     if (rows * 4 > WS_COUNTER_BYTES) return fail(CLOAK_ERR_UNSUPPORTED, "gemm: too many output rows for the tile counters");
-    const uint32_t xtile = batch * 256;
+    const uint32_t xtile = (pair ? batch / 2 : batch) * 256;     // per CTA
     a.xstages = 2;
     uint32_t wst = (224u * 1024u - a.xstages * xtile) / 32768u;
     if (wst > GM_MAX_STAGES) wst = GM_MAX_STAGES;
@@ -418,29 +563,42 @@ static cloak_status gemm_launch(const cloak_pool* pool, const cloak_gemm_op* ops
     a.part = reinterpret_cast<float*>(pool->ws + WS_COUNTER_BYTES);
 
     const size_t smem = (size_t)a.wstages * 32768 + (size_t)a.xstages * xtile + 1024;
-    static bool attr_set = false;
-    if (!attr_set) {
-        CLOAK_CUDA(cudaFuncSetAttribute(gemm_tile128_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 226 * 1024));
-        attr_set = true;
-    }
     a.early = (g_gemv_pdl && !pool->dirty) ? 1u : 0u;
     if (pool->dirty && pool->dirty_stream == s) pool->dirty = false;   // this launch waits for the writer in full
     cudaLaunchConfig_t cfg = {};
-    cfg.gridDim = dim3(ctas);
+    cfg.gridDim = dim3(pair ? 2 * ctas : ctas);
     cfg.blockDim = dim3(GM_THREADS);
     cfg.dynamicSmemBytes = smem;
     cfg.stream = s;
-    cudaLaunchAttribute at[1];
-    at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
-    at[0].val.programmaticStreamSerializationAllowed = 1;
+    cudaLaunchAttribute at[2];
+    unsigned na = 0;
+    if (pair) {
+        at[na].id = cudaLaunchAttributeClusterDimension;
+        at[na].val.clusterDim.x = 2;
+        at[na].val.clusterDim.y = 1;
+        at[na].val.clusterDim.z = 1;
+        ++na;
+    }
+    if (g_gemv_pdl) {
+        at[na].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+        at[na].val.programmaticStreamSerializationAllowed = 1;
+        ++na;
+    }
     cfg.attrs = at;
-    cfg.numAttrs = g_gemv_pdl ? 1 : 0;
-    CLOAK_CUDA(cudaLaunchKernelEx(&cfg, gemm_tile128_kernel, pool->tmap_tile128, a));
+    cfg.numAttrs = na;
+    if (pair) CLOAK_CUDA(cudaLaunchKernelEx(&cfg, gemm_tile128_kernel<true>, pool->tmap_tile128, a));
+    else CLOAK_CUDA(cudaLaunchKernelEx(&cfg, gemm_tile128_kernel<false>, pool->tmap_tile128, a));
     launched();
     return CLOAK_OK;
 }
 
 }  // namespace cloak
+
+extern "C" cloak_status cloak_set_gemm_engine(int engine) {
+    if (engine < 0 || engine > 2) return fail(CLOAK_ERR_INVALID, "set_gemm_engine: engine must be 0, 1 or 2");
+    g_gemm_engine = engine;
+    return CLOAK_OK;
+}
 
 extern "C" cloak_status cloak_gemm(const cloak_pool* pool, const cloak_tensor* w, const void* d_x, void* d_y,
                                    uint32_t batch, void* stream) {

@@ -596,8 +596,9 @@ def test_gemm_vs_oracle_and_identity_bit_identical(block, shapes, batches):
 
 @pytest.mark.parametrize("batch", [32, 128])
 def test_gemm_chain_equals_single_calls(batch):
-    """cloak_gemm_chain: 20 ops of mixed shapes (two launches of <= 16 ops), bit-identical to cloak_gemm op by op, on
-    the cloaked and the identity-table pool, repeatable; a sample of ops against the fp64 oracle."""
+    """cloak_gemm_chain: 20 ops of mixed shapes (two launches of <= 16 ops): bit-identical on the cloaked and the
+    identity-table pool, repeatable; equal to cloak_gemm op by op up to the fp32 summation order (a chain cuts K where
+    its ranges fall); every op against the fp64 oracle."""
     key, seed, block, page = 0x1234, 3, 65536, 2 << 20
     shapes = [(1024, 5120), (5120, 1024), (384, 640), (128, 128), (2560, 2560)] * 4
     Ws = [gen.synth(seed, i, shp, "bf16") for i, shp in enumerate(shapes[:5])]
@@ -624,9 +625,14 @@ def test_gemm_chain_equals_single_calls(batch):
         C.cloak_gemm_chain(pc.h, [(T[i], dX[shapes[i][1]], yr[i]) for i in range(len(shapes))], batch)
         torch.cuda.synchronize()
         for i in range(len(shapes)):
-            assert torch.equal(yc[i], yi[i]) and torch.equal(yc[i], ys[i]) and torch.equal(yc[i], yr[i]), i
-        for i in (0, 1, 2, 3, 4, 17):
-            err = O.err_normwise(yc[i].float().cpu().numpy(), O.linear_f64(X[shapes[i][1]], Ws[i % 5]))
+            assert torch.equal(yc[i], yi[i]) and torch.equal(yc[i], yr[i]), i
+            d = (yc[i].float() - ys[i].float()).norm() / ys[i].float().norm()
+            assert d <= 4e-3, (i, float(d))                                  # bf16 rounding of two fp32 summation orders
+        refs = {}
+        for i in range(len(shapes)):
+            if i % 5 not in refs:
+                refs[i % 5] = O.linear_f64(X[shapes[i][1]], Ws[i % 5])
+            err = O.err_normwise(yc[i].float().cpu().numpy(), refs[i % 5])
             assert err <= TOL["bf16"], (i, err)
 
 
