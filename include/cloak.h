@@ -265,9 +265,9 @@ cloak_status cloak_gemv_chain(const cloak_pool* pool, const cloak_gemv_op* h_ops
                               void* stream);
 /* A list of INDEPENDENT GEMMs over one pool in one persistent launch (per 16 ops): Y_i = X_i W_i^T as in cloak_gemm;
  * every op has its own output and no op may read what another op of the list writes.  The tiles of all ops of a launch
- * form ONE sequence that is cut into equal ranges, one per CTA: K is split where those boundaries fall, so a chain is
- * deterministic and the same on cloaked and identity-table pools, and equals cloak_gemm up to the fp32 summation
- * order.  The weight stream runs on across op boundaries
+ * form ONE sequence that is cut into chunks (cloak_set_gemm_schedule): K is split where those boundaries fall, so a
+ * chain is deterministic and the same on cloaked and identity-table pools, and equals cloak_gemm up to the fp32
+ * summation order.  The weight stream runs on across op boundaries
  * (BASELINE.json configs[3]: "cloaked decode GEMM" of every projection of the model).  h_ops is a HOST array, not
  * referenced after the call returns.  Asynchronous on `stream`. */
 typedef struct {
@@ -281,10 +281,12 @@ cloak_status cloak_gemm_chain(const cloak_pool* pool, const cloak_gemm_op* h_ops
  * programmatic dependent launch), 1 = always the one-shot split-K kernel, 2 = automatic without
  * programmatic dependent launch.  For A/B measurement; process-wide. */
 cloak_status cloak_set_gemv_engine(int engine);
-/* Selects the tcgen05 GEMM kernel: 0 = automatic (CTA pairs, `cta_group::2`, from batch 64 on), 1 = one CTA per
- * range at every batch, 2 = CTA pairs at every batch.  The variants split K at different points, so their outputs
- * agree within the bf16 tolerance, not bit for bit.  For A/B measurement; process-wide. */
-cloak_status cloak_set_gemm_engine(int engine);
+/* Schedule of the tcgen05 GEMM: the first `static_pct` percent of a launch's tiles (up to a tile-row boundary) are dealt
+ * out in equal shares, one per CTA; the tile rows after that are drawn from a counter as CTAs become free, whole or -- rows
+ * of more than `dyn_chunk_tiles` k tiles (0 = by batch) -- in equal pieces.  The chunk grid decides where K is split, so
+ * outputs under different settings agree within the bf16 tolerance, not bit for bit; under one setting they do not depend
+ * on which CTA drew which chunk.  Default (75, 0).  For A/B measurement; process-wide. */
+cloak_status cloak_set_gemm_schedule(int static_pct, int dyn_chunk_tiles);
 /* Host-buffer variant of cloak_gemv (end-to-end path): copies X up, runs, copies Y back, synchronises. */
 cloak_status cloak_gemv_host(const cloak_pool* pool, const cloak_tensor* w, const void* h_x, void* h_y,
                              uint32_t batch, void* stream);

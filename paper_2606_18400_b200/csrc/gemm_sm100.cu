@@ -11,18 +11,23 @@
 //     SWIZZLE_128B, which land in shared memory in the canonical K-major UMMA layout (8-row atoms of 1 KiB).
 //   * A operand = the W tile (M = 128 output features), B operand = X[batch, 64] boxes of a second map over X
 //     (N = batch), D = 128 lanes x batch fp32 columns in TMEM, two accumulator buffers.
-//   * Units = tiles, numbered tn-major (= TILE128 storage order), the ops of a launch back to back, cut into equal
-//     contiguous ranges, one per persistent CTA (stream-K over the whole op list): HBM-bound (AI = batch flop/B < ridge), so what matters is that every SM
-//     streams the same bytes with a full TMA ring.  Roles: warp 0 TMA producer, warp 1 MMA issuer (one lane)
-//     + TMEM allocator, warp 2 TMA producer for X (own shallow ring), warps 3-6 epilogue (tcgen05.ld 32x32b, one TMEM lane quarter each).
-//   * A tile row wholly inside a CTA's range is stored as bf16 straight from TMEM; one cut by a range boundary
-//     has its later contributors write fp32 partials; the row's first contributor adds them, in contributor order, to
-//     its own accumulator as it drains it (deterministic; identical for cloaked and identity-table pools).
-//   * PAIR variant (batch >= 64 by default): the grid is launched as clusters of two CTAs (one TPC) that work as a
-//     `cta_group::2` pair on TWO adjacent tile rows with the same k tile: each CTA streams its own W tile and only HALF
-//     of the X tile (batch/2 rows), the leader issues one M = 256 MMA that reads B from both CTAs' shared memory, and
-//     each CTA drains its own 128 TMEM lanes.  Units are then (tile-row pair, k tile), one range per pair.  At batch
-//     128 the X tile is as large as the W tile, so this takes the L2 -> SM traffic from 2 x W to 1.5 x W.
+//   * Units = tiles, numbered tn-major (= TILE128 storage order), the ops of a launch back to back: ONE sequence per
+//     launch, cut into CHUNKS.  The kernel is HBM-bound (AI = batch flop/B < ridge), so what matters is that every SM
+//     streams with a full TMA ring until the last byte of the launch has arrived -- and the SMs do not stream equally
+//     fast (with equal shares the fastest SM finished at 70 % of the launch, the mean at 81 %: ncu,
+//     profiles/r1_ncu_full_gemm_b32.md).  So a CTA first takes a static chunk (a share of ~3/4 of the equal split), then
+//     pulls small chunks from the rest of the sequence off an atomic counter until it is empty.
+//   * Roles: warp 0 = scheduler + TMA producer for W (one lane), warp 1 = MMA issuer (one lane) + TMEM allocator,
+//     warp 2 = TMA producer for X (own shallow ring), warps 3-6 = epilogue (tcgen05.ld 32x32b, one TMEM lane quarter
+//     each).  The scheduler hands every chunk to the other roles through a small shared-memory queue.
+//   * A tile row wholly inside a chunk is stored as bf16 straight from TMEM.  A row cut by chunk boundaries has
+//     contributors: each takes a ticket; all but the holder of the last ticket write fp32 partials, the last one adds
+//     them to its own accumulator IN CHUNK ORDER as it drains it.  The chunk grid is fixed by the shapes, only the
+//     assignment of chunks to CTAs varies, so the result does not depend on the schedule (deterministic; identical for
+//     cloaked and identity-table pools).
+//   * Measured and dropped: a `cta_group::2` CTA-pair variant (M = 256 over two tile rows, each CTA loading half of
+//     X: L2 -> SM traffic 2 x W -> 1.5 x W at batch 128) ran correctly and no faster (1.53 vs 1.51 ms for 8 layers of
+//     cfg3): the X traffic is not what bounds batch 128.
 #include <cuda_bf16.h>
 #include "common.cuh"
 #include "async.cuh"
@@ -34,23 +39,31 @@ constexpr int GM_MAX_OPS = 16;             // ops per launch (one X tensor map o
 struct GemmOp {
     uint64_t w_offset;
     __nv_bfloat16* y;
-    uint64_t part_base;  // float offset of this op's partials: [tile row][maxc][batch][128]
     uint32_t N;
     uint32_t kt;         // k tiles per tile row = K/128
-    uint32_t units;      // (N/128) * kt; pair variant: ceil(N/256) * kt
+    uint32_t units;      // (N/128) * kt
     uint32_t ubase;      // this op's first unit in the launch's unit sequence (ops back to back)
-    uint32_t maxc;       // max contributors per tile row
-    uint32_t row_base;   // index of this op's first tile-row counter
+    uint32_t row_base;   // index of this op's first tile row among the launch's tile rows (tickets, ready counters)
+    uint32_t dyn_row0;   // first tile row of this op in the dynamic part (N/128 if none)
+    uint32_t pieces;     // dynamic part: chunks per tile row, each plen tiles (the last one the rest)
+    uint32_t plen;
+    uint32_t cbase;      // dynamic part: number of the chunk (dyn_row0, piece 0)
+    uint32_t pad_;
 };
 
 struct GemmArgs {
     const uint32_t* T;
-    float* part;
-    uint32_t* counters;
+    float* part;         // fp32 partials: [chunk][2][batch/4][128][4]: slot 0 = the row that ENDS in the chunk, 1 = any other cut row
+    uint32_t* ticket;    // per tile row of the launch: contributors that have claimed their turn
+    uint32_t* ready;     // per tile row: partials published
+    uint32_t* sched;     // [0] next dynamic chunk, [1] CTAs done (the last one resets both)
     uint32_t log2b;
     uint32_t batch;
     uint32_t nops;
-    uint32_t per;        // units per range: the launch's units (all ops back to back) are cut into equal contiguous ranges
+    uint32_t sper;       // static part [0, dyn_base): CTA b starts with its b-th equal share, sper or sper + 1 units
+    uint32_t srem;       // ... the first srem shares have sper + 1
+    uint32_t dyn_base;   // first unit of the dynamic part (a tile-row boundary)
+    uint32_t ndyn;       // chunks of the dynamic part: whole tile rows, or equal pieces of a row that is longer than the cap
     uint32_t total;      // units of the launch
     uint32_t wstages;    // ring of 32 KiB weight tiles (HBM latency: deep)
     uint32_t xstages;    // ring of X tiles [batch x 128] (L2 latency: shallow)
@@ -60,53 +73,19 @@ struct GemmArgs {
     alignas(64) CUtensorMap map_x[GM_MAX_OPS];   // X of op j as a 2-D map [batch, K], boxes of [batch x 64]
 };
 
-constexpr int GM_THREADS = 224;            // warp 0 TMA (W), warp 1 MMA, warp 2 TMA (X), warps 3..6 epilogue
+constexpr int GM_THREADS = 224;            // warp 0 scheduler + TMA (W), warp 1 MMA, warp 2 TMA (X), warps 3..6 epilogue
 constexpr int GM_MAX_STAGES = 6;
+constexpr int GM_QUEUE = 8;                // chunks the scheduler may run ahead of the slowest role
+constexpr uint32_t GM_END = 0xffffffffu;
 
 __device__ __forceinline__ void tma_load_2d(uint32_t dst, const CUtensorMap* map, uint32_t c0, uint32_t c1, uint32_t bar) {
     asm volatile("cp.async.bulk.tensor.2d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3}], [%4];"
                  :: "r"(dst), "l"(map), "r"(c0), "r"(c1), "r"(bar) : "memory");
 }
-// cta_group::2 flavour: executed by both CTAs of the pair, the data lands in the issuing CTA's shared memory, the bytes
-// are counted on the LEADER's barrier (`bar` is a shared::cluster address).
-__device__ __forceinline__ void tma_load_2d_pair(uint32_t dst, const CUtensorMap* map, uint32_t c0, uint32_t c1, uint32_t bar) {
-    asm volatile("cp.async.bulk.tensor.2d.cta_group::2.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3}], [%4];"
-                 :: "r"(dst), "l"(map), "r"(c0), "r"(c1), "r"(bar) : "memory");
-}
-__device__ __forceinline__ uint32_t cluster_ctarank() {
-    uint32_t r;
-    asm volatile("mov.u32 %0, %%cluster_ctarank;" : "=r"(r));
-    return r;
-}
-// shared::cluster address of the same shared-memory offset in CTA `rank` of the cluster
-__device__ __forceinline__ uint32_t map_to_cta(uint32_t smem_addr, uint32_t rank) {
-    uint32_t r;
-    asm volatile("mapa.shared::cluster.u32 %0, %1, %2;" : "=r"(r) : "r"(smem_addr), "r"(rank));
-    return r;
-}
-__device__ __forceinline__ void mbar_arrive_cluster(uint32_t cluster_bar) {
-    asm volatile("mbarrier.arrive.release.cluster.shared::cluster.b64 _, [%0];" :: "r"(cluster_bar) : "memory");
-}
-__device__ __forceinline__ void cluster_sync_all() {
-    asm volatile("barrier.cluster.arrive.release;" ::: "memory");
-    asm volatile("barrier.cluster.wait.acquire;" ::: "memory");
-}
 __device__ __forceinline__ void tc_fence_after() { asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory"); }
 __device__ __forceinline__ void tc_fence_before() { asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory"); }
 __device__ __forceinline__ void tc_commit(uint32_t bar) {
     asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];" :: "r"(bar) : "memory");
-}
-// Pair flavours: the arrival goes to the barrier at this offset in BOTH CTAs; the MMA spans both CTAs' tensor cores.
-__device__ __forceinline__ void tc_commit_pair(uint32_t bar) {
-    asm volatile("tcgen05.commit.cta_group::2.mbarrier::arrive::one.shared::cluster.multicast::cluster.b64 [%0], %1;"
-                 :: "r"(bar), "h"((uint16_t)3) : "memory");
-}
-__device__ __forceinline__ void tc_mma_bf16_pair(uint32_t d_tmem, uint64_t adesc, uint64_t bdesc, uint32_t idesc, uint32_t acc) {
-    asm volatile(
-        "{\n\t.reg .pred p;\n\t"
-        "setp.ne.b32 p, %4, 0;\n\t"
-        "tcgen05.mma.cta_group::2.kind::f16 [%0], %1, %2, %3, p;\n\t}"
-        :: "r"(d_tmem), "l"(adesc), "l"(bdesc), "r"(idesc), "r"(acc) : "memory");
 }
 __device__ __forceinline__ void tc_mma_bf16(uint32_t d_tmem, uint64_t adesc, uint64_t bdesc, uint32_t idesc, uint32_t acc) {
     asm volatile(
@@ -132,24 +111,27 @@ __device__ __forceinline__ void gm_dep_wait() { asm volatile("griddepcontrol.wai
 __device__ __forceinline__ void gm_dep_launch() { asm volatile("griddepcontrol.launch_dependents;" ::: "memory"); }
 __device__ __forceinline__ void epi_bar() { asm volatile("bar.sync 1, 128;" ::: "memory"); }
 
-// A launch runs a list of independent ops (cloak_gemm_chain; cloak_gemm is a list of one): every role walks the list,
-// the rings, the accumulator double buffer and their phases simply continue from op to op, so the weight stream does not
+// Static part: first unit of share b, and the share that holds unit g.
+__device__ __forceinline__ uint32_t static_begin(const GemmArgs& a, uint32_t b) { return b * a.sper + min(b, a.srem); }
+__device__ __forceinline__ uint32_t static_chunk_of(const GemmArgs& a, uint32_t g) {
+    const uint32_t big = a.srem * (a.sper + 1);
+    return g < big ? g / (a.sper + 1) : a.srem + (g - big) / a.sper;
+}
+
+// A launch runs a list of independent ops (cloak_gemm_chain; cloak_gemm is a list of one): the rings, the accumulator
+// double buffer and their phases simply continue from chunk to chunk and from op to op, so the weight stream does not
 // stop at an op boundary (per-launch head and tail cost ~4 us each; q, k, v, o of a Qwen-32B layer are 13 % of the bytes
 // and were 35 % of the time as separate launches).
-template <bool PAIR>
 __global__ void __launch_bounds__(GM_THREADS, 1) gemm_tile128_kernel(const __grid_constant__ CUtensorMap map_w,
                                                                      const __grid_constant__ GemmArgs a) {
     extern __shared__ __align__(1024) unsigned char smem_raw[];
     __shared__ __align__(8) uint64_t wfull[GM_MAX_STAGES], wempty[GM_MAX_STAGES], xfull[GM_MAX_STAGES], xempty[GM_MAX_STAGES],
-        tmem_full[2], tmem_empty[2];
-    __shared__ uint32_t tmem_base_s;
+        tmem_full[2], tmem_empty[2], qfull[GM_QUEUE], qempty[GM_QUEUE];
+    __shared__ uint4 queue[GM_QUEUE];                        // {chunk index, first unit, end unit, -}; chunk index GM_END = stop
+    __shared__ uint32_t tmem_base_s, last_s;
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     // dynamic shared memory is only guaranteed 16-byte aligned: round up to the 1 KiB the 128-byte swizzle needs
-    // (same offset in both CTAs of a pair: same kernel, same static shared memory)
     const uint32_t smem_base = (smem_u32(smem_raw) + 1023u) & ~1023u;
-    const uint32_t crank = PAIR ? cluster_ctarank() : 0u;             // 0 = leader (issues the MMAs, owns the full barriers)
-    const uint32_t rank_in_grid = PAIR ? blockIdx.x / 2 : blockIdx.x;  // one range per CTA, or per CTA pair
-    const uint32_t gbeg = rank_in_grid * a.per, gend = min(gbeg + a.per, a.total);
 
     if (threadIdx.x == 0) {
         for (uint32_t s = 0; s < GM_MAX_STAGES; ++s) {
@@ -160,148 +142,167 @@ __global__ void __launch_bounds__(GM_THREADS, 1) gemm_tile128_kernel(const __gri
         }
         for (int i = 0; i < 2; ++i) {
             mbar_init(smem_u32(&tmem_full[i]), 1);
-            mbar_init(smem_u32(&tmem_empty[i]), PAIR ? 8 : 4);        // the epilogue warps of both CTAs arrive at the leader's
+            mbar_init(smem_u32(&tmem_empty[i]), 4);
+        }
+        for (int i = 0; i < GM_QUEUE; ++i) {
+            mbar_init(smem_u32(&qfull[i]), 1);
+            mbar_init(smem_u32(&qempty[i]), 6);              // X producer, MMA issuer, 4 epilogue warps
         }
         fence_barrier_init();
     }
     if (warp == 1) {
-        if (PAIR) {
-            asm volatile("tcgen05.alloc.cta_group::2.sync.aligned.shared::cta.b32 [%0], %1;"
-                         :: "r"(smem_u32(&tmem_base_s)), "r"(a.tmem_cols) : "memory");
-            asm volatile("tcgen05.relinquish_alloc_permit.cta_group::2.sync.aligned;" ::: "memory");
-        } else {
-            asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;"
-                         :: "r"(smem_u32(&tmem_base_s)), "r"(a.tmem_cols) : "memory");
-            asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
-        }
+        asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;"
+                     :: "r"(smem_u32(&tmem_base_s)), "r"(a.tmem_cols) : "memory");
+        asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
     }
     tc_fence_before();
     __syncthreads();
-    if (PAIR) cluster_sync_all();                                     // the peer's barriers are initialised before anything lands
     tc_fence_after();
     const uint32_t tmem_base = tmem_base_s;
 
-    const uint32_t xbox = (PAIR ? a.batch / 2 : a.batch) * 128;      // bytes of this CTA's X box [rows x 64 bf16]
+    const uint32_t xbox = a.batch * 128;                     // bytes of one X box [batch x 64 bf16]
     const uint32_t xtile = 2 * xbox;
     const uint32_t x_base = smem_base + a.wstages * 32768;
 
+    // Every role but the scheduler: next chunk from the queue (false = the launch's sequence is exhausted).
+    uint32_t qi = 0;
+    auto next_chunk = [&](uint32_t& cidx, uint32_t& gbeg, uint32_t& gend, bool one_lane) -> bool {
+        const uint32_t s = qi % GM_QUEUE;
+        mbar_wait(smem_u32(&qfull[s]), (qi / GM_QUEUE) & 1);
+        const uint4 c = queue[s];
+        if (!one_lane) __syncwarp();
+        if (one_lane || lane == 0) mbar_arrive(smem_u32(&qempty[s]));
+        ++qi;
+        cidx = c.x;
+        gbeg = c.y;
+        gend = c.z;
+        return c.x != GM_END;
+    };
+
     if (warp == 0 && lane == 0) {
-        // ---------------------------------------------------------------- TMA producer, weight tiles (through T)
+        // ---------------------------------------------------------------- scheduler + TMA producer, weight tiles (through T)
         if (!a.early) gm_dep_wait();
-        uint32_t it = 0;
-        for (uint32_t j = 0; j < a.nops; ++j) {
-            const GemmOp& op = a.ops[j];
-            if (op.ubase + op.units <= gbeg || op.ubase >= gend) continue;         // this range's part of the op, in op units
-            const uint32_t ubeg = max(gbeg, op.ubase) - op.ubase, uend = min(gend, op.ubase + op.units) - op.ubase;
-            const uint32_t tile_rows = op.N / 128;
-            for (uint32_t u = ubeg; u < uend; ++u, ++it) {
-                const uint32_t s = it % a.wstages, f = it / a.wstages;
-                if (f > 0) mbar_wait(smem_u32(&wempty[s]), (f - 1) & 1);
-                uint32_t tile = u, bar = smem_u32(&wfull[s]);
-                bool valid = true;
-                if (PAIR) {                                                          // unit = (tile-row pair, k tile)
-                    const uint32_t tp = u / op.kt, tk = u - tp * op.kt, tn = 2 * tp + crank;
-                    valid = tn < tile_rows;                                          // odd N/128: the last pair has one row only
-                    tile = tn * op.kt + tk;
-                    if (crank == 0) mbar_expect_tx(bar, (2 * tp + 1 < tile_rows) ? 65536 : 32768);
-                    bar = map_to_cta(bar, 0);
-                } else {
+        uint32_t it = 0, qp = 0;
+        auto push = [&](uint32_t cidx, uint32_t gbeg, uint32_t gend) {
+            const uint32_t s = qp % GM_QUEUE;
+            if (qp >= GM_QUEUE) mbar_wait(smem_u32(&qempty[s]), (qp / GM_QUEUE - 1) & 1);
+            queue[s] = make_uint4(cidx, gbeg, gend, 0u);
+            mbar_arrive(smem_u32(&qfull[s]));                                        // release: the entry is visible to the waiters
+            ++qp;
+        };
+        auto stream = [&](uint32_t gbeg, uint32_t gend) {
+            for (uint32_t j = 0; j < a.nops; ++j) {
+                const GemmOp& op = a.ops[j];
+                if (op.ubase + op.units <= gbeg || op.ubase >= gend) continue;     // this chunk's part of the op, in op units
+                const uint32_t ubeg = max(gbeg, op.ubase) - op.ubase, uend = min(gend, op.ubase + op.units) - op.ubase;
+                for (uint32_t u = ubeg; u < uend; ++u, ++it) {
+                    const uint32_t s = it % a.wstages, f = it / a.wstages;
+                    if (f > 0) mbar_wait(smem_u32(&wempty[s]), (f - 1) & 1);
+                    const uint64_t off = op.w_offset + (uint64_t)u * 32768;          // tile index == unit index
+                    const uint32_t slot = __ldg(a.T + (off >> a.log2b));
+                    const uint64_t byte = ((uint64_t)slot << a.log2b) + (off & ((1ull << a.log2b) - 1));
+                    const uint32_t row = (uint32_t)(byte >> 8);                      // pool viewed as rows of 256 B
+                    const uint32_t st = smem_base + s * 32768;
+                    const uint32_t bar = smem_u32(&wfull[s]);
                     mbar_expect_tx(bar, 32768);
-                }
-                if (!valid) continue;
-                const uint64_t off = op.w_offset + (uint64_t)tile * 32768;          // tile index in TILE128 storage order
-                const uint32_t slot = __ldg(a.T + (off >> a.log2b));
-                const uint64_t byte = ((uint64_t)slot << a.log2b) + (off & ((1ull << a.log2b) - 1));
-                const uint32_t row = (uint32_t)(byte >> 8);                          // pool viewed as rows of 256 B
-                const uint32_t st = smem_base + s * 32768;
-                if (PAIR) {
-                    tma_load_2d_pair(st, &map_w, 0, row, bar);
-                    tma_load_2d_pair(st + 16384, &map_w, 64, row, bar);
-                } else {
                     tma_load_2d(st, &map_w, 0, row, bar);
                     tma_load_2d(st + 16384, &map_w, 64, row, bar);
                 }
             }
+        };
+        const uint32_t sbeg = static_begin(a, blockIdx.x), send = static_begin(a, blockIdx.x + 1);
+        if (send > sbeg) {                                                           // (a tiny launch has no static part)
+            push(blockIdx.x, sbeg, send);
+            stream(sbeg, send);
+        }
+        if (a.early) gm_dep_wait();                                                  // the scheduler's counter is the predecessor's too
+        uint32_t k = atomicAdd(a.sched, 1u);
+        while (k < a.ndyn) {
+            uint32_t j = 0;                                                          // the op whose dynamic chunks hold number k
+            while (j + 1 < a.nops && a.ops[j + 1].cbase <= k) ++j;
+            const GemmOp& op = a.ops[j];
+            const uint32_t loc = k - op.cbase, tn = op.dyn_row0 + loc / op.pieces, pc = loc % op.pieces;
+            const uint32_t gbeg = op.ubase + tn * op.kt + pc * op.plen, gend = op.ubase + tn * op.kt + min((pc + 1) * op.plen, op.kt);
+            push(gridDim.x + k, gbeg, gend);
+            k = atomicAdd(a.sched, 1u);                                              // in flight while this chunk is issued
+            stream(gbeg, gend);
+        }
+        push(GM_END, GM_END, GM_END);
+        __threadfence();
+        if (atomicAdd(a.sched + 1, 1u) == gridDim.x - 1) {                           // every CTA has drawn its last chunk: reset
+            __threadfence();
+            a.sched[0] = 0;
+            a.sched[1] = 0;
         }
     } else if (warp == 2 && lane == 0) {
         // ---------------------------------------------------------------- TMA producer, activation tiles (L2-resident)
         gm_dep_wait();
-        uint32_t it = 0;
-        for (uint32_t j = 0; j < a.nops; ++j) {
-            const GemmOp& op = a.ops[j];
-            if (op.ubase + op.units <= gbeg || op.ubase >= gend) continue;         // this range's part of the op, in op units
-            const uint32_t ubeg = max(gbeg, op.ubase) - op.ubase, uend = min(gend, op.ubase + op.units) - op.ubase;
-            for (uint32_t u = ubeg; u < uend; ++u, ++it) {
-                const uint32_t s = it % a.xstages, f = it / a.xstages;
-                if (f > 0) mbar_wait(smem_u32(&xempty[s]), (f - 1) & 1);
-                const uint32_t tk = u % op.kt;
-                const uint32_t st = x_base + s * xtile;
-                uint32_t bar = smem_u32(&xfull[s]);
-                if (PAIR) {                                                          // rows [crank * batch/2, +batch/2) of X
-                    if (crank == 0) mbar_expect_tx(bar, 2 * xtile);
-                    bar = map_to_cta(bar, 0);
-                    tma_load_2d_pair(st, &a.map_x[j], tk * 128, crank * (a.batch / 2), bar);
-                    tma_load_2d_pair(st + xbox, &a.map_x[j], tk * 128 + 64, crank * (a.batch / 2), bar);
-                } else {
+        uint32_t it = 0, cidx, gbeg, gend;
+        while (next_chunk(cidx, gbeg, gend, true)) {
+            for (uint32_t j = 0; j < a.nops; ++j) {
+                const GemmOp& op = a.ops[j];
+                if (op.ubase + op.units <= gbeg || op.ubase >= gend) continue;
+                const uint32_t ubeg = max(gbeg, op.ubase) - op.ubase, uend = min(gend, op.ubase + op.units) - op.ubase;
+                for (uint32_t u = ubeg; u < uend; ++u, ++it) {
+                    const uint32_t s = it % a.xstages, f = it / a.xstages;
+                    if (f > 0) mbar_wait(smem_u32(&xempty[s]), (f - 1) & 1);
+                    const uint32_t tk = u % op.kt;
+                    const uint32_t st = x_base + s * xtile;
+                    const uint32_t bar = smem_u32(&xfull[s]);
                     mbar_expect_tx(bar, xtile);
                     tma_load_2d(st, &a.map_x[j], tk * 128, 0, bar);
                     tma_load_2d(st + xbox, &a.map_x[j], tk * 128 + 64, 0, bar);
                 }
             }
         }
-    } else if (warp == 1 && lane == 0 && crank == 0) {
-        // ---------------------------------------------------------------- MMA issuer (the pair's leader only)
-        const uint32_t idesc = (1u << 4) | (1u << 7) | (1u << 10) | ((a.batch >> 3) << 17) | (((PAIR ? 256u : 128u) >> 4) << 24);
-        uint32_t it = 0, seg = 0;                                               // both run on across the ops
+    } else if (warp == 1 && lane == 0) {
+        // ---------------------------------------------------------------- MMA issuer
+        const uint32_t idesc = (1u << 4) | (1u << 7) | (1u << 10) | ((a.batch >> 3) << 17) | ((128u >> 4) << 24);
+        uint32_t it = 0, seg = 0, cidx, gbeg, gend;                             // it, seg run on across chunks and ops
         auto acquire_acc = [&]() {                                              // accumulator seg & 1 drained by the epilogue?
             if (seg >= 2) {
                 mbar_wait(smem_u32(&tmem_empty[seg & 1]), ((seg >> 1) - 1) & 1);
                 tc_fence_after();
             }
         };
-        auto commit = [&](uint64_t* bar) {
-            if (PAIR) tc_commit_pair(smem_u32(bar));
-            else tc_commit(smem_u32(bar));
-        };
-        for (uint32_t j = 0; j < a.nops; ++j) {
-            const GemmOp& op = a.ops[j];
-            if (op.ubase + op.units <= gbeg || op.ubase >= gend) continue;         // this range's part of the op, in op units
-            const uint32_t ubeg = max(gbeg, op.ubase) - op.ubase, uend = min(gend, op.ubase + op.units) - op.ubase;
-            uint32_t cur_tn = ubeg / op.kt;
-            bool first = true;
-            acquire_acc();
-            for (uint32_t u = ubeg; u < uend; ++u, ++it) {
-                const uint32_t tn = u / op.kt;
-                if (tn != cur_tn) {
-                    commit(&tmem_full[seg & 1]);                                 // accumulator of the finished tile row (pair)
-                    ++seg;
-                    cur_tn = tn;
-                    first = true;
-                    acquire_acc();
-                }
-                const uint32_t ws = it % a.wstages, xs = it % a.xstages;
-                mbar_wait(smem_u32(&xfull[xs]), (it / a.xstages) & 1);
-                mbar_wait(smem_u32(&wfull[ws]), (it / a.wstages) & 1);
-                tc_fence_after();
-                const uint32_t st = smem_base + ws * 32768, sx = x_base + xs * xtile;
-                const uint32_t d = tmem_base + (seg & 1) * a.batch;
-#pragma unroll
-                for (int box = 0; box < 2; ++box) {
-                    const uint64_t ad = umma_desc_sw128(st + box * 16384);
-                    const uint64_t bd = umma_desc_sw128(sx + box * xbox);
-#pragma unroll
-                    for (int k = 0; k < 4; ++k) {                                // UMMA_K = 16 bf16 = 32 B inside the atom
-                        const uint32_t acc = (first && box == 0 && k == 0) ? 0u : 1u;
-                        if (PAIR) tc_mma_bf16_pair(d, ad + 2 * k, bd + 2 * k, idesc, acc);
-                        else tc_mma_bf16(d, ad + 2 * k, bd + 2 * k, idesc, acc);
+        while (next_chunk(cidx, gbeg, gend, true)) {
+            for (uint32_t j = 0; j < a.nops; ++j) {
+                const GemmOp& op = a.ops[j];
+                if (op.ubase + op.units <= gbeg || op.ubase >= gend) continue;
+                const uint32_t ubeg = max(gbeg, op.ubase) - op.ubase, uend = min(gend, op.ubase + op.units) - op.ubase;
+                uint32_t cur_tn = ubeg / op.kt;
+                bool first = true;
+                acquire_acc();
+                for (uint32_t u = ubeg; u < uend; ++u, ++it) {
+                    const uint32_t tn = u / op.kt;
+                    if (tn != cur_tn) {
+                        tc_commit(smem_u32(&tmem_full[seg & 1]));                // accumulator of the finished tile row
+                        ++seg;
+                        cur_tn = tn;
+                        first = true;
+                        acquire_acc();
                     }
+                    const uint32_t ws = it % a.wstages, xs = it % a.xstages;
+                    mbar_wait(smem_u32(&xfull[xs]), (it / a.xstages) & 1);
+                    mbar_wait(smem_u32(&wfull[ws]), (it / a.wstages) & 1);
+                    tc_fence_after();
+                    const uint32_t st = smem_base + ws * 32768, sx = x_base + xs * xtile;
+                    const uint32_t d = tmem_base + (seg & 1) * a.batch;
+#pragma unroll
+                    for (int box = 0; box < 2; ++box) {
+                        const uint64_t ad = umma_desc_sw128(st + box * 16384);
+                        const uint64_t bd = umma_desc_sw128(sx + box * xbox);
+#pragma unroll
+                        for (int k = 0; k < 4; ++k)                              // UMMA_K = 16 bf16 = 32 B inside the atom
+                            tc_mma_bf16(d, ad + 2 * k, bd + 2 * k, idesc, (first && box == 0 && k == 0) ? 0u : 1u);
+                    }
+                    first = false;
+                    tc_commit(smem_u32(&wempty[ws]));                            // frees both stages when the MMAs retire
+                    tc_commit(smem_u32(&xempty[xs]));
                 }
-                first = false;
-                commit(&wempty[ws]);                                             // frees both stages when the MMAs retire
-                commit(&xempty[xs]);
+                tc_commit(smem_u32(&tmem_full[seg & 1]));
+                ++seg;
             }
-            commit(&tmem_full[seg & 1]);
-            ++seg;
         }
     } else if (warp >= 3) {
         // ---------------------------------------------------------------- epilogue (4 warps = 4 TMEM lane quarters)
@@ -310,109 +311,138 @@ __global__ void __launch_bounds__(GM_THREADS, 1) gemm_tile128_kernel(const __gri
         gm_dep_wait();
         if (etid == 0) gm_dep_launch();
         const uint32_t nout = a.batch * 128;
-        const uint32_t eb0 = PAIR ? map_to_cta(smem_u32(&tmem_empty[0]), 0) : smem_u32(&tmem_empty[0]);   // the leader's
-        const uint32_t eb1 = PAIR ? map_to_cta(smem_u32(&tmem_empty[1]), 0) : smem_u32(&tmem_empty[1]);
-        uint32_t seg = 0;
-        for (uint32_t j = 0; j < a.nops; ++j) {
-            const GemmOp& op = a.ops[j];
-            const uint32_t kt = op.kt;
-            if (op.ubase + op.units <= gbeg || op.ubase >= gend) continue;         // this range's part of the op, in op units
-            const uint32_t ubeg = max(gbeg, op.ubase) - op.ubase, uend = min(gend, op.ubase + op.units) - op.ubase;
-            float* part = a.part + op.part_base;
-            uint32_t* counters = a.counters + op.row_base;
-            for (uint32_t u = ubeg; u < uend; ++seg) {
-                const uint32_t tg = u / kt;                                      // tile row, or tile-row pair
-                const uint32_t t_first = tg * kt, t_last = t_first + kt - 1;
-                const uint32_t seg_last = min(uend - 1, t_last);
-                const bool complete = (u == t_first) && (seg_last == t_last);
-                const uint32_t tn = PAIR ? 2 * tg + crank : tg;                  // this CTA's tile row
-                const bool valid = !PAIR || tn * 128 < op.N;
-                mbar_wait(smem_u32(&tmem_full[seg & 1]), (seg >> 1) & 1);
-                tc_fence_after();
-                const uint32_t taddr = tmem_base + ((q * 32) << 16) + (seg & 1) * a.batch;
-                const size_t n = (size_t)tn * 128 + r;
-                const uint32_t c_first = (op.ubase + t_first) / a.per, c_last = (op.ubase + t_last) / a.per;   // ranges that meet the row
-                const uint32_t ncontrib = c_last - c_first + 1, me = rank_in_grid - c_first;
-                float* mine = part + ((size_t)tn * op.maxc + me) * nout;
-                const bool finisher = valid && !complete && me == 0;
-                if (finisher) {
-                    // The row's FIRST contributor finishes it: for that CTA it is the last row of its range, the others met the
-                    // row at the start of theirs and have published long before.  (With "last to arrive reduces", whoever
-                    // was last fell behind, was last again, and the launch ended with its slowest CTA.)  Its own part never
-                    // leaves the chip: TMEM -> registers, + the others' partials in contributor order, -> Y.
-                    if (etid == 0) {
-                        uint32_t seen;
-                        do {
-                            asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(seen) : "l"(counters + tn) : "memory");
-                            if (seen != ncontrib - 1) __nanosleep(64);
-                        } while (seen != ncontrib - 1);
-                        counters[tn] = 0;                                        // self-reset for the next launch
+        uint32_t seg = 0, cidx, gbeg, gend;
+        while (next_chunk(cidx, gbeg, gend, false)) {
+            for (uint32_t j = 0; j < a.nops; ++j) {
+                const GemmOp& op = a.ops[j];
+                if (op.ubase + op.units <= gbeg || op.ubase >= gend) continue;
+                const uint32_t ubeg = max(gbeg, op.ubase) - op.ubase, uend = min(gend, op.ubase + op.units) - op.ubase;
+                const uint32_t kt = op.kt;
+                for (uint32_t u = ubeg; u < uend; ++seg) {
+                    const uint32_t tn = u / kt;
+                    const uint32_t t_first = tn * kt, t_last = t_first + kt - 1;
+                    const uint32_t seg_last = min(uend - 1, t_last);
+                    // the chunks that meet this tile row, in sequence order: its contributors
+                    uint32_t c_first, ncontrib;
+                    if (tn >= op.dyn_row0) {                                     // dynamic part: the row's pieces
+                        c_first = gridDim.x + op.cbase + (tn - op.dyn_row0) * op.pieces;
+                        ncontrib = op.pieces;
+                    } else {
+                        c_first = static_chunk_of(a, op.ubase + t_first);
+                        ncontrib = static_chunk_of(a, op.ubase + t_last) - c_first + 1;
                     }
-                    epi_bar();
-                    __threadfence();
-                }
-                if (valid) {
-                    const float* others = part + ((size_t)tn * op.maxc + 1) * nout + r;      // contributors 1 .. ncontrib-1
-                    for (uint32_t c = 0; c < a.batch; c += 16) {
-                        uint32_t v[16];
-                        if (finisher) {
-                            // up to 3 x 16 partial loads in flight per thread beside the TMEM load (L2-latency bound)
-                            float sum[16];
-                            for (uint32_t p = 0; p + 1 < ncontrib || p == 0; p += 3) {
-                                float x[3][16];
+                    const uint32_t me = cidx - c_first;
+                    const bool complete = ncontrib == 1;
+                    const uint32_t row = op.row_base + tn;
+                    bool last = false;
+                    if (!complete) {
+                        // Tickets: whoever draws the last one finishes the row.  With the static chunks that is the row's
+                        // first contributor (it meets the row at the END of its chunk, the next one at the start of its own);
+                        // in the dynamic part it is whoever comes last.
+                        if (etid == 0) last_s = (atomicAdd(a.ticket + row, 1u) == ncontrib - 1) ? 1u : 0u;
+                        epi_bar();
+                        last = last_s != 0;
+                    }
+                    mbar_wait(smem_u32(&tmem_full[seg & 1]), (seg >> 1) & 1);
+                    tc_fence_after();
+                    const uint32_t taddr = tmem_base + ((q * 32) << 16) + (seg & 1) * a.batch;
+                    const size_t n = (size_t)tn * 128 + r;
+                    if (last) {
+                        if (etid == 0) {
+                            uint32_t seen;
+                            do {
+                                asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(seen) : "l"(a.ready + row) : "memory");
+                                if (seen != ncontrib - 1) __nanosleep(64);
+                            } while (seen != ncontrib - 1);
+                            a.ticket[row] = 0;                                   // self-reset for the next launch
+                            a.ready[row] = 0;
+                        }
+                        epi_bar();
+                        __threadfence();
+                    }
+                    // partial of contributor p of this row: slot 0 of its chunk if the row ENDS there, else slot 1; a slot is
+                    // [batch/4][128 rows][4] fp32, so that a thread moves its row's values of 4 batch columns as one float4
+                    auto slot_of = [&](uint32_t p) {
+                        return reinterpret_cast<float4*>(a.part + ((size_t)(c_first + p) * 2 + (p == ncontrib - 1 ? 0 : 1)) * nout) + r;
+                    };
+                    float4* mine = slot_of(me);
+                    for (uint32_t c = 0; c < a.batch; c += 32) {                 // 32 batch columns per round (16 in a last odd one)
+                        const bool two = c + 16 < a.batch;
+                        uint32_t v0[16], v1[16];
+                        tc_ld16(taddr + c, v0);
+                        if (two) tc_ld16(taddr + c + 16, v1);
+                        if (last) {
+                            // own part from TMEM, the others' from L2, added in chunk order; 2 x 8 float4 loads in flight per thread
+                            float sum[32];
 #pragma unroll
-                                for (int pp = 0; pp < 3; ++pp) {
-                                    const float* src = others + (size_t)(p + pp) * nout + (size_t)c * 128;
+                            for (int i = 0; i < 32; ++i) sum[i] = 0.f;
+                            for (uint32_t p = 0; p < ncontrib; p += 2) {
+                                float4 x[2][8];
 #pragma unroll
-                                    for (int i = 0; i < 16; ++i) x[pp][i] = (p + pp + 1 < ncontrib) ? __ldcg(src + i * 128) : 0.f;
+                                for (int pp = 0; pp < 2; ++pp) {
+                                    const bool ld = p + pp < ncontrib && p + pp != me;
+                                    const float4* src = slot_of(ld ? p + pp : 0) + (size_t)(c / 4) * 128;
+#pragma unroll
+                                    for (int i = 0; i < 8; ++i)
+                                        x[pp][i] = (ld && (i < 4 || two)) ? __ldcg(src + i * 128) : make_float4(0.f, 0.f, 0.f, 0.f);
                                 }
-                                if (p == 0) {
-                                    tc_ld16(taddr + c, v);
 #pragma unroll
-                                    for (int i = 0; i < 16; ++i) sum[i] = __uint_as_float(v[i]);
+                                for (int pp = 0; pp < 2; ++pp) {
+                                    if (p + pp == me) {
+#pragma unroll
+                                        for (int i = 0; i < 16; ++i) {
+                                            sum[i] += __uint_as_float(v0[i]);
+                                            if (two) sum[16 + i] += __uint_as_float(v1[i]);
+                                        }
+                                    } else if (p + pp < ncontrib) {
+#pragma unroll
+                                        for (int i = 0; i < 8; ++i) {
+                                            sum[4 * i] += x[pp][i].x;
+                                            sum[4 * i + 1] += x[pp][i].y;
+                                            sum[4 * i + 2] += x[pp][i].z;
+                                            sum[4 * i + 3] += x[pp][i].w;
+                                        }
+                                    }
                                 }
-#pragma unroll
-                                for (int pp = 0; pp < 3; ++pp)
-                                    if (p + pp + 1 < ncontrib)
-#pragma unroll
-                                        for (int i = 0; i < 16; ++i) sum[i] += x[pp][i];
                             }
 #pragma unroll
-                            for (int i = 0; i < 16; ++i) op.y[(size_t)(c + i) * op.N + n] = __float2bfloat16_rn(sum[i]);
-                            continue;
-                        }
-                        tc_ld16(taddr + c, v);
-                        if (complete) {
+                            for (int i = 0; i < 32; ++i)
+                                if (i < 16 || two) op.y[(size_t)(c + i) * op.N + n] = __float2bfloat16_rn(sum[i]);
+                        } else if (complete) {
 #pragma unroll
-                            for (int i = 0; i < 16; ++i) op.y[(size_t)(c + i) * op.N + n] = __float2bfloat16_rn(__uint_as_float(v[i]));
+                            for (int i = 0; i < 16; ++i) {
+                                op.y[(size_t)(c + i) * op.N + n] = __float2bfloat16_rn(__uint_as_float(v0[i]));
+                                if (two) op.y[(size_t)(c + 16 + i) * op.N + n] = __float2bfloat16_rn(__uint_as_float(v1[i]));
+                            }
                         } else {
 #pragma unroll
-                            for (int i = 0; i < 16; ++i) __stcg(mine + (size_t)(c + i) * 128 + r, __uint_as_float(v[i]));
+                            for (int i = 0; i < 4; ++i) {
+                                __stcg(mine + (size_t)(c / 4 + i) * 128, make_float4(__uint_as_float(v0[4 * i]), __uint_as_float(v0[4 * i + 1]),
+                                                                                     __uint_as_float(v0[4 * i + 2]), __uint_as_float(v0[4 * i + 3])));
+                                if (two)
+                                    __stcg(mine + (size_t)(c / 4 + 4 + i) * 128, make_float4(__uint_as_float(v1[4 * i]), __uint_as_float(v1[4 * i + 1]),
+                                                                                             __uint_as_float(v1[4 * i + 2]), __uint_as_float(v1[4 * i + 3])));
+                            }
                         }
                     }
+                    tc_fence_before();
+                    __syncwarp();
+                    if (lane == 0) mbar_arrive(smem_u32(&tmem_empty[seg & 1]));
+                    if (!complete && !last) {                                    // publish this chunk's part of the cut row
+                        __threadfence();
+                        epi_bar();
+                        if (etid == 0) asm volatile("red.release.gpu.global.add.u32 [%0], %1;" :: "l"(a.ready + row), "r"(1u) : "memory");
+                    }
+                    u = seg_last + 1;
                 }
-                tc_fence_before();
-                __syncwarp();
-                if (lane == 0) {
-                    if (PAIR) mbar_arrive_cluster((seg & 1) ? eb1 : eb0);
-                    else mbar_arrive((seg & 1) ? eb1 : eb0);
-                }
-                if (valid && !complete && me != 0) {                             // publish this CTA's part of the cut row
-                    __threadfence();
-                    epi_bar();
-                    if (etid == 0) asm volatile("red.release.gpu.global.add.u32 [%0], %1;" :: "l"(counters + tn), "r"(1u) : "memory");
-                }
-                u = seg_last + 1;
             }
         }
     }
     tc_fence_before();
     __syncthreads();
-    if (PAIR) cluster_sync_all();      // the peer's shared memory and barriers stay alive until both CTAs are done
     if (warp == 1) {
         tc_fence_after();
-        if (PAIR) asm volatile("tcgen05.dealloc.cta_group::2.sync.aligned.b32 %0, %1;" :: "r"(tmem_base), "r"(a.tmem_cols) : "memory");
-        else asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" :: "r"(tmem_base), "r"(a.tmem_cols) : "memory");
+        asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" :: "r"(tmem_base), "r"(a.tmem_cols) : "memory");
     }
 }
 
@@ -433,12 +463,6 @@ static cloak_status make_map(CUtensorMap* map, const void* base, uint64_t inner,
 extern bool g_gemv_pdl;      // gemv_stream.cu: the PDL A/B switch (cloak_set_gemv_engine(2) turns it off)
 cloak_status check_linear(const cloak_pool* pool, const cloak_tensor* w, const void* x, void* y, const char* who);
 
-}  // namespace cloak
-
-using namespace cloak;
-
-namespace cloak {
-
 static cloak_status gemm_check(const cloak_pool* pool, const cloak_tensor* w, const void* d_x, void* d_y, uint32_t batch,
                                const char* who) {
     cloak_status st = check_linear(pool, w, d_x, d_y, who);
@@ -450,33 +474,12 @@ static cloak_status gemm_check(const cloak_pool* pool, const cloak_tensor* w, co
     return CLOAK_OK;
 }
 
-static int g_gemm_engine = 0;      // 0 auto, 1 one CTA per range, 2 CTA pairs (cloak_set_gemm_engine)
+// Schedule knobs (cloak_set_gemm_schedule): percentage of the launch's tiles that is dealt out statically, and the cap on
+// the tiles of a dynamic chunk (0 = by batch).
+static int g_static_pct = 75;
+static int g_dchunk = 0;
 
-// CTA pairs that can be resident at once (the split-K hand-over spins on other ranges: all of them must be running)
-static int max_pairs(int device, int sms) {
-    static int cached[64];
-    if (device < 0 || device >= 64) return 0;
-    if (cached[device]) return cached[device];
-    cudaLaunchConfig_t cfg = {};
-    cfg.gridDim = dim3(2 * (sms / 2));
-    cfg.blockDim = dim3(GM_THREADS);
-    cfg.dynamicSmemBytes = 226 * 1024;
-    cudaLaunchAttribute at[1];
-    at[0].id = cudaLaunchAttributeClusterDimension;
-    at[0].val.clusterDim.x = 2;
-    at[0].val.clusterDim.y = 1;
-    at[0].val.clusterDim.z = 1;
-    cfg.attrs = at;
-    cfg.numAttrs = 1;
-    int n = 0;
-    if (cudaOccupancyMaxActiveClusters(&n, gemm_tile128_kernel<true>, &cfg) != cudaSuccess) {
-        cudaGetLastError();
-        n = 0;
-    }
-    if (n > sms / 2) n = sms / 2;
-    cached[device] = n > 0 ? n : -1;
-    return cached[device];
-}
+constexpr uint32_t GM_MAX_ROWS = 100000;   // tile rows per launch: two counters each in the pool's counter scratch
 
 // One launch of n <= GM_MAX_OPS checked ops.
 static cloak_status gemm_launch(const cloak_pool* pool, const cloak_gemm_op* ops, uint32_t n, uint32_t batch, cudaStream_t s) {
@@ -487,69 +490,72 @@ static cloak_status gemm_launch(const cloak_pool* pool, const cloak_gemm_op* ops
         if (st != CLOAK_OK) return st;
         p->tmap_ready = true;
     }
-    static bool attr_set = false;
-    if (!attr_set) {
-        CLOAK_CUDA(cudaFuncSetAttribute(gemm_tile128_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, 226 * 1024));
-        CLOAK_CUDA(cudaFuncSetAttribute(gemm_tile128_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, 226 * 1024));
-        attr_set = true;
-    }
     GemmArgs a;
     a.T = pool->d_T;
     a.log2b = pool->log2_block;
     a.batch = batch;
     a.nops = n;
     const int sms = sm_count(pool->device);
-    // CTA pairs from batch 64 on: the X tile is then at least half a W tile, and sharing it between two tile rows pays
-    bool pair = g_gemm_engine == 2 || (g_gemm_engine == 0 && batch >= 64);
-    int ranges = sms;                   // ranges per op: one per CTA or per pair
-    if (pair) {
-        ranges = max_pairs(pool->device, sms);
-        if (ranges <= 0) {
-            pair = false;
-            ranges = sms;
-        }
-    }
-    uint32_t cap = 512 / batch;         // contributors per tile row (fp32 partials are batch * 512 B each): ~10 at batch 32, 4 at 128
-    cap = cap < 4 ? 4 : (cap > 10 ? 10 : cap);
-    // The launch's units -- all ops back to back, each tn-major -- are cut into equal contiguous ranges, one per CTA (pair):
-    // a range boundary costs one tile row of fp32 partials and one reduction, and there are ranges - 1 of them per
-    // LAUNCH, wherever the op boundaries fall (cut per op it was ranges - 1 per op: 14 x the partial traffic and the
-    // reductions for the 14 projections of two layers, and ops with few units left CTAs idle).
     uint64_t rows = 0, total = 0;
     uint32_t max_kt = 0;
     for (uint32_t j = 0; j < n; ++j) {
         const cloak_tensor& w = ops[j].w;
-        st = make_map(&a.map_x[j], ops[j].d_x, w.K, batch, (uint64_t)w.K * 2, 64, pair ? batch / 2 : batch);
+        if (w.K / 128 > max_kt) max_kt = w.K / 128;
+        st = make_map(&a.map_x[j], ops[j].d_x, w.K, batch, (uint64_t)w.K * 2, 64, batch);
         if (st != CLOAK_OK) return st;
         GemmOp& o = a.ops[j];
         o.w_offset = w.w_offset;
         o.y = static_cast<__nv_bfloat16*>(ops[j].d_y);
         o.N = w.N;
         o.kt = w.K / 128;
-        const uint32_t tile_rows = w.N / 128;
-        const uint64_t units64 = (uint64_t)(pair ? (tile_rows + 1) / 2 : tile_rows) * o.kt;   // pair: (tile-row pair, k tile)
-        if (total + units64 > 0xffffffffull) return fail(CLOAK_ERR_UNSUPPORTED, "gemm: too many tiles in one launch");
+        const uint64_t units64 = (uint64_t)(w.N / 128) * o.kt;
+        if (total + units64 > 0x7fffffffull) return fail(CLOAK_ERR_UNSUPPORTED, "gemm: too many tiles in one launch");
         o.units = (uint32_t)units64;
         o.ubase = (uint32_t)total;
         o.row_base = (uint32_t)rows;
+        o.pad_ = 0;
         total += units64;
-        rows += tile_rows;
-        if (o.kt > max_kt) max_kt = o.kt;
+        rows += w.N / 128;
     }
-    uint32_t per = (uint32_t)((total + ranges - 1) / ranges);
-    if (per < (max_kt + cap - 1) / cap) per = (max_kt + cap - 1) / cap;     // at most ~cap ranges meet one tile row
-    const uint32_t ctas = (uint32_t)((total + per - 1) / per);
-    a.per = per;
-    a.total = (uint32_t)total;
-    uint64_t part = 0;
+    if (rows > GM_MAX_ROWS) return fail(CLOAK_ERR_UNSUPPORTED, "gemm: too many output rows for the tile counters");
+    // The launch's tiles -- all ops back to back, each tn-major -- form one sequence.  Its first g_static_pct percent, up to a
+    // tile-row boundary, are the static part: CTA b takes the b-th equal share of it.  The rows after that are the dynamic
+    // part: whole tile rows (no split-K at all), or equal pieces of a row that is longer than the cap, drawn from a counter
+    // as the CTAs become free.  Every piece boundary costs one partial [batch x 128] fp32 and a share of a reduction, so the
+    // cap grows with the batch.
+    // At most ~cap chunks per tile row (the fp32 partials are batch * 512 B each): small launches use fewer CTAs.
+    uint32_t cap = 512 / batch;
+    cap = cap < 4 ? 4 : (cap > 10 ? 10 : cap);
+    const uint32_t minper = (max_kt + cap - 1) / cap;
+    uint64_t ctas64 = total / minper;
+    const uint32_t ctas = (uint32_t)(ctas64 < 1 ? 1 : (ctas64 > (uint64_t)sms ? (uint64_t)sms : ctas64));
+    uint32_t dmax = g_dchunk > 0 ? (uint32_t)g_dchunk : (batch >= 128 ? 40u : 20u);
+    if (dmax < minper) dmax = minper;
+    // A launch with less than a few dynamic chunks' worth of tiles per CTA is dealt out statically: its tail would be as
+    // long as a chunk, and there is little to balance.
+    const uint64_t target = (total / ctas < 4ull * dmax && g_dchunk == 0) ? total : total * (uint64_t)g_static_pct / 100;
+    uint32_t ndyn = 0;
+    a.dyn_base = (uint32_t)total;
     for (uint32_t j = 0; j < n; ++j) {
         GemmOp& o = a.ops[j];
-        o.maxc = (o.kt + per - 1) / per + 1;
-        o.part_base = part;
-        part += (uint64_t)(o.N / 128) * o.maxc * batch * 128;
+        const uint32_t tile_rows = o.N / 128;
+        if (o.ubase + (uint64_t)o.units <= target) o.dyn_row0 = tile_rows;                 // wholly static
+        else if (o.ubase >= target) o.dyn_row0 = 0;                                         // wholly dynamic
+        else o.dyn_row0 = (uint32_t)((target - o.ubase) / o.kt);                            // the boundary row: rounded down
+        if (o.dyn_row0 < tile_rows && a.dyn_base == (uint32_t)total) a.dyn_base = o.ubase + o.dyn_row0 * o.kt;
+        o.pieces = (o.kt + dmax - 1) / dmax;
+        o.plen = (o.kt + o.pieces - 1) / o.pieces;
+        o.pieces = (o.kt + o.plen - 1) / o.plen;                                            // no empty last piece
+        o.cbase = ndyn;
+        ndyn += (tile_rows - o.dyn_row0) * o.pieces;
     }
-    if (rows * 4 > WS_COUNTER_BYTES) return fail(CLOAK_ERR_UNSUPPORTED, "gemm: too many output rows for the tile counters");
-    const uint32_t xtile = (pair ? batch / 2 : batch) * 256;     // per CTA
+    a.sper = a.dyn_base / ctas;
+    a.srem = a.dyn_base % ctas;
+    a.ndyn = ndyn;
+    a.total = (uint32_t)total;
+    const uint64_t nchunks = (uint64_t)ctas + ndyn;
+    const uint64_t part_bytes = nchunks * 2 * batch * 128 * 4;
+    const uint32_t xtile = batch * 256;
     a.xstages = 2;
     uint32_t wst = (224u * 1024u - a.xstages * xtile) / 32768u;
     if (wst > GM_MAX_STAGES) wst = GM_MAX_STAGES;
@@ -557,46 +563,45 @@ static cloak_status gemm_launch(const cloak_pool* pool, const cloak_gemm_op* ops
     a.wstages = wst;
     a.tmem_cols = 32;
     while (a.tmem_cols < 2 * batch) a.tmem_cols <<= 1;
-    st = pool_workspace(pool, WS_COUNTER_BYTES + part * 4);
+    st = pool_workspace(pool, WS_COUNTER_BYTES + part_bytes);
     if (st != CLOAK_OK) return st;
-    a.counters = reinterpret_cast<uint32_t*>(pool->ws);
+    a.ticket = reinterpret_cast<uint32_t*>(pool->ws);
+    a.ready = a.ticket + rows;
+    a.sched = a.ready + rows;
     a.part = reinterpret_cast<float*>(pool->ws + WS_COUNTER_BYTES);
 
     const size_t smem = (size_t)a.wstages * 32768 + (size_t)a.xstages * xtile + 1024;
+    static bool attr_set = false;
+    if (!attr_set) {
+        CLOAK_CUDA(cudaFuncSetAttribute(gemm_tile128_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 226 * 1024));
+        attr_set = true;
+    }
     a.early = (g_gemv_pdl && !pool->dirty) ? 1u : 0u;
     if (pool->dirty && pool->dirty_stream == s) pool->dirty = false;   // this launch waits for the writer in full
     cudaLaunchConfig_t cfg = {};
-    cfg.gridDim = dim3(pair ? 2 * ctas : ctas);
+    cfg.gridDim = dim3(ctas);
     cfg.blockDim = dim3(GM_THREADS);
     cfg.dynamicSmemBytes = smem;
     cfg.stream = s;
-    cudaLaunchAttribute at[2];
-    unsigned na = 0;
-    if (pair) {
-        at[na].id = cudaLaunchAttributeClusterDimension;
-        at[na].val.clusterDim.x = 2;
-        at[na].val.clusterDim.y = 1;
-        at[na].val.clusterDim.z = 1;
-        ++na;
-    }
-    if (g_gemv_pdl) {
-        at[na].id = cudaLaunchAttributeProgrammaticStreamSerialization;
-        at[na].val.programmaticStreamSerializationAllowed = 1;
-        ++na;
-    }
+    cudaLaunchAttribute at[1];
+    at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    at[0].val.programmaticStreamSerializationAllowed = 1;
     cfg.attrs = at;
-    cfg.numAttrs = na;
-    if (pair) CLOAK_CUDA(cudaLaunchKernelEx(&cfg, gemm_tile128_kernel<true>, pool->tmap_tile128, a));
-    else CLOAK_CUDA(cudaLaunchKernelEx(&cfg, gemm_tile128_kernel<false>, pool->tmap_tile128, a));
+    cfg.numAttrs = g_gemv_pdl ? 1 : 0;
+    CLOAK_CUDA(cudaLaunchKernelEx(&cfg, gemm_tile128_kernel, pool->tmap_tile128, a));
     launched();
     return CLOAK_OK;
 }
 
 }  // namespace cloak
 
-extern "C" cloak_status cloak_set_gemm_engine(int engine) {
-    if (engine < 0 || engine > 2) return fail(CLOAK_ERR_INVALID, "set_gemm_engine: engine must be 0, 1 or 2");
-    g_gemm_engine = engine;
+using namespace cloak;
+
+extern "C" cloak_status cloak_set_gemm_schedule(int static_pct, int dyn_chunk_tiles) {
+    if (static_pct < 0 || static_pct > 100 || dyn_chunk_tiles < 0 || dyn_chunk_tiles > 4096)
+        return fail(CLOAK_ERR_INVALID, "set_gemm_schedule: static_pct in 0..100, dyn_chunk_tiles in 0..4096");
+    g_static_pct = static_pct;
+    g_dchunk = dyn_chunk_tiles;
     return CLOAK_OK;
 }
 
@@ -620,10 +625,10 @@ extern "C" cloak_status cloak_gemm_chain(const cloak_pool* pool, const cloak_gem
         if (st != CLOAK_OK) return st;
     }
     DeviceGuard g(pool->device);
-    for (uint32_t i = 0; i < n_ops;) {                      // at most GM_MAX_OPS ops and 2^18 tile rows per launch
+    for (uint32_t i = 0; i < n_ops;) {                      // at most GM_MAX_OPS ops and GM_MAX_ROWS tile rows per launch
         uint32_t n = 0;
         uint64_t rows = 0;
-        while (i + n < n_ops && n < (uint32_t)GM_MAX_OPS && rows + h_ops[i + n].w.N / 128 <= 200000) rows += h_ops[i + n++].w.N / 128;
+        while (i + n < n_ops && n < (uint32_t)GM_MAX_OPS && rows + h_ops[i + n].w.N / 128 <= GM_MAX_ROWS) rows += h_ops[i + n++].w.N / 128;
         if (n == 0) return fail(CLOAK_ERR_UNSUPPORTED, "gemm_chain: op %u has too many output rows", i);
         cloak_status st = gemm_launch(pool, h_ops + i, n, batch, (cudaStream_t)stream);
         if (st != CLOAK_OK) return st;
