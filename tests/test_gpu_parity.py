@@ -651,6 +651,49 @@ def test_gemm_argument_checks():
             assert ei.value.status == st
 
 
+@pytest.mark.parametrize("batch", [32, 128, 208])
+def test_gemm_schedules_agree(batch):
+    """cloak_set_gemm_schedule: the chunk grid (static share, dynamic chunk cap) decides where K is split.  Under every
+    setting -- all static, the default, nearly all dynamic with small pieces (many contributors per tile row) -- a chain
+    of 10 ops is repeatable bit for bit (which CTA draws which chunk varies from launch to launch), the same on the
+    cloaked and the identity-table pool, and within the bf16 tolerance of the fp64 oracle."""
+    key, seed, block, page = 0x1234, 3, 65536, 2 << 20
+    shapes = [(2560, 2560), (1024, 5120), (5120, 1024), (384, 640), (128, 128)] * 2
+    Ws = [gen.synth(seed, i, shp, "bf16") for i, shp in enumerate(shapes[:5])]
+    sizes = [2 * n * k for n, k in shapes]
+    offs, total = C.cloak_arena_plan(key, sizes, block)
+    try:
+        with Pool(total, block, page, key) as pc, Pool(total, block, page, key, C.CLOAK_POOL_IDENTITY) as pi:
+            for i, ((n, k), off) in enumerate(zip(shapes, offs)):
+                til = torch.empty(n * k, dtype=torch.bfloat16, device="cuda")
+                C.cloak_to_tile128(bf16_dev_from_bits(Ws[i % 5]), til, n, k, C.CLOAK_BF16)
+                for p in (pc, pi):
+                    C.cloak_shuffle(p.h, til, off, n * k * 2)
+            X = {k: gen.synth(seed + 100, k, (batch, k), "bf16", kind=gen.KIND_NORMAL) for k in {k for _, k in shapes}}
+            dX = {k: bf16_dev_from_bits(v) for k, v in X.items()}
+            T = [C.cloak_tensor(off, n, k, C.CLOAK_BF16, C.CLOAK_TILE128) for (n, k), off in zip(shapes, offs)]
+            refs = [O.linear_f64(X[k], Ws[i]) for i, (n, k) in enumerate(shapes[:5])]
+
+            def run(pool):
+                ys = [torch.zeros(batch, n, dtype=torch.bfloat16, device="cuda") for n, _ in shapes]
+                C.cloak_gemm_chain(pool.h, [(T[i], dX[shapes[i][1]], ys[i]) for i in range(len(shapes))], batch)
+                torch.cuda.synchronize()
+                return ys
+            for sched in ((100, 0), (75, 0), (10, 3), (0, 7), (50, 64)):
+                C.cloak_set_gemm_schedule(*sched)
+                a, b, c = run(pc), run(pc), run(pi)
+                for i in range(len(shapes)):
+                    assert torch.equal(a[i], b[i]) and torch.equal(a[i], c[i]), (sched, i)
+                    err = O.err_normwise(a[i].float().cpu().numpy(), refs[i % 5])
+                    assert err <= TOL["bf16"], (sched, i, err)
+    finally:
+        C.cloak_set_gemm_schedule(75, 0)
+    for bad in ((-1, 0), (101, 0), (75, -1), (75, 5000)):
+        with pytest.raises(C.CloakError) as ei:
+            C.cloak_set_gemm_schedule(*bad)
+        assert ei.value.status == C.CLOAK_ERR_INVALID
+
+
 # ------------------------------------------------------------------ errors
 def test_error_codes_on_device():
     with Pool(1 << 20, 4096, 65536, 1) as p:
