@@ -493,10 +493,15 @@ def main():
                     help="cfg1 (default) is the headline step; cfg2-4 are the other BASELINE.json configs "
                          "(paper_2606_18400_b200/workloads.py), each printing its own JSON line")
     ap.add_argument("--reps", type=int, default=10, help="repetitions per measurement for --workload cfg2-4")
+    ap.add_argument("--gemv-engine", type=int, default=0,
+                    help="A/B: cloak_set_gemv_engine (0 auto, 1 one-shot kernel, 2 no PDL)")
     args = ap.parse_args()
     if args.workload != "cfg1":
         from paper_2606_18400_b200 import workloads
-        return workloads.main([args.workload, "--reps", str(args.reps)])
+        return workloads.main([args.workload, "--reps", str(args.reps), "--gemv-engine", str(args.gemv_engine)])
+    if args.gemv_engine and args.impl == "cloak":
+        import paper_2606_18400_b200 as C
+        C.cloak_set_gemv_engine(args.gemv_engine)
     args.warmup = max(args.warmup, 3) if args.impl == "cloak" else args.warmup
     return run_reference(args) if args.impl == "reference" else run_cloak(args)
 

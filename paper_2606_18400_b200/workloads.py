@@ -539,8 +539,11 @@ def main(argv=None):
     ap.add_argument("--bytes", type=int, default=0, help="cfg4: buffer bytes (default 4 GiB)")
     ap.add_argument("--layers", type=int, default=0, help="cfg3: number of layers (default 64); moe: default 12 of 48")
     ap.add_argument("--gemm-schedule", default="", help="cfg3: static_pct,dyn_chunk_tiles (cloak_set_gemm_schedule), e.g. 100,0")
+    ap.add_argument("--gemv-engine", type=int, default=0, help="cloak_set_gemv_engine: 0 auto, 1 one-shot, 2 no PDL")
     ap.add_argument("--out", default="")
     args = ap.parse_args(argv)
+    if args.gemv_engine:
+        _imports()[1].cloak_set_gemv_engine(args.gemv_engine)
     if args.gemm_schedule:
         _imports()[1].cloak_set_gemm_schedule(*[int(v) for v in args.gemm_schedule.split(",")])
     line = json.dumps(RUNNERS[args.workload](args))
