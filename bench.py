@@ -13,6 +13,7 @@ Per-stage GB/s, fractions of the measured HBM peak and the cloaked-vs-native GEM
 `--impl reference` times the CPU oracle (oracle/) on a bounded sample of the same workload.
 """
 import argparse
+import importlib
 import json
 import os
 import subprocess
@@ -60,52 +61,7 @@ def step_bytes(shapes, names=None):
 
 
 # ------------------------------------------------------------------------------------------ clocks
-class ClockSampler:
-    Q = ("index,clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.active,clocks_event_reasons.hw_slowdown,"
-         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
-         "clocks_event_reasons.sw_power_cap")
-
-    def __init__(self, gpu_index):
-        self.lines, self.proc = [], None
-        try:
-            self.proc = subprocess.Popen(["nvidia-smi", f"--id={gpu_index}", f"--query-gpu={self.Q}",
-                                          "--format=csv,noheader,nounits", "-lms", "100"],
-                                         stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
-            self.t = threading.Thread(target=self._read, daemon=True)
-            self.t.start()
-        except OSError:
-            self.proc = None
-
-    def wait_first_sample(self, timeout=10.0):
-        t0 = time.time()
-        while self.proc is not None and not self.lines and time.time() - t0 < timeout:
-            time.sleep(0.02)
-
-    def _read(self):
-        for line in self.proc.stdout:
-            self.lines.append((time.time(), line.strip()))
-
-    def stop(self, t0, t1):
-        if self.proc is None:
-            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
-        time.sleep(0.15)
-        self.proc.terminate()
-        sm, smax, reasons = [], None, set()
-        for ts, line in self.lines:
-            f = [x.strip() for x in line.split(",")]
-            if len(f) < 9:
-                continue
-            try:
-                if t0 - 0.05 <= ts <= t1 + 0.15:
-                    sm.append(float(f[1]))
-                smax = float(f[2])
-            except ValueError:
-                continue
-            for name, v in zip(("hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"), f[5:9]):
-                if v.lower().startswith("active") and t0 - 0.05 <= ts <= t1 + 0.15:
-                    reasons.add(name)
-        return {"sm_mhz": float(np.median(sm)) if sm else None, "sm_max_mhz": smax, "reasons": sorted(reasons),
-                "samples": len(sm)}
+ClockSampler = importlib.import_module("paper_2606_18400_b200.clocks").ClockSampler   # (loads no CUDA library)
 
 
 # ------------------------------------------------------------------------------------------ CPU oracle arm

@@ -17,6 +17,8 @@ import time
 
 import numpy as np
 
+from .clocks import ClockSampler
+
 ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
 NOMINAL_HBM_GBS = 8000.0
 FALLBACK_HBM_GBS = 6650.0
@@ -388,6 +390,9 @@ def run_cfg3(args):
                 return C.cloak_gemm_ops([(T[f"l{l}.{nm}"], X[T[f"l{l}.{nm}"].K], yl[l][nm]) for l in range(layers) for nm in lnames])
 
             res = {}
+            sampler = ClockSampler(0)                   # SM clock, power, throttle reasons while this batch is measured
+            sampler.wait_first_sample()
+            t_start = time.time()
             for pool_name, pool in (("cloaked", pc), ("native", pn)):
                 y = Y[pool_name]
                 yl = [{nm: torch.zeros_like(y[nm]) for nm in lnames} for _ in range(layers)]
@@ -405,6 +410,8 @@ def run_cfg3(args):
                                                      for nm in lnames)
                 res[pool_name] = r
                 Y[pool_name + "_chain"] = yl
+            torch.cuda.synchronize()
+            res["clocks"] = sampler.stop(t_start, time.time())
             res["identical"] = bool(all(torch.equal(Y["cloaked"][nm], Y["native"][nm]) for nm in lnames)
                                     and all(torch.equal(a[nm], b[nm]) for a, b in zip(Y["cloaked_chain"], Y["native_chain"]) for nm in lnames))
             del Y
