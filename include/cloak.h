@@ -222,7 +222,8 @@ cloak_status cloak_to_tile128(const void* d_src, void* d_dst, uint32_t N, uint32
  *             a cloak_shuffle* / cloak_relayout into the pool (those calls mark the pool).  Code that writes
  *             pool memory by other means (through cloak_pool_info's d_base) must synchronise before the
  *             next cloak_gemv.
- * cloak_gemm: batch 16..256 (multiple of 16), dtype BF16, layout TILE128, block_bytes >= 32 KiB
+ * cloak_gemm: batch 1..256 (the MMA runs on the batch rounded up to a multiple of 16; the extra X rows are zero-filled by
+ * TMA and their outputs are not stored), dtype BF16, layout TILE128, block_bytes >= 32 KiB
  *             (tcgen05 tensor cores, accumulators in TMEM, tiles fetched by TMA through the table).
  * Asynchronous on `stream`. */
 typedef struct {

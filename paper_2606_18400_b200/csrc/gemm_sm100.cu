@@ -58,7 +58,8 @@ struct GemmArgs {
     uint32_t* ready;     // per tile row: partials published
     uint32_t* sched;     // [0] next dynamic chunk, [1] CTAs done (the last one resets both)
     uint32_t log2b;
-    uint32_t batch;
+    uint32_t batch;      // columns of the MMA (N): the caller's batch rounded up to a multiple of 16; X rows past the real batch
+    uint32_t nreal;      // are zero-filled by TMA (out of bounds of its map) and their Y columns are not stored
     uint32_t nops;
     uint32_t sper;       // static part [0, dyn_base): CTA b starts with its b-th equal share, sper or sper + 1 units
     uint32_t srem;       // ... the first srem shares have sper + 1
@@ -407,12 +408,12 @@ __global__ void __launch_bounds__(GM_THREADS, 1) gemm_tile128_kernel(const __gri
                             }
 #pragma unroll
                             for (int i = 0; i < 32; ++i)
-                                if (i < 16 || two) op.y[(size_t)(c + i) * op.N + n] = __float2bfloat16_rn(sum[i]);
+                                if (c + i < a.nreal) op.y[(size_t)(c + i) * op.N + n] = __float2bfloat16_rn(sum[i]);
                         } else if (complete) {
 #pragma unroll
                             for (int i = 0; i < 16; ++i) {
-                                op.y[(size_t)(c + i) * op.N + n] = __float2bfloat16_rn(__uint_as_float(v0[i]));
-                                if (two) op.y[(size_t)(c + 16 + i) * op.N + n] = __float2bfloat16_rn(__uint_as_float(v1[i]));
+                                if (c + i < a.nreal) op.y[(size_t)(c + i) * op.N + n] = __float2bfloat16_rn(__uint_as_float(v0[i]));
+                                if (c + 16 + i < a.nreal) op.y[(size_t)(c + 16 + i) * op.N + n] = __float2bfloat16_rn(__uint_as_float(v1[i]));
                             }
                         } else {
 #pragma unroll
@@ -467,7 +468,7 @@ static cloak_status gemm_check(const cloak_pool* pool, const cloak_tensor* w, co
                                const char* who) {
     cloak_status st = check_linear(pool, w, d_x, d_y, who);
     if (st != CLOAK_OK) return st;
-    if (batch < 16 || batch > 256 || batch % 16) return fail(CLOAK_ERR_INVALID, "%s: batch must be a multiple of 16 in 16..256", who);
+    if (batch < 1 || batch > 256) return fail(CLOAK_ERR_INVALID, "%s: batch must be in 1..256", who);
     if (w->dt != CLOAK_BF16 || w->layout != CLOAK_TILE128) return fail(CLOAK_ERR_UNSUPPORTED, "%s: needs CLOAK_BF16 in CLOAK_TILE128 layout", who);
     if (w->N % 128 || w->K % 128) return fail(CLOAK_ERR_ALIGN, "%s: N and K must be multiples of 128", who);
     if (pool->block < 32768) return fail(CLOAK_ERR_UNSUPPORTED, "%s: block_bytes must be >= 32 KiB (one 128x128 bf16 tile)", who);
@@ -493,7 +494,10 @@ static cloak_status gemm_launch(const cloak_pool* pool, const cloak_gemm_op* ops
     GemmArgs a;
     a.T = pool->d_T;
     a.log2b = pool->log2_block;
+    const uint32_t nreal = batch;
+    batch = (batch + 15) & ~15u;         // the MMA's N; TMA zero-fills the X rows past the real batch
     a.batch = batch;
+    a.nreal = nreal;
     a.nops = n;
     const int sms = sm_count(pool->device);
     uint64_t rows = 0, total = 0;
@@ -501,7 +505,7 @@ static cloak_status gemm_launch(const cloak_pool* pool, const cloak_gemm_op* ops
     for (uint32_t j = 0; j < n; ++j) {
         const cloak_tensor& w = ops[j].w;
         if (w.K / 128 > max_kt) max_kt = w.K / 128;
-        st = make_map(&a.map_x[j], ops[j].d_x, w.K, batch, (uint64_t)w.K * 2, 64, batch);
+        st = make_map(&a.map_x[j], ops[j].d_x, w.K, nreal, (uint64_t)w.K * 2, 64, batch);
         if (st != CLOAK_OK) return st;
         GemmOp& o = a.ops[j];
         o.w_offset = w.w_offset;

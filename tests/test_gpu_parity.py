@@ -556,6 +556,7 @@ GEMM_CASES = [
     (65536, [(1024, 5120), (5120, 1024)], [32, 128]),                   # cfg3's k/v shape and a tall one; stream-K cuts
     (65536, [(384, 640)], [48, 256]),                                   # odd tile counts, widest batch
     (2 << 20, [(512, 512)], [64]),                                      # block == page
+    (65536, [(1024, 2048), (384, 640)], [1, 4, 13, 200]),              # batches that are not multiples of 16 (zero-padded MMA columns)
 ]
 
 
@@ -643,7 +644,8 @@ def test_gemm_argument_checks():
         for w, batch, st in [
             (C.cloak_tensor(0, 128, 128, C.CLOAK_BF16, C.CLOAK_TILE128), 32, C.CLOAK_ERR_UNSUPPORTED),   # 4 KiB blocks
             (C.cloak_tensor(0, 128, 128, C.CLOAK_BF16, C.CLOAK_ROWMAJOR), 32, C.CLOAK_ERR_UNSUPPORTED),
-            (C.cloak_tensor(0, 128, 128, C.CLOAK_BF16, C.CLOAK_TILE128), 8, C.CLOAK_ERR_INVALID),
+            (C.cloak_tensor(0, 128, 128, C.CLOAK_BF16, C.CLOAK_TILE128), 0, C.CLOAK_ERR_INVALID),
+            (C.cloak_tensor(0, 128, 128, C.CLOAK_BF16, C.CLOAK_TILE128), 257, C.CLOAK_ERR_INVALID),
             (C.cloak_tensor(0, 100, 128, C.CLOAK_BF16, C.CLOAK_TILE128), 32, C.CLOAK_ERR_ALIGN),
         ]:
             with pytest.raises(C.CloakError) as ei:
