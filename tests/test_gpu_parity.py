@@ -868,3 +868,44 @@ def test_gemv_chain_random_lists_equal_single_calls(seed):
                 wi = [i for i in range(n_w) if T[i] is ops_s[j][0]][0]
                 ref = O.linear_f64(Xh[shapes[wi][1]], Ws[wi])
                 assert O.err_normwise(outs_c[j].float().cpu().numpy(), ref) <= TOL["bf16"], (seed, j)
+
+
+@pytest.mark.parametrize("seed", [0, 1, 2, 3, 4, 5])
+def test_gemm_chain_random_lists(seed):
+    """Random lists of 1..40 independent GEMMs (N, K from 128 to 3 584, any batch 1..256, random schedule: the static part, the
+    dynamic chunk cap and therefore the number of contributors per tile row all vary; several launches past 16 ops): every
+    op against the fp64 oracle, the whole list repeatable bit for bit and identical on the identity-table pool."""
+    rng = np.random.default_rng(500 + seed)
+    key, block, page = 0x1234, int(rng.choice([32768, 65536, 2 << 20])), 2 << 20
+    batch = int(rng.choice([1, 5, 16, 24, 32, 77, 128, 256]))
+    n_w = 5
+    shapes = [(128 * int(rng.integers(1, 17)), 128 * int(rng.choice([1, 2, 3, 5, 8, 13, 28]))) for _ in range(n_w)]
+    Ws = [gen.synth(seed, i, shp, "bf16") for i, shp in enumerate(shapes)]
+    offs, total = C.cloak_arena_plan(key, [2 * n * k for n, k in shapes], block)
+    sched = (int(rng.choice([0, 30, 75, 90, 100])), int(rng.choice([0, 1, 2, 5, 11, 40])))
+    try:
+        with Pool(total, block, page, key) as pc, Pool(total, block, page, key, C.CLOAK_POOL_IDENTITY) as pi:
+            for (n, k), off, Wm in zip(shapes, offs, Ws):
+                til = torch.empty(n * k, dtype=torch.bfloat16, device="cuda")
+                C.cloak_to_tile128(bf16_dev_from_bits(Wm), til, n, k, C.CLOAK_BF16)
+                for p in (pc, pi):
+                    C.cloak_shuffle(p.h, til, off, n * k * 2)
+            T = [C.cloak_tensor(o, n, k, C.CLOAK_BF16, C.CLOAK_TILE128) for (n, k), o in zip(shapes, offs)]
+            X = {k: gen.synth(seed + 50, k, (batch, k), "bf16", kind=gen.KIND_NORMAL) for k in {k for _, k in shapes}}
+            dX = {k: bf16_dev_from_bits(v) for k, v in X.items()}
+            refs = [O.linear_f64(X[k], Wm) for (n, k), Wm in zip(shapes, Ws)]
+            pick = [int(rng.integers(0, n_w)) for _ in range(int(rng.integers(1, 41)))]
+            C.cloak_set_gemm_schedule(*sched)
+
+            def run(pool):
+                ys = [torch.zeros(batch, shapes[w][0], dtype=torch.bfloat16, device="cuda") for w in pick]
+                C.cloak_gemm_chain(pool.h, [(T[w], dX[shapes[w][1]], y) for w, y in zip(pick, ys)], batch)
+                torch.cuda.synchronize()
+                return ys
+            a, b, c = run(pc), run(pc), run(pi)
+            for j, w in enumerate(pick):
+                assert torch.equal(a[j], b[j]) and torch.equal(a[j], c[j]), (sched, batch, j, shapes[w])
+                err = O.err_normwise(a[j].float().cpu().numpy(), refs[w])
+                assert err <= TOL["bf16"], (sched, batch, j, shapes[w], err)
+    finally:
+        C.cloak_set_gemm_schedule(75, 0)
