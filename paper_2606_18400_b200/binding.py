@@ -26,7 +26,7 @@ SYMBOLS = ["cloak_last_error", "cloak_version", "cloak_launch_count", "cloak_key
            "cloak_pool_info", "cloak_pool_tables", "cloak_pool_dump", "cloak_pool_map_ms", "cloak_pool_adjacency", "cloak_shuffle",
            "cloak_unshuffle", "cloak_shuffle_many", "cloak_unshuffle_many", "cloak_relayout", "cloak_rekey_inplace", "cloak_shuffle_host", "cloak_unshuffle_host",
            "cloak_set_copy_engine", "cloak_arena_plan", "cloak_permute_mlp_heads", "cloak_permute_experts", "cloak_load_mlp_heads", "cloak_to_tile128",
-           "cloak_gemv", "cloak_gemv_chain", "cloak_gemm", "cloak_gemm_chain", "cloak_set_gemv_engine", "cloak_set_gemm_schedule", "cloak_gemv_host", "cloak_silu_mul"]
+           "cloak_gemv", "cloak_gemv_chain", "cloak_gemm", "cloak_gemm_chain", "cloak_set_gemv_engine", "cloak_set_gemm_schedule", "cloak_gemm_plan", "cloak_gemv_host", "cloak_silu_mul"]
 
 
 class CloakError(RuntimeError):
@@ -85,6 +85,8 @@ lib.cloak_unshuffle_host.argtypes = [_P, _P, c_uint64, c_uint64, _P]
 lib.cloak_set_copy_engine.argtypes = [c_int]
 lib.cloak_set_gemv_engine.argtypes = [c_int]
 lib.cloak_set_gemm_schedule.argtypes = [c_int, c_int]
+lib.cloak_gemm_plan.argtypes = [c_uint32, POINTER(c_uint32), POINTER(c_uint32), c_uint32, c_uint32, c_uint32,
+                                POINTER(c_uint32), POINTER(c_uint32), POINTER(c_uint32), POINTER(c_uint32)]
 lib.cloak_arena_plan.argtypes = [c_uint64, c_uint32, POINTER(c_uint64), c_uint32, POINTER(c_uint64), POINTER(c_uint64)]
 lib.cloak_permute_mlp_heads.argtypes = [c_uint64, POINTER(cloak_block_shape)] + [_P] * 15
 lib.cloak_permute_experts.argtypes = [c_uint64, POINTER(cloak_moe_shape)] + [_P] * 9
@@ -235,6 +237,18 @@ def cloak_set_gemv_engine(engine):
 
 def cloak_set_gemm_schedule(static_pct, dyn_chunk_tiles=0):
     _check(lib.cloak_set_gemm_schedule(static_pct, dyn_chunk_tiles))
+
+
+def cloak_gemm_plan(shapes, batch, sms=148):
+    """Host only: (chunks, n_static) -- chunks[c] = (begin, end) in the launch's tile sequence -- for ops of shapes [(N, K)]."""
+    n = len(shapes)
+    Ns = (c_uint32 * n)(*[s[0] for s in shapes])
+    Ks = (c_uint32 * n)(*[s[1] for s in shapes])
+    nch, nst = c_uint32(0), c_uint32(0)
+    _check(lib.cloak_gemm_plan(n, Ns, Ks, batch, sms, 0, None, None, ctypes.byref(nch), ctypes.byref(nst)))
+    b, e = (c_uint32 * max(nch.value, 1))(), (c_uint32 * max(nch.value, 1))()
+    _check(lib.cloak_gemm_plan(n, Ns, Ks, batch, sms, nch.value, b, e, ctypes.byref(nch), ctypes.byref(nst)))
+    return [(b[i], e[i]) for i in range(nch.value)], nst.value
 
 
 def cloak_arena_plan(key, sizes, block_bytes):

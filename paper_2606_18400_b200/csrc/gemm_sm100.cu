@@ -112,11 +112,22 @@ __device__ __forceinline__ void gm_dep_wait() { asm volatile("griddepcontrol.wai
 __device__ __forceinline__ void gm_dep_launch() { asm volatile("griddepcontrol.launch_dependents;" ::: "memory"); }
 __device__ __forceinline__ void epi_bar() { asm volatile("bar.sync 1, 128;" ::: "memory"); }
 
+// The chunk grid, shared by the kernel and the host (cloak_gemm_plan exposes it to the tests).
 // Static part: first unit of share b, and the share that holds unit g.
-__device__ __forceinline__ uint32_t static_begin(const GemmArgs& a, uint32_t b) { return b * a.sper + min(b, a.srem); }
-__device__ __forceinline__ uint32_t static_chunk_of(const GemmArgs& a, uint32_t g) {
+__host__ __device__ __forceinline__ uint32_t static_begin(const GemmArgs& a, uint32_t b) { return b * a.sper + (b < a.srem ? b : a.srem); }
+__host__ __device__ __forceinline__ uint32_t static_chunk_of(const GemmArgs& a, uint32_t g) {
     const uint32_t big = a.srem * (a.sper + 1);
     return g < big ? g / (a.sper + 1) : a.srem + (g - big) / a.sper;
+}
+// Dynamic part: units [gbeg, gend) of chunk k < a.ndyn -- piece pc of tile row tn of the op whose chunks hold number k.
+__host__ __device__ __forceinline__ void dyn_chunk(const GemmArgs& a, uint32_t k, uint32_t& gbeg, uint32_t& gend) {
+    uint32_t j = 0;
+    while (j + 1 < a.nops && a.ops[j + 1].cbase <= k) ++j;
+    const GemmOp& op = a.ops[j];
+    const uint32_t loc = k - op.cbase, tn = op.dyn_row0 + loc / op.pieces, pc = loc % op.pieces;
+    const uint32_t last = (pc + 1) * op.plen < op.kt ? (pc + 1) * op.plen : op.kt;
+    gbeg = op.ubase + tn * op.kt + pc * op.plen;
+    gend = op.ubase + tn * op.kt + last;
 }
 
 // A launch runs a list of independent ops (cloak_gemm_chain; cloak_gemm is a list of one): the rings, the accumulator
@@ -219,11 +230,8 @@ __global__ void __launch_bounds__(GM_THREADS, 1) gemm_tile128_kernel(const __gri
         if (a.early) gm_dep_wait();                                                  // the scheduler's counter is the predecessor's too
         uint32_t k = atomicAdd(a.sched, 1u);
         while (k < a.ndyn) {
-            uint32_t j = 0;                                                          // the op whose dynamic chunks hold number k
-            while (j + 1 < a.nops && a.ops[j + 1].cbase <= k) ++j;
-            const GemmOp& op = a.ops[j];
-            const uint32_t loc = k - op.cbase, tn = op.dyn_row0 + loc / op.pieces, pc = loc % op.pieces;
-            const uint32_t gbeg = op.ubase + tn * op.kt + pc * op.plen, gend = op.ubase + tn * op.kt + min((pc + 1) * op.plen, op.kt);
+            uint32_t gbeg, gend;
+            dyn_chunk(a, k, gbeg, gend);
             push(gridDim.x + k, gbeg, gend);
             k = atomicAdd(a.sched, 1u);                                              // in flight while this chunk is issued
             stream(gbeg, gend);
@@ -482,56 +490,38 @@ static int g_dchunk = 0;
 
 constexpr uint32_t GM_MAX_ROWS = 100000;   // tile rows per launch: two counters each in the pool's counter scratch
 
-// One launch of n <= GM_MAX_OPS checked ops.
-static cloak_status gemm_launch(const cloak_pool* pool, const cloak_gemm_op* ops, uint32_t n, uint32_t batch, cudaStream_t s) {
-    cloak_status st;
-    if (!pool->tmap_ready) {
-        cloak_pool* p = const_cast<cloak_pool*>(pool);
-        st = make_map(&p->tmap_tile128, pool->base, 128, pool->bytes() / 256, 256, 64, 128);
-        if (st != CLOAK_OK) return st;
-        p->tmap_ready = true;
-    }
-    GemmArgs a;
-    a.T = pool->d_T;
-    a.log2b = pool->log2_block;
-    const uint32_t nreal = batch;
-    batch = (batch + 15) & ~15u;         // the MMA's N; TMA zero-fills the X rows past the real batch
-    a.batch = batch;
-    a.nreal = nreal;
-    a.nops = n;
-    const int sms = sm_count(pool->device);
+// The chunk grid of one launch: fills the schedule fields of a (ops[j].N/kt/units/ubase/row_base/dyn_row0/pieces/plen/cbase,
+// sper, srem, dyn_base, ndyn, total, nops) from the shapes alone.  `batch` is the MMA's N (a multiple of 16).
+// The launch's tiles -- all ops back to back, each tn-major -- form one sequence.  Its first g_static_pct percent, up to a
+// tile-row boundary, are the static part: CTA b takes the b-th equal share of it.  The rows after that are the dynamic
+// part: whole tile rows (no split-K at all), or equal pieces of a row that is longer than the cap, drawn from a counter
+// as the CTAs become free.  Every piece boundary costs one partial [batch x 128] fp32 and a share of a reduction, so the
+// cap grows with the batch.
+static cloak_status gemm_plan(GemmArgs& a, const uint32_t* N, const uint32_t* K, uint32_t n, uint32_t batch, int sms,
+                              uint32_t* ctas_out, uint64_t* rows_out) {
     uint64_t rows = 0, total = 0;
     uint32_t max_kt = 0;
+    a.nops = n;
     for (uint32_t j = 0; j < n; ++j) {
-        const cloak_tensor& w = ops[j].w;
-        if (w.K / 128 > max_kt) max_kt = w.K / 128;
-        st = make_map(&a.map_x[j], ops[j].d_x, w.K, nreal, (uint64_t)w.K * 2, 64, batch);
-        if (st != CLOAK_OK) return st;
         GemmOp& o = a.ops[j];
-        o.w_offset = w.w_offset;
-        o.y = static_cast<__nv_bfloat16*>(ops[j].d_y);
-        o.N = w.N;
-        o.kt = w.K / 128;
-        const uint64_t units64 = (uint64_t)(w.N / 128) * o.kt;
+        o.N = N[j];
+        o.kt = K[j] / 128;
+        if (o.kt > max_kt) max_kt = o.kt;
+        const uint64_t units64 = (uint64_t)(N[j] / 128) * o.kt;
         if (total + units64 > 0x7fffffffull) return fail(CLOAK_ERR_UNSUPPORTED, "gemm: too many tiles in one launch");
         o.units = (uint32_t)units64;
         o.ubase = (uint32_t)total;
         o.row_base = (uint32_t)rows;
         o.pad_ = 0;
         total += units64;
-        rows += w.N / 128;
+        rows += N[j] / 128;
     }
     if (rows > GM_MAX_ROWS) return fail(CLOAK_ERR_UNSUPPORTED, "gemm: too many output rows for the tile counters");
-    // The launch's tiles -- all ops back to back, each tn-major -- form one sequence.  Its first g_static_pct percent, up to a
-    // tile-row boundary, are the static part: CTA b takes the b-th equal share of it.  The rows after that are the dynamic
-    // part: whole tile rows (no split-K at all), or equal pieces of a row that is longer than the cap, drawn from a counter
-    // as the CTAs become free.  Every piece boundary costs one partial [batch x 128] fp32 and a share of a reduction, so the
-    // cap grows with the batch.
     // At most ~cap chunks per tile row (the fp32 partials are batch * 512 B each): small launches use fewer CTAs.
     uint32_t cap = 512 / batch;
     cap = cap < 4 ? 4 : (cap > 10 ? 10 : cap);
     const uint32_t minper = (max_kt + cap - 1) / cap;
-    uint64_t ctas64 = total / minper;
+    const uint64_t ctas64 = total / minper;
     const uint32_t ctas = (uint32_t)(ctas64 < 1 ? 1 : (ctas64 > (uint64_t)sms ? (uint64_t)sms : ctas64));
     uint32_t dmax = g_dchunk > 0 ? (uint32_t)g_dchunk : (batch >= 128 ? 40u : 20u);
     if (dmax < minper) dmax = minper;
@@ -557,7 +547,42 @@ static cloak_status gemm_launch(const cloak_pool* pool, const cloak_gemm_op* ops
     a.srem = a.dyn_base % ctas;
     a.ndyn = ndyn;
     a.total = (uint32_t)total;
-    const uint64_t nchunks = (uint64_t)ctas + ndyn;
+    *ctas_out = ctas;
+    *rows_out = rows;
+    return CLOAK_OK;
+}
+
+// One launch of n <= GM_MAX_OPS checked ops.
+static cloak_status gemm_launch(const cloak_pool* pool, const cloak_gemm_op* ops, uint32_t n, uint32_t batch, cudaStream_t s) {
+    cloak_status st;
+    if (!pool->tmap_ready) {
+        cloak_pool* p = const_cast<cloak_pool*>(pool);
+        st = make_map(&p->tmap_tile128, pool->base, 128, pool->bytes() / 256, 256, 64, 128);
+        if (st != CLOAK_OK) return st;
+        p->tmap_ready = true;
+    }
+    GemmArgs a;
+    a.T = pool->d_T;
+    a.log2b = pool->log2_block;
+    const uint32_t nreal = batch;
+    batch = (batch + 15) & ~15u;         // the MMA's N; TMA zero-fills the X rows past the real batch
+    a.batch = batch;
+    a.nreal = nreal;
+    const int sms = sm_count(pool->device);
+    uint32_t Ns[GM_MAX_OPS], Ks[GM_MAX_OPS], ctas = 0;
+    uint64_t rows = 0;
+    for (uint32_t j = 0; j < n; ++j) {
+        const cloak_tensor& w = ops[j].w;
+        Ns[j] = w.N;
+        Ks[j] = w.K;
+        st = make_map(&a.map_x[j], ops[j].d_x, w.K, nreal, (uint64_t)w.K * 2, 64, batch);
+        if (st != CLOAK_OK) return st;
+        a.ops[j].w_offset = w.w_offset;
+        a.ops[j].y = static_cast<__nv_bfloat16*>(ops[j].d_y);
+    }
+    st = gemm_plan(a, Ns, Ks, n, batch, sms, &ctas, &rows);
+    if (st != CLOAK_OK) return st;
+    const uint64_t nchunks = (uint64_t)ctas + a.ndyn;
     const uint64_t part_bytes = nchunks * 2 * batch * 128 * 4;
     const uint32_t xtile = batch * 256;
     a.xstages = 2;
@@ -606,6 +631,31 @@ extern "C" cloak_status cloak_set_gemm_schedule(int static_pct, int dyn_chunk_ti
         return fail(CLOAK_ERR_INVALID, "set_gemm_schedule: static_pct in 0..100, dyn_chunk_tiles in 0..4096");
     g_static_pct = static_pct;
     g_dchunk = dyn_chunk_tiles;
+    return CLOAK_OK;
+}
+
+extern "C" cloak_status cloak_gemm_plan(uint32_t n_ops, const uint32_t* h_N, const uint32_t* h_K, uint32_t batch, uint32_t sms,
+                                        uint32_t max_chunks, uint32_t* h_begin, uint32_t* h_end, uint32_t* h_nchunks,
+                                        uint32_t* h_nstatic) {
+    if (!h_N || !h_K || !h_nchunks || !h_nstatic || n_ops == 0 || n_ops > (uint32_t)GM_MAX_OPS)
+        return fail(CLOAK_ERR_INVALID, "gemm_plan: 1..%d ops", GM_MAX_OPS);
+    if (batch < 1 || batch > 256 || sms < 1) return fail(CLOAK_ERR_INVALID, "gemm_plan: batch in 1..256, sms >= 1");
+    for (uint32_t j = 0; j < n_ops; ++j)
+        if (h_N[j] == 0 || h_K[j] == 0 || h_N[j] % 128 || h_K[j] % 128) return fail(CLOAK_ERR_ALIGN, "gemm_plan: N and K must be multiples of 128");
+    GemmArgs a;
+    uint32_t ctas = 0;
+    uint64_t rows = 0;
+    cloak_status st = gemm_plan(a, h_N, h_K, n_ops, (batch + 15) & ~15u, (int)sms, &ctas, &rows);
+    if (st != CLOAK_OK) return st;
+    *h_nstatic = ctas;
+    *h_nchunks = ctas + a.ndyn;
+    if (!h_begin || !h_end) return CLOAK_OK;
+    if (max_chunks < ctas + a.ndyn) return fail(CLOAK_ERR_INVALID, "gemm_plan: %u chunks, room for %u", ctas + a.ndyn, max_chunks);
+    for (uint32_t b = 0; b < ctas; ++b) {                // the same functions the kernel calls
+        h_begin[b] = static_begin(a, b);
+        h_end[b] = static_begin(a, b + 1);
+    }
+    for (uint32_t k = 0; k < a.ndyn; ++k) dyn_chunk(a, k, h_begin[ctas + k], h_end[ctas + k]);
     return CLOAK_OK;
 }
 

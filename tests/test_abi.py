@@ -82,3 +82,58 @@ def test_product_does_not_import_the_oracle():
             if f.endswith(".py"):
                 txt = open(os.path.join(dp, f)).read()
                 assert "paper_2606_18400_b200" not in re.sub(r'""".*?"""', "", txt, flags=re.S), f
+
+
+def test_gemm_chunk_grid_on_the_host(C):
+    """cloak_gemm_plan (the functions the tcgen05 GEMM kernel itself calls for its work split, run on the host): for the
+    cfg1 / cfg3 layers and random op lists, under several schedules -- the chunks cover the launch's tile sequence exactly
+    once and in order; the static shares are equal to within one tile and there is one per CTA at most; every drawn chunk
+    is non-empty and lies inside ONE tile row of ONE op (whole rows never split K); and a tile row is met by a bounded
+    number of chunks (each extra one is a [batch x 128] fp32 partial and a share of a reduction)."""
+    import numpy as np
+    rng = np.random.default_rng(7)
+    qwen = [(5120, 5120), (1024, 5120), (1024, 5120), (5120, 5120), (27648, 5120), (27648, 5120), (5120, 27648)]
+    llama = [(4096, 4096), (1024, 4096), (1024, 4096), (4096, 4096), (14336, 4096), (14336, 4096), (4096, 14336)]
+    lists = [qwen * 2, llama, qwen[:1], [(128, 128)], [(384, 640), (128, 128)]]
+    lists += [[(128 * int(rng.integers(1, 40)), 128 * int(rng.integers(1, 60))) for _ in range(int(rng.integers(1, 17)))] for _ in range(20)]
+    try:
+        for sched in ((75, 0), (100, 0), (0, 0), (40, 3), (90, 64)):
+            C.cloak_set_gemm_schedule(*sched)
+            for shapes in lists:
+                for batch, sms in ((1, 148), (32, 148), (128, 148), (256, 132), (77, 8)):
+                    chunks, nstatic = C.cloak_gemm_plan(shapes, batch, sms)
+                    total = sum((n // 128) * (k // 128) for n, k in shapes)
+                    assert 1 <= nstatic <= sms
+                    # row boundaries of the sequence: op j, tile row r starts at ubase_j + r * kt_j
+                    starts, kts, u = [], [], 0
+                    for n, k in shapes:
+                        for r in range(n // 128):
+                            starts.append(u + r * (k // 128))
+                            kts.append(k // 128)
+                        u += (n // 128) * (k // 128)
+                    starts = np.array(starts)
+                    pos = 0
+                    sizes = []
+                    for c, (b, e) in enumerate(chunks):
+                        assert b == pos and e >= b, (sched, shapes, batch, c)
+                        pos = e
+                        if c < nstatic:
+                            sizes.append(e - b)
+                        else:
+                            assert e > b
+                            r = int(np.searchsorted(starts, b, side="right")) - 1
+                            assert e <= starts[r] + kts[r], (sched, shapes, batch, c)       # inside one tile row
+                    assert pos == total
+                    assert max(sizes) - min(sizes) <= 1
+                    # chunks per tile row
+                    edges = np.array([b for b, e in chunks if e > b])
+                    first = np.searchsorted(edges, starts, side="right") - 1
+                    last = np.searchsorted(edges, starts + np.array(kts) - 1, side="right") - 1
+                    per_row = last - first + 1
+                    if sched[1] == 0:
+                        assert per_row.max() <= 12, (sched, shapes, batch, int(per_row.max()))
+    finally:
+        C.cloak_set_gemm_schedule(75, 0)
+    for bad in [([(100, 128)], 32, 148), ([(128, 128)] * 17, 32, 148), ([(128, 128)], 0, 148), ([(128, 128)], 32, 0)]:
+        with pytest.raises(C.CloakError):
+            C.cloak_gemm_plan(*bad)
