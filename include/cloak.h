@@ -225,7 +225,10 @@ cloak_status cloak_to_tile128(const void* d_src, void* d_dst, uint32_t N, uint32
  * cloak_gemm: batch 1..256 (the MMA runs on the batch rounded up to a multiple of 16; the extra X rows are zero-filled by
  * TMA and their outputs are not stored), dtype BF16, layout TILE128, block_bytes >= 32 KiB
  *             (tcgen05 tensor cores, accumulators in TMEM, tiles fetched by TMA through the table).
- * Asynchronous on `stream`. */
+ * Asynchronous on `stream`.  Scratch (split-K counters and partials) belongs to the pool and grows on demand: the first
+ * call of a shape / batch larger than any before it allocates, which synchronises the device; so one pool serves one
+ * stream at a time, and before capturing these calls into a CUDA graph the same calls must have run once uncaptured
+ * (capture itself then launches kernels only; replays of one graph must not overlap each other). */
 typedef struct {
     uint64_t w_offset;
     uint32_t N, K;
