@@ -371,7 +371,7 @@ def run_cfg3(args):
         T = {nm: C.cloak_tensor(off[nm], shp[0], shp[1], C.CLOAK_BF16, C.CLOAK_TILE128) for nm, shp in tensors}
         lnames = [nm for nm, _ in gen.layer_shapes(H, I, c["n_q"], c["n_kv"], c["head_dim"])]
         out = {}
-        for batch in (32, 128):
+        for batch in ([int(v) for v in args.batches.split(",")] if getattr(args, "batches", "") else (32, 128)):
             X = {k: synth_cuda.fill(torch.empty(batch, k, dtype=torch.bfloat16, device="cuda"), c["seed"] + 100,
                                     2 * batch + i, kind=gen.KIND_NORMAL) for i, k in enumerate(sorted({H, I, Q}))}
             Y = {pn_: {nm: torch.zeros(batch, dict(tensors)[f"l0.{nm}"][0], dtype=torch.bfloat16, device="cuda") for nm in lnames}
@@ -545,6 +545,7 @@ def main(argv=None):
     ap.add_argument("--reps", type=int, default=10)
     ap.add_argument("--bytes", type=int, default=0, help="cfg4: buffer bytes (default 4 GiB)")
     ap.add_argument("--layers", type=int, default=0, help="cfg3: number of layers (default 64); moe: default 12 of 48")
+    ap.add_argument("--batches", default="", help="cfg3: batch sizes, e.g. 16,64,256 (default 32,128)")
     ap.add_argument("--gemm-schedule", default="", help="cfg3: static_pct,dyn_chunk_tiles (cloak_set_gemm_schedule), e.g. 100,0")
     ap.add_argument("--gemv-engine", type=int, default=0, help="cloak_set_gemv_engine: 0 auto, 1 one-shot, 2 no PDL")
     ap.add_argument("--out", default="")
