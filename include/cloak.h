@@ -61,7 +61,8 @@ uint64_t cloak_launch_count(void);
  * For i in [0, n): o = Philox4x32-10(ctr = (i, 0, stream_id lo, stream_id hi), key = (key lo, key hi)),
  * r_i = o[0]:o[1]; perm = indices sorted ascending by (r_i, i); inv[perm[j]] = j.
  * d_perm / d_inv: caller-owned device buffers of n uint32; either may be NULL (not both).
- * n in [1, 2^28].  Asynchronous on `stream` (workspace comes from the stream-ordered allocator). */
+ * n in [1, 2^28].  Asynchronous on `stream` (workspace comes from the library's own stream-ordered memory pool, which keeps
+ * at most 512 MiB of freed scratch cached; the process's default pool is not touched). */
 cloak_status cloak_keygen(uint64_t key, uint64_t stream_id, uint32_t n,
                           uint32_t* d_perm, uint32_t* d_inv, void* stream);
 
@@ -108,8 +109,9 @@ cloak_status cloak_pool_map_ms(const cloak_pool* pool, double* ms);
  *   *physical_blocks = the same through the page map, slot(i) = pageinv[blockinv[i] / bpp] * bpp + blockinv[i] % bpp
  *                      (the dump view D: what reading pages in physical order sees; G8: expect about 1 / nslots)
  *   *pages           = #{v : pageinv[v+1] == pageinv[v] + 1} / (npages - 1)
- * An identity pool reports 1, 1, 1.  Any output may be NULL.  Synchronous. */
-cloak_status cloak_pool_adjacency(const cloak_pool* pool, double* va_blocks, double* physical_blocks, double* pages);
+ * An identity pool reports 1, 1, 1.  Any output may be NULL.  Runs on `stream` and synchronises that stream only. */
+cloak_status cloak_pool_adjacency(const cloak_pool* pool, double* va_blocks, double* physical_blocks, double* pages,
+                                  void* stream);
 
 /* ---- S4 block shuffle / unshuffle, S8 re-layout (north_star (a)).
  * shuffle:   pool[T[i]*b + o] = logical[i*b + o] for the arena range [logical_offset, +bytes);
@@ -225,10 +227,18 @@ cloak_status cloak_to_tile128(const void* d_src, void* d_dst, uint32_t N, uint32
  * cloak_gemm: batch 1..256 (the MMA runs on the batch rounded up to a multiple of 16; the extra X rows are zero-filled by
  * TMA and their outputs are not stored), dtype BF16, layout TILE128, block_bytes >= 32 KiB
  *             (tcgen05 tensor cores, accumulators in TMEM, tiles fetched by TMA through the table).
- * Asynchronous on `stream`.  Scratch (split-K counters and partials) belongs to the pool and grows on demand: the first
- * call of a shape / batch larger than any before it allocates, which synchronises the device; so one pool serves one
- * stream at a time, and before capturing these calls into a CUDA graph the same calls must have run once uncaptured
- * (capture itself then launches kernels only; replays of one graph must not overlap each other). */
+ * Asynchronous on `stream`; no compute call synchronises or calls the driver's allocator.
+ * Scratch (split-K counters and fp32 partials) belongs to the pool.  16 MiB exist from cloak_pool_create on: enough for every
+ * cloak_gemv / cloak_gemv_chain of the streaming kernel and for small GEMMs.  A call that needs more (the cloak_*_scratch_bytes
+ * queries below say how much) grows the scratch in the order of ITS stream (stream-ordered allocation, counters zeroed on
+ * that stream, the old buffer released behind the kernels already queued) -- except while that stream is being captured into
+ * a CUDA graph, where the call fails with CLOAK_ERR_INVALID: reserve first.  With the scratch reserved, a first-use call can
+ * be captured without any warm-up.  The counters and partials are shared by all calls on one pool: those calls must be
+ * ordered with respect to each other (one stream, or events), and replays of one graph must not overlap each other.
+ * Different pools are independent and may run on different streams at the same time.
+ * Co-residency: the streaming GEMV's CTAs wait for one another, so it is launched as a COOPERATIVE grid (all CTAs resident or
+ * the launch waits / fails -- never a hang when other kernels hold SMs).  The GEMM needs no such guarantee: a CTA only ever
+ * waits for partials of CTAs that drew their ticket before it, i.e. that are already running. */
 typedef struct {
     uint64_t w_offset;
     uint32_t N, K;
@@ -239,6 +249,17 @@ cloak_status cloak_gemv(const cloak_pool* pool, const cloak_tensor* w, const voi
                         uint32_t batch, void* stream);
 cloak_status cloak_gemm(const cloak_pool* pool, const cloak_tensor* w, const void* d_x, void* d_y,
                         uint32_t batch, void* stream);
+/* Bytes of pool scratch the chain calls below need for these ops at this batch (the largest of the launches they split into);
+ * host only.  cloak_pool_reserve_workspace grows the pool's scratch to at least `bytes` (never shrinks); synchronous: it
+ * waits for the device, so call it at load time.  (cloak_gemv / cloak_gemm = a chain of one op.) */
+struct cloak_gemv_op;
+struct cloak_gemm_op;
+cloak_status cloak_gemv_chain_scratch_bytes(const cloak_pool* pool, const struct cloak_gemv_op* h_ops, uint32_t n_ops,
+                                            uint32_t batch, uint64_t* h_bytes);
+cloak_status cloak_gemm_chain_scratch_bytes(const cloak_pool* pool, const struct cloak_gemm_op* h_ops, uint32_t n_ops,
+                                            uint32_t batch, uint64_t* h_bytes);
+cloak_status cloak_pool_reserve_workspace(cloak_pool* pool, uint64_t bytes);
+
 /* A chain of GEMVs over one pool in ONE persistent launch (SURVEY.md 8(a) S6 at cfg2: "end-to-end cloaked decode
  * of all layers' projection GEMVs"; decode is bandwidth-bound, so the weight stream should
  * never stop).  Op i computes Y_i = X_i W_i^T like cloak_gemv, with two additions:
@@ -257,7 +278,7 @@ cloak_status cloak_gemm(const cloak_pool* pool, const cloak_tensor* w, const voi
  * distinct.  h_ops is a HOST array (copied into the launch parameters; not referenced after the call returns).
  * Chains longer than 48 ops, or mixing row sizes that need different chunk sizes, are split into several
  * launches (stream order keeps the semantics).  Asynchronous on `stream`. */
-typedef struct {
+typedef struct cloak_gemv_op {
     cloak_tensor w;
     const void* d_x;
     void* d_y;
@@ -274,7 +295,7 @@ cloak_status cloak_gemv_chain(const cloak_pool* pool, const cloak_gemv_op* h_ops
  * summation order.  The weight stream runs on across op boundaries
  * (BASELINE.json configs[3]: "cloaked decode GEMM" of every projection of the model).  h_ops is a HOST array, not
  * referenced after the call returns.  Asynchronous on `stream`. */
-typedef struct {
+typedef struct cloak_gemm_op {
     cloak_tensor w;
     const void* d_x;
     void* d_y;
@@ -283,7 +304,8 @@ cloak_status cloak_gemm_chain(const cloak_pool* pool, const cloak_gemm_op* h_ops
                               void* stream);
 /* Selects the bf16 GEMV kernel: 0 = automatic (streaming TMA kernel when K % 256 == 0, launched with
  * programmatic dependent launch), 1 = always the one-shot split-K kernel, 2 = automatic without
- * programmatic dependent launch.  For A/B measurement; process-wide. */
+ * programmatic dependent launch.  For A/B measurement; process-wide (an atomic: safe to flip from any thread, takes effect
+ * at the next launch). */
 cloak_status cloak_set_gemv_engine(int engine);
 /* Host only, no device work: the chunk grid one cloak_gemm_chain launch of n_ops <= 16 ops with these shapes would use on a
  * GPU with `sms` SMs under the current cloak_set_gemm_schedule.  The launch's 128x128 tiles -- the ops back to back, each in
@@ -300,7 +322,8 @@ cloak_status cloak_gemm_plan(uint32_t n_ops, const uint32_t* h_N, const uint32_t
  * outputs under different settings agree within the bf16 tolerance, not bit for bit; under one setting they do not depend
  * on which CTA drew which chunk.  Default (75, 0).  For A/B measurement; process-wide. */
 cloak_status cloak_set_gemm_schedule(int static_pct, int dyn_chunk_tiles);
-/* Host-buffer variant of cloak_gemv (end-to-end path): copies X up, runs, copies Y back, synchronises. */
+/* Host-buffer variant of cloak_gemv (end-to-end path): copies X up, runs, copies Y back, synchronises `stream` once (h_y is
+ * the caller's to read on return).  Device staging comes from the library's cached pool: no driver allocation per call. */
 cloak_status cloak_gemv_host(const cloak_pool* pool, const cloak_tensor* w, const void* h_x, void* h_y,
                              uint32_t batch, void* stream);
 

@@ -19,7 +19,10 @@ generator; worked examples W1-W5 of SURVEY.md 8(c).4 under tests/golden/; O(n^2)
 rank; bijection / restriction / forced-tie properties; byte-at-a-time restatement of O5;
 unshuffle(shuffle)=id; relayout A->A = id, A->B->A; MLP' = MLP and attention' = attention
 brute-forced in fp64; MoE' = MoE (expert + per-expert neuron permutation) brute-forced in fp64 with negative controls and
-the E = 1 / k = 1 reductions to the dense MLP; W = I and W = ones closed forms for GEMV.  Parity unpinned: none.
+the E = 1 / k = 1 reductions to the dense MLP, and the stored eps / pi_e worked example of tests/golden/moe_example.json
+(written by a pure-Python restatement that shares nothing with this package); attention closed forms (scale, causal mask,
+grouped KV); adjacent_fraction against a python-int brute force on a table with descending neighbours; W = I and W = ones
+closed forms for GEMV.  Parity unpinned: none.
 
 Citations: `P:<n>` = /root/reference/PAPER.md line n; `BJ:` = BASELINE.json north_star /
 configs; `O<n>`/`G<n>` = SURVEY.md section 8(c) definitions / readings.

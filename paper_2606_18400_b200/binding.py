@@ -26,7 +26,8 @@ SYMBOLS = ["cloak_last_error", "cloak_version", "cloak_launch_count", "cloak_key
            "cloak_pool_info", "cloak_pool_tables", "cloak_pool_dump", "cloak_pool_map_ms", "cloak_pool_adjacency", "cloak_shuffle",
            "cloak_unshuffle", "cloak_shuffle_many", "cloak_unshuffle_many", "cloak_relayout", "cloak_rekey_inplace", "cloak_shuffle_host", "cloak_unshuffle_host",
            "cloak_set_copy_engine", "cloak_arena_plan", "cloak_permute_mlp_heads", "cloak_permute_experts", "cloak_load_mlp_heads", "cloak_to_tile128",
-           "cloak_gemv", "cloak_gemv_chain", "cloak_gemm", "cloak_gemm_chain", "cloak_set_gemv_engine", "cloak_set_gemm_schedule", "cloak_gemm_plan", "cloak_gemv_host", "cloak_silu_mul"]
+           "cloak_gemv", "cloak_gemv_chain", "cloak_gemm", "cloak_gemm_chain", "cloak_gemv_chain_scratch_bytes",
+           "cloak_gemm_chain_scratch_bytes", "cloak_pool_reserve_workspace", "cloak_set_gemv_engine", "cloak_set_gemm_schedule", "cloak_gemm_plan", "cloak_gemv_host", "cloak_silu_mul"]
 
 
 class CloakError(RuntimeError):
@@ -73,7 +74,8 @@ lib.cloak_pool_info.argtypes = [_P, POINTER(_P), POINTER(_P), POINTER(c_uint32),
 lib.cloak_pool_tables.argtypes = [_P, _P, _P, _P, _P]
 lib.cloak_pool_dump.argtypes = [_P, _P, _P]
 lib.cloak_pool_map_ms.argtypes = [_P, POINTER(c_double)]
-lib.cloak_pool_adjacency.argtypes = [_P, POINTER(c_double), POINTER(c_double), POINTER(c_double)]
+lib.cloak_pool_adjacency.argtypes = [_P, POINTER(c_double), POINTER(c_double), POINTER(c_double), _P]
+lib.cloak_pool_reserve_workspace.argtypes = [_P, c_uint64]
 lib.cloak_shuffle.argtypes = [_P, _P, c_uint64, c_uint64, _P]
 lib.cloak_unshuffle.argtypes = [_P, _P, c_uint64, c_uint64, _P]
 lib.cloak_shuffle_many.argtypes = [_P, c_uint32, POINTER(c_void_p), POINTER(c_uint64), POINTER(c_uint64), _P]
@@ -95,6 +97,8 @@ lib.cloak_to_tile128.argtypes = [_P, _P, c_uint32, c_uint32, c_int, _P]
 lib.cloak_gemv.argtypes = [_P, POINTER(cloak_tensor), _P, _P, c_uint32, _P]
 lib.cloak_gemv_chain.argtypes = [_P, POINTER(cloak_gemv_op), c_uint32, c_uint32, _P]
 lib.cloak_gemm_chain.argtypes = [_P, POINTER(cloak_gemm_op), c_uint32, c_uint32, _P]
+lib.cloak_gemv_chain_scratch_bytes.argtypes = [_P, POINTER(cloak_gemv_op), c_uint32, c_uint32, POINTER(c_uint64)]
+lib.cloak_gemm_chain_scratch_bytes.argtypes = [_P, POINTER(cloak_gemm_op), c_uint32, c_uint32, POINTER(c_uint64)]
 lib.cloak_gemm.argtypes = [_P, POINTER(cloak_tensor), _P, _P, c_uint32, _P]
 lib.cloak_gemv_host.argtypes = [_P, POINTER(cloak_tensor), _P, _P, c_uint32, _P]
 lib.cloak_silu_mul.argtypes = [_P, _P, _P, c_uint64, c_int, _P]
@@ -183,10 +187,14 @@ def cloak_pool_map_ms(pool):
     return ms.value
 
 
-def cloak_pool_adjacency(pool):
+def cloak_pool_adjacency(pool, stream=None):
     va, ph, pg = c_double(), c_double(), c_double()
-    _check(lib.cloak_pool_adjacency(pool, byref(va), byref(ph), byref(pg)))
+    _check(lib.cloak_pool_adjacency(pool, byref(va), byref(ph), byref(pg), _stream(stream)))
     return dict(va_blocks=va.value, physical_blocks=ph.value, pages=pg.value)
+
+
+def cloak_pool_reserve_workspace(pool, nbytes):
+    _check(lib.cloak_pool_reserve_workspace(pool, nbytes))
 
 
 def cloak_shuffle(pool, d_logical, logical_offset, nbytes, stream=None):
@@ -305,6 +313,20 @@ def cloak_gemv_ops(ops):
 def cloak_gemv_chain(pool, ops, batch, stream=None):
     arr = ops if isinstance(ops, ctypes.Array) else cloak_gemv_ops(ops)
     _check(lib.cloak_gemv_chain(pool, arr, len(arr), batch, _stream(stream)))
+
+
+def cloak_gemv_chain_scratch_bytes(pool, ops, batch):
+    arr = ops if isinstance(ops, ctypes.Array) else cloak_gemv_ops(ops)
+    n = c_uint64()
+    _check(lib.cloak_gemv_chain_scratch_bytes(pool, arr, len(arr), batch, byref(n)))
+    return n.value
+
+
+def cloak_gemm_chain_scratch_bytes(pool, ops, batch):
+    arr = ops if isinstance(ops, ctypes.Array) else cloak_gemm_ops(ops)
+    n = c_uint64()
+    _check(lib.cloak_gemm_chain_scratch_bytes(pool, arr, len(arr), batch, byref(n)))
+    return n.value
 
 
 def cloak_gemm(pool, tensor, d_x, d_y, batch, stream=None):

@@ -82,8 +82,38 @@ inline void launched(unsigned n = 1) { g_launches.fetch_add(n, std::memory_order
 // keygen on the current device (keygen.cu).  Either output may be null.
 cloak_status keygen_device(uint64_t key, uint64_t stream_id, uint32_t n, uint32_t* d_perm, uint32_t* d_inv,
                            cudaStream_t s);
+// Opt-in to more than 48 KiB of dynamic shared memory, once per (kernel, device): the attribute belongs to the device's
+// context, so a per-process flag would leave a second GPU with the 48 KiB default.  `done` is the call site's own mask.
+template <typename K>
+inline cloak_status smem_opt_in(K* kernel, size_t bytes, int device, std::atomic<uint64_t>& done) {
+    const bool tracked = device >= 0 && device < 64;
+    const uint64_t bit = 1ull << (device & 63);
+    if (tracked && (done.load(std::memory_order_acquire) & bit)) return CLOAK_OK;
+    CLOAK_CUDA(cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes));
+    if (tracked) done.fetch_or(bit, std::memory_order_release);
+    return CLOAK_OK;
+}
+
+// Stream-ordered scratch from the library's OWN memory pool on the current device (release threshold 512 MiB), so that the
+// process's default pool -- and whatever the host framework does with it -- is left alone.  Capturable like cudaMallocAsync.
+cloak_status async_alloc(void** p, size_t bytes, cudaStream_t s);
+// ... released on every exit path
+struct AsyncBuf {
+    void* p = nullptr;
+    cudaStream_t s;
+    explicit AsyncBuf(cudaStream_t st) : s(st) {}
+    AsyncBuf(const AsyncBuf&) = delete;
+    AsyncBuf& operator=(const AsyncBuf&) = delete;
+    ~AsyncBuf() { if (p) cudaFreeAsync(p, s); }
+    cloak_status alloc(size_t bytes) { return async_alloc(&p, bytes, s); }
+};
+
+// Library-owned scratch of a pool (split-K counters, then fp32 partials): WS_DEFAULT_BYTES exist from cloak_pool_create on
+// (enough for every GEMV chain launch); a call that needs more grows it IN STREAM ORDER on its own stream (never a device
+// synchronisation) and fails during stream capture, where cloak_pool_reserve_workspace must have run before.
 constexpr size_t WS_COUNTER_BYTES = 1u << 20;
-cloak_status pool_workspace(const cloak_pool* pool, size_t bytes);
+constexpr size_t WS_DEFAULT_BYTES = 16u << 20;
+cloak_status pool_workspace(const cloak_pool* pool, size_t bytes, cudaStream_t s);
 // gemv_stream.cu: persistent TMA-fed bf16 GEMV chain (K % 256 == 0).  gemv_stream_chunk: the row-chunk size (in 512-byte units) the
 // kernel would use for a tensor, or -1 if it cannot take it; gemv_stream_launch: one launch of <= 48 ops that
 // share that chunk size.

@@ -207,23 +207,21 @@ __global__ void __launch_bounds__(TMA_WARPS * 32) copy_tma_many_kernel(const __g
 static cloak_status launch_tail(const cloak_pool* pool, char* logical_tail, uint32_t block_index, uint32_t tail,
                                 int to_pool, cudaStream_t s);
 
-static int g_engine = 0;   // 0 auto, 1 LDG, 2 TMA
+static std::atomic<int> g_engine{0};   // 0 auto, 1 LDG, 2 TMA
 
 static cloak_status launch_copy(const cloak_pool* pool, const CopyArgs& a, cudaStream_t s) {
     if (a.nblocks == 0) return CLOAK_OK;
     const int sms = sm_count(pool->device);
-    int engine = g_engine;
+    int engine = g_engine.load(std::memory_order_relaxed);
     if (engine == 0) engine = (a.log2b >= 12) ? 2 : 1;
     if (engine == 2 && a.log2b < 10) engine = 1;        // bulk copies below 1 KiB are not worth a ring
     if (engine == 2) {
         const uint32_t log2c = a.log2b < 13 ? a.log2b : 13;          // chunk = min(block, 8 KiB)
         const uint64_t units = (uint64_t)a.nblocks << (a.log2b - log2c);
         const size_t smem = (size_t)TMA_WARPS * TMA_STAGES << log2c;  // <= 128 KiB
-        static bool attr_set = false;
-        if (!attr_set) {
-            CLOAK_CUDA(cudaFuncSetAttribute(copy_tma_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024));
-            attr_set = true;
-        }
+        static std::atomic<uint64_t> opted{0};
+        cloak_status ost = smem_opt_in(copy_tma_kernel, 200 * 1024, pool->device, opted);
+        if (ost != CLOAK_OK) return ost;
         uint64_t ctas = (units + TMA_WARPS - 1) / TMA_WARPS;
         const uint64_t cap = (uint64_t)sms * (smem <= 100 * 1024 ? 2 : 1);
         if (ctas > cap) ctas = cap;
@@ -340,7 +338,7 @@ using namespace cloak;
 
 extern "C" cloak_status cloak_set_copy_engine(int engine) {
     if (engine < 0 || engine > 2) return fail(CLOAK_ERR_INVALID, "set_copy_engine: engine must be 0, 1 or 2");
-    g_engine = engine;
+    g_engine.store(engine);
     return CLOAK_OK;
 }
 
@@ -369,18 +367,16 @@ static cloak_status move_many(const cloak_pool* pool, uint32_t n, void* const* d
     }
     DeviceGuard g(pool->device);
     if (dir == TO_POOL) pool->wrote(s);
-    if (pool->log2_block < 10 || g_engine == 1) {          // tiny blocks or the LDG engine forced: range by range
+    if (pool->log2_block < 10 || g_engine.load(std::memory_order_relaxed) == 1) {          // tiny blocks or the LDG engine forced: range by range
         for (uint32_t r = 0; r < n; ++r) {
             cloak_status st = move_range(pool, (char*)d_logical[r], h_offsets[r], h_bytes[r], dir, s);
             if (st != CLOAK_OK) return st;
         }
         return CLOAK_OK;
     }
-    static bool attr_set = false;
-    if (!attr_set) {
-        CLOAK_CUDA(cudaFuncSetAttribute(copy_tma_many_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024));
-        attr_set = true;
-    }
+    static std::atomic<uint64_t> opted{0};
+    cloak_status ost = smem_opt_in(copy_tma_many_kernel, 200 * 1024, pool->device, opted);
+    if (ost != CLOAK_OK) return ost;
     const int sms = sm_count(pool->device);
     const uint32_t b = pool->block;
     for (uint32_t r0 = 0; r0 < n; r0 += MANY_MAX) {

@@ -84,6 +84,37 @@ int sm_count(int device) {
     return cached[device];
 }
 
+// ---- the library's stream-ordered memory pool, one per device
+static cudaMemPool_t g_mempool[64];
+static std::mutex g_mempool_mu;
+
+cloak_status async_alloc(void** p, size_t bytes, cudaStream_t s) {
+    int dev = 0;
+    CLOAK_CUDA(cudaGetDevice(&dev));
+    cudaMemPool_t mp = nullptr;
+    if (dev >= 0 && dev < 64) {
+        std::lock_guard<std::mutex> lock(g_mempool_mu);
+        if (!g_mempool[dev]) {
+            cudaMemPoolProps props = {};
+            props.allocType = cudaMemAllocationTypePinned;
+            props.handleTypes = cudaMemHandleTypeNone;
+            props.location.type = cudaMemLocationTypeDevice;
+            props.location.id = dev;
+            cudaMemPool_t np = nullptr;
+            if (cudaMemPoolCreate(&np, &props) == cudaSuccess) {
+                uint64_t keep = 512ull << 20;      // freed scratch stays cached up to this much; the rest goes back at a sync
+                cudaMemPoolSetAttribute(np, cudaMemPoolAttrReleaseThreshold, &keep);
+                g_mempool[dev] = np;
+            }
+            cudaGetLastError();
+        }
+        mp = g_mempool[dev];
+    }
+    if (mp) CLOAK_CUDA(cudaMallocFromPoolAsync(p, bytes, mp, s));
+    else CLOAK_CUDA(cudaMallocAsync(p, bytes, s));
+    return CLOAK_OK;
+}
+
 // ---- host Philox4x32-10 for the tiny tensor-order permutation of S3.
 static inline void philox_host(uint32_t c[4], uint32_t k0, uint32_t k1) {
     for (int r = 0; r < 10; ++r) {

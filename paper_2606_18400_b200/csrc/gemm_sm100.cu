@@ -1,4 +1,4 @@
-// S7 cloak_gemm: batch 16..256 contraction on tcgen05 tensor cores, W tiles fetched by TMA through the table.
+// S7 cloak_gemm: batch 1..256 (MMA columns rounded up to 16) contraction on tcgen05 tensor cores, W tiles fetched by TMA through the table.
 //
 // Definition (north_star (c) "batch>1 gather-fused GEMM ... tcgen05/TMEM tiles fed by TMA through
 // the permutation table"; BASELINE.json configs[3]):  Y[m, n] = sum_k X[m, k] * W[n, k], W in CLOAK_TILE128
@@ -469,7 +469,7 @@ static cloak_status make_map(CUtensorMap* map, const void* base, uint64_t inner,
     return CLOAK_OK;
 }
 
-extern bool g_gemv_pdl;      // gemv_stream.cu: the PDL A/B switch (cloak_set_gemv_engine(2) turns it off)
+extern std::atomic<bool> g_gemv_pdl;      // gemv_stream.cu: the PDL A/B switch (cloak_set_gemv_engine(2) turns it off)
 cloak_status check_linear(const cloak_pool* pool, const cloak_tensor* w, const void* x, void* y, const char* who);
 
 static cloak_status gemm_check(const cloak_pool* pool, const cloak_tensor* w, const void* d_x, void* d_y, uint32_t batch,
@@ -485,8 +485,8 @@ static cloak_status gemm_check(const cloak_pool* pool, const cloak_tensor* w, co
 
 // Schedule knobs (cloak_set_gemm_schedule): percentage of the launch's tiles that is dealt out statically, and the cap on
 // the tiles of a dynamic chunk (0 = by batch).
-static int g_static_pct = 75;
-static int g_dchunk = 0;
+static std::atomic<int> g_static_pct{75};
+static std::atomic<int> g_dchunk{0};
 
 constexpr uint32_t GM_MAX_ROWS = 100000;   // tile rows per launch: two counters each in the pool's counter scratch
 
@@ -523,11 +523,12 @@ static cloak_status gemm_plan(GemmArgs& a, const uint32_t* N, const uint32_t* K,
     const uint32_t minper = (max_kt + cap - 1) / cap;
     const uint64_t ctas64 = total / minper;
     const uint32_t ctas = (uint32_t)(ctas64 < 1 ? 1 : (ctas64 > (uint64_t)sms ? (uint64_t)sms : ctas64));
-    uint32_t dmax = g_dchunk > 0 ? (uint32_t)g_dchunk : (batch >= 128 ? 40u : 20u);
+    const int dchunk = g_dchunk.load(std::memory_order_relaxed), static_pct = g_static_pct.load(std::memory_order_relaxed);
+    uint32_t dmax = dchunk > 0 ? (uint32_t)dchunk : (batch >= 128 ? 40u : 20u);
     if (dmax < minper) dmax = minper;
     // A launch with less than a few dynamic chunks' worth of tiles per CTA is dealt out statically: its tail would be as
     // long as a chunk, and there is little to balance.
-    const uint64_t target = (total / ctas < 4ull * dmax && g_dchunk == 0) ? total : total * (uint64_t)g_static_pct / 100;
+    const uint64_t target = (total / ctas < 4ull * dmax && dchunk == 0) ? total : total * (uint64_t)static_pct / 100;
     uint32_t ndyn = 0;
     a.dyn_base = (uint32_t)total;
     for (uint32_t j = 0; j < n; ++j) {
@@ -592,7 +593,7 @@ static cloak_status gemm_launch(const cloak_pool* pool, const cloak_gemm_op* ops
     a.wstages = wst;
     a.tmem_cols = 32;
     while (a.tmem_cols < 2 * batch) a.tmem_cols <<= 1;
-    st = pool_workspace(pool, WS_COUNTER_BYTES + part_bytes);
+    st = pool_workspace(pool, WS_COUNTER_BYTES + part_bytes, s);
     if (st != CLOAK_OK) return st;
     a.ticket = reinterpret_cast<uint32_t*>(pool->ws);
     a.ready = a.ticket + rows;
@@ -600,12 +601,11 @@ static cloak_status gemm_launch(const cloak_pool* pool, const cloak_gemm_op* ops
     a.part = reinterpret_cast<float*>(pool->ws + WS_COUNTER_BYTES);
 
     const size_t smem = (size_t)a.wstages * 32768 + (size_t)a.xstages * xtile + 1024;
-    static bool attr_set = false;
-    if (!attr_set) {
-        CLOAK_CUDA(cudaFuncSetAttribute(gemm_tile128_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 226 * 1024));
-        attr_set = true;
-    }
-    a.early = (g_gemv_pdl && !pool->dirty) ? 1u : 0u;
+    static std::atomic<uint64_t> opted{0};
+    st = smem_opt_in(gemm_tile128_kernel, 226 * 1024, pool->device, opted);
+    if (st != CLOAK_OK) return st;
+    const bool pdl = g_gemv_pdl.load(std::memory_order_relaxed);
+    a.early = (pdl && !pool->dirty) ? 1u : 0u;
     if (pool->dirty && pool->dirty_stream == s) pool->dirty = false;   // this launch waits for the writer in full
     cudaLaunchConfig_t cfg = {};
     cfg.gridDim = dim3(ctas);
@@ -616,7 +616,7 @@ static cloak_status gemm_launch(const cloak_pool* pool, const cloak_gemm_op* ops
     at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
     at[0].val.programmaticStreamSerializationAllowed = 1;
     cfg.attrs = at;
-    cfg.numAttrs = g_gemv_pdl ? 1 : 0;
+    cfg.numAttrs = pdl ? 1 : 0;
     CLOAK_CUDA(cudaLaunchKernelEx(&cfg, gemm_tile128_kernel, pool->tmap_tile128, a));
     launched();
     return CLOAK_OK;
@@ -629,8 +629,8 @@ using namespace cloak;
 extern "C" cloak_status cloak_set_gemm_schedule(int static_pct, int dyn_chunk_tiles) {
     if (static_pct < 0 || static_pct > 100 || dyn_chunk_tiles < 0 || dyn_chunk_tiles > 4096)
         return fail(CLOAK_ERR_INVALID, "set_gemm_schedule: static_pct in 0..100, dyn_chunk_tiles in 0..4096");
-    g_static_pct = static_pct;
-    g_dchunk = dyn_chunk_tiles;
+    g_static_pct.store(static_pct);
+    g_dchunk.store(dyn_chunk_tiles);
     return CLOAK_OK;
 }
 
@@ -669,6 +669,37 @@ extern "C" cloak_status cloak_gemm(const cloak_pool* pool, const cloak_tensor* w
     op.d_x = d_x;
     op.d_y = d_y;
     return gemm_launch(pool, &op, 1, batch, (cudaStream_t)stream);
+}
+
+extern "C" cloak_status cloak_gemm_chain_scratch_bytes(const cloak_pool* pool, const cloak_gemm_op* h_ops, uint32_t n_ops,
+                                                       uint32_t batch, uint64_t* h_bytes) {
+    if (!h_ops || n_ops == 0 || !h_bytes) return fail(CLOAK_ERR_INVALID, "gemm_chain_scratch_bytes: NULL argument or no ops");
+    for (uint32_t i = 0; i < n_ops; ++i) {
+        cloak_status st = gemm_check(pool, &h_ops[i].w, h_ops[i].d_x, h_ops[i].d_y, batch, "gemm_chain_scratch_bytes");
+        if (st != CLOAK_OK) return st;
+    }
+    const int sms = sm_count(pool->device);
+    const uint32_t cols = (batch + 15) & ~15u;
+    uint64_t need = 0;
+    for (uint32_t i = 0; i < n_ops;) {                      // the same split into launches as cloak_gemm_chain
+        uint32_t n = 0, Ns[GM_MAX_OPS], Ks[GM_MAX_OPS];
+        uint64_t rows = 0;
+        while (i + n < n_ops && n < (uint32_t)GM_MAX_OPS && rows + h_ops[i + n].w.N / 128 <= GM_MAX_ROWS) {
+            Ns[n] = h_ops[i + n].w.N;
+            Ks[n] = h_ops[i + n].w.K;
+            rows += h_ops[i + n++].w.N / 128;
+        }
+        if (n == 0) return fail(CLOAK_ERR_UNSUPPORTED, "gemm_chain_scratch_bytes: op %u has too many output rows", i);
+        GemmArgs a;
+        uint32_t ctas = 0;
+        cloak_status st = gemm_plan(a, Ns, Ks, n, cols, sms, &ctas, &rows);
+        if (st != CLOAK_OK) return st;
+        const uint64_t b = WS_COUNTER_BYTES + ((uint64_t)ctas + a.ndyn) * 2 * cols * 128 * 4;
+        if (b > need) need = b;
+        i += n;
+    }
+    *h_bytes = need;
+    return CLOAK_OK;
 }
 
 extern "C" cloak_status cloak_gemm_chain(const cloak_pool* pool, const cloak_gemm_op* h_ops, uint32_t n_ops, uint32_t batch,

@@ -236,26 +236,31 @@ cloak_status check_linear(const cloak_pool* pool, const cloak_tensor* w, const v
     return CLOAK_OK;
 }
 
-// Library-owned scratch of a pool: WS_COUNTER_BYTES of self-resetting split-K counters (zeroed on
-// (re)allocation) followed by fp32 partials.  Grown on demand.  Calls that use it on one pool must be
-// stream-ordered with respect to each other.
-cloak_status pool_workspace(const cloak_pool* pool, size_t bytes) {
+// Library-owned scratch of a pool: WS_COUNTER_BYTES of self-resetting split-K counters (zeroed when allocated) followed
+// by fp32 partials.  Calls that use it on one pool must be stream-ordered with respect to each other.  Growth happens in
+// the order of stream `s`: the new buffer is allocated and its counters zeroed on s, the old one is freed on s, so
+// kernels already queued keep theirs; nothing synchronises.  Impossible while s is being captured into a graph (the
+// buffer would belong to the graph): cloak_pool_reserve_workspace beforehand.
+cloak_status pool_workspace(const cloak_pool* pool, size_t bytes, cudaStream_t s) {
     if (pool->ws_bytes >= bytes) return CLOAK_OK;
-    if (pool->ws) {
-        CLOAK_CUDA(cudaDeviceSynchronize());
-        cudaFree(pool->ws);
-        pool->ws = nullptr;
-        pool->ws_bytes = 0;
-    }
-    size_t want = bytes < (8u << 20) ? (8u << 20) : bytes;
-    CLOAK_CUDA(cudaMalloc((void**)&pool->ws, want));
-    CLOAK_CUDA(cudaMemset(pool->ws, 0, WS_COUNTER_BYTES));
+    cudaStreamCaptureStatus cap = cudaStreamCaptureStatusNone;
+    if (cudaStreamIsCapturing(s, &cap) != cudaSuccess) cudaGetLastError();
+    if (cap != cudaStreamCaptureStatusNone)
+        return fail(CLOAK_ERR_INVALID, "this call needs %zu bytes of pool scratch (the pool has %zu) and the stream is being captured: "
+                                       "call cloak_pool_reserve_workspace before the capture", bytes, pool->ws_bytes);
+    const size_t want = bytes < WS_DEFAULT_BYTES ? WS_DEFAULT_BYTES : bytes;
+    void* nw = nullptr;
+    cloak_status st = async_alloc(&nw, want, s);
+    if (st != CLOAK_OK) return st;
+    CLOAK_CUDA(cudaMemsetAsync(nw, 0, WS_COUNTER_BYTES, s));
+    if (pool->ws) CLOAK_CUDA(cudaFreeAsync(pool->ws, s));
+    pool->ws = static_cast<char*>(nw);
     pool->ws_bytes = want;
     return CLOAK_OK;
 }
 
-static bool g_force_oneshot = false;     // A/B switch (cloak_set_gemv_engine)
-extern bool g_gemv_pdl;                   // gemv_stream.cu
+static std::atomic<bool> g_force_oneshot{false};     // A/B switch (cloak_set_gemv_engine)
+extern std::atomic<bool> g_gemv_pdl;                 // gemv_stream.cu
 
 static cloak_status gemv_device(const cloak_pool* pool, const cloak_tensor* w, const void* d_x, void* d_y, uint32_t batch,
                                 cudaStream_t s) {
@@ -291,7 +296,7 @@ static cloak_status gemv_device(const cloak_pool* pool, const cloak_tensor* w, c
         if (S > 1) {
             if (tiles > GV_MAX_TILES) return fail(CLOAK_ERR_UNSUPPORTED, "gemv: N too large for the split-K counters");
             const size_t need = WS_COUNTER_BYTES + (size_t)S * batch * w->N * 4;
-            cloak_status st = pool_workspace(pool, need);
+            cloak_status st = pool_workspace(pool, need, s);
             if (st != CLOAK_OK) return st;
             counters = reinterpret_cast<uint32_t*>(pool->ws);
             part = reinterpret_cast<float*>(pool->ws + WS_COUNTER_BYTES);
@@ -383,6 +388,26 @@ extern "C" cloak_status cloak_gemv_chain(const cloak_pool* pool, const cloak_gem
     return CLOAK_OK;
 }
 
+extern "C" cloak_status cloak_gemv_chain_scratch_bytes(const cloak_pool* pool, const cloak_gemv_op* h_ops, uint32_t n_ops,
+                                                       uint32_t batch, uint64_t* h_bytes) {
+    if (!h_ops || n_ops == 0 || !h_bytes) return fail(CLOAK_ERR_INVALID, "gemv_chain_scratch_bytes: NULL argument or no ops");
+    uint64_t need = 0;
+    const uint64_t sms = (uint64_t)sm_count(pool ? pool->device : 0);
+    for (uint32_t i = 0; i < n_ops; ++i) {
+        const cloak_tensor& w = h_ops[i].w;
+        cloak_status st = gemv_check(pool, &w, h_ops[i].d_x, h_ops[i].d_y, batch, "gemv_chain_scratch_bytes");
+        if (st != CLOAK_OK) return st;
+        uint64_t b = 0;
+        if (!g_force_oneshot.load(std::memory_order_relaxed) && gemv_stream_chunk(pool, &w, batch) >= 1)
+            b = WS_COUNTER_BYTES + 48ull * sms * batch * 8 * 4;          // a full launch of the streaming kernel: one cut-tile partial per (op, CTA)
+        else if (w.dt == CLOAK_BF16 && (w.K + GV_KCTA - 1) / GV_KCTA > 1)
+            b = WS_COUNTER_BYTES + (uint64_t)((w.K + GV_KCTA - 1) / GV_KCTA) * batch * w.N * 4;
+        if (b > need) need = b;
+    }
+    *h_bytes = need;
+    return CLOAK_OK;
+}
+
 extern "C" cloak_status cloak_gemv_host(const cloak_pool* pool, const cloak_tensor* w, const void* h_x, void* h_y,
                                         uint32_t batch, void* stream) {
     cloak_status st = gemv_check(pool, w, h_x, h_y, batch, "gemv_host");
@@ -392,17 +417,14 @@ extern "C" cloak_status cloak_gemv_host(const cloak_pool* pool, const cloak_tens
     const size_t e = w->dt == CLOAK_F32 ? 4 : 2;
     const size_t xb = (size_t)batch * w->K * e, yb = (size_t)batch * w->N * e;
     const size_t xpad = (xb + 255) & ~(size_t)255;
-    char* buf = nullptr;
-    CLOAK_CUDA(cudaMallocAsync((void**)&buf, xpad + yb, s));
-    cudaError_t err = cudaMemcpyAsync(buf, h_x, xb, cudaMemcpyHostToDevice, s);
-    if (err == cudaSuccess) {
-        st = gemv_device(pool, w, buf, buf + xpad, batch, s);
-        if (st == CLOAK_OK) err = cudaMemcpyAsync(h_y, buf + xpad, yb, cudaMemcpyDeviceToHost, s);
-    }
-    cudaFreeAsync(buf, s);
-    cudaError_t e2 = cudaStreamSynchronize(s);
+    AsyncBuf buf(s);                            // from the library's cached pool: no driver allocation after the first call
+    st = buf.alloc(xpad + yb);
     if (st != CLOAK_OK) return st;
-    if (err != cudaSuccess) return fail(CLOAK_ERR_CUDA, "gemv_host copy: %s", cudaGetErrorString(err));
-    if (e2 != cudaSuccess) return fail(CLOAK_ERR_CUDA, "gemv_host sync: %s", cudaGetErrorString(e2));
+    char* d = static_cast<char*>(buf.p);
+    CLOAK_CUDA(cudaMemcpyAsync(d, h_x, xb, cudaMemcpyHostToDevice, s));
+    st = gemv_device(pool, w, d, d + xpad, batch, s);
+    if (st != CLOAK_OK) return st;
+    CLOAK_CUDA(cudaMemcpyAsync(h_y, d + xpad, yb, cudaMemcpyDeviceToHost, s));
+    CLOAK_CUDA(cudaStreamSynchronize(s));       // h_y is the caller's to read when the call returns
     return CLOAK_OK;
 }

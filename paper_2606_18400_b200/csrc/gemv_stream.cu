@@ -414,30 +414,55 @@ __global__ void __launch_bounds__(gs_threads(NT), 1) gemv_chain_kernel(const __g
     }
 }
 
-bool g_gemv_pdl = true;      // A/B switch (cloak_set_gemv_engine(2) turns PDL off)
+std::atomic<bool> g_gemv_pdl{true};      // A/B switch (cloak_set_gemv_engine(2) turns PDL off)
 
 // Counter words [0, GS_TILE_COUNTERS) of the pool's scratch are row-tile arrival counters, the rest op barriers.
 constexpr uint32_t GS_TILE_COUNTERS = (uint32_t)(WS_COUNTER_BYTES / 4) - 4 * GS_MAX_OPS;
 
+// Co-residency.  The CTAs of this kernel wait for one another (the owner of a cut row tile for the later contributors'
+// partials; the consumers of an `after` op for every CTA's arrival), so all of them must be on the machine at once.  One CTA
+// fits per SM (shared memory), and the grid is never larger than the SM count -- but another kernel holding SMs (a second
+// pool's chain on another stream, a framework kernel, an MPS / green-context SM limit) would leave some CTAs unscheduled and
+// the resident ones spinning for ever.  The launch is therefore COOPERATIVE: the driver starts the grid only when every CTA
+// can be resident, and fails the launch (cudaErrorCooperativeLaunchTooLarge) instead of hanging when that can never be.
+// Whether the cooperative attribute may be combined with programmatic stream serialization is probed on the first launch:
+// if the driver rejects the pair, PDL is dropped, not the guarantee.
+static std::atomic<int> g_coop_with_pdl{-1};     // -1 unknown, 0 rejected, 1 accepted
+
 template <int CU, int NT>
-static cloak_status launch(const ChainArgs& a, int ctas, cudaStream_t s) {
+static cloak_status launch(const ChainArgs& a, int ctas, int device, cudaStream_t s) {
     constexpr size_t smem = (size_t)gs_stages(CU) * GS_ROWS * (CU * 512u + GS_PAD);
-    static bool attr_set = false;
-    if (!attr_set) {
-        CLOAK_CUDA(cudaFuncSetAttribute(gemv_chain_kernel<CU, NT>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-        attr_set = true;
-    }
+    static std::atomic<uint64_t> opted{0};
+    auto* kernel = gemv_chain_kernel<CU, NT>;
+    cloak_status st = smem_opt_in(kernel, smem, device, opted);
+    if (st != CLOAK_OK) return st;
     cudaLaunchConfig_t cfg = {};
     cfg.gridDim = dim3(ctas);
     cfg.blockDim = dim3(gs_threads(NT));
     cfg.dynamicSmemBytes = smem;
     cfg.stream = s;
-    cudaLaunchAttribute at[1];
-    at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
-    at[0].val.programmaticStreamSerializationAllowed = 1;
+    cudaLaunchAttribute at[2];
+    at[0].id = cudaLaunchAttributeCooperative;
+    at[0].val.cooperative = 1;
+    at[1].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    at[1].val.programmaticStreamSerializationAllowed = 1;
     cfg.attrs = at;
-    cfg.numAttrs = g_gemv_pdl ? 1 : 0;
-    CLOAK_CUDA(cudaLaunchKernelEx(&cfg, gemv_chain_kernel<CU, NT>, a));
+    const bool want_pdl = g_gemv_pdl.load(std::memory_order_relaxed) && g_coop_with_pdl.load(std::memory_order_relaxed) != 0;
+    cfg.numAttrs = want_pdl ? 2 : 1;
+    cudaError_t e = cudaLaunchKernelEx(&cfg, kernel, a);
+    if (e != cudaSuccess && want_pdl && g_coop_with_pdl.load(std::memory_order_relaxed) < 0 &&
+        (e == cudaErrorInvalidValue || e == cudaErrorNotSupported || e == cudaErrorInvalidConfiguration)) {
+        cudaGetLastError();
+        g_coop_with_pdl.store(0, std::memory_order_relaxed);
+        cfg.numAttrs = 1;
+        e = cudaLaunchKernelEx(&cfg, kernel, a);
+    } else if (e == cudaSuccess && want_pdl) {
+        g_coop_with_pdl.store(1, std::memory_order_relaxed);
+    }
+    if (e != cudaSuccess) {
+        cudaGetLastError();
+        return fail(CLOAK_ERR_CUDA, "gemv chain launch (%d cooperative CTAs): %s", ctas, cudaGetErrorString(e));
+    }
     launched();
     return CLOAK_OK;
 }
@@ -518,18 +543,18 @@ cloak_status gemv_stream_launch(const cloak_pool* pool, const cloak_gemv_op* ops
         ranges_so_far += o.ctas;
     }
     const size_t need = WS_COUNTER_BYTES + (size_t)n * ctas * batch * GS_ROWS * 4;
-    cloak_status st = pool_workspace(pool, need);
+    cloak_status st = pool_workspace(pool, need, s);
     if (st != CLOAK_OK) return st;
     a.counters = reinterpret_cast<uint32_t*>(pool->ws);
     a.opsync = a.counters + GS_TILE_COUNTERS;
     a.part = reinterpret_cast<float*>(pool->ws + WS_COUNTER_BYTES);
-    a.early = (g_gemv_pdl && !pool->dirty) ? 1u : 0u;
+    a.early = (g_gemv_pdl.load(std::memory_order_relaxed) && g_coop_with_pdl.load(std::memory_order_relaxed) != 0 && !pool->dirty) ? 1u : 0u;
     if (pool->dirty && pool->dirty_stream == s) pool->dirty = false;   // this launch waits for the writer in full
     const bool nt2 = batch > 8;
-#define GS_CASE(C) case C: return nt2 ? launch<C, 2>(a, ctas, s) : launch<C, 1>(a, ctas, s)
+#define GS_CASE(C) case C: return nt2 ? launch<C, 2>(a, ctas, pool->device, s) : launch<C, 1>(a, ctas, pool->device, s)
     switch (cu) {
         GS_CASE(8); GS_CASE(7); GS_CASE(6); GS_CASE(5); GS_CASE(4); GS_CASE(3); GS_CASE(2);
-        default: return nt2 ? launch<1, 2>(a, ctas, s) : launch<1, 1>(a, ctas, s);
+        default: return nt2 ? launch<1, 2>(a, ctas, pool->device, s) : launch<1, 1>(a, ctas, pool->device, s);
     }
 #undef GS_CASE
 }

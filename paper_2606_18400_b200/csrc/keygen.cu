@@ -149,21 +149,10 @@ cloak_status keygen_device(uint64_t key, uint64_t stream_id, uint32_t n, uint32_
     const uint32_t nbuckets = 1u << bits;
     const size_t keys_b = (size_t)n * 8, idx_b = (size_t)n * 4, tab_b = ((size_t)nbuckets + 1) * 4;
     const size_t total = keys_b + idx_b + 2 * tab_b;
-    char* ws = nullptr;
-    {   // keep freed workspace cached in the stream-ordered pool instead of returning it to the OS at every sync
-        static bool tuned = false;
-        if (!tuned) {
-            int dev = 0;
-            cudaMemPool_t mp;
-            if (cudaGetDevice(&dev) == cudaSuccess && cudaDeviceGetDefaultMemPool(&mp, dev) == cudaSuccess) {
-                uint64_t keep = ~0ull;
-                cudaMemPoolSetAttribute(mp, cudaMemPoolAttrReleaseThreshold, &keep);
-            }
-            cudaGetLastError();
-            tuned = true;
-        }
-    }
-    CLOAK_CUDA(cudaMallocAsync((void**)&ws, total, s));
+    AsyncBuf buf(s);                     // released on every exit path
+    cloak_status ast = buf.alloc(total);
+    if (ast != CLOAK_OK) return ast;
+    char* ws = static_cast<char*>(buf.p);
     uint64_t* bk = (uint64_t*)ws;
     uint32_t* bi = (uint32_t*)(ws + keys_b);
     uint32_t* base = (uint32_t*)(ws + keys_b + idx_b);           // hist, then (scanned in place) base[0 .. nbuckets]
@@ -179,7 +168,6 @@ cloak_status keygen_device(uint64_t key, uint64_t stream_id, uint32_t n, uint32_
     bucket_rank_kernel<<<grid, 256, 0, s>>>(n, shift, base, bk, bi, d_perm, d_inv);
     launched();
     CLOAK_LAUNCH_CHECK();
-    CLOAK_CUDA(cudaFreeAsync(ws, s));
     return CLOAK_OK;
 }
 

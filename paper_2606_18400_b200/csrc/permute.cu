@@ -251,11 +251,12 @@ static cloak_status rows(const void* src, Dst dst, const uint32_t* map, uint32_t
 template <typename E, typename M, typename Dst>
 static cloak_status cols_ring(const void* src, Dst dst, const uint32_t* map, uint32_t seg, uint32_t nrows, uint32_t ncols,
                               size_t smem, uint32_t ns, int sms, cudaStream_t s) {
-    static bool attr_set = false;
-    if (!attr_set) {
-        CLOAK_CUDA(cudaFuncSetAttribute(gather_cols_kernel<E, M, Dst>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024));
-        attr_set = true;
-    }
+    static std::atomic<uint64_t> opted{0};
+    auto* kernel = gather_cols_kernel<E, M, Dst>;
+    int dev = 0;
+    CLOAK_CUDA(cudaGetDevice(&dev));
+    cloak_status ost = smem_opt_in(kernel, 200 * 1024, dev, opted);
+    if (ost != CLOAK_OK) return ost;
     const uint32_t ctas = nrows < (uint32_t)sms ? nrows : (uint32_t)sms;
     gather_cols_kernel<E, M, Dst><<<ctas, 512, smem, s>>>((const E*)src, dst, map, seg, nrows, ncols, ns);
     launched();
@@ -354,8 +355,9 @@ static cloak_status permute_impl(uint64_t key, const cloak_block_shape* sh, cons
     const uint32_t e = sh->dt == CLOAK_F32 ? 4 : 2;
     const int sms = sm_count(dev);
     const size_t n_scratch = (size_t)(mlp ? sh->inter : 0) + (heads ? sh->n_kv + sh->n_q : 0);
-    uint32_t* scratch = nullptr;
-    CLOAK_CUDA(cudaMallocAsync((void**)&scratch, n_scratch * 4, s));
+    AsyncBuf sbuf(s);
+    if (cloak_status ast = sbuf.alloc(n_scratch * 4)) return ast;
+    uint32_t* scratch = static_cast<uint32_t*>(sbuf.p);
     uint32_t* pi = scratch;
     uint32_t* kappa = scratch + (mlp ? sh->inter : 0);
     uint32_t* eta = kappa + sh->n_kv;
@@ -394,8 +396,7 @@ static cloak_status permute_impl(uint64_t key, const cloak_block_shape* sh, cons
     }
     if (forked) cudaEventRecord(fj.join, fj.aux);
     if (forked) cudaStreamWaitEvent(s, fj.join, 0);                // join: everything after this call sees both paths done
-    cudaFreeAsync(scratch, s);
-    return st;
+    return st;                                                     // (sbuf is freed on s, behind the join)
 }
 
 // Zero the rest of the block that holds arena byte `end` (G4: the tail of a tensor's last block is zero).
@@ -498,8 +499,9 @@ extern "C" cloak_status cloak_permute_experts(uint64_t key, const cloak_moe_shap
     // eps on the host (to walk the experts) and on the device (to gather the router's rows): the same Philox keygen
     std::vector<uint32_t> eps;
     keygen_host(key, (7ull << 32) | sh->layer, E, eps);
-    uint32_t* scratch = nullptr;
-    CLOAK_CUDA(cudaMallocAsync((void**)&scratch, ((size_t)E + I) * 4, s));
+    AsyncBuf sbuf(s);
+    if (cloak_status ast = sbuf.alloc(((size_t)E + I) * 4)) return ast;
+    uint32_t* scratch = static_cast<uint32_t*>(sbuf.p);
     uint32_t* d_eps = scratch;
     uint32_t* d_pi = scratch + E;
     cloak_status st = keygen_device(key, (7ull << 32) | sh->layer, E, d_eps, nullptr, s);
@@ -518,7 +520,6 @@ extern "C" cloak_status cloak_permute_experts(uint64_t key, const cloak_moe_shap
             st = e == 4 ? cols<uint32_t>(d, dd, d_pi, 1, H, I, sms, s) : cols<uint16_t>(d, dd, d_pi, 1, H, I, sms, s);
         }
     }
-    cudaFreeAsync(scratch, s);
     return st;
 }
 

@@ -181,6 +181,9 @@ static cloak_status create_impl(cloak_pool* p) {
             CLOAK_CUDA(cudaMalloc((void**)&p->base, p->bytes()));
         }
         CLOAK_CUDA(cudaMemsetAsync(p->base, 0, p->bytes(), s));
+        // scratch of the GEMV / GEMM calls: there from the start, so that no compute call allocates or synchronises
+        cloak_status e = pool_workspace(p, WS_DEFAULT_BYTES, s);
+        if (e != CLOAK_OK) return e;
         CLOAK_CUDA(cudaStreamSynchronize(s));
         return CLOAK_OK;
     };
@@ -278,23 +281,38 @@ extern "C" cloak_status cloak_pool_dump(const cloak_pool* pool, void* d_out, voi
     return CLOAK_OK;
 }
 
-extern "C" cloak_status cloak_pool_adjacency(const cloak_pool* pool, double* va_blocks, double* physical_blocks, double* pages) {
+extern "C" cloak_status cloak_pool_adjacency(const cloak_pool* pool, double* va_blocks, double* physical_blocks, double* pages,
+                                             void* stream) {
     using namespace cloak;
     if (!pool) return fail(CLOAK_ERR_INVALID, "pool_adjacency: NULL pool");
     DeviceGuard g(pool->device);
-    unsigned long long* d = nullptr;
-    CLOAK_CUDA(cudaMalloc((void**)&d, 3 * sizeof(unsigned long long)));
-    cudaMemset(d, 0, 3 * sizeof(unsigned long long));
+    cudaStream_t s = (cudaStream_t)stream;
+    AsyncBuf buf(s);
+    if (cloak_status ast = buf.alloc(3 * sizeof(unsigned long long))) return ast;
+    unsigned long long* d = static_cast<unsigned long long*>(buf.p);
+    CLOAK_CUDA(cudaMemsetAsync(d, 0, 3 * sizeof(unsigned long long), s));
     const uint32_t n = pool->nb > pool->npages ? pool->nb : pool->npages;
-    adjacency_kernel<<<(n + 255) / 256, 256>>>(pool->d_blockinv, pool->d_pageinv, pool->nb, pool->bpp, pool->npages, d);
+    adjacency_kernel<<<(n + 255) / 256, 256, 0, s>>>(pool->d_blockinv, pool->d_pageinv, pool->nb, pool->bpp, pool->npages, d);
     launched();
+    CLOAK_LAUNCH_CHECK();
     unsigned long long h[3] = {0, 0, 0};
-    cudaError_t e = cudaMemcpy(h, d, sizeof(h), cudaMemcpyDeviceToHost);
-    cudaFree(d);
-    if (e != cudaSuccess) return fail(CLOAK_ERR_CUDA, "pool_adjacency: %s", cudaGetErrorString(e));
+    CLOAK_CUDA(cudaMemcpyAsync(h, d, sizeof(h), cudaMemcpyDeviceToHost, s));
+    CLOAK_CUDA(cudaStreamSynchronize(s));
     if (va_blocks) *va_blocks = pool->nb > 1 ? (double)h[0] / (pool->nb - 1) : 0.0;
     if (physical_blocks) *physical_blocks = pool->nb > 1 ? (double)h[1] / (pool->nb - 1) : 0.0;
     if (pages) *pages = pool->npages > 1 ? (double)h[2] / (pool->npages - 1) : 0.0;
+    return CLOAK_OK;
+}
+
+extern "C" cloak_status cloak_pool_reserve_workspace(cloak_pool* pool, uint64_t bytes) {
+    using namespace cloak;
+    if (!pool) return fail(CLOAK_ERR_INVALID, "pool_reserve_workspace: NULL pool");
+    if (pool->ws_bytes >= bytes) return CLOAK_OK;
+    DeviceGuard g(pool->device);
+    CLOAK_CUDA(cudaDeviceSynchronize());                 // nothing in flight holds the old scratch
+    cloak_status st = pool_workspace(pool, bytes, nullptr);
+    if (st != CLOAK_OK) return st;
+    CLOAK_CUDA(cudaDeviceSynchronize());                 // the new counters are zero before any stream can use them
     return CLOAK_OK;
 }
 

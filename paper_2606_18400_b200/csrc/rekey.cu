@@ -90,17 +90,6 @@ __global__ void __launch_bounds__(RK_WARPS * 32) rekey_moves_kernel(RekeyArgs a)
 
 using namespace cloak;
 
-namespace {
-// stream-ordered allocation that is released on every exit path
-struct AsyncBuf {
-    void* p = nullptr;
-    cudaStream_t s;
-    explicit AsyncBuf(cudaStream_t st) : s(st) {}
-    ~AsyncBuf() { if (p) cudaFreeAsync(p, s); }
-    cudaError_t alloc(size_t bytes) { return cudaMallocAsync(&p, bytes, s); }
-};
-}  // namespace
-
 extern "C" cloak_status cloak_rekey_inplace(cloak_pool* pool, uint64_t new_key, uint64_t spare_bytes, void* stream) {
     if (!pool) return fail(CLOAK_ERR_INVALID, "rekey_inplace: NULL pool");
     if (pool->flags & CLOAK_POOL_IDENTITY) return fail(CLOAK_ERR_INVALID, "rekey_inplace: an identity pool has no key");
@@ -111,7 +100,7 @@ extern "C" cloak_status cloak_rekey_inplace(cloak_pool* pool, uint64_t new_key, 
 
     // ---- new block tables on the device, both block tables on the host
     AsyncBuf new_tables(s), work(s);
-    CLOAK_CUDA(new_tables.alloc((size_t)2 * n * 4));
+    if (cloak_status ast = new_tables.alloc((size_t)2 * n * 4)) return ast;
     uint32_t* d_new = static_cast<uint32_t*>(new_tables.p);    // blockperm_B | blockinv_B
     cloak_status st = keygen_device(new_key, 1ull << 32, n, d_new, d_new + n, s);
     if (st != CLOAK_OK) return st;
@@ -168,7 +157,7 @@ extern "C" cloak_status cloak_rekey_inplace(cloak_pool* pool, uint64_t new_key, 
     }
     const size_t mv_b = moves.size() * sizeof(uint2), st_b = start.size() * 4, sp_b = (size_t)nseg * b;
     const size_t mv_pad = (mv_b + 255) & ~(size_t)255, st_pad = (st_b + 255) & ~(size_t)255;
-    CLOAK_CUDA(work.alloc(mv_pad + st_pad + sp_b));
+    if (cloak_status ast = work.alloc(mv_pad + st_pad + sp_b)) return ast;
     char* d_buf = static_cast<char*>(work.p);
     CLOAK_CUDA(cudaMemcpyAsync(d_buf, moves.data(), mv_b, cudaMemcpyHostToDevice, s));
     CLOAK_CUDA(cudaMemcpyAsync(d_buf + mv_pad, start.data(), st_b, cudaMemcpyHostToDevice, s));
@@ -179,11 +168,8 @@ extern "C" cloak_status cloak_rekey_inplace(cloak_pool* pool, uint64_t new_key, 
     a.log2b = pool->log2_block;
     a.log2c = pool->log2_block < 13 ? pool->log2_block : 13;
     const size_t smem = (size_t)RK_WARPS * RK_STAGES << a.log2c;
-    static bool attr_set = false;
-    if (!attr_set) {
-        CLOAK_CUDA(cudaFuncSetAttribute(rekey_moves_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024));
-        attr_set = true;
-    }
+    static std::atomic<uint64_t> opted{0};
+    if (cloak_status ost = smem_opt_in(rekey_moves_kernel, 200 * 1024, pool->device, opted)) return ost;
     pool->wrote(s);
     for (int pass = 0; pass < 2; ++pass) {
         a.pipe_start = reinterpret_cast<const uint32_t*>(d_buf + mv_pad) + pass * (npipes + 1);

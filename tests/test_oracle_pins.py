@@ -1,11 +1,12 @@
 """Pins of the CPU oracle against things other than itself.  All CPU-only."""
 import ctypes
+import os
 import glob
 import numpy as np
 import pytest
 
 import oracle as O
-from util import fnv1a64_u32, worked, philox_kat
+from util import GOLDEN, fnv1a64_u32, worked, philox_kat
 
 
 # ---------------------------------------------------------------- O1 Philox
@@ -306,6 +307,28 @@ def test_mlp_function_preserved_fp64_and_rows_bit_exact():
     assert np.max(np.abs(y - yw)) > 1e-3
 
 
+def test_attention_closed_forms():
+    """Pins of attention_f64 that a symmetric mistake (wrong scale, missing causal mask) would not survive -- invariance
+    under the head permutation alone would.  H = 1 input feature, one head of d = 4, q = k = ones so that
+    Q_i . K_j = 4 x_i x_j and the scaled score is 4 x_i x_j / sqrt(4) = 2 x_i x_j; v = e_0, o = e_0^T so the output is the
+    softmax-weighted mean of x itself.  Token 0 sees only itself (causal): out_0 = x_0 whatever the scores."""
+    a, b = 0.3, -1.1
+    x = np.array([[a], [b]])
+    q = np.ones((4, 1))
+    k = np.ones((4, 1))
+    v = np.array([[1.0], [0.0], [0.0], [0.0]])
+    o = np.array([[1.0, 0.0, 0.0, 0.0]])
+    y = O.attention_f64(x, q, k, v, o, 1, 1, 4)
+    import math
+    w0, w1 = math.exp(2 * b * a), math.exp(2 * b * b)
+    assert abs(y[0, 0] - a) < 1e-15
+    assert abs(y[1, 0] - (w0 * a + w1 * b) / (w0 + w1)) < 1e-15
+    # grouped KV: 2 query heads share 1 KV head; zero queries -> uniform softmax -> running mean of V
+    x3 = np.array([[1.0], [2.0], [6.0]])
+    y3 = O.attention_f64(x3, np.zeros((8, 1)), np.ones((4, 1)), v, np.array([[1.0, 0, 0, 0, 1.0, 0, 0, 0]]), 2, 1, 4)
+    assert np.allclose(y3[:, 0], 2 * np.array([1.0, 1.5, 3.0]), rtol=0, atol=1e-15)
+
+
 def test_attention_function_preserved_fp64():
     rng = np.random.default_rng(1)
     H, n_q, n_kv, d, t = 32, 4, 2, 8, 5
@@ -372,6 +395,20 @@ def test_error_measures():
     assert abs(O.err_elementwise_floored(y, yr) - 0.001 / rms) < 1e-15
 
 
+def test_adjacent_fraction_brute_force_counts_ascending_neighbours_only():
+    """A hand-written table with ascending pairs (7,8) (2,3) (9,10), DESCENDING pairs (5,4) (1,0) and gaps: only
+    T[i+1] == T[i] + 1 counts (G8; cloak.h cloak_pool_adjacency).  Counting |delta| == 1 would give 5/9, T[i+1] == T[i] - 1
+    would give 2/9."""
+    T = [5, 4, 7, 8, 2, 3, 1, 0, 9, 10]
+    brute = sum(1 for i in range(len(T) - 1) if T[i + 1] == T[i] + 1)          # python ints, the definition
+    assert brute == 3
+    assert O.adjacent_fraction(np.array(T, dtype=np.uint32)) == 3 / 9
+    assert O.adjacent_fraction(np.array(T[::-1], dtype=np.uint32)) == 2 / 9    # reversed: only (0,1) and (4,5) ascend
+    assert O.adjacent_fraction(np.array([3], dtype=np.uint32)) == 0.0
+    # uint32 inputs must not wrap: 0 followed by 0xffffffff is not "adjacent"
+    assert O.adjacent_fraction(np.array([0, 0xFFFFFFFF, 0], dtype=np.uint32)) == 0.0
+
+
 def test_adjacent_fraction_is_about_one_over_n():
     g = O.pool_geometry(1 << 20, 4096, 65536)
     t = O.pool_tables(0x1234, g)
@@ -401,6 +438,26 @@ def test_moe_expert_permutation_preserves_the_function():
     # every permuted expert is the old one with its OWN neuron permutation (row pin)
     e_old = int(eps[1])
     assert np.array_equal(g2[1][0], gate[e_old][int(pis[e_old][0])]) and np.array_equal(r2[1], router[e_old])
+
+
+def test_moe_streams_reproduce_the_stored_worked_example():
+    """eps and pi_e for stored (key, layer, E, e): values written by tests/golden/make_moe_example.py, a pure-Python-int
+    restatement of Philox + sort that shares nothing with oracle/ (a wrong stream id, a swapped layer*E + e, or eps used
+    where its inverse belongs would change them)."""
+    import json
+    with open(os.path.join(GOLDEN, "moe_example.json")) as f:
+        ex = json.load(f)
+    key = int(ex["key"], 16)
+    for c in ex["cases"]:
+        eps = O.expert_perm(key, c["layer"], c["n_experts"])
+        assert eps[:8].tolist() == c["eps_head"][:8] and fnv1a64_u32(eps) == c["fnv_eps"]
+        if "eps" in c:
+            assert eps.tolist() == c["eps"]
+        for p in c["pi"]:
+            pi = O.expert_mlp_perm(key, c["layer"], c["n_experts"], p["expert"], c["inter"])
+            assert pi[:8].tolist() == p["head"] and fnv1a64_u32(pi) == p["fnv"]
+            if "perm" in p:
+                assert pi.tolist() == p["perm"]
 
 
 def test_moe_reduces_to_the_dense_mlp_and_topk_is_a_sort():
