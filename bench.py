@@ -30,10 +30,9 @@ import numpy as np  # noqa: E402
 METRIC = "shuffle GB/s and cloaked decode GEMV GB/s (frac of HBM peak); cloaked-vs-native overhead %"
 BATCHES = (1, 4, 16)
 KEY_A, KEY_B = 0x1234, 0x5678          # G11
-# dram__bytes_read.sum + dram__bytes_write.sum of one gemv_chain_kernel launch (the 7 projections at one batch), mean of
-# the three launches of a step in the committed `ncu --set full` capture; algorithmic bytes are 436 207 616.
-NCU_TRAFFIC_PER_LAUNCH = 442.2e6
-NCU_TRAFFIC_SOURCE = "profiles/r1_ncu_full_gemv_chain.md"
+# roofline.traffic: dram__bytes_read.sum + dram__bytes_write.sum of one gemv_chain_kernel launch (the 7 projections at one
+# batch; algorithmic bytes are 436 207 616), read from the kept summary of the `ncu --set full` capture of this command.
+NCU_TRAFFIC_FILE = "profiles/r2_ncu_gemv_chain_traffic.json"
 FALLBACK_HBM_GBS = 6650.0              # B200_PROFILING.md fallback when MEASURED_PEAKS.json is absent
 
 
@@ -43,6 +42,16 @@ def hbm_peak():
             return float(json.load(f)["hbm_gbs"]), "measured"
     except Exception:
         return FALLBACK_HBM_GBS, "fallback"
+
+
+def ncu_traffic():
+    """(bytes per launch, source) from the committed ncu summary, or (None, why)."""
+    try:
+        with open(os.path.join(ROOT, NCU_TRAFFIC_FILE)) as f:
+            d = json.load(f)
+        return float(d["dram_bytes_per_launch_mean"]), NCU_TRAFFIC_FILE
+    except Exception as e:          # noqa: BLE001
+        return None, f"{NCU_TRAFFIC_FILE} unreadable: {type(e).__name__}"
 
 
 def layer_tensors():
@@ -65,20 +74,37 @@ ClockSampler = importlib.import_module("paper_2606_18400_b200.clocks").ClockSamp
 
 
 # ------------------------------------------------------------------------------------------ CPU oracle arm
-ORACLE_SAMPLE = ("q", "k", "v", "o")       # the attention projections of the cfg1 layer: 84 MB of the 436 MB
+ORACLE_ATTN = ("q", "k", "v", "o")                               # the attention projections: 84 MB of the 436 MB
+ORACLE_LAYER = ("q", "k", "v", "o", "gate", "up", "down")        # the whole cfg1 layer
 
 
-def oracle_setup():
-    """Inputs of the bounded oracle sample, from the shared generator (not timed)."""
+def oracle_setup(names=ORACLE_LAYER):
+    """Inputs of the oracle arm (not timed).  They come from the shared generator: its CUDA twin when a GPU is there (the
+    numpy twin makes ~10 M elements/s, the layer has 218 M; tests/ check that the twins agree byte for byte), else numpy."""
     from synth import gen
     c, shapes = layer_tensors()
-    W = {nm: gen.synth(c["seed"], i, shp, "bf16") for i, (nm, shp) in enumerate(shapes) if nm in ORACLE_SAMPLE}
-    X = {b: gen.synth(c["seed"] + 100, b, (b, c["hidden"]), "bf16", kind=gen.KIND_NORMAL) for b in BATCHES}
+    fill = None
+    try:
+        import torch
+        if torch.cuda.is_available():
+            from synth import cuda as synth_cuda
+
+            def fill(seed, tid, shp, kind=gen.KIND_WEIGHT):
+                t = synth_cuda.fill(torch.empty(shp, dtype=torch.bfloat16, device="cuda"), seed, tid, kind=kind)
+                return t.view(torch.int16).cpu().numpy().view(np.uint16)
+    except ImportError:
+        pass
+    if fill is None:
+        def fill(seed, tid, shp, kind=gen.KIND_WEIGHT):
+            return gen.synth(seed, tid, shp, "bf16", kind=kind)
+    W = {nm: fill(c["seed"], i, shp) for i, (nm, shp) in enumerate(shapes) if nm in names}
+    X = {b: {k: fill(c["seed"] + 100, b * 2 + (k != c["hidden"]), (b, k), gen.KIND_NORMAL) for k in (c["hidden"], c["inter"])}
+         for b in BATCHES}
     return c, shapes, W, X
 
 
-def oracle_step(c, shapes, W, X):
-    """The same stages as the GPU step, restricted to ORACLE_SAMPLE, run by oracle/ as it stands."""
+def oracle_step(c, shapes, W, X, names=ORACLE_LAYER):
+    """The same stages as the GPU step over the tensors in `names`, run by oracle/ as it stands (never tuned for this)."""
     import oracle as O
     block, page = c["block"], c["page"]
     sizes = [2 * n * k for nm, (n, k) in shapes]
@@ -88,19 +114,22 @@ def oracle_step(c, shapes, W, X):
     kappa, eta = O.head_maps(KEY_A, 0, c["n_q"], c["n_kv"])
     q2, k2, v2, o2 = O.permute_heads(W["q"], W["k"], W["v"], W["o"], kappa, eta, c["head_dim"])   # S5
     P = dict(q=q2, k=k2, v=v2, o=o2)
+    if "gate" in names:
+        pi = O.mlp_perm(KEY_A, 0, c["inter"])
+        P["gate"], P["up"], P["down"] = O.permute_mlp(W["gate"], W["up"], W["down"], pi)
     off = {nm: o for (nm, _), o in zip(shapes, offs)}
     pool_a = np.zeros(g.nslots * block, np.uint8)
-    for nm in ORACLE_SAMPLE:                                                        # S4
+    for nm in names:                                                                # S4
         O.shuffle_into(pool_a, ta.T_vmm, P[nm].view(np.uint8).ravel(), off[nm], block)
-    pool_b = np.zeros(g.nslots * block, np.uint8)                                   # S8 (sample blocks only)
-    for nm in ORACLE_SAMPLE:
+    pool_b = np.zeros(g.nslots * block, np.uint8)                                   # S8 (the blocks of `names`)
+    for nm in names:
         L = O.unshuffle(pool_a, ta.T_vmm, total, block, off[nm], P[nm].size * 2)
         O.shuffle_into(pool_b, tb.T_vmm, L, off[nm], block)
     ys = []
     for b in BATCHES:                                                               # S6
-        for nm in ORACLE_SAMPLE:
-            ys.append(O.linear_f64(X[b], P[nm]))                                    # K = hidden for q, k, v, o
-    for nm in ORACLE_SAMPLE:                                                        # S4 unshuffle
+        for nm in names:
+            ys.append(O.linear_f64(X[b][P[nm].shape[1]], P[nm]))
+    for nm in names:                                                                # S4 unshuffle
         O.unshuffle(pool_a, ta.T_vmm, total, block, off[nm], P[nm].size * 2)
     return ys
 
@@ -114,27 +143,75 @@ def oracle_threads():
         return os.cpu_count() or 1
 
 
+def oracle_time(names, reps_max, budget_s, threads=None):
+    """Seconds per oracle step over `names`, at most reps_max repetitions / budget_s seconds; threads=1 limits numpy's BLAS
+    to one thread (the rest of the oracle is single-threaded Python + numpy anyway)."""
+    import contextlib
+    c, shapes, W, X = oracle_setup(names)
+    ctx = contextlib.nullcontext()
+    if threads is not None:
+        from threadpoolctl import threadpool_limits
+        ctx = threadpool_limits(limits=threads)
+    with ctx:
+        used = oracle_threads() if threads is None else threads
+        t0 = time.perf_counter()
+        reps = 0
+        while reps < 1 or (time.perf_counter() - t0 < budget_s and reps < reps_max):
+            oracle_step(c, shapes, W, X, names)
+            reps += 1
+        dt = (time.perf_counter() - t0) / reps
+    return dt, reps, used, step_bytes(shapes, names)
+
+
+def oracle_cfg3_layer(batch=32):
+    """SURVEY.md 8(d) "oracle beside it", cfg3: the fp64 contraction of ONE Qwen-32B-shaped layer's 7 projections at batch 32 on
+    the host cores (numpy BLAS, all threads), multiplied by 64 and stated as extrapolated.  The 62 GB model is never on the host."""
+    import oracle as O
+    from synth import gen
+    c = gen.CONFIGS[3]
+    shapes = gen.layer_shapes(c["hidden"], c["inter"], c["n_q"], c["n_kv"], c["head_dim"])
+    import torch
+    from synth import cuda as synth_cuda
+    t_total, nbytes = 0.0, 0
+    for i, (nm, (n, k)) in enumerate(shapes):               # tensor by tensor: a layer in fp64 would be 3.9 GB
+        W = synth_cuda.fill(torch.empty(n, k, dtype=torch.bfloat16, device="cuda"), c["seed"], i).view(torch.int16).cpu().numpy().view(np.uint16)
+        X = synth_cuda.fill(torch.empty(batch, k, dtype=torch.bfloat16, device="cuda"), c["seed"] + 100, i,
+                            kind=gen.KIND_NORMAL).view(torch.int16).cpu().numpy().view(np.uint16)
+        t0 = time.perf_counter()
+        O.linear_f64(X, W)
+        t_total += time.perf_counter() - t0
+        nbytes += 2 * n * k
+    return {"kind": "oracle", "what": f"linear_f64 of one layer's 7 projections at batch {batch} (bf16 -> fp64 conversion included)",
+            "cores": oracle_threads(), "one_layer_ms": t_total * 1e3, "one_layer_gbs": nbytes / t_total / 1e9,
+            "oracle_extrapolated": True, "t_ms_64_layers_extrapolated": t_total * 1e3 * c["layers"]}
+
+
 def run_reference(args):
     rank = int(os.environ.get("RANK", "0"))
     if rank != 0:
         return 0
-    c, shapes, W, X = oracle_setup()
-    sb = step_bytes(shapes, ORACLE_SAMPLE)
+    # each step is a bounded sample of the cfg1 workload: the whole layer when the run is short enough for that to end
+    # within a few minutes (~4 s per step on 16 cores), the attention projections (19 % of the bytes) otherwise
+    names = ORACLE_LAYER if args.steps + args.warmup <= 30 else ORACLE_ATTN
+    c, shapes, W, X = oracle_setup(names)
+    sb = step_bytes(shapes, names)
     for _ in range(args.warmup):
-        oracle_step(c, shapes, W, X)
+        oracle_step(c, shapes, W, X, names)
     t0 = time.perf_counter()
     for _ in range(args.steps):
-        oracle_step(c, shapes, W, X)
+        oracle_step(c, shapes, W, X, names)
     dt = time.perf_counter() - t0
     val = sb["total"] * args.steps / dt / 1e9
-    sample = f"cfg1 attention projections {'/'.join(ORACLE_SAMPLE)} ({sb['B']/1e6:.1f} MB of 436.2 MB), all stages"
+    sample = (f"cfg1 {'whole layer' if names == ORACLE_LAYER else 'attention projections ' + '/'.join(names)} "
+              f"({sb['B']/1e6:.1f} MB of 436.2 MB), all stages")
     line = {"impl": "reference", "metric": METRIC, "value": val, "unit": "GB/s", "n_gpus": args.gpus,
             "steps": args.steps, "warmup": args.warmup, "ms_per_step": dt / args.steps * 1e3,
             "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "bf16", "data": "synthetic",
-            "config": {"workload": "cfg1: one LLaMA-8B-shaped decoder layer (bounded oracle sample)", "sample": sample},
+            "config": {"workload": "cfg1: one LLaMA-8B-shaped decoder layer (oracle on the host cores)", "sample": sample},
             "cpu_baseline": {"value": val, "unit": "GB/s", "cores": oracle_threads(), "kind": "oracle", "sample": sample},
             "e2e": {"value": val, "unit": "GB/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
-            "gpu_launches": 0}
+            "gpu_launches": 0,
+            "note": "the numpy oracle as it stands, a deliberately plain program: a ratio against it is not a headline"}
     print(json.dumps(line))
     return 0
 
@@ -298,7 +375,7 @@ def run_cloak(args):
     barrier()
     wall1 = time.time()
     launches = launches_per_step * args.steps
-    clk = clocks.stop(wall0, wall1) if clocks else None
+    clk = clocks.window(wall0, wall1) if clocks else None
     total_ms = evs[0][0].elapsed_time(evs[-1][-1])
     stage_ms = {s: float(np.mean([evs[k][i].elapsed_time(evs[k][i + 1]) for k in range(args.steps)]))
                 for i, s in enumerate(STAGES)}
@@ -362,9 +439,23 @@ def run_cloak(args):
         barrier()
         dt = (time.perf_counter() - t0) / n_e2e
         e2e_bytes = 2 * sb["B"] + sb["B"]           # shuffle (2 B/B) + one batch-1 GEMV pass over the layer
+        # context: what the link itself delivers for the same bytes (one pinned -> device copy per tensor, nothing else)
+        dst = {nm: torch.empty_like(perm[nm]) for nm in perm}
+        for nm in perm:
+            dst[nm].copy_(hW[nm], non_blocking=True)
+        barrier()
+        t0 = time.perf_counter()
+        for _ in range(n_e2e):
+            for nm in perm:
+                dst[nm].copy_(hW[nm], non_blocking=True)
+        barrier()
+        h2d_peak = sb["B"] * n_e2e / (time.perf_counter() - t0) / 1e9
+        del dst
         e2e = {"value": world * e2e_bytes / dt / 1e9, "unit": "GB/s", "h2d_bytes_per_step": h2d,
                "d2h_bytes_per_step": d2h, "ms_per_step": dt * 1e3,
-               "what": "cloak_shuffle_host of the layer from pinned host memory + 7 cloak_gemv_host (batch 1)"}
+               "h2d_gbs": h2d / dt / 1e9, "h2d_peak_gbs_measured": h2d_peak, "frac_of_h2d_peak": h2d / dt / 1e9 / h2d_peak,
+               "what": "cloak_shuffle_host of the layer from pinned host memory + 7 cloak_gemv_host (batch 1); PCIe-bound: "
+                       "frac_of_h2d_peak = achieved host->device rate / a plain pinned copy of the same tensors"}
 
     map_ms = C.cloak_pool_map_ms(pool_a)
     adjacency = C.cloak_pool_adjacency(pool_a)          # layout quality (G8): neighbours that stayed neighbours
@@ -407,28 +498,48 @@ def run_cloak(args):
         "gemv_isolated_ms": {"cloaked": cloaked_iso_ms, "native": native_ms, "cloaked_7_separate_calls": per_call_ms,
                              "native_one_plain_allocation": plain_ms, "torch_matmul_context": matmul_ms},
         "cloaked_vs_native_overhead_pct": overhead,
+        "cloaked_vs_cublas_pct": {f"b{b}": (cloaked_iso_ms[b] - matmul_ms[b]) / matmul_ms[b] * 100.0 for b in BATCHES},
+        "overhead_note": "north_star's target is cloaked vs THE SAME KERNEL on the unshuffled (identity-table) layout: "
+                         "cloaked_vs_native_overhead_pct.  cloaked_vs_cublas_pct puts it next to torch.matmul (cuBLAS) on the plain "
+                         "permuted tensors with plain pointers, 7 calls per batch in one CUDA graph: negative = faster than cuBLAS.",
         "hbm_peak_gbs": peak, "hbm_peak_kind": peak_kind, "hbm_nominal_gbs": 8000.0,
         "pool_map_ms": map_ms, "layout_adjacency": adjacency, "pool_create_s": pool_create_s, "roundtrip_bit_exact": bool(ok),
         "roofline": {"bound": "hbm", "kernel": "gemv_chain_kernel", "achieved": achieved, "peak": peak, "unit": "GB/s",
-                     "frac": achieved / peak, "traffic": NCU_TRAFFIC_PER_LAUNCH, "traffic_source": NCU_TRAFFIC_SOURCE,
+                     "frac": achieved / peak, "traffic": ncu_traffic()[0], "traffic_source": ncu_traffic()[1],
                      "launches_per_step": gemv_launches,
                      "bytes_per_launch": sb["gemv"] / gemv_launches, "avg_launch_us": gemv_ms / gemv_launches * 1e3,
                      "peak_kind": peak_kind},
-        "clocks": clk, "e2e": e2e, "gpu_launches": int(launches),
+        "clocks": clk, "e2e": e2e, "gpu_launches": int(launches), "runtime_info": C.cloak_runtime_info(),
     }
+    if args.configs != "cfg1" and world == 1:
+        # ---- the other configs of BASELINE.json, in the same process and under the same clock sampler
+        from paper_2606_18400_b200 import workloads
+        torch.cuda.empty_cache()
+        want = args.configs.split(",")
+        if "cfg2" in want:
+            line["cfg2"] = workloads.bench_cfg2(clocks, args.min_seconds)
+            torch.cuda.empty_cache()
+        if "cfg3" in want:
+            line["cfg3"] = workloads.bench_cfg3(clocks, args.min_seconds)
+            torch.cuda.empty_cache()
+        if "cfg4" in want:
+            line["cfg4"] = workloads.bench_cfg4(clocks, args.min_seconds / 2)
+            torch.cuda.empty_cache()
+        line["gpu_launches_other_configs"] = int(sum(line[k]["gpu_launches"] for k in ("cfg2", "cfg3", "cfg4") if k in line))
+    if clocks is not None:
+        clocks.stop()
     if not args.no_cpu_baseline:
-        co, shp, W, Xo = oracle_setup()
-        sbo = step_bytes(shp, ORACLE_SAMPLE)
-        t0 = time.perf_counter()
-        reps = 0
-        while reps < 1 or (time.perf_counter() - t0 < 10.0 and reps < 20):
-            oracle_step(co, shp, W, Xo)
-            reps += 1
-        dt = (time.perf_counter() - t0) / reps
-        line["cpu_baseline"] = {"value": sbo["total"] / dt / 1e9, "unit": "GB/s", "cores": oracle_threads(),
-                                "kind": "oracle", "host_cpus": os.cpu_count(), "ms_per_step": dt * 1e3,
-                                "sample": f"cfg1 attention projections {'/'.join(ORACLE_SAMPLE)} "
-                                          f"({sbo['B']/1e6:.1f} MB of 436.2 MB), all stages, {reps} rep(s)"}
+        # the oracle beside it: the WHOLE cfg1 layer through the same stages, bounded by repetitions, once with
+        # numpy's BLAS on all cores and once limited to one thread
+        dt, reps, used, sbo = oracle_time(ORACLE_LAYER, 3, 12.0)
+        dt1, reps1, _, _ = oracle_time(ORACLE_LAYER, 1, 1.0, threads=1)
+        line["cpu_baseline"] = {"value": sbo["total"] / dt / 1e9, "unit": "GB/s", "cores": used, "kind": "oracle",
+                                "host_cpus": os.cpu_count(), "ms_per_step": dt * 1e3,
+                                "single_thread": {"value": sbo["total"] / dt1 / 1e9, "unit": "GB/s", "ms_per_step": dt1 * 1e3, "reps": reps1},
+                                "sample": f"cfg1 whole layer ({sbo['B']/1e6:.1f} MB), all stages of the step, {reps} rep(s); only the "
+                                          "fp64 contraction (numpy BLAS) is threaded, the byte loops are single-threaded Python + numpy"}
+        if "cfg3" in line:
+            line["cfg3"]["oracle"] = oracle_cfg3_layer()
     print(json.dumps(line))
     if dist is not None:
         dist.destroy_process_group()
@@ -449,6 +560,10 @@ def main():
                     help="cfg1 (default) is the headline step; cfg2-4 are the other BASELINE.json configs "
                          "(paper_2606_18400_b200/workloads.py), each printing its own JSON line")
     ap.add_argument("--reps", type=int, default=10, help="repetitions per measurement for --workload cfg2-4")
+    ap.add_argument("--configs", default="cfg1,cfg2,cfg3,cfg4",
+                    help="what the line carries besides the cfg1 step (`value`): cfg2, cfg3, cfg4 blocks (BASELINE.json configs[2..4]); "
+                         "`--configs cfg1` for the step alone.  N > 1 replicas run the step alone.")
+    ap.add_argument("--min-seconds", type=float, default=1.0, help="minimum length of each timed loop of the cfg2-4 blocks")
     ap.add_argument("--gemv-engine", type=int, default=0,
                     help="A/B: cloak_set_gemv_engine (0 auto, 1 one-shot kernel, 2 no PDL)")
     args = ap.parse_args()

@@ -54,6 +54,10 @@ const char* cloak_last_error(void);
 /* Library version / build info: a static string such as "cloak-b200 0.1 sm_100a". */
 const char* cloak_version(void);
 
+/* Facts the library found out at run time, as a thread-local string for logs and bench lines: whether the driver accepted
+ * the cooperative GEMV launch together with programmatic dependent launch, kernels launched so far. */
+const char* cloak_runtime_info(void);
+
 /* Process-wide number of CUDA kernels this library has launched so far (for bench.py's gpu_launches). */
 uint64_t cloak_launch_count(void);
 

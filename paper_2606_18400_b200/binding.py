@@ -22,7 +22,7 @@ STATUS_NAMES = {0: "CLOAK_OK", -1: "CLOAK_ERR_INVALID", -2: "CLOAK_ERR_ALIGN", -
                 -4: "CLOAK_ERR_OOM", -5: "CLOAK_ERR_CUDA"}
 
 # every symbol include/cloak.h declares
-SYMBOLS = ["cloak_last_error", "cloak_version", "cloak_launch_count", "cloak_keygen", "cloak_pool_create", "cloak_pool_destroy",
+SYMBOLS = ["cloak_last_error", "cloak_version", "cloak_runtime_info", "cloak_launch_count", "cloak_keygen", "cloak_pool_create", "cloak_pool_destroy",
            "cloak_pool_info", "cloak_pool_tables", "cloak_pool_dump", "cloak_pool_map_ms", "cloak_pool_adjacency", "cloak_shuffle",
            "cloak_unshuffle", "cloak_shuffle_many", "cloak_unshuffle_many", "cloak_relayout", "cloak_rekey_inplace", "cloak_shuffle_host", "cloak_unshuffle_host",
            "cloak_set_copy_engine", "cloak_arena_plan", "cloak_permute_mlp_heads", "cloak_permute_experts", "cloak_load_mlp_heads", "cloak_to_tile128",
@@ -66,6 +66,7 @@ lib = ctypes.CDLL(LIB_PATH)
 _P = c_void_p
 lib.cloak_last_error.restype = c_char_p
 lib.cloak_version.restype = c_char_p
+lib.cloak_runtime_info.restype = c_char_p
 lib.cloak_keygen.argtypes = [c_uint64, c_uint64, c_uint32, _P, _P, _P]
 lib.cloak_pool_create.argtypes = [c_int, c_uint64, c_uint32, c_uint64, c_uint64, c_uint32, POINTER(_P)]
 lib.cloak_pool_destroy.argtypes = [_P]
@@ -103,7 +104,7 @@ lib.cloak_gemm.argtypes = [_P, POINTER(cloak_tensor), _P, _P, c_uint32, _P]
 lib.cloak_gemv_host.argtypes = [_P, POINTER(cloak_tensor), _P, _P, c_uint32, _P]
 lib.cloak_silu_mul.argtypes = [_P, _P, _P, c_uint64, c_int, _P]
 lib.cloak_launch_count.restype = c_uint64
-for _n in SYMBOLS[3:]:
+for _n in SYMBOLS[4:]:
     getattr(lib, _n).restype = c_int
 
 
@@ -145,6 +146,10 @@ def cloak_last_error():
 
 def cloak_version():
     return lib.cloak_version().decode()
+
+
+def cloak_runtime_info():
+    return lib.cloak_runtime_info().decode()
 
 
 def cloak_launch_count():

@@ -32,13 +32,13 @@ class ClockSampler:
         for line in self.proc.stdout:
             self.lines.append((time.time(), line.strip()))
 
-    def stop(self, t0, t1):
+    def window(self, t0, t1):
+        """Clock / power / throttle summary of the samples taken in the wall-clock window [t0, t1]; the sampler keeps running."""
         if self.proc is None:
             return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
         time.sleep(0.15)
-        self.proc.terminate()
         sm, pw, smax, reasons = [], [], None, set()
-        for ts, line in self.lines:
+        for ts, line in list(self.lines):
             f = [x.strip() for x in line.split(",")]
             if len(f) < 9:
                 continue
@@ -53,4 +53,11 @@ class ClockSampler:
                 if v.lower().startswith("active") and t0 - 0.05 <= ts <= t1 + 0.15:
                     reasons.add(name)
         return {"sm_mhz": float(np.median(sm)) if sm else None, "sm_min_mhz": min(sm) if sm else None, "sm_max_mhz": smax,
-                "power_w_max": max(pw) if pw else None, "reasons": sorted(reasons), "samples": len(sm)}
+                "power_w_max": max(pw) if pw else None, "power_w_median": float(np.median(pw)) if pw else None,
+                "reasons": sorted(reasons), "samples": len(sm)}
+
+    def stop(self, t0=None, t1=None):
+        out = self.window(t0, t1) if t0 is not None else None
+        if self.proc is not None:
+            self.proc.terminate()
+        return out

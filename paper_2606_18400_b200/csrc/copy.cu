@@ -310,8 +310,9 @@ static cloak_status host_range(const cloak_pool* pool, char* h_logical, uint64_t
     if (chunk < b) chunk = b;
     chunk = chunk / b * b;
     if (chunk > bytes) chunk = (bytes + 15) & ~15ull;
-    char* stage = nullptr;
-    CLOAK_CUDA(cudaMallocAsync((void**)&stage, chunk, s));
+    AsyncBuf sbuf(s);                          // from the library's cached pool: no driver allocation after the first call
+    if (cloak_status ast = sbuf.alloc(chunk)) return ast;
+    char* stage = static_cast<char*>(sbuf.p);
     cloak_status st = CLOAK_OK;
     for (uint64_t at = 0; at < bytes && st == CLOAK_OK; at += chunk) {
         const uint64_t n = bytes - at < chunk ? bytes - at : chunk;
@@ -326,7 +327,6 @@ static cloak_status host_range(const cloak_pool* pool, char* h_logical, uint64_t
             if (e != cudaSuccess) { st = fail(CLOAK_ERR_CUDA, "unshuffle_host D2H: %s", cudaGetErrorString(e)); break; }
         }
     }
-    cudaFreeAsync(stage, s);
     cudaError_t e = cudaStreamSynchronize(s);
     if (st == CLOAK_OK && e != cudaSuccess) st = fail(CLOAK_ERR_CUDA, "host copy sync: %s", cudaGetErrorString(e));
     return st;

@@ -147,7 +147,17 @@ extern "C" const char* cloak_last_error(void) { return cloak::g_err; }
 
 extern "C" uint64_t cloak_launch_count(void) { return cloak::g_launches.load(); }
 
-extern "C" const char* cloak_version(void) { return "cloak-b200 0.1 sm_100a"; }
+extern "C" const char* cloak_version(void) { return "cloak-b200 0.2 sm_100a"; }
+
+namespace cloak { int gemv_coop_pdl_state(); }
+extern "C" const char* cloak_runtime_info(void) {
+    static thread_local char buf[256];
+    const int st = cloak::gemv_coop_pdl_state();
+    snprintf(buf, sizeof(buf), "gemv_chain: cooperative launch, programmatic dependent launch %s; kernels launched %llu",
+             st < 0 ? "not probed yet" : (st ? "accepted with it" : "rejected with it (dropped)"),
+             (unsigned long long)cloak::g_launches.load());
+    return buf;
+}
 
 extern "C" cloak_status cloak_arena_plan(uint64_t key, uint32_t T, const uint64_t* h_bytes, uint32_t block_bytes,
                                          uint64_t* h_offsets_out, uint64_t* h_total_out) {

@@ -428,6 +428,7 @@ constexpr uint32_t GS_TILE_COUNTERS = (uint32_t)(WS_COUNTER_BYTES / 4) - 4 * GS_
 // Whether the cooperative attribute may be combined with programmatic stream serialization is probed on the first launch:
 // if the driver rejects the pair, PDL is dropped, not the guarantee.
 static std::atomic<int> g_coop_with_pdl{-1};     // -1 unknown, 0 rejected, 1 accepted
+int gemv_coop_pdl_state() { return g_coop_with_pdl.load(std::memory_order_relaxed); }
 
 template <int CU, int NT>
 static cloak_status launch(const ChainArgs& a, int ctas, int device, cudaStream_t s) {

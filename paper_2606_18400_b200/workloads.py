@@ -536,6 +536,247 @@ def run_moe(args):
             "gpu_launches": C.cloak_launch_count() - launches0}
 
 
+# ------------------------------------------------------------------------------------------ brief blocks for bench.py
+# bench.py's default run carries cfg2, cfg3 and cfg4 next to the cfg1 step: one sub-object per measurement
+# with the report schema's fields, every timed loop at least `min_s` seconds long so that the clock record means something.
+def time_loop(torch, fn, min_s=1.0, min_reps=10, max_reps=50000, warmup=3):
+    """fn() repeated for at least min_s seconds of device time, one CUDA event per repetition on the launching stream."""
+    stream = torch.cuda.current_stream()
+    for _ in range(warmup):
+        fn()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record(stream)
+    for _ in range(3):
+        fn()
+    e1.record(stream)
+    torch.cuda.synchronize()
+    est = max(e0.elapsed_time(e1) / 3, 1e-3)
+    reps = int(min(max(min_reps, np.ceil(min_s * 1e3 / est)), max_reps))
+    ev = [torch.cuda.Event(enable_timing=True) for _ in range(reps + 1)]
+    w0 = time.time()
+    ev[0].record(stream)
+    for i in range(reps):
+        fn()
+        ev[i + 1].record(stream)
+    torch.cuda.synchronize()
+    w1 = time.time()
+    ts = np.array([ev[i].elapsed_time(ev[i + 1]) for i in range(reps)])
+    return {"t_ms_median": float(np.median(ts)), "t_ms_min": float(ts.min()), "t_ms_mean": float(ev[0].elapsed_time(ev[-1]) / reps),
+            "reps": reps, "wall": (w0, w1)}
+
+
+def ab_loop(torch, fn_a, fn_b, reps):
+    """fn_a and fn_b alternated rep by rep (drift hits both alike); medians in ms."""
+    stream = torch.cuda.current_stream()
+    ev = [torch.cuda.Event(enable_timing=True) for _ in range(2 * reps + 1)]
+    ev[0].record(stream)
+    for i in range(reps):
+        fn_a()
+        ev[2 * i + 1].record(stream)
+        fn_b()
+        ev[2 * i + 2].record(stream)
+    torch.cuda.synchronize()
+    ta = [ev[2 * i].elapsed_time(ev[2 * i + 1]) for i in range(reps)]
+    tb = [ev[2 * i + 1].elapsed_time(ev[2 * i + 2]) for i in range(reps)]
+    return float(np.median(ta)), float(np.median(tb))
+
+
+def measure(torch, sampler, peak, nbytes, fn, fn_identity=None, min_s=1.0, flops=None, extra=None):
+    """One report-schema entry: the cloaked call timed for >= min_s seconds, then (if given) alternated with the same call
+    on the identity-table pool for the overhead figure."""
+    r = time_loop(torch, fn, min_s)
+    w0, w1 = r.pop("wall")
+    gbs = nbytes / r["t_ms_median"] / 1e6
+    out = {"bytes_algorithmic": int(nbytes), **r, "gbs": gbs, "frac_measured": gbs / peak, "frac_nominal": gbs / NOMINAL_HBM_GBS}
+    if flops:
+        out["flops"] = float(flops)
+        out["tflops"] = flops / r["t_ms_median"] / 1e9
+    out["clocks"] = sampler.window(w0, w1) if sampler is not None else None
+    if fn_identity is not None:
+        for _ in range(3):
+            fn_identity()
+        pairs = int(min(max(20, np.ceil(0.5 * min_s * 1e3 / r["t_ms_median"])), 5000))
+        tc, ti = ab_loop(torch, fn, fn_identity, pairs)
+        out.update({"t_identity_ms": ti, "t_cloaked_ms_alternated": tc, "overhead_pct": (tc - ti) / ti * 100.0})
+    if extra:
+        out.update(extra)
+    return out
+
+
+def _graph(torch, fn):
+    """fn() (C-ABI launches on torch's current stream) run once, then captured into a CUDA graph."""
+    fn()
+    torch.cuda.synchronize()
+    g = torch.cuda.CUDAGraph()
+    with torch.cuda.graph(g):
+        fn()
+    torch.cuda.synchronize()
+    return g
+
+
+def bench_cfg2(sampler, min_s=1.0):
+    """cfg2 for the bench line: mapper ms, whole-model cloak_shuffle_many / cloak_unshuffle_many, the 225-op decode chain
+    (graph replay) cloaked vs identity table."""
+    torch, C, synth_cuda, gen = _imports()
+    c = gen.CONFIGS[2]
+    peak, _ = hbm_peak()
+    tensors = gen.model_tensors(2)
+    sizes = [2 * n * k for _, (n, k) in tensors]
+    offs, total = C.cloak_arena_plan(c["key"], sizes, c["block"])
+    off = {nm: o for (nm, _), o in zip(tensors, offs)}
+    payload = sum(sizes)
+    pc = C.cloak_pool_create(0, total, c["block"], c["page"], c["key"])
+    pn = C.cloak_pool_create(0, total, c["block"], c["page"], c["key"], C.CLOAK_POOL_IDENTITY)
+    launches0 = C.cloak_launch_count()
+    out = {"workload": "cfg2: 32-layer LLaMA-8B-shaped model, bf16, 226 tensors, 64 KiB blocks, 2 MiB VMM pages",
+           "payload_bytes": payload, "npages": C.cloak_pool_info(pc)["npages"],
+           "pool_map_ms": {"cloaked": C.cloak_pool_map_ms(pc), "identity": C.cloak_pool_map_ms(pn)}}
+    try:
+        keep = {nm: torch.empty(shp, dtype=torch.bfloat16, device="cuda") for nm, shp in tensors}
+        t0 = time.perf_counter()
+        _load_model(torch, C, synth_cuda, gen, 2, (), offs, False, keep=keep)
+        out["generate_permute_s"] = time.perf_counter() - t0
+        m_t, m_o, m_b = [keep[nm] for nm, _ in tensors], [off[nm] for nm, _ in tensors], [keep[nm].numel() * 2 for nm, _ in tensors]
+        C.cloak_shuffle_many(pn, m_t, m_o, m_b)
+        out["shuffle"] = measure(torch, sampler, peak, 2 * payload, lambda: C.cloak_shuffle_many(pc, m_t, m_o, m_b),
+                                 lambda: C.cloak_shuffle_many(pn, m_t, m_o, m_b), min_s, extra={"call": "cloak_shuffle_many, 226 ranges, 2 launches"})
+        back = torch.empty(payload // 2, dtype=torch.bfloat16, device="cuda")
+        views, at = [], 0
+        for nm, (n, k) in tensors:
+            views.append(back[at:at + n * k].view(n, k))
+            at += n * k
+        out["unshuffle"] = measure(torch, sampler, peak, 2 * payload, lambda: C.cloak_unshuffle_many(pc, views, m_o, m_b), None, min_s,
+                                   extra={"call": "cloak_unshuffle_many, 226 ranges, 2 launches"})
+        out["roundtrip_bit_exact"] = bool(all(torch.equal(v, keep[nm]) for v, (nm, _) in zip(views, tensors)))
+        del back, views, keep, m_t
+        torch.cuda.empty_cache()
+        # ---- decode chain at batch 1 (same op list as run_cfg2)
+        H, I, Q = c["hidden"], c["inter"], c["n_q"] * c["head_dim"]
+        xh = synth_cuda.fill(torch.empty(1, H, dtype=torch.bfloat16, device="cuda"), c["seed"] + 100, 0, kind=gen.KIND_NORMAL)
+        xa = synth_cuda.fill(torch.empty(1, Q, dtype=torch.bfloat16, device="cuda"), c["seed"] + 100, 1, kind=gen.KIND_NORMAL)
+        T = {nm: C.cloak_tensor(off[nm], shp[0], shp[1], C.CLOAK_BF16, C.CLOAK_ROWMAJOR) for nm, shp in tensors}
+        read_bytes = payload - sizes[0]
+        graphs, Y = {}, {}
+        for name, pool in (("cloaked", pc), ("native", pn)):
+            y = {nm: torch.zeros(1, shp[0], dtype=torch.bfloat16, device="cuda") for nm, shp in tensors if nm != "embed"}
+            act = torch.empty(1, I, dtype=torch.bfloat16, device="cuda")
+            ops = []
+            for l in range(c["layers"]):
+                p = f"l{l}."
+                ops += [(T[p + nm], xh, y[p + nm], 0) for nm in ("q", "k", "v")]
+                ops += [(T[p + "o"], xa, y[p + "o"], 0), (T[p + "gate"], xh, y[p + "gate"], 0),
+                        (T[p + "up"], xh, y[p + "up"], 0, y[p + "gate"], act), (T[p + "down"], act, y[p + "down"], 1)]
+            ops.append((T["lm_head"], xh, y["lm_head"], 0))
+            ops = C.cloak_gemv_ops(ops)
+            graphs[name] = (_graph(torch, lambda: C.cloak_gemv_chain(pool, ops, 1)), ops, act)
+            Y[name] = y
+        d = measure(torch, sampler, peak, read_bytes, graphs["cloaked"][0].replay, graphs["native"][0].replay, min_s,
+                    extra={"call": "cloak_gemv_chain, 225 ops, batch 1, CUDA-graph replay"})
+        d["tokens_per_s"] = 1e3 / d["t_ms_median"]
+        d["ideal_tokens_per_s_at_measured_peak"] = peak * 1e9 / read_bytes
+        d["cloaked_identical_to_native"] = bool(all(torch.equal(Y["cloaked"][nm], Y["native"][nm]) for nm in Y["cloaked"]))
+        out["decode_chain"] = d
+    finally:
+        torch.cuda.synchronize()
+        C.cloak_pool_destroy(pc)
+        C.cloak_pool_destroy(pn)
+    out["gpu_launches"] = C.cloak_launch_count() - launches0
+    return out
+
+
+def bench_cfg3(sampler, min_s=1.0, layers=None, batches=(32, 128), depths=(8, 64)):
+    """cfg3 for the bench line: the tcgen05 GEMM chain over the first 8 layers and over all 64 layers of the 62 GB TILE128 pool
+    at batch 32 and 128 (graph replay), cloaked vs identity table."""
+    torch, C, synth_cuda, gen = _imports()
+    c = gen.CONFIGS[3]
+    layers = int(layers or c["layers"])
+    peak, _ = hbm_peak()
+    tensors = gen.model_tensors(3)[:7 * layers]
+    sizes = [2 * n * k for _, (n, k) in tensors]
+    offs, total = C.cloak_arena_plan(c["key"], sizes, c["block"])
+    off = {nm: o for (nm, _), o in zip(tensors, offs)}
+    pc = C.cloak_pool_create(0, total, c["block"], c["page"], c["key"])
+    pn = C.cloak_pool_create(0, total, c["block"], c["page"], c["key"], C.CLOAK_POOL_IDENTITY)
+    launches0 = C.cloak_launch_count()
+    out = {"workload": "cfg3: Qwen-32B-shaped model, %d layers, bf16 TILE128, 64 KiB blocks, 2 MiB VMM pages" % layers,
+           "payload_bytes": sum(sizes), "npages": C.cloak_pool_info(pc)["npages"],
+           "pool_map_ms": {"cloaked": C.cloak_pool_map_ms(pc), "identity": C.cloak_pool_map_ms(pn)}, "gemm": {}}
+    try:
+        t0 = time.perf_counter()
+        _load_model(torch, C, synth_cuda, gen, 3, (pc, pn), offs, True, layers=layers)
+        out["generate_permute_tile_load_s"] = time.perf_counter() - t0
+        torch.cuda.empty_cache()
+        H, I, Q = c["hidden"], c["inter"], c["n_q"] * c["head_dim"]
+        T = {nm: C.cloak_tensor(off[nm], shp[0], shp[1], C.CLOAK_BF16, C.CLOAK_TILE128) for nm, shp in tensors}
+        lnames = [nm for nm, _ in gen.layer_shapes(H, I, c["n_q"], c["n_kv"], c["head_dim"])]
+        for batch in batches:
+            X = {k: synth_cuda.fill(torch.empty(batch, k, dtype=torch.bfloat16, device="cuda"), c["seed"] + 100, 2 * batch + i,
+                                    kind=gen.KIND_NORMAL) for i, k in enumerate(sorted({H, I, Q}))}
+            for depth in [d for d in depths if d <= layers]:
+                nbytes = sum(sizes[:7 * depth])
+                g, ys = {}, {}
+                for name, pool in (("cloaked", pc), ("native", pn)):
+                    yl = [{nm: torch.zeros(batch, dict(tensors)[f"l0.{nm}"][0], dtype=torch.bfloat16, device="cuda") for nm in lnames}
+                          for _ in range(depth)]
+                    ops = C.cloak_gemm_ops([(T[f"l{l}.{nm}"], X[T[f"l{l}.{nm}"].K], yl[l][nm]) for l in range(depth) for nm in lnames])
+                    C.cloak_pool_reserve_workspace(pool, C.cloak_gemm_chain_scratch_bytes(pool, ops, batch))
+                    g[name] = (_graph(torch, lambda: C.cloak_gemm_chain(pool, ops, batch)), ops)
+                    ys[name] = yl
+                d = measure(torch, sampler, peak, nbytes, g["cloaked"][0].replay, g["native"][0].replay, min_s,
+                            flops=2.0 * batch * (nbytes / 2),
+                            extra={"call": "cloak_gemm_chain, %d ops, batch %d, CUDA-graph replay" % (7 * depth, batch)})
+                d["cloaked_identical_to_native"] = bool(all(torch.equal(a[nm], b[nm]) for a, b in zip(ys["cloaked"], ys["native"]) for nm in lnames))
+                out["gemm"][f"b{batch}_{depth}layers"] = d
+                del g, ys
+            del X
+            torch.cuda.empty_cache()
+    finally:
+        torch.cuda.synchronize()
+        C.cloak_pool_destroy(pc)
+        C.cloak_pool_destroy(pn)
+    out["gpu_launches"] = C.cloak_launch_count() - launches0
+    return out
+
+
+def bench_cfg4(sampler, min_s=0.5):
+    """cfg4 for the bench line: shuffle (vs identity table), unshuffle and re-layout A -> B of the 4 GiB buffer at the five
+    block sizes, beside a device-to-device copy."""
+    torch, C, synth_cuda, gen = _imports()
+    c = gen.CONFIGS[4]
+    nbytes = int(c["bytes"])
+    peak, _ = hbm_peak()
+    L = synth_cuda.fill(torch.empty(nbytes // 2, dtype=torch.bfloat16, device="cuda"), c["seed"], 0)
+    back = torch.empty_like(L)
+    launches0 = C.cloak_launch_count()
+    out = {"workload": "cfg4: granularity sweep, 4 GiB bf16 buffer, 2 MiB VMM pages, keys 0x1234 -> 0x5678", "bytes": nbytes,
+           "memcpy_d2d": measure(torch, sampler, peak, 2 * nbytes, lambda: back.copy_(L), None, min_s, extra={"call": "torch copy_ (context)"}),
+           "sweep": {}}
+    ok = True
+    for b in c["blocks"]:
+        pa = C.cloak_pool_create(0, nbytes, b, c["page"], c["key"])
+        pb = C.cloak_pool_create(0, nbytes, b, c["page"], c["key_b"])
+        pn = C.cloak_pool_create(0, nbytes, b, c["page"], c["key"], C.CLOAK_POOL_IDENTITY)
+        try:
+            r = {"block_bytes": b, "nblocks": nbytes // b, "pool_map_ms": C.cloak_pool_map_ms(pa)}
+            r["shuffle"] = measure(torch, sampler, peak, 2 * nbytes, lambda: C.cloak_shuffle(pa, L, 0, nbytes),
+                                   lambda: C.cloak_shuffle(pn, L, 0, nbytes), min_s)
+            r["unshuffle"] = measure(torch, sampler, peak, 2 * nbytes, lambda: C.cloak_unshuffle(pa, back, 0, nbytes), None, min_s)
+            r["roundtrip_bit_exact"] = bool(torch.equal(back, L))
+            r["relayout"] = measure(torch, sampler, peak, 2 * nbytes, lambda: C.cloak_relayout(pa, pb), None, min_s)
+            back.zero_()
+            C.cloak_unshuffle(pb, back, 0, nbytes)
+            r["relayout_bit_exact"] = bool(torch.equal(back, L))
+            ok = ok and r["roundtrip_bit_exact"] and r["relayout_bit_exact"]
+            out["sweep"][f"{b // 1024}KiB"] = r
+        finally:
+            torch.cuda.synchronize()
+            for p in (pa, pb, pn):
+                C.cloak_pool_destroy(p)
+    out["all_bit_exact"] = ok
+    out["gpu_launches"] = C.cloak_launch_count() - launches0
+    return out
+
+
 RUNNERS = {"cfg2": run_cfg2, "cfg3": run_cfg3, "cfg4": run_cfg4, "moe": run_moe}
 
 

@@ -589,7 +589,7 @@ def test_two_pools_two_streams_first_use_captured_without_warmup():
             assert err <= TOL["bf16"], err
         assert all(torch.equal(outs[0][0][nm], outs[1][0][nm]) for nm in outs[0][0])      # two keys, one function
         # a call that needs more scratch than the pool has fails inside a capture instead of allocating there ...
-        p, st = pools[0], streams[0]
+        p, st = pools[1], streams[1]                                      # (T, Tt hold the offsets of the last pool built)
         big = torch.zeros(256, Tt["gate"].N, dtype=torch.bfloat16, device="cuda")
         xbig = torch.zeros(256, H, dtype=torch.bfloat16, device="cuda")
         more = C.cloak_gemm_chain_scratch_bytes(p.h, [(Tt["gate"], xbig, big)] * 16, 256)
@@ -603,7 +603,7 @@ def test_two_pools_two_streams_first_use_captured_without_warmup():
             with torch.cuda.stream(st):
                 y1 = torch.zeros(bm, Tt["gate"].N, dtype=torch.bfloat16, device="cuda")
                 C.cloak_gemm_chain(p.h, [(Tt["gate"], xbig, big)] * 16, 256)
-                C.cloak_gemm(p.h, Tt["gate"], outs[0][5], y1, bm)
+                C.cloak_gemm(p.h, Tt["gate"], outs[1][5], y1, bm)
             st.synchronize()
             check_linear(y1.float().cpu().numpy(), xm, Ws["gate"], "bf16", "two_streams:after_growth", TOL["bf16"])
     finally:
