@@ -217,6 +217,15 @@ def run_reference(args):
 
 
 # ------------------------------------------------------------------------------------------ replicas (N > 1)
+def sm_weights_summary(C):
+    """The per-SM streaming weights the library measured on this device (calibrate.cu), summarised."""
+    w = np.array(C.cloak_sm_weights(0))
+    if w.size == 0:
+        return {"measured": False}
+    return {"measured": True, "n_sm": int(w.size), "min": float(w.min()), "max": float(w.max()),
+            "tiers": {f"{v:.3f}": int(c) for v, c in zip(*np.unique(np.round(w * 8) / 8, return_counts=True))}}
+
+
 def max_over_ranks(ms, dist, device):
     """The path does not shard (replicas only): every rank times its own replica of the step and the
     job's time is the slowest rank's.  One scalar all_reduce(MAX); `dist` is None on a single rank."""
@@ -503,7 +512,7 @@ def run_cloak(args):
                          "cloaked_vs_native_overhead_pct.  cloaked_vs_cublas_pct puts it next to torch.matmul (cuBLAS) on the plain "
                          "permuted tensors with plain pointers, 7 calls per batch in one CUDA graph: negative = faster than cuBLAS.",
         "hbm_peak_gbs": peak, "hbm_peak_kind": peak_kind, "hbm_nominal_gbs": 8000.0,
-        "pool_map_ms": map_ms, "layout_adjacency": adjacency, "pool_create_s": pool_create_s, "roundtrip_bit_exact": bool(ok),
+        "sm_weights": sm_weights_summary(C), "pool_map_ms": map_ms, "layout_adjacency": adjacency, "pool_create_s": pool_create_s, "roundtrip_bit_exact": bool(ok),
         "roofline": {"bound": "hbm", "kernel": "gemv_chain_kernel", "achieved": achieved, "peak": peak, "unit": "GB/s",
                      "frac": achieved / peak, "traffic": ncu_traffic()[0], "traffic_source": ncu_traffic()[1],
                      "launches_per_step": gemv_launches,
@@ -564,15 +573,21 @@ def main():
                     help="what the line carries besides the cfg1 step (`value`): cfg2, cfg3, cfg4 blocks (BASELINE.json configs[2..4]); "
                          "`--configs cfg1` for the step alone.  N > 1 replicas run the step alone.")
     ap.add_argument("--min-seconds", type=float, default=1.0, help="minimum length of each timed loop of the cfg2-4 blocks")
+    ap.add_argument("--sm-weighting", type=int, default=1, help="A/B: cloak_set_sm_weighting (1 measured per-SM shares, 0 equal shares)")
+    ap.add_argument("--copy-hint", type=int, default=-1, help="A/B: cloak_set_copy_cache_hint (bit 0 stores, bit 1 loads evict_first)")
     ap.add_argument("--gemv-engine", type=int, default=0,
                     help="A/B: cloak_set_gemv_engine (0 auto, 1 one-shot kernel, 2 no PDL)")
     args = ap.parse_args()
     if args.workload != "cfg1":
         from paper_2606_18400_b200 import workloads
         return workloads.main([args.workload, "--reps", str(args.reps), "--gemv-engine", str(args.gemv_engine)])
-    if args.gemv_engine and args.impl == "cloak":
+    if args.impl == "cloak":
         import paper_2606_18400_b200 as C
-        C.cloak_set_gemv_engine(args.gemv_engine)
+        if args.gemv_engine:
+            C.cloak_set_gemv_engine(args.gemv_engine)
+        C.cloak_set_sm_weighting(args.sm_weighting)
+        if args.copy_hint >= 0:
+            C.cloak_set_copy_cache_hint(args.copy_hint)
     args.warmup = max(args.warmup, 3) if args.impl == "cloak" else args.warmup
     return run_reference(args) if args.impl == "reference" else run_cloak(args)
 

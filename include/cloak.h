@@ -160,6 +160,10 @@ cloak_status cloak_unshuffle_host(const cloak_pool* pool, void* h_logical, uint6
  * LDG/STG, 2 = TMA bulk copy through a shared-memory ring.  For A/B measurement; process-wide. */
 cloak_status cloak_set_copy_engine(int engine);
 
+/* L2 eviction hints of the TMA copy engine: bit 0 = its stores are evict_first, bit 1 = its loads are.  Default 1: a streaming
+ * copy should not leave the 126 MB L2 full of dirty lines for the next kernel to write back.  For A/B measurement; process-wide. */
+cloak_status cloak_set_copy_cache_hint(int hint);
+
 /* ---- S3 tensor order.  Host helper, no device work.
  * (order, _) = keygen(key, 3<<32, T); the arena holds tensors order[0], order[1], ... back to back, each
  * padded to a multiple of block_bytes.  h_offsets_out: T entries; h_total_out: padded arena bytes. */
@@ -311,6 +315,21 @@ cloak_status cloak_gemm_chain(const cloak_pool* pool, const cloak_gemm_op* h_ops
  * programmatic dependent launch.  For A/B measurement; process-wide (an atomic: safe to flip from any thread, takes effect
  * at the next launch). */
 cloak_status cloak_set_gemv_engine(int engine);
+/* Per-SM streaming weights (calibrate.cu).  The SMs of a B200 do not pull a read stream out of HBM equally fast (three tiers,
+ * up to 1.7 x apart, a property of the individual part); the first cloak_pool_create on a device measures it once (a 1 GiB
+ * scratch buffer, a few ms), and the streaming GEMV cuts large ops into STATIC shares proportional to it instead of equal
+ * ones (the split is fixed for the life of the process: results stay deterministic, and the same on cloaked and identity-table
+ * pools; between processes the last bits of a split-K sum may differ where a weight moved by a quantisation step).
+ * cloak_sm_weights: the relative speeds (mean 1) of the device's SMs, indexed by SM id; *h_nsm = 0 if they could not be
+ * measured (kernels then use equal shares).  h_weights may be NULL to query the count.  Measures if that has not happened yet.
+ * cloak_set_sm_weighting: 0 = equal shares, 1 = measured weights (default).  For A/B measurement; process-wide. */
+cloak_status cloak_sm_weights(int device, uint32_t capacity, float* h_weights, uint32_t* h_nsm);
+cloak_status cloak_set_sm_weighting(int mode);
+/* Tracing: while d_trace is not NULL, every streaming-GEMV launch records, per CTA b, four 64-bit words at d_trace[4*b]: the
+ * SM id, %globaltimer (ns) at CTA start, when its producer had issued its last copy, and when its consumers were done.  The
+ * buffer (DEVICE memory, 8-byte aligned, room for 4 words x the device's SM count) is the caller's and is overwritten by
+ * every launch.  NULL switches it off (default).  Process-wide. */
+cloak_status cloak_set_trace(void* d_trace);
 /* Host only, no device work: the chunk grid one cloak_gemm_chain launch of n_ops <= 16 ops with these shapes would use on a
  * GPU with `sms` SMs under the current cloak_set_gemm_schedule.  The launch's 128x128 tiles -- the ops back to back, each in
  * storage order -- are numbered 0 .. total-1; chunk c covers tiles [h_begin[c], h_end[c]).  Chunks 0 .. *h_nstatic-1 are the

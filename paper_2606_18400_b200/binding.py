@@ -25,9 +25,9 @@ STATUS_NAMES = {0: "CLOAK_OK", -1: "CLOAK_ERR_INVALID", -2: "CLOAK_ERR_ALIGN", -
 SYMBOLS = ["cloak_last_error", "cloak_version", "cloak_runtime_info", "cloak_launch_count", "cloak_keygen", "cloak_pool_create", "cloak_pool_destroy",
            "cloak_pool_info", "cloak_pool_tables", "cloak_pool_dump", "cloak_pool_map_ms", "cloak_pool_adjacency", "cloak_shuffle",
            "cloak_unshuffle", "cloak_shuffle_many", "cloak_unshuffle_many", "cloak_relayout", "cloak_rekey_inplace", "cloak_shuffle_host", "cloak_unshuffle_host",
-           "cloak_set_copy_engine", "cloak_arena_plan", "cloak_permute_mlp_heads", "cloak_permute_experts", "cloak_load_mlp_heads", "cloak_to_tile128",
+           "cloak_set_copy_engine", "cloak_set_copy_cache_hint", "cloak_arena_plan", "cloak_permute_mlp_heads", "cloak_permute_experts", "cloak_load_mlp_heads", "cloak_to_tile128",
            "cloak_gemv", "cloak_gemv_chain", "cloak_gemm", "cloak_gemm_chain", "cloak_gemv_chain_scratch_bytes",
-           "cloak_gemm_chain_scratch_bytes", "cloak_pool_reserve_workspace", "cloak_set_gemv_engine", "cloak_set_gemm_schedule", "cloak_gemm_plan", "cloak_gemv_host", "cloak_silu_mul"]
+           "cloak_gemm_chain_scratch_bytes", "cloak_pool_reserve_workspace", "cloak_set_gemv_engine", "cloak_sm_weights", "cloak_set_sm_weighting", "cloak_set_trace", "cloak_set_gemm_schedule", "cloak_gemm_plan", "cloak_gemv_host", "cloak_silu_mul"]
 
 
 class CloakError(RuntimeError):
@@ -86,7 +86,11 @@ lib.cloak_rekey_inplace.argtypes = [_P, c_uint64, c_uint64, _P]
 lib.cloak_shuffle_host.argtypes = [_P, _P, c_uint64, c_uint64, _P]
 lib.cloak_unshuffle_host.argtypes = [_P, _P, c_uint64, c_uint64, _P]
 lib.cloak_set_copy_engine.argtypes = [c_int]
+lib.cloak_set_copy_cache_hint.argtypes = [c_int]
 lib.cloak_set_gemv_engine.argtypes = [c_int]
+lib.cloak_sm_weights.argtypes = [c_int, c_uint32, _P, POINTER(c_uint32)]
+lib.cloak_set_sm_weighting.argtypes = [c_int]
+lib.cloak_set_trace.argtypes = [_P]
 lib.cloak_set_gemm_schedule.argtypes = [c_int, c_int]
 lib.cloak_gemm_plan.argtypes = [c_uint32, POINTER(c_uint32), POINTER(c_uint32), c_uint32, c_uint32, c_uint32,
                                 POINTER(c_uint32), POINTER(c_uint32), POINTER(c_uint32), POINTER(c_uint32)]
@@ -244,8 +248,31 @@ def cloak_set_copy_engine(engine):
     _check(lib.cloak_set_copy_engine(engine))
 
 
+def cloak_set_copy_cache_hint(hint):
+    _check(lib.cloak_set_copy_cache_hint(hint))
+
+
 def cloak_set_gemv_engine(engine):
     _check(lib.cloak_set_gemv_engine(engine))
+
+
+def cloak_sm_weights(device=0):
+    """Relative streaming speeds of the device's SMs (mean 1), indexed by SM id; [] if they could not be measured."""
+    n = c_uint32()
+    _check(lib.cloak_sm_weights(device, 0, None, byref(n)))
+    if n.value == 0:
+        return []
+    w = (ctypes.c_float * n.value)()
+    _check(lib.cloak_sm_weights(device, n.value, w, byref(n)))
+    return list(w)
+
+
+def cloak_set_sm_weighting(mode):
+    _check(lib.cloak_set_sm_weighting(mode))
+
+
+def cloak_set_trace(d_trace):
+    _check(lib.cloak_set_trace(_ptr(d_trace)))
 
 
 def cloak_set_gemm_schedule(static_pct, dyn_chunk_tiles=0):

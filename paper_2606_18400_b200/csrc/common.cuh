@@ -120,6 +120,10 @@ cloak_status pool_workspace(const cloak_pool* pool, size_t bytes, cudaStream_t s
 int gemv_stream_chunk(const cloak_pool* pool, const cloak_tensor* w, uint32_t batch);
 cloak_status gemv_stream_launch(const cloak_pool* pool, const cloak_gemv_op* ops, uint32_t n, int cu, uint32_t batch,
                                 cudaStream_t s);
+// calibrate.cu: per-SM streaming weights of a device (measured once, at the first pool_create on it) and the cumulative
+// table cum[0 .. nsm] (16-bit fixed point, indexed by %smid) for kernels that run one CTA on every SM; nullptr = equal shares.
+void ensure_sm_weights(int device);
+const uint32_t* sm_cum_table(int device, uint32_t nsm);
 // Host-side Philox keygen used only by cloak_arena_plan (T is tiny; no device work wanted there).
 void keygen_host(uint64_t key, uint64_t stream_id, uint32_t n, std::vector<uint32_t>& perm);
 

@@ -27,6 +27,7 @@ struct CopyArgs {
     uint32_t first;            // table index of block 0 of this call
     uint32_t nblocks;
     uint32_t log2b;
+    uint32_t hint;             // L2 eviction hints of the TMA engine: bit 0 = stores evict_first, bit 1 = loads evict_first
 };
 
 // 16-byte and 32-byte (sm_100 256-bit LDG/STG) streaming vectors.
@@ -99,6 +100,7 @@ __global__ void __launch_bounds__(TMA_WARPS * 32) copy_tma_kernel(CopyArgs a, ui
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
 
+    const uint64_t pol = l2_policy_evict_first();
     const uint64_t npipes = (uint64_t)gridDim.x * TMA_WARPS;
     const uint64_t pipe = (uint64_t)blockIdx.x * TMA_WARPS + w;
     // number of units this pipeline owns: u = pipe + i * npipes
@@ -111,7 +113,9 @@ __global__ void __launch_bounds__(TMA_WARPS * 32) copy_tma_kernel(CopyArgs a, ui
         const int s = (int)(i % TMA_STAGES);
         const uint32_t bar = smem_u32(&bars[w][s]);
         mbar_expect_tx(bar, chunk);
-        bulk_g2s(smem_u32(ring + (size_t)s * chunk), a.src + ((uint64_t)sj << a.log2b) + ((u & cmask) << log2c), chunk, bar);
+        const char* src = a.src + ((uint64_t)sj << a.log2b) + ((u & cmask) << log2c);
+        if (a.hint & 2) bulk_g2s_hint(smem_u32(ring + (size_t)s * chunk), src, chunk, bar, pol);
+        else bulk_g2s(smem_u32(ring + (size_t)s * chunk), src, chunk, bar);
     };
 
     const uint64_t pre = mine < TMA_STAGES ? mine : TMA_STAGES;
@@ -122,7 +126,9 @@ __global__ void __launch_bounds__(TMA_WARPS * 32) copy_tma_kernel(CopyArgs a, ui
         const uint64_t u = pipe + i * npipes;
         const uint32_t j = (uint32_t)(u >> lc);
         const uint32_t dj = a.dst_tab ? __ldg(a.dst_tab + a.first + j) : j;
-        bulk_s2g(a.dst + ((uint64_t)dj << a.log2b) + ((u & cmask) << log2c), smem_u32(ring + (size_t)s * chunk), chunk);
+        char* dst = a.dst + ((uint64_t)dj << a.log2b) + ((u & cmask) << log2c);
+        if (a.hint & 1) bulk_s2g_hint(dst, smem_u32(ring + (size_t)s * chunk), chunk, pol);
+        else bulk_s2g(dst, smem_u32(ring + (size_t)s * chunk), chunk);
         bulk_commit();
         // Refill the stage used by the *previous* unit once its store has finished reading shared memory.
         if (i >= 1 && i - 1 + TMA_STAGES < mine) {
@@ -142,6 +148,7 @@ struct ManyArgs {
     char* pool;
     const uint32_t* tab;
     uint32_t log2b, log2c, n, to_pool;
+    uint32_t hint, pad_;             // as CopyArgs::hint
     uint64_t ustart[MANY_MAX + 1];   // prefix sums of the ranges' units (chunks)
     char* logical[MANY_MAX];         // first byte of range r in the caller's memory
     uint32_t first[MANY_MAX];        // table index of its first block
@@ -160,6 +167,7 @@ __global__ void __launch_bounds__(TMA_WARPS * 32) copy_tma_many_kernel(const __g
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
 
+    const uint64_t pol = l2_policy_evict_first();
     const uint64_t total_units = a.ustart[a.n];
     const uint64_t npipes = (uint64_t)gridDim.x * TMA_WARPS;
     const uint64_t pipe = (uint64_t)blockIdx.x * TMA_WARPS + w;
@@ -184,7 +192,8 @@ __global__ void __launch_bounds__(TMA_WARPS * 32) copy_tma_many_kernel(const __g
         const int s = (int)(i % TMA_STAGES);
         const uint32_t bar = smem_u32(&bars[w][s]);
         mbar_expect_tx(bar, chunk);
-        bulk_g2s(smem_u32(ring + (size_t)s * chunk), a.to_pool ? lg : pl, chunk, bar);
+        if (a.hint & 2) bulk_g2s_hint(smem_u32(ring + (size_t)s * chunk), a.to_pool ? lg : pl, chunk, bar, pol);
+        else bulk_g2s(smem_u32(ring + (size_t)s * chunk), a.to_pool ? lg : pl, chunk, bar);
     };
     const uint64_t pre = mine < TMA_STAGES ? mine : TMA_STAGES;
     for (uint64_t i = 0; i < pre; ++i) issue_load(i);
@@ -193,7 +202,8 @@ __global__ void __launch_bounds__(TMA_WARPS * 32) copy_tma_many_kernel(const __g
         mbar_wait(smem_u32(&bars[w][s]), (uint32_t)((i / TMA_STAGES) & 1));
         char *lg, *pl;
         locate(pipe + i * npipes, lg, pl);
-        bulk_s2g(a.to_pool ? pl : lg, smem_u32(ring + (size_t)s * chunk), chunk);
+        if (a.hint & 1) bulk_s2g_hint(a.to_pool ? pl : lg, smem_u32(ring + (size_t)s * chunk), chunk, pol);
+        else bulk_s2g(a.to_pool ? pl : lg, smem_u32(ring + (size_t)s * chunk), chunk);
         bulk_commit();
         if (i >= 1 && i - 1 + TMA_STAGES < mine) {
             bulk_wait_read<1>();
@@ -208,6 +218,7 @@ static cloak_status launch_tail(const cloak_pool* pool, char* logical_tail, uint
                                 int to_pool, cudaStream_t s);
 
 static std::atomic<int> g_engine{0};   // 0 auto, 1 LDG, 2 TMA
+static std::atomic<int> g_hint{1};     // L2 hints of the TMA engine (cloak_set_copy_cache_hint): default stores evict_first
 
 static cloak_status launch_copy(const cloak_pool* pool, const CopyArgs& a, cudaStream_t s) {
     if (a.nblocks == 0) return CLOAK_OK;
@@ -266,6 +277,7 @@ static cloak_status move_range(const cloak_pool* pool, char* d_logical, uint64_t
     a.first = first;
     a.nblocks = full;
     a.log2b = pool->log2_block;
+    a.hint = (uint32_t)g_hint.load(std::memory_order_relaxed);
     if (dir == TO_POOL) { a.src = d_logical; a.dst = pool->base; a.src_tab = nullptr; a.dst_tab = pool->d_T; pool->wrote(s); }
     else                { a.src = pool->base; a.dst = d_logical; a.src_tab = pool->d_T; a.dst_tab = nullptr; }
     cloak_status st = launch_copy(pool, a, s);
@@ -342,6 +354,12 @@ extern "C" cloak_status cloak_set_copy_engine(int engine) {
     return CLOAK_OK;
 }
 
+extern "C" cloak_status cloak_set_copy_cache_hint(int hint) {
+    if (hint < 0 || hint > 3) return fail(CLOAK_ERR_INVALID, "set_copy_cache_hint: 0..3 (bit 0 stores, bit 1 loads evict_first)");
+    g_hint.store(hint);
+    return CLOAK_OK;
+}
+
 extern "C" cloak_status cloak_shuffle(cloak_pool* pool, const void* d_logical, uint64_t logical_offset, uint64_t bytes,
                                       void* stream) {
     cloak_status st = check_range(pool, d_logical, logical_offset, bytes, "shuffle");
@@ -386,6 +404,8 @@ static cloak_status move_many(const cloak_pool* pool, uint32_t n, void* const* d
         a.log2b = pool->log2_block;
         a.log2c = a.log2b < 13 ? a.log2b : 13;
         a.to_pool = dir == TO_POOL;
+        a.hint = (uint32_t)g_hint.load(std::memory_order_relaxed);
+        a.pad_ = 0;
         a.n = n - r0 < (uint32_t)MANY_MAX ? n - r0 : (uint32_t)MANY_MAX;
         uint64_t units = 0;
         for (uint32_t r = 0; r < a.n; ++r) {
@@ -455,6 +475,7 @@ extern "C" cloak_status cloak_relayout(const cloak_pool* from_a, cloak_pool* to_
     a.first = 0;
     a.nblocks = from_a->nb;       // whole blocks: the zero tail of the last block travels with it
     a.log2b = from_a->log2_block;
+    a.hint = (uint32_t)g_hint.load(std::memory_order_relaxed);
     to_b->wrote((cudaStream_t)stream);
     return launch_copy(from_a, a, (cudaStream_t)stream);
 }

@@ -347,6 +347,13 @@ extern "C" cloak_status cloak_set_gemv_engine(int engine) {
     return CLOAK_OK;
 }
 
+namespace cloak { extern std::atomic<unsigned long long*> g_trace; }
+extern "C" cloak_status cloak_set_trace(void* d_trace) {
+    if ((uintptr_t)d_trace & 7) return fail(CLOAK_ERR_ALIGN, "set_trace: buffer must be 8-byte aligned");
+    g_trace.store(static_cast<unsigned long long*>(d_trace));
+    return CLOAK_OK;
+}
+
 extern "C" cloak_status cloak_gemv(const cloak_pool* pool, const cloak_tensor* w, const void* d_x, void* d_y,
                                    uint32_t batch, void* stream) {
     cloak_status st = gemv_check(pool, w, d_x, d_y, batch, "gemv");

@@ -51,13 +51,15 @@ struct ChainOp {             // 80 bytes of kernel parameter space per op (10 x 
     uint32_t per;            // units per CTA
     uint32_t ctas;           // CTAs that own units of this op (indices 0 .. ctas-1)
     uint32_t tile_base;      // index of this op's first row-tile counter
-    uint32_t flags;          // OP_SIGNAL
+    uint32_t flags;          // OP_SIGNAL | OP_WEIGHTED
     uint32_t wait_op;        // NO_WAIT, or the index of the op whose completion by ALL CTAs this op's consumers wait for
     uint32_t rot;            // range r of this op belongs to CTA (r + rot) % grid: an op with fewer ranges than CTAs starts
                              // where the previous one stopped, so the idle CTAs are different ones each time (an op with a
                              // gate epilogue keeps the rotation of the op that produced the gate: same rows, same CTA)
 };
-enum { OP_SIGNAL = 2 };      // some later op waits for this one: every CTA reports here when it is done with it (and all before)
+enum { OP_SIGNAL = 2,        // some later op waits for this one: every CTA reports here when it is done with it (and all before)
+       OP_WEIGHTED = 4 };    // the op's ranges are proportional to the SMs' measured streaming speeds: range index = %smid, bounds
+                             // from ChainArgs::cum (calibrate.cu); otherwise equal ranges of `per` units, range index from blockIdx
 constexpr uint32_t NO_WAIT = 0xffffffffu;
 constexpr int GS_MAX_OPS = 48;              // 48 x 80 B + header < 4 KiB of kernel parameters
 
@@ -67,6 +69,8 @@ struct ChainArgs {
     float* part;             // [op][cta][batch * 8]: partial of the cut row tile a CTA meets first in that op
     uint32_t* counters;      // [tile_base + tile]: arrivals of the non-owning contributors; owner resets to 0
     uint32_t* opsync;        // [GS_MAX_OPS] arrivals per signalling op, [GS_MAX_OPS] CTAs done with the launch: the last resets all
+    const uint32_t* cum;     // per-SM cumulative weights, [gridDim.x + 1], 16-bit fixed point (cum[gridDim.x] = 65536); NULL = none
+    unsigned long long* trace;   // NULL, or [gridDim.x][4]: %smid, globaltimer at CTA start, producer done, consumers done
     uint32_t log2b;
     uint32_t batch;
     uint32_t nops;
@@ -130,6 +134,25 @@ __device__ __forceinline__ void red_release_add(uint32_t* p, uint32_t v) {
 // of its wait still observes everything older than its immediate predecessor.
 __device__ __forceinline__ void grid_dep_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
 __device__ __forceinline__ void grid_dep_launch() { asm volatile("griddepcontrol.launch_dependents;" ::: "memory"); }
+__device__ __forceinline__ uint32_t my_smid() {
+    uint32_t s;
+    asm volatile("mov.u32 %0, %%smid;" : "=r"(s));
+    return s;
+}
+__device__ __forceinline__ unsigned long long global_ns() {
+    unsigned long long t;
+    asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t));
+    return t;
+}
+// This CTA's range index of an op and the units [ubeg, uend) it owns.
+__device__ __forceinline__ uint32_t op_rank(const ChainOp& op, uint32_t smid) {
+    return (op.flags & OP_WEIGHTED) ? smid : (blockIdx.x + gridDim.x - op.rot) % gridDim.x;
+}
+__device__ __forceinline__ uint32_t range_begin(const uint32_t* cum, const ChainOp& op, uint32_t r) {
+    if (op.flags & OP_WEIGHTED) return (uint32_t)(((uint64_t)op.units * __ldg(cum + r)) >> 16);
+    const uint64_t b = (uint64_t)r * op.per;
+    return b < op.units ? (uint32_t)b : op.units;
+}
 __device__ __forceinline__ void consumer_bar() { asm volatile("bar.sync 1, %0;" :: "n"(GS_CONSUMERS * 32) : "memory"); }
 
 // silu(g) * u for bf16 inputs, fp32 arithmetic, round to nearest even: bit for bit cloak_silu_mul's result.
@@ -184,11 +207,12 @@ __global__ void __launch_bounds__(gs_threads(NT), 1) gemv_chain_kernel(const __g
         if (!a.early) grid_dep_wait();
         uint32_t s = 0, ph = 0;
         bool wrapped = false;
+        const uint32_t smid = my_smid();
         for (uint32_t j = 0; j < a.nops; ++j) {
             const ChainOp& op = a.ops[j];
             const uint32_t kch = op.kch;
-            const uint32_t vr = (blockIdx.x + gridDim.x - op.rot) % gridDim.x;   // this CTA's range of the op
-            const uint32_t ubeg = vr * op.per, uend = min(ubeg + op.per, op.units);
+            const uint32_t vr = op_rank(op, smid);                                   // this CTA's range of the op
+            const uint32_t ubeg = range_begin(a.cum, op, vr), uend = range_begin(a.cum, op, vr + 1);
             if (ubeg >= uend) continue;
             const uint32_t tile_lo = ubeg / kch, tile_hi = (uend - 1) / kch;
             const uint64_t row_bytes = (uint64_t)op.K * 2;
@@ -227,6 +251,7 @@ __global__ void __launch_bounds__(gs_threads(NT), 1) gemv_chain_kernel(const __g
                 }
             }
         }
+        if (a.trace && lane == 0) a.trace[4 * blockIdx.x + 2] = global_ns();
         return;
     }
 
@@ -241,15 +266,17 @@ __global__ void __launch_bounds__(gs_threads(NT), 1) gemv_chain_kernel(const __g
 
     // X, Y, partials and counters all belong to stream order: nothing below touches them before the predecessor
     // has completed.  Meanwhile the producer is already filling the ring.
+    const unsigned long long t_start = a.trace ? global_ns() : 0ull;
     grid_dep_wait();
     if (ctid == 0) grid_dep_launch();
 
     uint32_t s = 0, ph = 0;
+    const uint32_t smid = my_smid();
     for (uint32_t j = 0; j < a.nops; ++j) {
         const ChainOp& op = a.ops[j];
-        const uint32_t kch = op.kch, per = op.per;
-        const uint32_t vr = (blockIdx.x + gridDim.x - op.rot) % gridDim.x;       // this CTA's range of the op
-        const uint32_t ubeg = vr * per, uend = min(ubeg + per, op.units);
+        const uint32_t kch = op.kch;
+        const uint32_t vr = op_rank(op, smid);                                       // this CTA's range of the op
+        const uint32_t ubeg = range_begin(a.cum, op, vr), uend = range_begin(a.cum, op, vr + 1);
         const bool have = ubeg < uend;
 
         if (have && op.wait_op != NO_WAIT) {
@@ -380,7 +407,11 @@ __global__ void __launch_bounds__(gs_threads(NT), 1) gemv_chain_kernel(const __g
 
             if (cut_tail) {
                 // owner of the tail tile: wait for the other contributors (CTAs after this one), add in CTA order
-                const uint32_t nc = (tile_hi * kch + kch - 1) / per - vr;
+                // the later ranges that begin inside the tile (none of them empty: the host makes sure of that)
+                uint32_t nc = 0;
+                for (uint32_t q = vr + 1; q < gridDim.x && range_begin(a.cum, op, q) <= tile_hi * kch + kch - 1 &&
+                                          range_begin(a.cum, op, q) < op.units; ++q)
+                    ++nc;
                 uint32_t* cnt = a.counters + op.tile_base + tile_hi;
                 if (ctid == 0) {
                     while (ld_acquire(cnt) != nc) __nanosleep(32);
@@ -405,6 +436,11 @@ __global__ void __launch_bounds__(gs_threads(NT), 1) gemv_chain_kernel(const __g
             }
         }
     }
+    if (a.trace && ctid == 0) {
+        a.trace[4 * blockIdx.x + 0] = smid;
+        a.trace[4 * blockIdx.x + 1] = t_start;
+        a.trace[4 * blockIdx.x + 3] = global_ns();
+    }
     // the arrival counters are reset for the next launch by the last CTA to get here (nobody reads them any more)
     if (a.any_signal && ctid == 0) {
         if (atomicAdd(a.opsync + GS_MAX_OPS, 1u) == gridDim.x - 1) {
@@ -427,6 +463,7 @@ constexpr uint32_t GS_TILE_COUNTERS = (uint32_t)(WS_COUNTER_BYTES / 4) - 4 * GS_
 // can be resident, and fails the launch (cudaErrorCooperativeLaunchTooLarge) instead of hanging when that can never be.
 // Whether the cooperative attribute may be combined with programmatic stream serialization is probed on the first launch:
 // if the driver rejects the pair, PDL is dropped, not the guarantee.
+std::atomic<unsigned long long*> g_trace{nullptr};     // cloak_set_trace
 static std::atomic<int> g_coop_with_pdl{-1};     // -1 unknown, 0 rejected, 1 accepted
 int gemv_coop_pdl_state() { return g_coop_with_pdl.load(std::memory_order_relaxed); }
 
@@ -543,6 +580,15 @@ cloak_status gemv_stream_launch(const cloak_pool* pool, const cloak_gemv_op* ops
             if (o.gate && (const void*)a.ops[k].y == (const void*)o.gate) o.rot = a.ops[k].rot;     // same rows, same CTA
         ranges_so_far += o.ctas;
     }
+    // Shares proportional to the SMs' measured streaming speeds (calibrate.cu), for ops large enough that every share is
+    // many units, in launches that put one CTA on every SM and do not rotate: such an op ends on all SMs at once instead of
+    // when the slowest tier of SMs is done (the others' producers then run ahead into the next op, but at every `after` the
+    // whole grid waits for the last).  Shape alone decides, so gate and up of one MLP get the same split.
+    a.cum = (!rotate_all && ctas == sms) ? sm_cum_table(pool->device, (uint32_t)sms) : nullptr;
+    if (a.cum)
+        for (uint32_t j = 0; j < n; ++j)
+            if (a.ops[j].rot == 0 && a.ops[j].units >= 16u * (uint32_t)ctas) a.ops[j].flags |= OP_WEIGHTED;
+    a.trace = g_trace.load(std::memory_order_relaxed);
     const size_t need = WS_COUNTER_BYTES + (size_t)n * ctas * batch * GS_ROWS * 4;
     cloak_status st = pool_workspace(pool, need, s);
     if (st != CLOAK_OK) return st;

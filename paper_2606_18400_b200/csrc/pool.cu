@@ -147,6 +147,7 @@ static cloak_status create_impl(cloak_pool* p) {
     p->d_pageinv = p->d_pageperm + p->npages;
     p->d_T = p->d_pageinv + p->npages;
 
+    ensure_sm_weights(p->device);          // once per device: the streaming GEMV's shares follow the SMs' measured speeds
     cudaStream_t s;
     CLOAK_CUDA(cudaStreamCreateWithFlags(&s, cudaStreamNonBlocking));
     cloak_status st = CLOAK_OK;
