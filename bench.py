@@ -573,7 +573,7 @@ def main():
                     help="what the line carries besides the cfg1 step (`value`): cfg2, cfg3, cfg4 blocks (BASELINE.json configs[2..4]); "
                          "`--configs cfg1` for the step alone.  N > 1 replicas run the step alone.")
     ap.add_argument("--min-seconds", type=float, default=1.0, help="minimum length of each timed loop of the cfg2-4 blocks")
-    ap.add_argument("--sm-weighting", type=int, default=1, help="A/B: cloak_set_sm_weighting (1 measured per-SM shares, 0 equal shares)")
+    ap.add_argument("--sm-weighting", type=int, default=0, help="A/B: cloak_set_sm_weighting (1 measured per-SM shares, 0 equal shares)")
     ap.add_argument("--copy-hint", type=int, default=-1, help="A/B: cloak_set_copy_cache_hint (bit 0 stores, bit 1 loads evict_first)")
     ap.add_argument("--gemv-engine", type=int, default=0,
                     help="A/B: cloak_set_gemv_engine (0 auto, 1 one-shot kernel, 2 no PDL)")

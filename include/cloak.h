@@ -160,8 +160,10 @@ cloak_status cloak_unshuffle_host(const cloak_pool* pool, void* h_logical, uint6
  * LDG/STG, 2 = TMA bulk copy through a shared-memory ring.  For A/B measurement; process-wide. */
 cloak_status cloak_set_copy_engine(int engine);
 
-/* L2 eviction hints of the TMA copy engine: bit 0 = its stores are evict_first, bit 1 = its loads are.  Default 1: a streaming
- * copy should not leave the 126 MB L2 full of dirty lines for the next kernel to write back.  For A/B measurement; process-wide. */
+/* L2 eviction hints of the TMA copy engine: bit 0 = its stores are evict_first, bit 1 = its loads are.  Meant to keep a streaming
+ * copy from leaving the 126 MB L2 full of dirty lines that the next kernel then pays to write back (the GEMV that follows a
+ * re-layout runs 90 us instead of 80); measured on B200: the hint changes neither the copy nor its successor, so the default is 0
+ * (none).  For A/B measurement; process-wide. */
 cloak_status cloak_set_copy_cache_hint(int hint);
 
 /* ---- S3 tensor order.  Host helper, no device work.
@@ -317,12 +319,13 @@ cloak_status cloak_gemm_chain(const cloak_pool* pool, const cloak_gemm_op* h_ops
 cloak_status cloak_set_gemv_engine(int engine);
 /* Per-SM streaming weights (calibrate.cu).  The SMs of a B200 do not pull a read stream out of HBM equally fast (three tiers,
  * up to 1.7 x apart, a property of the individual part); the first cloak_pool_create on a device measures it once (a 1 GiB
- * scratch buffer, a few ms), and the streaming GEMV cuts large ops into STATIC shares proportional to it instead of equal
- * ones (the split is fixed for the life of the process: results stay deterministic, and the same on cloaked and identity-table
- * pools; between processes the last bits of a split-K sum may differ where a weight moved by a quantisation step).
+ * scratch buffer, a few ms), and the streaming GEMV CAN cut large ops into static shares proportional to it instead of equal
+ * ones (the split is then fixed for the life of the process: results stay deterministic, and the same on cloaked and
+ * identity-table pools).  Measured: the GEMV's SMs are limited by their own ring, not by the contended path, and equal shares
+ * already end together; weighted shares are 7 % slower.  So the switch is OFF by default and kept for A/B measurement.
  * cloak_sm_weights: the relative speeds (mean 1) of the device's SMs, indexed by SM id; *h_nsm = 0 if they could not be
  * measured (kernels then use equal shares).  h_weights may be NULL to query the count.  Measures if that has not happened yet.
- * cloak_set_sm_weighting: 0 = equal shares, 1 = measured weights (default).  For A/B measurement; process-wide. */
+ * cloak_set_sm_weighting: 0 = equal shares (default), 1 = measured weights.  Process-wide. */
 cloak_status cloak_sm_weights(int device, uint32_t capacity, float* h_weights, uint32_t* h_nsm);
 cloak_status cloak_set_sm_weighting(int mode);
 /* Tracing: while d_trace is not NULL, every streaming-GEMV launch records, per CTA b, four 64-bit words at d_trace[4*b]: the

@@ -10,6 +10,14 @@
 // shares proportional to speed: balanced like the queue, with no atomics on the producer's path and a split that is
 // fixed for the life of the process (deterministic results).
 //
+// Result (round 2, B200): the weights are real and stable, but the streaming GEMV does NOT profit from
+// them: its SMs are not limited by the contended path to L2 but by their own ring (bytes in flight / loaded latency, the
+// stage also being held while the consumers work through it), so with equal shares all 148 producers already end within
+// 4 us of each other (68 .. 72 us of a 75 us launch), and weighted shares make the "fast" SMs finish LAST: cfg1 layer
+// 79.9 -> 85.5 us (batch 1), 93.7 -> 101.9 us (batch 16).  A pure read stream of large pieces, which does saturate the path,
+// gains 6 % from a dynamic queue over equal shares (58.9 vs 62.4 us for 436 MB).  So the measurement and the weighted split
+// stay in the library as an A/B switch, OFF by default (cloak_set_sm_weighting).
+//
 // How.  One CTA per SM (192 KiB of shared memory each) draws 32 KiB chunks of a scratch buffer from an atomic counter and
 // pulls them with cp.async.bulk through a 6-stage ring; chunks drawn per %smid over two measured passes = the weight.
 // Quantised to 1/64 of the mean so that run-to-run noise (~1 %) rarely moves a share.  The table handed to kernels is
@@ -67,7 +75,7 @@ struct SmWeights {
 };
 static SmWeights g_smw[64];
 static std::mutex g_smw_mu;
-static std::atomic<int> g_weighting{1};      // cloak_set_sm_weighting
+static std::atomic<int> g_weighting{0};      // cloak_set_sm_weighting; off by default (see the note at the top)
 
 static void measure(int device, SmWeights& out) {
     out.state.store(-1);

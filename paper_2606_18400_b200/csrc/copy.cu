@@ -218,7 +218,7 @@ static cloak_status launch_tail(const cloak_pool* pool, char* logical_tail, uint
                                 int to_pool, cudaStream_t s);
 
 static std::atomic<int> g_engine{0};   // 0 auto, 1 LDG, 2 TMA
-static std::atomic<int> g_hint{1};     // L2 hints of the TMA engine (cloak_set_copy_cache_hint): default stores evict_first
+static std::atomic<int> g_hint{0};     // L2 hints of the TMA engine (cloak_set_copy_cache_hint): measured, no effect -> default none
 
 static cloak_status launch_copy(const cloak_pool* pool, const CopyArgs& a, cudaStream_t s) {
     if (a.nblocks == 0) return CLOAK_OK;
