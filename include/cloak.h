@@ -89,8 +89,9 @@ cloak_status cloak_pool_create(int device, uint64_t payload_bytes, uint32_t bloc
                                uint64_t page_bytes, uint64_t key, uint32_t flags, cloak_pool** out);
 cloak_status cloak_pool_destroy(cloak_pool* pool);
 
-/* Any output pointer may be NULL.  *d_base: device address of the pool (the VA view V for real pages,
- * the dump view D for emulated pages).  *d_table: device array T[0..nb).  *is_vmm: 1 for real pages. */
+/* Any output pointer may be NULL.  *d_base: device address of the pool (the VA view V for real pages -- its first half: a pool of
+ * real pages reserves twice its size of virtual addresses, and after a cloak_rekey_pages_* a page may live in the second half,
+ * nslots*block bytes further on, which the table T accounts for -- the dump view D for emulated pages).  *d_table: device array T[0..nb).  *is_vmm: 1 for real pages. */
 cloak_status cloak_pool_info(const cloak_pool* pool, void** d_base, const uint32_t** d_table,
                              uint32_t* nb, uint32_t* nslots, uint32_t* npages, int* is_vmm);
 
@@ -148,6 +149,29 @@ cloak_status cloak_relayout(const cloak_pool* from_a, cloak_pool* to_b, void* st
  * pools of a few hundred MB; 1/64 of the pool is on any).  The cycle decomposition runs on the host: the call
  * synchronises `stream` and returns when the pool is re-keyed; GEMVs issued afterwards read through the new table. */
 cloak_status cloak_rekey_inplace(cloak_pool* pool, uint64_t new_key, uint64_t spare_bytes, void* stream);
+
+/* Re-randomise the PHYSICAL PAGE MAP of a pool under live decode ("At initialization and
+ * then periodically randomizes the mapping of virtual addresses to physical HBM pages", :205-207 "using CUDA VMM APIs ... The only
+ * overhead arises from synchronization points needed to safely remap pages", cadence :207 / :283).
+ * (pageperm', pageinv') = keygen(new_key, 2<<32, npages).  Afterwards VA page v is backed by physical page pageinv'[v] (physical
+ * index = handle-creation order, G6): the dump view becomes D'[pageinv'[v]*P + o] = D[pageinv[v]*P + o]; the VA view, the block
+ * tables' logical content and every result read through the pool are unchanged, bit for bit.  Real (VMM) pages only.
+ *   _begin   draws the new page map (synchronises `stream` once), creates `spare_pages` (1..64; 0 = 1) spare physical pages: the
+ *            only extra memory, released when the re-key completes.  One re-key per pool at a time.
+ *   _step    NON-BLOCKING, to be called between decode steps: unmaps the old addresses of the moves the stream has passed, and
+ *            starts up to max_moves (<= 16) new page moves -- cuMemMap of the destination physical page at the page's address in the
+ *            OTHER half of the pool's (doubled) virtual range, then on `stream` a 2 MiB copy and the switch of the page's block-table
+ *            entries.  Kernels launched before the switch read the old address, kernels launched after it the new one; CUDA graphs
+ *            of cloak_gemv_chain / cloak_gemm_chain stay valid (they hold the table's address, not its contents).  With k spare
+ *            pages k cycles of the page permutation are followed at once, one move each per call.  *h_remaining (may be NULL) =
+ *            pages not yet home; 0 means the re-key is complete and cloak_pool_tables / cloak_pool_dump show the new map.
+ *            Host cost: ~0.3 ms of driver calls per move on B200, on the calling thread, while the GPU runs what was launched before.
+ *   _finish  runs the remaining moves to the end, waiting for each batch (the stop-the-world form), and synchronises `stream`.
+ * While a re-key is in progress, all calls on the pool must be issued on that one `stream`; cloak_rekey_inplace is refused;
+ * cloak_pool_info's d_base addresses half 0 only (tests read the VA view through cloak_unshuffle). */
+cloak_status cloak_rekey_pages_begin(cloak_pool* pool, uint64_t new_key, uint32_t spare_pages, void* stream);
+cloak_status cloak_rekey_pages_step(cloak_pool* pool, uint32_t max_moves, void* stream, uint32_t* h_remaining);
+cloak_status cloak_rekey_pages_finish(cloak_pool* pool, void* stream);
 
 /* Host-buffer variants (end-to-end path): h_logical is a HOST buffer (pinned for full speed); the
  * library stages it through device memory in chunks.  They synchronise `stream` before returning. */

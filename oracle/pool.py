@@ -129,6 +129,21 @@ def relayout(pool_A, T_A, T_B, g):
     return shuffle_into(out, T_B, L, 0, g.b)
 
 
+def rekey_pages(D, g, pageinv_old, pageinv_new):
+    """NEXT-1: the physical page map re-drawn, the VA view untouched ("periodically randomizes the mapping of
+    virtual addresses to physical HBM pages"; "tensor pointers and access semantics remain unchanged").
+
+    D is the dump view under the old page map.  VA page v sat on physical page pageinv_old[v] and sits on
+    pageinv_new[v] afterwards:   D'[pageinv_new[v]*P + o] = D[pageinv_old[v]*P + o]   for every VA page v.
+    """
+    D = np.asarray(D, dtype=np.uint8)
+    out = np.empty_like(D)
+    for v in range(g.npages):
+        src, dst = int(pageinv_old[v]) * g.P, int(pageinv_new[v]) * g.P
+        out[dst:dst + g.P] = D[src:src + g.P]
+    return out
+
+
 def arena_plan(key, sizes, b):
     """O7 tensor order: offsets[t] for tensors of sizes[t] bytes, each padded to a block multiple.
 

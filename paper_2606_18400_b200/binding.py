@@ -24,7 +24,7 @@ STATUS_NAMES = {0: "CLOAK_OK", -1: "CLOAK_ERR_INVALID", -2: "CLOAK_ERR_ALIGN", -
 # every symbol include/cloak.h declares
 SYMBOLS = ["cloak_last_error", "cloak_version", "cloak_runtime_info", "cloak_launch_count", "cloak_keygen", "cloak_pool_create", "cloak_pool_destroy",
            "cloak_pool_info", "cloak_pool_tables", "cloak_pool_dump", "cloak_pool_map_ms", "cloak_pool_adjacency", "cloak_shuffle",
-           "cloak_unshuffle", "cloak_shuffle_many", "cloak_unshuffle_many", "cloak_relayout", "cloak_rekey_inplace", "cloak_shuffle_host", "cloak_unshuffle_host",
+           "cloak_unshuffle", "cloak_shuffle_many", "cloak_unshuffle_many", "cloak_relayout", "cloak_rekey_inplace", "cloak_rekey_pages_begin", "cloak_rekey_pages_step", "cloak_rekey_pages_finish", "cloak_shuffle_host", "cloak_unshuffle_host",
            "cloak_set_copy_engine", "cloak_set_copy_cache_hint", "cloak_arena_plan", "cloak_permute_mlp_heads", "cloak_permute_experts", "cloak_load_mlp_heads", "cloak_to_tile128",
            "cloak_gemv", "cloak_gemv_chain", "cloak_gemm", "cloak_gemm_chain", "cloak_gemv_chain_scratch_bytes",
            "cloak_gemm_chain_scratch_bytes", "cloak_pool_reserve_workspace", "cloak_set_gemv_engine", "cloak_sm_weights", "cloak_set_sm_weighting", "cloak_set_trace", "cloak_set_gemm_schedule", "cloak_gemm_plan", "cloak_gemv_host", "cloak_silu_mul"]
@@ -83,6 +83,9 @@ lib.cloak_shuffle_many.argtypes = [_P, c_uint32, POINTER(c_void_p), POINTER(c_ui
 lib.cloak_unshuffle_many.argtypes = [_P, c_uint32, POINTER(c_void_p), POINTER(c_uint64), POINTER(c_uint64), _P]
 lib.cloak_relayout.argtypes = [_P, _P, _P]
 lib.cloak_rekey_inplace.argtypes = [_P, c_uint64, c_uint64, _P]
+lib.cloak_rekey_pages_begin.argtypes = [_P, c_uint64, c_uint32, _P]
+lib.cloak_rekey_pages_step.argtypes = [_P, c_uint32, _P, POINTER(c_uint32)]
+lib.cloak_rekey_pages_finish.argtypes = [_P, _P]
 lib.cloak_shuffle_host.argtypes = [_P, _P, c_uint64, c_uint64, _P]
 lib.cloak_unshuffle_host.argtypes = [_P, _P, c_uint64, c_uint64, _P]
 lib.cloak_set_copy_engine.argtypes = [c_int]
@@ -234,6 +237,21 @@ def cloak_relayout(from_a, to_b, stream=None):
 
 def cloak_rekey_inplace(pool, new_key, spare_bytes=0, stream=None):
     _check(lib.cloak_rekey_inplace(pool, new_key, spare_bytes, _stream(stream)))
+
+
+def cloak_rekey_pages_begin(pool, new_key, spare_pages=1, stream=None):
+    _check(lib.cloak_rekey_pages_begin(pool, new_key, spare_pages, _stream(stream)))
+
+
+def cloak_rekey_pages_step(pool, max_moves, stream=None):
+    """Returns the number of pages not yet home (0 = the re-key is complete)."""
+    left = c_uint32()
+    _check(lib.cloak_rekey_pages_step(pool, max_moves, _stream(stream), byref(left)))
+    return left.value
+
+
+def cloak_rekey_pages_finish(pool, stream=None):
+    _check(lib.cloak_rekey_pages_finish(pool, _stream(stream)))
 
 
 def cloak_shuffle_host(pool, h_logical, logical_offset, nbytes, stream=None):

@@ -137,8 +137,9 @@ static void measure(int device, SmWeights& out) {
 }
 
 // Measured at most once per device and process; call with the device current, outside stream capture (pool_create does).
-void ensure_sm_weights(int device) {
+void ensure_sm_weights(int device, bool only_if_enabled) {
     if (device < 0 || device >= 64) return;
+    if (only_if_enabled && !g_weighting.load(std::memory_order_relaxed)) return;
     std::lock_guard<std::mutex> lock(g_smw_mu);
     if (g_smw[device].state.load() == 0) measure(device, g_smw[device]);
 }
@@ -165,7 +166,7 @@ extern "C" cloak_status cloak_sm_weights(int device, uint32_t capacity, float* h
     {
         DeviceGuard g(device);
         if (!g.ok) return fail(CLOAK_ERR_CUDA, "sm_weights: cannot select device %d", device);
-        ensure_sm_weights(device);
+        ensure_sm_weights(device, false);
     }
     const SmWeights& w = g_smw[device];
     if (w.state.load() != 1) {

@@ -558,7 +558,8 @@ static cloak_status gemm_launch(const cloak_pool* pool, const cloak_gemm_op* ops
     cloak_status st;
     if (!pool->tmap_ready) {
         cloak_pool* p = const_cast<cloak_pool*>(pool);
-        st = make_map(&p->tmap_tile128, pool->base, 128, pool->bytes() / 256, 256, 64, 128);
+        // (real pages: both halves of the pool's virtual range, see cloak_pool::page_half; unmapped parts are never addressed)
+        st = make_map(&p->tmap_tile128, pool->base, 128, (pool->vmm ? 2 : 1) * (pool->bytes() / 256), 256, 64, 128);
         if (st != CLOAK_OK) return st;
         p->tmap_ready = true;
     }

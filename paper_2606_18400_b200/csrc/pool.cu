@@ -5,6 +5,7 @@
 // Table 1b :192-201); pages are allocated in permuted order *before* any weight is transferred
 // (PAPER.md:217).  Definitions O4-O5 and reading G6 of SURVEY.md 8(c): handle-creation order stands for
 // physical order; emulated pages fold the page map into the table.
+#include <string.h>
 #include <chrono>
 #include "common.cuh"
 
@@ -17,12 +18,20 @@ __global__ void iota_kernel(uint32_t* a, uint32_t n) {
 
 // T[i] = blockinv[i] (real pages)  or  pageinv[blockinv[i] / bpp] * bpp + blockinv[i] % bpp (emulated).
 __global__ void build_table_kernel(const uint32_t* __restrict__ blockinv, const uint32_t* __restrict__ pageinv,
-                                   uint32_t* __restrict__ T, uint32_t nb, uint32_t bpp, int vmm) {
+                                   const uint32_t* __restrict__ pageoff, uint32_t* __restrict__ T, uint32_t nb, uint32_t bpp,
+                                   int vmm) {
     uint32_t i = blockIdx.x * blockDim.x + threadIdx.x;
     if (i < nb) {
         uint32_t s = blockinv[i];
-        T[i] = vmm ? s : pageinv[s / bpp] * bpp + s % bpp;
+        T[i] = vmm ? s + pageoff[s / bpp] : pageinv[s / bpp] * bpp + s % bpp;
     }
+}
+cloak_status launch_build_table(const cloak_pool* p, cudaStream_t s) {
+    build_table_kernel<<<(p->nb + 255) / 256, 256, 0, s>>>(p->d_blockinv, p->d_pageinv, p->d_pageoff, p->d_T, p->nb, p->bpp,
+                                                           p->vmm ? 1 : 0);
+    launched();
+    CLOAK_LAUNCH_CHECK();
+    return CLOAK_OK;
 }
 
 // Layout quality: how many logical neighbours (i, i+1) are still neighbours in the VA view, in the
@@ -58,9 +67,17 @@ static cloak_status destroy_impl(cloak_pool* p) {
             d->MemUnmap((CUdeviceptr)p->alias, p->bytes());
             d->MemAddressFree((CUdeviceptr)p->alias, p->bytes());
         }
+        rekey_pages_abandon(p);
         if (p->base) {
-            d->MemUnmap((CUdeviceptr)p->base, p->bytes());
-            d->MemAddressFree((CUdeviceptr)p->base, p->bytes());
+            bool all0 = true;
+            for (uint8_t h : p->page_half) all0 = all0 && h == 0;
+            if (all0 && p->page_half.size() == p->npages && p->handles.size() >= p->npages) {
+                d->MemUnmap((CUdeviceptr)p->base, p->bytes());
+            } else {                                               // pages sit in either half (or creation failed half-way)
+                for (uint32_t v = 0; v < p->npages && v < p->page_half.size(); ++v)
+                    d->MemUnmap((CUdeviceptr)p->page_va(v, p->page_half[v]), p->page);
+            }
+            d->MemAddressFree((CUdeviceptr)p->base, 2 * p->bytes());
         }
         for (auto h : p->handles) d->MemRelease(h);
     } else if (p->base) {
@@ -82,7 +99,7 @@ static cloak_status map_pages(cloak_pool* p, const std::vector<uint32_t>& pagein
     prop.location.id = p->device;
     auto t0 = std::chrono::steady_clock::now();
     CUdeviceptr va = 0;
-    CLOAK_CU(d->MemAddressReserve(&va, p->bytes(), 0, 0, 0));
+    CLOAK_CU(d->MemAddressReserve(&va, 2 * p->bytes(), 0, 0, 0));     // two halves (see cloak_pool::page_half); half 1 starts unmapped
     p->base = (char*)va;
     p->handles.reserve(p->npages);
     for (uint32_t i = 0; i < p->npages; ++i) {          // creation order == physical page index (G6)
@@ -139,15 +156,16 @@ static cloak_status create_impl(cloak_pool* p) {
         CLOAK_CU(d->MemGetAllocationGranularity(&gran, &prop, CU_MEM_ALLOC_GRANULARITY_MINIMUM));
         p->vmm = gran != 0 && p->page % gran == 0;
     }
-    const size_t ntab = 2 * (size_t)p->nslots + 2 * (size_t)p->npages + p->nb;
+    const size_t ntab = 2 * (size_t)p->nslots + 3 * (size_t)p->npages + p->nb;
     CLOAK_CUDA(cudaMalloc((void**)&p->d_tables, ntab * sizeof(uint32_t)));
     p->d_blockperm = p->d_tables;
     p->d_blockinv = p->d_blockperm + p->nslots;
     p->d_pageperm = p->d_blockinv + p->nslots;
     p->d_pageinv = p->d_pageperm + p->npages;
-    p->d_T = p->d_pageinv + p->npages;
+    p->d_pageoff = p->d_pageinv + p->npages;
+    p->d_T = p->d_pageoff + p->npages;
 
-    ensure_sm_weights(p->device);          // once per device: the streaming GEMV's shares follow the SMs' measured speeds
+    ensure_sm_weights(p->device, true);    // once per device, if cloak_set_sm_weighting(1): the GEMV's shares follow the SMs' measured speeds
     cudaStream_t s;
     CLOAK_CUDA(cudaStreamCreateWithFlags(&s, cudaStreamNonBlocking));
     cloak_status st = CLOAK_OK;
@@ -168,11 +186,14 @@ static cloak_status create_impl(cloak_pool* p) {
             e = keygen_device(p->key, 2ull << 32, p->npages, p->d_pageperm, p->d_pageinv, s);
             if (e != CLOAK_OK) return e;
         }
-        build_table_kernel<<<(p->nb + 255) / 256, 256, 0, s>>>(p->d_blockinv, p->d_pageinv, p->d_T, p->nb, p->bpp,
-                                                               p->vmm ? 1 : 0);
-        launched();
-        CLOAK_LAUNCH_CHECK();
-        std::vector<uint32_t> pageinv(p->npages);
+        CLOAK_CUDA(cudaMemsetAsync(p->d_pageoff, 0, (size_t)p->npages * 4, s));       // every page starts in half 0
+        cloak_status bt = launch_build_table(p, s);
+        if (bt != CLOAK_OK) return bt;
+        p->h_pageperm.resize(p->npages);
+        p->h_pageinv.resize(p->npages);
+        p->page_half.assign(p->npages, 0);
+        std::vector<uint32_t>& pageinv = p->h_pageinv;
+        CLOAK_CUDA(cudaMemcpyAsync(p->h_pageperm.data(), p->d_pageperm, (size_t)p->npages * 4, cudaMemcpyDeviceToHost, s));
         CLOAK_CUDA(cudaMemcpyAsync(pageinv.data(), p->d_pageinv, (size_t)p->npages * 4, cudaMemcpyDeviceToHost, s));
         CLOAK_CUDA(cudaStreamSynchronize(s));
         if (p->vmm) {
@@ -263,8 +284,9 @@ extern "C" cloak_status cloak_pool_tables(const cloak_pool* pool, uint32_t* h_bl
     DeviceGuard g(pool->device);
     if (h_blockperm) CLOAK_CUDA(cudaMemcpy(h_blockperm, pool->d_blockperm, (size_t)pool->nslots * 4, cudaMemcpyDeviceToHost));
     if (h_blockinv) CLOAK_CUDA(cudaMemcpy(h_blockinv, pool->d_blockinv, (size_t)pool->nslots * 4, cudaMemcpyDeviceToHost));
-    if (h_pageperm) CLOAK_CUDA(cudaMemcpy(h_pageperm, pool->d_pageperm, (size_t)pool->npages * 4, cudaMemcpyDeviceToHost));
-    if (h_pageinv) CLOAK_CUDA(cudaMemcpy(h_pageinv, pool->d_pageinv, (size_t)pool->npages * 4, cudaMemcpyDeviceToHost));
+    // the page map in force (host copies: a finished page re-key publishes them at once, the device copies in stream order)
+    if (h_pageperm) memcpy(h_pageperm, pool->h_pageperm.data(), (size_t)pool->npages * 4);
+    if (h_pageinv) memcpy(h_pageinv, pool->h_pageinv.data(), (size_t)pool->npages * 4);
     return CLOAK_OK;
 }
 

@@ -20,16 +20,6 @@
 
 namespace cloak {
 
-// T[i] = blockinv[i] (real pages)  or  pageinv[blockinv[i] / bpp] * bpp + blockinv[i] % bpp (emulated), as in pool.cu.
-static __global__ void rekey_table_kernel(const uint32_t* __restrict__ blockinv, const uint32_t* __restrict__ pageinv,
-                                          uint32_t* __restrict__ T, uint32_t nb, uint32_t bpp, int vmm) {
-    const uint32_t i = blockIdx.x * blockDim.x + threadIdx.x;
-    if (i < nb) {
-        const uint32_t v = blockinv[i];
-        T[i] = vmm ? v : pageinv[v / bpp] * bpp + v % bpp;
-    }
-}
-
 constexpr int RK_WARPS = 4;          // independent pipelines per CTA
 constexpr int RK_STAGES = 4;
 constexpr uint32_t RK_SPARE = 0x80000000u;   // a move endpoint with this bit set is a block of the spare buffer
@@ -94,6 +84,7 @@ extern "C" cloak_status cloak_rekey_inplace(cloak_pool* pool, uint64_t new_key, 
     if (!pool) return fail(CLOAK_ERR_INVALID, "rekey_inplace: NULL pool");
     if (pool->flags & CLOAK_POOL_IDENTITY) return fail(CLOAK_ERR_INVALID, "rekey_inplace: an identity pool has no key");
     if (pool->log2_block < 4) return fail(CLOAK_ERR_UNSUPPORTED, "rekey_inplace: block_bytes must be >= 16");
+    if (pool->rk) return fail(CLOAK_ERR_INVALID, "rekey_inplace: a page re-key of this pool is in progress");
     DeviceGuard g(pool->device);
     cudaStream_t s = (cudaStream_t)stream;
     const uint32_t n = pool->nslots, b = pool->block, bpp = pool->bpp;
@@ -112,8 +103,9 @@ extern "C" cloak_status cloak_rekey_inplace(cloak_pool* pool, uint64_t new_key, 
 
     // ---- sigma over the slots of the pool's memory: the block in slot_A(i) goes to slot_B(i), i over ALL nslots
     // logical indices (the zero pad blocks move too, so the result is the oracle's relayout, pad slots included)
-    auto mem_slot = [&](uint32_t v) { return pool->vmm ? v : pageinv[v / bpp] * bpp + v % bpp; };
-    std::vector<uint32_t> sigma(n);
+    // (real pages: the slot's page may sit in either half of the pool's virtual range, see cloak_pool::page_half)
+    auto mem_slot = [&](uint32_t v) { return pool->vmm ? v + (uint32_t)pool->page_half[v / bpp] * n : pageinv[v / bpp] * bpp + v % bpp; };
+    std::vector<uint32_t> sigma(2 * (size_t)n, 0xffffffffu);          // indexed by memory slot; slots of unmapped halves stay unused
     for (uint32_t i = 0; i < n; ++i) sigma[mem_slot(inv_a[i])] = mem_slot(inv_b[i]);
 
     // ---- segment length from the spare budget (default: one page)
@@ -125,12 +117,12 @@ extern "C" cloak_status cloak_rekey_inplace(cloak_pool* pool, uint64_t new_key, 
     if (m < 2) m = 2;
 
     // ---- cycles -> segments -> per-pipeline move lists (pass 1: saves; pass 2: the segments, each in execution order)
-    std::vector<uint8_t> seen(n, 0);
+    std::vector<uint8_t> seen(2 * (size_t)n, 0);
     std::vector<uint32_t> cyc;
     std::vector<std::vector<uint2>> save(npipes), run(npipes);
     uint32_t nseg = 0;
-    for (uint32_t s0 = 0; s0 < n; ++s0) {
-        if (seen[s0] || sigma[s0] == s0) { seen[s0] = 1; continue; }
+    for (uint32_t s0 = 0; s0 < 2 * n; ++s0) {
+        if (seen[s0] || sigma[s0] == s0 || sigma[s0] == 0xffffffffu) { seen[s0] = 1; continue; }
         cyc.clear();
         for (uint32_t v = s0; !seen[v]; v = sigma[v]) { seen[v] = 1; cyc.push_back(v); }
         const uint32_t L = (uint32_t)cyc.size();
@@ -178,10 +170,7 @@ extern "C" cloak_status cloak_rekey_inplace(cloak_pool* pool, uint64_t new_key, 
     }
     CLOAK_LAUNCH_CHECK();
     CLOAK_CUDA(cudaMemcpyAsync(pool->d_blockperm, d_new, (size_t)2 * n * 4, cudaMemcpyDeviceToDevice, s));   // perm | inv are adjacent
-    rekey_table_kernel<<<(pool->nb + 255) / 256, 256, 0, s>>>(pool->d_blockinv, pool->d_pageinv, pool->d_T, pool->nb, bpp,
-                                                              pool->vmm ? 1 : 0);
-    launched();
-    CLOAK_LAUNCH_CHECK();
+    if (cloak_status bt = launch_build_table(pool, s)) return bt;
     pool->key = new_key;
     // the host lists were copied from pageable memory: the copies above have consumed them when the calls returned
     CLOAK_CUDA(cudaStreamSynchronize(s));

@@ -395,6 +395,37 @@ def test_error_measures():
     assert abs(O.err_elementwise_floored(y, yr) - 0.001 / rms) < 1e-15
 
 
+def test_rekey_pages_moves_physical_pages_and_leaves_the_va_view_alone():
+    """NEXT-1 oracle.  Hand example on W1's pool (3 pages of 4 slots, V holds logical
+    blocks [8,4,1,2 | 11,10,7,9 | 0,6,5,3], pageinv = [2,0,1], D = [11,10,7,9 | 0,6,5,3 | 8,4,1,2]).  With the new page map
+    pageinv' = [1,2,0] VA page 0 goes to physical page 1, page 1 to 2, page 2 to 0:  D' = [0,6,5,3 | 8,4,1,2 | 11,10,7,9].
+    Then the general pins: D' equals the dump of the SAME V under the new map (two routes), the old map gives D back, and a
+    re-key to the same map is the identity.  (A mistake such as moving page pageperm[v] instead of pageinv[v], or applying
+    the new map to D's index instead of V's, fails the hand example: W1's page permutation is not an involution.)"""
+    g = O.pool_geometry(192, 16, 64)
+    V_blocks = [8, 4, 1, 2, 11, 10, 7, 9, 0, 6, 5, 3]
+    V = np.repeat(np.array(V_blocks, dtype=np.uint8), 16)
+    D = O.dump_view(V, g, [2, 0, 1])
+    assert D[::16].tolist() == [11, 10, 7, 9, 0, 6, 5, 3, 8, 4, 1, 2]                   # W1's dump view
+    D2 = O.rekey_pages(D, g, [2, 0, 1], [1, 2, 0])
+    assert D2[::16].tolist() == [0, 6, 5, 3, 8, 4, 1, 2, 11, 10, 7, 9]                   # written out by hand above
+    rng = np.random.default_rng(7)
+    g = O.pool_geometry(40 * 4096, 256, 4096)
+    V = rng.integers(0, 256, g.nslots * g.b, dtype=np.uint8)
+    ta, tb = O.pool_tables(0x1234, g), O.pool_tables(0x5678, g)
+    Da = O.dump_view(V, g, ta.pageinv)
+    Db = O.rekey_pages(Da, g, ta.pageinv, tb.pageinv)
+    assert np.array_equal(Db, O.dump_view(V, g, tb.pageinv)) and not np.array_equal(Da, Db)
+    assert np.array_equal(O.rekey_pages(Db, g, tb.pageinv, ta.pageinv), Da)
+    assert np.array_equal(O.rekey_pages(Da, g, ta.pageinv, ta.pageinv), Da)
+    # brute force, byte by byte, on a small case
+    ref = np.empty_like(Da)
+    for v in range(g.npages):
+        for o in range(g.P):
+            ref[int(tb.pageinv[v]) * g.P + o] = Da[int(ta.pageinv[v]) * g.P + o]
+    assert np.array_equal(ref, Db)
+
+
 def test_adjacent_fraction_brute_force_counts_ascending_neighbours_only():
     """A hand-written table with ascending pairs (7,8) (2,3) (9,10), DESCENDING pairs (5,4) (1,0) and gaps: only
     T[i+1] == T[i] + 1 counts (G8; cloak.h cloak_pool_adjacency).  Counting |delta| == 1 would give 5/9, T[i+1] == T[i] - 1
