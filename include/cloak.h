@@ -242,6 +242,31 @@ cloak_status cloak_load_mlp_heads(uint64_t key, const cloak_block_shape* shape, 
                                   const void* d_q, const void* d_k, const void* d_v, const void* d_o,
                                   const uint64_t* h_offsets, void* stream);
 
+/* ---- S3 + S5 + layout + S4 in one pass: the load path of a whole model (PAPER.md:173-177 the load is
+ * "the only phase in which the full set of weight transfers crosses the PCIe bus", Tier 1 hides its order; :217 the permutation
+ * and the pages are decided before any weight is transferred).
+ * Each item is one tensor of a decoder layer (role GATE .. O: shape from `shape`, permutation that of cloak_permute_mlp_heads
+ * for item.layer -- shape->layer is ignored) or a PLAIN [N, K] matrix that is not permuted (embeddings, lm_head, a router).
+ * The tensor is read ONCE from item.src -- a device pointer, or a pointer to pinned (page-locked, device-mapped) host memory,
+ * which the gather kernels then read across PCIe themselves: no staging copy -- and written straight through the pool's block
+ * table at arena byte item.arena_offset (a block multiple) in `layout` (CLOAK_ROWMAJOR, or CLOAK_TILE128: the storage
+ * conversion is an address computation in the same pass; N and K multiples of 128).  The pool bytes afterwards equal those of
+ * cloak_permute_mlp_heads (-> cloak_to_tile128) -> cloak_shuffle, tail of a final partial block zeroed: 2 bytes of traffic per
+ * payload byte instead of 4 or 6.  The items are issued in ascending arena_offset, i.e. in cloak_arena_plan's keyed tensor
+ * order, whatever order the caller lists them in.  h_items is a HOST array, not referenced after the call returns; ranges must
+ * not overlap.  Asynchronous on `stream`. */
+typedef enum { CLOAK_ROLE_GATE = 0, CLOAK_ROLE_UP = 1, CLOAK_ROLE_DOWN = 2, CLOAK_ROLE_Q = 3, CLOAK_ROLE_K = 4,
+               CLOAK_ROLE_V = 5, CLOAK_ROLE_O = 6, CLOAK_ROLE_PLAIN = 7 } cloak_role;
+typedef struct {
+    const void* src;
+    uint64_t arena_offset;
+    uint32_t layer;
+    uint32_t role;      /* cloak_role */
+    uint32_t N, K;      /* CLOAK_ROLE_PLAIN only */
+} cloak_load_item;
+cloak_status cloak_load_tensors(uint64_t key, const cloak_block_shape* shape, cloak_pool* pool,
+                                const cloak_load_item* h_items, uint32_t n, cloak_layout layout, void* stream);
+
 /* Storage-layout conversion ROWMAJOR -> TILE128 of a logical [N, K] matrix (N, K multiples of 128).
  * Out of place.  Asynchronous on `stream`. */
 cloak_status cloak_to_tile128(const void* d_src, void* d_dst, uint32_t N, uint32_t K, cloak_dtype dt,

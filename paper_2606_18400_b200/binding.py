@@ -25,7 +25,7 @@ STATUS_NAMES = {0: "CLOAK_OK", -1: "CLOAK_ERR_INVALID", -2: "CLOAK_ERR_ALIGN", -
 SYMBOLS = ["cloak_last_error", "cloak_version", "cloak_runtime_info", "cloak_launch_count", "cloak_keygen", "cloak_pool_create", "cloak_pool_destroy",
            "cloak_pool_info", "cloak_pool_tables", "cloak_pool_dump", "cloak_pool_map_ms", "cloak_pool_adjacency", "cloak_shuffle",
            "cloak_unshuffle", "cloak_shuffle_many", "cloak_unshuffle_many", "cloak_relayout", "cloak_rekey_inplace", "cloak_rekey_pages_begin", "cloak_rekey_pages_step", "cloak_rekey_pages_finish", "cloak_shuffle_host", "cloak_unshuffle_host",
-           "cloak_set_copy_engine", "cloak_set_copy_cache_hint", "cloak_arena_plan", "cloak_permute_mlp_heads", "cloak_permute_experts", "cloak_load_mlp_heads", "cloak_to_tile128",
+           "cloak_set_copy_engine", "cloak_set_copy_cache_hint", "cloak_arena_plan", "cloak_permute_mlp_heads", "cloak_permute_experts", "cloak_load_mlp_heads", "cloak_load_tensors", "cloak_to_tile128",
            "cloak_gemv", "cloak_gemv_chain", "cloak_gemm", "cloak_gemm_chain", "cloak_gemv_chain_scratch_bytes",
            "cloak_gemm_chain_scratch_bytes", "cloak_pool_reserve_workspace", "cloak_set_gemv_engine", "cloak_sm_weights", "cloak_set_sm_weighting", "cloak_set_trace", "cloak_set_gemm_schedule", "cloak_gemm_plan", "cloak_gemv_host", "cloak_silu_mul"]
 
@@ -43,6 +43,13 @@ class cloak_block_shape(Structure):
 
 class cloak_moe_shape(Structure):
     _fields_ = [("hidden", c_uint32), ("inter", c_uint32), ("n_experts", c_uint32), ("dt", c_int), ("layer", c_uint32)]
+
+
+class cloak_load_item(Structure):
+    _fields_ = [("src", c_void_p), ("arena_offset", c_uint64), ("layer", c_uint32), ("role", c_uint32), ("N", c_uint32), ("K", c_uint32)]
+
+
+CLOAK_ROLE = {"gate": 0, "up": 1, "down": 2, "q": 3, "k": 4, "v": 5, "o": 6, "plain": 7}
 
 
 class cloak_tensor(Structure):
@@ -102,6 +109,7 @@ lib.cloak_permute_mlp_heads.argtypes = [c_uint64, POINTER(cloak_block_shape)] + 
 lib.cloak_permute_experts.argtypes = [c_uint64, POINTER(cloak_moe_shape)] + [_P] * 9
 lib.cloak_load_mlp_heads.argtypes = [c_uint64, POINTER(cloak_block_shape), _P] + [_P] * 7 + [POINTER(c_uint64), _P]
 lib.cloak_to_tile128.argtypes = [_P, _P, c_uint32, c_uint32, c_int, _P]
+lib.cloak_load_tensors.argtypes = [c_uint64, POINTER(cloak_block_shape), _P, POINTER(cloak_load_item), c_uint32, c_int, _P]
 lib.cloak_gemv.argtypes = [_P, POINTER(cloak_tensor), _P, _P, c_uint32, _P]
 lib.cloak_gemv_chain.argtypes = [_P, POINTER(cloak_gemv_op), c_uint32, c_uint32, _P]
 lib.cloak_gemm_chain.argtypes = [_P, POINTER(cloak_gemm_op), c_uint32, c_uint32, _P]
@@ -339,6 +347,21 @@ def cloak_load_mlp_heads(key, shape, pool, offsets, gate=None, up=None, down=Non
     arr = (c_uint64 * 7)(*offsets)
     ptrs = [_ptr(t) for t in (gate, up, down, q, k, v, o)]
     _check(lib.cloak_load_mlp_heads(key, byref(shape), pool, *ptrs, arr, _stream(stream)))
+
+
+def cloak_load_items(items):
+    """Marshals [(src, arena_offset, layer, role name or number[, N, K]), ...] into a ctypes array for cloak_load_tensors."""
+    arr = (cloak_load_item * len(items))()
+    for o, it in zip(arr, items):
+        src, off, layer, role = it[:4]
+        N, K = it[4:] if len(it) == 6 else (0, 0)
+        o.src, o.arena_offset, o.layer, o.role, o.N, o.K = _ptr(src), off, layer, CLOAK_ROLE.get(role, role), N, K
+    return arr
+
+
+def cloak_load_tensors(key, shape, pool, items, layout=CLOAK_ROWMAJOR, stream=None):
+    arr = items if isinstance(items, ctypes.Array) else cloak_load_items(items)
+    _check(lib.cloak_load_tensors(key, byref(shape), pool, arr, len(arr), layout, _stream(stream)))
 
 
 def cloak_to_tile128(d_src, d_dst, N, K, dt, stream=None):

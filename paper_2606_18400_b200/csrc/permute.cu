@@ -11,6 +11,7 @@
 //             flight), the expanded column map sits in shared memory too, output vectors are assembled from
 //             shared memory and stored coalesced; column groups that are whole 16-byte vectors (heads) skip
 //             the staging and move vectors directly.
+#include <algorithm>
 #include "common.cuh"
 #include "async.cuh"
 #include "philox.cuh"
@@ -56,16 +57,26 @@ __device__ __forceinline__ int4 ldg_stream(const void* p) {
 // Where a gathered 16-byte vector goes.  PlainDst: a caller-owned tensor.  PoolDst: straight into a pool through its
 // block table (the fused load path: permutation and block scatter in ONE pass over the bytes
 // instead of two) -- vector index v of the tensor is arena byte off + 16 v, translated like every other access.
+// store(row, cv, vpr, x): vector cv of row `row` of a matrix whose rows hold vpr vectors.
 struct PlainDst {
     int4* p;
-    __device__ __forceinline__ void store(uint64_t v, const int4& x) const { p[v] = x; }
+    __device__ __forceinline__ void store(uint64_t row, uint32_t cv, uint32_t vpr, const int4& x) const { p[row * vpr + cv] = x; }
 };
+// vptr == 0: CLOAK_ROWMAJOR storage.  vptr != 0: CLOAK_TILE128 storage (O11), vptr = vectors per tile row (16 for bf16, 32 for
+// f32): the vector belongs to tile (row / 128, cv / vptr), at vector (row % 128) * vptr + cv % vptr inside it -- the storage
+// conversion costs an address computation, not a pass over the bytes.
 struct PoolDst {
     char* pool;
     const uint32_t* T;
     uint64_t off;
     uint32_t log2b;
-    __device__ __forceinline__ void store(uint64_t v, const int4& x) const {
+    uint32_t vptr;
+    __device__ __forceinline__ void store(uint64_t row, uint32_t cv, uint32_t vpr, const int4& x) const {
+        uint64_t v = row * vpr + cv;
+        if (vptr) {
+            const uint64_t tile = (row >> 7) * (vpr / vptr) + cv / vptr;
+            v = tile * 128 * vptr + (row & 127) * vptr + cv % vptr;
+        }
         const uint64_t a = off + (v << 4);
         const uint32_t slot = __ldg(T + (a >> log2b));
         *reinterpret_cast<int4*>(pool + ((uint64_t)slot << log2b) + (a & ((1ull << log2b) - 1))) = x;
@@ -83,7 +94,7 @@ __global__ void __launch_bounds__(256) gather_rows_kernel(const int4* __restrict
 #pragma unroll
         for (int k = 0; k < ROWS_PER_IT; ++k) {
             const uint32_t r = r0 + k;
-            srow[k] = r < nrows ? __ldg(map + r / seg) * seg + r % seg : 0u;
+            srow[k] = r >= nrows ? 0u : (map ? __ldg(map + r / seg) * seg + r % seg : r);     // (no map: rows as they are)
         }
         for (uint32_t v = threadIdx.x; v < vpr; v += blockDim.x) {
             int4 x[ROWS_PER_IT];
@@ -92,7 +103,7 @@ __global__ void __launch_bounds__(256) gather_rows_kernel(const int4* __restrict
                 if (r0 + k < nrows) x[k] = ldg_stream(src + (uint64_t)srow[k] * vpr + v);
 #pragma unroll
             for (int k = 0; k < ROWS_PER_IT; ++k)
-                if (r0 + k < nrows) dst.store((uint64_t)(r0 + k) * vpr + v, x[k]);
+                if (r0 + k < nrows) dst.store(r0 + k, v, vpr, x[k]);
         }
     }
 }
@@ -139,17 +150,17 @@ __global__ void __launch_bounds__(512) gather_cols_kernel(const E* __restrict__ 
         if (two) mbar_wait(smem_u32(&full[sb]), ((k + 1) / ns) & 1);
         const E* ra = reinterpret_cast<const E*>(ring + (size_t)sa * row_bytes);
         const E* rb = reinterpret_cast<const E*>(ring + (size_t)sb * row_bytes);
-        const uint64_t va = (uint64_t)(blockIdx.x + k * gridDim.x) * vpr, vb = va + (uint64_t)gridDim.x * vpr;
+        const uint64_t rowa = blockIdx.x + (uint64_t)k * gridDim.x, rowb = rowa + gridDim.x;
         for (uint32_t v = threadIdx.x; v < vpr; v += blockDim.x) {
             const CmVec c = cmv[v];
             union { int4 q; E e[EPV]; } oa, ob;
 #pragma unroll
             for (int j = 0; j < EPV; ++j) oa.e[j] = ra[c.m[j]];
-            dst.store(va + v, oa.q);
+            dst.store(rowa, v, vpr, oa.q);
             if (two) {
 #pragma unroll
                 for (int j = 0; j < EPV; ++j) ob.e[j] = rb[c.m[j]];
-                dst.store(vb + v, ob.q);
+                dst.store(rowb, v, vpr, ob.q);
             }
         }
         __syncthreads();                                       // every thread is done with both stages
@@ -178,7 +189,7 @@ __global__ void __launch_bounds__(256) gather_colvecs_kernel(const int4* __restr
                 if (r0 + k < nrows) x[k] = ldg_stream(src + (uint64_t)(r0 + k) * vpr + sv);
 #pragma unroll
             for (int k = 0; k < ROWS_PER_IT; ++k)
-                if (r0 + k < nrows) dst.store((uint64_t)(r0 + k) * vpr + v, x[k]);
+                if (r0 + k < nrows) dst.store(r0 + k, v, vpr, x[k]);
         }
     }
 }
@@ -466,7 +477,7 @@ extern "C" cloak_status cloak_load_mlp_heads(uint64_t key, const cloak_block_sha
     DeviceGuard g(pool->device);
     cudaStream_t s = (cudaStream_t)stream;
     pool->wrote(s);
-    st = permute_impl(key, sh, in, [&](int i) { return PoolDst{pool->base, pool->d_T, h_offsets[i], pool->log2_block}; },
+    st = permute_impl(key, sh, in, [&](int i) { return PoolDst{pool->base, pool->d_T, h_offsets[i], pool->log2_block, 0u}; },
                       pool->device, s);
     for (int i = 0; i < 7 && st == CLOAK_OK; ++i)
         if (in[i] && (h_offsets[i] + bytes[i]) % pool->block) {
@@ -475,6 +486,119 @@ extern "C" cloak_status cloak_load_mlp_heads(uint64_t key, const cloak_block_sha
             CLOAK_LAUNCH_CHECK();
         }
     return st;
+}
+
+// NEXT-2 as the survey words it: every tensor of a model -- permuted (S5), laid out (ROWMAJOR or TILE128) and scattered through
+// the block table (S4) in ONE pass over its bytes, sourced from wherever the caller holds the checkpoint (device memory, or
+// pinned host memory that the kernels read over PCIe themselves: no staging copy), issued in the order the tensors occupy the
+// arena, i.e. the keyed tensor order of cloak_arena_plan -- not the model's order (the load is "the only phase
+// in which the full set of weight transfers crosses the PCIe bus", so its order is what Tier 1 hides; :217: permutation and
+// pages are decided before any weight is transferred).
+extern "C" cloak_status cloak_load_tensors(uint64_t key, const cloak_block_shape* sh, cloak_pool* pool,
+                                           const cloak_load_item* h_items, uint32_t n, cloak_layout layout, void* stream) {
+    if (!sh || !pool || !h_items || n == 0) return fail(CLOAK_ERR_INVALID, "load_tensors: NULL argument or no items");
+    if (sh->dt != CLOAK_F32 && sh->dt != CLOAK_BF16) return fail(CLOAK_ERR_UNSUPPORTED, "load_tensors: unknown dtype");
+    if (layout != CLOAK_ROWMAJOR && layout != CLOAK_TILE128) return fail(CLOAK_ERR_UNSUPPORTED, "load_tensors: unknown layout");
+    if (pool->block < 16) return fail(CLOAK_ERR_UNSUPPORTED, "load_tensors: block_bytes must be >= 16");
+    const uint64_t e = sh->dt == CLOAK_F32 ? 4 : 2;
+    const uint32_t epv = (uint32_t)(16 / e);
+    bool mlp = false, heads = false;
+    for (uint32_t i = 0; i < n; ++i) {
+        if (h_items[i].role > CLOAK_ROLE_PLAIN) return fail(CLOAK_ERR_INVALID, "load_tensors: item %u: unknown role", i);
+        if (h_items[i].role <= CLOAK_ROLE_DOWN) mlp = true;
+        else if (h_items[i].role <= CLOAK_ROLE_O) heads = true;
+    }
+    if (mlp || heads) {
+        cloak_status st = check_shape(sh, mlp, heads, "load_tensors");
+        if (st != CLOAK_OK) return st;
+    }
+    const uint64_t qd = (uint64_t)sh->n_q * sh->head_dim, kvd = (uint64_t)sh->n_kv * sh->head_dim;
+    struct Item { const void* src; uint64_t off; uint32_t layer, role, N, K; };
+    std::vector<Item> items(n);
+    std::vector<uint32_t> layers;
+    for (uint32_t i = 0; i < n; ++i) {
+        const cloak_load_item& it = h_items[i];
+        Item x{it.src, it.arena_offset, it.layer, it.role, it.N, it.K};
+        switch (it.role) {
+            case CLOAK_ROLE_GATE: case CLOAK_ROLE_UP: x.N = sh->inter; x.K = sh->hidden; break;
+            case CLOAK_ROLE_DOWN: x.N = sh->hidden; x.K = sh->inter; break;
+            case CLOAK_ROLE_Q: x.N = (uint32_t)qd; x.K = sh->hidden; break;
+            case CLOAK_ROLE_K: case CLOAK_ROLE_V: x.N = (uint32_t)kvd; x.K = sh->hidden; break;
+            case CLOAK_ROLE_O: x.N = sh->hidden; x.K = (uint32_t)qd; break;
+            default: break;
+        }
+        if (!x.src || ((uintptr_t)x.src & 15)) return fail(CLOAK_ERR_ALIGN, "load_tensors: item %u: source NULL or not 16-byte aligned", i);
+        if (x.N == 0 || x.K == 0 || x.K % epv) return fail(CLOAK_ERR_ALIGN, "load_tensors: item %u: K must be a non-zero multiple of %u", i, epv);
+        if (layout == CLOAK_TILE128 && (x.N % 128 || x.K % 128)) return fail(CLOAK_ERR_ALIGN, "load_tensors: item %u: TILE128 needs N and K multiples of 128", i);
+        if (x.off % pool->block) return fail(CLOAK_ERR_ALIGN, "load_tensors: item %u: offset is not a block multiple", i);
+        if (x.off + (uint64_t)x.N * x.K * e > (uint64_t)pool->nb * pool->block) return fail(CLOAK_ERR_INVALID, "load_tensors: item %u exceeds the pool's arena", i);
+        items[i] = x;
+        if (x.role != CLOAK_ROLE_PLAIN && std::find(layers.begin(), layers.end(), x.layer) == layers.end()) layers.push_back(x.layer);
+    }
+    // the keyed tensor order: ascending arena offset (cloak_arena_plan placed the tensors in keygen(key, TENSOR) order)
+    std::sort(items.begin(), items.end(), [](const Item& a, const Item& b) { return a.off < b.off; });
+    for (uint32_t i = 1; i < n; ++i)
+        if (items[i].off < items[i - 1].off + (uint64_t)items[i - 1].N * items[i - 1].K * e)
+            return fail(CLOAK_ERR_INVALID, "load_tensors: items overlap in the arena");
+    DeviceGuard g(pool->device);
+    cudaStream_t s = (cudaStream_t)stream;
+    const int sms = sm_count(pool->device);
+    // the maps of every layer that occurs, once: pi | kappa | eta per layer
+    const size_t per_layer = (size_t)(mlp ? sh->inter : 0) + (heads ? sh->n_kv + sh->n_q : 0);
+    AsyncBuf sbuf(s);
+    uint32_t* scratch = nullptr;
+    if (per_layer && !layers.empty()) {
+        if (cloak_status ast = sbuf.alloc(per_layer * layers.size() * 4)) return ast;
+        scratch = static_cast<uint32_t*>(sbuf.p);
+        for (size_t li = 0; li < layers.size(); ++li) {
+            uint32_t* pi = scratch + li * per_layer;
+            uint32_t* kappa = pi + (mlp ? sh->inter : 0);
+            if (mlp)
+                if (cloak_status st = keygen_device(key, (4ull << 32) | layers[li], sh->inter, pi, nullptr, s)) return st;
+            if (heads) {
+                head_maps_kernel<<<1, 1024, 0, s>>>((uint32_t)key, (uint32_t)(key >> 32), layers[li], sh->n_q, sh->n_kv, kappa,
+                                                    kappa + sh->n_kv);
+                launched();
+                CLOAK_LAUNCH_CHECK();
+            }
+        }
+    }
+    pool->wrote(s);
+    const uint32_t vptr = layout == CLOAK_TILE128 ? (uint32_t)(128 * e / 16) : 0u;     // vectors per tile row
+    for (const Item& x : items) {
+        PoolDst dst{pool->base, pool->d_T, x.off, pool->log2_block, vptr};
+        const uint32_t* pi = nullptr;
+        const uint32_t *kappa = nullptr, *eta = nullptr;
+        if (x.role != CLOAK_ROLE_PLAIN) {
+            const size_t li = std::find(layers.begin(), layers.end(), x.layer) - layers.begin();
+            pi = scratch + li * per_layer;
+            kappa = pi + (mlp ? sh->inter : 0);
+            eta = kappa + sh->n_kv;
+        }
+        const uint64_t row_bytes = (uint64_t)x.K * e;
+        const uint32_t d = sh->head_dim;
+        cloak_status st = CLOAK_OK;
+        switch (x.role) {
+            case CLOAK_ROLE_GATE: case CLOAK_ROLE_UP: st = rows(x.src, dst, pi, 1, x.N, row_bytes, sms, s); break;
+            case CLOAK_ROLE_Q: st = rows(x.src, dst, eta, d, x.N, row_bytes, sms, s); break;
+            case CLOAK_ROLE_K: case CLOAK_ROLE_V: st = rows(x.src, dst, kappa, d, x.N, row_bytes, sms, s); break;
+            case CLOAK_ROLE_DOWN:
+                st = e == 4 ? cols<uint32_t>(x.src, dst, pi, 1, x.N, x.K, sms, s) : cols<uint16_t>(x.src, dst, pi, 1, x.N, x.K, sms, s);
+                break;
+            case CLOAK_ROLE_O:
+                st = e == 4 ? cols<uint32_t>(x.src, dst, eta, d, x.N, x.K, sms, s) : cols<uint16_t>(x.src, dst, eta, d, x.N, x.K, sms, s);
+                break;
+            default: st = rows(x.src, dst, nullptr, 1, x.N, row_bytes, sms, s); break;
+        }
+        if (st != CLOAK_OK) return st;
+        const uint64_t end = x.off + (uint64_t)x.N * x.K * e;
+        if (end % pool->block) {
+            zero_block_tail_kernel<<<1, 256, 0, s>>>(pool->base, pool->d_T, end, pool->log2_block);
+            launched();
+            CLOAK_LAUNCH_CHECK();
+        }
+    }
+    return CLOAK_OK;
 }
 
 extern "C" cloak_status cloak_permute_experts(uint64_t key, const cloak_moe_shape* sh, const void* d_router,

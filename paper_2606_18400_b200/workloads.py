@@ -1,6 +1,6 @@
 """Measurement drivers for BASELINE.json configs[2..4]; configs[1] is bench.py's own step.
 
-    python -m paper_2606_18400_b200.workloads cfg2|cfg3|cfg4|moe [--reps R] [--out file.json]
+    python -m paper_2606_18400_b200.workloads cfg2|cfg3|cfg4|moe|rekey [--reps R] [--out file.json]
     python bench.py --workload cfg2|cfg3|cfg4            (same thing)
 
 Each prints ONE JSON line.  Everything on the timed path is a C-ABI call of libcloak.so (through the ctypes
@@ -777,7 +777,132 @@ def bench_cfg4(sampler, min_s=0.5):
     return out
 
 
-RUNNERS = {"cfg2": run_cfg2, "cfg3": run_cfg3, "cfg4": run_cfg4, "moe": run_moe}
+# ------------------------------------------------------------------------------------------ NEXT-1: page re-key under live decode
+def run_rekey(args):
+    """The cfg2 decode chain (225 GEMVs, batch 1, CUDA-graph replay) run continuously while the pool's PHYSICAL PAGE MAP is
+    re-randomised (cloak_rekey_pages_begin / _step): per-step latency (CUDA event to CUDA event) p50 / p99 / max against the
+    cadence of the re-key -- one full re-randomisation of the 7 658 pages every 1 000 / 1 500 decode steps
+    and at one page per step.  The serving loop keeps one step in flight: launch step i, then do the re-key's driver calls
+    for it while the GPU runs, then wait for step i-1."""
+    torch, C, synth_cuda, gen = _imports()
+    c = gen.CONFIGS[2]
+    layers = int(args.layers or c["layers"])
+    peak, peak_kind = hbm_peak()
+    tensors = [t for t in gen.model_tensors(2) if "." not in t[0] or int(t[0][1:].split(".")[0]) < layers]
+    sizes = [2 * n * k for _, (n, k) in tensors]
+    offs, total = C.cloak_arena_plan(c["key"], sizes, c["block"])
+    off = {nm: o for (nm, _), o in zip(tensors, offs)}
+    pc = C.cloak_pool_create(0, total, c["block"], c["page"], c["key"])
+    npages = C.cloak_pool_info(pc)["npages"]
+    out = {"workload": "rekey: cfg2 decode chain (%d layers + lm_head, batch 1) under periodic page-map re-randomisation" % layers,
+           "npages": npages, "arena_bytes": total, "hbm_peak_gbs": peak, "cadences": {}}
+    try:
+        lshapes = gen.layer_shapes(c["hidden"], c["inter"], c["n_q"], c["n_kv"], c["head_dim"])
+        raw = {nm: torch.empty(shp, dtype=torch.bfloat16, device="cuda") for nm, shp in lshapes}
+        tid = {nm: i for i, (nm, _) in enumerate(gen.model_tensors(2))}
+        for l in range(layers):
+            for nm, _ in lshapes:
+                synth_cuda.fill(raw[nm], c["seed"], tid[f"l{l}.{nm}"])
+            sh = C.cloak_block_shape(c["hidden"], c["inter"], c["n_q"], c["n_kv"], c["head_dim"], C.CLOAK_BF16, l)
+            C.cloak_load_mlp_heads(c["key"], sh, pc, {nm: off[f"l{l}.{nm}"] for nm, _ in lshapes}, **raw)
+        for nm in ("embed", "lm_head"):
+            t = synth_cuda.fill(torch.empty(dict(tensors)[nm], dtype=torch.bfloat16, device="cuda"), c["seed"], tid[nm])
+            C.cloak_shuffle(pc, t, off[nm], t.numel() * 2)
+            del t
+        H, I, Q = c["hidden"], c["inter"], c["n_q"] * c["head_dim"]
+        xh = synth_cuda.fill(torch.empty(1, H, dtype=torch.bfloat16, device="cuda"), c["seed"] + 100, 0, kind=gen.KIND_NORMAL)
+        xa = synth_cuda.fill(torch.empty(1, Q, dtype=torch.bfloat16, device="cuda"), c["seed"] + 100, 1, kind=gen.KIND_NORMAL)
+        T = {nm: C.cloak_tensor(off[nm], shp[0], shp[1], C.CLOAK_BF16, C.CLOAK_ROWMAJOR) for nm, shp in tensors}
+        y = {nm: torch.zeros(1, shp[0], dtype=torch.bfloat16, device="cuda") for nm, shp in tensors if nm != "embed"}
+        act = torch.empty(1, I, dtype=torch.bfloat16, device="cuda")
+        ops = []
+        for l in range(layers):
+            p = f"l{l}."
+            ops += [(T[p + nm], xh, y[p + nm], 0) for nm in ("q", "k", "v")]
+            ops += [(T[p + "o"], xa, y[p + "o"], 0), (T[p + "gate"], xh, y[p + "gate"], 0),
+                    (T[p + "up"], xh, y[p + "up"], 0, y[p + "gate"], act), (T[p + "down"], act, y[p + "down"], 1)]
+        ops.append((T["lm_head"], xh, y["lm_head"], 0))
+        ops = C.cloak_gemv_ops(ops)
+        g = _graph(torch, lambda: C.cloak_gemv_chain(pc, ops, 1))
+        g.replay()
+        torch.cuda.synchronize()
+        ref = {nm: t.clone() for nm, t in y.items()}
+        stream = torch.cuda.current_stream()
+
+        def serve(nsteps, moves_per_step, spares, new_key):
+            """nsteps decode steps (or until the re-key is complete when moves_per_step > 0); per-step GPU latency in ms."""
+            if moves_per_step:
+                C.cloak_rekey_pages_begin(pc, new_key, spares)
+            ev = [torch.cuda.Event(enable_timing=True) for _ in range(nsteps + 1)]
+            host = []
+            ev[0].record(stream)
+            done_at, i = None, 0
+            t_wall = time.perf_counter()
+            while i < nsteps:
+                g.replay()
+                ev[i + 1].record(stream)
+                if moves_per_step and done_at is None:
+                    t0 = time.perf_counter()
+                    if C.cloak_rekey_pages_step(pc, moves_per_step) == 0:
+                        done_at = i + 1
+                    host.append((time.perf_counter() - t0) * 1e3)
+                if i >= 1:
+                    ev[i].synchronize()                       # the loop keeps one step in flight
+                i += 1
+                if moves_per_step and done_at is not None and i >= done_at + 50:
+                    break
+            torch.cuda.synchronize()
+            wall = time.perf_counter() - t_wall
+            lat = np.array([ev[k].elapsed_time(ev[k + 1]) for k in range(i)])
+            same = bool(all(torch.equal(y[nm], ref[nm]) for nm in y))
+            r = {"steps": int(i), "p50_ms": float(np.percentile(lat, 50)), "p99_ms": float(np.percentile(lat, 99)),
+                 "max_ms": float(lat.max()), "mean_ms": float(lat.mean()), "tokens_per_s": i / wall,
+                 "outputs_identical_to_before": same,
+                 "latency_histogram_ms": {f"<={b}": int(np.count_nonzero(lat <= b)) for b in (3, 4, 6, 10, 20, 50, 100, 1000, 10000)},
+                 "slowest_steps": [(int(k), round(float(lat[k]), 2)) for k in np.argsort(lat)[::-1][:12]]}
+            if moves_per_step:
+                r.update({"moves_per_step": moves_per_step, "spare_pages": spares, "rekey_complete_after_steps": done_at,
+                          "host_ms_per_step_call_median": float(np.median(host)) if host else None,
+                          "host_ms_per_page": float(np.median(host)) / moves_per_step if host else None})
+            return r
+
+        sampler = ClockSampler(0)
+        sampler.wait_first_sample()
+        w0 = time.time()
+        out["baseline_no_rekey"] = serve(2000, 0, 0, 0)
+        keys = [0x5678, 0x9abc, 0xdef0, 0x1357]
+        for (label, cadence), key in zip((("every_1000_steps", 1000), ("every_1500_steps", 1500), ("one_page_per_step", npages),
+                                          ("stop_the_world", 0)), keys):
+            if cadence:
+                k = int(np.ceil(npages / cadence))
+                # a move retires two steps after it was issued (one step in flight + its own), so 3 k spare pages keep k cycles ready
+                r = serve(4 * cadence + 400, k, max(1, min(3 * k, 64)), key)
+                base = out["baseline_no_rekey"]
+                r["p50_overhead_pct"] = (r["p50_ms"] - base["p50_ms"]) / base["p50_ms"] * 100
+                r["mean_overhead_pct"] = (r["mean_ms"] - base["mean_ms"]) / base["mean_ms"] * 100
+            else:
+                torch.cuda.synchronize()
+                t0 = time.perf_counter()
+                C.cloak_rekey_pages_begin(pc, key, 16)
+                C.cloak_rekey_pages_finish(pc)
+                ms = (time.perf_counter() - t0) * 1e3
+                g.replay()
+                torch.cuda.synchronize()
+                r = {"ms": ms, "ms_per_page": ms / npages, "spare_pages": 16,
+                     "outputs_identical_to_before": bool(all(torch.equal(y[nm], ref[nm]) for nm in y)),
+                     "amortised_pct_of_decode": {f"every_{n}_steps": ms / (n * out["baseline_no_rekey"]["p50_ms"]) * 100 for n in (1000, 1500)}}
+            if pc is not None and r.get("rekey_complete_after_steps") is None and cadence:
+                C.cloak_rekey_pages_finish(pc)               # (did not complete inside the step budget: finish it off)
+            out["cadences"][label] = r
+        out["clocks"] = sampler.stop(w0, time.time())
+    finally:
+        torch.cuda.synchronize()
+        C.cloak_pool_destroy(pc)
+    out["paper_context"] = "PAPER.md:207 / :271 / :283 (L40S, vLLM): re-shuffle every 1000-1500 iterations, < 2 % end-to-end; 1.5 s per shuffle (:265)"
+    return out
+
+
+RUNNERS = {"cfg2": run_cfg2, "cfg3": run_cfg3, "cfg4": run_cfg4, "moe": run_moe, "rekey": run_rekey}
 
 
 def main(argv=None):
