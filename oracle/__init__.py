@@ -32,7 +32,7 @@ from .keygen import (keygen, sort_pairs, STREAM_BLOCK, STREAM_PAGE, STREAM_TENSO
                      stream_mlp, stream_kvhead, stream_qgroup)
 from .pool import (PoolGeometry, pool_geometry, PoolTables, pool_tables, shuffle_va,
                    shuffle_into, dump_view, unshuffle, relayout, rekey_pages, arena_plan,
-                   adjacent_fraction)
+                   adjacent_fraction, run_lengths, run_stats)
 from .permute import (mlp_perm, head_maps, permute_mlp, permute_heads, expand_head_rows)
 from .moe import (stream_expert, stream_expert_mlp, expert_perm, expert_mlp_perm, permute_experts,
                   topk_experts, moe_f64)

@@ -167,3 +167,33 @@ def adjacent_fraction(T):
     if T.size < 2:
         return 0.0
     return float(np.count_nonzero(T[1:] - T[:-1] == 1)) / (T.size - 1)
+
+
+def run_lengths(T):
+    """NEXT-3: lengths of the maximal runs i, i+1, ... of logically consecutive items with T[i+1] == T[i] + 1, in order.
+    (the paper's contiguity metric counts address ranges that stayed physically contiguous.)"""
+    T = [int(x) for x in np.asarray(T).ravel()]
+    out, cur = [], 0
+    for i in range(len(T)):
+        if i > 0 and T[i] == T[i - 1] + 1:
+            cur += 1
+        else:
+            if cur:
+                out.append(cur)
+            cur = 1
+    if cur:
+        out.append(cur)
+    return out
+
+
+def run_stats(T):
+    """What cloak_pool_layout_report returns for one sequence: items, runs, longest run, items in runs of >= 2, the
+    adjacent-pair fraction, and the histogram by power of two (bucket k: 2^k <= L < 2^(k+1))."""
+    L = run_lengths(T)
+    n = sum(L)
+    hist = {}
+    for x in L:
+        k = x.bit_length() - 1
+        hist[k] = hist.get(k, 0) + 1
+    return dict(items=n, runs=len(L), longest_run=max(L) if L else 0, items_in_runs_of_2_or_more=sum(x for x in L if x >= 2),
+                adjacent_fraction=(n - len(L)) / (n - 1) if n > 1 else 0.0, histogram=hist)

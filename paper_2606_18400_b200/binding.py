@@ -23,7 +23,7 @@ STATUS_NAMES = {0: "CLOAK_OK", -1: "CLOAK_ERR_INVALID", -2: "CLOAK_ERR_ALIGN", -
 
 # every symbol include/cloak.h declares
 SYMBOLS = ["cloak_last_error", "cloak_version", "cloak_runtime_info", "cloak_launch_count", "cloak_keygen", "cloak_pool_create", "cloak_pool_destroy",
-           "cloak_pool_info", "cloak_pool_tables", "cloak_pool_dump", "cloak_pool_map_ms", "cloak_pool_adjacency", "cloak_shuffle",
+           "cloak_pool_info", "cloak_pool_tables", "cloak_pool_dump", "cloak_pool_map_ms", "cloak_pool_adjacency", "cloak_pool_layout_report", "cloak_shuffle",
            "cloak_unshuffle", "cloak_shuffle_many", "cloak_unshuffle_many", "cloak_relayout", "cloak_rekey_inplace", "cloak_rekey_pages_begin", "cloak_rekey_pages_step", "cloak_rekey_pages_finish", "cloak_shuffle_host", "cloak_unshuffle_host",
            "cloak_set_copy_engine", "cloak_set_copy_cache_hint", "cloak_arena_plan", "cloak_permute_mlp_heads", "cloak_permute_experts", "cloak_load_mlp_heads", "cloak_load_tensors", "cloak_to_tile128",
            "cloak_gemv", "cloak_gemv_chain", "cloak_gemm", "cloak_gemm_chain", "cloak_gemv_chain_scratch_bytes",
@@ -50,6 +50,15 @@ class cloak_load_item(Structure):
 
 
 CLOAK_ROLE = {"gate": 0, "up": 1, "down": 2, "q": 3, "k": 4, "v": 5, "o": 6, "plain": 7}
+
+
+class cloak_run_stats(Structure):
+    _fields_ = [("items", c_uint64), ("runs", c_uint64), ("longest_run", c_uint64), ("items_in_runs_of_2_or_more", c_uint64),
+                ("adjacent_fraction", c_double), ("histogram", c_uint64 * 32)]
+
+
+class cloak_layout_report(Structure):
+    _fields_ = [("va_blocks", cloak_run_stats), ("physical_blocks", cloak_run_stats), ("pages", cloak_run_stats)]
 
 
 class cloak_tensor(Structure):
@@ -84,6 +93,7 @@ lib.cloak_pool_dump.argtypes = [_P, _P, _P]
 lib.cloak_pool_map_ms.argtypes = [_P, POINTER(c_double)]
 lib.cloak_pool_adjacency.argtypes = [_P, POINTER(c_double), POINTER(c_double), POINTER(c_double), _P]
 lib.cloak_pool_reserve_workspace.argtypes = [_P, c_uint64]
+lib.cloak_pool_layout_report.argtypes = [_P, POINTER(cloak_layout_report), _P]
 lib.cloak_shuffle.argtypes = [_P, _P, c_uint64, c_uint64, _P]
 lib.cloak_unshuffle.argtypes = [_P, _P, c_uint64, c_uint64, _P]
 lib.cloak_shuffle_many.argtypes = [_P, c_uint32, POINTER(c_void_p), POINTER(c_uint64), POINTER(c_uint64), _P]
@@ -211,6 +221,18 @@ def cloak_pool_adjacency(pool, stream=None):
     va, ph, pg = c_double(), c_double(), c_double()
     _check(lib.cloak_pool_adjacency(pool, byref(va), byref(ph), byref(pg), _stream(stream)))
     return dict(va_blocks=va.value, physical_blocks=ph.value, pages=pg.value)
+
+
+def cloak_pool_layout_report(pool, stream=None):
+    """{view: {items, runs, longest_run, items_in_runs_of_2_or_more, adjacent_fraction, histogram: {"2^k": count}}}"""
+    rep = cloak_layout_report()
+    _check(lib.cloak_pool_layout_report(pool, byref(rep), _stream(stream)))
+    out = {}
+    for name in ("va_blocks", "physical_blocks", "pages"):
+        r = getattr(rep, name)
+        out[name] = dict(items=r.items, runs=r.runs, longest_run=r.longest_run, items_in_runs_of_2_or_more=r.items_in_runs_of_2_or_more,
+                         adjacent_fraction=r.adjacent_fraction, histogram={f"2^{k}": r.histogram[k] for k in range(32) if r.histogram[k]})
+    return out
 
 
 def cloak_pool_reserve_workspace(pool, nbytes):

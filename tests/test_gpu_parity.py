@@ -139,6 +139,40 @@ def test_pool_adjacency_matches_the_oracle(payload, block, page):
         assert C.cloak_pool_adjacency(pi.h) == dict(va_blocks=1.0, physical_blocks=1.0, pages=1.0)
 
 
+@pytest.mark.parametrize("payload,block,page,flags", [(3 << 20, 4096, 65536, 0), (300 << 20, 65536, 2 << 20, 0), (1 << 20, 256, 1024, 0),
+                                                      ((37 << 20) + 4096, 4096, 2 << 20, 0), (40 << 20, 65536, 2 << 20, 1)])
+def test_pool_layout_report_matches_the_oracle(payload, block, page, flags):
+    """NEXT-3: runs of logically consecutive blocks / pages that stayed consecutive (VA view, physical view, page map) --
+    counts, longest run, histogram by power of two -- against oracle.run_stats on the oracle's own tables; an identity pool
+    (flags = 1) is one run of everything.  After a page re-key the report follows the new page map."""
+    key = 0x1234
+    g = O.pool_geometry(payload, block, page)
+    t = O.pool_tables(key, g)
+
+    def check(rep, blockinv, pageinv):
+        phys = [int(pageinv[int(s) // g.bpp]) * g.bpp + int(s) % g.bpp for s in blockinv[:g.nb]]
+        for name, seq in (("va_blocks", blockinv[:g.nb]), ("physical_blocks", phys), ("pages", pageinv)):
+            ref = O.run_stats(seq)
+            got = rep[name]
+            assert {k: got[k] for k in ("items", "runs", "longest_run", "items_in_runs_of_2_or_more")} == \
+                   {k: ref[k] for k in ("items", "runs", "longest_run", "items_in_runs_of_2_or_more")}, name
+            assert abs(got["adjacent_fraction"] - ref["adjacent_fraction"]) < 1e-12
+            assert got["histogram"] == {f"2^{k}": c for k, c in ref["histogram"].items()}, name
+    with Pool(payload, block, page, key, flags) as p:
+        rep = C.cloak_pool_layout_report(p.h)
+        if flags & C.CLOAK_POOL_IDENTITY:
+            check(rep, np.arange(g.nslots), np.arange(g.npages))
+            assert rep["physical_blocks"]["runs"] == 1 and rep["pages"]["longest_run"] == g.npages
+        else:
+            check(rep, t.blockinv, t.pageinv)
+            adj = C.cloak_pool_adjacency(p.h)
+            assert abs(adj["physical_blocks"] - rep["physical_blocks"]["adjacent_fraction"]) < 1e-12
+            if p.info["is_vmm"]:
+                C.cloak_rekey_pages_begin(p.h, 0x5678, 2)
+                C.cloak_rekey_pages_finish(p.h)
+                check(C.cloak_pool_layout_report(p.h), t.blockinv, O.pool_tables(0x5678, g).pageinv)
+
+
 @pytest.mark.parametrize("block,page,n", [(4096, 65536, 5), (65536, 2 << 20, 150), (256, 1024, 4)])
 def test_shuffle_many_equals_one_call_per_range(block, page, n):
     """cloak_shuffle_many / cloak_unshuffle_many: n tensors of mixed sizes (ragged tails, > 128 ranges -> two launches) in

@@ -440,6 +440,28 @@ def test_adjacent_fraction_brute_force_counts_ascending_neighbours_only():
     assert O.adjacent_fraction(np.array([0, 0xFFFFFFFF, 0], dtype=np.uint32)) == 0.0
 
 
+def test_run_lengths_hand_example_and_closed_forms():
+    """NEXT-3 oracle twin of cloak_pool_layout_report.  Hand example: T = [5,6,7 | 2 | 9,10 | 0] has runs of 3, 1, 2, 1 (written
+    out by eye): 4 runs, longest 3, 5 items in runs of two or more, 3 of 6 neighbour pairs kept, histogram 2^0: two runs,
+    2^1: two runs.  Closed forms: the identity is one run of everything, a descending table is all singletons, and the pair
+    fraction from the runs equals adjacent_fraction (two routes) on a real keyed table."""
+    T = [5, 6, 7, 2, 9, 10, 0]
+    assert O.run_lengths(T) == [3, 1, 2, 1]
+    st = O.run_stats(T)
+    assert (st["items"], st["runs"], st["longest_run"], st["items_in_runs_of_2_or_more"]) == (7, 4, 3, 5)
+    assert st["adjacent_fraction"] == 3 / 6 == O.adjacent_fraction(T) and st["histogram"] == {0: 2, 1: 2}
+    ident = O.run_stats(np.arange(1000))
+    assert (ident["runs"], ident["longest_run"], ident["adjacent_fraction"], ident["histogram"]) == (1, 1000, 1.0, {9: 1})
+    desc = O.run_stats(np.arange(1000)[::-1])
+    assert (desc["runs"], desc["longest_run"], desc["items_in_runs_of_2_or_more"], desc["histogram"]) == (1000, 1, 0, {0: 1000})
+    assert O.run_lengths([7]) == [1] and O.run_lengths([]) == []
+    g = O.pool_geometry(1 << 20, 4096, 65536)
+    t = O.pool_tables(0x1234, g)
+    st = O.run_stats(t.T_emulated)
+    assert st["adjacent_fraction"] == O.adjacent_fraction(t.T_emulated) and sum(O.run_lengths(t.T_emulated)) == g.nb
+    assert sum(c << k for k, c in st["histogram"].items()) <= g.nb          # bucket lower bounds never exceed the item count
+
+
 def test_adjacent_fraction_is_about_one_over_n():
     g = O.pool_geometry(1 << 20, 4096, 65536)
     t = O.pool_tables(0x1234, g)
