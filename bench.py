@@ -479,6 +479,10 @@ def run_cloak(args):
 
     map_ms = C.cloak_pool_map_ms(pool_a)
     adjacency = C.cloak_pool_adjacency(pool_a)          # layout quality (G8): neighbours that stayed neighbours
+    layout_report = {"cloaked": C.cloak_pool_layout_report(pool_a), "identity_pool": C.cloak_pool_layout_report(pool_n),
+                     "paper_context": "PAPER.md:226-227 (L40S, vLLM): VA ranges backed by contiguous physical pages, default -> CloakLM: "
+                                      "91.41 % -> 2.38 % (Llama 3.1 8B), 95.57 % -> 1.57 % (Qwen3 14B); unit undefined (G12): "
+                                      "`pages.adjacent_fraction` is the closest analogue here"}
     torch.cuda.synchronize()
     for p in (pool_a, pool_b, pool_n, pool_p):
         C.cloak_pool_destroy(p)
@@ -523,7 +527,7 @@ def run_cloak(args):
                          "cloaked_vs_native_overhead_pct.  cloaked_vs_cublas_pct puts it next to torch.matmul (cuBLAS) on the plain "
                          "permuted tensors with plain pointers, 7 calls per batch in one CUDA graph: negative = faster than cuBLAS.",
         "hbm_peak_gbs": peak, "hbm_peak_kind": peak_kind, "hbm_nominal_gbs": 8000.0,
-        "sm_weights": sm_weights_summary(C), "pool_map_ms": map_ms, "layout_adjacency": adjacency, "pool_create_s": pool_create_s, "roundtrip_bit_exact": bool(ok),
+        "sm_weights": sm_weights_summary(C), "pool_map_ms": map_ms, "layout_adjacency": adjacency, "layout_report": layout_report, "pool_create_s": pool_create_s, "roundtrip_bit_exact": bool(ok),
         "roofline": {"bound": "hbm", "kernel": "gemv_chain_kernel", "achieved": achieved, "peak": peak, "unit": "GB/s",
                      "frac": achieved / peak, "traffic": ncu_traffic()[0], "traffic_source": ncu_traffic()[1],
                      "launches_per_step": gemv_launches,

@@ -630,6 +630,7 @@ def bench_cfg2(sampler, min_s=1.0):
     launches0 = C.cloak_launch_count()
     out = {"workload": "cfg2: 32-layer LLaMA-8B-shaped model, bf16, 226 tensors, 64 KiB blocks, 2 MiB VMM pages",
            "payload_bytes": payload, "npages": C.cloak_pool_info(pc)["npages"],
+           "layout_report": {"cloaked": C.cloak_pool_layout_report(pc), "identity_pool": C.cloak_pool_layout_report(pn)},
            "pool_map_ms": {"cloaked": C.cloak_pool_map_ms(pc), "identity": C.cloak_pool_map_ms(pn)}}
     try:
         keep = {nm: torch.empty(shp, dtype=torch.bfloat16, device="cuda") for nm, shp in tensors}
