@@ -232,6 +232,10 @@ cloak_status cloak_permute_mlp_heads(uint64_t key, const cloak_block_shape* shap
                                      void* d_gate_o, void* d_up_o, void* d_down_o,
                                      void* d_q_o, void* d_k_o, void* d_v_o, void* d_o_o, void* stream);
 
+/* Column gather of 2-byte elements (down's columns): 0 = automatic (two source rows interleaved into 32-bit pairs in shared
+ * memory, one LDS per output element PAIR), 1 = the element-by-element gather.  For A/B measurement; process-wide. */
+cloak_status cloak_set_gather_engine(int engine);
+
 /* ---- S5 for mixture-of-experts layers (the paper evaluates Qwen3-MoE).
  * Shapes (row-major, contiguous): router [n_experts, hidden]; gate, up [n_experts, inter, hidden]; down [n_experts, hidden, inter].
  *   (eps, _)  = keygen(key, (7<<32)|layer, n_experts):  new expert e' is old expert eps[e'];  router'[e',:] = router[eps[e'],:]

@@ -171,6 +171,76 @@ __global__ void __launch_bounds__(512) gather_cols_kernel(const E* __restrict__ 
     }
 }
 
+// The same for 2-byte elements, organised around what bounds it: shared-memory WAVEFRONTS.  A 2-byte gather from a random
+// column is one LDS per element whose 32 lanes collide on the banks (~3.5 wavefronts per instruction): the kernel above spends
+// ~30 wavefronts per 512 output bytes and runs at 4.4 TB/s with the DRAM pipe 41 % busy (profiles/r1_ncu_full_gather.md).  Here
+// two source rows are first INTERLEAVED element by element into one row of 32-bit pairs (a conflict-free pass of 16-byte loads,
+// two PRMTs per word and 16-byte stores), so that one 32-bit LDS at a source column returns that column of BOTH rows: half the
+// gather instructions and half the colliding wavefronts per output byte.  Ring of TMA-fetched source rows as above.
+template <typename M, typename Dst>
+__global__ void __launch_bounds__(1024) gather_cols_pair_kernel(const uint16_t* __restrict__ src, Dst dst,
+                                                               const uint32_t* __restrict__ map, uint32_t seg,
+                                                               uint32_t nrows, uint32_t ncols, uint32_t ns) {
+    extern __shared__ __align__(128) unsigned char sm[];
+    __shared__ __align__(8) uint64_t full[8];
+    M* colmap = reinterpret_cast<M*>(sm);
+    const uint32_t row_bytes = ncols * 2;
+    unsigned char* pairs = sm + (((size_t)ncols * sizeof(M) + 127) & ~(size_t)127);      // [ncols] x (row a, row b)
+    unsigned char* ring = pairs + 2 * (size_t)row_bytes;
+    for (uint32_t c = threadIdx.x; c < ncols; c += blockDim.x) colmap[c] = (M)(__ldg(map + c / seg) * seg + c % seg);
+    if (threadIdx.x == 0) {
+        for (uint32_t i = 0; i < ns; ++i) mbar_init(smem_u32(&full[i]), 1);
+        fence_barrier_init();
+    }
+    __syncthreads();
+    const uint32_t mine = blockIdx.x < nrows ? (nrows - blockIdx.x + gridDim.x - 1) / gridDim.x : 0;
+    auto issue = [&](uint32_t k) {
+        const uint32_t st = k % ns, bar = smem_u32(&full[st]);
+        mbar_expect_tx(bar, row_bytes);
+        bulk_g2s(smem_u32(ring + (size_t)st * row_bytes), src + (uint64_t)(blockIdx.x + k * gridDim.x) * ncols, row_bytes, bar);
+    };
+    if (threadIdx.x == 0)
+        for (uint32_t k = 0; k < ns && k < mine; ++k) issue(k);
+    struct alignas(sizeof(M) * 8) CmVec { M m[8]; };
+    const CmVec* cmv = reinterpret_cast<const CmVec*>(colmap);
+    const uint32_t vpr = ncols / 8;
+    const uint32_t* pw = reinterpret_cast<const uint32_t*>(pairs);
+    for (uint32_t k = 0; k < mine; k += 2) {
+        const bool two = k + 1 < mine;
+        const uint32_t sa = k % ns, sb = (k + 1) % ns;
+        mbar_wait(smem_u32(&full[sa]), (k / ns) & 1);
+        if (two) mbar_wait(smem_u32(&full[sb]), ((k + 1) / ns) & 1);
+        const int4* ra = reinterpret_cast<const int4*>(ring + (size_t)sa * row_bytes);
+        const int4* rb = reinterpret_cast<const int4*>(ring + (size_t)(two ? sb : sa) * row_bytes);
+        int4* pv = reinterpret_cast<int4*>(pairs);
+        for (uint32_t v = threadIdx.x; v < vpr; v += blockDim.x) {          // interleave: pair word c = (a[c], b[c])
+            const int4 a = ra[v], b = rb[v];
+            pv[2 * v] = make_int4(__byte_perm(a.x, b.x, 0x5410), __byte_perm(a.x, b.x, 0x7632), __byte_perm(a.y, b.y, 0x5410),
+                                  __byte_perm(a.y, b.y, 0x7632));
+            pv[2 * v + 1] = make_int4(__byte_perm(a.z, b.z, 0x5410), __byte_perm(a.z, b.z, 0x7632), __byte_perm(a.w, b.w, 0x5410),
+                                      __byte_perm(a.w, b.w, 0x7632));
+        }
+        __syncthreads();                                       // pairs complete; both ring stages are free again
+        if (threadIdx.x == 0) {
+            if (k + ns < mine) issue(k + ns);
+            if (two && k + 1 + ns < mine) issue(k + 1 + ns);
+        }
+        const uint64_t rowa = blockIdx.x + (uint64_t)k * gridDim.x, rowb = rowa + gridDim.x;
+        for (uint32_t v = threadIdx.x; v < vpr; v += blockDim.x) {
+            const CmVec c = cmv[v];
+            uint32_t p[8];
+#pragma unroll
+            for (int j = 0; j < 8; ++j) p[j] = pw[c.m[j]];
+            dst.store(rowa, v, vpr, make_int4(__byte_perm(p[0], p[1], 0x5410), __byte_perm(p[2], p[3], 0x5410),
+                                              __byte_perm(p[4], p[5], 0x5410), __byte_perm(p[6], p[7], 0x5410)));
+            if (two)
+                dst.store(rowb, v, vpr, make_int4(__byte_perm(p[0], p[1], 0x7632), __byte_perm(p[2], p[3], 0x7632),
+                                                  __byte_perm(p[4], p[5], 0x7632), __byte_perm(p[6], p[7], 0x7632)));
+        }
+        __syncthreads();                                       // the pair buffer is rewritten by the next pass
+    }
+}
+
 // Column groups that are whole 16-byte vectors (seg % (16 / sizeof(E)) == 0, e.g. heads of 128 columns): the gather
 // is a vector-level index remap, no staging needed.  vmap[v'] = source vector of destination vector v'.
 template <typename Dst>
@@ -275,6 +345,25 @@ static cloak_status cols_ring(const void* src, Dst dst, const uint32_t* map, uin
     return CLOAK_OK;
 }
 
+static std::atomic<bool> g_cols_pairs{true};     // A/B switch (cloak_set_gather_engine)
+
+template <typename M, typename Dst>
+static cloak_status cols_pair(const void* src, Dst dst, const uint32_t* map, uint32_t seg, uint32_t nrows, uint32_t ncols,
+                              size_t smem, uint32_t ns, int sms, cudaStream_t s) {
+    static std::atomic<uint64_t> opted{0};
+    auto* kernel = gather_cols_pair_kernel<M, Dst>;
+    int dev = 0;
+    CLOAK_CUDA(cudaGetDevice(&dev));
+    if (cloak_status ost = smem_opt_in(kernel, 200 * 1024, dev, opted)) return ost;
+    const uint32_t rows_per_cta = 2;
+    uint32_t ctas = (nrows + rows_per_cta - 1) / rows_per_cta;
+    if (ctas > (uint32_t)sms) ctas = (uint32_t)sms;
+    gather_cols_pair_kernel<M, Dst><<<ctas, 1024, smem, s>>>((const uint16_t*)src, dst, map, seg, nrows, ncols, ns);
+    launched();
+    CLOAK_LAUNCH_CHECK();
+    return CLOAK_OK;
+}
+
 // Only a caller-owned tensor can take the element-by-element fallback.
 template <typename E>
 static cloak_status cols_fallback(const void* src, PlainDst dst, const uint32_t* map, uint32_t seg, uint32_t nrows,
@@ -306,6 +395,14 @@ static cloak_status cols(const void* src, Dst dst, const uint32_t* map, uint32_t
     const size_t msz = ncols <= 65536 ? 2 : 4;
     const size_t cm = ((size_t)ncols * msz + 127) & ~(size_t)127;
     const size_t budget = 200 * 1024;
+    if (sizeof(E) == 2 && g_cols_pairs.load(std::memory_order_relaxed) && cm + 4 * row_bytes <= budget) {
+        // 2-byte elements: the pair-interleaved gather (map + pair buffer of two rows + a ring of at least two source rows)
+        uint32_t ns = (uint32_t)((budget - cm - 2 * row_bytes) / row_bytes);
+        if (ns > 6) ns = 6;
+        const size_t smem = cm + 2 * row_bytes + (size_t)ns * row_bytes;
+        return msz == 2 ? cols_pair<uint16_t, Dst>(src, dst, map, seg, nrows, ncols, smem, ns, sms, s)
+                        : cols_pair<uint32_t, Dst>(src, dst, map, seg, nrows, ncols, smem, ns, sms, s);
+    }
     uint32_t ns = cm < budget ? (uint32_t)((budget - cm) / row_bytes) : 0;
     if (ns > 6) ns = 6;
     if (ns >= 2) {
@@ -419,6 +516,12 @@ __global__ void zero_block_tail_kernel(char* pool, const uint32_t* T, uint64_t e
 }
 
 }  // namespace cloak
+
+extern "C" cloak_status cloak_set_gather_engine(int engine) {
+    if (engine < 0 || engine > 1) return fail(CLOAK_ERR_INVALID, "set_gather_engine: 0 (pair-interleaved column gather) or 1 (element gather)");
+    g_cols_pairs.store(engine == 0);
+    return CLOAK_OK;
+}
 
 extern "C" cloak_status cloak_permute_mlp_heads(uint64_t key, const cloak_block_shape* sh, const void* d_gate,
                                                 const void* d_up, const void* d_down, const void* d_q, const void* d_k,
