@@ -107,6 +107,8 @@ cloak_status cloak_pool_dump(const cloak_pool* pool, void* d_out, void* stream);
 
 /* Milliseconds the host-side mapper (reserve/create/map/set-access) took in cloak_pool_create. */
 cloak_status cloak_pool_map_ms(const cloak_pool* pool, double* ms);
+/* ... and its three phases: cuMemCreate of every page, cuMemMap in keyed order, cuMemSetAccess (0 for emulated pools). */
+cloak_status cloak_pool_map_phases(const cloak_pool* pool, double* create_ms, double* map_ms, double* access_ms);
 
 /* Layout-quality report (the paper's only security-side metric that needs no attacker is a
  * contiguity percentage).  Fractions of logical neighbours that are still neighbours:

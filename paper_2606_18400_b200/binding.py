@@ -23,7 +23,7 @@ STATUS_NAMES = {0: "CLOAK_OK", -1: "CLOAK_ERR_INVALID", -2: "CLOAK_ERR_ALIGN", -
 
 # every symbol include/cloak.h declares
 SYMBOLS = ["cloak_last_error", "cloak_version", "cloak_runtime_info", "cloak_launch_count", "cloak_keygen", "cloak_pool_create", "cloak_pool_destroy",
-           "cloak_pool_info", "cloak_pool_tables", "cloak_pool_dump", "cloak_pool_map_ms", "cloak_pool_adjacency", "cloak_pool_layout_report", "cloak_shuffle",
+           "cloak_pool_info", "cloak_pool_tables", "cloak_pool_dump", "cloak_pool_map_ms", "cloak_pool_map_phases", "cloak_pool_adjacency", "cloak_pool_layout_report", "cloak_shuffle",
            "cloak_unshuffle", "cloak_shuffle_many", "cloak_unshuffle_many", "cloak_relayout", "cloak_rekey_inplace", "cloak_rekey_pages_begin", "cloak_rekey_pages_step", "cloak_rekey_pages_finish", "cloak_shuffle_host", "cloak_unshuffle_host",
            "cloak_set_copy_engine", "cloak_set_copy_cache_hint", "cloak_set_gather_engine", "cloak_arena_plan", "cloak_permute_mlp_heads", "cloak_permute_experts", "cloak_load_mlp_heads", "cloak_load_tensors", "cloak_to_tile128",
            "cloak_gemv", "cloak_gemv_chain", "cloak_gemm", "cloak_gemm_chain", "cloak_gemv_chain_scratch_bytes",
@@ -91,6 +91,7 @@ lib.cloak_pool_info.argtypes = [_P, POINTER(_P), POINTER(_P), POINTER(c_uint32),
 lib.cloak_pool_tables.argtypes = [_P, _P, _P, _P, _P]
 lib.cloak_pool_dump.argtypes = [_P, _P, _P]
 lib.cloak_pool_map_ms.argtypes = [_P, POINTER(c_double)]
+lib.cloak_pool_map_phases.argtypes = [_P, POINTER(c_double), POINTER(c_double), POINTER(c_double)]
 lib.cloak_pool_adjacency.argtypes = [_P, POINTER(c_double), POINTER(c_double), POINTER(c_double), _P]
 lib.cloak_pool_reserve_workspace.argtypes = [_P, c_uint64]
 lib.cloak_pool_layout_report.argtypes = [_P, POINTER(cloak_layout_report), _P]
@@ -216,6 +217,12 @@ def cloak_pool_map_ms(pool):
     ms = c_double()
     _check(lib.cloak_pool_map_ms(pool, byref(ms)))
     return ms.value
+
+
+def cloak_pool_map_phases(pool):
+    a, b, c = c_double(), c_double(), c_double()
+    _check(lib.cloak_pool_map_phases(pool, byref(a), byref(b), byref(c)))
+    return dict(create_ms=a.value, map_ms=b.value, set_access_ms=c.value)
 
 
 def cloak_pool_adjacency(pool, stream=None):

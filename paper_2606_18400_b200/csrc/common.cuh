@@ -146,7 +146,7 @@ struct cloak_pool {
     uint32_t flags = 0;
     uint32_t nb = 0, bpp = 0, npages = 0, nslots = 0;
     bool vmm = false;
-    double map_ms = 0.0;
+    double map_ms = 0.0, map_create_ms = 0.0, map_map_ms = 0.0, map_access_ms = 0.0;   // the VMM mapper and its three phases
     char* base = nullptr;       // V (vmm) or D (emulated)
     // Real pages reserve TWO virtual ranges of bytes() each, back to back ("halves"): VA page v is mapped in half
     // page_half[v], at base + ((uint64_t)page_half[v] * npages + v) * page, and the authorised table carries the half:

@@ -226,6 +226,53 @@ def run_cfg2(args):
                       "note": "GB/s = 2 x payload / time for both, so the fused path's advantage shows as a higher rate"}
         del raw, tmp
 
+        # ---- NEXT-2 at model scale: the whole RAW checkpoint in pinned host memory, loaded by ONE cloak_load_tensors call (the
+        # kernels read across PCIe, permute and scatter in the same pass, keyed tensor order); beside it the plain pinned copy
+        host_load = None
+        if not getattr(args, "no_host_load", False):
+            tid = {nm: i for i, (nm, _) in enumerate(tensors)}
+            t0 = time.perf_counter()
+            hraw = {}
+            tmp_d = {}
+            for nm, shp in tensors:
+                key_ = shp
+                if key_ not in tmp_d:
+                    tmp_d[key_] = torch.empty(shp, dtype=torch.bfloat16, device="cuda")
+                synth_cuda.fill(tmp_d[key_], c["seed"], tid[nm])
+                hraw[nm] = torch.empty(shp, dtype=torch.bfloat16).pin_memory()
+                hraw[nm].copy_(tmp_d[key_])
+            torch.cuda.synchronize()
+            prep_s = time.perf_counter() - t0
+            items = []
+            for nm, shp in tensors:
+                if "." in nm:
+                    l, role = nm[1:].split(".")
+                    items.append((hraw[nm], off[nm], int(l), role))
+                else:
+                    items.append((hraw[nm], off[nm], 0, "plain", shp[0], shp[1]))
+            items = C.cloak_load_items(items)
+            sh0 = C.cloak_block_shape(c["hidden"], c["inter"], c["n_q"], c["n_kv"], c["head_dim"], C.CLOAK_BF16, 0)
+            ts = []
+            for _ in range(3):
+                torch.cuda.synchronize()
+                t0 = time.perf_counter()
+                C.cloak_load_tensors(c["key"], sh0, pc, items, C.CLOAK_ROWMAJOR)
+                torch.cuda.synchronize()
+                ts.append((time.perf_counter() - t0) * 1e3)
+            dst = torch.empty(max(sizes) // 2, dtype=torch.bfloat16, device="cuda")
+            torch.cuda.synchronize()
+            t0 = time.perf_counter()
+            for nm, shp in tensors:
+                dst[:hraw[nm].numel()].view(shp).copy_(hraw[nm], non_blocking=True)
+            torch.cuda.synchronize()
+            plain_ms = (time.perf_counter() - t0) * 1e3
+            ms = float(np.median(ts))
+            host_load = {"bytes": payload, "load_tensors_ms": ms, "gbs": payload / ms / 1e6, "plain_pinned_copy_ms": plain_ms,
+                         "plain_pinned_copy_gbs": payload / plain_ms / 1e6, "frac_of_plain_copy": plain_ms / ms,
+                         "mapper_plus_load_s": (C.cloak_pool_map_ms(pc) + ms) / 1e3, "pinned_alloc_and_fill_s": prep_s,
+                         "paper_context": "PAPER.md:226 (L40S): physical shuffle latency of Llama 3.1 8B 1.58 s"}
+            del hraw, tmp_d, dst, items
+
         keep = {nm: torch.empty(shp, dtype=torch.bfloat16, device="cuda") for nm, shp in tensors}
         load_s = _load_model(torch, C, synth_cuda, gen, 2, (pc, pn), offs, False, keep=keep)
 
@@ -337,7 +384,7 @@ def run_cfg2(args):
             "unshuffle": dict(rate(2 * payload, un_med, peak), ms_min=un_min), "roundtrip_bit_exact": bool(roundtrip),
             "shuffle_many": dict(rate(2 * payload, shm_med, peak), ms_min=shm_min, launches=2),
             "unshuffle_many": dict(rate(2 * payload, unm_med, peak), ms_min=unm_min, launches=2),
-            "load_paths": load_paths,
+            "load_paths": load_paths, "load_from_pinned_host": host_load,
             "decode_chain": res, "decode_read_bytes": read_bytes,
             "ideal_tokens_per_s_at_measured_peak": peak * 1e9 / read_bytes,
             "cloaked_vs_native_overhead_pct": ov, "cloaked_identical_to_native": bool(identical),
@@ -903,7 +950,32 @@ def run_rekey(args):
     return out
 
 
-RUNNERS = {"cfg2": run_cfg2, "cfg3": run_cfg3, "cfg4": run_cfg4, "moe": run_moe, "rekey": run_rekey}
+# ------------------------------------------------------------------------------------------ S2: the VMM mapper
+def run_mapper(args):
+    """S2 alone: cloak_pool_create / cloak_pool_destroy of a cfg2-sized pool (7 658 pages of 2 MiB), `--reps` times: median and
+    spread of the mapper and of its phases (cuMemCreate, cuMemMap, cuMemSetAccess), and of the teardown."""
+    torch, C, synth_cuda, gen = _imports()
+    c = gen.CONFIGS[2]
+    sizes = [2 * n * k for _, (n, k) in gen.model_tensors(2)]
+    _, total = C.cloak_arena_plan(c["key"], sizes, c["block"])
+    rows = []
+    for _ in range(max(3, args.reps if args.reps != 10 else 5)):
+        t0 = time.perf_counter()
+        p = C.cloak_pool_create(0, total, c["block"], c["page"], c["key"])
+        t1 = time.perf_counter()
+        r = dict(C.cloak_pool_map_phases(p), mapper_ms=C.cloak_pool_map_ms(p), pool_create_ms=(t1 - t0) * 1e3, npages=C.cloak_pool_info(p)["npages"])
+        t0 = time.perf_counter()
+        C.cloak_pool_destroy(p)
+        r["pool_destroy_ms"] = (time.perf_counter() - t0) * 1e3
+        rows.append(r)
+    med = {k: float(np.median([r[k] for r in rows])) for k in rows[0]}
+    return {"workload": "mapper: cfg2-sized pool, %d pages of 2 MiB" % rows[0]["npages"], "runs": rows, "median": med,
+            "min": {k: float(np.min([r[k] for r in rows])) for k in rows[0]}, "max": {k: float(np.max([r[k] for r in rows])) for k in rows[0]},
+            "us_per_page": {k: med[k] * 1e3 / rows[0]["npages"] for k in ("create_ms", "map_ms", "set_access_ms", "mapper_ms")},
+            "paper_context": "PAPER.md:226 / :265 (L40S): physical page shuffle of Llama 3.1 8B 1.58 s, ~1.5 s per GPU"}
+
+
+RUNNERS = {"cfg2": run_cfg2, "cfg3": run_cfg3, "cfg4": run_cfg4, "moe": run_moe, "rekey": run_rekey, "mapper": run_mapper}
 
 
 def main(argv=None):
