@@ -393,7 +393,7 @@ def run_cloak(args):
     # ---- the same GEMV chains on the identity-table ("native") pool: the overhead denominator.  Same launch mode,
     # cloaked and native interleaved rep by rep so that drift hits both alike.
     native_ms, cloaked_iso_ms, per_call_ms, plain_ms, matmul_ms = {}, {}, {}, {}, {}
-    for b in BATCHES:
+    for b in (() if args.no_ab else BATCHES):
         gemv_chain(pool_n, b)
         gemv_chain(pool_p, b)
         gemv_chain(pool_n, b, per_call=True)
@@ -427,7 +427,7 @@ def run_cloak(args):
 
     # ---- e2e: the same stages through the C ABI with HOST buffers (pinned), copies inside the timed region
     e2e = None
-    if rank == 0 or world > 1:
+    if (rank == 0 or world > 1) and not args.no_ab:
         hW = {nm: perm[nm].cpu().pin_memory() for nm in perm}            # permuted weights, for the staged variant
         hR = {nm: raw[nm].cpu().pin_memory() for nm in raw}              # the checkpoint as it is: raw weights in pinned host memory
         load_items = C.cloak_load_items([(hR[nm], o, 0, nm) for (nm, _), o in zip(shapes, offs)])
@@ -501,6 +501,8 @@ def run_cloak(args):
                   "unshuffle": sb["unshuffle"]}.get(s, sb["B"])
         stages[s] = {"ms": stage_ms[s], "gbs": gbs(nbytes, stage_ms[s]) if nbytes else None,
                      "frac_hbm": gbs(nbytes, stage_ms[s]) / peak if nbytes else None}
+    if args.no_ab:
+        native_ms = cloaked_iso_ms = per_call_ms = plain_ms = matmul_ms = {b: float("nan") for b in BATCHES}
     overhead = {f"b{b}": (cloaked_iso_ms[b] - native_ms[b]) / native_ms[b] * 100.0 for b in BATCHES}
     gemv_ms = sum(stage_ms[f"gemv_b{b}"] for b in BATCHES)
     gemv_launches = len(BATCHES)                        # one chain launch (7 projections) per batch
@@ -588,6 +590,7 @@ def main():
                     help="what the line carries besides the cfg1 step (`value`): cfg2, cfg3, cfg4 blocks (BASELINE.json configs[2..4]); "
                          "`--configs cfg1` for the step alone.  N > 1 replicas run the step alone.")
     ap.add_argument("--min-seconds", type=float, default=1.0, help="minimum length of each timed loop of the cfg2-4 blocks")
+    ap.add_argument("--no-ab", action="store_true", help="skip the isolated native / per-call / cuBLAS A/B runs and the e2e leg (for ncu launch lists of the step alone)")
     ap.add_argument("--sm-weighting", type=int, default=0, help="A/B: cloak_set_sm_weighting (1 measured per-SM shares, 0 equal shares)")
     ap.add_argument("--copy-hint", type=int, default=-1, help="A/B: cloak_set_copy_cache_hint (bit 0 stores, bit 1 loads evict_first)")
     ap.add_argument("--gemv-engine", type=int, default=0,

@@ -318,9 +318,12 @@ cloak_status cloak_to_tile128(const void* d_src, void* d_dst, uint32_t N, uint32
  * be captured without any warm-up.  The counters and partials are shared by all calls on one pool: those calls must be
  * ordered with respect to each other (one stream, or events), and replays of one graph must not overlap each other.
  * Different pools are independent and may run on different streams at the same time.
- * Co-residency: the streaming GEMV's CTAs wait for one another, so it is launched as a COOPERATIVE grid (all CTAs resident or
- * the launch waits / fails -- never a hang when other kernels hold SMs).  The GEMM needs no such guarantee: a CTA only ever
- * waits for partials of CTAs that drew their ticket before it, i.e. that are already running. */
+ * Co-residency.  A cloak_gemv_chain launch that contains an `after` op has a grid-wide barrier inside and is launched as a
+ * COOPERATIVE grid (all CTAs resident, or the launch waits / fails -- never a hang when other kernels hold SMs, e.g. two pools'
+ * chains on two streams).  Launches without one (cloak_gemv, chains of independent ops) wait only for the few CTAs that
+ * FOLLOW them in index order, which publish before they wait for anybody; with CTAs dispatched in index order -- what every
+ * NVIDIA GPU does, though CUDA does not promise it -- that cannot deadlock, and they stay ordinary launches.  The GEMM waits
+ * only for partials of CTAs that drew their ticket before the waiter, i.e. that are already running: no assumption at all. */
 typedef struct {
     uint64_t w_offset;
     uint32_t N, K;

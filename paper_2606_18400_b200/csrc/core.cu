@@ -153,7 +153,8 @@ namespace cloak { int gemv_coop_pdl_state(); }
 extern "C" const char* cloak_runtime_info(void) {
     static thread_local char buf[256];
     const int st = cloak::gemv_coop_pdl_state();
-    snprintf(buf, sizeof(buf), "gemv_chain: cooperative launch, programmatic dependent launch %s; kernels launched %llu",
+    snprintf(buf, sizeof(buf), "gemv_chain: cooperative launch where a chain has `after` ops (programmatic dependent launch %s), "
+                               "plain launch + programmatic dependent launch elsewhere; kernels launched %llu",
              st < 0 ? "not probed yet" : (st ? "accepted with it" : "rejected with it (dropped)"),
              (unsigned long long)cloak::g_launches.load());
     return buf;

@@ -455,13 +455,21 @@ std::atomic<bool> g_gemv_pdl{true};      // A/B switch (cloak_set_gemv_engine(2)
 // Counter words [0, GS_TILE_COUNTERS) of the pool's scratch are row-tile arrival counters, the rest op barriers.
 constexpr uint32_t GS_TILE_COUNTERS = (uint32_t)(WS_COUNTER_BYTES / 4) - 4 * GS_MAX_OPS;
 
-// Co-residency.  The CTAs of this kernel wait for one another (the owner of a cut row tile for the later contributors'
-// partials; the consumers of an `after` op for every CTA's arrival), so all of them must be on the machine at once.  One CTA
-// fits per SM (shared memory), and the grid is never larger than the SM count -- but another kernel holding SMs (a second
-// pool's chain on another stream, a framework kernel, an MPS / green-context SM limit) would leave some CTAs unscheduled and
-// the resident ones spinning for ever.  The launch is therefore COOPERATIVE: the driver starts the grid only when every CTA
-// can be resident, and fails the launch (cudaErrorCooperativeLaunchTooLarge) instead of hanging when that can never be.
-// Whether the cooperative attribute may be combined with programmatic stream serialization is probed on the first launch:
+// Co-residency.  The CTAs of this kernel wait for one another in two ways.
+//   (1) The consumers of an `after` op wait for EVERY CTA's arrival at an earlier op: a grid-wide barrier.  If some CTAs have no
+//       SM to run on -- another kernel holds SMs: a second pool's chain on another stream, a framework kernel, an MPS / green-
+//       context SM limit -- the resident ones spin for ever.  A launch that contains such an op is therefore COOPERATIVE: the
+//       driver starts the grid only when every CTA can be resident (one per SM; the grid is never larger than the SM count) and
+//       fails the launch (cudaErrorCooperativeLaunchTooLarge) instead of hanging when that can never be.  The price: a
+//       cooperative grid cannot begin while its stream predecessor still holds SMs, so programmatic dependent launch gains
+//       nothing between such launches (cfg2's 5-launch decode chain +1.4 %; a 12-layer MoE chain of ~25 launches +19 %).
+//   (2) The owner of a cut row tile waits for the partials of the FEW CTAs that follow it in range order, which publish them at
+//       the START of their ranges and wait for nobody first.  CTAs are dispatched in index order, so whatever subset is
+//       resident, the waits form a chain that ends at a CTA that is running or done: progress without full residency (the
+//       dispatch order is how every NVIDIA GPU behaves, not an architectural promise -- cloak.h says so).  Launches with only
+//       this kind of wait (cloak_gemv, chains of independent ops) stay ordinary launches and keep programmatic dependent
+//       launch, which hides ~1 us per launch boundary (cfg1 layer as 7 calls: 92.5 us against 99.7 us cooperative).
+// Whether the cooperative attribute may be combined with programmatic stream serialization is probed on the first such launch:
 // if the driver rejects the pair, PDL is dropped, not the guarantee.
 std::atomic<unsigned long long*> g_trace{nullptr};     // cloak_set_trace
 static std::atomic<int> g_coop_with_pdl{-1};     // -1 unknown, 0 rejected, 1 accepted
@@ -469,6 +477,7 @@ int gemv_coop_pdl_state() { return g_coop_with_pdl.load(std::memory_order_relaxe
 
 template <int CU, int NT>
 static cloak_status launch(const ChainArgs& a, int ctas, int device, cudaStream_t s) {
+    const bool coop = a.any_signal != 0;
     constexpr size_t smem = (size_t)gs_stages(CU) * GS_ROWS * (CU * 512u + GS_PAD);
     static std::atomic<uint64_t> opted{0};
     auto* kernel = gemv_chain_kernel<CU, NT>;
@@ -484,22 +493,22 @@ static cloak_status launch(const ChainArgs& a, int ctas, int device, cudaStream_
     at[0].val.cooperative = 1;
     at[1].id = cudaLaunchAttributeProgrammaticStreamSerialization;
     at[1].val.programmaticStreamSerializationAllowed = 1;
-    cfg.attrs = at;
-    const bool want_pdl = g_gemv_pdl.load(std::memory_order_relaxed) && g_coop_with_pdl.load(std::memory_order_relaxed) != 0;
-    cfg.numAttrs = want_pdl ? 2 : 1;
+    cfg.attrs = coop ? at : at + 1;
+    const bool want_pdl = g_gemv_pdl.load(std::memory_order_relaxed) && (!coop || g_coop_with_pdl.load(std::memory_order_relaxed) != 0);
+    cfg.numAttrs = (coop ? 1 : 0) + (want_pdl ? 1 : 0);
     cudaError_t e = cudaLaunchKernelEx(&cfg, kernel, a);
-    if (e != cudaSuccess && want_pdl && g_coop_with_pdl.load(std::memory_order_relaxed) < 0 &&
+    if (e != cudaSuccess && coop && want_pdl && g_coop_with_pdl.load(std::memory_order_relaxed) < 0 &&
         (e == cudaErrorInvalidValue || e == cudaErrorNotSupported || e == cudaErrorInvalidConfiguration)) {
         cudaGetLastError();
         g_coop_with_pdl.store(0, std::memory_order_relaxed);
         cfg.numAttrs = 1;
         e = cudaLaunchKernelEx(&cfg, kernel, a);
-    } else if (e == cudaSuccess && want_pdl) {
+    } else if (e == cudaSuccess && coop && want_pdl) {
         g_coop_with_pdl.store(1, std::memory_order_relaxed);
     }
     if (e != cudaSuccess) {
         cudaGetLastError();
-        return fail(CLOAK_ERR_CUDA, "gemv chain launch (%d cooperative CTAs): %s", ctas, cudaGetErrorString(e));
+        return fail(CLOAK_ERR_CUDA, "gemv chain launch (%d %sCTAs): %s", ctas, coop ? "cooperative " : "", cudaGetErrorString(e));
     }
     launched();
     return CLOAK_OK;
@@ -595,7 +604,7 @@ cloak_status gemv_stream_launch(const cloak_pool* pool, const cloak_gemv_op* ops
     a.counters = reinterpret_cast<uint32_t*>(pool->ws);
     a.opsync = a.counters + GS_TILE_COUNTERS;
     a.part = reinterpret_cast<float*>(pool->ws + WS_COUNTER_BYTES);
-    a.early = (g_gemv_pdl.load(std::memory_order_relaxed) && g_coop_with_pdl.load(std::memory_order_relaxed) != 0 && !pool->dirty) ? 1u : 0u;
+    a.early = (g_gemv_pdl.load(std::memory_order_relaxed) && !pool->dirty) ? 1u : 0u;
     if (pool->dirty && pool->dirty_stream == s) pool->dirty = false;   // this launch waits for the writer in full
     const bool nt2 = batch > 8;
 #define GS_CASE(C) case C: return nt2 ? launch<C, 2>(a, ctas, pool->device, s) : launch<C, 1>(a, ctas, pool->device, s)

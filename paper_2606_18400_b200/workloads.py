@@ -975,7 +975,33 @@ def run_mapper(args):
             "paper_context": "PAPER.md:226 / :265 (L40S): physical page shuffle of Llama 3.1 8B 1.58 s, ~1.5 s per GPU"}
 
 
-RUNNERS = {"cfg2": run_cfg2, "cfg3": run_cfg3, "cfg4": run_cfg4, "moe": run_moe, "rekey": run_rekey, "mapper": run_mapper}
+# ------------------------------------------------------------------------------------------ S5 A/B: the column gather
+def run_permute_ab(args):
+    """cloak_permute_mlp_heads of the cfg1 layer, and of `down` alone, under both column-gather engines (cloak_set_gather_engine:
+    1 = element gather, 0 = pair-interleaved gather); the outputs must be identical."""
+    torch, C, synth_cuda, gen = _imports()
+    c = gen.CONFIGS[1]
+    shapes = gen.layer_shapes(c["hidden"], c["inter"], c["n_q"], c["n_kv"], c["head_dim"])
+    raw = {nm: synth_cuda.fill(torch.empty(shp, dtype=torch.bfloat16, device="cuda"), c["seed"], i) for i, (nm, shp) in enumerate(shapes)}
+    out = {nm: torch.empty_like(t) for nm, t in raw.items()}
+    sh = C.cloak_block_shape(c["hidden"], c["inter"], c["n_q"], c["n_kv"], c["head_dim"], C.CLOAK_BF16, 0)
+    peak, _ = hbm_peak()
+    B = sum(t.numel() * 2 for t in raw.values())
+    res, keep = {}, {}
+    try:
+        for eng, name in ((1, "element_gather"), (0, "pair_interleaved_gather")):
+            C.cloak_set_gather_engine(eng)
+            full, _ = time_gpu(torch, lambda: C.cloak_permute_mlp_heads(c["key"], sh, **raw, **{k + "_o": v for k, v in out.items()}), 30)
+            down, _ = time_gpu(torch, lambda: C.cloak_permute_mlp_heads(c["key"], sh, down=raw["down"], down_o=out["down"]), 30)
+            keep[eng] = {nm: t.clone() for nm, t in out.items()}
+            res[name] = {"layer_permute": rate(2 * B, full, peak), "down_alone_incl_keygen": rate(4 * raw["down"].numel(), down, peak)}
+    finally:
+        C.cloak_set_gather_engine(0)
+    res["identical"] = bool(all(torch.equal(keep[0][nm], keep[1][nm]) for nm in out))
+    return {"workload": "permute_ab: cfg1 layer, S5 under both column-gather engines", **res}
+
+
+RUNNERS = {"cfg2": run_cfg2, "cfg3": run_cfg3, "cfg4": run_cfg4, "moe": run_moe, "rekey": run_rekey, "mapper": run_mapper, "permute_ab": run_permute_ab}
 
 
 def main(argv=None):
