@@ -52,12 +52,35 @@ def test_argument_checks_without_a_device(C):
         (lambda: C.cloak_silu_mul(None, None, None, 4, C.CLOAK_F32), C.CLOAK_ERR_INVALID),
         (lambda: C.cloak_relayout(None, None), C.CLOAK_ERR_INVALID),
         (lambda: C.cloak_pool_destroy(None), C.CLOAK_ERR_INVALID),
+        # round 2's calls
+        (lambda: C.cloak_pool_reserve_workspace(None, 1 << 20), C.CLOAK_ERR_INVALID),
+        (lambda: C.cloak_rekey_pages_begin(None, 1, 1), C.CLOAK_ERR_INVALID),
+        (lambda: C.cloak_rekey_pages_step(None, 1), C.CLOAK_ERR_INVALID),
+        (lambda: C.cloak_rekey_pages_finish(None), C.CLOAK_ERR_INVALID),
+        (lambda: C.cloak_pool_layout_report(None), C.CLOAK_ERR_INVALID),
+        (lambda: C.cloak_pool_adjacency(None), C.CLOAK_ERR_INVALID),
+        (lambda: C.cloak_pool_map_phases(None), C.CLOAK_ERR_INVALID),
+        (lambda: C.cloak_set_sm_weighting(7), C.CLOAK_ERR_INVALID),
+        (lambda: C.cloak_set_copy_cache_hint(4), C.CLOAK_ERR_INVALID),
+        (lambda: C.cloak_set_gather_engine(2), C.CLOAK_ERR_INVALID),
+        (lambda: C.cloak_set_trace(12), C.CLOAK_ERR_ALIGN),
+        (lambda: C.cloak_load_tensors(1, C.cloak_block_shape(256, 768, 4, 2, 64, C.CLOAK_BF16, 0), None, [(16, 0, 0, "gate")]), C.CLOAK_ERR_INVALID),
+        (lambda: C.cloak_gemv_chain_scratch_bytes(None, [], 1), C.CLOAK_ERR_INVALID),
+        (lambda: C.cloak_gemm_chain_scratch_bytes(None, [], 1), C.CLOAK_ERR_INVALID),
     ]
     for fn, st in cases:
         with pytest.raises(C.CloakError) as ei:
             fn()
         assert ei.value.status == st, C.cloak_last_error()
         assert C.cloak_last_error()
+
+
+def test_runtime_info_and_knobs_are_callable_without_a_device(C):
+    assert "gemv_chain" in C.cloak_runtime_info()
+    C.cloak_set_sm_weighting(0)
+    C.cloak_set_copy_cache_hint(0)
+    C.cloak_set_gather_engine(0)
+    C.cloak_set_trace(None)
 
 
 def test_no_cpu_fallback(C):

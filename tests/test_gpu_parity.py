@@ -962,6 +962,25 @@ def test_error_codes_on_device():
         with pytest.raises(C.CloakError) as ei:
             C.cloak_gemv(p.h, C.cloak_tensor(0, 1 << 20, 256, C.CLOAK_F32, C.CLOAK_ROWMAJOR), x, x, 1)
         assert ei.value.status == C.CLOAK_ERR_INVALID
+        with pytest.raises(C.CloakError) as ei:                       # emulated pages cannot be re-mapped
+            C.cloak_rekey_pages_begin(p.h, 2, 1)
+        assert ei.value.status == C.CLOAK_ERR_UNSUPPORTED
+        assert C.cloak_rekey_pages_step(p.h, 4) == 0                   # no re-key in progress: nothing left, no error
+        C.cloak_pool_reserve_workspace(p.h, 1 << 20)                   # already there: a no-op
+        C.cloak_pool_reserve_workspace(p.h, 40 << 20)                  # grows
+    with Pool(8 << 20, 65536, 2 << 20, 1) as p, Pool(8 << 20, 65536, 2 << 20, 1, C.CLOAK_POOL_IDENTITY) as pi:
+        with pytest.raises(C.CloakError) as ei:
+            C.cloak_rekey_pages_begin(pi.h, 2, 1)
+        assert ei.value.status == C.CLOAK_ERR_INVALID
+        with pytest.raises(C.CloakError) as ei:
+            C.cloak_rekey_pages_begin(p.h, 2, 65)
+        assert ei.value.status == C.CLOAK_ERR_INVALID
+        C.cloak_rekey_pages_begin(p.h, 2, 1)
+        for call in (lambda: C.cloak_rekey_pages_begin(p.h, 3, 1), lambda: C.cloak_rekey_inplace(p.h, 3, 0)):
+            with pytest.raises(C.CloakError) as ei:                   # one re-key at a time
+                call()
+            assert ei.value.status == C.CLOAK_ERR_INVALID
+        # (the pool is destroyed with the re-key unfinished: its teardown must cope)
 
 
 # ------------------------------------------------------------------ NEXT-4: mixture-of-experts layers
