@@ -428,6 +428,12 @@ cloak_status cloak_set_gemm_schedule(int static_pct, int dyn_chunk_tiles);
 cloak_status cloak_gemv_host(const cloak_pool* pool, const cloak_tensor* w, const void* h_x, void* h_y,
                              uint32_t batch, void* stream);
 
+/* Host-buffer form of cloak_gemv_chain for INDEPENDENT ops (no d_gate / d_act / after): every op's d_x and d_y are HOST pointers
+ * (pinned for full speed).  All X are copied up, the ops run (one chain launch where the streaming kernel takes them all), all Y
+ * are copied back, and `stream` is synchronised once. */
+cloak_status cloak_gemv_chain_host(const cloak_pool* pool, const cloak_gemv_op* h_ops, uint32_t n_ops, uint32_t batch,
+                                   void* stream);
+
 /* Decode-chain glue: out[i] = silu(g[i]) * u[i] (the gated MLP's activation, O9), n elements. */
 cloak_status cloak_silu_mul(const void* d_g, const void* d_u, void* d_out, uint64_t n, cloak_dtype dt,
                             void* stream);

@@ -27,7 +27,7 @@ SYMBOLS = ["cloak_last_error", "cloak_version", "cloak_runtime_info", "cloak_lau
            "cloak_unshuffle", "cloak_shuffle_many", "cloak_unshuffle_many", "cloak_relayout", "cloak_rekey_inplace", "cloak_rekey_pages_begin", "cloak_rekey_pages_step", "cloak_rekey_pages_finish", "cloak_shuffle_host", "cloak_unshuffle_host",
            "cloak_set_copy_engine", "cloak_set_copy_cache_hint", "cloak_set_gather_engine", "cloak_arena_plan", "cloak_permute_mlp_heads", "cloak_permute_experts", "cloak_load_mlp_heads", "cloak_load_tensors", "cloak_to_tile128",
            "cloak_gemv", "cloak_gemv_chain", "cloak_gemm", "cloak_gemm_chain", "cloak_gemv_chain_scratch_bytes",
-           "cloak_gemm_chain_scratch_bytes", "cloak_pool_reserve_workspace", "cloak_set_gemv_engine", "cloak_sm_weights", "cloak_set_sm_weighting", "cloak_set_trace", "cloak_set_gemm_schedule", "cloak_gemm_plan", "cloak_gemv_host", "cloak_silu_mul"]
+           "cloak_gemm_chain_scratch_bytes", "cloak_pool_reserve_workspace", "cloak_set_gemv_engine", "cloak_sm_weights", "cloak_set_sm_weighting", "cloak_set_trace", "cloak_set_gemm_schedule", "cloak_gemm_plan", "cloak_gemv_host", "cloak_gemv_chain_host", "cloak_silu_mul"]
 
 
 class CloakError(RuntimeError):
@@ -129,6 +129,7 @@ lib.cloak_gemv_chain_scratch_bytes.argtypes = [_P, POINTER(cloak_gemv_op), c_uin
 lib.cloak_gemm_chain_scratch_bytes.argtypes = [_P, POINTER(cloak_gemm_op), c_uint32, c_uint32, POINTER(c_uint64)]
 lib.cloak_gemm.argtypes = [_P, POINTER(cloak_tensor), _P, _P, c_uint32, _P]
 lib.cloak_gemv_host.argtypes = [_P, POINTER(cloak_tensor), _P, _P, c_uint32, _P]
+lib.cloak_gemv_chain_host.argtypes = [_P, POINTER(cloak_gemv_op), c_uint32, c_uint32, _P]
 lib.cloak_silu_mul.argtypes = [_P, _P, _P, c_uint64, c_int, _P]
 lib.cloak_launch_count.restype = c_uint64
 for _n in SYMBOLS[4:]:
@@ -455,6 +456,12 @@ def cloak_gemm_chain(pool, ops, batch, stream=None):
 
 def cloak_gemv_host(pool, tensor, h_x, h_y, batch, stream=None):
     _check(lib.cloak_gemv_host(pool, byref(tensor), _ptr(h_x), _ptr(h_y), batch, _stream(stream)))
+
+
+def cloak_gemv_chain_host(pool, ops, batch, stream=None):
+    """ops as for cloak_gemv_chain, with HOST x / y buffers (numpy arrays or pinned torch tensors)."""
+    arr = ops if isinstance(ops, ctypes.Array) else cloak_gemv_ops(ops)
+    _check(lib.cloak_gemv_chain_host(pool, arr, len(arr), batch, _stream(stream)))
 
 
 def cloak_silu_mul(d_g, d_u, d_out, n, dt, stream=None):

@@ -395,6 +395,53 @@ extern "C" cloak_status cloak_gemv_chain(const cloak_pool* pool, const cloak_gem
     return CLOAK_OK;
 }
 
+// Host-buffer form of cloak_gemv_chain for independent ops: every op's d_x / d_y are HOST pointers.  All X go up, the chain
+// runs, all Y come back; the stream is synchronised ONCE (cloak_gemv_host does that per projection).
+extern "C" cloak_status cloak_gemv_chain_host(const cloak_pool* pool, const cloak_gemv_op* h_ops, uint32_t n_ops, uint32_t batch,
+                                              void* stream) {
+    if (!h_ops || n_ops == 0) return fail(CLOAK_ERR_INVALID, "gemv_chain_host: no ops");
+    size_t total = 0;
+    std::vector<size_t> xo(n_ops), yo(n_ops);
+    for (uint32_t i = 0; i < n_ops; ++i) {
+        cloak_status st = gemv_check(pool, &h_ops[i].w, h_ops[i].d_x, h_ops[i].d_y, batch, "gemv_chain_host");
+        if (st != CLOAK_OK) return st;
+        if (h_ops[i].d_gate || h_ops[i].d_act || h_ops[i].after)
+            return fail(CLOAK_ERR_INVALID, "gemv_chain_host: op %u: ops must be independent (no d_gate / d_act / after)", i);
+        const size_t e = h_ops[i].w.dt == CLOAK_F32 ? 4 : 2;
+        xo[i] = total;
+        total += ((size_t)batch * h_ops[i].w.K * e + 255) & ~(size_t)255;
+        yo[i] = total;
+        total += ((size_t)batch * h_ops[i].w.N * e + 255) & ~(size_t)255;
+    }
+    DeviceGuard g(pool->device);
+    cudaStream_t s = (cudaStream_t)stream;
+    AsyncBuf buf(s);
+    if (cloak_status ast = buf.alloc(total)) return ast;
+    char* d = static_cast<char*>(buf.p);
+    std::vector<cloak_gemv_op> ops(h_ops, h_ops + n_ops);
+    for (uint32_t i = 0; i < n_ops; ++i) {
+        const size_t e = ops[i].w.dt == CLOAK_F32 ? 4 : 2;
+        CLOAK_CUDA(cudaMemcpyAsync(d + xo[i], h_ops[i].d_x, (size_t)batch * ops[i].w.K * e, cudaMemcpyHostToDevice, s));
+        ops[i].d_x = d + xo[i];
+        ops[i].d_y = d + yo[i];
+    }
+    bool all_stream = !g_force_oneshot.load(std::memory_order_relaxed);
+    for (uint32_t i = 0; i < n_ops && all_stream; ++i) all_stream = gemv_stream_chunk(pool, &ops[i].w, batch) >= 1;
+    cloak_status st = CLOAK_OK;
+    if (all_stream) {
+        st = cloak_gemv_chain(pool, ops.data(), n_ops, batch, stream);
+    } else {
+        for (uint32_t i = 0; i < n_ops && st == CLOAK_OK; ++i) st = gemv_device(pool, &ops[i].w, ops[i].d_x, ops[i].d_y, batch, s);
+    }
+    if (st != CLOAK_OK) return st;
+    for (uint32_t i = 0; i < n_ops; ++i) {
+        const size_t e = ops[i].w.dt == CLOAK_F32 ? 4 : 2;
+        CLOAK_CUDA(cudaMemcpyAsync(h_ops[i].d_y, d + yo[i], (size_t)batch * ops[i].w.N * e, cudaMemcpyDeviceToHost, s));
+    }
+    CLOAK_CUDA(cudaStreamSynchronize(s));
+    return CLOAK_OK;
+}
+
 extern "C" cloak_status cloak_gemv_chain_scratch_bytes(const cloak_pool* pool, const cloak_gemv_op* h_ops, uint32_t n_ops,
                                                        uint32_t batch, uint64_t* h_bytes) {
     if (!h_ops || n_ops == 0 || !h_bytes) return fail(CLOAK_ERR_INVALID, "gemv_chain_scratch_bytes: NULL argument or no ops");

@@ -601,6 +601,14 @@ def test_gemv_host_entry_point():
         C.cloak_gemv_host(p.h, C.cloak_tensor(0, N, K, C.CLOAK_BF16, C.CLOAK_ROWMAJOR), hx, hy, 4)
         got = O.bf16_bits_to_f32(hy.numpy().view(np.uint16))
         check_linear(got, X, Wm, "bf16", f"gemv_host:{N}x{K}:b4", TOL["bf16"])
+        # the chain form: several independent ops, host x / y, one synchronisation; equals the single host calls bit for bit
+        hy2 = [torch.zeros(4, N, dtype=torch.int16).pin_memory() for _ in range(3)]
+        w = C.cloak_tensor(0, N, K, C.CLOAK_BF16, C.CLOAK_ROWMAJOR)
+        C.cloak_gemv_chain_host(p.h, [(w, hx, y, 0) for y in hy2], 4)
+        assert all(torch.equal(y, hy) for y in hy2)
+        with pytest.raises(C.CloakError) as ei:                       # dependent ops have no host form
+            C.cloak_gemv_chain_host(p.h, [(w, hx, hy2[0], 0), (w, hx, hy2[1], 1)], 4)
+        assert ei.value.status == C.CLOAK_ERR_INVALID
 
 
 def test_cfg0_mlp_end_to_end_permuted_and_cloaked():
