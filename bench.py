@@ -446,9 +446,8 @@ def run_cloak(args):
         host_ops = C.cloak_gemv_ops([(tens[nm], hX[nm], hY[nm], 0) for nm, _ in shapes])
         n_e2e = max(1, min(args.steps, 5))
         times = {}
-        for variant in ("shuffle_host", "load_in_place", "load"):
-            C.cloak_set_load_engine(1 if variant == "load_in_place" else 0)
-            for _ in range(3):                  # warm-up: the library's stream-ordered pool settles on its staging buffers
+        for variant in ("shuffle_host", "load"):
+            for _ in range(2):                  # warm-up: the library's stream-ordered pool settles on its buffers
                 e2e_step(variant)
             barrier()
             t0 = time.perf_counter()
@@ -473,11 +472,9 @@ def run_cloak(args):
         e2e = {"value": world * e2e_bytes / dt / 1e9, "unit": "GB/s", "h2d_bytes_per_step": h2d,
                "d2h_bytes_per_step": d2h, "ms_per_step": dt * 1e3,
                "h2d_gbs": h2d / dt / 1e9, "h2d_peak_gbs_measured": h2d_peak, "frac_of_h2d_peak": h2d / dt / 1e9 / h2d_peak,
-               "variants_ms_per_step": {"load_tensors_sources_read_in_place_by_the_kernels": times["load_in_place"] * 1e3,
-                                        "cloak_shuffle_host_of_pre_permuted_weights": times["shuffle_host"] * 1e3},
-               "what": "cloak_load_tensors of the layer's RAW weights from pinned host memory (each tensor crosses PCIe by the copy engine "
-                       "into a staging buffer while the previous one is permuted and scattered through the table in one pass; keyed tensor "
-                       "order) + cloak_gemv_chain_host of the 7 projections (batch 1); PCIe-bound: frac_of_h2d_peak = achieved "
+               "variants_ms_per_step": {"cloak_shuffle_host_of_pre_permuted_weights": times["shuffle_host"] * 1e3},
+               "what": "cloak_load_tensors of the layer's RAW weights from pinned host memory (the gather kernels read across PCIe, "
+                       "permute and scatter through the table in one pass; keyed tensor order) + cloak_gemv_chain_host of the 7 projections (batch 1); PCIe-bound: frac_of_h2d_peak = achieved "
                        "host->device rate / a plain pinned copy of the same tensors"}
 
     map_ms = C.cloak_pool_map_ms(pool_a)

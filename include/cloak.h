@@ -270,10 +270,9 @@ cloak_status cloak_load_mlp_heads(uint64_t key, const cloak_block_shape* shape, 
  * and the pages are decided before any weight is transferred).
  * Each item is one tensor of a decoder layer (role GATE .. O: shape from `shape`, permutation that of cloak_permute_mlp_heads
  * for item.layer -- shape->layer is ignored) or a PLAIN [N, K] matrix that is not permuted (embeddings, lm_head, a router).
- * The tensor is read ONCE from item.src -- a device pointer, or a pointer to pinned (page-locked, device-mapped) host memory
- * (pageable host memory is refused with CLOAK_ERR_INVALID).  A pinned host tensor of up to 256 MiB crosses PCIe by the copy
- * engine into one of two staging buffers on a second stream, the transfer of tensor i+1 overlapping the gather of tensor i; a
- * larger one is read across PCIe by the gather kernels themselves (cloak_set_load_engine(1): always) -- and written straight through the pool's block
+ * The tensor is read ONCE from item.src -- a device pointer, or a pointer to pinned (page-locked, device-mapped) host memory,
+ * which the gather kernels then read across PCIe themselves: no staging copy (pageable host memory is refused with
+ * CLOAK_ERR_INVALID) -- and written straight through the pool's block
  * table at arena byte item.arena_offset (a block multiple) in `layout` (CLOAK_ROWMAJOR, or CLOAK_TILE128: the storage
  * conversion is an address computation in the same pass; N and K multiples of 128).  The pool bytes afterwards equal those of
  * cloak_permute_mlp_heads (-> cloak_to_tile128) -> cloak_shuffle, tail of a final partial block zeroed: 2 bytes of traffic per
@@ -291,10 +290,6 @@ typedef struct {
 } cloak_load_item;
 cloak_status cloak_load_tensors(uint64_t key, const cloak_block_shape* shape, cloak_pool* pool,
                                 const cloak_load_item* h_items, uint32_t n, cloak_layout layout, void* stream);
-
-/* Host sources of cloak_load_tensors: 0 = automatic (copy engine + staging up to 256 MiB per tensor, else read in place by the
- * kernels), 1 = always read in place.  For A/B measurement; process-wide. */
-cloak_status cloak_set_load_engine(int engine);
 
 /* Storage-layout conversion ROWMAJOR -> TILE128 of a logical [N, K] matrix (N, K multiples of 128).
  * Out of place.  Asynchronous on `stream`. */

@@ -25,7 +25,7 @@ STATUS_NAMES = {0: "CLOAK_OK", -1: "CLOAK_ERR_INVALID", -2: "CLOAK_ERR_ALIGN", -
 SYMBOLS = ["cloak_last_error", "cloak_version", "cloak_runtime_info", "cloak_launch_count", "cloak_keygen", "cloak_pool_create", "cloak_pool_destroy",
            "cloak_pool_info", "cloak_pool_tables", "cloak_pool_dump", "cloak_pool_map_ms", "cloak_pool_map_phases", "cloak_pool_adjacency", "cloak_pool_layout_report", "cloak_shuffle",
            "cloak_unshuffle", "cloak_shuffle_many", "cloak_unshuffle_many", "cloak_relayout", "cloak_rekey_inplace", "cloak_rekey_pages_begin", "cloak_rekey_pages_step", "cloak_rekey_pages_finish", "cloak_shuffle_host", "cloak_unshuffle_host",
-           "cloak_set_copy_engine", "cloak_set_copy_cache_hint", "cloak_set_gather_engine", "cloak_arena_plan", "cloak_permute_mlp_heads", "cloak_permute_experts", "cloak_load_mlp_heads", "cloak_load_tensors", "cloak_set_load_engine", "cloak_to_tile128",
+           "cloak_set_copy_engine", "cloak_set_copy_cache_hint", "cloak_set_gather_engine", "cloak_arena_plan", "cloak_permute_mlp_heads", "cloak_permute_experts", "cloak_load_mlp_heads", "cloak_load_tensors", "cloak_to_tile128",
            "cloak_gemv", "cloak_gemv_chain", "cloak_gemm", "cloak_gemm_chain", "cloak_gemv_chain_scratch_bytes",
            "cloak_gemm_chain_scratch_bytes", "cloak_pool_reserve_workspace", "cloak_set_gemv_engine", "cloak_sm_weights", "cloak_set_sm_weighting", "cloak_set_trace", "cloak_set_gemm_schedule", "cloak_gemm_plan", "cloak_gemv_host", "cloak_gemv_chain_host", "cloak_silu_mul"]
 
@@ -109,7 +109,6 @@ lib.cloak_unshuffle_host.argtypes = [_P, _P, c_uint64, c_uint64, _P]
 lib.cloak_set_copy_engine.argtypes = [c_int]
 lib.cloak_set_copy_cache_hint.argtypes = [c_int]
 lib.cloak_set_gather_engine.argtypes = [c_int]
-lib.cloak_set_load_engine.argtypes = [c_int]
 lib.cloak_set_gemv_engine.argtypes = [c_int]
 lib.cloak_sm_weights.argtypes = [c_int, c_uint32, _P, POINTER(c_uint32)]
 lib.cloak_set_sm_weighting.argtypes = [c_int]
@@ -312,10 +311,6 @@ def cloak_set_copy_cache_hint(hint):
 
 def cloak_set_gather_engine(engine):
     _check(lib.cloak_set_gather_engine(engine))
-
-
-def cloak_set_load_engine(engine):
-    _check(lib.cloak_set_load_engine(engine))
 
 
 def cloak_set_gemv_engine(engine):

@@ -346,7 +346,6 @@ static cloak_status cols_ring(const void* src, Dst dst, const uint32_t* map, uin
 }
 
 static std::atomic<bool> g_cols_pairs{true};     // A/B switch (cloak_set_gather_engine)
-static std::atomic<int> g_load_engine{0};        // A/B switch (cloak_set_load_engine)
 
 template <typename M, typename Dst>
 static cloak_status cols_pair(const void* src, Dst dst, const uint32_t* map, uint32_t seg, uint32_t nrows, uint32_t ncols,
@@ -667,14 +666,10 @@ extern "C" cloak_status cloak_load_tensors(uint64_t key, const cloak_block_shape
             }
         }
     }
-    pool->wrote(s);
-    const uint32_t vptr = layout == CLOAK_TILE128 ? (uint32_t)(128 * e / 16) : 0u;     // vectors per tile row
-    // Where each source lives.  Device memory and pinned host memory can be read by the kernels; pageable host memory cannot.
-    // A pinned host tensor of up to 256 MiB is brought over by the copy engine into one of two staging buffers on a second
-    // stream, so that the transfer of tensor i+1 overlaps the gather of tensor i (measured on B200: the copy engine moves
-    // 55 GB/s across PCIe, SM loads 51 GB/s); larger ones (embeddings) are read in place.  cloak_set_load_engine: 1 = always in place.
-    std::vector<uint8_t> staged(n, 0);
-    size_t stage_cap = 0;
+    // Device memory and pinned host memory can be read by the kernels; pageable host memory cannot.  (Bringing pinned host
+    // tensors over with the copy engine into a staging buffer first -- 55 GB/s against the 51 GB/s of SM loads across PCIe --
+    // was measured, in stream order and overlapped through a second stream, and dropped: 8.57-8.9 ms for the cfg1 layer against
+    // 8.57 ms in place; the in-place read needs no buffer and no extra stream.)
     for (uint32_t i = 0; i < n; ++i) {
         cudaPointerAttributes at;
         if (cudaPointerGetAttributes(&at, items[i].src) != cudaSuccess) {
@@ -683,47 +678,10 @@ extern "C" cloak_status cloak_load_tensors(uint64_t key, const cloak_block_shape
         }
         if (at.type == cudaMemoryTypeUnregistered)
             return fail(CLOAK_ERR_INVALID, "load_tensors: a source is pageable host memory: pin it (cudaHostAlloc / cudaHostRegister) or copy it to the device");
-        const size_t bytes = (size_t)items[i].N * items[i].K * e;
-        if (at.type == cudaMemoryTypeHost && g_load_engine.load(std::memory_order_relaxed) != 1 && bytes <= (256u << 20)) {
-            staged[i] = 1;
-            if (bytes > stage_cap) stage_cap = bytes;
-        }
     }
-    AsyncBuf stage(s);
-    cudaStream_t cs = nullptr;
-    cudaEvent_t copied[2] = {nullptr, nullptr}, freed[2] = {nullptr, nullptr}, ready = nullptr;
-    struct StageGuard {                                   // the second stream and its events live for this call only
-        cudaStream_t& cs; cudaEvent_t (&a)[2]; cudaEvent_t (&b)[2]; cudaEvent_t& r;
-        ~StageGuard() {
-            for (int k = 0; k < 2; ++k) { if (a[k]) cudaEventDestroy(a[k]); if (b[k]) cudaEventDestroy(b[k]); }
-            if (r) cudaEventDestroy(r);
-            if (cs) cudaStreamDestroy(cs);               // (work already queued on it still completes)
-        }
-    } stage_guard{cs, copied, freed, ready};
-    if (stage_cap) {
-        stage_cap = (stage_cap + 255) & ~(size_t)255;
-        if (cloak_status ast = stage.alloc(2 * stage_cap)) return ast;
-        CLOAK_CUDA(cudaStreamCreateWithFlags(&cs, cudaStreamNonBlocking));
-        for (int k = 0; k < 2; ++k) {
-            CLOAK_CUDA(cudaEventCreateWithFlags(&copied[k], cudaEventDisableTiming));
-            CLOAK_CUDA(cudaEventCreateWithFlags(&freed[k], cudaEventDisableTiming));
-        }
-        CLOAK_CUDA(cudaEventCreateWithFlags(&ready, cudaEventDisableTiming));
-        CLOAK_CUDA(cudaEventRecord(ready, s));            // the staging buffers exist (stream-ordered allocation on s)
-        CLOAK_CUDA(cudaStreamWaitEvent(cs, ready, 0));
-    }
-    uint32_t nstaged = 0, idx = 0;
-    for (const Item& x0 : items) {
-        Item x = x0;
-        if (staged[idx++]) {
-            const int k = nstaged & 1;
-            char* buf = static_cast<char*>(stage.p) + (size_t)k * stage_cap;
-            if (nstaged >= 2) CLOAK_CUDA(cudaStreamWaitEvent(cs, freed[k], 0));       // the gather that read this buffer is done
-            CLOAK_CUDA(cudaMemcpyAsync(buf, x.src, (size_t)x.N * x.K * e, cudaMemcpyHostToDevice, cs));
-            CLOAK_CUDA(cudaEventRecord(copied[k], cs));
-            CLOAK_CUDA(cudaStreamWaitEvent(s, copied[k], 0));
-            x.src = buf;
-        }
+    pool->wrote(s);
+    const uint32_t vptr = layout == CLOAK_TILE128 ? (uint32_t)(128 * e / 16) : 0u;     // vectors per tile row
+    for (const Item& x : items) {
         PoolDst dst{pool->base, pool->d_T, x.off, pool->log2_block, vptr};
         const uint32_t* pi = nullptr;
         const uint32_t *kappa = nullptr, *eta = nullptr;
@@ -749,10 +707,6 @@ extern "C" cloak_status cloak_load_tensors(uint64_t key, const cloak_block_shape
             default: st = rows(x.src, dst, nullptr, 1, x.N, row_bytes, sms, s); break;
         }
         if (st != CLOAK_OK) return st;
-        if (x.src != x0.src) {
-            CLOAK_CUDA(cudaEventRecord(freed[nstaged & 1], s));
-            ++nstaged;
-        }
         const uint64_t end = x.off + (uint64_t)x.N * x.K * e;
         if (end % pool->block) {
             zero_block_tail_kernel<<<1, 256, 0, s>>>(pool->base, pool->d_T, end, pool->log2_block);
@@ -760,12 +714,6 @@ extern "C" cloak_status cloak_load_tensors(uint64_t key, const cloak_block_shape
             CLOAK_LAUNCH_CHECK();
         }
     }
-    return CLOAK_OK;
-}
-
-extern "C" cloak_status cloak_set_load_engine(int engine) {
-    if (engine < 0 || engine > 1) return fail(CLOAK_ERR_INVALID, "set_load_engine: 0 (automatic) or 1 (host sources always read in place)");
-    g_load_engine.store(engine);
     return CLOAK_OK;
 }
 
