@@ -545,9 +545,12 @@ def test_load_tensors_one_pass_from_host_or_device(layout, where, dtype, block):
         C.cloak_load_tensors(key, sh, p.h, items[::-1], C.CLOAK_TILE128 if layout == "tile128" else C.CLOAK_ROWMAJOR)   # any listing order
         torch.cuda.synchronize()
         assert np.array_equal(p.raw(), ref)
-        # argument checks: overlap, bad role, unaligned offset
+        # argument checks: overlap, bad role, unaligned offset, a pageable host source (the kernels could not read it)
+        pageable = np.zeros(I * H * e + 64, np.uint8)
+        pageable = pageable[(-pageable.ctypes.data) % 64:]
         for bad, st in (([items[0], items[0]], C.CLOAK_ERR_INVALID), ([(items[0][0], offs[0], 0, 9)], C.CLOAK_ERR_INVALID),
-                        ([(items[0][0], offs[0] + 16, 0, "gate")], C.CLOAK_ERR_ALIGN)):
+                        ([(items[0][0], offs[0] + 16, 0, "gate")], C.CLOAK_ERR_ALIGN),
+                        ([(pageable, offs[names.index((0, "gate", (I, H)))], 0, "gate")], C.CLOAK_ERR_INVALID)):
             with pytest.raises(C.CloakError) as ei:
                 C.cloak_load_tensors(key, sh, p.h, bad)
             assert ei.value.status == st
