@@ -594,7 +594,7 @@ def main():
     ap.add_argument("--sm-weighting", type=int, default=0, help="A/B: cloak_set_sm_weighting (1 measured per-SM shares, 0 equal shares)")
     ap.add_argument("--copy-hint", type=int, default=-1, help="A/B: cloak_set_copy_cache_hint (bit 0 stores, bit 1 loads evict_first)")
     ap.add_argument("--gemv-engine", type=int, default=0,
-                    help="A/B: cloak_set_gemv_engine (0 auto, 1 one-shot kernel, 2 no PDL)")
+                    help="A/B: cloak_set_gemv_engine (0 auto, 1 one-shot kernel, 2 no PDL, 3 exclusive mode)")
     args = ap.parse_args()
     if args.workload != "cfg1":
         from paper_2606_18400_b200 import workloads

@@ -390,7 +390,10 @@ cloak_status cloak_gemm_chain(const cloak_pool* pool, const cloak_gemm_op* h_ops
                               void* stream);
 /* Selects the bf16 GEMV kernel: 0 = automatic (streaming TMA kernel when K % 256 == 0, launched with
  * programmatic dependent launch), 1 = always the one-shot split-K kernel, 2 = automatic without
- * programmatic dependent launch.  For A/B measurement; process-wide (an atomic: safe to flip from any thread, takes effect
+ * programmatic dependent launch, 3 = automatic in EXCLUSIVE mode: the caller vouches that no other kernel holds SMs while a
+ * chain runs (one stream, nothing else on the device), and chains with `after` ops are then ordinary launches too, which
+ * keeps programmatic dependent launch across their launch boundaries (a multi-launch chain is several per cent faster); with
+ * a foreign kernel on the device such a chain can hang.  For A/B measurement; process-wide (an atomic: safe to flip from any thread, takes effect
  * at the next launch). */
 cloak_status cloak_set_gemv_engine(int engine);
 /* Per-SM streaming weights (calibrate.cu).  The SMs of a B200 do not pull a read stream out of HBM equally fast (three tiers,

@@ -472,12 +472,13 @@ constexpr uint32_t GS_TILE_COUNTERS = (uint32_t)(WS_COUNTER_BYTES / 4) - 4 * GS_
 // Whether the cooperative attribute may be combined with programmatic stream serialization is probed on the first such launch:
 // if the driver rejects the pair, PDL is dropped, not the guarantee.
 std::atomic<unsigned long long*> g_trace{nullptr};     // cloak_set_trace
+std::atomic<bool> g_gemv_exclusive{false};             // cloak_set_gemv_engine(3): the caller vouches that nothing else holds SMs
 static std::atomic<int> g_coop_with_pdl{-1};     // -1 unknown, 0 rejected, 1 accepted
 int gemv_coop_pdl_state() { return g_coop_with_pdl.load(std::memory_order_relaxed); }
 
 template <int CU, int NT>
 static cloak_status launch(const ChainArgs& a, int ctas, int device, cudaStream_t s) {
-    const bool coop = a.any_signal != 0;
+    const bool coop = a.any_signal != 0 && !g_gemv_exclusive.load(std::memory_order_relaxed);
     constexpr size_t smem = (size_t)gs_stages(CU) * GS_ROWS * (CU * 512u + GS_PAD);
     static std::atomic<uint64_t> opted{0};
     auto* kernel = gemv_chain_kernel<CU, NT>;

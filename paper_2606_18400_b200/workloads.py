@@ -1012,7 +1012,7 @@ def main(argv=None):
     ap.add_argument("--layers", type=int, default=0, help="cfg3: number of layers (default 64); moe: default 12 of 48")
     ap.add_argument("--batches", default="", help="cfg3: batch sizes, e.g. 16,64,256 (default 32,128)")
     ap.add_argument("--gemm-schedule", default="", help="cfg3: static_pct,dyn_chunk_tiles (cloak_set_gemm_schedule), e.g. 100,0")
-    ap.add_argument("--gemv-engine", type=int, default=0, help="cloak_set_gemv_engine: 0 auto, 1 one-shot, 2 no PDL")
+    ap.add_argument("--gemv-engine", type=int, default=0, help="cloak_set_gemv_engine: 0 auto, 1 one-shot, 2 no PDL, 3 exclusive mode (no cooperative launches)")
     ap.add_argument("--sm-weighting", type=int, default=-1, help="cloak_set_sm_weighting (1 = per-SM weighted shares in the streaming GEMV)")
     ap.add_argument("--out", default="")
     args = ap.parse_args(argv)
