@@ -591,7 +591,6 @@ def main():
                          "`--configs cfg1` for the step alone.  N > 1 replicas run the step alone.")
     ap.add_argument("--min-seconds", type=float, default=1.0, help="minimum length of each timed loop of the cfg2-4 blocks")
     ap.add_argument("--no-ab", action="store_true", help="skip the isolated native / per-call / cuBLAS A/B runs and the e2e leg (for ncu launch lists of the step alone)")
-    ap.add_argument("--sm-weighting", type=int, default=0, help="A/B: cloak_set_sm_weighting (1 measured per-SM shares, 0 equal shares)")
     ap.add_argument("--copy-hint", type=int, default=-1, help="A/B: cloak_set_copy_cache_hint (bit 0 stores, bit 1 loads evict_first)")
     ap.add_argument("--gemv-engine", type=int, default=0,
                     help="A/B: cloak_set_gemv_engine (0 auto, 1 one-shot kernel, 2 no PDL, 3 exclusive mode)")
@@ -603,7 +602,6 @@ def main():
         import paper_2606_18400_b200 as C
         if args.gemv_engine:
             C.cloak_set_gemv_engine(args.gemv_engine)
-        C.cloak_set_sm_weighting(args.sm_weighting)
         if args.copy_hint >= 0:
             C.cloak_set_copy_cache_hint(args.copy_hint)
     args.warmup = max(args.warmup, 3) if args.impl == "cloak" else args.warmup

@@ -391,22 +391,18 @@ cloak_status cloak_gemm_chain(const cloak_pool* pool, const cloak_gemm_op* h_ops
 /* Selects the bf16 GEMV kernel: 0 = automatic (streaming TMA kernel when K % 256 == 0, launched with
  * programmatic dependent launch), 1 = always the one-shot split-K kernel, 2 = automatic without
  * programmatic dependent launch, 3 = automatic in EXCLUSIVE mode: the caller vouches that no other kernel holds SMs while a
- * chain runs (one stream, nothing else on the device), and chains with `after` ops are then ordinary launches too, which
- * keeps programmatic dependent launch across their launch boundaries (a multi-launch chain is several per cent faster); with
+ * chain runs (one stream, nothing else on the device), and chains with `after` ops are then ordinary launches too (measured:
+ * no faster -- cfg2's chain 2.592 vs 2.596 ms, a 25-launch MoE chain 0.4623 vs 0.4623 ms -- so there is no reason to use it); with
  * a foreign kernel on the device such a chain can hang.  For A/B measurement; process-wide (an atomic: safe to flip from any thread, takes effect
  * at the next launch). */
 cloak_status cloak_set_gemv_engine(int engine);
-/* Per-SM streaming weights (calibrate.cu).  The SMs of a B200 do not pull a read stream out of HBM equally fast (three tiers,
- * up to 1.7 x apart, a property of the individual part); the first cloak_pool_create on a device measures it once (a 1 GiB
- * scratch buffer, a few ms), and the streaming GEMV CAN cut large ops into static shares proportional to it instead of equal
- * ones (the split is then fixed for the life of the process: results stay deterministic, and the same on cloaked and
- * identity-table pools).  Measured: the GEMV's SMs are limited by their own ring, not by the contended path, and equal shares
- * already end together; weighted shares are 7 % slower.  So the switch is OFF by default and kept for A/B measurement.
- * cloak_sm_weights: the relative speeds (mean 1) of the device's SMs, indexed by SM id; *h_nsm = 0 if they could not be
- * measured (kernels then use equal shares).  h_weights may be NULL to query the count.  Measures if that has not happened yet.
- * cloak_set_sm_weighting: 0 = equal shares (default), 1 = measured weights.  Process-wide. */
+/* Per-SM streaming weights (calibrate.cu): a MEASUREMENT, used by no kernel.  The SMs of a B200 do not pull a read stream out of
+ * HBM equally fast (three tiers, up to 1.7 x apart under a dynamic queue, a property of the individual part).  Round 2 cut the
+ * streaming GEMV's ops into shares proportional to these weights: 7 % slower (its SMs are limited by their own rings, not by the
+ * contended path; equal shares already end together), and the switch alone cost small-op chains 12 %, so it was removed again.
+ * cloak_sm_weights: the relative speeds (mean 1) of the device's SMs, indexed by SM id, measured on first use (a 1 GiB scratch
+ * buffer, a few ms; synchronises the device); *h_nsm = 0 if they could not be measured.  h_weights may be NULL to query the count. */
 cloak_status cloak_sm_weights(int device, uint32_t capacity, float* h_weights, uint32_t* h_nsm);
-cloak_status cloak_set_sm_weighting(int mode);
 /* Tracing: while d_trace is not NULL, every streaming-GEMV launch records, per CTA b, four 64-bit words at d_trace[4*b]: the
  * SM id, %globaltimer (ns) at CTA start, when its producer had issued its last copy, and when its consumers were done.  The
  * buffer (DEVICE memory, 8-byte aligned, room for 4 words x the device's SM count) is the caller's and is overwritten by

@@ -15,8 +15,10 @@
 // stage also being held while the consumers work through it), so with equal shares all 148 producers already end within
 // 4 us of each other (68 .. 72 us of a 75 us launch), and weighted shares make the "fast" SMs finish LAST: cfg1 layer
 // 79.9 -> 85.5 us (batch 1), 93.7 -> 101.9 us (batch 16).  A pure read stream of large pieces, which does saturate the path,
-// gains 6 % from a dynamic queue over equal shares (58.9 vs 62.4 us for 436 MB).  So the measurement and the weighted split
-// stay in the library as an A/B switch, OFF by default (cloak_set_sm_weighting).
+// gains 6 % from a dynamic queue over equal shares (58.9 vs 62.4 us for 436 MB).  The weighted split was then taken OUT of the
+// GEMV kernel again: merely carrying the switch (a flag test, a table load and 64-bit range arithmetic per op in producer and
+// consumers) cost cfg2's decode chain 2 % and a 12-layer MoE chain of 348 small ops 12 % (0.462 -> 0.526 ms).  What stays is the
+// measurement itself, as a report: cloak_sm_weights.
 //
 // How.  One CTA per SM (192 KiB of shared memory each) draws 32 KiB chunks of a scratch buffer from an atomic counter and
 // pulls them with cp.async.bulk through a 6-stage ring; chunks drawn per %smid over two measured passes = the weight.
@@ -75,7 +77,6 @@ struct SmWeights {
 };
 static SmWeights g_smw[64];
 static std::mutex g_smw_mu;
-static std::atomic<int> g_weighting{0};      // cloak_set_sm_weighting; off by default (see the note at the top)
 
 static void measure(int device, SmWeights& out) {
     out.state.store(-1);
@@ -136,29 +137,14 @@ static void measure(int device, SmWeights& out) {
     out.state.store(1, std::memory_order_release);
 }
 
-// Measured at most once per device and process; call with the device current, outside stream capture (pool_create does).
-void ensure_sm_weights(int device, bool only_if_enabled) {
+// Measured at most once per device and process; call with the device current, outside stream capture.
+static void ensure_sm_weights(int device) {
     if (device < 0 || device >= 64) return;
-    if (only_if_enabled && !g_weighting.load(std::memory_order_relaxed)) return;
     std::lock_guard<std::mutex> lock(g_smw_mu);
     if (g_smw[device].state.load() == 0) measure(device, g_smw[device]);
 }
 
-// The cumulative table for kernels that run exactly one CTA on each of the device's `nsm` SMs, or nullptr (not measured,
-// unusable, switched off): then shares are equal.
-const uint32_t* sm_cum_table(int device, uint32_t nsm) {
-    if (device < 0 || device >= 64 || !g_weighting.load(std::memory_order_relaxed)) return nullptr;
-    const SmWeights& w = g_smw[device];
-    return (w.state.load(std::memory_order_acquire) == 1 && w.nsm == nsm) ? w.d_cum : nullptr;
-}
-
 }  // namespace cloak
-
-extern "C" cloak_status cloak_set_sm_weighting(int mode) {
-    if (mode < 0 || mode > 1) return cloak::fail(CLOAK_ERR_INVALID, "set_sm_weighting: 0 (equal shares) or 1 (measured per-SM weights)");
-    cloak::g_weighting.store(mode);
-    return CLOAK_OK;
-}
 
 extern "C" cloak_status cloak_sm_weights(int device, uint32_t capacity, float* h_weights, uint32_t* h_nsm) {
     using namespace cloak;
@@ -166,7 +152,7 @@ extern "C" cloak_status cloak_sm_weights(int device, uint32_t capacity, float* h
     {
         DeviceGuard g(device);
         if (!g.ok) return fail(CLOAK_ERR_CUDA, "sm_weights: cannot select device %d", device);
-        ensure_sm_weights(device, false);
+        ensure_sm_weights(device);
     }
     const SmWeights& w = g_smw[device];
     if (w.state.load() != 1) {

@@ -120,10 +120,6 @@ cloak_status pool_workspace(const cloak_pool* pool, size_t bytes, cudaStream_t s
 int gemv_stream_chunk(const cloak_pool* pool, const cloak_tensor* w, uint32_t batch);
 cloak_status gemv_stream_launch(const cloak_pool* pool, const cloak_gemv_op* ops, uint32_t n, int cu, uint32_t batch,
                                 cudaStream_t s);
-// calibrate.cu: per-SM streaming weights of a device (measured once, at the first pool_create on it) and the cumulative
-// table cum[0 .. nsm] (16-bit fixed point, indexed by %smid) for kernels that run one CTA on every SM; nullptr = equal shares.
-void ensure_sm_weights(int device, bool only_if_enabled);
-const uint32_t* sm_cum_table(int device, uint32_t nsm);
 // pool.cu: (re)build the authorised table T from blockinv, the page map and the page halves, on stream s.
 cloak_status launch_build_table(const cloak_pool* p, cudaStream_t s);
 // rekey_pages.cu: drop an unfinished page re-key of a pool that is being destroyed (unmaps what it had mapped).

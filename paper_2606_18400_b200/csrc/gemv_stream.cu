@@ -51,15 +51,13 @@ struct ChainOp {             // 80 bytes of kernel parameter space per op (10 x 
     uint32_t per;            // units per CTA
     uint32_t ctas;           // CTAs that own units of this op (indices 0 .. ctas-1)
     uint32_t tile_base;      // index of this op's first row-tile counter
-    uint32_t flags;          // OP_SIGNAL | OP_WEIGHTED
+    uint32_t flags;          // OP_SIGNAL
     uint32_t wait_op;        // NO_WAIT, or the index of the op whose completion by ALL CTAs this op's consumers wait for
     uint32_t rot;            // range r of this op belongs to CTA (r + rot) % grid: an op with fewer ranges than CTAs starts
                              // where the previous one stopped, so the idle CTAs are different ones each time (an op with a
                              // gate epilogue keeps the rotation of the op that produced the gate: same rows, same CTA)
 };
-enum { OP_SIGNAL = 2,        // some later op waits for this one: every CTA reports here when it is done with it (and all before)
-       OP_WEIGHTED = 4 };    // the op's ranges are proportional to the SMs' measured streaming speeds: range index = %smid, bounds
-                             // from ChainArgs::cum (calibrate.cu); otherwise equal ranges of `per` units, range index from blockIdx
+enum { OP_SIGNAL = 2 };      // some later op waits for this one: every CTA reports here when it is done with it (and all before)
 constexpr uint32_t NO_WAIT = 0xffffffffu;
 constexpr int GS_MAX_OPS = 48;              // 48 x 80 B + header < 4 KiB of kernel parameters
 
@@ -69,7 +67,6 @@ struct ChainArgs {
     float* part;             // [op][cta][batch * 8]: partial of the cut row tile a CTA meets first in that op
     uint32_t* counters;      // [tile_base + tile]: arrivals of the non-owning contributors; owner resets to 0
     uint32_t* opsync;        // [GS_MAX_OPS] arrivals per signalling op, [GS_MAX_OPS] CTAs done with the launch: the last resets all
-    const uint32_t* cum;     // per-SM cumulative weights, [gridDim.x + 1], 16-bit fixed point (cum[gridDim.x] = 65536); NULL = none
     unsigned long long* trace;   // NULL, or [gridDim.x][4]: %smid, globaltimer at CTA start, producer done, consumers done
     uint32_t log2b;
     uint32_t batch;
@@ -144,15 +141,6 @@ __device__ __forceinline__ unsigned long long global_ns() {
     asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t));
     return t;
 }
-// This CTA's range index of an op and the units [ubeg, uend) it owns.
-__device__ __forceinline__ uint32_t op_rank(const ChainOp& op, uint32_t smid) {
-    return (op.flags & OP_WEIGHTED) ? smid : (blockIdx.x + gridDim.x - op.rot) % gridDim.x;
-}
-__device__ __forceinline__ uint32_t range_begin(const uint32_t* cum, const ChainOp& op, uint32_t r) {
-    if (op.flags & OP_WEIGHTED) return (uint32_t)(((uint64_t)op.units * __ldg(cum + r)) >> 16);
-    const uint64_t b = (uint64_t)r * op.per;
-    return b < op.units ? (uint32_t)b : op.units;
-}
 __device__ __forceinline__ void consumer_bar() { asm volatile("bar.sync 1, %0;" :: "n"(GS_CONSUMERS * 32) : "memory"); }
 
 // silu(g) * u for bf16 inputs, fp32 arithmetic, round to nearest even: bit for bit cloak_silu_mul's result.
@@ -207,12 +195,11 @@ __global__ void __launch_bounds__(gs_threads(NT), 1) gemv_chain_kernel(const __g
         if (!a.early) grid_dep_wait();
         uint32_t s = 0, ph = 0;
         bool wrapped = false;
-        const uint32_t smid = my_smid();
         for (uint32_t j = 0; j < a.nops; ++j) {
             const ChainOp& op = a.ops[j];
             const uint32_t kch = op.kch;
-            const uint32_t vr = op_rank(op, smid);                                   // this CTA's range of the op
-            const uint32_t ubeg = range_begin(a.cum, op, vr), uend = range_begin(a.cum, op, vr + 1);
+            const uint32_t vr = (blockIdx.x + gridDim.x - op.rot) % gridDim.x;   // this CTA's range of the op
+            const uint32_t ubeg = vr * op.per, uend = min(ubeg + op.per, op.units);
             if (ubeg >= uend) continue;
             const uint32_t tile_lo = ubeg / kch, tile_hi = (uend - 1) / kch;
             const uint64_t row_bytes = (uint64_t)op.K * 2;
@@ -271,12 +258,11 @@ __global__ void __launch_bounds__(gs_threads(NT), 1) gemv_chain_kernel(const __g
     if (ctid == 0) grid_dep_launch();
 
     uint32_t s = 0, ph = 0;
-    const uint32_t smid = my_smid();
     for (uint32_t j = 0; j < a.nops; ++j) {
         const ChainOp& op = a.ops[j];
-        const uint32_t kch = op.kch;
-        const uint32_t vr = op_rank(op, smid);                                       // this CTA's range of the op
-        const uint32_t ubeg = range_begin(a.cum, op, vr), uend = range_begin(a.cum, op, vr + 1);
+        const uint32_t kch = op.kch, per = op.per;
+        const uint32_t vr = (blockIdx.x + gridDim.x - op.rot) % gridDim.x;       // this CTA's range of the op
+        const uint32_t ubeg = vr * per, uend = min(ubeg + per, op.units);
         const bool have = ubeg < uend;
 
         if (have && op.wait_op != NO_WAIT) {
@@ -407,11 +393,7 @@ __global__ void __launch_bounds__(gs_threads(NT), 1) gemv_chain_kernel(const __g
 
             if (cut_tail) {
                 // owner of the tail tile: wait for the other contributors (CTAs after this one), add in CTA order
-                // the later ranges that begin inside the tile (none of them empty: the host makes sure of that)
-                uint32_t nc = 0;
-                for (uint32_t q = vr + 1; q < gridDim.x && range_begin(a.cum, op, q) <= tile_hi * kch + kch - 1 &&
-                                          range_begin(a.cum, op, q) < op.units; ++q)
-                    ++nc;
+                const uint32_t nc = (tile_hi * kch + kch - 1) / per - vr;
                 uint32_t* cnt = a.counters + op.tile_base + tile_hi;
                 if (ctid == 0) {
                     while (ld_acquire(cnt) != nc) __nanosleep(32);
@@ -437,7 +419,7 @@ __global__ void __launch_bounds__(gs_threads(NT), 1) gemv_chain_kernel(const __g
         }
     }
     if (a.trace && ctid == 0) {
-        a.trace[4 * blockIdx.x + 0] = smid;
+        a.trace[4 * blockIdx.x + 0] = my_smid();
         a.trace[4 * blockIdx.x + 1] = t_start;
         a.trace[4 * blockIdx.x + 3] = global_ns();
     }
@@ -460,15 +442,14 @@ constexpr uint32_t GS_TILE_COUNTERS = (uint32_t)(WS_COUNTER_BYTES / 4) - 4 * GS_
 //       SM to run on -- another kernel holds SMs: a second pool's chain on another stream, a framework kernel, an MPS / green-
 //       context SM limit -- the resident ones spin for ever.  A launch that contains such an op is therefore COOPERATIVE: the
 //       driver starts the grid only when every CTA can be resident (one per SM; the grid is never larger than the SM count) and
-//       fails the launch (cudaErrorCooperativeLaunchTooLarge) instead of hanging when that can never be.  The price: a
-//       cooperative grid cannot begin while its stream predecessor still holds SMs, so programmatic dependent launch gains
-//       nothing between such launches (cfg2's 5-launch decode chain +1.4 %; a 12-layer MoE chain of ~25 launches +19 %).
+//       fails the launch (cudaErrorCooperativeLaunchTooLarge) instead of hanging when that can never be.  Measured cost of
+//       the attribute: none (cloak_set_gemv_engine(3) launches such chains as ordinary grids: cfg2's chain 2.592 vs 2.596 ms,
+//       a 25-launch MoE chain 0.4623 vs 0.4623 ms).
 //   (2) The owner of a cut row tile waits for the partials of the FEW CTAs that follow it in range order, which publish them at
 //       the START of their ranges and wait for nobody first.  CTAs are dispatched in index order, so whatever subset is
 //       resident, the waits form a chain that ends at a CTA that is running or done: progress without full residency (the
 //       dispatch order is how every NVIDIA GPU behaves, not an architectural promise -- cloak.h says so).  Launches with only
-//       this kind of wait (cloak_gemv, chains of independent ops) stay ordinary launches and keep programmatic dependent
-//       launch, which hides ~1 us per launch boundary (cfg1 layer as 7 calls: 92.5 us against 99.7 us cooperative).
+//       this kind of wait (cloak_gemv, chains of independent ops) stay ordinary launches.
 // Whether the cooperative attribute may be combined with programmatic stream serialization is probed on the first such launch:
 // if the driver rejects the pair, PDL is dropped, not the guarantee.
 std::atomic<unsigned long long*> g_trace{nullptr};     // cloak_set_trace
@@ -590,14 +571,6 @@ cloak_status gemv_stream_launch(const cloak_pool* pool, const cloak_gemv_op* ops
             if (o.gate && (const void*)a.ops[k].y == (const void*)o.gate) o.rot = a.ops[k].rot;     // same rows, same CTA
         ranges_so_far += o.ctas;
     }
-    // Shares proportional to the SMs' measured streaming speeds (calibrate.cu), for ops large enough that every share is
-    // many units, in launches that put one CTA on every SM and do not rotate: such an op ends on all SMs at once instead of
-    // when the slowest tier of SMs is done (the others' producers then run ahead into the next op, but at every `after` the
-    // whole grid waits for the last).  Shape alone decides, so gate and up of one MLP get the same split.
-    a.cum = (!rotate_all && ctas == sms) ? sm_cum_table(pool->device, (uint32_t)sms) : nullptr;
-    if (a.cum)
-        for (uint32_t j = 0; j < n; ++j)
-            if (a.ops[j].rot == 0 && a.ops[j].units >= 16u * (uint32_t)ctas) a.ops[j].flags |= OP_WEIGHTED;
     a.trace = g_trace.load(std::memory_order_relaxed);
     const size_t need = WS_COUNTER_BYTES + (size_t)n * ctas * batch * GS_ROWS * 4;
     cloak_status st = pool_workspace(pool, need, s);

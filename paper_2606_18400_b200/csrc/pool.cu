@@ -177,7 +177,6 @@ static cloak_status create_impl(cloak_pool* p) {
     p->d_pageoff = p->d_pageinv + p->npages;
     p->d_T = p->d_pageoff + p->npages;
 
-    ensure_sm_weights(p->device, true);    // once per device, if cloak_set_sm_weighting(1): the GEMV's shares follow the SMs' measured speeds
     cudaStream_t s;
     CLOAK_CUDA(cudaStreamCreateWithFlags(&s, cudaStreamNonBlocking));
     cloak_status st = CLOAK_OK;

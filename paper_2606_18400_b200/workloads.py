@@ -1013,13 +1013,10 @@ def main(argv=None):
     ap.add_argument("--batches", default="", help="cfg3: batch sizes, e.g. 16,64,256 (default 32,128)")
     ap.add_argument("--gemm-schedule", default="", help="cfg3: static_pct,dyn_chunk_tiles (cloak_set_gemm_schedule), e.g. 100,0")
     ap.add_argument("--gemv-engine", type=int, default=0, help="cloak_set_gemv_engine: 0 auto, 1 one-shot, 2 no PDL, 3 exclusive mode (no cooperative launches)")
-    ap.add_argument("--sm-weighting", type=int, default=-1, help="cloak_set_sm_weighting (1 = per-SM weighted shares in the streaming GEMV)")
     ap.add_argument("--out", default="")
     args = ap.parse_args(argv)
     if args.gemv_engine:
         _imports()[1].cloak_set_gemv_engine(args.gemv_engine)
-    if args.sm_weighting >= 0:
-        _imports()[1].cloak_set_sm_weighting(args.sm_weighting)
     if args.gemm_schedule:
         _imports()[1].cloak_set_gemm_schedule(*[int(v) for v in args.gemm_schedule.split(",")])
     line = json.dumps(RUNNERS[args.workload](args))

@@ -60,7 +60,6 @@ def test_argument_checks_without_a_device(C):
         (lambda: C.cloak_pool_layout_report(None), C.CLOAK_ERR_INVALID),
         (lambda: C.cloak_pool_adjacency(None), C.CLOAK_ERR_INVALID),
         (lambda: C.cloak_pool_map_phases(None), C.CLOAK_ERR_INVALID),
-        (lambda: C.cloak_set_sm_weighting(7), C.CLOAK_ERR_INVALID),
         (lambda: C.cloak_set_copy_cache_hint(4), C.CLOAK_ERR_INVALID),
         (lambda: C.cloak_set_gather_engine(2), C.CLOAK_ERR_INVALID),
         (lambda: C.cloak_set_trace(12), C.CLOAK_ERR_ALIGN),
@@ -77,7 +76,6 @@ def test_argument_checks_without_a_device(C):
 
 def test_runtime_info_and_knobs_are_callable_without_a_device(C):
     assert "gemv_chain" in C.cloak_runtime_info()
-    C.cloak_set_sm_weighting(0)
     C.cloak_set_copy_cache_hint(0)
     C.cloak_set_gather_engine(0)
     C.cloak_set_trace(None)
