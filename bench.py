@@ -554,7 +554,7 @@ def run_cloak(args):
         line["gpu_launches_other_configs"] = int(sum(line[k]["gpu_launches"] for k in ("cfg2", "cfg3", "cfg4") if k in line))
     if clocks is not None:
         clocks.stop()
-    if not args.no_cpu_baseline:
+    if not args.no_cpu_baseline and world == 1:      # (the oracle is timed on rank 0 at N = 1 only)
         # the oracle beside it: the WHOLE cfg1 layer through the same stages, bounded by repetitions, once with
         # numpy's BLAS on all cores and once limited to one thread
         dt, reps, used, sbo = oracle_time(ORACLE_LAYER, 3, 12.0)
