@@ -27,7 +27,7 @@ SYMBOLS = ["cloak_last_error", "cloak_version", "cloak_runtime_info", "cloak_lau
            "cloak_unshuffle", "cloak_shuffle_many", "cloak_unshuffle_many", "cloak_relayout", "cloak_rekey_inplace", "cloak_rekey_pages_begin", "cloak_rekey_pages_step", "cloak_rekey_pages_finish", "cloak_shuffle_host", "cloak_unshuffle_host",
            "cloak_set_copy_engine", "cloak_set_copy_cache_hint", "cloak_set_gather_engine", "cloak_arena_plan", "cloak_permute_mlp_heads", "cloak_permute_experts", "cloak_load_mlp_heads", "cloak_load_tensors", "cloak_to_tile128",
            "cloak_gemv", "cloak_gemv_chain", "cloak_gemm", "cloak_gemm_chain", "cloak_gemv_chain_scratch_bytes",
-           "cloak_gemm_chain_scratch_bytes", "cloak_pool_reserve_workspace", "cloak_set_gemv_engine", "cloak_sm_weights", "cloak_set_trace", "cloak_set_gemm_schedule", "cloak_gemm_plan", "cloak_gemv_host", "cloak_gemv_chain_host", "cloak_silu_mul"]
+           "cloak_gemm_chain_scratch_bytes", "cloak_pool_reserve_workspace", "cloak_set_gemv_engine", "cloak_sm_weights", "cloak_set_trace", "cloak_set_gemm_schedule", "cloak_set_gemm_engine", "cloak_gemm_plan", "cloak_gemv_host", "cloak_gemv_chain_host", "cloak_silu_mul"]
 
 
 class CloakError(RuntimeError):
@@ -113,6 +113,7 @@ lib.cloak_set_gemv_engine.argtypes = [c_int]
 lib.cloak_sm_weights.argtypes = [c_int, c_uint32, _P, POINTER(c_uint32)]
 lib.cloak_set_trace.argtypes = [_P]
 lib.cloak_set_gemm_schedule.argtypes = [c_int, c_int]
+lib.cloak_set_gemm_engine.argtypes = [c_int]
 lib.cloak_gemm_plan.argtypes = [c_uint32, POINTER(c_uint32), POINTER(c_uint32), c_uint32, c_uint32, c_uint32,
                                 POINTER(c_uint32), POINTER(c_uint32), POINTER(c_uint32), POINTER(c_uint32)]
 lib.cloak_arena_plan.argtypes = [c_uint64, c_uint32, POINTER(c_uint64), c_uint32, POINTER(c_uint64), POINTER(c_uint64)]
@@ -333,6 +334,10 @@ def cloak_set_trace(d_trace):
 
 def cloak_set_gemm_schedule(static_pct, dyn_chunk_tiles=0):
     _check(lib.cloak_set_gemm_schedule(static_pct, dyn_chunk_tiles))
+
+
+def cloak_set_gemm_engine(engine):
+    _check(lib.cloak_set_gemm_engine(engine))
 
 
 def cloak_gemm_plan(shapes, batch, sms=148):

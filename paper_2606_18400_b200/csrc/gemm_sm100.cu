@@ -48,7 +48,7 @@ struct GemmOp {
     uint32_t pieces;     // dynamic part: chunks per tile row, each plen tiles (the last one the rest)
     uint32_t plen;
     uint32_t cbase;      // dynamic part: number of the chunk (dyn_row0, piece 0)
-    uint32_t pad_;
+    uint32_t n_real;     // N of the matrix (row stride of Y); == N unless the launch groups rows
 };
 
 struct GemmArgs {
@@ -70,6 +70,11 @@ struct GemmArgs {
     uint32_t xstages;    // ring of X tiles [batch x 128] (L2 latency: shallow)
     uint32_t tmem_cols;  // power of two >= 2*batch
     uint32_t early;      // 1: W unchanged since before the preceding kernel -> stream it ahead of griddepcontrol.wait
+    uint32_t nacc;       // ROW GROUPS: 1, 2 or 4 tile rows share each X tile.  A unit is then the nacc tiles (nacc*p + rr, tk), rr < nacc, of a
+                         // GROUP p of tile rows: the X tile comes out of L2 once instead of nacc times (at batch 128 the X traffic equals
+                         // the weight traffic and is worth 12-15 % of the kernel).  ops[].N / units / row_base /
+                         // dyn_row0 ... then count GROUPS (the plan ran on N / nacc), ops[].n_real is the matrix's N; nacc accumulators
+                         // per segment, double-buffered: 2 * nacc * batch <= 512 TMEM columns.
     GemmOp ops[GM_MAX_OPS];
     alignas(64) CUtensorMap map_x[GM_MAX_OPS];   // X of op j as a 2-D map [batch, K], boxes of [batch x 64]
 };
@@ -207,18 +212,22 @@ __global__ void __launch_bounds__(GM_THREADS, 1) gemm_tile128_kernel(const __gri
                 const GemmOp& op = a.ops[j];
                 if (op.ubase + op.units <= gbeg || op.ubase >= gend) continue;     // this chunk's part of the op, in op units
                 const uint32_t ubeg = max(gbeg, op.ubase) - op.ubase, uend = min(gend, op.ubase + op.units) - op.ubase;
-                for (uint32_t u = ubeg; u < uend; ++u, ++it) {
-                    const uint32_t s = it % a.wstages, f = it / a.wstages;
-                    if (f > 0) mbar_wait(smem_u32(&wempty[s]), (f - 1) & 1);
-                    const uint64_t off = op.w_offset + (uint64_t)u * 32768;          // tile index == unit index
-                    const uint32_t slot = __ldg(a.T + (off >> a.log2b));
-                    const uint64_t byte = ((uint64_t)slot << a.log2b) + (off & ((1ull << a.log2b) - 1));
-                    const uint32_t row = (uint32_t)(byte >> 8);                      // pool viewed as rows of 256 B
-                    const uint32_t st = smem_base + s * 32768;
-                    const uint32_t bar = smem_u32(&wfull[s]);
-                    mbar_expect_tx(bar, 32768);
-                    tma_load_2d(st, &map_w, 0, row, bar);
-                    tma_load_2d(st + 16384, &map_w, 64, row, bar);
+                for (uint32_t u = ubeg; u < uend; ++u) {
+                    for (uint32_t rr = 0; rr < a.nacc; ++rr, ++it) {
+                        const uint32_t s = it % a.wstages, f = it / a.wstages;
+                        if (f > 0) mbar_wait(smem_u32(&wempty[s]), (f - 1) & 1);
+                        // tile index: tile tk of row nacc * p + rr of the unit's group (nacc == 1: the unit itself)
+                        const uint32_t tile = ((u / op.kt) * a.nacc + rr) * op.kt + u % op.kt;
+                        const uint64_t off = op.w_offset + (uint64_t)tile * 32768;
+                        const uint32_t slot = __ldg(a.T + (off >> a.log2b));
+                        const uint64_t byte = ((uint64_t)slot << a.log2b) + (off & ((1ull << a.log2b) - 1));
+                        const uint32_t row = (uint32_t)(byte >> 8);                  // pool viewed as rows of 256 B
+                        const uint32_t st = smem_base + s * 32768;
+                        const uint32_t bar = smem_u32(&wfull[s]);
+                        mbar_expect_tx(bar, 32768);
+                        tma_load_2d(st, &map_w, 0, row, bar);
+                        tma_load_2d(st + 16384, &map_w, 64, row, bar);
+                    }
                 }
             }
         };
@@ -267,7 +276,8 @@ __global__ void __launch_bounds__(GM_THREADS, 1) gemm_tile128_kernel(const __gri
     } else if (warp == 1 && lane == 0) {
         // ---------------------------------------------------------------- MMA issuer
         const uint32_t idesc = (1u << 4) | (1u << 7) | (1u << 10) | ((a.batch >> 3) << 17) | ((128u >> 4) << 24);
-        uint32_t it = 0, seg = 0, cidx, gbeg, gend;                             // it, seg run on across chunks and ops
+        uint32_t it = 0, wit = 0, seg = 0, cidx, gbeg, gend;                    // it (X ring), wit (W ring), seg run on across chunks and ops
+        const uint32_t nacc = a.nacc;                                           // accumulators per segment
         auto acquire_acc = [&]() {                                              // accumulator seg & 1 drained by the epilogue?
             if (seg >= 2) {
                 mbar_wait(smem_u32(&tmem_empty[seg & 1]), ((seg >> 1) - 1) & 1);
@@ -291,22 +301,26 @@ __global__ void __launch_bounds__(GM_THREADS, 1) gemm_tile128_kernel(const __gri
                         first = true;
                         acquire_acc();
                     }
-                    const uint32_t ws = it % a.wstages, xs = it % a.xstages;
+                    const uint32_t xs = it % a.xstages;
                     mbar_wait(smem_u32(&xfull[xs]), (it / a.xstages) & 1);
-                    mbar_wait(smem_u32(&wfull[ws]), (it / a.wstages) & 1);
-                    tc_fence_after();
-                    const uint32_t st = smem_base + ws * 32768, sx = x_base + xs * xtile;
-                    const uint32_t d = tmem_base + (seg & 1) * a.batch;
+                    const uint32_t sx = x_base + xs * xtile;
+                    for (uint32_t rr = 0; rr < nacc; ++rr, ++wit) {              // the group's weight tiles against one X tile
+                        const uint32_t ws = wit % a.wstages;
+                        mbar_wait(smem_u32(&wfull[ws]), (wit / a.wstages) & 1);
+                        tc_fence_after();
+                        const uint32_t st = smem_base + ws * 32768;
+                        const uint32_t d = tmem_base + ((seg & 1) * nacc + rr) * a.batch;
 #pragma unroll
-                    for (int box = 0; box < 2; ++box) {
-                        const uint64_t ad = umma_desc_sw128(st + box * 16384);
-                        const uint64_t bd = umma_desc_sw128(sx + box * xbox);
+                        for (int box = 0; box < 2; ++box) {
+                            const uint64_t ad = umma_desc_sw128(st + box * 16384);
+                            const uint64_t bd = umma_desc_sw128(sx + box * xbox);
 #pragma unroll
-                        for (int k = 0; k < 4; ++k)                              // UMMA_K = 16 bf16 = 32 B inside the atom
-                            tc_mma_bf16(d, ad + 2 * k, bd + 2 * k, idesc, (first && box == 0 && k == 0) ? 0u : 1u);
+                            for (int k = 0; k < 4; ++k)                          // UMMA_K = 16 bf16 = 32 B inside the atom
+                                tc_mma_bf16(d, ad + 2 * k, bd + 2 * k, idesc, (first && box == 0 && k == 0) ? 0u : 1u);
+                        }
+                        tc_commit(smem_u32(&wempty[ws]));                        // frees the stage when its MMAs retire
                     }
                     first = false;
-                    tc_commit(smem_u32(&wempty[ws]));                            // frees both stages when the MMAs retire
                     tc_commit(smem_u32(&xempty[xs]));
                 }
                 tc_commit(smem_u32(&tmem_full[seg & 1]));
@@ -342,7 +356,10 @@ __global__ void __launch_bounds__(GM_THREADS, 1) gemm_tile128_kernel(const __gri
                     }
                     const uint32_t me = cidx - c_first;
                     const bool complete = ncontrib == 1;
-                    const uint32_t row = op.row_base + tn;
+                    // one accumulator per tile row of the group: rows nacc * tn + rr, same contributors, own tickets
+                    for (uint32_t rr = 0; rr < a.nacc; ++rr) {
+                    const uint32_t tnr = a.nacc * tn + rr;
+                    const uint32_t row = (op.row_base + tn) * a.nacc + rr;
                     bool last = false;
                     if (!complete) {
                         // Tickets: whoever draws the last one finishes the row.  With the static chunks that is the row's
@@ -352,10 +369,10 @@ __global__ void __launch_bounds__(GM_THREADS, 1) gemm_tile128_kernel(const __gri
                         epi_bar();
                         last = last_s != 0;
                     }
-                    mbar_wait(smem_u32(&tmem_full[seg & 1]), (seg >> 1) & 1);
+                    if (rr == 0) mbar_wait(smem_u32(&tmem_full[seg & 1]), (seg >> 1) & 1);
                     tc_fence_after();
-                    const uint32_t taddr = tmem_base + ((q * 32) << 16) + (seg & 1) * a.batch;
-                    const size_t n = (size_t)tn * 128 + r;
+                    const uint32_t taddr = tmem_base + ((q * 32) << 16) + ((seg & 1) * a.nacc + rr) * a.batch;
+                    const size_t n = (size_t)tnr * 128 + r;
                     if (last) {
                         if (etid == 0) {
                             uint32_t seen;
@@ -372,7 +389,7 @@ __global__ void __launch_bounds__(GM_THREADS, 1) gemm_tile128_kernel(const __gri
                     // partial of contributor p of this row: slot 0 of its chunk if the row ENDS there, else slot 1; a slot is
                     // [batch/4][128 rows][4] fp32, so that a thread moves its row's values of 4 batch columns as one float4
                     auto slot_of = [&](uint32_t p) {
-                        return reinterpret_cast<float4*>(a.part + ((size_t)(c_first + p) * 2 + (p == ncontrib - 1 ? 0 : 1)) * nout) + r;
+                        return reinterpret_cast<float4*>(a.part + (((size_t)(c_first + p) * 2 + (p == ncontrib - 1 ? 0 : 1)) * a.nacc + rr) * nout) + r;
                     };
                     float4* mine = slot_of(me);
                     for (uint32_t c = 0; c < a.batch; c += 32) {                 // 32 batch columns per round (16 in a last odd one)
@@ -416,12 +433,12 @@ __global__ void __launch_bounds__(GM_THREADS, 1) gemm_tile128_kernel(const __gri
                             }
 #pragma unroll
                             for (int i = 0; i < 32; ++i)
-                                if (c + i < a.nreal) op.y[(size_t)(c + i) * op.N + n] = __float2bfloat16_rn(sum[i]);
+                                if (c + i < a.nreal) op.y[(size_t)(c + i) * op.n_real + n] = __float2bfloat16_rn(sum[i]);
                         } else if (complete) {
 #pragma unroll
                             for (int i = 0; i < 16; ++i) {
-                                if (c + i < a.nreal) op.y[(size_t)(c + i) * op.N + n] = __float2bfloat16_rn(__uint_as_float(v0[i]));
-                                if (c + 16 + i < a.nreal) op.y[(size_t)(c + 16 + i) * op.N + n] = __float2bfloat16_rn(__uint_as_float(v1[i]));
+                                if (c + i < a.nreal) op.y[(size_t)(c + i) * op.n_real + n] = __float2bfloat16_rn(__uint_as_float(v0[i]));
+                                if (c + 16 + i < a.nreal) op.y[(size_t)(c + 16 + i) * op.n_real + n] = __float2bfloat16_rn(__uint_as_float(v1[i]));
                             }
                         } else {
 #pragma unroll
@@ -436,11 +453,12 @@ __global__ void __launch_bounds__(GM_THREADS, 1) gemm_tile128_kernel(const __gri
                     }
                     tc_fence_before();
                     __syncwarp();
-                    if (lane == 0) mbar_arrive(smem_u32(&tmem_empty[seg & 1]));
+                    if (lane == 0 && rr + 1 == a.nacc) mbar_arrive(smem_u32(&tmem_empty[seg & 1]));    // all accumulators drained
                     if (!complete && !last) {                                    // publish this chunk's part of the cut row
                         __threadfence();
                         epi_bar();
                         if (etid == 0) asm volatile("red.release.gpu.global.add.u32 [%0], %1;" :: "l"(a.ready + row), "r"(1u) : "memory");
+                    }
                     }
                     u = seg_last + 1;
                 }
@@ -489,6 +507,20 @@ static std::atomic<int> g_static_pct{75};
 static std::atomic<int> g_dchunk{0};
 
 constexpr uint32_t GM_MAX_ROWS = 100000;   // tile rows per launch: two counters each in the pool's counter scratch
+static std::atomic<int> g_gemm_engine{0};  // cloak_set_gemm_engine: 0 = pairs of tile rows, 1 = never, 2 = groups of four where TMEM allows
+// Measured (16 Qwen-32B-shaped layers, >= 1 s loops, of the measured copy peak): single rows 0.912 / 0.827 / 0.713 at batch 32 / 64 /
+// 128; pairs 0.987 / 0.910 / 0.799; fours (batch <= 64) 0.926 / 0.855 -- a group of four quarters the dynamic chunk and doubles
+// the rows a chunk boundary cuts, which costs more than the second halving of the X traffic returns.
+// Tile rows per group for an MMA batch (2 * nacc * batch <= 512 TMEM columns) and a list of matrices (N a multiple of 128 * nacc).
+template <typename GetN>
+static uint32_t gemm_grouping(uint32_t mma_batch, uint32_t n, GetN N) {
+    const int eng = g_gemm_engine.load(std::memory_order_relaxed);
+    uint32_t nacc = eng == 1 ? 1u : (mma_batch <= 64 && eng == 2 ? 4u : (mma_batch <= 128 ? 2u : 1u));
+    if (mma_batch < 32) nacc = 1;                   // (below that the X tile is a small fraction of the weight tile)
+    for (uint32_t j = 0; j < n; ++j)
+        while (nacc > 1 && N(j) % (128 * nacc)) nacc /= 2;
+    return nacc;
+}
 
 // The chunk grid of one launch: fills the schedule fields of a (ops[j].N/kt/units/ubase/row_base/dyn_row0/pieces/plen/cbase,
 // sper, srem, dyn_base, ndyn, total, nops) from the shapes alone.  `batch` is the MMA's N (a multiple of 16).
@@ -497,8 +529,9 @@ constexpr uint32_t GM_MAX_ROWS = 100000;   // tile rows per launch: two counters
 // part: whole tile rows (no split-K at all), or equal pieces of a row that is longer than the cap, drawn from a counter
 // as the CTAs become free.  Every piece boundary costs one partial [batch x 128] fp32 and a share of a reduction, so the
 // cap grows with the batch.
+// nacc: the launch groups tile rows -- N[] are then the matrices' N / nacc, a unit is nacc tiles and a dynamic chunk holds 1 / nacc as many.
 static cloak_status gemm_plan(GemmArgs& a, const uint32_t* N, const uint32_t* K, uint32_t n, uint32_t batch, int sms,
-                              uint32_t* ctas_out, uint64_t* rows_out) {
+                              uint32_t* ctas_out, uint64_t* rows_out, uint32_t nacc = 1) {
     uint64_t rows = 0, total = 0;
     uint32_t max_kt = 0;
     a.nops = n;
@@ -512,7 +545,7 @@ static cloak_status gemm_plan(GemmArgs& a, const uint32_t* N, const uint32_t* K,
         o.units = (uint32_t)units64;
         o.ubase = (uint32_t)total;
         o.row_base = (uint32_t)rows;
-        o.pad_ = 0;
+        o.n_real = nacc * N[j];
         total += units64;
         rows += N[j] / 128;
     }
@@ -525,6 +558,7 @@ static cloak_status gemm_plan(GemmArgs& a, const uint32_t* N, const uint32_t* K,
     const uint32_t ctas = (uint32_t)(ctas64 < 1 ? 1 : (ctas64 > (uint64_t)sms ? (uint64_t)sms : ctas64));
     const int dchunk = g_dchunk.load(std::memory_order_relaxed), static_pct = g_static_pct.load(std::memory_order_relaxed);
     uint32_t dmax = dchunk > 0 ? (uint32_t)dchunk : (batch >= 128 ? 40u : 20u);
+    if (dchunk == 0) dmax /= nacc;
     if (dmax < minper) dmax = minper;
     // A launch with less than a few dynamic chunks' worth of tiles per CTA is dealt out statically: its tail would be as
     // long as a chunk, and there is little to balance.
@@ -573,19 +607,25 @@ static cloak_status gemm_launch(const cloak_pool* pool, const cloak_gemm_op* ops
     const int sms = sm_count(pool->device);
     uint32_t Ns[GM_MAX_OPS], Ks[GM_MAX_OPS], ctas = 0;
     uint64_t rows = 0;
+    // Row groups (GemmArgs::nacc): as many tile rows per X tile as the 512 TMEM columns hold accumulators for, if every matrix
+    // of the launch has a multiple of that many tile rows.
+    const uint32_t nacc = gemm_grouping(batch, n, [&](uint32_t j) { return ops[j].w.N; });
+    a.nacc = nacc;
     for (uint32_t j = 0; j < n; ++j) {
         const cloak_tensor& w = ops[j].w;
-        Ns[j] = w.N;
+        Ns[j] = w.N / nacc;
         Ks[j] = w.K;
         st = make_map(&a.map_x[j], ops[j].d_x, w.K, nreal, (uint64_t)w.K * 2, 64, batch);
         if (st != CLOAK_OK) return st;
         a.ops[j].w_offset = w.w_offset;
         a.ops[j].y = static_cast<__nv_bfloat16*>(ops[j].d_y);
     }
-    st = gemm_plan(a, Ns, Ks, n, batch, sms, &ctas, &rows);
+    st = gemm_plan(a, Ns, Ks, n, batch, sms, &ctas, &rows, nacc);
     if (st != CLOAK_OK) return st;
+    rows *= nacc;                                    // ticket / ready counters: one per real tile row
+    if ((2 * rows + 2) * 4 > WS_COUNTER_BYTES) return fail(CLOAK_ERR_UNSUPPORTED, "gemm: too many output rows for the tile counters");
     const uint64_t nchunks = (uint64_t)ctas + a.ndyn;
-    const uint64_t part_bytes = nchunks * 2 * batch * 128 * 4;
+    const uint64_t part_bytes = nchunks * 2 * nacc * batch * 128 * 4;
     const uint32_t xtile = batch * 256;
     a.xstages = 2;
     uint32_t wst = (224u * 1024u - a.xstages * xtile) / 32768u;
@@ -593,7 +633,7 @@ static cloak_status gemm_launch(const cloak_pool* pool, const cloak_gemm_op* ops
     if (wst < 2) return fail(CLOAK_ERR_UNSUPPORTED, "gemm: batch too large for the shared-memory ring");
     a.wstages = wst;
     a.tmem_cols = 32;
-    while (a.tmem_cols < 2 * batch) a.tmem_cols <<= 1;
+    while (a.tmem_cols < 2 * nacc * batch) a.tmem_cols <<= 1;
     st = pool_workspace(pool, WS_COUNTER_BYTES + part_bytes, s);
     if (st != CLOAK_OK) return st;
     a.ticket = reinterpret_cast<uint32_t*>(pool->ws);
@@ -632,6 +672,12 @@ extern "C" cloak_status cloak_set_gemm_schedule(int static_pct, int dyn_chunk_ti
         return fail(CLOAK_ERR_INVALID, "set_gemm_schedule: static_pct in 0..100, dyn_chunk_tiles in 0..4096");
     g_static_pct.store(static_pct);
     g_dchunk.store(dyn_chunk_tiles);
+    return CLOAK_OK;
+}
+
+extern "C" cloak_status cloak_set_gemm_engine(int engine) {
+    if (engine < 0 || engine > 2) return fail(CLOAK_ERR_INVALID, "set_gemm_engine: 0 (pairs of tile rows), 1 (never) or 2 (fours where TMEM allows)");
+    g_gemm_engine.store(engine);
     return CLOAK_OK;
 }
 
@@ -693,9 +739,11 @@ extern "C" cloak_status cloak_gemm_chain_scratch_bytes(const cloak_pool* pool, c
         if (n == 0) return fail(CLOAK_ERR_UNSUPPORTED, "gemm_chain_scratch_bytes: op %u has too many output rows", i);
         GemmArgs a;
         uint32_t ctas = 0;
-        cloak_status st = gemm_plan(a, Ns, Ks, n, cols, sms, &ctas, &rows);
+        const uint32_t nacc = gemm_grouping(cols, n, [&](uint32_t j) { return Ns[j]; });
+        for (uint32_t j = 0; j < n; ++j) Ns[j] /= nacc;
+        cloak_status st = gemm_plan(a, Ns, Ks, n, cols, sms, &ctas, &rows, nacc);
         if (st != CLOAK_OK) return st;
-        const uint64_t b = WS_COUNTER_BYTES + ((uint64_t)ctas + a.ndyn) * 2 * cols * 128 * 4;
+        const uint64_t b = WS_COUNTER_BYTES + ((uint64_t)ctas + a.ndyn) * 2 * nacc * cols * 128 * 4;
         if (b > need) need = b;
         i += n;
     }

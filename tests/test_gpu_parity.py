@@ -926,6 +926,51 @@ def test_gemm_chain_equals_single_calls(batch):
             check_linear(yc[i].float().cpu().numpy(), X[shapes[i][1]], Ws[i % 5], "bf16", f"gemm_chain:b{batch}:op{i}", TOL["bf16"])
 
 
+@pytest.mark.parametrize("batch", [32, 50, 64, 128])
+def test_gemm_row_groups(batch):
+    """cloak_set_gemm_engine: tile rows in pairs (default), singly, or in fours share each X tile -- two or four accumulators
+    per segment in TMEM, units of two / four weight tiles, tickets per row.  Under each setting: every op against the fp64
+    oracle, the chain repeatable bit for bit and identical on the identity-table pool; single calls too.  Shapes with 2, 4, 6, 8
+    and 20 tile rows (6 is not a multiple of four: the launch falls back to pairs), one launch that mixes in an odd row count
+    (falls back to single rows)."""
+    key, seed, block, page = 0x1234, 13, 65536, 2 << 20
+    shapes = [(1024, 2560), (512, 1280), (256, 5120), (2560, 640), (768, 1024)]
+    Ws = [gen.synth(seed, i, shp, "bf16") for i, shp in enumerate(shapes)] + [gen.synth(seed, 9, (384, 640), "bf16")]
+    all_shapes = shapes + [(384, 640)]
+    offs, total = C.cloak_arena_plan(key, [2 * n * k for n, k in all_shapes], block)
+    try:
+        with Pool(total, block, page, key) as pc, Pool(total, block, page, key, C.CLOAK_POOL_IDENTITY) as pi:
+            for (n, k), off, Wm in zip(all_shapes, offs, Ws):
+                til = torch.empty(n * k, dtype=torch.bfloat16, device="cuda")
+                C.cloak_to_tile128(bf16_dev_from_bits(Wm), til, n, k, C.CLOAK_BF16)
+                for p in (pc, pi):
+                    C.cloak_shuffle(p.h, til, off, n * k * 2)
+            T = [C.cloak_tensor(o, n, k, C.CLOAK_BF16, C.CLOAK_TILE128) for (n, k), o in zip(all_shapes, offs)]
+            X = {k: gen.synth(seed + 50, k, (batch, k), "bf16", kind=gen.KIND_NORMAL) for k in {k for _, k in all_shapes}}
+            dX = {k: bf16_dev_from_bits(v) for k, v in X.items()}
+
+            def run(pool, idx, single=False):
+                ys = [torch.zeros(batch, all_shapes[w][0], dtype=torch.bfloat16, device="cuda") for w in idx]
+                if single:
+                    for w, y in zip(idx, ys):
+                        C.cloak_gemm(pool.h, T[w], dX[all_shapes[w][1]], y, batch)
+                else:
+                    C.cloak_gemm_chain(pool.h, [(T[w], dX[all_shapes[w][1]], y) for w, y in zip(idx, ys)], batch)
+                torch.cuda.synchronize()
+                return ys
+            for eng in (0, 1, 2):
+                C.cloak_set_gemm_engine(eng)
+                for idx in ([0, 1, 2, 3, 0, 2], [0, 1, 2, 3, 4], [0, 5, 3]):          # fours possible | pairs at most | single rows
+                    a, b, c = run(pc, idx), run(pc, idx), run(pi, idx)
+                    s1 = run(pc, idx, single=True)
+                    for j, w in enumerate(idx):
+                        assert torch.equal(a[j], b[j]) and torch.equal(a[j], c[j]), (eng, idx, j)
+                        check_linear(a[j].float().cpu().numpy(), X[all_shapes[w][1]], Ws[w], "bf16", f"gemm_groups:b{batch}:e{eng}:op{w}", TOL["bf16"])
+                        check_linear(s1[j].float().cpu().numpy(), X[all_shapes[w][1]], Ws[w], "bf16", f"gemm_groups_single:b{batch}:e{eng}:op{w}", TOL["bf16"])
+    finally:
+        C.cloak_set_gemm_engine(0)
+
+
 def test_gemm_argument_checks():
     with Pool(1 << 20, 4096, 65536, 1) as p:
         x = torch.zeros(32, 128, dtype=torch.bfloat16, device="cuda")
