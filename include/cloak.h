@@ -424,10 +424,13 @@ cloak_status cloak_gemm_plan(uint32_t n_ops, const uint32_t* h_N, const uint32_t
  * on which CTA drew which chunk.  Default (75, 0).  For A/B measurement; process-wide. */
 cloak_status cloak_set_gemm_schedule(int static_pct, int dyn_chunk_tiles);
 /* Row groups in the tcgen05 GEMM: 0 = automatic -- at an MMA batch of 32 .. 128 (the caller's batch rounded up to 16), when every
- * matrix of the launch has an even number of 128-row tile rows, a CTA works on TWO tile rows at a time, which share each X tile
- * (the X traffic out of L2 halves; two accumulator pairs in TMEM: +8-10 % at batch 32 .. 128); 1 = never; 2 = groups of four
- * rows at an MMA batch <= 64 (measured slower than pairs).  The grouping changes where K is split, so outputs under different
- * settings agree within the bf16 tolerance, not bit for bit.  For A/B measurement; process-wide. */
+ * matrix of the launch has an even number of 128-row tile rows and the launch holds at least 160 weight tiles per SM (a layer's
+ * MLP or more in one chain launch; below that the doubled split-K partials cost more than the X traffic saves, measured),
+ * a CTA works on TWO tile rows at a time, which share each X tile (the X
+ * traffic out of L2 halves; two accumulator pairs in TMEM: +8-10 % at batch 32 .. 128); 1 = never; 2 = groups of four rows at
+ * an MMA batch <= 64 (measured slower than pairs), else pairs, wherever N allows -- whatever the launch size or batch;
+ * 3 = pairs wherever N allows.  The grouping changes where K is split, so outputs under different settings agree within the bf16
+ * tolerance, not bit for bit.  2 and 3 are for A/B measurement and the tests; process-wide. */
 cloak_status cloak_set_gemm_engine(int engine);
 /* Host-buffer variant of cloak_gemv (end-to-end path): copies X up, runs, copies Y back, synchronises `stream` once (h_y is
  * the caller's to read on return).  Device staging comes from the library's cached pool: no driver allocation per call. */

@@ -507,18 +507,37 @@ static std::atomic<int> g_static_pct{75};
 static std::atomic<int> g_dchunk{0};
 
 constexpr uint32_t GM_MAX_ROWS = 100000;   // tile rows per launch: two counters each in the pool's counter scratch
-static std::atomic<int> g_gemm_engine{0};  // cloak_set_gemm_engine: 0 = pairs of tile rows, 1 = never, 2 = groups of four where TMEM allows
+static std::atomic<int> g_gemm_engine{0};  // cloak_set_gemm_engine: 0 = pairs of tile rows where they still fill the SMs, 1 = never, 2 = fours / 3 = pairs wherever N allows
 // Measured (16 Qwen-32B-shaped layers, >= 1 s loops, of the measured copy peak): single rows 0.912 / 0.827 / 0.713 at batch 32 / 64 /
 // 128; pairs 0.987 / 0.910 / 0.799; fours (batch <= 64) 0.926 / 0.855 -- a group of four quarters the dynamic chunk and doubles
 // the rows a chunk boundary cuts, which costs more than the second halving of the X traffic returns.
 // Tile rows per group for an MMA batch (2 * nacc * batch <= 512 TMEM columns) and a list of matrices (N a multiple of 128 * nacc).
-template <typename GetN>
-static uint32_t gemm_grouping(uint32_t mma_batch, uint32_t n, GetN N) {
+// A chunk boundary cuts nacc tile rows instead of one (nacc fp32 partials and as many reductions), so a group pays only in a
+// launch that gives every CTA a long share: measured on Qwen-32B-shaped projections, pairs lose below ~150 tiles per CTA
+// (one projection: gate 50 -> 56 us at batch 32, 60 -> 80 us at batch 128) and win above ~175 (a layer's MLP or more).
+// Nor may the grouped units stop filling the SMs under gemm_plan's cap on chunks per row.
+constexpr uint64_t GM_GROUP_MIN_TILES_PER_CTA = 160;
+static uint32_t gemm_plan_ctas(uint64_t total, uint32_t max_kt, uint32_t batch, int sms) {
+    uint32_t cap = 512 / batch;
+    cap = cap < 4 ? 4 : (cap > 10 ? 10 : cap);
+    const uint32_t minper = (max_kt + cap - 1) / cap;
+    const uint64_t c = total / minper;
+    return (uint32_t)(c < 1 ? 1 : (c > (uint64_t)sms ? (uint64_t)sms : c));
+}
+template <typename GetN, typename GetK>
+static uint32_t gemm_grouping(uint32_t mma_batch, uint32_t n, int sms, GetN N, GetK K) {
     const int eng = g_gemm_engine.load(std::memory_order_relaxed);
     uint32_t nacc = eng == 1 ? 1u : (mma_batch <= 64 && eng == 2 ? 4u : (mma_batch <= 128 ? 2u : 1u));
-    if (mma_batch < 32) nacc = 1;                   // (below that the X tile is a small fraction of the weight tile)
-    for (uint32_t j = 0; j < n; ++j)
+    if (mma_batch < 32 && eng == 0) nacc = 1;       // (below that the X tile is a small fraction of the weight tile)
+    uint64_t tiles = 0;
+    uint32_t max_kt = 0;
+    for (uint32_t j = 0; j < n; ++j) {
         while (nacc > 1 && N(j) % (128 * nacc)) nacc /= 2;
+        tiles += (uint64_t)(N(j) / 128) * (K(j) / 128);
+        if (K(j) / 128 > max_kt) max_kt = K(j) / 128;
+    }
+    if (eng == 0 && tiles < GM_GROUP_MIN_TILES_PER_CTA * (uint64_t)sms) nacc = 1;
+    while (eng == 0 && nacc > 1 && gemm_plan_ctas(tiles / nacc, max_kt, mma_batch, sms) < gemm_plan_ctas(2 * tiles / nacc, max_kt, mma_batch, sms)) nacc /= 2;
     return nacc;
 }
 
@@ -554,8 +573,7 @@ static cloak_status gemm_plan(GemmArgs& a, const uint32_t* N, const uint32_t* K,
     uint32_t cap = 512 / batch;
     cap = cap < 4 ? 4 : (cap > 10 ? 10 : cap);
     const uint32_t minper = (max_kt + cap - 1) / cap;
-    const uint64_t ctas64 = total / minper;
-    const uint32_t ctas = (uint32_t)(ctas64 < 1 ? 1 : (ctas64 > (uint64_t)sms ? (uint64_t)sms : ctas64));
+    const uint32_t ctas = gemm_plan_ctas(total, max_kt, batch, sms);
     const int dchunk = g_dchunk.load(std::memory_order_relaxed), static_pct = g_static_pct.load(std::memory_order_relaxed);
     uint32_t dmax = dchunk > 0 ? (uint32_t)dchunk : (batch >= 128 ? 40u : 20u);
     if (dchunk == 0) dmax /= nacc;
@@ -609,7 +627,7 @@ static cloak_status gemm_launch(const cloak_pool* pool, const cloak_gemm_op* ops
     uint64_t rows = 0;
     // Row groups (GemmArgs::nacc): as many tile rows per X tile as the 512 TMEM columns hold accumulators for, if every matrix
     // of the launch has a multiple of that many tile rows.
-    const uint32_t nacc = gemm_grouping(batch, n, [&](uint32_t j) { return ops[j].w.N; });
+    const uint32_t nacc = gemm_grouping(batch, n, sms, [&](uint32_t j) { return ops[j].w.N; }, [&](uint32_t j) { return ops[j].w.K; });
     a.nacc = nacc;
     for (uint32_t j = 0; j < n; ++j) {
         const cloak_tensor& w = ops[j].w;
@@ -676,7 +694,7 @@ extern "C" cloak_status cloak_set_gemm_schedule(int static_pct, int dyn_chunk_ti
 }
 
 extern "C" cloak_status cloak_set_gemm_engine(int engine) {
-    if (engine < 0 || engine > 2) return fail(CLOAK_ERR_INVALID, "set_gemm_engine: 0 (pairs of tile rows), 1 (never) or 2 (fours where TMEM allows)");
+    if (engine < 0 || engine > 3) return fail(CLOAK_ERR_INVALID, "set_gemm_engine: 0 (automatic: pairs of tile rows), 1 (never), 2 (fours wherever N and TMEM allow) or 3 (pairs wherever N allows)");
     g_gemm_engine.store(engine);
     return CLOAK_OK;
 }
@@ -739,7 +757,7 @@ extern "C" cloak_status cloak_gemm_chain_scratch_bytes(const cloak_pool* pool, c
         if (n == 0) return fail(CLOAK_ERR_UNSUPPORTED, "gemm_chain_scratch_bytes: op %u has too many output rows", i);
         GemmArgs a;
         uint32_t ctas = 0;
-        const uint32_t nacc = gemm_grouping(cols, n, [&](uint32_t j) { return Ns[j]; });
+        const uint32_t nacc = gemm_grouping(cols, n, sms, [&](uint32_t j) { return Ns[j]; }, [&](uint32_t j) { return Ks[j]; });
         for (uint32_t j = 0; j < n; ++j) Ns[j] /= nacc;
         cloak_status st = gemm_plan(a, Ns, Ks, n, cols, sms, &ctas, &rows, nacc);
         if (st != CLOAK_OK) return st;

@@ -926,9 +926,9 @@ def test_gemm_chain_equals_single_calls(batch):
             check_linear(yc[i].float().cpu().numpy(), X[shapes[i][1]], Ws[i % 5], "bf16", f"gemm_chain:b{batch}:op{i}", TOL["bf16"])
 
 
-@pytest.mark.parametrize("batch", [32, 50, 64, 128])
+@pytest.mark.parametrize("batch", [16, 32, 50, 64, 128])
 def test_gemm_row_groups(batch):
-    """cloak_set_gemm_engine: tile rows in pairs (default), singly, or in fours share each X tile -- two or four accumulators
+    """cloak_set_gemm_engine: tile rows in pairs (3; 0 = where the launch is large enough), singly (1), or in fours (2) share each X tile -- two or four accumulators
     per segment in TMEM, units of two / four weight tiles, tickets per row.  Under each setting: every op against the fp64
     oracle, the chain repeatable bit for bit and identical on the identity-table pool; single calls too.  Shapes with 2, 4, 6, 8
     and 20 tile rows (6 is not a multiple of four: the launch falls back to pairs), one launch that mixes in an odd row count
@@ -958,7 +958,7 @@ def test_gemm_row_groups(batch):
                     C.cloak_gemm_chain(pool.h, [(T[w], dX[all_shapes[w][1]], y) for w, y in zip(idx, ys)], batch)
                 torch.cuda.synchronize()
                 return ys
-            for eng in (0, 1, 2):
+            for eng in (0, 1, 2, 3):
                 C.cloak_set_gemm_engine(eng)
                 for idx in ([0, 1, 2, 3, 0, 2], [0, 1, 2, 3, 4], [0, 5, 3]):          # fours possible | pairs at most | single rows
                     a, b, c = run(pc, idx), run(pc, idx), run(pi, idx)
