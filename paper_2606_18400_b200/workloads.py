@@ -446,14 +446,18 @@ def run_cfg3(args):
                 ops = sweep_ops(yl)
                 flops = 2.0 * batch * (payload / 2)
                 r = {}
+                modes = [m for m in ("per_call", "chain") if m in getattr(args, "modes", "per_call,chain").split(",")]
                 for mode, fn in (("per_call", lambda: sweep(pool, y)), ("chain", lambda: C.cloak_gemm_chain(pool, ops, batch))):
+                    if mode not in modes:
+                        continue
                     med, mn = time_gpu(torch, fn, args.reps, warmup=2)
                     gmed, gmn = time_gpu(torch, graphed(torch, fn), args.reps, warmup=2)
                     r[mode] = {"stream": dict(rate(payload, med, peak), ms_min=mn, tflops=flops / med / 1e9),
                                "graph": dict(rate(payload, gmed, peak), ms_min=gmn, tflops=flops / gmed / 1e9)}
                 # the call-by-call sweep reuses one output set, so what it leaves behind is the last layer's; a chain cuts K
                 # where its ranges fall, so the two agree up to the fp32 summation order
-                r["chain_vs_per_call_max_rel"] = max(float((yl[layers - 1][nm].float() - y[nm].float()).norm() / y[nm].float().norm())
+                if len(modes) == 2:
+                    r["chain_vs_per_call_max_rel"] = max(float((yl[layers - 1][nm].float() - y[nm].float()).norm() / y[nm].float().norm())
                                                      for nm in lnames)
                 res[pool_name] = r
                 Y[pool_name + "_chain"] = yl
@@ -463,7 +467,7 @@ def run_cfg3(args):
                                     and all(torch.equal(a[nm], b[nm]) for a, b in zip(Y["cloaked_chain"], Y["native_chain"]) for nm in lnames))
             del Y
             res["overhead_pct"] = {f"{mode}_{k}": (res["cloaked"][mode][k]["ms"] - res["native"][mode][k]["ms"])
-                                   / res["native"][mode][k]["ms"] * 100 for mode in ("per_call", "chain") for k in ("stream", "graph")}
+                                   / res["native"][mode][k]["ms"] * 100 for mode in modes for k in ("stream", "graph")}
             out[f"b{batch}"] = res
     finally:
         torch.cuda.synchronize()
@@ -474,7 +478,7 @@ def run_cfg3(args):
             "payload_bytes": payload, "npages": info["npages"], "nblocks": info["nb"], "reps": args.reps,
             "hbm_peak_gbs": peak, "hbm_peak_kind": peak_kind, "hbm_nominal_gbs": NOMINAL_HBM_GBS,
             "pool_map_ms": map_ms, "pool_create_s": create_s, "generate_permute_tile_load_s": load_s,
-            "gemm": out, "launches_per_sweep": 7 * layers, "gpu_launches": C.cloak_launch_count() - launches0}
+            "gemm": out, "gemm_engine": int(getattr(args, "gemm_engine", 0)), "modes": getattr(args, "modes", "per_call,chain"), "launches_per_sweep": 7 * layers, "gpu_launches": C.cloak_launch_count() - launches0}
 
 
 # ------------------------------------------------------------------------------------------ MoE (NEXT-4)
@@ -1012,11 +1016,15 @@ def main(argv=None):
     ap.add_argument("--layers", type=int, default=0, help="cfg3: number of layers (default 64); moe: default 12 of 48")
     ap.add_argument("--batches", default="", help="cfg3: batch sizes, e.g. 16,64,256 (default 32,128)")
     ap.add_argument("--gemm-schedule", default="", help="cfg3: static_pct,dyn_chunk_tiles (cloak_set_gemm_schedule), e.g. 100,0")
+    ap.add_argument("--gemm-engine", type=int, default=0, help="cloak_set_gemm_engine: 0 auto (row pairs in long launches), 1 single rows, 2 fours, 3 pairs always")
+    ap.add_argument("--modes", default="per_call,chain", help="cfg3: which call patterns to time (per_call, chain)")
     ap.add_argument("--gemv-engine", type=int, default=0, help="cloak_set_gemv_engine: 0 auto, 1 one-shot, 2 no PDL, 3 exclusive mode (no cooperative launches)")
     ap.add_argument("--out", default="")
     args = ap.parse_args(argv)
     if args.gemv_engine:
         _imports()[1].cloak_set_gemv_engine(args.gemv_engine)
+    if args.gemm_engine:
+        _imports()[1].cloak_set_gemm_engine(args.gemm_engine)
     if args.gemm_schedule:
         _imports()[1].cloak_set_gemm_schedule(*[int(v) for v in args.gemm_schedule.split(",")])
     line = json.dumps(RUNNERS[args.workload](args))
