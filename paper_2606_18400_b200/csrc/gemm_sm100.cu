@@ -25,9 +25,12 @@
 //     them to its own accumulator IN CHUNK ORDER as it drains it.  The chunk grid is fixed by the shapes, only the
 //     assignment of chunks to CTAs varies, so the result does not depend on the schedule (deterministic; identical for
 //     cloaked and identity-table pools).
-//   * Measured and dropped: a `cta_group::2` CTA-pair variant (M = 256 over two tile rows, each CTA loading half of
-//     X: L2 -> SM traffic 2 x W -> 1.5 x W at batch 128) ran correctly and no faster (1.53 vs 1.51 ms for 8 layers of
-//     cfg3): the X traffic is not what bounds batch 128.
+//   * Row groups (GemmArgs::nacc = 2 in long launches, see gemm_grouping): a unit is then one k step of TWO adjacent tile
+//     rows -- two weight tiles, ONE X tile, two MMAs per X stage into two accumulators (4 x batch TMEM columns with the
+//     double buffer) -- which halves the X traffic from L2 (xbar2l1tex 1.96 x W -> 1.51 x W) and is worth 8-10 % at batch
+//     32 .. 128; the schedule then runs over pair rows, tickets and partials stay per real tile row.
+//   * Measured and dropped in round 1: a `cta_group::2` CTA-pair variant (M = 256 over two tile rows, each CTA loading half
+//     of X) on the then static schedule: correct and no faster (1.53 vs 1.51 ms for 8 layers of cfg3).
 #include <cuda_bf16.h>
 #include "common.cuh"
 #include "async.cuh"
