@@ -82,6 +82,9 @@ inline void launched(unsigned n = 1) { g_launches.fetch_add(n, std::memory_order
 // keygen on the current device (keygen.cu).  Either output may be null.
 cloak_status keygen_device(uint64_t key, uint64_t stream_id, uint32_t n, uint32_t* d_perm, uint32_t* d_inv,
                            cudaStream_t s);
+// nbatch permutations of n <= 4096 in one launch (keygen.cu: keygen_small_batch_kernel).
+cloak_status keygen_small_batch(uint64_t key, uint64_t stream_base, uint64_t id_base, const uint32_t* d_sel, uint32_t nbatch,
+                                uint32_t n, uint32_t* d_rowmap, uint32_t* d_colmap, cudaStream_t s);
 // Opt-in to more than 48 KiB of dynamic shared memory, once per (kernel, device): the attribute belongs to the device's
 // context, so a per-process flag would leave a second GPU with the 48 KiB default.  `done` is the call site's own mask.
 template <typename K>

@@ -241,6 +241,80 @@ __global__ void __launch_bounds__(1024) gather_cols_pair_kernel(const uint16_t* 
     }
 }
 
+// SHORT rows of 2-byte elements, many matrices per launch (the MoE experts' `down`, O8: 128 matrices of [hidden x 768], a row
+// is 1.5 KiB -- in the kernel above 96 of 1024 threads would have work).  blockIdx.y = matrix b: source matrix segsrc[b], column
+// map map[b*ncols ..], destination matrix b.  A stage is a block of 2*rp CONSECUTIVE source rows -- contiguous in memory, one
+// bulk copy -- which are interleaved into rp rows of 32-bit pairs (rows 2p and 2p+1) and gathered as above, all threads busy.
+template <typename M>
+__global__ void __launch_bounds__(512) gather_cols_short_kernel(const uint16_t* __restrict__ src, int4* __restrict__ dst,
+                                                                const uint32_t* __restrict__ map,
+                                                                const uint32_t* __restrict__ segsrc, uint32_t nrows,
+                                                                uint32_t ncols, uint32_t rp, uint32_t ns) {
+    extern __shared__ __align__(128) unsigned char sm[];
+    __shared__ __align__(8) uint64_t full[8];
+    M* colmap = reinterpret_cast<M*>(sm);
+    const uint32_t row_bytes = ncols * 2, vpr = ncols / 8, stage_bytes = 2 * rp * row_bytes;
+    unsigned char* pairs = sm + (((size_t)ncols * sizeof(M) + 127) & ~(size_t)127);      // [rp][ncols] x (row 2p, row 2p+1)
+    unsigned char* ring = pairs + stage_bytes;
+    const uint32_t b = blockIdx.y;
+    src += (uint64_t)(segsrc ? __ldg(segsrc + b) : b) * nrows * ncols;
+    dst += (uint64_t)b * nrows * vpr;
+    map += (uint64_t)b * ncols;
+    for (uint32_t c = threadIdx.x; c < ncols; c += blockDim.x) colmap[c] = (M)__ldg(map + c);
+    if (threadIdx.x == 0) {
+        for (uint32_t i = 0; i < ns; ++i) mbar_init(smem_u32(&full[i]), 1);
+        fence_barrier_init();
+    }
+    __syncthreads();
+    const uint32_t nblk = (nrows + 2 * rp - 1) / (2 * rp);
+    const uint32_t mine = blockIdx.x < nblk ? (nblk - blockIdx.x + gridDim.x - 1) / gridDim.x : 0;
+    auto rows_of = [&](uint32_t k) {                           // rows in this CTA's k-th block
+        const uint32_t r0 = (blockIdx.x + k * gridDim.x) * 2 * rp;
+        return nrows - r0 < 2 * rp ? nrows - r0 : 2 * rp;
+    };
+    auto issue = [&](uint32_t k) {
+        const uint32_t st = k % ns, bar = smem_u32(&full[st]), bytes = rows_of(k) * row_bytes;
+        mbar_expect_tx(bar, bytes);
+        bulk_g2s(smem_u32(ring + (size_t)st * stage_bytes), src + (uint64_t)(blockIdx.x + k * gridDim.x) * 2 * rp * ncols, bytes, bar);
+    };
+    if (threadIdx.x == 0)
+        for (uint32_t k = 0; k < ns && k < mine; ++k) issue(k);
+    struct alignas(sizeof(M) * 8) CmVec { M m[8]; };
+    const CmVec* cmv = reinterpret_cast<const CmVec*>(colmap);
+    const uint32_t* pw = reinterpret_cast<const uint32_t*>(pairs);
+    int4* pv = reinterpret_cast<int4*>(pairs);
+    for (uint32_t k = 0; k < mine; ++k) {
+        const uint32_t nr = rows_of(k), np = (nr + 1) / 2;
+        mbar_wait(smem_u32(&full[k % ns]), (k / ns) & 1);
+        const int4* rv = reinterpret_cast<const int4*>(ring + (size_t)(k % ns) * stage_bytes);
+        for (uint32_t i = threadIdx.x; i < np * vpr; i += blockDim.x) {      // interleave: pair word (p, c) = (row 2p [c], row 2p+1 [c])
+            const uint32_t p = i / vpr, v = i - p * vpr;
+            const int4 x = rv[(2 * p) * vpr + v], y = 2 * p + 1 < nr ? rv[(2 * p + 1) * vpr + v] : x;
+            pv[(size_t)p * 2 * vpr + 2 * v] = make_int4(__byte_perm(x.x, y.x, 0x5410), __byte_perm(x.x, y.x, 0x7632),
+                                                        __byte_perm(x.y, y.y, 0x5410), __byte_perm(x.y, y.y, 0x7632));
+            pv[(size_t)p * 2 * vpr + 2 * v + 1] = make_int4(__byte_perm(x.z, y.z, 0x5410), __byte_perm(x.z, y.z, 0x7632),
+                                                            __byte_perm(x.w, y.w, 0x5410), __byte_perm(x.w, y.w, 0x7632));
+        }
+        __syncthreads();                                       // pairs complete; the ring stage is free again
+        if (threadIdx.x == 0 && k + ns < mine) issue(k + ns);
+        const uint64_t r0 = (uint64_t)(blockIdx.x + k * gridDim.x) * 2 * rp;
+        for (uint32_t i = threadIdx.x; i < np * vpr; i += blockDim.x) {
+            const uint32_t p = i / vpr, v = i - p * vpr;
+            const CmVec c = cmv[v];
+            const uint32_t* row = pw + (size_t)p * ncols;
+            uint32_t q[8];
+#pragma unroll
+            for (int j = 0; j < 8; ++j) q[j] = row[c.m[j]];
+            dst[(r0 + 2 * p) * vpr + v] = make_int4(__byte_perm(q[0], q[1], 0x5410), __byte_perm(q[2], q[3], 0x5410),
+                                                    __byte_perm(q[4], q[5], 0x5410), __byte_perm(q[6], q[7], 0x5410));
+            if (2 * p + 1 < nr)
+                dst[(r0 + 2 * p + 1) * vpr + v] = make_int4(__byte_perm(q[0], q[1], 0x7632), __byte_perm(q[2], q[3], 0x7632),
+                                                            __byte_perm(q[4], q[5], 0x7632), __byte_perm(q[6], q[7], 0x7632));
+        }
+        __syncthreads();                                       // the pair buffer is rewritten by the next pass
+    }
+}
+
 // Column groups that are whole 16-byte vectors (seg % (16 / sizeof(E)) == 0, e.g. heads of 128 columns): the gather
 // is a vector-level index remap, no staging needed.  vmap[v'] = source vector of destination vector v'.
 template <typename Dst>
@@ -411,6 +485,40 @@ static cloak_status cols(const void* src, Dst dst, const uint32_t* map, uint32_t
                         : cols_ring<E, uint32_t, Dst>(src, dst, map, seg, nrows, ncols, smem, ns, sms, s);
     }
     return cols_fallback<E>(src, dst, map, seg, nrows, ncols, sms, s);
+}
+
+
+// nmat matrices of [nrows x ncols] 2-byte elements with SHORT rows in one launch: dst matrix b <- columns of src matrix
+// segsrc[b] gathered by map[b*ncols ..].  Returns CLOAK_ERR_UNSUPPORTED (without setting the error text) if the shape does
+// not suit the kernel; the caller then takes the matrix-by-matrix path.
+static bool cols_short_fits(uint32_t ncols) { return ncols % 8 == 0 && (size_t)ncols * 2 <= 8192; }
+static cloak_status cols_short_batch(const void* src, void* dst, const uint32_t* map, const uint32_t* segsrc, uint32_t nmat,
+                                     uint32_t nrows, uint32_t ncols, int sms, cudaStream_t s) {
+    const size_t row_bytes = (size_t)ncols * 2;
+    uint32_t rp = (uint32_t)(16384 / row_bytes);
+    if (rp < 1) rp = 1;
+    if (rp > (nrows + 1) / 2) rp = (nrows + 1) / 2;
+    const uint32_t ns = 2;
+    const size_t msz = ncols <= 65536 ? 2 : 4;
+    const size_t cm = ((size_t)ncols * msz + 127) & ~(size_t)127;
+    const size_t smem = cm + (size_t)(1 + ns) * 2 * rp * row_bytes;
+    static std::atomic<uint64_t> opted2{0}, opted4{0};
+    int dev = 0;
+    CLOAK_CUDA(cudaGetDevice(&dev));
+    const uint32_t nblk = (nrows + 2 * rp - 1) / (2 * rp);
+    uint32_t gx = ((uint32_t)sms * 2 + nmat - 1) / nmat;      // ~2 CTAs per SM over all matrices
+    if (gx > nblk) gx = nblk;
+    if (gx < 1) gx = 1;
+    if (msz == 2) {
+        if (cloak_status ost = smem_opt_in(gather_cols_short_kernel<uint16_t>, 112 * 1024, dev, opted2)) return ost;
+        gather_cols_short_kernel<uint16_t><<<dim3(gx, nmat), 512, smem, s>>>((const uint16_t*)src, (int4*)dst, map, segsrc, nrows, ncols, rp, ns);
+    } else {
+        if (cloak_status ost = smem_opt_in(gather_cols_short_kernel<uint32_t>, 112 * 1024, dev, opted4)) return ost;
+        gather_cols_short_kernel<uint32_t><<<dim3(gx, nmat), 512, smem, s>>>((const uint16_t*)src, (int4*)dst, map, segsrc, nrows, ncols, rp, ns);
+    }
+    launched();
+    CLOAK_LAUNCH_CHECK();
+    return CLOAK_OK;
 }
 
 }  // namespace cloak
@@ -747,6 +855,20 @@ extern "C" cloak_status cloak_permute_experts(uint64_t key, const cloak_moe_shap
     cloak_status st = keygen_device(key, (7ull << 32) | sh->layer, E, d_eps, nullptr, s);
     const uint64_t hrow = (uint64_t)H * e, emat = (uint64_t)I * H * e;
     if (st == CLOAK_OK) st = rows(d_router, PlainDst{static_cast<int4*>(d_router_o)}, d_eps, 1, E, hrow, sms, s);
+    if (st == CLOAK_OK && e == 2 && I <= 4096 && cols_short_fits(I) && (uint64_t)E * I <= 0xffffffffull && E <= 65535) {
+        // Batched path (short expert rows: Qwen3-MoE / DeepSeek-style experts): all E neuron permutations in one launch, gate and
+        // up as ONE row gather each over the [E*I x H] stack (source row eps[en]*I + pi_eo[j]), down as one column-gather launch
+        // over the E matrices: 5 launches per layer instead of ~5 per expert.
+        AsyncBuf mbuf(s);
+        if (cloak_status ast = mbuf.alloc((size_t)E * I * 8)) return ast;
+        uint32_t* rowmap = static_cast<uint32_t*>(mbuf.p);
+        uint32_t* colmap = rowmap + (size_t)E * I;
+        st = keygen_small_batch(key, 8ull << 32, (uint64_t)sh->layer * E, d_eps, E, I, rowmap, colmap, s);
+        if (st == CLOAK_OK) st = rows(d_gate, PlainDst{static_cast<int4*>(d_gate_o)}, rowmap, 1, E * I, hrow, sms, s);
+        if (st == CLOAK_OK) st = rows(d_up, PlainDst{static_cast<int4*>(d_up_o)}, rowmap, 1, E * I, hrow, sms, s);
+        if (st == CLOAK_OK) st = cols_short_batch(d_down, d_down_o, colmap, d_eps, E, H, I, sms, s);
+        return st;
+    }
     for (uint32_t en = 0; en < E && st == CLOAK_OK; ++en) {
         const uint32_t eo = eps[en];                               // new expert en is old expert eo, with eo's own pi
         st = keygen_device(key, (8ull << 32) | ((uint64_t)sh->layer * E + eo), I, d_pi, nullptr, s);

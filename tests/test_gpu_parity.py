@@ -1076,9 +1076,13 @@ def test_error_codes_on_device():
 
 
 # ------------------------------------------------------------------ NEXT-4: mixture-of-experts layers
-@pytest.mark.parametrize("E,H,I,dtype,layer", [(6, 64, 40, "f32", 0), (8, 256, 1000, "bf16", 3), (32, 2048, 768, "bf16", 47)])
+@pytest.mark.parametrize("E,H,I,dtype,layer", [(6, 64, 40, "f32", 0), (8, 256, 1000, "bf16", 3), (32, 2048, 768, "bf16", 47),
+                                                  (5, 264, 4096, "bf16", 1), (3, 72, 4104, "bf16", 2), (7, 128, 8, "bf16", 9), (4, 64, 1000, "f32", 4)])
 def test_permute_experts_bit_exact(E, H, I, dtype, layer):
-    """cloak_permute_experts against the oracle: router rows and whole experts by eps, each expert's neurons by its own pi."""
+    """cloak_permute_experts against the oracle: router rows and whole experts by eps, each expert's neurons by its own pi.
+    bf16 with inter <= 4096 takes the batched path (one keygen launch for all experts, one row gather each for gate and up, one
+    short-row column gather for down: ragged last row block at hidden = 264, the 8 KiB row limit at inter = 4096, one vector per
+    row at inter = 8); inter = 4104 and f32 take the expert-by-expert path."""
     key, seed = 0x1234, 9
     router = gen.synth(seed, 0, (E, H), dtype)
     gate, up = gen.synth(seed, 1, (E, I, H), dtype), gen.synth(seed, 2, (E, I, H), dtype)
