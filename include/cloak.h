@@ -412,14 +412,16 @@ cloak_status cloak_sm_weights(int device, uint32_t capacity, float* h_weights, u
  * every launch.  NULL switches it off (default).  Process-wide. */
 cloak_status cloak_set_trace(void* d_trace);
 /* Host only, no device work: the chunk grid one cloak_gemm_chain launch of n_ops <= 16 ops with these shapes would use on a
- * GPU with `sms` SMs under the current cloak_set_gemm_schedule.  The launch's 128x128 tiles -- the ops back to back, each in
- * storage order -- are numbered 0 .. total-1; chunk c covers tiles [h_begin[c], h_end[c]).  Chunks 0 .. *h_nstatic-1 are the
- * static shares (CTA c starts with chunk c; a share may be empty), the rest are drawn in order from a counter.  h_begin /
- * h_end may be NULL to query the counts; otherwise they hold max_chunks entries (CLOAK_ERR_INVALID if too few).  Computed by
- * the very functions the kernel calls. */
+ * GPU with `sms` SMs under the current cloak_set_gemm_schedule and cloak_set_gemm_engine.  *h_group = g is the number of tile
+ * rows a work unit spans (1, or 2 / 4 where the launch groups rows).  The launch's units -- the ops back to back; op j has
+ * (N_j / 128 / g) group rows of K_j / 128 units each, unit t of group row R being k step t of tile rows g R .. g R + g - 1 --
+ * are numbered 0 .. total-1; chunk c covers units [h_begin[c], h_end[c]).  Chunks 0 .. *h_nstatic-1 are the static shares (CTA c
+ * starts with chunk c; a share may be empty), the rest are drawn in order from a counter.  h_begin / h_end may be NULL to query
+ * the counts; otherwise they hold max_chunks entries (CLOAK_ERR_INVALID if too few).  Computed by the very functions the
+ * kernel calls. */
 cloak_status cloak_gemm_plan(uint32_t n_ops, const uint32_t* h_N, const uint32_t* h_K, uint32_t batch, uint32_t sms,
                              uint32_t max_chunks, uint32_t* h_begin, uint32_t* h_end, uint32_t* h_nchunks,
-                             uint32_t* h_nstatic);
+                             uint32_t* h_nstatic, uint32_t* h_group);
 /* Schedule of the tcgen05 GEMM: the first `static_pct` percent of a launch's tiles (up to a tile-row boundary) are dealt
  * out in equal shares, one per CTA; the tile rows after that are drawn from a counter as CTAs become free, whole or -- rows
  * of more than `dyn_chunk_tiles` k tiles (0 = by batch) -- in equal pieces.  The chunk grid decides where K is split, so

@@ -115,7 +115,7 @@ lib.cloak_set_trace.argtypes = [_P]
 lib.cloak_set_gemm_schedule.argtypes = [c_int, c_int]
 lib.cloak_set_gemm_engine.argtypes = [c_int]
 lib.cloak_gemm_plan.argtypes = [c_uint32, POINTER(c_uint32), POINTER(c_uint32), c_uint32, c_uint32, c_uint32,
-                                POINTER(c_uint32), POINTER(c_uint32), POINTER(c_uint32), POINTER(c_uint32)]
+                                POINTER(c_uint32), POINTER(c_uint32), POINTER(c_uint32), POINTER(c_uint32), POINTER(c_uint32)]
 lib.cloak_arena_plan.argtypes = [c_uint64, c_uint32, POINTER(c_uint64), c_uint32, POINTER(c_uint64), POINTER(c_uint64)]
 lib.cloak_permute_mlp_heads.argtypes = [c_uint64, POINTER(cloak_block_shape)] + [_P] * 15
 lib.cloak_permute_experts.argtypes = [c_uint64, POINTER(cloak_moe_shape)] + [_P] * 9
@@ -341,15 +341,16 @@ def cloak_set_gemm_engine(engine):
 
 
 def cloak_gemm_plan(shapes, batch, sms=148):
-    """Host only: (chunks, n_static) -- chunks[c] = (begin, end) in the launch's tile sequence -- for ops of shapes [(N, K)]."""
+    """Host only: (chunks, n_static, group) -- chunks[c] = (begin, end) in the launch's unit sequence, a unit spanning `group`
+    tile rows -- for ops of shapes [(N, K)]."""
     n = len(shapes)
     Ns = (c_uint32 * n)(*[s[0] for s in shapes])
     Ks = (c_uint32 * n)(*[s[1] for s in shapes])
-    nch, nst = c_uint32(0), c_uint32(0)
-    _check(lib.cloak_gemm_plan(n, Ns, Ks, batch, sms, 0, None, None, ctypes.byref(nch), ctypes.byref(nst)))
+    nch, nst, grp = c_uint32(0), c_uint32(0), c_uint32(0)
+    _check(lib.cloak_gemm_plan(n, Ns, Ks, batch, sms, 0, None, None, ctypes.byref(nch), ctypes.byref(nst), ctypes.byref(grp)))
     b, e = (c_uint32 * max(nch.value, 1))(), (c_uint32 * max(nch.value, 1))()
-    _check(lib.cloak_gemm_plan(n, Ns, Ks, batch, sms, nch.value, b, e, ctypes.byref(nch), ctypes.byref(nst)))
-    return [(b[i], e[i]) for i in range(nch.value)], nst.value
+    _check(lib.cloak_gemm_plan(n, Ns, Ks, batch, sms, nch.value, b, e, ctypes.byref(nch), ctypes.byref(nst), ctypes.byref(grp)))
+    return [(b[i], e[i]) for i in range(nch.value)], nst.value, grp.value
 
 
 def cloak_arena_plan(key, sizes, block_bytes):

@@ -704,8 +704,8 @@ extern "C" cloak_status cloak_set_gemm_engine(int engine) {
 
 extern "C" cloak_status cloak_gemm_plan(uint32_t n_ops, const uint32_t* h_N, const uint32_t* h_K, uint32_t batch, uint32_t sms,
                                         uint32_t max_chunks, uint32_t* h_begin, uint32_t* h_end, uint32_t* h_nchunks,
-                                        uint32_t* h_nstatic) {
-    if (!h_N || !h_K || !h_nchunks || !h_nstatic || n_ops == 0 || n_ops > (uint32_t)GM_MAX_OPS)
+                                        uint32_t* h_nstatic, uint32_t* h_group) {
+    if (!h_N || !h_K || !h_nchunks || !h_nstatic || !h_group || n_ops == 0 || n_ops > (uint32_t)GM_MAX_OPS)
         return fail(CLOAK_ERR_INVALID, "gemm_plan: 1..%d ops", GM_MAX_OPS);
     if (batch < 1 || batch > 256 || sms < 1) return fail(CLOAK_ERR_INVALID, "gemm_plan: batch in 1..256, sms >= 1");
     for (uint32_t j = 0; j < n_ops; ++j)
@@ -713,8 +713,13 @@ extern "C" cloak_status cloak_gemm_plan(uint32_t n_ops, const uint32_t* h_N, con
     GemmArgs a;
     uint32_t ctas = 0;
     uint64_t rows = 0;
-    cloak_status st = gemm_plan(a, h_N, h_K, n_ops, (batch + 15) & ~15u, (int)sms, &ctas, &rows);
+    const uint32_t cols = (batch + 15) & ~15u;
+    const uint32_t nacc = gemm_grouping(cols, n_ops, (int)sms, [&](uint32_t j) { return h_N[j]; }, [&](uint32_t j) { return h_K[j]; });
+    uint32_t Ng[GM_MAX_OPS];
+    for (uint32_t j = 0; j < n_ops; ++j) Ng[j] = h_N[j] / nacc;
+    cloak_status st = gemm_plan(a, Ng, h_K, n_ops, cols, (int)sms, &ctas, &rows, nacc);
     if (st != CLOAK_OK) return st;
+    *h_group = nacc;
     *h_nstatic = ctas;
     *h_nchunks = ctas + a.ndyn;
     if (!h_begin || !h_end) return CLOAK_OK;

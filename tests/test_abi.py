@@ -110,8 +110,9 @@ def test_product_does_not_import_the_oracle():
 
 def test_gemm_chunk_grid_on_the_host(C):
     """cloak_gemm_plan (the functions the tcgen05 GEMM kernel itself calls for its work split, run on the host): for the
-    cfg1 / cfg3 layers and random op lists, under several schedules -- the chunks cover the launch's tile sequence exactly
-    once and in order; the static shares are equal to within one tile and there is one per CTA at most; every drawn chunk
+    cfg1 / cfg3 layers and random op lists, under several schedules and row groupings -- the grouping is what cloak.h says
+    (pairs by default only in launches of >= 160 tiles per SM whose matrices all have an even number of tile rows); the chunks
+    cover the launch's unit sequence exactly once and in order; the static shares are equal to within one tile and there is one per CTA at most; every drawn chunk
     is non-empty and lies inside ONE tile row of ONE op (whole rows never split K); and a tile row is met by a bounded
     number of chunks (each extra one is a [batch x 128] fp32 partial and a share of a reduction)."""
     import numpy as np
@@ -120,21 +121,33 @@ def test_gemm_chunk_grid_on_the_host(C):
     llama = [(4096, 4096), (1024, 4096), (1024, 4096), (4096, 4096), (14336, 4096), (14336, 4096), (4096, 14336)]
     lists = [qwen * 2, llama, qwen[:1], [(128, 128)], [(384, 640), (128, 128)]]
     lists += [[(128 * int(rng.integers(1, 40)), 128 * int(rng.integers(1, 60))) for _ in range(int(rng.integers(1, 17)))] for _ in range(20)]
+    seen = set()
     try:
-        for sched in ((75, 0), (100, 0), (0, 0), (40, 3), (90, 64)):
+        for eng, sched in [(0, sc) for sc in ((75, 0), (100, 0), (0, 0), (40, 3), (90, 64))] + [(1, (75, 0)), (2, (75, 0)), (3, (75, 0)), (3, (0, 0))]:
             C.cloak_set_gemm_schedule(*sched)
+            C.cloak_set_gemm_engine(eng)
             for shapes in lists:
-                for batch, sms in ((1, 148), (32, 148), (128, 148), (256, 132), (77, 8)):
-                    chunks, nstatic = C.cloak_gemm_plan(shapes, batch, sms)
-                    total = sum((n // 128) * (k // 128) for n, k in shapes)
+                for batch, sms in ((1, 148), (32, 148), (128, 148), (256, 132), (77, 8), (64, 148)):
+                    chunks, nstatic, g = C.cloak_gemm_plan(shapes, batch, sms)
+                    mma = (batch + 15) // 16 * 16
+                    # the grouping: a power of two that divides every matrix's tile rows, and whose accumulators (two buffers) fit TMEM
+                    assert g in (1, 2, 4) and all((n // 128) % g == 0 for n, _ in shapes) and 2 * g * mma <= 512, (eng, shapes, batch, g)
+                    if eng == 1 or (eng == 0 and (mma < 32 or sum((n // 128) * (k // 128) for n, k in shapes) < 160 * sms)):
+                        assert g == 1
+                    if eng == 3 and mma <= 128 and all((n // 128) % 2 == 0 for n, _ in shapes):
+                        assert g == 2
+                    if eng == 2 and mma <= 64 and all((n // 128) % 4 == 0 for n, _ in shapes):
+                        assert g == 4
+                    seen.add((eng, g))
+                    total = sum((n // 128 // g) * (k // 128) for n, k in shapes)
                     assert 1 <= nstatic <= sms
-                    # row boundaries of the sequence: op j, tile row r starts at ubase_j + r * kt_j
+                    # group-row boundaries of the sequence: op j, group row r starts at ubase_j + r * kt_j
                     starts, kts, u = [], [], 0
                     for n, k in shapes:
-                        for r in range(n // 128):
+                        for r in range(n // 128 // g):
                             starts.append(u + r * (k // 128))
                             kts.append(k // 128)
-                        u += (n // 128) * (k // 128)
+                        u += (n // 128 // g) * (k // 128)
                     starts = np.array(starts)
                     pos = 0
                     sizes = []
@@ -146,18 +159,20 @@ def test_gemm_chunk_grid_on_the_host(C):
                         else:
                             assert e > b
                             r = int(np.searchsorted(starts, b, side="right")) - 1
-                            assert e <= starts[r] + kts[r], (sched, shapes, batch, c)       # inside one tile row
+                            assert e <= starts[r] + kts[r], (sched, shapes, batch, c)       # inside one group row
                     assert pos == total
                     assert max(sizes) - min(sizes) <= 1
-                    # chunks per tile row
+                    # chunks per group row
                     edges = np.array([b for b, e in chunks if e > b])
                     first = np.searchsorted(edges, starts, side="right") - 1
                     last = np.searchsorted(edges, starts + np.array(kts) - 1, side="right") - 1
                     per_row = last - first + 1
                     if sched[1] == 0:
                         assert per_row.max() <= 12, (sched, shapes, batch, int(per_row.max()))
+        assert {(0, 1), (0, 2), (1, 1), (2, 4), (2, 2), (3, 2), (3, 1)} <= seen, seen
     finally:
         C.cloak_set_gemm_schedule(75, 0)
+        C.cloak_set_gemm_engine(0)
     for bad in [([(100, 128)], 32, 148), ([(128, 128)] * 17, 32, 148), ([(128, 128)], 0, 148), ([(128, 128)], 32, 0)]:
         with pytest.raises(C.CloakError):
             C.cloak_gemm_plan(*bad)
