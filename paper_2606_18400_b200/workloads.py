@@ -774,10 +774,26 @@ def bench_cfg3(sampler, min_s=1.0, layers=None, batches=(32, 128), depths=(8, 64
                     C.cloak_pool_reserve_workspace(pool, C.cloak_gemm_chain_scratch_bytes(pool, ops, batch))
                     g[name] = (_graph(torch, lambda: C.cloak_gemm_chain(pool, ops, batch)), ops)
                     ys[name] = yl
+                # the same chain captured with single tile rows (cloak_set_gemm_engine(1)), alternated replay by replay with the
+                # default grouping: what sharing the X tile between two rows is worth on THIS board under THIS power state
+                C.cloak_set_gemm_engine(1)
+                try:
+                    ops_c = g["cloaked"][1]
+                    C.cloak_pool_reserve_workspace(pc, C.cloak_gemm_chain_scratch_bytes(pc, ops_c, batch))
+                    g1 = _graph(torch, lambda: C.cloak_gemm_chain(pc, ops_c, batch))
+                finally:
+                    C.cloak_set_gemm_engine(0)
+                for _ in range(3):
+                    g1.replay()
+                t_once = time_loop(torch, g1.replay, 0.05)["t_ms_median"]
+                tp, ts1 = ab_loop(torch, g["cloaked"][0].replay, g1.replay, int(min(max(10, np.ceil(0.5 * min_s * 1e3 / t_once)), 2000)))
+                del g1
                 d = measure(torch, sampler, peak, nbytes, g["cloaked"][0].replay, g["native"][0].replay, min_s,
                             flops=2.0 * batch * (nbytes / 2),
                             extra={"call": "cloak_gemm_chain, %d ops, batch %d, CUDA-graph replay" % (7 * depth, batch)})
                 d["cloaked_identical_to_native"] = bool(all(torch.equal(a[nm], b[nm]) for a, b in zip(ys["cloaked"], ys["native"]) for nm in lnames))
+                d.update({"t_row_pairs_ms_alternated": tp, "t_single_rows_ms": ts1, "row_pairs_gain_pct": (ts1 - tp) / ts1 * 100.0,
+                          "single_rows_frac_measured": nbytes / ts1 / 1e6 / peak})
                 out["gemm"][f"b{batch}_{depth}layers"] = d
                 del g, ys
             del X
