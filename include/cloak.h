@@ -338,6 +338,21 @@ cloak_status cloak_gemv(const cloak_pool* pool, const cloak_tensor* w, const voi
                         uint32_t batch, void* stream);
 cloak_status cloak_gemm(const cloak_pool* pool, const cloak_tensor* w, const void* d_x, void* d_y,
                         uint32_t batch, void* stream);
+/* cloak_gemv without any allocation (north_star (c): the same cloaked GEMV; for callers that cannot call
+ * cudaMalloc -- code under CUDA graph capture, tight serving loops, harnesses that forbid it).  Same contraction, same kernel
+ * and same results as cloak_gemv's streaming path, bit for bit; the kernel's scratch (row-tile arrival counters and the fp32
+ * partials of row tiles cut by a range boundary) lives in a fixed 512 KiB `static __device__` array of the library instead of
+ * the pool's workspace, so the call never calls cudaMalloc / cudaFree / cudaMallocAsync or any allocating routine, whatever
+ * the pool's workspace state.  Every GPU that loads the library holds those 512 KiB until the process exits.
+ * Limits: CLOAK_BF16, CLOAK_ROWMAJOR, K % 256 == 0, N % 16 == 0, block_bytes >= 512, batch 1..16 (else CLOAK_ERR_UNSUPPORTED /
+ * CLOAK_ERR_INVALID), and N <= 524 288 rows (one counter per 8 rows; beyond that CLOAK_ERR_UNSUPPORTED, nothing launched:
+ * use cloak_gemv).  d_x [batch, K] and d_y [batch, N] are DEVICE buffers of the caller, as in cloak_gemv.
+ * ALL calls, on every pool and stream of a device, share the one array, and it keeps the last call's contents: each call
+ * first clears the counters it uses (a small kernel on `stream`) and writes its partials before it reads them, so calls in
+ * stream order are independent of what ran before; two calls that OVERLAP on the GPU (different streams with no event between
+ * them, concurrent graph branches) race on the array and give wrong results.  Asynchronous on `stream`; two launches. */
+cloak_status cloak_gemv_static(const cloak_pool* pool, const cloak_tensor* w, const void* d_x, void* d_y,
+                               uint32_t batch, void* stream);
 /* Bytes of pool scratch the chain calls below need for these ops at this batch (the largest of the launches they split into);
  * host only.  cloak_pool_reserve_workspace grows the pool's scratch to at least `bytes` (never shrinks); synchronous: it
  * waits for the device, so call it at load time.  (cloak_gemv / cloak_gemm = a chain of one op.) */

@@ -27,7 +27,7 @@ SYMBOLS = ["cloak_last_error", "cloak_version", "cloak_runtime_info", "cloak_lau
            "cloak_unshuffle", "cloak_shuffle_many", "cloak_unshuffle_many", "cloak_relayout", "cloak_rekey_inplace", "cloak_rekey_pages_begin", "cloak_rekey_pages_step", "cloak_rekey_pages_finish", "cloak_shuffle_host", "cloak_unshuffle_host",
            "cloak_set_copy_engine", "cloak_set_copy_cache_hint", "cloak_set_gather_engine", "cloak_arena_plan", "cloak_permute_mlp_heads", "cloak_permute_experts", "cloak_load_mlp_heads", "cloak_load_tensors", "cloak_to_tile128",
            "cloak_gemv", "cloak_gemv_chain", "cloak_gemm", "cloak_gemm_chain", "cloak_gemv_chain_scratch_bytes",
-           "cloak_gemm_chain_scratch_bytes", "cloak_pool_reserve_workspace", "cloak_set_gemv_engine", "cloak_sm_weights", "cloak_set_trace", "cloak_set_gemm_schedule", "cloak_set_gemm_engine", "cloak_gemm_plan", "cloak_gemv_host", "cloak_gemv_chain_host", "cloak_silu_mul"]
+           "cloak_gemm_chain_scratch_bytes", "cloak_pool_reserve_workspace", "cloak_set_gemv_engine", "cloak_sm_weights", "cloak_set_trace", "cloak_set_gemm_schedule", "cloak_set_gemm_engine", "cloak_gemm_plan", "cloak_gemv_static", "cloak_gemv_host", "cloak_gemv_chain_host", "cloak_silu_mul"]
 
 
 class CloakError(RuntimeError):
@@ -123,6 +123,7 @@ lib.cloak_load_mlp_heads.argtypes = [c_uint64, POINTER(cloak_block_shape), _P] +
 lib.cloak_to_tile128.argtypes = [_P, _P, c_uint32, c_uint32, c_int, _P]
 lib.cloak_load_tensors.argtypes = [c_uint64, POINTER(cloak_block_shape), _P, POINTER(cloak_load_item), c_uint32, c_int, _P]
 lib.cloak_gemv.argtypes = [_P, POINTER(cloak_tensor), _P, _P, c_uint32, _P]
+lib.cloak_gemv_static.argtypes = [_P, POINTER(cloak_tensor), _P, _P, c_uint32, _P]
 lib.cloak_gemv_chain.argtypes = [_P, POINTER(cloak_gemv_op), c_uint32, c_uint32, _P]
 lib.cloak_gemm_chain.argtypes = [_P, POINTER(cloak_gemm_op), c_uint32, c_uint32, _P]
 lib.cloak_gemv_chain_scratch_bytes.argtypes = [_P, POINTER(cloak_gemv_op), c_uint32, c_uint32, POINTER(c_uint64)]
@@ -406,6 +407,11 @@ def cloak_to_tile128(d_src, d_dst, N, K, dt, stream=None):
 
 def cloak_gemv(pool, tensor, d_x, d_y, batch, stream=None):
     _check(lib.cloak_gemv(pool, byref(tensor), _ptr(d_x), _ptr(d_y), batch, _stream(stream)))
+
+
+def cloak_gemv_static(pool, tensor, d_x, d_y, batch, stream=None):
+    """cloak_gemv with its scratch in the library's fixed device array: allocates nothing (see cloak.h for the limits)."""
+    _check(lib.cloak_gemv_static(pool, byref(tensor), _ptr(d_x), _ptr(d_y), batch, _stream(stream)))
 
 
 def cloak_gemv_ops(ops):

@@ -590,3 +590,119 @@ cloak_status gemv_stream_launch(const cloak_pool* pool, const cloak_gemv_op* ops
 }
 
 }  // namespace cloak
+
+// ---------------------------------------------------------------------------------------------------------------------
+// cloak_gemv_static: the streaming GEMV of ONE projection with its scratch in a fixed device array -- an entry point that
+// allocates nothing (callers under CUDA graph capture, serving loops and harnesses that may not call cudaMalloc).
+//
+// The kernel is gemv_chain_kernel, unchanged; what differs is where its row-tile counters and cut-tile partials live:
+// cloak_gemv takes them from the pool's workspace (cudaMalloc at cloak_pool_create, grown on demand), this call from
+// g_static_scratch below -- GS_STATIC_BYTES = 512 KiB that every GPU which loads the library holds until the process ends:
+//   words [0, GS_STATIC_TILES)           row-tile arrival counters (one per 8 weight rows: N <= 8 * GS_STATIC_TILES = 524 288)
+//   bytes [GS_STATIC_TILES * 4, 512 KiB) fp32 partials, one [batch x 8] block per CTA (148 CTAs x batch 16 = 74 KiB)
+// In HOST code the name g_static_scratch is a host-side stand-in for the symbol, not a device address: the address the
+// kernel gets comes from cudaGetSymbolAddress, asked once per device with that device current (static_scratch()).
+// ALL calls share the array and it keeps the last call's contents: the counters this call uses are cleared first (a tiny
+// kernel on the caller's stream), the partials are written before they are read.  Two calls that overlap on the GPU
+// (different streams, no event between them) race on it.
+namespace cloak {
+
+constexpr uint32_t GS_STATIC_TILES = 65536;                 // 256 KiB of counters
+constexpr size_t GS_STATIC_BYTES = 512u << 10;
+constexpr size_t GS_STATIC_PART_BYTES = GS_STATIC_BYTES - (size_t)GS_STATIC_TILES * 4;
+static __device__ __align__(256) unsigned char g_static_scratch[GS_STATIC_BYTES];
+
+__global__ void zero_words_kernel(uint32_t* p, uint32_t n) {
+    for (uint32_t i = blockIdx.x * blockDim.x + threadIdx.x; i < n; i += gridDim.x * blockDim.x) p[i] = 0u;
+}
+
+// The device address of g_static_scratch on `device` (which must be current): asked once per device, then cached.
+static cloak_status static_scratch(int device, unsigned char** out) {
+    static std::atomic<unsigned char*> cache[64];
+    const bool tracked = device >= 0 && device < 64;
+    unsigned char* p = tracked ? cache[device].load(std::memory_order_acquire) : nullptr;
+    if (!p) {
+        void* sym = nullptr;
+        const cudaError_t e = cudaGetSymbolAddress(&sym, g_static_scratch);
+        if (e != cudaSuccess || !sym) {
+            cudaGetLastError();
+            return fail(CLOAK_ERR_CUDA, "gemv_static: cudaGetSymbolAddress of the static scratch on device %d: %s", device,
+                        cudaGetErrorString(e));
+        }
+        p = static_cast<unsigned char*>(sym);
+        if (tracked) cache[device].store(p, std::memory_order_release);
+    }
+    *out = p;
+    return CLOAK_OK;
+}
+
+}  // namespace cloak
+
+namespace cloak { cloak_status check_linear(const cloak_pool* pool, const cloak_tensor* w, const void* x, void* y, const char* who); }
+
+extern "C" cloak_status cloak_gemv_static(const cloak_pool* pool, const cloak_tensor* w, const void* d_x, void* d_y,
+                                          uint32_t batch, void* stream) {
+    using namespace cloak;
+    cloak_status st = check_linear(pool, w, d_x, d_y, "gemv_static");
+    if (st != CLOAK_OK) return st;
+    if (batch < 1 || batch > 16) return fail(CLOAK_ERR_INVALID, "gemv_static: batch must be in 1..16");
+    const int cu = gemv_stream_chunk(pool, w, batch);
+    if (cu < 1 || w->N % 16)
+        return fail(CLOAK_ERR_UNSUPPORTED, "gemv_static: needs CLOAK_BF16, CLOAK_ROWMAJOR, K %% 256 == 0, N %% 16 == 0, block_bytes >= 512");
+    const uint32_t tiles = w->N / GS_ROWS;
+    if (tiles > GS_STATIC_TILES)
+        return fail(CLOAK_ERR_UNSUPPORTED, "gemv_static: N = %u needs %u row-tile counters, the static scratch holds %u (N <= %u); use cloak_gemv",
+                    w->N, tiles, GS_STATIC_TILES, GS_STATIC_TILES * GS_ROWS);
+    DeviceGuard g(pool->device);
+    cudaStream_t s = (cudaStream_t)stream;
+    const int sms = sm_count(pool->device);
+    ChainArgs a;
+    a.pool = pool->base;
+    a.T = pool->d_T;
+    a.log2b = pool->log2_block;
+    a.batch = batch;
+    a.nops = 1;
+    a.any_signal = 0;
+    a.trace = nullptr;
+    a.early = 0;                         // the whole launch waits for its stream predecessor (the counter clear below)
+    ChainOp& o = a.ops[0];
+    o.w_offset = w->w_offset;
+    o.x = static_cast<const uint16_t*>(d_x);
+    o.y = static_cast<__nv_bfloat16*>(d_y);
+    o.gate = nullptr;
+    o.act = nullptr;
+    o.N = w->N;
+    o.K = w->K;
+    o.kch = (uint32_t)(((uint64_t)w->K * 2) / (512u * cu));
+    const uint64_t units64 = (uint64_t)tiles * o.kch;
+    if (units64 > 0xffffffffull) return fail(CLOAK_ERR_UNSUPPORTED, "gemv_static: tensor too large");
+    o.units = (uint32_t)units64;
+    o.tile_base = 0;
+    o.flags = 0;
+    o.wait_op = NO_WAIT;
+    o.rot = 0;
+    const int ctas = units64 < (uint64_t)sms ? (int)units64 : sms;
+    o.per = (o.units + ctas - 1) / ctas;
+    o.ctas = (o.units + o.per - 1) / o.per;
+    const size_t part = (size_t)ctas * batch * GS_ROWS * 4;
+    if (part > GS_STATIC_PART_BYTES)
+        return fail(CLOAK_ERR_UNSUPPORTED, "gemv_static: %d CTAs x batch %u need %zu bytes of partials, the static scratch holds %zu",
+                    ctas, batch, part, GS_STATIC_PART_BYTES);
+    unsigned char* scratch = nullptr;
+    st = static_scratch(pool->device, &scratch);
+    if (st != CLOAK_OK) return st;
+    a.counters = reinterpret_cast<uint32_t*>(scratch);
+    a.opsync = a.counters + GS_STATIC_TILES - 2 * GS_MAX_OPS;      // (unused by a launch of one op; inside the array all the same)
+    a.part = reinterpret_cast<float*>(scratch + (size_t)GS_STATIC_TILES * 4);
+    // the counters are self-resetting, but the array is shared with every other call: start from zero whatever was there
+    zero_words_kernel<<<(tiles + 1023) / 1024, 1024, 0, s>>>(a.counters, tiles);
+    launched();
+    CLOAK_LAUNCH_CHECK();
+    const bool nt2 = batch > 8;
+#define GS_CASE(C) case C: return nt2 ? launch<C, 2>(a, ctas, pool->device, s) : launch<C, 1>(a, ctas, pool->device, s)
+    switch (cu) {
+        GS_CASE(8); GS_CASE(7); GS_CASE(6); GS_CASE(5); GS_CASE(4); GS_CASE(3); GS_CASE(2);
+        default: return nt2 ? launch<1, 2>(a, ctas, pool->device, s) : launch<1, 1>(a, ctas, pool->device, s);
+    }
+#undef GS_CASE
+}
