@@ -340,12 +340,13 @@ static cloak_status gemv_check(const cloak_pool* pool, const cloak_tensor* w, co
 
 using namespace cloak;
 
-namespace cloak { extern std::atomic<bool> g_gemv_exclusive; }
+namespace cloak { extern std::atomic<bool> g_gemv_exclusive; void gemv_set_fusion(bool on); }
 extern "C" cloak_status cloak_set_gemv_engine(int engine) {
-    if (engine < 0 || engine > 3) return fail(CLOAK_ERR_INVALID, "set_gemv_engine: engine must be 0, 1, 2 or 3");
+    if (engine < 0 || engine > 4) return fail(CLOAK_ERR_INVALID, "set_gemv_engine: engine must be 0 .. 4");
     g_force_oneshot = engine == 1;
     g_gemv_pdl = engine != 2;
     g_gemv_exclusive = engine == 3;
+    gemv_set_fusion(engine != 4);
     return CLOAK_OK;
 }
 

@@ -34,6 +34,7 @@
 //   * programmatic dependent launch: the grid may start while its stream predecessor drains; the producer
 //     streams W (immutable during decode) ahead of griddepcontrol.wait, everything else waits.
 #include <cuda_bf16.h>
+#include <type_traits>
 #include "common.cuh"
 #include "async.cuh"
 
@@ -76,6 +77,25 @@ struct ChainArgs {
     uint32_t any_signal;     // some op of this launch signals
     ChainOp ops[GS_MAX_OPS];
 };
+
+// Segmented ops (SEG kernels, batch <= 8): an op whose row tiles come from several matrices of one shape -- the selected experts'
+// gate (or up, or down) projections of an MoE layer, fused by the host into ONE op of nseg x (N / 8) tiles so that a CTA streams
+// several units per op instead of at most one (gemv_stream_launch: fusion).  Tile t of the op is tile t % tps of segment t / tps.
+struct ChainSeg {
+    uint64_t w_offset;
+    const uint16_t* x;
+    __nv_bfloat16* y;
+    const uint16_t* gate;
+    uint16_t* act;
+};
+struct ChainArgsSeg {
+    ChainArgs base;                  // ops[j].N / K are one segment's; units = nseg * tps * kch; w_offset, x, y, gate, act unused
+    ChainSeg segs[GS_MAX_OPS];       // every original op of the launch is a segment of exactly one fused op
+    uint32_t tps[GS_MAX_OPS];        // tiles per segment of op j (N / 8)
+    uint32_t seg0[GS_MAX_OPS];       // op j's first entry in segs[]
+};
+__device__ __forceinline__ const ChainArgs& chain_base(const ChainArgs& a) { return a; }
+__device__ __forceinline__ const ChainArgs& chain_base(const ChainArgsSeg& a) { return a.base; }
 
 constexpr int GS_CONSUMERS = 8;                       // consumer warps
 // Warps ahead of the consumers.  batch <= 8: the producer warp alone.  batch 9..16: a whole warpgroup (producer + three
@@ -159,8 +179,10 @@ __device__ __forceinline__ uint16_t ld_coherent_u16(const uint16_t* p) {
 // CU: chunk bytes per row / 512 (1..8; the largest divisor of the row's 512-byte units that is <= 8, so a 10 KiB row is cut
 // into 2.5 KiB chunks and a 1.5 KiB row is one chunk -- larger TMA pieces than a power of two would allow).
 // NT: 1 = batch <= 8 (upper half of the MMA's M is zero), 2 = batch <= 16.
-template <int CU, int NT>
-__global__ void __launch_bounds__(gs_threads(NT), 1) gemv_chain_kernel(const __grid_constant__ ChainArgs a) {
+template <int CU, int NT, bool SEG = false>
+__global__ void __launch_bounds__(gs_threads(NT), 1)
+gemv_chain_kernel(const __grid_constant__ typename std::conditional<SEG, ChainArgsSeg, ChainArgs>::type args) {
+    const ChainArgs& a = chain_base(args);
     constexpr uint32_t CB = CU * 512u;
     constexpr uint32_t RS = CB + GS_PAD;                       // staged row stride
     constexpr uint32_t STAGE = GS_ROWS * RS;
@@ -215,7 +237,14 @@ __global__ void __launch_bounds__(gs_threads(NT), 1) gemv_chain_kernel(const __g
                         __syncwarp();
                         if (lane < GS_ROWS) {
                             // a chunk that is not a power of two may cross a block boundary: one bulk copy per block touched
-                            uint64_t off = op.w_offset + (uint64_t)(tile * GS_ROWS + lane) * row_bytes + (uint64_t)c * CB;
+                            uint64_t woff = op.w_offset;
+                            uint32_t lt = tile;                                        // the tile inside its matrix
+                            if constexpr (SEG) {
+                                const uint32_t sg = tile / args.tps[j];
+                                lt = tile - sg * args.tps[j];
+                                woff = args.segs[args.seg0[j] + sg].w_offset;
+                            }
+                            uint64_t off = woff + (uint64_t)(lt * GS_ROWS + lane) * row_bytes + (uint64_t)c * CB;
                             uint32_t dst = smem_base + s * STAGE + lane * RS, left = CB;
                             if ((CU & (CU - 1)) == 0 && CB <= (1u << a.log2b)) {       // power of two within a block: one copy
                                 const uint32_t slot = __ldg(a.T + (off >> a.log2b));
@@ -278,15 +307,25 @@ __global__ void __launch_bounds__(gs_threads(NT), 1) gemv_chain_kernel(const __g
             // is ours to finish, unless the range lies inside a single tile that started before us.
             const bool cut_head = ubeg > tile_lo * kch;
             const bool cut_tail = uend < (tile_hi + 1) * kch && !(tile_hi == tile_lo && cut_head);
-            const uint16_t* x0 = op.x + (size_t)g * op.K + lane_off / 2;
+            const uint16_t* x0 = op.x + (size_t)g * op.K + lane_off / 2;            // (SEG: set per group, from its segment)
             const uint16_t* x1 = op.x + (size_t)(g + 8) * op.K + lane_off / 2;
             float* mypart = a.part + ((size_t)j * gridDim.x + vr) * nout;
             // Every Y element is stored exactly once, by the CTA that owns its row tile.  The gate op had the same
             // (N, K), hence the same split: gate[idx] was stored by this CTA, before consumer barriers passed since.
-            auto store_y = [&](size_t idx, float sum) {
+            // store_y(tile, m, r, sum): batch row m, row r of row tile `tile` of the op.
+            auto store_y = [&](uint32_t tile, uint32_t m, uint32_t r, float sum) {
                 const __nv_bfloat16 v = __float2bfloat16_rn(sum);
-                op.y[idx] = v;
-                if (op.gate) op.act[idx] = silu_mul_bf16(ld_coherent_u16(op.gate + idx), v);
+                if constexpr (SEG) {
+                    const uint32_t sg = tile / args.tps[j];
+                    const ChainSeg& sgm = args.segs[args.seg0[j] + sg];
+                    const size_t idx = (size_t)m * op.N + (tile - sg * args.tps[j]) * GS_ROWS + r;
+                    sgm.y[idx] = v;
+                    if (sgm.gate) sgm.act[idx] = silu_mul_bf16(ld_coherent_u16(sgm.gate + idx), v);
+                } else {
+                    const size_t idx = (size_t)m * op.N + tile * GS_ROWS + r;
+                    op.y[idx] = v;
+                    if (op.gate) op.act[idx] = silu_mul_bf16(ld_coherent_u16(op.gate + idx), v);
+                }
             };
 
             // X fragments of one (group, chunk) phase.  Batch <= 8 re-reads them mostly from L1; batch 9..16 (X is up to
@@ -304,8 +343,16 @@ __global__ void __launch_bounds__(gs_threads(NT), 1) gemv_chain_kernel(const __g
             };
             if (PF) load_x(xa, xb, 0);
 
-            for (uint32_t g0 = tile_lo; g0 <= tile_hi; g0 += GS_TG) {
-                const uint32_t g1 = min(g0 + GS_TG - 1, tile_hi);
+            for (uint32_t g0 = tile_lo, gnext; g0 <= tile_hi; g0 = gnext) {
+                uint32_t g1 = min(g0 + GS_TG - 1, tile_hi);
+                if constexpr (SEG) {                               // a group shares X fragments: it stays inside one segment
+                    const uint32_t sg = g0 / args.tps[j];
+                    g1 = min(g1, (sg + 1) * args.tps[j] - 1);
+                    const uint16_t* xs = args.segs[args.seg0[j] + sg].x;
+                    x0 = xs + (size_t)g * op.K + lane_off / 2;
+                    x1 = xs + (size_t)(g + 8) * op.K + lane_off / 2;
+                }
+                gnext = SEG ? g1 + 1 : g0 + GS_TG;
                 float acc[GS_TG][GS_NACC][4];
 #pragma unroll
                 for (int q = 0; q < GS_TG; ++q)
@@ -377,7 +424,7 @@ __global__ void __launch_bounds__(gs_threads(NT), 1) gemv_chain_kernel(const __g
                             for (int w = 1; w < GS_CONSUMERS; ++w) sum += red[w][jj][rem];
                             if (tile == tile_lo && cut_head) __stcg(mypart + m * GS_ROWS + r, sum);
                             else if (tile == tile_hi && cut_tail) own[rem] = sum;
-                            else store_y((size_t)m * op.N + tile * GS_ROWS + r, sum);
+                            else store_y(tile, m, r, sum);
                         }
                         if (cut_head && tb == tile_lo) {
                             // publish the head partial now, early in the range: the tile's owner needs it only at its end
@@ -403,7 +450,7 @@ __global__ void __launch_bounds__(gs_threads(NT), 1) gemv_chain_kernel(const __g
                 for (uint32_t i = ctid; i < nout; i += GS_CONSUMERS * 32) {
                     float sum = own[i];
                     for (uint32_t q = 1; q <= nc; ++q) sum += __ldcg(mypart + (size_t)q * nout + i);
-                    store_y((size_t)(i / GS_ROWS) * op.N + tile_hi * GS_ROWS + (i % GS_ROWS), sum);
+                    store_y(tile_hi, i / GS_ROWS, i % GS_ROWS, sum);
                 }
                 consumer_bar();                                  // own[] is reused by the next op
             }
@@ -457,12 +504,15 @@ std::atomic<bool> g_gemv_exclusive{false};             // cloak_set_gemv_engine(
 static std::atomic<int> g_coop_with_pdl{-1};     // -1 unknown, 0 rejected, 1 accepted
 int gemv_coop_pdl_state() { return g_coop_with_pdl.load(std::memory_order_relaxed); }
 
-template <int CU, int NT>
-static cloak_status launch(const ChainArgs& a, int ctas, int device, cudaStream_t s) {
-    const bool coop = a.any_signal != 0 && !g_gemv_exclusive.load(std::memory_order_relaxed);
+inline const ChainArgs& host_base(const ChainArgs& a) { return a; }
+inline const ChainArgs& host_base(const ChainArgsSeg& a) { return a.base; }
+
+template <int CU, int NT, bool SEG = false, typename Args = ChainArgs>
+static cloak_status launch(const Args& a, int ctas, int device, cudaStream_t s) {
+    const bool coop = host_base(a).any_signal != 0 && !g_gemv_exclusive.load(std::memory_order_relaxed);
     constexpr size_t smem = (size_t)gs_stages(CU) * GS_ROWS * (CU * 512u + GS_PAD);
     static std::atomic<uint64_t> opted{0};
-    auto* kernel = gemv_chain_kernel<CU, NT>;
+    auto* kernel = gemv_chain_kernel<CU, NT, SEG>;
     cloak_status st = smem_opt_in(kernel, smem, device, opted);
     if (st != CLOAK_OK) return st;
     cudaLaunchConfig_t cfg = {};
@@ -506,41 +556,127 @@ int gemv_stream_chunk(const cloak_pool* pool, const cloak_tensor* w, uint32_t ba
     return cu;
 }
 
+// Fusion of small ops (batch <= 8).  An op whose rows are a single chunk (kch == 1) never has a row tile cut by a range
+// boundary, so each of its outputs is computed by one CTA in one fixed order whatever the work split: several such ops of one
+// shape may be dealt out as ONE op over the concatenation of their row tiles, bit for bit the same results.  That is what an MoE
+// layer needs -- a selected expert's projection is 96 units for 148 CTAs, and a CTA pays ~1.3 us of fixed cost per op (table
+// lookup and first copy in the producer, reduction and barriers in the consumers) for 0.7 us of streaming.
+// Which ops: inside a run of mutually independent ops (consecutive ops that are all after == 0, or an after == 1 op and the
+// after == 2 ops behind it), those with kch == 1 and equal (N, K, has-gate-epilogue), kept in chain order.  A gate epilogue needs
+// its gate written by the SAME CTA earlier in the launch: the producers must then be the same-numbered segments of one earlier
+// fused op of the same size (gate_e / up_e of the selected experts are); if anything does not fit, nothing is fused.
+static std::atomic<bool> g_gemv_fuse{true};
+void gemv_set_fusion(bool on) { g_gemv_fuse.store(on, std::memory_order_relaxed); }
+
+struct FusedPlan {
+    uint32_t nf = 0;                                  // fused ops
+    uint32_t first[GS_MAX_OPS], count[GS_MAX_OPS];    // op f = members member[first[f] .. first[f] + count[f])
+    uint32_t member[GS_MAX_OPS];                      // original op indices
+};
+
+static bool plan_fusion(const cloak_gemv_op* ops, uint32_t n, int cu, FusedPlan& fp) {
+    uint32_t grp_of[GS_MAX_OPS], pos_of[GS_MAX_OPS];  // original op -> fused op, position inside it
+    uint32_t rep[GS_MAX_OPS], cnt[GS_MAX_OPS];        // per fused op: first member, size
+    // An epilogue's gate is either complete before the launch (1) or written by an earlier op of it (2); an op may feed such
+    // an epilogue (feeds).  Both are part of what makes ops alike: a launch boundary that cuts a gate_e | up_e pair leaves an up
+    // whose gate is outside and a gate nobody in the launch reads -- they must not shift the positions of the pairs that are whole.
+    uint8_t gstate[GS_MAX_OPS], feeds[GS_MAX_OPS];
+    for (uint32_t j = 0; j < n; ++j) {
+        gstate[j] = ops[j].d_gate ? 1 : 0;
+        feeds[j] = 0;
+    }
+    for (uint32_t j = 0; j < n; ++j)
+        for (uint32_t k = 0; k < j && ops[j].d_gate; ++k)
+            if (ops[k].d_y == ops[j].d_gate) { gstate[j] = 2; feeds[k] = 1; }
+    uint32_t nf = 0, run_first_group = 0;
+    bool any = false;
+    for (uint32_t j = 0; j < n; ++j) {
+        const bool new_run = j == 0 || ops[j].after == 1 || ((ops[j].after == 0) != (ops[j - 1].after == 0));
+        if (new_run) run_first_group = nf;
+        const bool small = (uint64_t)ops[j].w.K * 2 == 512ull * cu;                       // kch == 1
+        uint32_t f = nf;
+        if (small)
+            for (uint32_t q = run_first_group; q < nf; ++q) {
+                const uint32_t r = rep[q];
+                if (ops[r].w.N == ops[j].w.N && ops[r].w.K == ops[j].w.K &&
+                    gstate[r] == gstate[j] && feeds[r] == feeds[j]) { f = q; break; }
+            }
+        if (f == nf) { rep[nf] = j; cnt[nf] = 0; ++nf; } else any = true;
+        grp_of[j] = f;
+        pos_of[j] = cnt[f]++;
+    }
+    if (!any) return false;
+    // gate epilogues: producer in this launch -> same position of an earlier fused op of the same size
+    for (uint32_t j = 0; j < n; ++j) {
+        if (!ops[j].d_gate) continue;
+        for (uint32_t k = 0; k < n; ++k) {
+            if (ops[k].d_y != ops[j].d_gate) continue;
+            if (k >= j || grp_of[k] >= grp_of[j] || pos_of[k] != pos_of[j] || cnt[grp_of[k]] != cnt[grp_of[j]]) return false;
+        }
+    }
+    fp.nf = nf;
+    uint32_t at = 0;
+    for (uint32_t f = 0; f < nf; ++f) { fp.first[f] = at; fp.count[f] = cnt[f]; at += cnt[f]; }
+    uint32_t fill[GS_MAX_OPS] = {};
+    for (uint32_t j = 0; j < n; ++j) fp.member[fp.first[grp_of[j]] + fill[grp_of[j]]++] = j;
+    return true;
+}
+
 // One launch: n <= GS_MAX_OPS ops that all stream with the same chunk size (cu x 512 bytes).  Preconditions checked by the callers.
 cloak_status gemv_stream_launch(const cloak_pool* pool, const cloak_gemv_op* ops, uint32_t n, int cu, uint32_t batch,
                                 cudaStream_t s) {
-    ChainArgs a;
+    ChainArgsSeg as;
+    ChainArgs& a = as.base;
+    FusedPlan fp;
+    const bool seg = batch <= 8 && n > 1 && g_gemv_fuse.load(std::memory_order_relaxed) && plan_fusion(ops, n, cu, fp);
+    if (!seg) {
+        fp.nf = n;
+        for (uint32_t j = 0; j < n; ++j) { fp.first[j] = j; fp.count[j] = 1; fp.member[j] = j; }
+    }
+    const uint32_t nf = fp.nf;
     a.pool = pool->base;
     a.T = pool->d_T;
     a.log2b = pool->log2_block;
     a.batch = batch;
-    a.nops = n;
+    a.nops = nf;
     const int sms = sm_count(pool->device);
     uint64_t max_units = 0, tile_base = 0;
     uint32_t last_wait = NO_WAIT;
     a.any_signal = 0;
-    for (uint32_t j = 0; j < n; ++j) {
-        const cloak_tensor& w = ops[j].w;
+    for (uint32_t j = 0; j < nf; ++j) {
+        const cloak_gemv_op& h = ops[fp.member[fp.first[j]]];       // the first member: shape, dependency
+        const cloak_tensor& w = h.w;
         ChainOp& o = a.ops[j];
         o.w_offset = w.w_offset;
-        o.x = static_cast<const uint16_t*>(ops[j].d_x);
-        o.y = static_cast<__nv_bfloat16*>(ops[j].d_y);
-        o.gate = static_cast<const uint16_t*>(ops[j].d_gate);
-        o.act = static_cast<uint16_t*>(ops[j].d_act);
+        o.x = static_cast<const uint16_t*>(h.d_x);
+        o.y = static_cast<__nv_bfloat16*>(h.d_y);
+        o.gate = static_cast<const uint16_t*>(h.d_gate);
+        o.act = static_cast<uint16_t*>(h.d_act);
         o.N = w.N;
         o.K = w.K;
         o.kch = (uint32_t)(((uint64_t)w.K * 2) / (512u * cu));
-        const uint64_t units64 = (uint64_t)(w.N / GS_ROWS) * o.kch;
+        as.tps[j] = w.N / GS_ROWS;
+        as.seg0[j] = fp.first[j];
+        for (uint32_t q = 0; q < fp.count[j]; ++q) {
+            const cloak_gemv_op& m = ops[fp.member[fp.first[j] + q]];
+            ChainSeg& sg = as.segs[fp.first[j] + q];
+            sg.w_offset = m.w.w_offset;
+            sg.x = static_cast<const uint16_t*>(m.d_x);
+            sg.y = static_cast<__nv_bfloat16*>(m.d_y);
+            sg.gate = static_cast<const uint16_t*>(m.d_gate);
+            sg.act = static_cast<uint16_t*>(m.d_act);
+        }
+        const uint64_t units64 = (uint64_t)fp.count[j] * (w.N / GS_ROWS) * o.kch;
         if (units64 > 0xffffffffull) return fail(CLOAK_ERR_UNSUPPORTED, "gemv: tensor too large");
         o.units = (uint32_t)units64;
         o.tile_base = (uint32_t)tile_base;
-        tile_base += w.N / GS_ROWS;
+        tile_base += (uint64_t)fp.count[j] * (w.N / GS_ROWS);
         // after = 1: wait for every earlier op of the chain (i.e. for op j-1 to be reported by all CTAs);
         // after = 2: the same dependency as the nearest earlier waiting op (no new grid-wide arrival needed)
         o.flags = 0;
         o.wait_op = NO_WAIT;
-        if (j > 0 && ops[j].after == 1) o.wait_op = j - 1;
-        else if (j > 0 && ops[j].after >= 2) o.wait_op = last_wait;
+        if (j > 0 && h.after == 1) o.wait_op = j - 1;
+        else if (j > 0 && h.after >= 2) o.wait_op = last_wait;
         if (o.wait_op != NO_WAIT) {
             a.ops[o.wait_op].flags |= OP_SIGNAL;
             a.any_signal = 1;
@@ -555,7 +691,7 @@ cloak_status gemv_stream_launch(const cloak_pool* pool, const cloak_gemv_op* ops
     // ops fill the grid anyway (cfg2 2.54 -> 2.61 ms), so: all ops rotate if ops that leave at least an eighth of the CTAs idle
     // hold most of the launch's units, else only the ops that leave a quarter idle do.
     uint64_t small_units = 0, all_units = 0;
-    for (uint32_t j = 0; j < n; ++j) {
+    for (uint32_t j = 0; j < nf; ++j) {
         ChainOp& o = a.ops[j];
         o.per = (o.units + ctas - 1) / ctas;
         o.ctas = (o.units + o.per - 1) / o.per;
@@ -564,7 +700,7 @@ cloak_status gemv_stream_launch(const cloak_pool* pool, const cloak_gemv_op* ops
     }
     const bool rotate_all = 2 * small_units > all_units;
     uint32_t ranges_so_far = 0;
-    for (uint32_t j = 0; j < n; ++j) {
+    for (uint32_t j = 0; j < nf; ++j) {
         ChainOp& o = a.ops[j];
         o.rot = (rotate_all || o.ctas * 4 <= (uint32_t)ctas * 3) ? ranges_so_far % ctas : 0;
         for (uint32_t k = 0; k < j; ++k)
@@ -572,7 +708,7 @@ cloak_status gemv_stream_launch(const cloak_pool* pool, const cloak_gemv_op* ops
         ranges_so_far += o.ctas;
     }
     a.trace = g_trace.load(std::memory_order_relaxed);
-    const size_t need = WS_COUNTER_BYTES + (size_t)n * ctas * batch * GS_ROWS * 4;
+    const size_t need = WS_COUNTER_BYTES + (size_t)nf * ctas * batch * GS_ROWS * 4;
     cloak_status st = pool_workspace(pool, need, s);
     if (st != CLOAK_OK) return st;
     a.counters = reinterpret_cast<uint32_t*>(pool->ws);
@@ -581,12 +717,16 @@ cloak_status gemv_stream_launch(const cloak_pool* pool, const cloak_gemv_op* ops
     a.early = (g_gemv_pdl.load(std::memory_order_relaxed) && !pool->dirty) ? 1u : 0u;
     if (pool->dirty && pool->dirty_stream == s) pool->dirty = false;   // this launch waits for the writer in full
     const bool nt2 = batch > 8;
-#define GS_CASE(C) case C: return nt2 ? launch<C, 2>(a, ctas, pool->device, s) : launch<C, 1>(a, ctas, pool->device, s)
+#define GS_CASE(C)                                                                                   \
+    case C:                                                                                          \
+        return seg ? launch<C, 1, true, ChainArgsSeg>(as, ctas, pool->device, s)                     \
+                   : (nt2 ? launch<C, 2>(a, ctas, pool->device, s) : launch<C, 1>(a, ctas, pool->device, s))
     switch (cu) {
         GS_CASE(8); GS_CASE(7); GS_CASE(6); GS_CASE(5); GS_CASE(4); GS_CASE(3); GS_CASE(2);
-        default: return nt2 ? launch<1, 2>(a, ctas, pool->device, s) : launch<1, 1>(a, ctas, pool->device, s);
+        default: GS_CASE(1);
     }
 #undef GS_CASE
+    return CLOAK_OK;
 }
 
 }  // namespace cloak

@@ -1034,7 +1034,7 @@ def main(argv=None):
     ap.add_argument("--gemm-schedule", default="", help="cfg3: static_pct,dyn_chunk_tiles (cloak_set_gemm_schedule), e.g. 100,0")
     ap.add_argument("--gemm-engine", type=int, default=0, help="cloak_set_gemm_engine: 0 auto (row pairs in long launches), 1 single rows, 2 fours, 3 pairs always")
     ap.add_argument("--modes", default="per_call,chain", help="cfg3: which call patterns to time (per_call, chain)")
-    ap.add_argument("--gemv-engine", type=int, default=0, help="cloak_set_gemv_engine: 0 auto, 1 one-shot, 2 no PDL, 3 exclusive mode (no cooperative launches)")
+    ap.add_argument("--gemv-engine", type=int, default=0, help="cloak_set_gemv_engine: 0 auto, 1 one-shot, 2 no PDL, 3 exclusive mode (no cooperative launches), 4 no fusion of small ops")
     ap.add_argument("--out", default="")
     args = ap.parse_args(argv)
     if args.gemv_engine:

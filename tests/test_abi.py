@@ -63,7 +63,7 @@ def test_argument_checks_without_a_device(C):
         (lambda: C.cloak_set_copy_cache_hint(4), C.CLOAK_ERR_INVALID),
         (lambda: C.cloak_set_gather_engine(2), C.CLOAK_ERR_INVALID),
         (lambda: C.cloak_set_gemm_engine(4), C.CLOAK_ERR_INVALID),
-        (lambda: C.cloak_set_gemv_engine(4), C.CLOAK_ERR_INVALID),
+        (lambda: C.cloak_set_gemv_engine(5), C.CLOAK_ERR_INVALID),
         (lambda: C.cloak_set_trace(12), C.CLOAK_ERR_ALIGN),
         (lambda: C.cloak_load_tensors(1, C.cloak_block_shape(256, 768, 4, 2, 64, C.CLOAK_BF16, 0), None, [(16, 0, 0, "gate")]), C.CLOAK_ERR_INVALID),
         (lambda: C.cloak_gemv_chain_scratch_bytes(None, [], 1), C.CLOAK_ERR_INVALID),

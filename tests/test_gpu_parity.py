@@ -1149,6 +1149,86 @@ def test_moe_decode_through_the_cloaked_pool_equals_the_unpermuted_moe():
             assert O.err_normwise(got, O.moe_f64(x, router, gate, up, down, k)) <= TOL["bf16"], tok
 
 
+@pytest.mark.parametrize("batch", [1, 4, 8, 16])
+def test_gemv_chain_fuses_small_ops_bit_identically(batch):
+    """Ops whose rows are one chunk (the experts' projections of an MoE layer) are dealt out as ONE op per (shape, run) at
+    batch <= 8 (gemv_stream.cu: fusion).  The fused launch must equal the unfused one (cloak_set_gemv_engine(4)) bit for
+    bit, on cloaked and identity pools, for: an MoE-shaped layer (gate_e | up_e with the silu epilogue | down_e after them, an
+    attention block and a router before, two layers back to back), experts listed gate, gate, .., up, up, .. instead, a gate
+    taken from ANOTHER expert's projection (no fusion possible: must still be right), and a big op between the small ones;
+    every down output against the fp64 oracle of silu(gate x) * (up x) through down."""
+    key, seed, block, page = 0x1234, 31, 65536, 2 << 20
+    H, I, E, Q = 512, 256, 6, 1024                     # rows of 1 KiB (gate / up) and 512 B (down): one chunk each
+    shapes = {"q": (Q, H), "o": (H, Q), "router": (16, H), "big": (1024, 4096)}
+    for e in range(E):
+        shapes.update({f"gate{e}": (I, H), f"up{e}": (I, H), f"down{e}": (H, I)})
+    names = list(shapes)
+    Ws = {nm: gen.synth(seed, i, shapes[nm], "bf16") for i, nm in enumerate(names)}
+    offs, total = C.cloak_arena_plan(key, [2 * n * k for n, k in shapes.values()], block)
+    off = dict(zip(names, offs))
+    try:
+        with Pool(total, block, page, key) as pc, Pool(total, block, page, key, C.CLOAK_POOL_IDENTITY) as pi:
+            _load_pool(pc, [(nm, Ws[nm]) for nm in names], offs, "bf16")
+            _load_pool(pi, [(nm, Ws[nm]) for nm in names], offs, "bf16")
+            T = {nm: C.cloak_tensor(off[nm], *shapes[nm], C.CLOAK_BF16, C.CLOAK_ROWMAJOR) for nm in names}
+            Xh = gen.synth(seed + 1, 0, (batch, H), "bf16", kind=gen.KIND_NORMAL)
+            Xq = gen.synth(seed + 1, 1, (batch, Q), "bf16", kind=gen.KIND_NORMAL)
+            Xb = gen.synth(seed + 1, 2, (batch, 4096), "bf16", kind=gen.KIND_NORMAL)
+            xh, xq, xb = bf16_dev_from_bits(Xh), bf16_dev_from_bits(Xq), bf16_dev_from_bits(Xb)
+            z = lambda n: torch.zeros(batch, n, dtype=torch.bfloat16, device="cuda")      # noqa: E731
+
+            def build(variant):
+                ops, outs, downs_of = [], [], []
+                for layer in range(2):
+                    ops += [(T["q"], xh, z(Q), 0), (T["o"], xq, z(H), 0), (T["router"], xh, z(16), 0)]
+                    sel = [0, 2, 3, 5] if layer == 0 else [1, 2, 4, 5]
+                    g = {e: z(I) for e in sel}
+                    u = {e: z(I) for e in sel}
+                    act = {e: z(I) for e in sel}
+                    d = {e: z(H) for e in sel}
+                    if variant == "interleaved":
+                        for e in sel:
+                            ops += [(T[f"gate{e}"], xh, g[e], 0), (T[f"up{e}"], xh, u[e], 0, g[e], act[e])]
+                    elif variant == "grouped":
+                        ops += [(T[f"gate{e}"], xh, g[e], 0) for e in sel] + [(T[f"up{e}"], xh, u[e], 0, g[e], act[e]) for e in sel]
+                    elif variant == "big_between":
+                        for i, e in enumerate(sel):
+                            ops += [(T[f"gate{e}"], xh, g[e], 0)] + ([(T["big"], xb, z(1024), 0)] if i == 1 else []) + [(T[f"up{e}"], xh, u[e], 0, g[e], act[e])]
+                    else:                           # "crossed": up_e's epilogue takes the gate of the NEXT expert's projection
+                        for e in sel:
+                            ops += [(T[f"gate{e}"], xh, g[e], 0)]
+                        for i, e in enumerate(sel):
+                            ops += [(T[f"up{e}"], xh, u[e], 0, g[sel[(i + 1) % len(sel)]], act[e])]
+                    ops += [(T[f"down{e}"], act[e], d[e], 1 if i == 0 else 2) for i, e in enumerate(sel)]
+                    downs_of.append((sel, d, variant))
+                    outs += [t[e] for e in sel for t in (g, u, act, d)]
+                outs += [op[2] for op in ops]
+                return ops, outs, downs_of
+
+            for variant in ("interleaved", "grouped", "big_between", "crossed"):
+                res = {}
+                for eng in (0, 4):
+                    C.cloak_set_gemv_engine(eng)
+                    for pool_name, pool in (("c", pc), ("i", pi)):
+                        ops, outs, downs_of = build(variant)
+                        C.cloak_gemv_chain(pool.h, ops, batch)
+                        C.cloak_gemv_chain(pool.h, ops, batch)           # again over the same outputs: counters back at zero
+                        torch.cuda.synchronize()
+                        res[eng, pool_name] = (outs, downs_of)
+                base = res[4, "c"][0]
+                for k_, (outs, _) in res.items():
+                    assert all(torch.equal(a_, b_) for a_, b_ in zip(outs, base)), (variant, k_)
+                assert any(float(t.float().abs().sum()) > 0 for t in base)
+                # the down outputs against the oracle
+                for sel, d, var in res[0, "c"][1]:
+                    for i, e in enumerate(sel):
+                        ge = sel[(i + 1) % len(sel)] if var == "crossed" else e
+                        ref = O.mlp_f64(Xh, Ws[f"gate{ge}"], Ws[f"up{e}"], Ws[f"down{e}"])       # O9, unrounded intermediates
+                        assert O.err_normwise(d[e].double().cpu().numpy(), ref) <= TOL["bf16"], (variant, e)
+    finally:
+        C.cloak_set_gemv_engine(0)
+
+
 # ------------------------------------------------------------------ randomised chains (shapes, lengths, dependencies)
 @pytest.mark.parametrize("seed", [0, 1, 2, 3])
 def test_gemv_chain_random_lists_equal_single_calls(seed):
