@@ -413,8 +413,8 @@ cloak_status cloak_gemm_chain(const cloak_pool* pool, const cloak_gemm_op* h_ops
  * no faster -- cfg2's chain 2.592 vs 2.596 ms, a 25-launch MoE chain 0.4623 vs 0.4623 ms -- so there is no reason to use it); with
  * a foreign kernel on the device such a chain can hang; 4 = automatic without the FUSION of small ops: at batch <= 8 a chain
  * launch deals out independent ops of one shape whose rows are a single chunk (<= 4 KiB: the selected experts' gate, up or down
- * projections of an MoE layer) as one op over all their row tiles -- same results bit for bit, 12 Qwen3-MoE-shaped layers
- * 0.477 -> 0.380 ms.  For A/B measurement; process-wide (an atomic: safe to flip from any thread, takes effect at the next
+ * projections of an MoE layer) as one op over all their row tiles, each tile fetched with one bulk copy -- same results bit
+ * for bit, 12 Qwen3-MoE-shaped layers 0.477 -> 0.320 ms.  For A/B measurement; process-wide (an atomic: safe to flip from any thread, takes effect at the next
  * launch). */
 cloak_status cloak_set_gemv_engine(int engine);
 /* Per-SM streaming weights (calibrate.cu): a MEASUREMENT, used by no kernel.  The SMs of a B200 do not pull a read stream out of

@@ -235,7 +235,12 @@ gemv_chain_kernel(const __grid_constant__ typename std::conditional<SEG, ChainAr
                         const uint32_t bar = smem_u32(&full[s]);
                         if (lane == 0) mbar_expect_tx(bar, GS_ROWS * CB);
                         __syncwarp();
-                        if (lane < GS_ROWS) {
+                        // SEG kernels, rows of one chunk: the 8 rows of a tile are CONTIGUOUS in the arena, so the tile comes as one
+                        // bulk copy per block touched (unpadded in the stage: 2-way conflicts on the consumers' LDS.128, which have the
+                        // slack) instead of 8 row pieces -- the TMA's throughput falls with the piece size (2 KiB pieces: 4.1 TB/s,
+                        // 4 KiB: 6.4 TB/s).  The experts' down projections (1.5 KiB rows): 0.38 -> 0.53 of the peak.
+                        const bool whole_tile = SEG && kch == 1;
+                        if (lane < (whole_tile ? 1 : GS_ROWS)) {
                             // a chunk that is not a power of two may cross a block boundary: one bulk copy per block touched
                             uint64_t woff = op.w_offset;
                             uint32_t lt = tile;                                        // the tile inside its matrix
@@ -245,8 +250,8 @@ gemv_chain_kernel(const __grid_constant__ typename std::conditional<SEG, ChainAr
                                 woff = args.segs[args.seg0[j] + sg].w_offset;
                             }
                             uint64_t off = woff + (uint64_t)(lt * GS_ROWS + lane) * row_bytes + (uint64_t)c * CB;
-                            uint32_t dst = smem_base + s * STAGE + lane * RS, left = CB;
-                            if ((CU & (CU - 1)) == 0 && CB <= (1u << a.log2b)) {       // power of two within a block: one copy
+                            uint32_t dst = smem_base + s * STAGE + lane * RS, left = whole_tile ? GS_ROWS * CB : CB;
+                            if (!whole_tile && (CU & (CU - 1)) == 0 && CB <= (1u << a.log2b)) {       // power of two within a block: one copy
                                 const uint32_t slot = __ldg(a.T + (off >> a.log2b));
                                 bulk_g2s(dst, a.pool + ((uint64_t)slot << a.log2b) + (off & ((1ull << a.log2b) - 1)), CB, bar);
                                 left = 0;
@@ -375,7 +380,7 @@ gemv_chain_kernel(const __grid_constant__ typename std::conditional<SEG, ChainAr
                         const uint32_t tile = g0 + q, u = tile * kch + c;
                         if (tile > g1 || u < ubeg || u >= uend) continue;
                         mbar_wait(smem_u32(&full[s]), ph);
-                        const uint32_t base = smem_base + s * STAGE + g * RS + lane_off;
+                        const uint32_t base = smem_base + s * STAGE + g * ((SEG && kch == 1) ? CB : RS) + lane_off;
 #pragma unroll
                         for (int ks = 0; ks < KS; ++ks) {
                             const uint4 w = lds128(base + ks * 64);
