@@ -1149,8 +1149,8 @@ def test_moe_decode_through_the_cloaked_pool_equals_the_unpermuted_moe():
             assert O.err_normwise(got, O.moe_f64(x, router, gate, up, down, k)) <= TOL["bf16"], tok
 
 
-@pytest.mark.parametrize("batch", [1, 4, 8, 16])
-def test_gemv_chain_fuses_small_ops_bit_identically(batch):
+@pytest.mark.parametrize("batch,I", [(1, 256), (4, 256), (8, 512), (3, 512), (16, 256)])
+def test_gemv_chain_fuses_small_ops_bit_identically(batch, I):
     """Ops whose rows are one chunk (the experts' projections of an MoE layer) are dealt out as ONE op per (shape, run) at
     batch <= 8 (gemv_stream.cu: fusion).  The fused launch must equal the unfused one (cloak_set_gemv_engine(4)) bit for
     bit, on cloaked and identity pools, for: an MoE-shaped layer (gate_e | up_e with the silu epilogue | down_e after them, an
@@ -1158,7 +1158,8 @@ def test_gemv_chain_fuses_small_ops_bit_identically(batch):
     taken from ANOTHER expert's projection (no fusion possible: must still be right), and a big op between the small ones;
     every down output against the fp64 oracle of silu(gate x) * (up x) through down."""
     key, seed, block, page = 0x1234, 31, 65536, 2 << 20
-    H, I, E, Q = 512, 256, 6, 1024                     # rows of 1 KiB (gate / up) and 512 B (down): one chunk each
+    H, E, Q = 512, 6, 1024          # rows of 1 KiB (gate / up) and 512 B (down, I = 256): one chunk each, downs in launches of their
+                                    # own; I = 512: one chunk size for all three -- the fused downs wait for the fused ups INSIDE a launch
     shapes = {"q": (Q, H), "o": (H, Q), "router": (16, H), "big": (1024, 4096)}
     for e in range(E):
         shapes.update({f"gate{e}": (I, H), f"up{e}": (I, H), f"down{e}": (H, I)})
