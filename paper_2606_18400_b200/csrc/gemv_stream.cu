@@ -611,12 +611,17 @@ static bool plan_fusion(const cloak_gemv_op* ops, uint32_t n, int cu, FusedPlan&
         pos_of[j] = cnt[f]++;
     }
     if (!any) return false;
-    // gate epilogues: producer in this launch -> same position of an earlier fused op of the same size
+    // gate epilogues: producer in this launch -> same position of ONE earlier fused op of the same size for the whole group (the
+    // group then copies that op's rotation, gemv_stream_launch: same rows, same CTA)
+    uint32_t pgrp[GS_MAX_OPS];
+    for (uint32_t f = 0; f < nf; ++f) pgrp[f] = 0xffffffffu;
     for (uint32_t j = 0; j < n; ++j) {
         if (!ops[j].d_gate) continue;
         for (uint32_t k = 0; k < n; ++k) {
             if (ops[k].d_y != ops[j].d_gate) continue;
             if (k >= j || grp_of[k] >= grp_of[j] || pos_of[k] != pos_of[j] || cnt[grp_of[k]] != cnt[grp_of[j]]) return false;
+            if (pgrp[grp_of[j]] == 0xffffffffu) pgrp[grp_of[j]] = grp_of[k];
+            if (pgrp[grp_of[j]] != grp_of[k]) return false;
         }
     }
     fp.nf = nf;

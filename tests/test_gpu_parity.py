@@ -1231,23 +1231,25 @@ def test_gemv_chain_fuses_small_ops_bit_identically(batch, I):
 
 
 # ------------------------------------------------------------------ randomised chains (shapes, lengths, dependencies)
-@pytest.mark.parametrize("seed", [0, 1, 2, 3])
+@pytest.mark.parametrize("seed", [0, 1, 2, 3, 10, 11, 12, 13, 14, 15, 16, 17])
 def test_gemv_chain_random_lists_equal_single_calls(seed):
     """Random op lists (1..60 ops, rows of 512 B .. 28 KiB, N from 16 to 4 096, mixed chunk sizes -> several launches,
     random `after` 0/1/2 with real data dependencies, random gate epilogues): bit-identical to the same ops issued one
     cloak_gemv / cloak_silu_mul at a time, and every op fed by a generator vector against the fp64 oracle."""
     rng = np.random.default_rng(100 + seed)
     key, block, page = 0x1234, 65536, 2 << 20
-    batch = int(rng.choice([1, 3, 8, 9, 16]))
-    n_w = 6
-    shapes = [(int(rng.choice([16, 48, 256, 1024, 4096])), int(rng.choice([256, 512, 768, 2048, 3584, 14336]))) for _ in range(n_w)]
+    small = seed >= 10        # seeds >= 10: few tensors, rows of one chunk, batch <= 8 -- the launch planner fuses whatever it may
+    batch = int(rng.choice([1, 3, 8] if small else [1, 3, 8, 9, 16]))
+    n_w = 3 if small else 6
+    shapes = [(int(rng.choice([16, 48, 256, 512] if small else [16, 48, 256, 1024, 4096])),
+               int(rng.choice([256, 512, 1024, 2048] if small else [256, 512, 768, 2048, 3584, 14336]))) for _ in range(n_w)]
     Ws = [gen.synth(seed, i, shp, "bf16") for i, shp in enumerate(shapes)]
     offs, total = C.cloak_arena_plan(key, [2 * n * k for n, k in shapes], block)
     with Pool(total, block, page, key) as p:
         _load_pool(p, [(f"w{i}", w) for i, w in enumerate(Ws)], offs, "bf16")
         T = [C.cloak_tensor(o, n, k, C.CLOAK_BF16, C.CLOAK_ROWMAJOR) for (n, k), o in zip(shapes, offs)]
         X0 = {k: bf16_dev_from_bits(gen.synth(seed + 50, k, (batch, k), "bf16", kind=gen.KIND_NORMAL)) for k in {k for _, k in shapes}}
-        n_ops = int(rng.integers(1, 61))
+        n_ops = int(rng.integers(20, 61)) if small else int(rng.integers(1, 61))
         ops_c, ops_s, outs_c, outs_s, last_dep = [], [], [], [], False
         for j in range(n_ops):
             wi = int(rng.integers(0, n_w))
