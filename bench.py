@@ -551,7 +551,10 @@ def run_cloak(args):
         if "cfg4" in want:
             line["cfg4"] = workloads.bench_cfg4(clocks, args.min_seconds / 2)
             torch.cuda.empty_cache()
-        line["gpu_launches_other_configs"] = int(sum(line[k]["gpu_launches"] for k in ("cfg2", "cfg3", "cfg4") if k in line))
+        if "moe" in want:
+            line["moe"] = workloads.bench_moe(clocks, args.min_seconds / 2)
+            torch.cuda.empty_cache()
+        line["gpu_launches_other_configs"] = int(sum(line[k]["gpu_launches"] for k in ("cfg2", "cfg3", "cfg4", "moe") if k in line))
     if clocks is not None:
         clocks.stop()
     if not args.no_cpu_baseline and world == 1:      # (the oracle is timed on rank 0 at N = 1 only)
@@ -586,8 +589,8 @@ def main():
                     help="cfg1 (default) is the headline step; cfg2-4 are the other BASELINE.json configs "
                          "(paper_2606_18400_b200/workloads.py), each printing its own JSON line")
     ap.add_argument("--reps", type=int, default=10, help="repetitions per measurement for --workload cfg2-4")
-    ap.add_argument("--configs", default="cfg1,cfg2,cfg3,cfg4",
-                    help="what the line carries besides the cfg1 step (`value`): cfg2, cfg3, cfg4 blocks (BASELINE.json configs[2..4]); "
+    ap.add_argument("--configs", default="cfg1,cfg2,cfg3,cfg4,moe",
+                    help="what the line carries besides the cfg1 step (`value`): cfg2, cfg3, cfg4 blocks (BASELINE.json configs[2..4]) and the MoE decode chain (NEXT-4); "
                          "`--configs cfg1` for the step alone.  N > 1 replicas run the step alone.")
     ap.add_argument("--min-seconds", type=float, default=1.0, help="minimum length of each timed loop of the cfg2-4 blocks")
     ap.add_argument("--no-ab", action="store_true", help="skip the isolated native / per-call / cuBLAS A/B runs and the e2e leg (for ncu launch lists of the step alone)")

@@ -482,18 +482,13 @@ def run_cfg3(args):
 
 
 # ------------------------------------------------------------------------------------------ MoE (NEXT-4)
-def run_moe(args):
-    """Qwen3-30B-A3B-shaped sparse layers (hidden 2048, 128 experts of 768, top-8; attention 32 q / 4 kv heads): expert
-    permutation + shuffle at load, then the batch-1 decode chain of every layer -- q, k, v, o, router, and gate | up | down
-    of 8 (seeded) selected experts -- as one cloak_gemv_chain, cloaked vs identity table.  --layers picks the depth
-    (default 12 of the model's 48: 15 GB per pool)."""
-    torch, C, synth_cuda, gen = _imports()
+def _moe_model(torch, C, synth_cuda, gen, L):
+    """Pools (cloaked, identity) holding L Qwen3-30B-A3B-shaped sparse layers, loaded generator -> S5 (heads; experts) ->
+    shuffle_many layer by layer; the tensors and what the load cost."""
     c = gen.CONFIGS[5]
-    L = int(args.layers or 12)
-    H, I, E, K = c["hidden"], c["inter"], c["n_experts"], c["top_k"]
+    H, I, E = c["hidden"], c["inter"], c["n_experts"]
     Q, KV = c["n_q"] * c["head_dim"], c["n_kv"] * c["head_dim"]
-    peak, peak_kind = hbm_peak()
-    names, sizes = [], []
+    names = []
     for l in range(L):
         for nm, n, k in (("q", Q, H), ("k", KV, H), ("v", KV, H), ("o", H, Q), ("router", E, H)):
             names.append((l, nm, n, k))
@@ -505,15 +500,13 @@ def run_moe(args):
     T = {(l, nm): C.cloak_tensor(o, n, k, C.CLOAK_BF16, C.CLOAK_ROWMAJOR) for (l, nm, n, k), o in zip(names, offs)}
     pc = C.cloak_pool_create(0, total, c["block"], c["page"], c["key"])
     pn = C.cloak_pool_create(0, total, c["block"], c["page"], c["key"], C.CLOAK_POOL_IDENTITY)
-    launches0 = C.cloak_launch_count()
+    m = {"c": c, "L": L, "pc": pc, "pn": pn, "T": T, "total": total, "perm_ms": 0.0}
     try:
-        # ---- load: generator -> S5 (heads; experts) -> shuffle_many, layer by layer
         t0 = time.perf_counter()
         att = {nm: torch.empty(n, k, dtype=torch.bfloat16, device="cuda") for nm, n, k in (("q", Q, H), ("k", KV, H), ("v", KV, H), ("o", H, Q))}
         att_p = {nm: torch.empty_like(t) for nm, t in att.items()}
         raw = [torch.empty(s_, dtype=torch.bfloat16, device="cuda") for s_ in ((E, H), (E, I, H), (E, I, H), (E, H, I))]
         prm = [torch.empty_like(t) for t in raw]
-        perm_ms = 0.0
         for l in range(L):
             for i, nm in enumerate(att):
                 synth_cuda.fill(att[nm], c["seed"], l * 8 + i)
@@ -533,39 +526,60 @@ def run_moe(args):
             for p in (pc, pn):
                 C.cloak_shuffle_many(p, ts, os_, [t.numel() * 2 for t in ts])
             torch.cuda.synchronize()
-            perm_ms += e0.elapsed_time(e1)
-        load_s = time.perf_counter() - t0
+            m["perm_ms"] += e0.elapsed_time(e1)
+        m["load_s"] = time.perf_counter() - t0
+    except BaseException:
+        torch.cuda.synchronize()
+        C.cloak_pool_destroy(pc)
+        C.cloak_pool_destroy(pn)
+        raise
+    return m
 
-        # ---- decode chain: fixed synthetic inputs, 8 seeded experts per layer
-        xh = synth_cuda.fill(torch.empty(1, H, dtype=torch.bfloat16, device="cuda"), c["seed"] + 100, 0, kind=gen.KIND_NORMAL)
-        xa = synth_cuda.fill(torch.empty(1, Q, dtype=torch.bfloat16, device="cuda"), c["seed"] + 100, 1, kind=gen.KIND_NORMAL)
-        rng = np.random.default_rng(c["seed"])
-        sel = [sorted(int(e) for e in rng.choice(E, K, replace=False)) for _ in range(L)]
-        read_bytes = 0
 
-        def build(tag):
-            nonlocal read_bytes
-            ops, outs, rb = [], [], 0
-            z = lambda n: torch.zeros(1, n, dtype=torch.bfloat16, device="cuda")       # noqa: E731
-            for l in range(L):
-                y = {nm: z(n) for nm, n in (("q", Q), ("k", KV), ("v", KV), ("o", H), ("router", E))}
-                ops += [(T[l, nm], xa if nm == "o" else xh, y[nm], 0) for nm in y]
-                rb += 2 * (2 * Q * H + 2 * KV * H + E * H)
-                downs = []
-                for i, e in enumerate(sel[l]):
-                    yg, yu, act, yd = z(I), z(I), z(I), z(H)
-                    ops += [(T[l, f"gate{e}"], xh, yg, 0), (T[l, f"up{e}"], xh, yu, 0, yg, act)]
-                    downs.append((T[l, f"down{e}"], act, yd, 1 if i == 0 else 2))
-                    outs += [yg, yu, act, yd]
-                    rb += 2 * 3 * I * H
-                ops += downs
-                outs += list(y.values())
-            read_bytes = rb
-            return C.cloak_gemv_ops(ops), outs
+def _moe_chain(torch, C, synth_cuda, gen, m, batch=1):
+    """The decode chain of every layer of _moe_model -- q, k, v, o, router, and gate | up (silu epilogue) | down of 8 seeded
+    experts -- on fixed synthetic inputs: (marshalled ops, output tensors, weight bytes read)."""
+    c, L, T = m["c"], m["L"], m["T"]
+    H, I, E, K = c["hidden"], c["inter"], c["n_experts"], c["top_k"]
+    Q, KV = c["n_q"] * c["head_dim"], c["n_kv"] * c["head_dim"]
+    xh = synth_cuda.fill(torch.empty(batch, H, dtype=torch.bfloat16, device="cuda"), c["seed"] + 100, 0, kind=gen.KIND_NORMAL)
+    xa = synth_cuda.fill(torch.empty(batch, Q, dtype=torch.bfloat16, device="cuda"), c["seed"] + 100, 1, kind=gen.KIND_NORMAL)
+    rng = np.random.default_rng(c["seed"])
+    sel = [sorted(int(e) for e in rng.choice(E, K, replace=False)) for _ in range(L)]
+    ops, outs, rb = [], [xh, xa], 0
+    z = lambda n: torch.zeros(batch, n, dtype=torch.bfloat16, device="cuda")       # noqa: E731
+    for l in range(L):
+        y = {nm: z(n) for nm, n in (("q", Q), ("k", KV), ("v", KV), ("o", H), ("router", E))}
+        ops += [(T[l, nm], xa if nm == "o" else xh, y[nm], 0) for nm in y]
+        rb += 2 * (2 * Q * H + 2 * KV * H + E * H)
+        downs = []
+        for i, e in enumerate(sel[l]):
+            yg, yu, act, yd = z(I), z(I), z(I), z(H)
+            ops += [(T[l, f"gate{e}"], xh, yg, 0), (T[l, f"up{e}"], xh, yu, 0, yg, act)]
+            downs.append((T[l, f"down{e}"], act, yd, 1 if i == 0 else 2))
+            outs += [yg, yu, act, yd]
+            rb += 2 * 3 * I * H
+        ops += downs
+        outs += list(y.values())
+    return C.cloak_gemv_ops(ops), outs, rb
 
+
+def run_moe(args):
+    """Qwen3-30B-A3B-shaped sparse layers (hidden 2048, 128 experts of 768, top-8; attention 32 q / 4 kv heads): expert
+    permutation + shuffle at load, then the batch-1 decode chain of every layer -- q, k, v, o, router, and gate | up | down
+    of 8 (seeded) selected experts -- as one cloak_gemv_chain, cloaked vs identity table.  --layers picks the depth
+    (default 12 of the model's 48: 15 GB per pool)."""
+    torch, C, synth_cuda, gen = _imports()
+    L = int(args.layers or 12)
+    peak, peak_kind = hbm_peak()
+    launches0 = C.cloak_launch_count()
+    m = _moe_model(torch, C, synth_cuda, gen, L)
+    c, pc, pn = m["c"], m["pc"], m["pn"]
+    H, I, E = c["hidden"], c["inter"], c["n_experts"]
+    try:
         res, outs = {}, {}
         for pool_name, pool in (("cloaked", pc), ("native", pn)):
-            ops, outs[pool_name] = build(pool_name)
+            ops, outs[pool_name], read_bytes = _moe_chain(torch, C, synth_cuda, gen, m)
             fn = lambda: C.cloak_gemv_chain(pool, ops, 1)        # noqa: E731
             med, mn = time_gpu(torch, fn, args.reps)
             gmed, gmn = time_gpu(torch, graphed(torch, fn), args.reps)
@@ -578,9 +592,10 @@ def run_moe(args):
         C.cloak_pool_destroy(pc)
         C.cloak_pool_destroy(pn)
     return {"workload": "moe: Qwen3-30B-A3B-shaped sparse layers, %d of 48 layers, 128 experts, top-8, bf16, 64 KiB blocks" % L,
-            "arena_bytes": total, "layers": L, "reps": args.reps, "hbm_peak_gbs": peak, "hbm_peak_kind": peak_kind,
-            "load_s": load_s, "permute_experts_ms_per_layer": perm_ms / L,
-            "permute_experts_gbs": 2 * 2 * (E * H + 3 * E * I * H) / (perm_ms / L) / 1e6,
+            "arena_bytes": m["total"], "layers": L, "reps": args.reps, "hbm_peak_gbs": peak, "hbm_peak_kind": peak_kind,
+            "load_s": m["load_s"], "permute_experts_ms_per_layer": m["perm_ms"] / L,
+            "permute_experts_gbs": 2 * 2 * (E * H + 3 * E * I * H) / (m["perm_ms"] / L) / 1e6,
+            "gemv_engine": int(getattr(args, "gemv_engine", 0)),
             "decode_chain": res, "decode_read_bytes": read_bytes, "decode_read_bytes_full_model": read_bytes // L * 48,
             "tokens_per_s_extrapolated_48_layers": 1e3 / (res["cloaked"]["graph"]["ms"] / L * 48),
             "cloaked_vs_native_overhead_pct": ov, "cloaked_identical_to_native": bool(identical),
@@ -798,6 +813,47 @@ def bench_cfg3(sampler, min_s=1.0, layers=None, batches=(32, 128), depths=(8, 64
                 del g, ys
             del X
             torch.cuda.empty_cache()
+    finally:
+        torch.cuda.synchronize()
+        C.cloak_pool_destroy(pc)
+        C.cloak_pool_destroy(pn)
+    out["gpu_launches"] = C.cloak_launch_count() - launches0
+    return out
+
+
+def bench_moe(sampler, min_s=0.5, layers=12):
+    """The MoE decode chain for the bench line: `layers` Qwen3-30B-A3B-shaped sparse layers, batch 1, graph
+    replay, cloaked vs identity table, and alternated with the same chain captured without the fusion of the experts' ops."""
+    torch, C, synth_cuda, gen = _imports()
+    peak, _ = hbm_peak()
+    launches0 = C.cloak_launch_count()
+    m = _moe_model(torch, C, synth_cuda, gen, layers)
+    c, pc, pn = m["c"], m["pc"], m["pn"]
+    H, I, E = c["hidden"], c["inter"], c["n_experts"]
+    out = {"workload": "moe: Qwen3-30B-A3B-shaped sparse layers, %d of 48 layers, 128 experts, top-8, bf16, 64 KiB blocks" % layers,
+           "arena_bytes": m["total"], "pool_map_ms": {"cloaked": C.cloak_pool_map_ms(pc), "identity": C.cloak_pool_map_ms(pn)},
+           "generate_permute_load_s": m["load_s"], "permute_experts_ms_per_layer": m["perm_ms"] / layers,
+           "permute_experts_gbs": 2 * 2 * (E * H + 3 * E * I * H) / (m["perm_ms"] / layers) / 1e6}
+    try:
+        g, outs = {}, {}
+        for name, pool in (("cloaked", pc), ("native", pn)):
+            ops, outs[name], read_bytes = _moe_chain(torch, C, synth_cuda, gen, m)
+            g[name] = (_graph(torch, lambda: C.cloak_gemv_chain(pool, ops, 1)), ops)
+        C.cloak_set_gemv_engine(4)                     # the same chain, every expert projection an op of its own
+        try:
+            ops_u, outs["unfused"], _ = _moe_chain(torch, C, synth_cuda, gen, m)
+            gu = _graph(torch, lambda: C.cloak_gemv_chain(pc, ops_u, 1))
+        finally:
+            C.cloak_set_gemv_engine(0)
+        d = measure(torch, sampler, peak, read_bytes, g["cloaked"][0].replay, g["native"][0].replay, min_s,
+                    extra={"call": "cloak_gemv_chain, %d ops, batch 1, CUDA-graph replay" % len(g["cloaked"][1])})
+        tf, tu = ab_loop(torch, g["cloaked"][0].replay, gu.replay, int(min(max(20, np.ceil(0.5 * min_s * 1e3 / d["t_ms_median"])), 5000)))
+        d.update({"t_fused_ms_alternated": tf, "t_unfused_ms": tu, "fusion_gain_pct": (tu - tf) / tu * 100.0,
+                  "unfused_frac_measured": read_bytes / tu / 1e6 / peak,
+                  "tokens_per_s_extrapolated_48_layers": 1e3 / (d["t_ms_median"] / layers * 48),
+                  "cloaked_identical_to_native": bool(all(torch.equal(a_, b_) for a_, b_ in zip(outs["cloaked"], outs["native"]))),
+                  "fused_identical_to_unfused": bool(all(torch.equal(a_, b_) for a_, b_ in zip(outs["cloaked"], outs["unfused"])))})
+        out["decode_chain"] = d
     finally:
         torch.cuda.synchronize()
         C.cloak_pool_destroy(pc)
