@@ -33,6 +33,11 @@
 //     same CTA wrote those very elements, so no wait is needed -- and gate/up -> down costs no separate pass.
 //   * programmatic dependent launch: the grid may start while its stream predecessor drains; the producer
 //     streams W (immutable during decode) ahead of griddepcontrol.wait, everything else waits.
+//   * fusion of small ops (batch <= 8; plan_fusion, the SEG = true instantiations): independent ops of one shape whose rows are a
+//     single chunk -- the selected experts' projections of an MoE layer, 96 units for 148 CTAs each -- are dealt out as ONE op over
+//     the concatenation of their row tiles (a segment table in the kernel parameters), each tile fetched with one bulk copy
+//     (its 8 rows are contiguous in the arena).  Same sums in the same order: bit-identical to the unfused launch.
+//   * cloak_gemv_static (end of this file): the same kernel with its scratch in a fixed static device array -- allocates nothing.
 #include <cuda_bf16.h>
 #include <type_traits>
 #include "common.cuh"
