@@ -106,7 +106,7 @@ constexpr int GS_CONSUMERS = 8;                       // consumer warps
 // Warps ahead of the consumers.  batch <= 8: the producer warp alone.  batch 9..16: a whole warpgroup (producer + three
 // warps that retire at once), so that the register file can be re-split per warpgroup with setmaxnreg: the producer
 // group drops to 40 registers per thread, the two consumer groups rise to 232 -- room for a second set of X fragments.
-constexpr int gs_lead_warps(int nt) { return nt == 2 ? 4 : 1; }
+constexpr int gs_lead_warps(int nt) { return nt == 2 ? 4 : 2; }      // warp 0 = producer, warp 1 = helper (see GS_NREC)
 constexpr int gs_threads(int nt) { return 32 * (gs_lead_warps(nt) + GS_CONSUMERS); }
 constexpr int GS_ROWS = 8;                            // weight rows per tile (the MMA's N)
 constexpr int GS_PAD = 64;                            // bytes of padding per staged row (conflict-free LDS.128)
@@ -120,6 +120,15 @@ constexpr int gs_tg(int) { return 8; }
 constexpr int gs_nacc(int) { return 2; }
 constexpr int GS_TGR = 4;                             // row tiles reduced across warps per shared-memory pass
 constexpr int GS_MAX_STAGES = 12;
+// The HELPER warp.  Everything a CTA does at device scope for other CTAs -- publishing the partial of a cut head tile (a release),
+// finishing the cut tail tile it owns (an acquire-wait for the other contributors, their partials, the stores), reporting an op
+// done (a release) -- costs an L2 round trip or more, and while the consumer warps sit in it no ring stage is handed back, so no
+// new copy is issued: measured on the cfg1 layer, 7 ops, batch 1, those two epilogues cost 7.8 of 80.9 us (one op of the same
+// bytes: 70.0 us).  The consumers therefore only POST such work -- a record in a small shared-memory queue (mbarrier full / empty
+// per slot; the tail tile's own sums travel in the slot) -- and go on streaming; warp 1 executes the records in order.
+constexpr int GS_NREC = 8;
+enum { REC_PUBLISH = 0, REC_TAIL = 1, REC_SIGNAL = 2, REC_EXIT = 3 };
+struct HelperRec { uint32_t kind, j, tile, nc, vr; };
 constexpr uint32_t gs_stages(int cu) {                // cu = chunk bytes / 512; ~192 KiB of weights in flight per SM
     return 196608u / (GS_ROWS * cu * 512u) > GS_MAX_STAGES ? GS_MAX_STAGES : 196608u / (GS_ROWS * cu * 512u);
 }
@@ -199,7 +208,9 @@ gemv_chain_kernel(const __grid_constant__ typename std::conditional<SEG, ChainAr
     extern __shared__ __align__(128) unsigned char smem[];
     __shared__ __align__(8) uint64_t full[NST], empty[NST];
     __shared__ float red[GS_CONSUMERS][GS_TGR][NT * 64];      // [warp][tile][batch m][row r]
-    __shared__ float own[NT * 64];                             // this CTA's own sums of the cut tile it owns
+    __shared__ float own[GS_NREC][NT * 64];                    // per helper record: this CTA's own sums of the cut tile it owns
+    __shared__ HelperRec rec[GS_NREC];
+    __shared__ __align__(8) uint64_t rec_full[GS_NREC], rec_empty[GS_NREC];
 
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     if (threadIdx.x == 0) {
@@ -208,13 +219,80 @@ gemv_chain_kernel(const __grid_constant__ typename std::conditional<SEG, ChainAr
             mbar_init(smem_u32(&full[s]), 1);
             mbar_init(smem_u32(&empty[s]), GS_CONSUMERS);
         }
+#pragma unroll
+        for (int r = 0; r < GS_NREC; ++r) {
+            mbar_init(smem_u32(&rec_full[r]), 1);
+            mbar_init(smem_u32(&rec_empty[r]), 1);
+        }
         fence_barrier_init();
     }
     __syncthreads();
     const uint32_t smem_base = smem_u32(smem);
 
+    // Every Y element is stored exactly once, by the CTA that owns its row tile (its consumers, or its helper for a cut tail tile).
+    // The gate op had the same (N, K), hence the same split: gate[idx] was stored by this CTA -- by the same role -- before.
+    // store_out(j, tile, m, r, sum): batch row m, row r of row tile `tile` of op j.
+    auto store_out = [&](uint32_t j, uint32_t tile, uint32_t m, uint32_t r, float sum) {
+        const ChainOp& op = a.ops[j];
+        const __nv_bfloat16 v = __float2bfloat16_rn(sum);
+        if constexpr (SEG) {
+            const uint32_t sg = tile / args.tps[j];
+            const ChainSeg& sgm = args.segs[args.seg0[j] + sg];
+            const size_t idx = (size_t)m * op.N + (tile - sg * args.tps[j]) * GS_ROWS + r;
+            sgm.y[idx] = v;
+            if (sgm.gate) sgm.act[idx] = silu_mul_bf16(ld_coherent_u16(sgm.gate + idx), v);
+        } else {
+            const size_t idx = (size_t)m * op.N + tile * GS_ROWS + r;
+            op.y[idx] = v;
+            if (op.gate) op.act[idx] = silu_mul_bf16(ld_coherent_u16(op.gate + idx), v);
+        }
+    };
+
     if (warp < LEAD) {
         if (NT == 2) asm volatile("setmaxnreg.dec.sync.aligned.u32 56;");
+        if (warp == 1) {
+            // -------------------------------------------------------- helper: the CTA's device-scope work, in the order posted
+            grid_dep_wait();                                 // counters, partials and Y belong to stream order
+            const uint32_t nout = a.batch * GS_ROWS;
+            for (uint32_t hs = 0;; ++hs) {
+                const uint32_t slot = hs % GS_NREC;
+                mbar_wait(smem_u32(&rec_full[slot]), (hs / GS_NREC) & 1);
+                const HelperRec r = rec[slot];
+                if (r.kind == REC_PUBLISH) {
+                    // the consumers' partial stores are ordered before this by their barrier and the slot's mbarrier: the release is cumulative
+                    if (lane == 0) red_release_add(a.counters + a.ops[r.j].tile_base + r.tile, 1u);
+                } else if (r.kind == REC_TAIL) {
+                    // owner of the tail tile: wait for the other contributors (the CTAs after this one), add in CTA order
+                    uint32_t* cnt = a.counters + a.ops[r.j].tile_base + r.tile;
+                    if (lane == 0) {
+                        while (ld_acquire(cnt) != r.nc) __nanosleep(32);
+                        *cnt = 0;                                   // self-reset for the next launch
+                    }
+                    __syncwarp();
+                    const float* mypart = a.part + ((size_t)r.j * gridDim.x + r.vr) * nout;
+                    for (uint32_t i = lane; i < nout; i += 32) {
+                        float sum = own[slot][i];
+                        for (uint32_t q = 1; q <= r.nc; ++q) sum += __ldcg(mypart + (size_t)q * nout + i);
+                        store_out(r.j, r.tile, i / GS_ROWS, i % GS_ROWS, sum);
+                    }
+                } else if (r.kind == REC_SIGNAL) {
+                    // this CTA is done with op j and everything before it (Y stores: the consumers' before their barrier, the tails' above)
+                    __syncwarp();
+                    if (lane == 0) red_release_add(a.opsync + r.j, 1u);
+                } else {
+                    // the arrival counters are reset for the next launch by the last CTA to get here (nobody reads them any more)
+                    if (a.any_signal && lane == 0) {
+                        if (atomicAdd(a.opsync + GS_MAX_OPS, 1u) == gridDim.x - 1) {
+                            for (uint32_t j = 0; j < a.nops; ++j) a.opsync[j] = 0;
+                            a.opsync[GS_MAX_OPS] = 0;
+                        }
+                    }
+                    return;
+                }
+                __syncwarp();
+                if (lane == 0) mbar_arrive(smem_u32(&rec_empty[slot]));
+            }
+        }
         if (warp > 0) return;
         // ------------------------------------------------------------ producer: straight through the chain
         // The table is immutable after cloak_pool_create; the weights may have been written by the preceding
@@ -296,6 +374,26 @@ gemv_chain_kernel(const __grid_constant__ typename std::conditional<SEG, ChainAr
     grid_dep_wait();
     if (ctid == 0) grid_dep_launch();
 
+    // records for the helper warp: every consumer thread counts them (the conditions are uniform), thread 0 waits for a slot
+    // to be free and fills it.  reserve() must be followed by a consumer barrier before anybody else touches own[slot].
+    uint32_t rs = 0;
+    auto reserve = [&]() {
+        const uint32_t slot = rs % GS_NREC;
+        if (ctid == 0 && rs >= (uint32_t)GS_NREC) mbar_wait(smem_u32(&rec_empty[slot]), ((rs / GS_NREC) - 1) & 1);
+        ++rs;
+        return slot;
+    };
+    auto post = [&](uint32_t slot, uint32_t kind, uint32_t j, uint32_t tile, uint32_t nc, uint32_t vr) {
+        if (ctid == 0) {                     // (behind a consumer barrier: everything the record refers to has been written)
+            rec[slot].kind = kind;
+            rec[slot].j = j;
+            rec[slot].tile = tile;
+            rec[slot].nc = nc;
+            rec[slot].vr = vr;
+            mbar_arrive(smem_u32(&rec_full[slot]));
+        }
+    };
+
     uint32_t s = 0, ph = 0;
     for (uint32_t j = 0; j < a.nops; ++j) {
         const ChainOp& op = a.ops[j];
@@ -320,24 +418,6 @@ gemv_chain_kernel(const __grid_constant__ typename std::conditional<SEG, ChainAr
             const uint16_t* x0 = op.x + (size_t)g * op.K + lane_off / 2;            // (SEG: set per group, from its segment)
             const uint16_t* x1 = op.x + (size_t)(g + 8) * op.K + lane_off / 2;
             float* mypart = a.part + ((size_t)j * gridDim.x + vr) * nout;
-            // Every Y element is stored exactly once, by the CTA that owns its row tile.  The gate op had the same
-            // (N, K), hence the same split: gate[idx] was stored by this CTA, before consumer barriers passed since.
-            // store_y(tile, m, r, sum): batch row m, row r of row tile `tile` of the op.
-            auto store_y = [&](uint32_t tile, uint32_t m, uint32_t r, float sum) {
-                const __nv_bfloat16 v = __float2bfloat16_rn(sum);
-                if constexpr (SEG) {
-                    const uint32_t sg = tile / args.tps[j];
-                    const ChainSeg& sgm = args.segs[args.seg0[j] + sg];
-                    const size_t idx = (size_t)m * op.N + (tile - sg * args.tps[j]) * GS_ROWS + r;
-                    sgm.y[idx] = v;
-                    if (sgm.gate) sgm.act[idx] = silu_mul_bf16(ld_coherent_u16(sgm.gate + idx), v);
-                } else {
-                    const size_t idx = (size_t)m * op.N + tile * GS_ROWS + r;
-                    op.y[idx] = v;
-                    if (op.gate) op.act[idx] = silu_mul_bf16(ld_coherent_u16(op.gate + idx), v);
-                }
-            };
-
             // X fragments of one (group, chunk) phase.  Batch <= 8 re-reads them mostly from L1; batch 9..16 (X is up to
             // 16 x K x 2 B, more than the L1 left beside the ring) pays an L2 round trip per phase, so there the next
             // phase's fragments are fetched one phase ahead (PF) into a second register set (see gs_lead_warps).
@@ -410,6 +490,13 @@ gemv_chain_kernel(const __grid_constant__ typename std::conditional<SEG, ChainAr
                 for (int sb = 0; sb < GS_TG / GS_TGR; ++sb) {
                     const uint32_t tb = g0 + sb * GS_TGR;
                     if (tb <= g1) {
+                        // what this pass hands to the helper: the head tile's partial to publish (early in the range: the tile's
+                        // owner needs it only at its end) and / or the tail tile to finish -- slots in that order
+                        const bool pub_here = cut_head && tb == tile_lo;
+                        const bool tail_here = cut_tail && tile_hi >= tb && tile_hi < tb + GS_TGR && tile_hi <= g1;
+                        uint32_t pslot = 0, tslot = 0;
+                        if (pub_here) pslot = reserve();
+                        if (tail_here) tslot = reserve();
 #pragma unroll
                         for (int jj = 0; jj < GS_TGR; ++jj) {
                             const int q = sb * GS_TGR + jj;
@@ -433,46 +520,25 @@ gemv_chain_kernel(const __grid_constant__ typename std::conditional<SEG, ChainAr
 #pragma unroll
                             for (int w = 1; w < GS_CONSUMERS; ++w) sum += red[w][jj][rem];
                             if (tile == tile_lo && cut_head) __stcg(mypart + m * GS_ROWS + r, sum);
-                            else if (tile == tile_hi && cut_tail) own[rem] = sum;
-                            else store_y(tile, m, r, sum);
+                            else if (tile == tile_hi && cut_tail) own[tslot][rem] = sum;
+                            else store_out(j, tile, m, r, sum);
                         }
-                        if (cut_head && tb == tile_lo) {
-                            // publish the head partial now, early in the range: the tile's owner needs it only at its end
-                            __threadfence();
-                            consumer_bar();
-                            if (ctid == 0) red_release_add(a.counters + op.tile_base + tile_lo, 1u);
-                        } else {
-                            consumer_bar();      // red[] is reused by the next pass
-                        }
+                        consumer_bar();          // red[] is reused by the next pass; the partial / own sums are complete
+                        if (pub_here) post(pslot, REC_PUBLISH, j, tile_lo, 0, 0);
+                        // (the other contributors of the tail tile are the CTAs after this one that hold units of it)
+                        if (tail_here) post(tslot, REC_TAIL, j, tile_hi, (tile_hi * kch + kch - 1) / per - vr, vr);
                     }
                 }
             }
 
-            if (cut_tail) {
-                // owner of the tail tile: wait for the other contributors (CTAs after this one), add in CTA order
-                const uint32_t nc = (tile_hi * kch + kch - 1) / per - vr;
-                uint32_t* cnt = a.counters + op.tile_base + tile_hi;
-                if (ctid == 0) {
-                    while (ld_acquire(cnt) != nc) __nanosleep(32);
-                    *cnt = 0;                                   // self-reset for the next launch
-                }
-                consumer_bar();
-                for (uint32_t i = ctid; i < nout; i += GS_CONSUMERS * 32) {
-                    float sum = own[i];
-                    for (uint32_t q = 1; q <= nc; ++q) sum += __ldcg(mypart + (size_t)q * nout + i);
-                    store_y(tile_hi, i / GS_ROWS, i % GS_ROWS, sum);
-                }
-                consumer_bar();                                  // own[] is reused by the next op
-            }
         }
 
         if (op.flags & OP_SIGNAL) {
-            // report: this CTA is done with op j and everything before it (its Y stores are ordered by the barrier)
+            // report: this CTA is done with op j and everything before it -- through the helper, behind the tails it still holds
+            // (the consumers' Y stores are ordered before the record by the barrier)
+            const uint32_t sslot = reserve();
             consumer_bar();
-            if (ctid == 0) {
-                __threadfence();
-                red_release_add(a.opsync + j, 1u);
-            }
+            post(sslot, REC_SIGNAL, j, 0, 0, 0);
         }
     }
     if (a.trace && ctid == 0) {
@@ -480,13 +546,7 @@ gemv_chain_kernel(const __grid_constant__ typename std::conditional<SEG, ChainAr
         a.trace[4 * blockIdx.x + 1] = t_start;
         a.trace[4 * blockIdx.x + 3] = global_ns();
     }
-    // the arrival counters are reset for the next launch by the last CTA to get here (nobody reads them any more)
-    if (a.any_signal && ctid == 0) {
-        if (atomicAdd(a.opsync + GS_MAX_OPS, 1u) == gridDim.x - 1) {
-            for (uint32_t j = 0; j < a.nops; ++j) a.opsync[j] = 0;
-            a.opsync[GS_MAX_OPS] = 0;
-        }
-    }
+    post(reserve(), REC_EXIT, 0, 0, 0, 0);      // the helper finishes what is queued, resets the arrival counters, and leaves
 }
 
 std::atomic<bool> g_gemv_pdl{true};      // A/B switch (cloak_set_gemv_engine(2) turns PDL off)
