@@ -45,7 +45,7 @@
 
 namespace cloak {
 
-struct ChainOp {             // 80 bytes of kernel parameter space per op (10 x 8)
+struct ChainOp {             // 88 bytes of kernel parameter space per op (11 x 8)
     uint64_t w_offset;
     const uint16_t* x;       // [batch, K]
     __nv_bfloat16* y;        // [batch, N]
@@ -54,8 +54,10 @@ struct ChainOp {             // 80 bytes of kernel parameter space per op (10 x 
     uint32_t N, K;
     uint32_t kch;            // chunks per row = K*2 / CB
     uint32_t units;          // tiles * kch
-    uint32_t per;            // units per CTA
-    uint32_t ctas;           // CTAs that own units of this op (indices 0 .. ctas-1)
+    uint32_t per;            // units per range: range r (of min(units, grid) ranges) starts at r * per + min(r, rem) and holds
+    uint32_t rem;            //   per + (r < rem) units -- equal to within one unit
+    uint32_t ctas;           // ranges = CTAs that own units of this op (host side only)
+    uint32_t pad_;
     uint32_t tile_base;      // index of this op's first row-tile counter
     uint32_t flags;          // OP_SIGNAL
     uint32_t wait_op;        // NO_WAIT, or the index of the op whose completion by ALL CTAs this op's consumers wait for
@@ -304,7 +306,7 @@ gemv_chain_kernel(const __grid_constant__ typename std::conditional<SEG, ChainAr
             const ChainOp& op = a.ops[j];
             const uint32_t kch = op.kch;
             const uint32_t vr = (blockIdx.x + gridDim.x - op.rot) % gridDim.x;   // this CTA's range of the op
-            const uint32_t ubeg = vr * op.per, uend = min(ubeg + op.per, op.units);
+            const uint32_t ubeg = vr * op.per + min(vr, op.rem), uend = min(ubeg + op.per + (vr < op.rem ? 1u : 0u), op.units);
             if (ubeg >= uend) continue;
             const uint32_t tile_lo = ubeg / kch, tile_hi = (uend - 1) / kch;
             const uint64_t row_bytes = (uint64_t)op.K * 2;
@@ -399,7 +401,7 @@ gemv_chain_kernel(const __grid_constant__ typename std::conditional<SEG, ChainAr
         const ChainOp& op = a.ops[j];
         const uint32_t kch = op.kch, per = op.per;
         const uint32_t vr = (blockIdx.x + gridDim.x - op.rot) % gridDim.x;       // this CTA's range of the op
-        const uint32_t ubeg = vr * per, uend = min(ubeg + per, op.units);
+        const uint32_t ubeg = vr * per + min(vr, op.rem), uend = min(ubeg + per + (vr < op.rem ? 1u : 0u), op.units);
         const bool have = ubeg < uend;
 
         if (have && op.wait_op != NO_WAIT) {
@@ -526,7 +528,11 @@ gemv_chain_kernel(const __grid_constant__ typename std::conditional<SEG, ChainAr
                         consumer_bar();          // red[] is reused by the next pass; the partial / own sums are complete
                         if (pub_here) post(pslot, REC_PUBLISH, j, tile_lo, 0, 0);
                         // (the other contributors of the tail tile are the CTAs after this one that hold units of it)
-                        if (tail_here) post(tslot, REC_TAIL, j, tile_hi, (tile_hi * kch + kch - 1) / per - vr, vr);
+                        if (tail_here) {
+                            const uint32_t ul = tile_hi * kch + kch - 1, big = op.rem * (per + 1);      // the tile's last unit; its range:
+                            const uint32_t rl = ul < big ? ul / (per + 1) : op.rem + (ul - big) / per;
+                            post(tslot, REC_TAIL, j, tile_hi, rl - vr, vr);
+                        }
                     }
                 }
             }
@@ -768,18 +774,37 @@ cloak_status gemv_stream_launch(const cloak_pool* pool, const cloak_gemv_op* ops
     uint64_t small_units = 0, all_units = 0;
     for (uint32_t j = 0; j < nf; ++j) {
         ChainOp& o = a.ops[j];
-        o.per = (o.units + ctas - 1) / ctas;
-        o.ctas = (o.units + o.per - 1) / o.per;
+        o.ctas = o.units < (uint32_t)ctas ? o.units : (uint32_t)ctas;
+        o.per = o.units / o.ctas;
+        o.rem = o.units % o.ctas;
+        o.pad_ = 0;
         all_units += o.units;
         if (o.ctas * 8 <= (uint32_t)ctas * 7) small_units += o.units;
     }
     const bool rotate_all = 2 * small_units > all_units;
+    // An op that fills the grid gives `rem` of its ranges one unit more than the others: they go to the CTAs (a contiguous run,
+    // modulo the grid) that hold the least so far, so that over the launch every CTA streams the same bytes to within a unit or
+    // two -- with the extras always on CTAs 0 .. rem-1 the first CTAs of the cfg1 layer held 93 units of 32 KiB, the mean 90.
+    std::vector<uint32_t> load(ctas, 0);
+    auto add_load = [&](const ChainOp& o) {
+        for (uint32_t r = 0; r < o.ctas; ++r) load[(r + o.rot) % ctas] += o.per + (r < o.rem ? 1u : 0u);
+    };
     uint32_t ranges_so_far = 0;
     for (uint32_t j = 0; j < nf; ++j) {
         ChainOp& o = a.ops[j];
         o.rot = (rotate_all || o.ctas * 4 <= (uint32_t)ctas * 3) ? ranges_so_far % ctas : 0;
+        if (o.ctas == (uint32_t)ctas && o.rem > 0) {
+            uint64_t win = 0, best = ~0ull;
+            for (uint32_t r = 0; r < o.rem; ++r) win += load[r];
+            for (uint32_t start = 0; start < (uint32_t)ctas; ++start) {       // window = CTAs start .. start + rem - 1
+                if (win < best) { best = win; o.rot = start; }
+                win += load[(start + o.rem) % ctas];
+                win -= load[start];
+            }
+        }
         for (uint32_t k = 0; k < j; ++k)
             if (o.gate && (const void*)a.ops[k].y == (const void*)o.gate) o.rot = a.ops[k].rot;     // same rows, same CTA
+        add_load(o);
         ranges_so_far += o.ctas;
     }
     a.trace = g_trace.load(std::memory_order_relaxed);
@@ -897,8 +922,10 @@ extern "C" cloak_status cloak_gemv_static(const cloak_pool* pool, const cloak_te
     o.wait_op = NO_WAIT;
     o.rot = 0;
     const int ctas = units64 < (uint64_t)sms ? (int)units64 : sms;
-    o.per = (o.units + ctas - 1) / ctas;
-    o.ctas = (o.units + o.per - 1) / o.per;
+    o.ctas = o.units < (uint32_t)ctas ? o.units : (uint32_t)ctas;
+    o.per = o.units / o.ctas;
+    o.rem = o.units % o.ctas;
+    o.pad_ = 0;
     const size_t part = (size_t)ctas * batch * GS_ROWS * 4;
     if (part > GS_STATIC_PART_BYTES)
         return fail(CLOAK_ERR_UNSUPPORTED, "gemv_static: %d CTAs x batch %u need %zu bytes of partials, the static scratch holds %zu",
