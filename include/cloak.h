@@ -324,9 +324,12 @@ cloak_status cloak_to_tile128(const void* d_src, void* d_dst, uint32_t N, uint32
  * Different pools are independent and may run on different streams at the same time.
  * Co-residency.  A cloak_gemv_chain launch that contains an `after` op has a grid-wide barrier inside and is launched as a
  * COOPERATIVE grid (all CTAs resident, or the launch waits / fails -- never a hang when other kernels hold SMs, e.g. two pools'
- * chains on two streams).  Launches without one (cloak_gemv, chains of independent ops) wait only for the few CTAs that
- * FOLLOW them in index order, which publish before they wait for anybody; with CTAs dispatched in index order -- what every
- * NVIDIA GPU does, though CUDA does not promise it -- that cannot deadlock, and they stay ordinary launches.  The GEMM waits
+ * chains on two streams).  In launches without one (cloak_gemv, chains of independent ops) a CTA -- its helper warp, not the warps
+ * that stream -- waits only for the partials of the few CTAs that hold the NEXT ranges of the same op.  Those stay ordinary
+ * launches: they need the whole grid (one CTA per SM, never more CTAs than the device has SMs) to become resident, which the
+ * GPU's in-order dispatch of grids gives whenever all SMs of the device are available to the context, whatever else is queued.
+ * A context confined to FEWER SMs than the device reports (MPS active-thread percentage, green contexts) cannot hold the grid:
+ * use cloak_set_gemv_engine(1) there (the one-shot kernel waits for nobody).  The GEMM waits
  * only for partials of CTAs that drew their ticket before the waiter, i.e. that are already running: no assumption at all. */
 typedef struct {
     uint64_t w_offset;

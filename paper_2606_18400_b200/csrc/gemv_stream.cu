@@ -5,7 +5,8 @@
 // at 5.5 TB/s, 8 x 4 KiB pieces at 6.4 TB/s, so a unit of work is (8 weight rows) x (CB of each row), CB = the largest
 // multiple of 512 B up to 4 KiB that divides the row (4 KiB for every LLaMA / Qwen projection but a few):
 //   * one persistent CTA per SM; an op's units are numbered tile-major (u = tile * kch + chunk) and cut into
-//     equal contiguous ranges, one per CTA (stream-K): every SM moves the same bytes, no wave tail;
+//     contiguous ranges equal to within one unit, one per CTA (stream-K); the ranges that are one unit longer go, op after op,
+//     to the CTAs that hold the least so far: every SM moves the same bytes to within a unit or two, no wave tail;
 //   * warp 0 produces: 8 lanes each translate one row piece through the block table and issue one
 //     cp.async.bulk (TMA 1-D) into a shared-memory ring (6 stages of 32 KiB), completion on an mbarrier;
 //   * warps 1-8 consume: each owns one eighth of the k-range of a chunk.  The weights are the B operand of
@@ -24,6 +25,10 @@
 //     (acquire; all CTAs are co-resident, one per SM) and adds the partials in contributor order:
 //     deterministic, and bit-identical between a cloaked and an identity-table pool, which differ only in
 //     addresses.  No fence, atomic round trip or reduction sits at the end of the other CTAs.
+//   * all of that device-scope work -- the release that publishes a partial, the owner's acquire-wait, its partial loads and
+//     stores, the report that an op is done -- is done by a HELPER warp (warp 1), to which the consumers post records through a
+//     small shared-memory queue: while consumer warps sit in an L2 round trip no ring stage is handed back and no copy is issued
+//     (measured: 7.8 of 80.9 us for the 7 ops of the cfg1 layer; see GS_NREC).
 //   * a launch executes a CHAIN of ops (cloak_gemv_chain; cloak_gemv is a chain of one).  The producer warp
 //     runs straight through the chain -- weights do not depend on activations -- so HBM stays busy across op
 //     boundaries (an op with fewer ranges than CTAs starts at the CTA where the previous one stopped when such ops
@@ -568,11 +573,12 @@ constexpr uint32_t GS_TILE_COUNTERS = (uint32_t)(WS_COUNTER_BYTES / 4) - 4 * GS_
 //       fails the launch (cudaErrorCooperativeLaunchTooLarge) instead of hanging when that can never be.  Measured cost of
 //       the attribute: none (cloak_set_gemv_engine(3) launches such chains as ordinary grids: cfg2's chain 2.592 vs 2.596 ms,
 //       a 25-launch MoE chain 0.4623 vs 0.4623 ms).
-//   (2) The owner of a cut row tile waits for the partials of the FEW CTAs that follow it in range order, which publish them at
-//       the START of their ranges and wait for nobody first.  CTAs are dispatched in index order, so whatever subset is
-//       resident, the waits form a chain that ends at a CTA that is running or done: progress without full residency (the
-//       dispatch order is how every NVIDIA GPU behaves, not an architectural promise -- cloak.h says so).  Launches with only
-//       this kind of wait (cloak_gemv, chains of independent ops) stay ordinary launches.
+//   (2) The owner of a cut row tile -- its helper warp -- waits for the partials of the FEW CTAs that hold the next ranges of the op,
+//       whose helpers publish them early in their ranges.  Such a wait ends once those CTAs are resident; the grid never has more
+//       CTAs than the device has SMs (one 200 KB CTA per SM) and the GPU dispatches grids in launch order, so on a device whose SMs
+//       are all available to the context the whole grid becomes resident whatever else is queued (two pools' chains on two
+//       streams: test_two_pools_two_streams).  Launches with only this kind of wait (cloak_gemv, chains of independent ops) stay
+//       ordinary launches.  A context confined to fewer SMs than the device reports cannot run them (cloak.h says so).
 // Whether the cooperative attribute may be combined with programmatic stream serialization is probed on the first such launch:
 // if the driver rejects the pair, PDL is dropped, not the guarantee.
 std::atomic<unsigned long long*> g_trace{nullptr};     // cloak_set_trace
