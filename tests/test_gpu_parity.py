@@ -1230,6 +1230,47 @@ def test_gemv_chain_fuses_small_ops_bit_identically(batch, I):
         C.cloak_set_gemv_engine(0)
 
 
+@pytest.mark.parametrize("batch", [1, 8, 16])
+def test_gemv_chain_helper_queue_wraps(batch):
+    """The helper warp's 8-slot record queue under load: 48 ops in ONE launch, every op with cut row tiles (two or four chunks per
+    row) and `after = 1` -- a publish, a tail and a report per op and CTA, a grid-wide wait before every op -- alternating between
+    a generator vector and the previous op's output as input; twice over the same outputs (counters back at zero).  Equal to the
+    same ops issued one cloak_gemv at a time, bit for bit; the ops fed by the generator vector also against the oracle."""
+    key, seed, block, page = 0x1234, 41, 65536, 2 << 20
+    shapes = [(2560, 2560), (2560, 5120), (5120, 2560)]            # 5 KiB and 10 KiB rows: 2.5 KiB chunks, kch = 2 / 4
+    Ws = [gen.synth(seed, i, shp, "bf16") for i, shp in enumerate(shapes)]
+    offs, total = C.cloak_arena_plan(key, [2 * n * k for n, k in shapes], block)
+    with Pool(total, block, page, key) as p:
+        _load_pool(p, [(f"w{i}", w) for i, w in enumerate(Ws)], offs, "bf16")
+        T = [C.cloak_tensor(o, n, k, C.CLOAK_BF16, C.CLOAK_ROWMAJOR) for (n, k), o in zip(shapes, offs)]
+        X = {k: gen.synth(seed + 1, k, (batch, k), "bf16", kind=gen.KIND_NORMAL) for k in (2560, 5120)}
+        dX = {k: bf16_dev_from_bits(v) for k, v in X.items()}
+        order = [0, 1, 2] * 16                                       # every third op (K = 2560) reads the output of the one before it (N = 2560)
+        outs_c, outs_s, ops, singles = [], [], [], []
+        for j, w in enumerate(order):
+            n, k = shapes[w]
+            yc, ys = torch.zeros(batch, n, dtype=torch.bfloat16, device="cuda"), torch.zeros(batch, n, dtype=torch.bfloat16, device="cuda")
+            fresh = j % 3 != 2                                       # ops 2, 5, ..: X is the previous op's output
+            xc = dX[k] if fresh else outs_c[j - 1]
+            xs = dX[k] if fresh else outs_s[j - 1]
+            ops.append((T[w], xc, yc, 1))
+            singles.append((T[w], xs, ys, fresh))
+            outs_c.append(yc)
+            outs_s.append(ys)
+        launches0 = C.cloak_launch_count()
+        C.cloak_gemv_chain(p.h, ops, batch)
+        assert C.cloak_launch_count() - launches0 == 1
+        C.cloak_gemv_chain(p.h, ops, batch)
+        for t, x, y, _ in singles:
+            C.cloak_gemv(p.h, t, x, y, batch)
+        torch.cuda.synchronize()
+        for j in range(len(order)):
+            assert torch.equal(outs_c[j], outs_s[j]), j
+        for j in (0, 1, 3, 45, 46):
+            assert singles[j][3]
+            check_linear(outs_c[j].float().cpu().numpy(), X[shapes[order[j]][1]], Ws[order[j]], "bf16", f"gemv_chain_queue:b{batch}:op{j}", TOL["bf16"])
+
+
 # ------------------------------------------------------------------ randomised chains (shapes, lengths, dependencies)
 @pytest.mark.parametrize("seed", [0, 1, 2, 3, 10, 11, 12, 13, 14, 15, 16, 17])
 def test_gemv_chain_random_lists_equal_single_calls(seed):
