@@ -9,7 +9,7 @@
 //     to the CTAs that hold the least so far: every SM moves the same bytes to within a unit or two, no wave tail;
 //   * warp 0 produces: 8 lanes each translate one row piece through the block table and issue one
 //     cp.async.bulk (TMA 1-D) into a shared-memory ring (6 stages of 32 KiB), completion on an mbarrier;
-//   * warps 1-8 consume: each owns one eighth of the k-range of a chunk.  The weights are the B operand of
+//   * eight consumer warps (behind the producer and the helper warp): each owns one eighth of the k-range of a chunk.  The weights are the B operand of
 //     mma.sync.m16n8k16 (8 weight rows = N), the activations the A operand (batch rows = M, zero-padded to 8 or
 //     16).  Lane (g, t) reads one 16-byte vector of weight row g per 64-byte step; since a contraction may visit
 //     k in any order, the vector's elements are *declared* to be the MMA's k-slots (2t, 2t+1, 2t+8, 2t+9) and
@@ -110,9 +110,9 @@ __device__ __forceinline__ const ChainArgs& chain_base(const ChainArgs& a) { ret
 __device__ __forceinline__ const ChainArgs& chain_base(const ChainArgsSeg& a) { return a.base; }
 
 constexpr int GS_CONSUMERS = 8;                       // consumer warps
-// Warps ahead of the consumers.  batch <= 8: the producer warp alone.  batch 9..16: a whole warpgroup (producer + three
-// warps that retire at once), so that the register file can be re-split per warpgroup with setmaxnreg: the producer
-// group drops to 40 registers per thread, the two consumer groups rise to 232 -- room for a second set of X fragments.
+// Warps ahead of the consumers.  batch <= 8: the producer warp and the helper warp.  batch 9..16: a whole warpgroup (producer,
+// helper and two warps that retire at once), so that the register file can be re-split per warpgroup with setmaxnreg: the lead
+// group drops to 56 registers per thread, the two consumer groups rise to 224 -- room for a second set of X fragments.
 constexpr int gs_lead_warps(int nt) { return nt == 2 ? 4 : 2; }      // warp 0 = producer, warp 1 = helper (see GS_NREC)
 constexpr int gs_threads(int nt) { return 32 * (gs_lead_warps(nt) + GS_CONSUMERS); }
 constexpr int GS_ROWS = 8;                            // weight rows per tile (the MMA's N)
