@@ -401,6 +401,10 @@ gemv_chain_kernel(const __grid_constant__ typename std::conditional<SEG, ChainAr
         }
     };
 
+    // X fragments of this warp's k-slice, two register sets (see "X fragments of one phase" below); they outlive an op
+    uint4 xa[KS], xb[KS], na[KS], nb[KS];
+    const uint16_t* held_x = nullptr;            // batch 9..16: the X whose chunks 0 and 1 sit in (xa, xb) and (na, nb)
+
     uint32_t s = 0, ph = 0;
     for (uint32_t j = 0; j < a.nops; ++j) {
         const ChainOp& op = a.ops[j];
@@ -414,6 +418,7 @@ gemv_chain_kernel(const __grid_constant__ typename std::conditional<SEG, ChainAr
             if (ctid == 0)
                 while (ld_acquire(a.opsync + op.wait_op) != gridDim.x) __nanosleep(32);
             consumer_bar();
+            held_x = nullptr;                    // X may have been written inside this launch: nothing held is good any more
         }
 
         if (have) {
@@ -428,7 +433,10 @@ gemv_chain_kernel(const __grid_constant__ typename std::conditional<SEG, ChainAr
             // X fragments of one (group, chunk) phase.  Batch <= 8 re-reads them mostly from L1; batch 9..16 (X is up to
             // 16 x K x 2 B, more than the L1 left beside the ring) pays an L2 round trip per phase, so there the next
             // phase's fragments are fetched one phase ahead (PF) into a second register set (see gs_lead_warps).
-            uint4 xa[KS], xb[KS], na[KS], nb[KS];
+            // Batch 9..16, rows of TWO chunks (K = 4096 at 4 KiB chunks): both chunks' fragments fit the two register sets, so they
+            // are loaded once per X -- consecutive ops that read the same activations (q, k, v; gate, up) and all their groups
+            // share them -- instead of once per phase: the SMs' ingest is what bounds batch 16.
+            const bool resident = PF && kch == 2;
             auto load_x = [&](uint4 (&pa)[KS], uint4 (&pb)[KS], uint32_t c) {
                 const uint32_t xk = c * (CB / 2);
                 const uint4 z = make_uint4(0, 0, 0, 0);
@@ -438,7 +446,16 @@ gemv_chain_kernel(const __grid_constant__ typename std::conditional<SEG, ChainAr
                     pb[ks] = (NT == 2 && xv1) ? ldg_coherent(x1 + xk + ks * 32) : z;
                 }
             };
-            if (PF) load_x(xa, xb, 0);
+            if (resident) {
+                if (held_x != x0) {
+                    load_x(xa, xb, 0);
+                    load_x(na, nb, 1);
+                    held_x = x0;
+                }
+            } else if (PF) {
+                load_x(xa, xb, 0);
+                held_x = nullptr;
+            }
 
             for (uint32_t g0 = tile_lo, gnext; g0 <= tile_hi; g0 = gnext) {
                 uint32_t g1 = min(g0 + GS_TG - 1, tile_hi);
@@ -458,15 +475,8 @@ gemv_chain_kernel(const __grid_constant__ typename std::conditional<SEG, ChainAr
 #pragma unroll
                         for (int i = 0; i < 4; ++i) acc[q][n][i] = 0.f;
 
-                for (uint32_t c = 0; c < kch; ++c) {
-                    // this warp's X fragments for chunk c: fetched once, reused for every row tile of the group
-                    bool more = false;
-                    if (!PF) {
-                        load_x(xa, xb, c);
-                    } else {
-                        more = (c + 1 < kch) || (g0 + GS_TG <= tile_hi);
-                        if (more) load_x(na, nb, c + 1 < kch ? c + 1 : 0);      // the next phase's, behind this phase's work
-                    }
+                // one (group, chunk) phase: the group's row tiles of chunk c against the fragments (pa, pb)
+                auto phase = [&](const uint4 (&pa)[KS], const uint4 (&pb)[KS], uint32_t c) {
 #pragma unroll
                     for (int q = 0; q < GS_TG; ++q) {
                         const uint32_t tile = g0 + q, u = tile * kch + c;
@@ -476,18 +486,34 @@ gemv_chain_kernel(const __grid_constant__ typename std::conditional<SEG, ChainAr
 #pragma unroll
                         for (int ks = 0; ks < KS; ++ks) {
                             const uint4 w = lds128(base + ks * 64);
-                            mma_16816(acc[q][0], xa[ks].x, xb[ks].x, xa[ks].y, xb[ks].y, w.x, w.y);
-                            mma_16816(acc[q][GS_NACC - 1], xa[ks].z, xb[ks].z, xa[ks].w, xb[ks].w, w.z, w.w);
+                            mma_16816(acc[q][0], pa[ks].x, pb[ks].x, pa[ks].y, pb[ks].y, w.x, w.y);
+                            mma_16816(acc[q][GS_NACC - 1], pa[ks].z, pb[ks].z, pa[ks].w, pb[ks].w, w.z, w.w);
                         }
                         __syncwarp();
                         if (lane == 0) mbar_arrive(smem_u32(&empty[s]));
                         if (++s == NST) { s = 0; ph ^= 1; }
                     }
-                    if (PF && more) {
+                };
+                if (resident) {
+                    phase(xa, xb, 0);
+                    phase(na, nb, 1);
+                } else {
+                    for (uint32_t c = 0; c < kch; ++c) {
+                        // this warp's X fragments for chunk c: fetched once, reused for every row tile of the group
+                        bool more = false;
+                        if (!PF) {
+                            load_x(xa, xb, c);
+                        } else {
+                            more = (c + 1 < kch) || (g0 + GS_TG <= tile_hi);
+                            if (more) load_x(na, nb, c + 1 < kch ? c + 1 : 0);      // the next phase's, behind this phase's work
+                        }
+                        phase(xa, xb, c);
+                        if (PF && more) {
 #pragma unroll
-                        for (int ks = 0; ks < KS; ++ks) {
-                            xa[ks] = na[ks];
-                            xb[ks] = nb[ks];
+                            for (int ks = 0; ks < KS; ++ks) {
+                                xa[ks] = na[ks];
+                                xb[ks] = nb[ks];
+                            }
                         }
                     }
                 }
